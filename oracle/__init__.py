@@ -1,0 +1,120 @@
+"""ctypes front-end of the CPU ORACLE (oracle/bie_oracle.c).
+
+TEST INFRASTRUCTURE ONLY: imported by tests/, by __graft_entry__.smoke() and by the cpu_baseline /
+``--impl reference`` legs of bench.py.  Nothing under paper_2108_01786_b200/ imports this package and
+this package imports nothing from it (argument marshalling below is numpy only).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from typing import Optional, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "bie_oracle.c")
+_LIB = os.path.join(_HERE, "libbie_oracle.so")
+_lib: Optional[ctypes.CDLL] = None
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 -fopenmp (no fast-math) -> oracle/libbie_oracle.so."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".{os.getpid()}.tmp"
+        subprocess.check_call(["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared",
+                               "-ffp-contract=off", "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def lib() -> ctypes.CDLL:
+    global _lib
+    if _lib is None:
+        build()
+        L = ctypes.CDLL(_LIB)
+        dp = ctypes.POINTER(ctypes.c_double)
+        ip = ctypes.POINTER(ctypes.c_int)
+        L.oracle_num_threads.restype = ctypes.c_int
+        L.oracle_set_num_threads.argtypes = [ctypes.c_int]
+        L.oracle_cot_half.argtypes = [ctypes.c_double, ctypes.c_double, dp, dp]
+        L.oracle_build.restype = ctypes.c_int
+        L.oracle_build.argtypes = [ctypes.c_int, ip, ip, dp, dp, dp, ctypes.c_int, dp, ctypes.c_long]
+        L.oracle_matvec.argtypes = [ctypes.c_long, dp, ctypes.c_long, dp, dp]
+        L.oracle_gmres.restype = ctypes.c_int
+        L.oracle_gmres.argtypes = [ctypes.c_long, dp, ctypes.c_long, dp, ctypes.c_double, ctypes.c_int,
+                                   ctypes.c_int, dp, ip, dp, dp]
+        _lib = L
+    return _lib
+
+
+def _dp(a: np.ndarray):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def _ip(a: np.ndarray):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_int))
+
+
+def num_threads() -> int:
+    return int(lib().oracle_num_threads())
+
+
+def set_num_threads(t: int) -> None:
+    lib().oracle_set_num_threads(int(t))
+
+
+def cot_half(x: float, y: float) -> complex:
+    re = ctypes.c_double()
+    im = ctypes.c_double()
+    lib().oracle_cot_half(float(x), float(y), ctypes.byref(re), ctypes.byref(im))
+    return complex(re.value, im.value)
+
+
+def _c128_as_f64(z: np.ndarray) -> np.ndarray:
+    z = np.ascontiguousarray(z, dtype=np.complex128)
+    return z.view(np.float64)
+
+
+def build_matrix(counts, kinds, zeta, dzeta, d2zeta, variant: int = 0,
+                 out: Optional[np.ndarray] = None) -> np.ndarray:
+    """Matrix of Eq. (3.16) (variant 0) or the uncorrected operator B of Eq. (3.10) (variant 1)."""
+    counts = np.ascontiguousarray(counts, dtype=np.int32)
+    kinds = np.ascontiguousarray(kinds, dtype=np.int32)
+    n = int(counts.sum())
+    z, dz, d2z = _c128_as_f64(zeta), _c128_as_f64(dzeta), _c128_as_f64(d2zeta)
+    assert z.size == 2 * n and dz.size == 2 * n and d2z.size == 2 * n
+    A = out if out is not None else np.empty((n, n), dtype=np.float64)
+    assert A.flags.c_contiguous and A.shape == (n, n)
+    rc = lib().oracle_build(int(counts.size), _ip(counts), _ip(kinds), _dp(z), _dp(dz), _dp(d2z),
+                            int(variant), _dp(A), n)
+    if rc != 0:
+        raise ValueError(f"oracle_build failed: {rc}")
+    return A
+
+
+def matvec(A: np.ndarray, x: np.ndarray) -> np.ndarray:
+    A = np.ascontiguousarray(A, dtype=np.float64)
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    n = A.shape[0]
+    y = np.empty(n, dtype=np.float64)
+    lib().oracle_matvec(n, _dp(A), A.shape[1], _dp(x), _dp(y))
+    return y
+
+
+def gmres(A: np.ndarray, b: np.ndarray, tol: float = 1e-13, restart: int = 50,
+          max_iters: int = 1000) -> Tuple[np.ndarray, int, float, np.ndarray, int]:
+    """-> (x, iters, relres_true, res_hist[0..iters], status)   status 0 = converged, 1 = max_iters."""
+    A = np.ascontiguousarray(A, dtype=np.float64)
+    b = np.ascontiguousarray(b, dtype=np.float64)
+    n = A.shape[0]
+    x = np.empty(n, dtype=np.float64)
+    hist = np.zeros(max_iters + 1, dtype=np.float64)
+    iters = ctypes.c_int()
+    relres = ctypes.c_double()
+    rc = lib().oracle_gmres(n, _dp(A), A.shape[1], _dp(b), float(tol), int(restart), int(max_iters),
+                            _dp(x), ctypes.byref(iters), ctypes.byref(relres), _dp(hist))
+    if rc < 0:
+        raise ValueError(f"oracle_gmres failed: {rc}")
+    return x, int(iters.value), float(relres.value), hist[:iters.value + 1].copy(), int(rc)

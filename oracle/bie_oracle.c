@@ -1,0 +1,270 @@
+/*
+ * bie_oracle.c -- CPU ORACLE for the boundary-integral hot path of arXiv 2108.01786.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Plain, slow, obviously-correct FP64 C written
+ * from the paper; it shares no code, header, table or helper with the CUDA path
+ * (paper_2108_01786_b200/csrc/).  Only tests/, __graft_entry__.smoke() and the cpu_baseline /
+ * --impl reference legs of bench.py may load it.
+ *
+ * What it computes (every function cites the passage it follows; PAPER.md = /root/reference/PAPER.md):
+ *
+ *   oracle_cot_half   cot((x+iy)/2), the periodised Cauchy kernel of Eq. (3.4):
+ *                     PV sum_k 1/(zeta + 2 pi k - z) = (1/2) cot((zeta - z)/2).
+ *   oracle_build      the collocation matrix of Eq. (3.16), entry by entry, from
+ *                     Table 1, the diagonal limit, the block
+ *                     structure of Eq. (3.10), the trapezoid weights 1/M_j
+ *                      and E_m = M_m^{-1} e e^T.
+ *   oracle_matvec     y = A x, the plain definition (long-double accumulation).
+ *   oracle_gmres      restarted GMRES(m) of Saad & Schultz (ref. [38] cited at PAPER.md:L855), modified
+ *                     Gram-Schmidt + Givens rotations, x0 = 0, stop when the recurrence residual
+ *                     |g_{j+1}| <= tol * ||b|| (PAPER.md:L869 defines i_max by this criterion).
+ *
+ * Pins (tests/test_oracle_pins.py, run with -m "not gpu"): P1 cot vs 40-digit mpmath and vs the image
+ * sum (3.4); P2 block row sums from Eq. (6.3); P3 analytic-function reproduction; P4 spectral
+ * convergence; P5 adaptive quadrature of the kernel; P6 flat/flat closed-form solution; P7 GMRES vs
+ * LAPACK dgesv.  Nothing here is "parity unpinned".
+ *
+ * Readings of the paper where it is silent or garbled are listed in DESIGN.md ("Readings").
+ */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+int oracle_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void oracle_set_num_threads(int t)
+{
+#ifdef _OPENMP
+    if (t > 0) omp_set_num_threads(t);
+#else
+    (void)t;
+#endif
+}
+
+/* cot((x+iy)/2) in the half-angle form (reading R6; accuracy-critical: the form with
+ * cosh y - cos x in the denominator loses 4 digits for near neighbours):
+ *   cot((x+iy)/2) = ( sin(x/2)cos(x/2) - i sinh(y/2)cosh(y/2) ) / ( sin^2(x/2) + sinh^2(y/2) ).
+ * 2pi-periodic in x, which is the sum over periodic images of Eq. (3.4). */
+void oracle_cot_half(double x, double y, double *re, double *im)
+{
+    double sx = sin(0.5 * x), cx = cos(0.5 * x);
+    double sh = sinh(0.5 * y), ch = cosh(0.5 * y);
+    double d = sx * sx + sh * sh;
+    *re = (sx * cx) / d;
+    *im = -(sh * ch) / d;
+}
+
+/* Matrix of Eq. (3.16).
+ *
+ * components: c = 0..ncomp-1 with counts[c] = M_c nodes alpha_{cl} = 2 pi l / M_c,
+ * kinds[c]: 0 free surface (component 0), 1 bottom (component 1), 2 obstacle (clockwise).
+ * zeta/dzeta/d2zeta: interleaved (re,im), n = sum counts, components concatenated.
+ * Row = target node (k,m); column = source node (j,l).  For (k,m) != (j,l)
+ *      c = zeta'_j[l] / (2 M_j) * cot((zeta_j[l] - zeta_k[m]) / 2)          (Table 1)
+ * and for (k,m) == (j,l)
+ *      c = zeta''_k[m] / (2 zeta'_k[m] M_k)
+ * entry:  k = 0, j = 0 :  Im c - 1/2 delta          (-1/2 I + K_00)           (Eq. 3.10)
+ *         k = 0, j >= 1:  Re c                      (G_0j)
+ *         k >= 1, j = 0: -Re c                      (-G_k0)
+ *         k >= 1, j >= 1: Im c + 1/2 delta - [k = j is an obstacle]/M_k   (1/2 I + K_kj - E_k)
+ * variant 0: as above; variant 1: without the E_k term (the operator B of Eq. (3.10)).
+ * A is row-major n x n with leading dimension lda >= n.  Returns 0, or <0 on bad arguments. */
+int oracle_build(int ncomp, const int *counts, const int *kinds,
+                 const double *zeta, const double *dzeta, const double *d2zeta,
+                 int variant, double *A, long lda)
+{
+    if (ncomp < 1 || !counts || !kinds || !zeta || !dzeta || !d2zeta || !A) return -1;
+    long n = 0;
+    for (int c = 0; c < ncomp; ++c) {
+        if (counts[c] < 1) return -2;
+        if (kinds[c] < 0 || kinds[c] > 2) return -2;
+        if ((kinds[c] == 0) != (c == 0)) return -2; /* the free surface is component 0, and only it */
+        n += counts[c];
+    }
+    if (lda < n) return -3;
+    int *comp = (int *)malloc(sizeof(int) * (size_t)n);
+    if (!comp) return -4;
+    {
+        long p = 0;
+        for (int c = 0; c < ncomp; ++c)
+            for (int l = 0; l < counts[c]; ++l) comp[p++] = c;
+    }
+#pragma omp parallel for schedule(static)
+    for (long t = 0; t < n; ++t) {
+        const int k = comp[t];
+        const double ztr = zeta[2 * t], zti = zeta[2 * t + 1];
+        double *row = A + t * lda;
+        for (long s = 0; s < n; ++s) {
+            const int j = comp[s];
+            const double Mj = (double)counts[j];
+            double cre, cim;
+            if (s == t) {
+                /* zeta'' / (2 zeta' M) */
+                double ar = d2zeta[2 * s], ai = d2zeta[2 * s + 1];
+                double br = dzeta[2 * s], bi = dzeta[2 * s + 1];
+                double den = br * br + bi * bi;
+                cre = (ar * br + ai * bi) / den / (2.0 * Mj);
+                cim = (ai * br - ar * bi) / den / (2.0 * Mj);
+            } else {
+                double x = zeta[2 * s] - ztr, y = zeta[2 * s + 1] - zti;
+                double cr, ci;
+                oracle_cot_half(x, y, &cr, &ci);
+                double qr = dzeta[2 * s] / (2.0 * Mj), qi = dzeta[2 * s + 1] / (2.0 * Mj);
+                cre = qr * cr - qi * ci;
+                cim = qr * ci + qi * cr;
+            }
+            double e;
+            if (k == 0 && j == 0)
+                e = cim - (s == t ? 0.5 : 0.0);
+            else if (k == 0)
+                e = cre;
+            else if (j == 0)
+                e = -cre;
+            else {
+                e = cim + (s == t ? 0.5 : 0.0);
+                if (variant == 0 && k == j && kinds[k] == 2) e -= 1.0 / Mj;
+            }
+            row[s] = e;
+        }
+    }
+    free(comp);
+    return 0;
+}
+
+/* y = A x, plain definition, long-double accumulation so the oracle is the more accurate side. */
+void oracle_matvec(long n, const double *A, long lda, const double *x, double *y)
+{
+#pragma omp parallel for schedule(static)
+    for (long i = 0; i < n; ++i) {
+        const double *row = A + i * lda;
+        long double acc = 0.0L;
+        for (long j = 0; j < n; ++j) acc += (long double)row[j] * (long double)x[j];
+        y[i] = (double)acc;
+    }
+}
+
+static double dot_ld(long n, const double *a, const double *b)
+{
+    long double acc = 0.0L;
+    for (long i = 0; i < n; ++i) acc += (long double)a[i] * (long double)b[i];
+    return (double)acc;
+}
+
+/* Restarted GMRES(m), Saad-Schultz (ref. [38]), unpreconditioned, on the unscaled
+ * system (3.16); readings R8-R10:
+ *   1. x = 0, bn = ||b||, iters = 0.
+ *   2. cycle: r = b - A x (first cycle r = b); beta = ||r||; stop if beta <= tol bn.
+ *      v_1 = r / beta, g = beta e_1.
+ *   3. j = 1..m: w = A v_j; modified Gram-Schmidt against v_1..v_j -> h_{1..j,j};
+ *      h_{j+1,j} = ||w||; v_{j+1} = w / h_{j+1,j}; apply rotations 1..j-1 to column j; rotation j from
+ *      (h_jj, h_{j+1,j}) with d = hypot; g_{j+1} = -s_j g_j, g_j = c_j g_j; iters += 1;
+ *      leave the loop when |g_{j+1}| <= tol bn   (i_max of PAPER.md:L869 counts these steps).
+ *   4. y = R^{-1} g, x += sum y_i v_i; converged -> stop, else restart at 2.
+ * Outputs: x, *iters, *relres = ||b - A x|| / bn (true residual; reported, never used to continue),
+ * res_hist[i] (i = 0..iters; optional) = recurrence residual / bn after i steps.
+ * Returns 0 converged, 1 max_iters reached, <0 bad arguments. */
+int oracle_gmres(long n, const double *A, long lda, const double *b,
+                 double tol, int restart, int max_iters,
+                 double *x, int *iters_out, double *relres_out, double *res_hist)
+{
+    if (n < 1 || !A || !b || !x || restart < 1 || max_iters < 0 || lda < n) return -1;
+    const int m = restart;
+    double *V = (double *)malloc(sizeof(double) * (size_t)(m + 1) * (size_t)n);
+    double *H = (double *)calloc((size_t)(m + 1) * (size_t)m, sizeof(double)); /* H[i + j*(m+1)] */
+    double *cs = (double *)malloc(sizeof(double) * (size_t)m);
+    double *sn = (double *)malloc(sizeof(double) * (size_t)m);
+    double *g = (double *)malloc(sizeof(double) * (size_t)(m + 1));
+    double *w = (double *)malloc(sizeof(double) * (size_t)n);
+    double *yv = (double *)malloc(sizeof(double) * (size_t)m);
+    if (!V || !H || !cs || !sn || !g || !w || !yv) {
+        free(V); free(H); free(cs); free(sn); free(g); free(w); free(yv);
+        return -4;
+    }
+    for (long i = 0; i < n; ++i) x[i] = 0.0;
+    const double bn = sqrt(dot_ld(n, b, b));
+    int iters = 0, converged = 0, first = 1;
+    if (res_hist) res_hist[0] = 1.0;
+    if (bn == 0.0) converged = 1;
+    while (!converged && iters < max_iters) {
+        /* step 2 */
+        if (first) {
+            memcpy(w, b, sizeof(double) * (size_t)n);
+            first = 0;
+        } else {
+            oracle_matvec(n, A, lda, x, w);
+            for (long i = 0; i < n; ++i) w[i] = b[i] - w[i];
+        }
+        double beta = sqrt(dot_ld(n, w, w));
+        if (beta <= tol * bn) { converged = 1; break; }
+        for (long i = 0; i < n; ++i) V[i] = w[i] / beta;
+        g[0] = beta;
+        int k = 0;
+        /* step 3 */
+        for (int j = 0; j < m && iters < max_iters; ++j) {
+            double *vj = V + (size_t)j * (size_t)n;
+            oracle_matvec(n, A, lda, vj, w);
+            double *hcol = H + (size_t)j * (size_t)(m + 1);
+            for (int i = 0; i <= j; ++i) {
+                const double *vi = V + (size_t)i * (size_t)n;
+                double h = dot_ld(n, vi, w);
+                hcol[i] = h;
+                for (long r = 0; r < n; ++r) w[r] -= h * vi[r];
+            }
+            double hn = sqrt(dot_ld(n, w, w));
+            hcol[j + 1] = hn;
+            if (hn != 0.0) {
+                double *vn = V + (size_t)(j + 1) * (size_t)n;
+                for (long r = 0; r < n; ++r) vn[r] = w[r] / hn;
+            }
+            for (int i = 0; i < j; ++i) {
+                double t0 = cs[i] * hcol[i] + sn[i] * hcol[i + 1];
+                double t1 = -sn[i] * hcol[i] + cs[i] * hcol[i + 1];
+                hcol[i] = t0;
+                hcol[i + 1] = t1;
+            }
+            double d = hypot(hcol[j], hcol[j + 1]);
+            if (d == 0.0) { cs[j] = 1.0; sn[j] = 0.0; }
+            else { cs[j] = hcol[j] / d; sn[j] = hcol[j + 1] / d; }
+            hcol[j] = d;
+            hcol[j + 1] = 0.0;
+            g[j + 1] = -sn[j] * g[j];
+            g[j] = cs[j] * g[j];
+            ++iters;
+            k = j + 1;
+            if (res_hist) res_hist[iters] = fabs(g[j + 1]) / bn;
+            if (fabs(g[j + 1]) <= tol * bn || hn == 0.0) { converged = 1; break; }
+        }
+        /* step 4: back-substitution R y = g (size k), x += V y */
+        for (int i = k - 1; i >= 0; --i) {
+            double s = g[i];
+            for (int c = i + 1; c < k; ++c) s -= H[(size_t)c * (size_t)(m + 1) + i] * yv[c];
+            yv[i] = s / H[(size_t)i * (size_t)(m + 1) + i];
+        }
+        for (int i = 0; i < k; ++i) {
+            const double *vi = V + (size_t)i * (size_t)n;
+            const double yi = yv[i];
+            for (long r = 0; r < n; ++r) x[r] += yi * vi[r];
+        }
+    }
+    /* true residual */
+    double relres = 0.0;
+    if (bn != 0.0) {
+        oracle_matvec(n, A, lda, x, w);
+        for (long i = 0; i < n; ++i) w[i] = b[i] - w[i];
+        relres = sqrt(dot_ld(n, w, w)) / bn;
+    }
+    if (iters_out) *iters_out = iters;
+    if (relres_out) *relres_out = relres;
+    free(V); free(H); free(cs); free(sn); free(g); free(w); free(yv);
+    return converged ? 0 : 1;
+}

@@ -1,0 +1,399 @@
+"""Pins of the CPU oracle (oracle/) against what the paper and the mathematics fix.  CPU only.
+
+Each test names the passage it pins (PAPER.md = /root/reference/PAPER.md) and the mistake it is
+meant to catch.  None of them re-types the oracle's own formula: they use 40-digit values (mpmath,
+stored under tests/golden/), closed forms, invariants from Eq. (6.3), adaptive quadrature of the
+kernels of Table 1 written with numpy's complex tan (not the oracle's half-angle form), the
+Cauchy-integral reproduction of an analytic function, and LAPACK.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2108_01786_b200 import inputs
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def _build(geo, variant=0):
+    return oracle.build_matrix(geo.counts, geo.kinds, geo.zeta, geo.dzeta, geo.d2zeta, variant)
+
+
+# --------------------------------------------------------------------------------------------
+# P1  the per-pair arithmetic: cot((x+iy)/2), Eq. (3.4)
+# --------------------------------------------------------------------------------------------
+def _golden_cot():
+    rows = []
+    with open(os.path.join(HERE, "golden", "cot_half_40digits.txt")) as f:
+        for line in f:
+            if line.startswith("#"):
+                continue
+            xh, yh, re, im = line.split()
+            rows.append((float.fromhex(xh), float.fromhex(yh), float(re), float(im)))
+    return rows
+
+
+def test_p1_cot_against_40_digit_values():
+    """A wrong sign, a missing half angle or a cancellation-prone denominator fails here."""
+    worst = 0.0
+    for x, y, re, im in _golden_cot():
+        c = oracle.cot_half(x, y)
+        ref = complex(re, im)
+        # the argument x is reduced mod 2 pi inside sin/cos: allow eps*|x|/dist-to-pole conditioning
+        w = complex(x, y)
+        dist = min(abs(w - 2 * np.pi * k) for k in range(-3, 4))
+        cond = 1.0 + abs(x) / max(dist, 1e-300)
+        err = abs(c - ref) / abs(ref)
+        assert err <= 4e-16 * cond + 4e-16, (x, y, err)
+        worst = max(worst, err)
+    assert worst < 1e-9
+
+
+def test_p1_cot_is_the_periodic_image_sum():
+    """Eq. (3.4): (1/2)cot(w/2) = PV sum_k 1/(w + 2 pi k); symmetric truncation error is O(1/K)."""
+    rng = np.random.default_rng(1)
+    K = 200000
+    k = np.arange(1, K + 1, dtype=np.float64)
+    for _ in range(5):
+        w = complex(rng.uniform(-3, 3), rng.uniform(-2, 2))
+        s = 1.0 / w + np.sum(1.0 / (w + 2 * np.pi * k) + 1.0 / (w - 2 * np.pi * k))
+        c = 0.5 * oracle.cot_half(w.real, w.imag)
+        assert abs(s - c) < 5.0 * abs(w) / K + 1e-9
+
+
+def test_p1_flat_over_flat_entry_closed_form():
+    """zeta_0 = a, zeta_1 = a - iH: G_01 = (1/2) sin x/(cosh H - cos x), K_00 = K_11 = 0
+    (follows from Table 1, with zeta' = 1)."""
+    M0, M1, H = 24, 20, 0.7
+    geo = inputs.flat_flat(M0, M1, H)
+    B = _build(geo, variant=1)
+    a0 = 2 * np.pi * np.arange(M0) / M0
+    a1 = 2 * np.pi * np.arange(M1) / M1
+    x = a1[None, :] - a0[:, None]
+    G01 = 0.5 * np.sin(x) / (np.cosh(H) - np.cos(x)) / M1
+    assert np.max(np.abs(B[:M0, M0:] - G01)) < 1e-15
+    # -G_10: source on the surface, target on the bottom: w = a0 - a1 + iH
+    x = a0[None, :] - a1[:, None]
+    G10 = 0.5 * np.sin(x) / (np.cosh(H) - np.cos(x)) / M0
+    assert np.max(np.abs(B[M0:, :M0] + G10)) < 1e-15
+    assert np.max(np.abs(B[:M0, :M0] + 0.5 * np.eye(M0))) < 1e-16
+    assert np.max(np.abs(B[M0:, M0:] - 0.5 * np.eye(M1))) < 1e-16
+
+
+# --------------------------------------------------------------------------------------------
+# P2  block row sums from Eq. (6.3)
+# --------------------------------------------------------------------------------------------
+def test_p2_block_row_sums_config1():
+    """Constant densities: Phi_0 = -+omega_0/2 above/below Gamma_0, Phi_1 = +-i omega_1/2, Phi_j = 0
+    outside / -i omega_j inside obstacle j.  Pins the +-1/2, orientation, Re/Im selection, the
+    diagonal term, the weights 1/M_j and E_m."""
+    P = inputs.make_config(1)
+    g = P.geometry
+    B = _build(g, variant=1)
+    A = _build(g, variant=0)
+    s0, s1, s2 = g.component(0), g.component(1), g.component(2)
+    one = lambda s: np.where((np.arange(g.n) >= s.start) & (np.arange(g.n) < s.stop), 1.0, 0.0)
+    tol = 2e-14
+    r = B @ one(s0)  # omega = 1_0: phi~ on Gamma_0^- is -1/2; psi~ on solids is 0
+    assert np.max(np.abs(r[s0] + 0.5)) < tol and np.max(np.abs(r[s1.start:])) < tol
+    r = B @ one(s1)  # omega = 1_1: Phi_1 = i/2 above the bottom: phi~ = 0 on Gamma_0, psi~ = 1/2 on solids
+    assert np.max(np.abs(r[s0])) < tol and np.max(np.abs(r[s1.start:] - 0.5)) < tol
+    r = B @ one(s2)  # kernel of B (3.12)
+    assert np.max(np.abs(r)) < tol
+    r = A @ one(s2)  # A 1_m = -1_m  (3.13)
+    assert np.max(np.abs(r + one(s2))) < tol
+    # block-wise statements
+    assert np.max(np.abs(B[s0, s0].sum(1) + 0.5)) < tol        # K_00 1 = 0
+    assert np.max(np.abs(B[s2, s2].sum(1))) < tol              # (1/2 I + K_22) 1 = 0  => K_22 1 = -1/2
+    assert np.max(np.abs(B[s2, s1].sum(1) - 0.5)) < tol        # K_21 1 = 1/2
+    assert np.max(np.abs(B[s1, s2].sum(1))) < tol              # K_12 1 = 0
+    assert np.max(np.abs(B[s1, s0].sum(1))) < tol              # G_10 1 = 0
+    assert np.max(np.abs(B[s0, s2].sum(1))) < tol              # G_02 1 = 0
+    # E_m only touches the obstacle's diagonal block
+    D = A - B
+    mask = np.zeros_like(D, dtype=bool)
+    mask[s2, s2] = True
+    assert np.max(np.abs(D[~mask])) == 0.0
+    assert np.max(np.abs(D[s2, s2] + 1.0 / g.counts[2])) < 1e-17
+
+
+def test_p2_row_sums_ragged_two_obstacles():
+    P = inputs.small_problem(96, 80, [48, 40], seed=3)
+    g = P.geometry
+    B = _build(g, variant=1)
+    A = _build(g, variant=0)
+    for m in (2, 3):
+        v = np.zeros(g.n)
+        v[g.component(m)] = 1.0
+        assert np.max(np.abs(B @ v)) < 1e-12
+        assert np.max(np.abs(A @ v + v)) < 1e-12
+
+
+def test_counterclockwise_obstacle_breaks_the_kernel():
+    """Orientation is part of the contract (reading R1): with a counter-clockwise
+    ellipse (1/2 I + K_mm) 1 = 1 instead of 0."""
+    P = inputs.make_config(1)
+    g = P.geometry
+    s2 = g.component(2)
+    # reverse the parameterisation of the obstacle: a -> -a
+    idx = np.r_[0, np.arange(g.counts[2] - 1, 0, -1)] + s2.start
+    z, dz, d2z = g.zeta.copy(), g.dzeta.copy(), g.d2zeta.copy()
+    z[s2], dz[s2], d2z[s2] = g.zeta[idx], -g.dzeta[idx], g.d2zeta[idx]
+    B = oracle.build_matrix(g.counts, g.kinds, z, dz, d2z, 1)
+    assert np.max(np.abs(B[s2, s2].sum(1) - 1.0)) < 1e-13
+
+
+# --------------------------------------------------------------------------------------------
+# P3 / P4  Cauchy-integral reproduction of an analytic function (north_star check)
+# --------------------------------------------------------------------------------------------
+def _cauchy_sum(g, omega, zpts):
+    """Trapezoid rule for Eq. (3.3), written with numpy's complex tan:
+    Phi_0(z) = (1/2 pi i) int (1/2)cot((zeta_0 - z)/2) omega_0 zeta_0' da, solids carry an extra i."""
+    out = np.zeros(len(zpts), dtype=np.complex128)
+    for k in range(g.counts.size):
+        s = g.component(k)
+        sig = 1.0 if g.kinds[k] == inputs.KIND_SURFACE else 1j
+        Mk = int(g.counts[k])
+        for i, z in enumerate(zpts):
+            ker = 0.5 / np.tan(0.5 * (g.zeta[s] - z))
+            out[i] += (sig / (1j * Mk)) * np.sum(ker * omega[s] * g.dzeta[s])
+    return out
+
+
+def _interior_points():
+    return np.array([0.3 - 0.4j, 2.0 - 0.5j, 4.0 - 1.5j, 5.5 - 0.45j, 1.0 - 1.6j, 3.1 - 0.3j])
+
+
+def _f_poles(z):
+    """2 pi-periodic, analytic in the fluid of the config-1-like geometries, with poles above the free
+    surface, inside the obstacle and below the bottom, so that ALL densities are excited (the entire
+    function e^{iz} alone is reproduced by the bottom density only: omega_0 = omega_2 = 0)."""
+    cot = lambda w: 1.0 / np.tan(w)
+    return (np.exp(1j * z) + 0.3 * cot(0.5 * (z - (1.0 + 0.6j)))
+            + (0.1 + 0.04j) * cot(0.5 * (z - (-1.0j))) + 0.1j * cot(0.5 * (z - (2.0 - 2.6j))))
+
+
+def _reproduction_error(g, f=_f_poles):
+    b = inputs.rhs_analytic(g, f)
+    A = _build(g)
+    x, iters, relres, hist, status = oracle.gmres(A, b, 1e-14, 60, 400)
+    assert status == 0
+    zp = _interior_points()
+    return np.max(np.abs(_cauchy_sum(g, x, zp) - f(zp))), x
+
+
+def test_p3_entire_function_uses_the_bottom_density_only():
+    """f = e^{iz} (config 1's right-hand side) is entire and decays upwards: no jump across Gamma_0 or the
+    obstacle, so omega_0 = 0 and omega_2 = 0 and Phi_1 alone reproduces f."""
+    P = inputs.make_config(1)
+    g = P.geometry
+    err, x = _reproduction_error(g, lambda z: np.exp(1j * z))
+    assert err < 2e-14
+    assert np.max(np.abs(x[g.component(0)])) < 1e-13 and np.max(np.abs(x[g.component(2)])) < 1e-13
+    assert np.max(np.abs(x[g.component(1)])) > 1.0
+
+
+def test_p3_analytic_function_reproduction_config1():
+    """b_0 = Re f, b_k = Im f for f = e^{iz}; by the uniqueness argument the sum of
+    Cauchy integrals equals f inside the fluid and <1_m, omega> = 0.  End-to-end pin of the whole
+    matrix (Plemelj 1/2, signs, Re/Im pattern, weights, diagonal, E_m) and of the solver."""
+    P = inputs.make_config(1)
+    g = P.geometry
+    err, x = _reproduction_error(g)
+    assert err < 2e-13, err
+    assert abs(np.mean(x[g.component(2)])) < 1e-13          # psi|_2 = <1_2, omega> = 0
+    for k in range(3):                                      # every density is excited by this f
+        assert np.max(np.abs(x[g.component(k)])) > 0.05
+
+
+def test_p3_fails_without_the_pieces():
+    """Mutation check of the pin itself: dropping the diagonal limit, flipping the sign of the
+    -G_k0 blocks, or using weights 1/M_k (target) instead of 1/M_j (source) must break P3."""
+    P = inputs.make_config(1)
+    g = P.geometry
+    f = _f_poles
+    b = inputs.rhs_analytic(g, f)
+    A = _build(g)
+    zp = _interior_points()
+    s0 = g.component(0)
+
+    def err_of(Am):
+        x = np.linalg.solve(Am, b)
+        return np.max(np.abs(_cauchy_sum(g, x, zp) - f(zp)))
+
+    assert err_of(A) < 2e-13
+    A1 = A.copy()
+    d = np.arange(g.n)
+    diag_k = np.imag(g.d2zeta / (2 * g.dzeta)) / np.repeat(g.counts, g.counts)
+    A1[d, d] -= diag_k
+    assert err_of(A1) > 1e-6
+    A2 = A.copy()
+    A2[s0.stop:, s0] *= -1.0
+    assert err_of(A2) > 1e-3
+    A3 = A.copy()
+    A3[s0, s0.stop:] *= -1.0
+    assert err_of(A3) > 1e-3
+
+
+def test_p4_spectral_convergence():
+    """Trapezoid collocation is spectrally accurate: the reproduction error decays
+    geometrically under refinement M -> 2M until roundoff."""
+    errs = []
+    for M in (16, 32, 64, 128, 256):
+        eta = inputs.Series(np.array([1.0, 2.0]), np.array([0.05 + 0j, 0.01 - 0.02j]))
+        geo = inputs.assemble([inputs.graph_curve(M, 0.0, eta),
+                               inputs.graph_curve(M, -2.0, None),
+                               inputs.ellipse_curve(M, -1.0j, 0.4, 0.2, 0.3)], [0, 1, 2])
+        errs.append(_reproduction_error(geo)[0])
+    assert errs[0] > 1e-3                    # under-resolved: the pin is sensitive
+    assert errs[1] < errs[0] / 10
+    assert errs[2] < errs[1] / 100
+    assert errs[3] < errs[2] / 1e4           # error ~ e^{-c M}: the decrements grow
+    assert errs[4] < 5e-14, errs             # roundoff floor
+
+
+# --------------------------------------------------------------------------------------------
+# P5  adaptive quadrature of the kernels of Table 1 on tiny inputs
+# --------------------------------------------------------------------------------------------
+def test_p5_rows_against_adaptive_quadrature():
+    """(1/2pi) int K_kj(alpha_m, beta) omega(beta) d beta by Gauss-Kronrod (scipy quad) on analytic
+    curves, integrand written from Table 1 with numpy's tan and set to the limit
+    Im{zeta''/(2 zeta')} at beta = alpha; compared with (matrix row) . (samples).
+    A missing diagonal term leaves an O(1/M) error; a wrong Re/Im or sign is O(1)."""
+    from scipy.integrate import quad
+
+    M0, M1, M2 = 64, 48, 40
+    c0 = lambda a: a + 1j * (0.1 * np.cos(a) + 0.03 * np.sin(2 * a))
+    d0 = lambda a: 1 + 1j * (-0.1 * np.sin(a) + 0.06 * np.cos(2 * a))
+    e0 = lambda a: 1j * (-0.1 * np.cos(a) - 0.12 * np.sin(2 * a))
+    c1 = lambda a: a + 1j * (-1.5 + 0.2 * np.cos(a))
+    d1 = lambda a: 1 + 1j * (-0.2 * np.sin(a))
+    e1 = lambda a: 1j * (-0.2 * np.cos(a))
+    rot, zc, q, bb = np.exp(0.4j), 3.0 - 0.7j, 0.35, 0.2
+    c2 = lambda a: zc + rot * (q * np.cos(a) - 1j * bb * np.sin(a))
+    d2 = lambda a: rot * (-q * np.sin(a) - 1j * bb * np.cos(a))
+    e2 = lambda a: rot * (-q * np.cos(a) + 1j * bb * np.sin(a))
+    curves = [(c0, d0, e0, M0), (c1, d1, e1, M1), (c2, d2, e2, M2)]
+    parts = []
+    for c, d, e, M in curves:
+        a = 2 * np.pi * np.arange(M) / M
+        parts.append((c(a), d(a), e(a)))
+    geo = inputs.assemble(parts, [0, 1, 2])
+    B = _build(geo, variant=1)
+    om = lambda b: 1.0 + 0.5 * np.cos(b) + 0.25 * np.sin(2 * b)
+
+    def kern(k, j, a, b):
+        ck, cj, dj, ej = curves[k][0], curves[j][0], curves[j][1], curves[j][2]
+        if k == j and abs(b - a) < 1e-9:
+            c = ej(a) / (2 * dj(a))
+        else:
+            c = 0.5 * dj(b) / np.tan(0.5 * (cj(b) - ck(a)))
+        if k == 0 and j == 0:
+            return c.imag
+        if k == 0:
+            return c.real
+        if j == 0:
+            return -c.real
+        return c.imag
+
+    for (k, m) in [(0, 5), (1, 17), (2, 3), (2, 21), (0, 40)]:
+        a = 2 * np.pi * m / curves[k][3]
+        row = geo.component(k).start + m
+        for j in range(3):
+            val, _ = quad(lambda b: kern(k, j, a, b) * om(b) / (2 * np.pi), 0, 2 * np.pi,
+                          points=[a] if k == j and a > 0 else None, epsabs=1e-13, epsrel=1e-13, limit=400)
+            sj = geo.component(j)
+            bj = 2 * np.pi * np.arange(curves[j][3]) / curves[j][3]
+            num = B[row, sj] @ om(bj)
+            if k == j:  # remove the +-1/2 identity
+                num -= (-0.5 if k == 0 else 0.5) * om(a)
+            assert abs(num - val) < 2e-11, (k, m, j, num, val)
+
+
+# --------------------------------------------------------------------------------------------
+# P6  flat surface over flat bottom: closed-form solution of the linear system
+# --------------------------------------------------------------------------------------------
+def test_p6_flat_flat_closed_form_solution():
+    """zeta_0 = a, zeta_1 = a - iH, b = (cos p a, 0):  omega_0 = -2 cos(pa)/(1+e^{-2pH}),
+    omega_1 = 2 e^{-pH} sin(pa)/(1+e^{-2pH})  (Fourier analysis of Table 1 for flat boundaries)."""
+    M0, M1, H, p = 64, 48, 1.3, 3
+    geo = inputs.flat_flat(M0, M1, H)
+    A = _build(geo)
+    a0 = 2 * np.pi * np.arange(M0) / M0
+    a1 = 2 * np.pi * np.arange(M1) / M1
+    # operator identities G_01 cos(p.) = -1/2 e^{-pH} sin(p.), G_01 sin(p.) = 1/2 e^{-pH} cos(p.)
+    G01 = A[:M0, M0:]
+    assert np.max(np.abs(G01 @ np.cos(p * a1) + 0.5 * np.exp(-p * H) * np.sin(p * a0))) < 1e-14
+    assert np.max(np.abs(G01 @ np.sin(p * a1) - 0.5 * np.exp(-p * H) * np.cos(p * a0))) < 1e-14
+    b = np.concatenate([np.cos(p * a0), np.zeros(M1)])
+    x, iters, relres, hist, status = oracle.gmres(A, b, 1e-14, 50, 200)
+    assert status == 0 and relres < 1e-13
+    den = 1 + np.exp(-2 * p * H)
+    assert np.max(np.abs(x[:M0] + 2 * np.cos(p * a0) / den)) < 1e-13
+    assert np.max(np.abs(x[M0:] - 2 * np.exp(-p * H) * np.sin(p * a1) / den)) < 1e-13
+
+
+# --------------------------------------------------------------------------------------------
+# P7  GMRES against LAPACK and its own invariants
+# --------------------------------------------------------------------------------------------
+def test_p7_gmres_matches_lapack_and_is_monotone():
+    rng = np.random.default_rng(11)
+    n = 120
+    A = np.eye(n) * 0.5 + rng.standard_normal((n, n)) / (4 * np.sqrt(n))
+    b = rng.standard_normal(n)
+    xref = np.linalg.solve(A, b)
+    for restart in (n, 25, 7):
+        x, iters, relres, hist, status = oracle.gmres(A, b, 1e-13, restart, 2000)
+        assert status == 0
+        assert relres <= 2e-13
+        assert np.linalg.norm(x - xref) / np.linalg.norm(xref) < 1e-11
+        assert np.all(np.diff(hist) <= 1e-15), "recurrence residual must not increase"
+        assert hist[-1] <= 1e-13 and (iters < 2 or hist[-2] > 1e-13), "stops at the first step below tol"
+        assert iters <= n if restart == n else True
+    # unrestarted GMRES terminates in at most n steps on any nonsingular matrix
+    x, iters, *_ = oracle.gmres(A, b, 1e-13, n, 2000)
+    assert iters <= n
+
+
+def test_p7_gmres_krylov_exactness_low_rank():
+    """A = I + (rank-3): GMRES converges in at most 4 steps (minimal polynomial degree 4)."""
+    rng = np.random.default_rng(2)
+    n = 60
+    U = rng.standard_normal((n, 3))
+    W = rng.standard_normal((n, 3))
+    A = np.eye(n) + U @ W.T / n
+    b = rng.standard_normal(n)
+    x, iters, relres, hist, status = oracle.gmres(A, b, 1e-12, 30, 100)
+    assert status == 0 and iters <= 4
+    assert np.linalg.norm(A @ x - b) / np.linalg.norm(b) < 1e-12
+
+
+def test_p7_gmres_edge_cases():
+    A = np.array([[2.0, 0.0], [0.0, 4.0]])
+    x, iters, relres, hist, status = oracle.gmres(A, np.zeros(2), 1e-13, 5, 10)
+    assert iters == 0 and status == 0 and np.all(x == 0)
+    x, iters, relres, hist, status = oracle.gmres(A, np.array([1.0, 1.0]), 1e-13, 5, 1)
+    assert iters == 1 and status == 1  # max_iters reached, x is the 1-step minimiser
+    x, iters, relres, hist, status = oracle.gmres(A, np.array([1.0, 0.0]), 1e-13, 5, 10)
+    assert iters == 1 and status == 0 and abs(x[0] - 0.5) < 1e-16  # lucky breakdown
+
+
+def test_matvec_is_the_plain_definition():
+    rng = np.random.default_rng(4)
+    A = rng.standard_normal((37, 37))
+    x = rng.standard_normal(37)
+    y = oracle.matvec(A, x)
+    import math
+    for i in (0, 13, 36):
+        assert abs(y[i] - math.fsum(A[i, j] * x[j] for j in range(37))) < 1e-14
+
+
+def test_config_iteration_counts_in_paper_range():
+    """Plausibility only (i_max 30-120 at tol 1e-15): configs 1-2 at tol 1e-13."""
+    for c, lo, hi in ((1, 10, 40), (2, 20, 60)):
+        P = inputs.make_config(c)
+        A = _build(P.geometry)
+        x, iters, relres, hist, status = oracle.gmres(A, P.rhs[0], P.tol, P.restart, P.max_iters)
+        assert status == 0 and lo <= iters <= hi and relres < 2e-13
