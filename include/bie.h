@@ -1,0 +1,169 @@
+/*
+ * bie.h -- C ABI of the B200-native boundary-integral hot path of arXiv 2108.01786
+ *          (Ambrose, Camassa, Marzuola, McLaughlin, Robinson, Wilkening: "Numerical Algorithms for
+ *          Water Waves with Background Flow over Obstacles and Topography").
+ *
+ * PAPER.md below is /root/reference/PAPER.md; a citation is a line range plus the equation it falls in.
+ *
+ * The path: (a) dense construction of the collocation matrix of Eq. (3.16) whose
+ * entries are the periodised Cauchy kernel zeta'_j/2 cot((zeta_j - zeta_k)/2) of Table 1
+ * on the trapezoidal rule, with the analytic diagonal limit
+ * (PAPER.md:L265), the +-1/2 I of Eq. (3.10) and the rank-(N-1) stream-function
+ * correction E_m; (b) restarted GMRES on that system: dense FP64
+ * matvec, Gram-Schmidt, Givens rotations, all on the device.
+ *
+ * Conventions common to all calls
+ *   - Everything is FP64.  Complex arrays are interleaved (re, im) doubles.
+ *   - "dev" pointers are device memory of the ctx's GPU, caller-owned, 16-byte aligned; "host" pointers
+ *     are ordinary host memory.  The library never frees or keeps caller buffers beyond a call, except
+ *     that the node tables derived from the last geometry live in the ctx (O(n) bytes, grown on demand).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls are
+ *     asynchronous on it unless stated otherwise.
+ *   - Components: component 0 is the free surface Gamma_0, component 1 the bottom
+ *     Gamma_1, components 2.. the obstacles, parameterised CLOCKWISE (fluid on the left of solids, on
+ *     the right of Gamma_0).  counts[c] = M_c nodes at alpha_{cl} = 2 pi l / M_c;
+ *     n = sum_c M_c.  Node arrays hold the components concatenated in this order.
+ *   - Matrices are row-major, row = target node (k,m), column = source node (j,l), leading dimension
+ *     lda >= n, lda even (so that every row is 16-byte aligned).
+ *   - Return value: 0 = OK; > 0 = numerical status (BIE_MAX_ITERS: outputs still valid);
+ *     < 0 = error, nothing useful was written.  -(100 + e) reports cudaError_t e.  No exceptions cross
+ *     the ABI.  There is no CPU fallback: without an sm_100 device bie_create fails.
+ */
+#ifndef BIE_H
+#define BIE_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define BIE_OK 0
+#define BIE_MAX_ITERS 1        /* bie_gmres: max_iters reached before |g_{j+1}| <= tol ||b||        */
+#define BIE_ERR_NULL (-1)      /* a required pointer is NULL                                        */
+#define BIE_ERR_GEOMETRY (-2)  /* ncomp < 1, a count < 1, kinds not (0, 1?, 2, 2, ...), n too large  */
+#define BIE_ERR_LAYOUT (-3)    /* lda < n, lda odd, or a device pointer not 16-byte aligned          */
+#define BIE_ERR_WORKSPACE (-4) /* workspace too small (see bie_*_workspace_bytes)                    */
+#define BIE_ERR_DEVICE (-5)    /* not a compute-capability-10.x device                               */
+#define BIE_ERR_ARG (-6)       /* restart < 1, max_iters < 0, tol < 0, unknown variant/flags         */
+#define BIE_ERR_CUDA_BASE (-100)
+
+#define BIE_KIND_SURFACE 0
+#define BIE_KIND_BOTTOM 1
+#define BIE_KIND_OBSTACLE 2
+
+/* bie_build `variant` */
+#define BIE_VARIANT_A 0 /* Eq. (3.16): 1/2 I + K_mm - E_m on obstacle diagonal blocks  */
+#define BIE_VARIANT_B 1 /* the uncorrected operator B of Eq. (3.10), for invariants    */
+
+typedef struct bie_ctx bie_ctx;
+
+/* Creates a context on CUDA device `device` (makes it current for the calling thread during each call).
+ * Fails with BIE_ERR_DEVICE unless the device has compute capability 10.x (B200: sm_100a code only). */
+int bie_create(bie_ctx** ctx, int device);
+int bie_destroy(bie_ctx* ctx);
+
+/* Static, human-readable text for a return code. */
+const char* bie_strerror(int code);
+
+/* Number of SMs of the ctx's device and the FP64 FMA lanes per SM per clock the build roofline assumes
+ * (64 on sm_100).  Used by bench.py for the "alu" roofline denominators. */
+int bie_device_info(bie_ctx* ctx, int* sm_count, int* fp64_fma_per_sm_clk, int* l2_bytes_mib);
+
+/* ---------------------------------------------------------------------------------------------------
+ * (a) Matrix build, SURVEY 8(a) rows a1-a3.
+ *
+ * For target node t = (k,m) and source node s = (j,l), s != t (Table 1; weights
+ * 1/M_j PAPER.md:L302):
+ *        c = zeta'_j[l] / (2 M_j) * cot((zeta_j[l] - zeta_k[m]) / 2),
+ * and for s == t the limit   c = zeta''_k[m] / (2 zeta'_k[m] M_k).   Entry A[t][s]:
+ *        k = 0,  j = 0  :  Im c - 1/2 [s==t]                              (-1/2 I + K_00)
+ *        k = 0,  j >= 1 :  Re c                                           (G_0j)
+ *        k >= 1, j = 0  : -Re c                                           (-G_k0)
+ *        k >= 1, j >= 1 :  Im c + 1/2 [s==t] - [k == j is an obstacle]/M_k   (1/2 I + K_kj - E_k)
+ * (Eq. (3.10); Eq. (3.16) and E_m PAPER.md:L308-L324).  variant = BIE_VARIANT_B omits E_k.
+ *
+ * counts, kinds: host int32[ncomp].  kinds[0] must be BIE_KIND_SURFACE and no other component may be;
+ * at most one BIE_KIND_BOTTOM.  zeta, dzeta, d2zeta: dev, interleaved complex, length n.  The values are
+ * used exactly as given (no differentiation inside).  A: dev, n x lda doubles, fully overwritten in the
+ * first n columns of its n rows.
+ * Launches: one node-preparation kernel and one tile kernel.  The node tables stay in the ctx for
+ * bie_matvec_free / bie_gmres(A == NULL).
+ */
+int bie_build(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds,
+              const double* zeta, const double* dzeta, const double* d2zeta,
+              int variant, double* A, int64_t lda, void* stream);
+
+/* rebuild only the blocks that involve component 0 (row block 0 and column block 0),
+ * for a sequence of stages in which only the free surface moved (solids "do not change in time",
+ * PAPER.md:L498).  Same arguments as bie_build; the solid-solid blocks of A are left untouched. */
+int bie_build_update(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds,
+                     const double* zeta, const double* dzeta, const double* d2zeta,
+                     int variant, double* A, int64_t lda, void* stream);
+
+/* Prepares the node tables of a geometry in the ctx without writing a matrix (for the matrix-free
+ * operator).  Same geometry arguments as bie_build. */
+int bie_set_geometry(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds,
+                     const double* zeta, const double* dzeta, const double* d2zeta,
+                     int variant, void* stream);
+
+/* ---------------------------------------------------------------------------------------------------
+ * (b) Matvec:  y = A x   (dev, dev, dev; x and y of length n, must not alias).
+ * bie_matvec reads the stored matrix (HBM-bound); bie_matvec_free recomputes the entries of the geometry
+ * last given to bie_build / bie_set_geometry on the fly (FP64-bound, no matrix traffic).
+ */
+int bie_matvec(bie_ctx* ctx, int n, const double* A, int64_t lda, const double* x, double* y, void* stream);
+int bie_matvec_free(bie_ctx* ctx, int n, const double* x, double* y, void* stream);
+
+/* ---------------------------------------------------------------------------------------------------
+ * (c) Restarted GMRES(restart), SURVEY 8(a) rows a5-a10 (Saad & Schultz, ref. [38] cited at
+ * PAPER.md:L855), unpreconditioned, x0 = 0, on the system as stored:
+ *   cycle:  r = b - A x (first cycle r = b), beta = ||r||, v_1 = r/beta, g = beta e_1;
+ *   step j: w = A v_j; orthogonalise w against v_1..v_j by classical Gram-Schmidt applied twice (CGS2);
+ *           h_{j+1,j} = ||w||, v_{j+1} = w/h_{j+1,j}; previous Givens rotations on column j of H, new
+ *           rotation, g_{j+1} = -s_j g_j; iters += 1; stop when |g_{j+1}| <= tol * ||b||
+ *           (the criterion behind i_max) or iters == max_iters;
+ *   cycle end: y = R^{-1} g, x += V y; restart if not converged.
+ * The whole solve is ONE cooperative kernel launch; nothing returns to the host until it ends.
+ *
+ * A == NULL selects the matrix-free operator of the ctx's current geometry (then lda is ignored and n must
+ * match it).  rhs, x: dev, length n.  iters_out (int32) and relres_out (double: TRUE relative residual
+ * ||b - A x|| / ||b||, reported, never used to continue) are DEVICE pointers (may be NULL).
+ * workspace: dev, at least bie_gmres_workspace_bytes(n, restart) bytes, contents undefined afterwards.
+ * Returns BIE_OK immediately after the launch (convergence status is in *iters_out vs max_iters, and in
+ * status_out if not NULL: dev int32, 0 converged / 1 max_iters / 2 breakdown (h_{j+1,j} == 0, converged)).
+ */
+size_t bie_gmres_workspace_bytes(int n, int restart);
+int bie_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, const double* rhs,
+              double tol, int restart, int max_iters,
+              double* x, int32_t* iters_out, double* relres_out, int32_t* status_out,
+              void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------------------------------
+ * End-to-end call with HOST buffers (what bench.py's "e2e" times): copies the node data and rhs to the
+ * device, builds A, solves, copies x / iters / relres back and SYNCHRONISES the stream before returning.
+ * zeta, dzeta, d2zeta, rhs, x: host (pinned memory makes the copies asynchronous).  dev_workspace: dev, at
+ * least bie_solve_workspace_bytes(n, restart) bytes (holds node data, A with lda = n rounded up to even,
+ * rhs, x and the GMRES workspace).  matrix_free != 0 skips the dense matrix and solves with the
+ * matrix-free operator.  Returns BIE_OK, BIE_MAX_ITERS or an error.
+ */
+size_t bie_solve_workspace_bytes(int n, int restart, int matrix_free);
+int bie_solve_host(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds,
+                   const double* zeta, const double* dzeta, const double* d2zeta, const double* rhs,
+                   double tol, int restart, int max_iters, int matrix_free,
+                   double* x, int32_t* iters_out, double* relres_out,
+                   void* dev_workspace, size_t dev_workspace_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------------------------------
+ * Roofline probe (measurement support, not part of the method): launches a kernel of dependent-chain-free
+ * DFMA work, `fma_per_thread` FMAs in each of grid*block threads filling every SM, so that bench.py can
+ * time the FP64 pipe's sustained rate on this very GPU.  out: dev, >= 8 bytes (keeps the work alive).
+ * *total_fma (host) receives the number of FMAs issued.
+ */
+int bie_probe_dfma(bie_ctx* ctx, int64_t fma_per_thread, double* out, int64_t* total_fma, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BIE_H */

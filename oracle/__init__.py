@@ -41,7 +41,11 @@ def lib() -> ctypes.CDLL:
         L.oracle_cot_half.argtypes = [ctypes.c_double, ctypes.c_double, dp, dp]
         L.oracle_build.restype = ctypes.c_int
         L.oracle_build.argtypes = [ctypes.c_int, ip, ip, dp, dp, dp, ctypes.c_int, dp, ctypes.c_long]
+        L.oracle_build_rows.restype = ctypes.c_int
+        L.oracle_build_rows.argtypes = [ctypes.c_int, ip, ip, dp, dp, dp, ctypes.c_int, ctypes.c_long,
+                                        ctypes.POINTER(ctypes.c_long), dp]
         L.oracle_matvec.argtypes = [ctypes.c_long, dp, ctypes.c_long, dp, dp]
+        L.oracle_matvec_rect.argtypes = [ctypes.c_long, ctypes.c_long, dp, ctypes.c_long, dp, dp]
         L.oracle_gmres.restype = ctypes.c_int
         L.oracle_gmres.argtypes = [ctypes.c_long, dp, ctypes.c_long, dp, ctypes.c_double, ctypes.c_int,
                                    ctypes.c_int, dp, ip, dp, dp]
@@ -94,12 +98,29 @@ def build_matrix(counts, kinds, zeta, dzeta, d2zeta, variant: int = 0,
     return A
 
 
+def build_rows(counts, kinds, zeta, dzeta, d2zeta, rows, variant: int = 0) -> np.ndarray:
+    """The listed rows of build_matrix's result (len(rows) x n)."""
+    counts = np.ascontiguousarray(counts, dtype=np.int32)
+    kinds = np.ascontiguousarray(kinds, dtype=np.int32)
+    rows = np.ascontiguousarray(rows, dtype=np.int64)
+    n = int(counts.sum())
+    z, dz, d2z = _c128_as_f64(zeta), _c128_as_f64(dzeta), _c128_as_f64(d2zeta)
+    out = np.empty((rows.size, n), dtype=np.float64)
+    rc = lib().oracle_build_rows(int(counts.size), _ip(counts), _ip(kinds), _dp(z), _dp(dz), _dp(d2z),
+                                 int(variant), rows.size, rows.ctypes.data_as(ctypes.POINTER(ctypes.c_long)), _dp(out))
+    if rc != 0:
+        raise ValueError(f"oracle_build_rows failed: {rc}")
+    return out
+
+
 def matvec(A: np.ndarray, x: np.ndarray) -> np.ndarray:
+    """y = A x for a C-contiguous (nrows x ncols) block, ncols = len(x)."""
     A = np.ascontiguousarray(A, dtype=np.float64)
     x = np.ascontiguousarray(x, dtype=np.float64)
-    n = A.shape[0]
-    y = np.empty(n, dtype=np.float64)
-    lib().oracle_matvec(n, _dp(A), A.shape[1], _dp(x), _dp(y))
+    nrows, ncols = A.shape
+    assert x.size == ncols
+    y = np.empty(nrows, dtype=np.float64)
+    lib().oracle_matvec_rect(nrows, ncols, _dp(A), ncols, _dp(x), _dp(y))
     return y
 
 

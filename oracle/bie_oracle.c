@@ -64,6 +64,47 @@ void oracle_cot_half(double x, double y, double *re, double *im)
     *im = -(sh * ch) / d;
 }
 
+/* One row (target node t) of the matrix of Eq. (3.16); the formulas are documented at oracle_build below.
+ * comp[s] = component of node s. */
+static void oracle_row(long t, long n, const int *comp, const int *counts, const int *kinds,
+                       const double *zeta, const double *dzeta, const double *d2zeta, int variant, double *row)
+{
+    const int k = comp[t];
+    const double ztr = zeta[2 * t], zti = zeta[2 * t + 1];
+    for (long s = 0; s < n; ++s) {
+        const int j = comp[s];
+        const double Mj = (double)counts[j];
+        double cre, cim;
+        if (s == t) {
+            /* zeta'' / (2 zeta' M) */
+            double ar = d2zeta[2 * s], ai = d2zeta[2 * s + 1];
+            double br = dzeta[2 * s], bi = dzeta[2 * s + 1];
+            double den = br * br + bi * bi;
+            cre = (ar * br + ai * bi) / den / (2.0 * Mj);
+            cim = (ai * br - ar * bi) / den / (2.0 * Mj);
+        } else {
+            double x = zeta[2 * s] - ztr, y = zeta[2 * s + 1] - zti;
+            double cr, ci;
+            oracle_cot_half(x, y, &cr, &ci);
+            double qr = dzeta[2 * s] / (2.0 * Mj), qi = dzeta[2 * s + 1] / (2.0 * Mj);
+            cre = qr * cr - qi * ci;
+            cim = qr * ci + qi * cr;
+        }
+        double e;
+        if (k == 0 && j == 0)
+            e = cim - (s == t ? 0.5 : 0.0);
+        else if (k == 0)
+            e = cre;
+        else if (j == 0)
+            e = -cre;
+        else {
+            e = cim + (s == t ? 0.5 : 0.0);
+            if (variant == 0 && k == j && kinds[k] == 2) e -= 1.0 / Mj;
+        }
+        row[s] = e;
+    }
+}
+
 /* Matrix of Eq. (3.16).
  *
  * components: c = 0..ncomp-1 with counts[c] = M_c nodes alpha_{cl} = 2 pi l / M_c,
@@ -100,57 +141,59 @@ int oracle_build(int ncomp, const int *counts, const int *kinds,
             for (int l = 0; l < counts[c]; ++l) comp[p++] = c;
     }
 #pragma omp parallel for schedule(static)
-    for (long t = 0; t < n; ++t) {
-        const int k = comp[t];
-        const double ztr = zeta[2 * t], zti = zeta[2 * t + 1];
-        double *row = A + t * lda;
-        for (long s = 0; s < n; ++s) {
-            const int j = comp[s];
-            const double Mj = (double)counts[j];
-            double cre, cim;
-            if (s == t) {
-                /* zeta'' / (2 zeta' M) */
-                double ar = d2zeta[2 * s], ai = d2zeta[2 * s + 1];
-                double br = dzeta[2 * s], bi = dzeta[2 * s + 1];
-                double den = br * br + bi * bi;
-                cre = (ar * br + ai * bi) / den / (2.0 * Mj);
-                cim = (ai * br - ar * bi) / den / (2.0 * Mj);
-            } else {
-                double x = zeta[2 * s] - ztr, y = zeta[2 * s + 1] - zti;
-                double cr, ci;
-                oracle_cot_half(x, y, &cr, &ci);
-                double qr = dzeta[2 * s] / (2.0 * Mj), qi = dzeta[2 * s + 1] / (2.0 * Mj);
-                cre = qr * cr - qi * ci;
-                cim = qr * ci + qi * cr;
-            }
-            double e;
-            if (k == 0 && j == 0)
-                e = cim - (s == t ? 0.5 : 0.0);
-            else if (k == 0)
-                e = cre;
-            else if (j == 0)
-                e = -cre;
-            else {
-                e = cim + (s == t ? 0.5 : 0.0);
-                if (variant == 0 && k == j && kinds[k] == 2) e -= 1.0 / Mj;
-            }
-            row[s] = e;
-        }
-    }
+    for (long t = 0; t < n; ++t)
+        oracle_row(t, n, comp, counts, kinds, zeta, dzeta, d2zeta, variant, A + t * lda);
     free(comp);
     return 0;
 }
 
-/* y = A x, plain definition, long-double accumulation so the oracle is the more accurate side. */
-void oracle_matvec(long n, const double *A, long lda, const double *x, double *y)
+/* The listed rows of the same matrix (for sampled parity checks at sizes where the full matrix is too
+ * slow): out is nrows x n, row i = row rows[i] of oracle_build's A.  Same arithmetic, same row function. */
+int oracle_build_rows(int ncomp, const int *counts, const int *kinds,
+                      const double *zeta, const double *dzeta, const double *d2zeta,
+                      int variant, long nrows, const long *rows, double *out)
+{
+    if (ncomp < 1 || !counts || !kinds || !zeta || !dzeta || !d2zeta || !rows || !out) return -1;
+    long n = 0;
+    for (int c = 0; c < ncomp; ++c) {
+        if (counts[c] < 1) return -2;
+        if (kinds[c] < 0 || kinds[c] > 2) return -2;
+        if ((kinds[c] == 0) != (c == 0)) return -2;
+        n += counts[c];
+    }
+    for (long i = 0; i < nrows; ++i)
+        if (rows[i] < 0 || rows[i] >= n) return -3;
+    int *comp = (int *)malloc(sizeof(int) * (size_t)n);
+    if (!comp) return -4;
+    {
+        long p = 0;
+        for (int c = 0; c < ncomp; ++c)
+            for (int l = 0; l < counts[c]; ++l) comp[p++] = c;
+    }
+#pragma omp parallel for schedule(static)
+    for (long i = 0; i < nrows; ++i)
+        oracle_row(rows[i], n, comp, counts, kinds, zeta, dzeta, d2zeta, variant, out + i * n);
+    free(comp);
+    return 0;
+}
+
+/* y = A x for a rectangular nrows x ncols block, plain definition, long-double accumulation so the
+ * oracle is the more accurate side. */
+void oracle_matvec_rect(long nrows, long ncols, const double *A, long lda, const double *x, double *y)
 {
 #pragma omp parallel for schedule(static)
-    for (long i = 0; i < n; ++i) {
+    for (long i = 0; i < nrows; ++i) {
         const double *row = A + i * lda;
         long double acc = 0.0L;
-        for (long j = 0; j < n; ++j) acc += (long double)row[j] * (long double)x[j];
+        for (long j = 0; j < ncols; ++j) acc += (long double)row[j] * (long double)x[j];
         y[i] = (double)acc;
     }
+}
+
+/* y = A x, square. */
+void oracle_matvec(long n, const double *A, long lda, const double *x, double *y)
+{
+    oracle_matvec_rect(n, n, A, lda, x, y);
 }
 
 static double dot_ld(long n, const double *a, const double *b)

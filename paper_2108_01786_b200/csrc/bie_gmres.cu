@@ -1,0 +1,432 @@
+// bie_gmres.cu -- SURVEY 8(a) rows a5-a10: restarted GMRES(m) (Saad & Schultz, ref. [38] cited at
+// PAPER.md:L855; stopping rule behind i_max) as ONE persistent cooperative kernel.
+//
+// The paper ran the GEMV on the GPU and shipped every Krylov vector over PCIe to orthogonalise on the CPU
+// (PAPER.md:L857).  Here nothing leaves the device: one CTA per SM owns a contiguous block R of rows of A and,
+// with it, the same rows of every Krylov vector.  Per Arnoldi step
+//     w[R]  = A[R,:] v_j                     (bie_cta_gemv, HBM-bound; or bie_cta_matvec_free)
+//     h    += V_j^T w ; w -= V_j h           twice (CGS2): local dots over R, one grid barrier, fixed-order sum
+//     h_{j+1,j} = ||w||                      local sum of squares, one grid barrier
+// i.e. three grid barriers per step.  v_{j+1} is never broadcast normalised: the unnormalised w goes to a
+// global buffer before the norm barrier and every CTA scales it by 1/h_{j+1,j} while loading it into shared
+// memory for the next GEMV.  Every CTA reduces the per-CTA partials in the same fixed order, so all CTAs hold
+// bit-identical h, Givens rotations and residuals and take the same branch without further communication.
+// The Givens/least-squares part (a8) is a few hundred flops done redundantly by thread 0 of every CTA; CTA 0
+// keeps R and does the back-substitution (a9) at the end of a cycle.
+#include <cstring>
+#include "bie_common.cuh"
+#include "bie_gemv.cuh"
+#include "bie_free.cuh"
+
+#define GM_THREADS 512
+
+struct GmresArgs {
+    const double* A;
+    long long lda;
+    int n;
+    const double* b;
+    double tol;
+    int m;
+    int max_iters;
+    double* x;
+    int32_t* iters_out;
+    double* relres_out;
+    int32_t* status_out;
+    double* V;     // [(m+1)][nld]
+    double* wbuf;  // [nld]
+    double* part;  // [3][m+2][G]
+    double* R;     // [m][m+1]  column j at R + j*(m+1)
+    double* yv;    // [m]
+    unsigned int* sync;
+    int nld;
+    int rows_per_cta;
+    int chunk;
+    NodeTable nt;
+    CompTable ct;
+};
+
+// ---- grid barrier (cooperative launch guarantees co-residency) -------------------------------------
+__device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p)
+{
+    unsigned int v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void grid_barrier(unsigned int* ctr, unsigned int& target)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        target += gridDim.x;
+        __threadfence();
+        atomicAdd(ctr, 1u);
+        while (ld_acquire_u32(ctr) < target) { }
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+// sum over the CTA; result to all threads.  red: shared, >= 33 doubles
+__device__ __forceinline__ double block_sum(double v, double* red)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    v = bie_warp_sum(v);
+    __syncthreads();
+    if (lane == 0) red[warp] = v;
+    __syncthreads();
+    if (warp == 0) {
+        double s = (lane < (int)(blockDim.x >> 5)) ? red[lane] : 0.0;
+        s = bie_warp_sum(s);
+        if (lane == 0) red[32] = s;
+    }
+    __syncthreads();
+    return red[32];
+}
+
+// sum of the G per-CTA partials p[0..G), same order in every CTA; all lanes of the calling warp get it
+__device__ __forceinline__ double warp_sum_partials(const double* p, int G)
+{
+    double s = 0.0;
+    for (int c = threadIdx.x & 31; c < G; c += 32) s += __ldcg(p + c);
+    return bie_warp_sum(s);
+}
+
+template <bool STREAM, bool XS, bool FREE>
+__device__ __forceinline__ void cta_apply(const GmresArgs& a, int r0, int r1, const double* xin, double scale,
+                                          double* xs, double* gpart, double* y_local)
+{
+    if (FREE) {
+        bie_cta_matvec_free(a.nt, a.ct, r0, r1, xin, gpart, y_local);
+        if (scale != 1.0) {
+            for (int r = threadIdx.x; r < r1 - r0; r += blockDim.x) y_local[r] *= scale;
+            __syncthreads();
+        }
+    } else if (XS) {
+        const int n2 = a.n >> 1;
+        for (int i = threadIdx.x; i < n2; i += blockDim.x) {
+            double2 v = __ldcg(reinterpret_cast<const double2*>(xin) + i);
+            v.x *= scale; v.y *= scale;
+            reinterpret_cast<double2*>(xs)[i] = v;
+        }
+        if ((a.n & 1) && threadIdx.x == 0) xs[a.n - 1] = __ldcg(xin + a.n - 1) * scale;
+        __syncthreads();
+        bie_cta_gemv<STREAM, true>(a.A, a.lda, a.n, r0, r1, a.chunk, xs, gpart, y_local);
+    } else {
+        bie_cta_gemv<STREAM, false>(a.A, a.lda, a.n, r0, r1, a.chunk, xin, gpart, y_local);
+        if (scale != 1.0) {
+            for (int r = threadIdx.x; r < r1 - r0; r += blockDim.x) y_local[r] *= scale;
+            __syncthreads();
+        }
+    }
+}
+
+// one classical Gram-Schmidt pass against v_0..v_j: hloc[i] (+)= <v_i, w>, w -= sum_i <v_i, w> v_i
+__device__ __forceinline__ void cgs_pass(const GmresArgs& a, int r0, int rows, int j, double* part_slot,
+                                         double* w_local, double* hloc, double* hacc, bool accumulate,
+                                         unsigned int& target)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    const int G = gridDim.x;
+    for (int i = warp; i <= j; i += nwarp) {
+        const double* vi = a.V + (size_t)i * a.nld + r0;
+        double s = 0.0;
+        for (int r = lane; r < rows; r += 32) s = fma(vi[r], w_local[r], s);
+        s = bie_warp_sum(s);
+        if (lane == 0) part_slot[(size_t)i * G + blockIdx.x] = s;
+    }
+    grid_barrier(a.sync, target);
+    for (int i = warp; i <= j; i += nwarp) {
+        const double h = warp_sum_partials(part_slot + (size_t)i * G, G);
+        if (lane == 0) {
+            hloc[i] = h;
+            hacc[i] = accumulate ? hacc[i] + h : h;
+        }
+    }
+    __syncthreads();
+    for (int r = threadIdx.x; r < rows; r += blockDim.x) {
+        double s = 0.0;
+        const double* v = a.V + r0 + r;
+#pragma unroll 4
+        for (int i = 0; i <= j; ++i) s = fma(hloc[i], v[(size_t)i * a.nld], s);
+        w_local[r] -= s;
+    }
+    __syncthreads();
+}
+
+template <bool STREAM, bool XS, bool FREE>
+__global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArgs a)
+{
+    extern __shared__ __align__(16) double smem[];
+    const int G = gridDim.x;
+    const int n = a.n, m = a.m;
+    const int r0 = blockIdx.x * a.rows_per_cta;
+    const int r1 = min(r0 + a.rows_per_cta, n);
+    const int rows = r1 - r0;  // >= 1 by construction of the grid
+    const int rows2 = (a.rows_per_cta + 1) & ~1;
+    // shared layout
+    double* y_local = smem;               // [rows2]   result of the operator
+    double* w_local = y_local + rows2;    // [rows2]   the vector being orthogonalised
+    double* hcol = w_local + rows2;       // [m+2]     column j of H (accumulated h)
+    double* hloc = hcol + (m + 2);        // [m+2]     coefficients of the current pass
+    double* cs = hloc + (m + 2);          // [m]
+    double* sn = cs + m;                  // [m]
+    double* g = sn + m;                   // [m+1]
+    double* red = g + (m + 1);            // [34]
+    double* gpart = red + 34 + ((m & 1) ? 0 : 1);  // GEMV partials or matrix-free scratch (16-byte aligned)
+    double* xs = gpart + (FREE ? free_scratch_doubles(a.rows_per_cta)
+                               : ((gemv_part_doubles(a.rows_per_cta, n, a.chunk) + 1) & ~1));
+    double* part1 = a.part;
+    double* part2 = a.part + (size_t)(m + 2) * G;
+    double* part3 = a.part + 2 * (size_t)(m + 2) * G;
+    unsigned int target = 0;
+
+    // ---- a5: ||b||, x = 0 -------------------------------------------------------------------------
+    double p = 0.0;
+    for (int r = threadIdx.x; r < rows; r += blockDim.x) {
+        const double v = a.b[r0 + r];
+        p = fma(v, v, p);
+        a.x[r0 + r] = 0.0;
+    }
+    p = block_sum(p, red);
+    if (threadIdx.x == 0) part3[blockIdx.x] = p;
+    grid_barrier(a.sync, target);
+    const double bn = sqrt(warp_sum_partials(part3, G));
+    const double thresh = a.tol * bn;
+
+    int iters = 0, status = 0;
+    bool done = (bn == 0.0);
+    bool first = true;
+    while (!done) {
+        // ---- cycle start: r = b - A x ------------------------------------------------------------
+        if (first) {
+            for (int r = threadIdx.x; r < rows; r += blockDim.x) w_local[r] = a.b[r0 + r];
+            first = false;
+        } else {
+            cta_apply<STREAM, XS, FREE>(a, r0, r1, a.x, 1.0, xs, gpart, y_local);
+            for (int r = threadIdx.x; r < rows; r += blockDim.x) w_local[r] = a.b[r0 + r] - y_local[r];
+        }
+        __syncthreads();
+        p = 0.0;
+        for (int r = threadIdx.x; r < rows; r += blockDim.x) {
+            const double v = w_local[r];
+            p = fma(v, v, p);
+            a.wbuf[r0 + r] = v;
+        }
+        p = block_sum(p, red);
+        if (threadIdx.x == 0) part3[blockIdx.x] = p;
+        grid_barrier(a.sync, target);
+        const double beta = sqrt(warp_sum_partials(part3, G));
+        if (beta <= thresh) break;                         // converged (status 0)
+        if (iters >= a.max_iters) { status = BIE_MAX_ITERS; break; }
+        double inv = 1.0 / beta;
+        for (int r = threadIdx.x; r < rows; r += blockDim.x) a.V[r0 + r] = w_local[r] * inv;
+        if (threadIdx.x == 0) g[0] = beta;
+        __syncthreads();
+
+        // ---- Arnoldi steps ------------------------------------------------------------------------
+        int k = 0;
+        bool conv = false;
+        for (int j = 0; j < m; ++j) {
+            // a6: w = A v_j, with v_j = wbuf * inv
+            cta_apply<STREAM, XS, FREE>(a, r0, r1, a.wbuf, inv, xs, gpart, y_local);
+            for (int r = threadIdx.x; r < rows; r += blockDim.x) w_local[r] = y_local[r];
+            __syncthreads();
+            // a7: CGS2
+            cgs_pass(a, r0, rows, j, part1, w_local, hloc, hcol, false, target);
+            cgs_pass(a, r0, rows, j, part2, w_local, hloc, hcol, true, target);
+            p = 0.0;
+            for (int r = threadIdx.x; r < rows; r += blockDim.x) {
+                const double v = w_local[r];
+                p = fma(v, v, p);
+                a.wbuf[r0 + r] = v;
+            }
+            p = block_sum(p, red);
+            if (threadIdx.x == 0) part3[blockIdx.x] = p;
+            grid_barrier(a.sync, target);
+            const double hn = sqrt(warp_sum_partials(part3, G));
+            inv = (hn != 0.0) ? 1.0 / hn : 0.0;
+            {
+                double* vn = a.V + (size_t)(j + 1) * a.nld + r0;
+                for (int r = threadIdx.x; r < rows; r += blockDim.x) vn[r] = w_local[r] * inv;
+            }
+            // a8: Givens rotations on column j, new rotation, recurrence residual
+            if (threadIdx.x == 0) {
+                hcol[j + 1] = hn;
+                for (int i = 0; i < j; ++i) {
+                    const double t0 = cs[i] * hcol[i] + sn[i] * hcol[i + 1];
+                    const double t1 = -sn[i] * hcol[i] + cs[i] * hcol[i + 1];
+                    hcol[i] = t0;
+                    hcol[i + 1] = t1;
+                }
+                const double d = hypot(hcol[j], hcol[j + 1]);
+                if (d == 0.0) { cs[j] = 1.0; sn[j] = 0.0; }
+                else { cs[j] = hcol[j] / d; sn[j] = hcol[j + 1] / d; }
+                hcol[j] = d;
+                hcol[j + 1] = 0.0;
+                g[j + 1] = -sn[j] * g[j];
+                g[j] = cs[j] * g[j];
+            }
+            __syncthreads();
+            if (blockIdx.x == 0)
+                for (int i = threadIdx.x; i <= j; i += blockDim.x) a.R[(size_t)j * (m + 1) + i] = hcol[i];
+            ++iters;
+            k = j + 1;
+            conv = (fabs(g[j + 1]) <= thresh) || (hn == 0.0);
+            if (hn == 0.0 && !(fabs(g[j + 1]) <= thresh)) status = 2;
+            __syncthreads();
+            if (conv || iters >= a.max_iters) break;
+        }
+        // ---- a9: y = R^{-1} g (CTA 0), x += V y ---------------------------------------------------
+        if (blockIdx.x == 0) {
+            __syncthreads();
+            if (threadIdx.x < 32) {
+                const int lane = threadIdx.x;
+                for (int i = k - 1; i >= 0; --i) {
+                    double s = 0.0;
+                    for (int c = i + 1 + lane; c < k; c += 32) s = fma(a.R[(size_t)c * (m + 1) + i], hloc[c], s);
+                    s = bie_warp_sum(s);
+                    if (lane == 0) hloc[i] = (g[i] - s) / a.R[(size_t)i * (m + 1) + i];
+                    __syncwarp();
+                }
+                for (int i = lane; i < k; i += 32) a.yv[i] = hloc[i];
+            }
+        }
+        grid_barrier(a.sync, target);
+        for (int i = threadIdx.x; i < k; i += blockDim.x) hloc[i] = __ldcg(a.yv + i);
+        __syncthreads();
+        for (int r = threadIdx.x; r < rows; r += blockDim.x) {
+            double s = 0.0;
+            const double* v = a.V + r0 + r;
+            for (int i = 0; i < k; ++i) s = fma(hloc[i], v[(size_t)i * a.nld], s);
+            a.x[r0 + r] += s;
+        }
+        grid_barrier(a.sync, target);  // x complete (next residual / final residual read all of it)
+        if (conv) break;
+        if (iters >= a.max_iters) { status = BIE_MAX_ITERS; break; }
+    }
+
+    // ---- a10: outputs; true residual ||b - A x|| / ||b|| (reported only) -----------------------------
+    double relres = 0.0;
+    if (a.relres_out && bn != 0.0) {
+        cta_apply<STREAM, XS, FREE>(a, r0, r1, a.x, 1.0, xs, gpart, y_local);
+        p = 0.0;
+        for (int r = threadIdx.x; r < rows; r += blockDim.x) {
+            const double v = a.b[r0 + r] - y_local[r];
+            p = fma(v, v, p);
+        }
+        p = block_sum(p, red);
+        if (threadIdx.x == 0) part1[blockIdx.x] = p;
+        grid_barrier(a.sync, target);
+        relres = sqrt(warp_sum_partials(part1, G)) / bn;
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        if (a.iters_out) *a.iters_out = iters;
+        if (a.relres_out) *a.relres_out = relres;
+        if (a.status_out) *a.status_out = status;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------------
+static inline size_t al256(size_t b) { return (b + 255) & ~(size_t)255; }
+
+struct GmresPlan {
+    int G, rows_per_cta, chunk, nld;
+    bool xs, stream;
+    size_t smem;
+    size_t offV, offW, offP, offR, offY, total;
+};
+
+static int gmres_plan(int n, int restart, int sm_count, int max_smem, int l2_bytes, long long lda, bool free_op,
+                      GmresPlan* pl)
+{
+    const int m = restart;
+    pl->rows_per_cta = (n + sm_count - 1) / sm_count;
+    if (free_op && pl->rows_per_cta < 64) pl->rows_per_cta = 64 < n ? 64 : n;  // keep the lanes busy
+    pl->G = (n + pl->rows_per_cta - 1) / pl->rows_per_cta;
+    pl->chunk = gemv_chunk(pl->rows_per_cta, n, GM_THREADS / 32);
+    pl->nld = (n + 1) & ~1;
+    const int rows2 = (pl->rows_per_cta + 1) & ~1;
+    size_t base = 2 * (size_t)rows2 + 2 * (size_t)(m + 2) + 2 * (size_t)m + (size_t)(m + 1) + 34 + 1;
+    base += free_op ? (size_t)free_scratch_doubles(pl->rows_per_cta)
+                    : (size_t)((gemv_part_doubles(pl->rows_per_cta, n, pl->chunk) + 1) & ~1);
+    base *= sizeof(double);
+    pl->xs = !free_op && base + sizeof(double) * ((size_t)n + 2) <= (size_t)max_smem;
+    pl->smem = base + (pl->xs ? sizeof(double) * ((size_t)n + 2) : 0);
+    if (pl->smem > (size_t)max_smem) return BIE_ERR_ARG;
+    if (free_op && pl->rows_per_cta > 2 * FREE_THREADS) return BIE_ERR_ARG;
+    pl->stream = !free_op && (double)n * (double)lda * 8.0 > 0.6 * (double)l2_bytes;
+    size_t o = 0;
+    pl->offV = o; o += al256(sizeof(double) * (size_t)(m + 1) * pl->nld);
+    pl->offW = o; o += al256(sizeof(double) * (size_t)pl->nld);
+    pl->offP = o; o += al256(sizeof(double) * 3 * (size_t)(m + 2) * sm_count);
+    pl->offR = o; o += al256(sizeof(double) * (size_t)m * (m + 1));
+    pl->offY = o; o += al256(sizeof(double) * (size_t)m);
+    pl->total = o;
+    return BIE_OK;
+}
+
+size_t bie_gmres_ws_bytes(int n, int restart)
+{
+    if (n < 1 || restart < 1) return 0;
+    GmresPlan pl;
+    // the workspace layout does not depend on the operator or on the device beyond the SM count bound
+    const int m = restart;
+    const int nld = (n + 1) & ~1;
+    size_t o = 0;
+    o += al256(sizeof(double) * (size_t)(m + 1) * nld);
+    o += al256(sizeof(double) * (size_t)nld);
+    o += al256(sizeof(double) * 3 * (size_t)(m + 2) * 256);  // <= 256 SMs
+    o += al256(sizeof(double) * (size_t)m * (m + 1));
+    o += al256(sizeof(double) * (size_t)m);
+    (void)pl;
+    return o + 256;
+}
+
+template <bool STREAM, bool XS, bool FREE>
+static int launch_gmres(const GmresArgs& a, const GmresPlan& pl, cudaStream_t st)
+{
+    auto k = bie_gmres_kernel<STREAM, XS, FREE>;
+    BIE_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+    void* params[] = {(void*)&a};
+    BIE_CUDA(cudaLaunchCooperativeKernel((const void*)k, dim3(pl.G), dim3(GM_THREADS), params, pl.smem, st));
+    return BIE_OK;
+}
+
+int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, const double* rhs, double tol,
+                     int restart, int max_iters, double* x, int32_t* iters_out, double* relres_out,
+                     int32_t* status_out, void* ws, size_t ws_bytes, cudaStream_t st)
+{
+    if (!ctx || !rhs || !x || !ws) return BIE_ERR_NULL;
+    if (n < 1 || restart < 1 || max_iters < 0 || !(tol >= 0.0)) return BIE_ERR_ARG;
+    const bool free_op = (A == nullptr);
+    if (free_op) {
+        if (!ctx->have_geom || ctx->n != n) return BIE_ERR_GEOMETRY;
+    } else if (lda < n || (lda & 1) || (((uintptr_t)A) & 15u)) return BIE_ERR_LAYOUT;
+    if ((((uintptr_t)rhs) | ((uintptr_t)x)) & 15u) return BIE_ERR_LAYOUT;
+    if (!ctx->coop_ok) return BIE_ERR_DEVICE;
+    if (ctx->sm_count > 256) return BIE_ERR_DEVICE;
+    if (restart > n) restart = n;  // the Krylov space cannot exceed n
+    GmresPlan pl;
+    int rc = gmres_plan(n, restart, ctx->sm_count, ctx->max_smem_optin, ctx->l2_bytes, free_op ? n : lda, free_op, &pl);
+    if (rc != BIE_OK) return rc;
+    // align the caller's workspace to 256 bytes
+    uintptr_t base = ((uintptr_t)ws + 255) & ~(uintptr_t)255;
+    if (base - (uintptr_t)ws + pl.total > ws_bytes) return BIE_ERR_WORKSPACE;
+    GmresArgs a;
+    a.A = A; a.lda = lda; a.n = n; a.b = rhs; a.tol = tol; a.m = restart; a.max_iters = max_iters;
+    a.x = x; a.iters_out = iters_out; a.relres_out = relres_out; a.status_out = status_out;
+    a.V = (double*)(base + pl.offV);
+    a.wbuf = (double*)(base + pl.offW);
+    a.part = (double*)(base + pl.offP);
+    a.R = (double*)(base + pl.offR);
+    a.yv = (double*)(base + pl.offY);
+    a.sync = ctx->sync_buf;
+    a.nld = pl.nld; a.rows_per_cta = pl.rows_per_cta; a.chunk = pl.chunk;
+    if (free_op) { a.nt = bie_node_table(ctx); a.ct = ctx->comps; }
+    else { memset(&a.nt, 0, sizeof(a.nt)); memset(&a.ct, 0, sizeof(a.ct)); }
+    BIE_CUDA(cudaMemsetAsync(ctx->sync_buf, 0, sizeof(unsigned int), st));
+    if (free_op) return launch_gmres<false, false, true>(a, pl, st);
+    if (pl.stream) return pl.xs ? launch_gmres<true, true, false>(a, pl, st) : launch_gmres<true, false, false>(a, pl, st);
+    return pl.xs ? launch_gmres<false, true, false>(a, pl, st) : launch_gmres<false, false, false>(a, pl, st);
+}

@@ -1,0 +1,124 @@
+// bie_nodes.cu -- SURVEY 8(a) row a1: per-node factors of the pair arithmetic (see bie_common.cuh).
+//
+// One thread per node.  The only transcendentals of the whole matrix build are evaluated here, O(n) of
+// them: sincos(x/2), exp(+-y/2).  Also the source weight q = zeta'/(2 M_j), the complete
+// diagonal entry from the limit K_jj(a,a) = Im{zeta''/(2 zeta')} with the -+1/2 of
+// Eq. (3.10) and the -1/M_m of E_m.
+#include "bie_common.cuh"
+
+struct PrepArgs {
+    CompTable comps;
+    int kinds[BIE_MAX_COMP];
+};
+
+__global__ void __launch_bounds__(256)
+bie_prepare_nodes_kernel(PrepArgs pa, int n, int npad, int variant,
+                         const double2* __restrict__ zeta, const double2* __restrict__ dzeta,
+                         const double2* __restrict__ d2zeta, double* __restrict__ buf, int* __restrict__ comp)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= npad) return;
+    double* S = buf;
+    double* C = buf + (size_t)npad;
+    double* P = buf + 2 * (size_t)npad;
+    double* N = buf + 3 * (size_t)npad;
+    double* QR = buf + 4 * (size_t)npad;
+    double* QI = buf + 5 * (size_t)npad;
+    double* X = buf + 6 * (size_t)npad;
+    double* Y = buf + 7 * (size_t)npad;
+    double* DG = buf + 8 * (size_t)npad;
+    double* EM = buf + 9 * (size_t)npad;
+    if (i >= n) {  // padding: benign values, never stored to A
+        S[i] = 0.0; C[i] = 1.0; P[i] = 1.0; N[i] = 1.0; QR[i] = 0.0; QI[i] = 0.0;
+        X[i] = 0.0; Y[i] = 1.0e3; DG[i] = 0.0; EM[i] = 0.0; comp[i] = -1;
+        return;
+    }
+    int k = 0;
+    while (k + 1 < pa.comps.ncomp && i >= pa.comps.off[k + 1]) ++k;
+    const double M = (double)(pa.comps.off[k + 1] - pa.comps.off[k]);
+    const double2 z = zeta[i], dz = dzeta[i], d2 = d2zeta[i];
+    double s, c;
+    sincos(0.5 * z.x, &s, &c);
+    S[i] = s; C[i] = c;
+    P[i] = exp(0.5 * z.y);
+    N[i] = exp(-0.5 * z.y);
+    QR[i] = dz.x / (2.0 * M);
+    QI[i] = dz.y / (2.0 * M);
+    X[i] = z.x; Y[i] = z.y;
+    // Im{ zeta'' / (2 zeta' M) }
+    const double den = dz.x * dz.x + dz.y * dz.y;
+    double d = (d2.y * dz.x - d2.x * dz.y) / den / (2.0 * M);
+    const double em = (variant == BIE_VARIANT_A && pa.kinds[k] == BIE_KIND_OBSTACLE) ? 1.0 / M : 0.0;
+    d += (k == 0) ? -0.5 : 0.5;
+    d -= em;
+    DG[i] = d; EM[i] = em;
+    comp[i] = k;
+}
+
+NodeTable bie_node_table(const bie_ctx* ctx)
+{
+    NodeTable t;
+    const size_t np = (size_t)bie_npad(ctx->n);
+    t.S = ctx->node_buf;
+    t.C = ctx->node_buf + np;
+    t.P = ctx->node_buf + 2 * np;
+    t.N = ctx->node_buf + 3 * np;
+    t.QR = ctx->node_buf + 4 * np;
+    t.QI = ctx->node_buf + 5 * np;
+    t.X = ctx->node_buf + 6 * np;
+    t.Y = ctx->node_buf + 7 * np;
+    t.DIAG = ctx->node_buf + 8 * np;
+    t.EM = ctx->node_buf + 9 * np;
+    t.COMP = ctx->comp_buf;
+    t.n = ctx->n;
+    t.npad = (int)np;
+    return t;
+}
+
+int bie_prepare_nodes(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds,
+                      const double* zeta, const double* dzeta, const double* d2zeta, int variant,
+                      cudaStream_t st)
+{
+    if (!ctx || !counts || !kinds || !zeta || !dzeta || !d2zeta) return BIE_ERR_NULL;
+    if (ncomp < 1 || ncomp > BIE_MAX_COMP) return BIE_ERR_GEOMETRY;
+    if (variant != BIE_VARIANT_A && variant != BIE_VARIANT_B) return BIE_ERR_ARG;
+    long long n = 0;
+    int nbottom = 0;
+    for (int c = 0; c < ncomp; ++c) {
+        if (counts[c] < 1) return BIE_ERR_GEOMETRY;
+        if (kinds[c] < 0 || kinds[c] > 2) return BIE_ERR_GEOMETRY;
+        if ((kinds[c] == BIE_KIND_SURFACE) != (c == 0)) return BIE_ERR_GEOMETRY;
+        if (kinds[c] == BIE_KIND_BOTTOM) ++nbottom;
+        n += counts[c];
+    }
+    if (nbottom > 1 || n > (1 << 30)) return BIE_ERR_GEOMETRY;
+    if ((((uintptr_t)zeta) | ((uintptr_t)dzeta) | ((uintptr_t)d2zeta)) & 15u) return BIE_ERR_LAYOUT;
+    const int npad = bie_npad((int)n);
+    if (npad > ctx->cap) {
+        // grow the ctx's node storage (the only allocation outside bie_create; O(n) bytes)
+        if (ctx->node_buf) cudaFree(ctx->node_buf);
+        if (ctx->comp_buf) cudaFree(ctx->comp_buf);
+        ctx->node_buf = nullptr; ctx->comp_buf = nullptr; ctx->cap = 0;
+        BIE_CUDA(cudaMalloc((void**)&ctx->node_buf, sizeof(double) * BIE_NODE_ARRAYS * (size_t)npad));
+        BIE_CUDA(cudaMalloc((void**)&ctx->comp_buf, sizeof(int) * (size_t)npad));
+        ctx->cap = npad;
+    }
+    PrepArgs pa;
+    pa.comps.ncomp = ncomp;
+    pa.comps.off[0] = 0;
+    for (int c = 0; c < BIE_MAX_COMP; ++c) {
+        pa.kinds[c] = c < ncomp ? kinds[c] : 0;
+        pa.comps.off[c + 1] = c < ncomp ? pa.comps.off[c] + counts[c] : (int)n;
+    }
+    ctx->n = (int)n;
+    ctx->ncomp = ncomp;
+    ctx->variant = variant;
+    for (int c = 0; c < ncomp; ++c) { ctx->counts[c] = counts[c]; ctx->kinds[c] = kinds[c]; }
+    ctx->comps = pa.comps;
+    ctx->have_geom = 1;
+    bie_prepare_nodes_kernel<<<(npad + 255) / 256, 256, 0, st>>>(
+        pa, (int)n, npad, variant, (const double2*)zeta, (const double2*)dzeta, (const double2*)d2zeta,
+        ctx->node_buf, ctx->comp_buf);
+    BIE_CUDA(cudaGetLastError());
+    return BIE_OK;
+}

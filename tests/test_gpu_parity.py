@@ -1,0 +1,351 @@
+"""GPU parity: the CUDA path (through the C ABI, paper_2108_01786_b200.bie) against the CPU oracle (oracle/),
+element by element on the same seeded inputs.  Tolerances are BASELINE.json's north_star:
+
+    matrix entries   max|A_gpu - A_cpu| / max|A_cpu| <= 1e-12          (reading R7: max-norm)
+    GMRES solutions  ||x_gpu - x_cpu|| / ||x_cpu||   <= 1e-10 at tol 1e-13
+    iteration counts within +-1
+    matvec           max|y_gpu - y_cpu| / max|y_cpu| <= 1e-13          (n eps sqrt-sum bound)
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2108_01786_b200 import inputs
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL_ENTRY = 1e-12
+TOL_X = 1e-10
+TOL_MV = 1e-13
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    from paper_2108_01786_b200 import bie
+    assert torch.cuda.is_available(), "the gpu tests need a B200"
+    c = bie.Context(0)
+    yield c
+    c.close()
+
+
+_CFG = {}
+
+
+def cfg(i):
+    if i not in _CFG:
+        _CFG[i] = inputs.make_config(i)
+    return _CFG[i]
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def geo_dev(g):
+    return dev(g.zeta), dev(g.dzeta), dev(g.d2zeta)
+
+
+def gpu_build(ctx, g, variant=0, lda=None, fill=None):
+    n = g.n
+    lda = lda or (n + (n & 1))
+    A = torch.empty((n, lda), dtype=torch.float64, device="cuda")
+    if fill is not None:
+        A.fill_(fill)
+    z, dz, d2z = geo_dev(g)
+    ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A, variant=variant)
+    torch.cuda.synchronize()
+    return A
+
+
+def oracle_build(g, variant=0):
+    return oracle.build_matrix(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, variant)
+
+
+def rel_max(a, b):
+    return float(np.max(np.abs(a - b)) / np.max(np.abs(b)))
+
+
+# ------------------------------------------------------------------------------------------------
+# (a) build
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("c", [1, 2, 3])
+def test_build_parity_full_matrix(ctx, c):
+    g = cfg(c).geometry
+    A = gpu_build(ctx, g)[:, :g.n].cpu().numpy()
+    Ao = oracle_build(g)
+    assert np.all(np.isfinite(A))
+    assert rel_max(A, Ao) <= TOL_ENTRY
+
+
+def test_build_variant_b_and_padding_untouched(ctx):
+    g = cfg(1).geometry
+    n = g.n
+    A = gpu_build(ctx, g, variant=1, lda=n + 6, fill=7.0).cpu().numpy()
+    assert rel_max(A[:, :n], oracle_build(g, 1)) <= TOL_ENTRY
+    assert np.all(A[:, n:] == 7.0)  # columns beyond n belong to the caller
+
+
+@pytest.mark.parametrize("shape", [(37, 29, [19, 23]), (5, 3, []), (1, 1, [1]), (64, 64, [64]), (300, 171, [33, 2, 129]),
+                                   (257, 255, [130])])
+def test_build_ragged_sizes(ctx, shape):
+    """counts that are not multiples of the tile, odd n, single-node components, no obstacle"""
+    P = inputs.small_problem(*shape, seed=3)
+    g = P.geometry
+    for variant in (0, 1):
+        A = gpu_build(ctx, g, variant=variant)[:, :g.n].cpu().numpy()
+        assert rel_max(A, oracle_build(g, variant)) <= TOL_ENTRY
+
+
+def test_build_flat_flat_no_obstacle(ctx):
+    g = inputs.flat_flat(48, 40, 0.7)
+    A = gpu_build(ctx, g)[:, :g.n].cpu().numpy()
+    assert rel_max(A, oracle_build(g)) <= TOL_ENTRY
+
+
+def _sample_rows(g, rng, k=48):
+    off = g.offsets
+    rows = set(int(r) for r in rng.integers(0, g.n, size=k))
+    for o in off[:-1]:
+        rows.update([int(o), int(o) + 1])
+    for o in off[1:]:
+        rows.update([int(o) - 1])
+    return np.array(sorted(rows), dtype=np.int64)
+
+
+@pytest.mark.parametrize("c", [4, 5])
+def test_build_parity_full_size_sampled_rows(ctx, c):
+    """BASELINE.json's large configs in the launch configuration bench.py times: the whole matrix is built on
+    the GPU; sampled rows (random + both ends of every component) are compared element by element."""
+    g = cfg(c).geometry
+    A = gpu_build(ctx, g)
+    rows = _sample_rows(g, np.random.default_rng(c))
+    Ag = A[torch.from_numpy(rows).cuda(), :g.n].cpu().numpy()
+    Ao = oracle.build_rows(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, rows)
+    assert np.all(np.isfinite(Ag))
+    assert float(np.max(np.abs(Ag - Ao))) <= TOL_ENTRY * 0.5  # max|A| >= 0.5 (the +-1/2 diagonal)
+    # property that holds at any size: every finite-entry check on the whole matrix
+    assert bool(torch.isfinite(A[:, :g.n]).all())
+    del A
+
+
+def test_build_update_only_touches_surface_blocks(ctx):
+    """a4: after Gamma_0 moved, bie_build_update rewrites row block 0 and column block 0 and leaves the
+    solid-solid blocks -- the result equals a full build of the new geometry."""
+    P = cfg(4)
+    g0, g1 = P.stages[0], P.stages[1]
+    A = gpu_build(ctx, g0)
+    z, dz, d2z = geo_dev(g1)
+    ctx.bie_build_update(g1.counts, g1.kinds, z, dz, d2z, A)
+    torch.cuda.synchronize()
+    rows = _sample_rows(g1, np.random.default_rng(11), k=24)
+    Ag = A[torch.from_numpy(rows).cuda(), :g1.n].cpu().numpy()
+    Ao = oracle.build_rows(g1.counts, g1.kinds, g1.zeta, g1.dzeta, g1.d2zeta, rows)
+    assert float(np.max(np.abs(Ag - Ao))) <= TOL_ENTRY * 0.5
+    # and a marker written into a solid-solid entry survives an update (those tiles are not rewritten)
+    M0 = int(g1.counts[0])
+    A[M0 + 300, M0 + 700] = 123.0
+    ctx.bie_build_update(g1.counts, g1.kinds, z, dz, d2z, A)
+    torch.cuda.synchronize()
+    assert float(A[M0 + 300, M0 + 700]) == 123.0
+    del A
+
+
+# ------------------------------------------------------------------------------------------------
+# (b) matvec
+# ------------------------------------------------------------------------------------------------
+def _x(n, seed):
+    return np.random.default_rng(seed).standard_normal(n)
+
+
+@pytest.mark.parametrize("c", [1, 2, 3])
+def test_matvec_parity(ctx, c):
+    g = cfg(c).geometry
+    Ao = oracle_build(g)
+    x = _x(g.n, c)
+    yo = oracle.matvec(Ao, x)
+    y = torch.empty(g.n, dtype=torch.float64, device="cuda")
+    ctx.bie_matvec(dev(Ao), dev(x), y)  # the oracle's matrix: only the GEMV is under test
+    assert rel_max(y.cpu().numpy(), yo) <= TOL_MV
+
+
+@pytest.mark.parametrize("n,lda", [(1, 2), (2, 2), (3, 4), (63, 64), (129, 200), (1023, 1024), (4099, 4100)])
+def test_matvec_ragged(ctx, n, lda):
+    rng = np.random.default_rng(n)
+    A = rng.standard_normal((n, lda))
+    x = rng.standard_normal(n)
+    yo = oracle.matvec(np.ascontiguousarray(A[:, :n]), x)
+    y = torch.empty(n + (n & 1), dtype=torch.float64, device="cuda")
+    ctx.bie_matvec(dev(A), dev(x), y[:n], lda=lda)
+    assert float(np.max(np.abs(y[:n].cpu().numpy() - yo))) <= TOL_MV * np.sqrt(n) * np.max(np.abs(A)) * np.max(np.abs(x))
+
+
+@pytest.mark.parametrize("c", [4, 5])
+def test_matvec_full_size_streaming_path(ctx, c):
+    """the matrices larger than L2 (the path bench.py times): GPU-built matrix, sampled rows of A x against the
+    oracle's rows, plus the property y = A 1_m = -1_m is not used here because Gamma_0 is under-resolved."""
+    g = cfg(c).geometry
+    A = gpu_build(ctx, g)
+    x = _x(g.n, c)
+    y = torch.empty(g.n, dtype=torch.float64, device="cuda")
+    ctx.bie_matvec(A, dev(x), y)
+    rows = _sample_rows(g, np.random.default_rng(100 + c))
+    Ao = oracle.build_rows(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, rows)
+    yo = oracle.matvec(Ao, x)
+    yg = y.cpu().numpy()[rows]
+    assert float(np.max(np.abs(yg - yo))) <= 1e-12 * max(1.0, float(np.max(np.abs(yo))))
+    del A
+
+
+@pytest.mark.parametrize("c", [1, 2, 3])
+def test_matvec_free_parity(ctx, c):
+    g = cfg(c).geometry
+    Ao = oracle_build(g)
+    x = _x(g.n, 10 + c)
+    yo = oracle.matvec(Ao, x)
+    z, dz, d2z = geo_dev(g)
+    ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z)
+    y = torch.empty(g.n, dtype=torch.float64, device="cuda")
+    ctx.bie_matvec_free(dev(x), y)
+    assert rel_max(y.cpu().numpy(), yo) <= 1e-12
+
+
+@pytest.mark.parametrize("shape", [(37, 29, [19, 23]), (5, 3, []), (1, 1, [1]), (300, 171, [33, 2, 129])])
+def test_matvec_free_ragged(ctx, shape):
+    g = inputs.small_problem(*shape, seed=5).geometry
+    for variant in (0, 1):
+        Ao = oracle_build(g, variant)
+        x = _x(g.n, 3)
+        z, dz, d2z = geo_dev(g)
+        ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z, variant=variant)
+        y = torch.empty(g.n + 1, dtype=torch.float64, device="cuda")
+        ctx.bie_matvec_free(dev(x), y[:g.n])
+        assert rel_max(y[:g.n].cpu().numpy(), oracle.matvec(Ao, x)) <= 1e-12
+
+
+# ------------------------------------------------------------------------------------------------
+# (c) GMRES
+# ------------------------------------------------------------------------------------------------
+def gpu_gmres(ctx, A, b, tol, restart, max_iters=1000):
+    from paper_2108_01786_b200 import bie
+    n = b.size
+    ws = torch.empty(bie.Context.bie_gmres_workspace_bytes(n, restart), dtype=torch.uint8, device="cuda")
+    oi = torch.full((2,), -7, dtype=torch.int32, device="cuda")
+    of = torch.full((1,), -7.0, dtype=torch.float64, device="cuda")
+    x = torch.empty(n + (n & 1), dtype=torch.float64, device="cuda")
+    ctx.bie_gmres(A, dev(b), x[:n], tol, restart, max_iters, ws, oi, of)
+    torch.cuda.synchronize()
+    return x[:n].cpu().numpy(), int(oi[0]), float(of[0]), int(oi[1])
+
+
+@pytest.mark.parametrize("c", [1, 2, 3, 4, 5])
+def test_gmres_parity(ctx, c):
+    P = cfg(c)
+    g, b = P.geometry, P.rhs[0]
+    Ao = oracle_build(g)
+    xo, ito, rro, _, sto = oracle.gmres(Ao, b, P.tol, P.restart, P.max_iters)
+    assert sto == 0
+    A = gpu_build(ctx, g)  # the GPU's own matrix: the whole hot path
+    x, it, rr, st = gpu_gmres(ctx, A, b, P.tol, P.restart, P.max_iters)
+    assert st == 0
+    assert abs(it - ito) <= 1, (it, ito)
+    assert np.linalg.norm(x - xo) / np.linalg.norm(xo) <= TOL_X
+    assert rr <= 10 * P.tol  # reported true residual (reading R10)
+    # and the GPU solution satisfies the ORACLE's system
+    r = b - oracle.matvec(Ao, x)
+    assert np.linalg.norm(r) / np.linalg.norm(b) <= 10 * P.tol
+    del A
+
+
+@pytest.mark.parametrize("c", [1, 2, 5])
+def test_gmres_matrix_free_parity(ctx, c):
+    P = cfg(c)
+    g, b = P.geometry, P.rhs[0]
+    Ao = oracle_build(g)
+    xo, ito, _, _, _ = oracle.gmres(Ao, b, P.tol, P.restart, P.max_iters)
+    z, dz, d2z = geo_dev(g)
+    ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z)
+    x, it, rr, st = gpu_gmres(ctx, None, b, P.tol, P.restart, P.max_iters)
+    assert st == 0 and abs(it - ito) <= 1
+    assert np.linalg.norm(x - xo) / np.linalg.norm(xo) <= TOL_X
+    assert rr <= 10 * P.tol
+
+
+def test_gmres_restart_and_iteration_cap(ctx):
+    """small restart forces several cycles; iteration counts still agree; max_iters is honoured"""
+    P = cfg(2)
+    g, b = P.geometry, P.rhs[0]
+    Ao = oracle_build(g)
+    A = dev(Ao)
+    for restart in (7, 20):
+        xo, ito, _, _, _ = oracle.gmres(Ao, b, 1e-13, restart, 1000)
+        x, it, rr, st = gpu_gmres(ctx, A, b, 1e-13, restart, 1000)
+        assert st == 0 and abs(it - ito) <= 1, (restart, it, ito)
+        assert np.linalg.norm(x - xo) / np.linalg.norm(xo) <= TOL_X
+    xo, ito, rro, _, sto = oracle.gmres(Ao, b, 1e-13, 20, 13)
+    x, it, rr, st = gpu_gmres(ctx, A, b, 1e-13, 20, 13)
+    assert (sto, ito) == (1, 13) and (st, it) == (1, 13)
+    assert np.linalg.norm(x - xo) / np.linalg.norm(xo) <= 1e-9
+    assert abs(rr - rro) <= 1e-6 * rro
+
+
+def test_gmres_degenerate_cases(ctx):
+    rng = np.random.default_rng(0)
+    # zero right-hand side: x = 0, 0 iterations
+    A = np.eye(6) + 0.1 * rng.standard_normal((6, 6))
+    x, it, rr, st = gpu_gmres(ctx, dev(A), np.zeros(6), 1e-13, 50)
+    assert it == 0 and st == 0 and np.all(x == 0.0) and rr == 0.0
+    # max_iters = 0
+    b = rng.standard_normal(6)
+    x, it, rr, st = gpu_gmres(ctx, dev(A), b, 1e-13, 50, 0)
+    assert it == 0 and st == 1 and np.all(x == 0.0) and abs(rr - 1.0) < 1e-15
+    # restart > n is clipped to n: exact solve in <= n steps
+    x, it, rr, st = gpu_gmres(ctx, dev(A), b, 1e-13, 50)
+    assert st == 0 and it <= 6 and np.linalg.norm(A @ x - b) <= 1e-12 * np.linalg.norm(b)
+    # n = 1, and identity (happy breakdown after one step: h_{2,1} = 0)
+    x, it, rr, st = gpu_gmres(ctx, dev(np.array([[2.0, 0.0]])), np.array([3.0]), 1e-13, 5)
+    assert it == 1 and abs(x[0] - 1.5) < 1e-15
+    x, it, rr, st = gpu_gmres(ctx, dev(np.eye(8)), b[:1].repeat(8), 1e-13, 5)
+    assert it == 1 and st in (0, 2) and np.allclose(x, b[0], rtol=1e-15)
+
+
+def test_solve_host_end_to_end(ctx):
+    from paper_2108_01786_b200 import bie
+    P = cfg(2)
+    g, b = P.geometry, P.rhs[0]
+    Ao = oracle_build(g)
+    xo, ito, _, _, _ = oracle.gmres(Ao, b, P.tol, P.restart, P.max_iters)
+    for mf in (False, True):
+        ws = torch.empty(bie.Context.bie_solve_workspace_bytes(g.n, P.restart, mf), dtype=torch.uint8, device="cuda")
+        x = np.empty(g.n)
+        it, rr, st = ctx.bie_solve_host(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, b, x, P.tol, P.restart,
+                                        P.max_iters, ws, matrix_free=mf)
+        assert st == 0 and abs(it - ito) <= 1 and rr <= 10 * P.tol
+        assert np.linalg.norm(x - xo) / np.linalg.norm(xo) <= TOL_X
+
+
+def test_error_codes(ctx):
+    from paper_2108_01786_b200 import bie
+    g = cfg(1).geometry
+    z, dz, d2z = geo_dev(g)
+    A = torch.empty((g.n, g.n + 1), dtype=torch.float64, device="cuda")
+    with pytest.raises(bie.BieError) as e:  # odd lda
+        ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A)
+    assert e.value.code == -3
+    with pytest.raises(bie.BieError) as e:  # the free surface must be component 0
+        ctx.bie_build(g.counts, [1, 0, 2], z, dz, d2z, torch.empty((g.n, g.n), dtype=torch.float64, device="cuda"))
+    assert e.value.code == -2
+    ws = torch.empty(16, dtype=torch.uint8, device="cuda")
+    oi = torch.zeros(2, dtype=torch.int32, device="cuda")
+    of = torch.zeros(1, dtype=torch.float64, device="cuda")
+    b = torch.zeros(g.n, dtype=torch.float64, device="cuda")
+    with pytest.raises(bie.BieError) as e:  # workspace too small
+        ctx.bie_gmres(torch.empty((g.n, g.n), dtype=torch.float64, device="cuda"), b, b.clone(), 1e-13, 50, 10, ws, oi, of)
+    assert e.value.code == -4
+
+
+def test_probe_dfma_runs(ctx):
+    out = torch.zeros(1, dtype=torch.float64, device="cuda")
+    total = ctx.bie_probe_dfma(1 << 12, out)
+    torch.cuda.synchronize()
+    assert total == (1 << 12) * 256 * 8 * ctx.sm_count
