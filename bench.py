@@ -1,0 +1,372 @@
+#!/usr/bin/env python
+"""bench.py -- one "step" = one pass of the whole hot path over one synthetic geometry:
+node preparation + dense build of the matrix of Eq. (3.16) (bie_build) + restarted GMRES on it (bie_gmres).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference] [--matrix-free]
+
+Prints ONE JSON line (rank 0).  Default workload: BASELINE.json configs[4] (n = 16384, 2.1 GB matrix, restart 100,
+tol 1e-13), the largest single-GPU configuration; its matrix is 17x the L2, so every GEMV streams from HBM.
+
+  value         whole-step throughput: n^2 matrix entries built AND solved per second, inputs resident in HBM
+  build/gmres   the two halves of BASELINE.json's metric on their own: Gentries/s of the build, ms of the solve
+  e2e           the same step through bie_solve_host with pinned HOST buffers (H2D of nodes+rhs, D2H of the density)
+  roofline      dominant kernel = the persistent GMRES kernel (HBM-bound GEMVs): algorithmic bytes / event time
+  roofline_build  the entry builder against the FP64 pipe (DFMA rate measured by bie_probe_dfma in this run)
+  cpu_baseline  the oracle (oracle/, as it stands) on this box's host cores, on a bounded sample of the same workload
+
+--impl reference times the oracle alone (this tier has no reference implementation).
+N > 1: replicas only: every rank runs the same step on its own GPU, no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "matrix build Gentries/s and GMRES solve ms (FP64); % of FP64 / HBM roofline"
+UNIT = "Gentries/s"
+FP64_INSTR_PER_ENTRY = 19      # FP64-pipe instructions per matrix entry (SASS count)
+HBM_FALLBACK_GBS = 6650.0      # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+# dram__bytes_read.sum + dram__bytes_write.sum of the GMRES kernel, one launch, from the committed ncu capture
+# (profiles/r01_ncu_full_gmres_cfg5.md); None for workloads that were not captured
+TRAFFIC_BYTES = {}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--matrix-free", action="store_true", help="solve with the matrix-free operator (no dense build)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="budget of the oracle sample")
+    return ap.parse_args()
+
+
+def hbm_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md)"
+
+
+def n_gemv(iters: int, restart: int) -> int:
+    """GEMVs of one bie_gmres launch: one per Arnoldi step, one residual per restart, one final true residual"""
+    cycles = max(1, -(-iters // restart))
+    return iters + (cycles - 1) + 1
+
+
+# ---------------------------------------------------------------------------------------------------
+# clocks during the timed region
+# ---------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [t.strip() for t in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        hi = [s for s, p in zip(sm, pw) if p >= 0.5 * max(pw)] or sm  # samples under load
+        return {"sm_mhz": float(np.median(hi)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------------------------------
+# oracle legs (the only places bench.py executes oracle/)
+# ---------------------------------------------------------------------------------------------------
+def oracle_sample(P, iters: int, seconds: float):
+    """Times the oracle, as it stands, on a bounded sample of the workload: a block of R rows of the matrix
+    (oracle_build_rows), the GEMV on that block (oracle_matvec_rect) and, when the whole problem fits the budget,
+    nothing is extrapolated.  Returns (step_seconds_estimate, description, cores)."""
+    import oracle
+    g = P.geometry
+    n = g.n
+    cores = oracle.num_threads()
+    rng = np.random.default_rng(0)
+    # rate of the build on 64 rows, then as many rows as fit ~40 % of the budget
+    rows = np.sort(rng.choice(n, size=min(n, 64), replace=False))
+    t = time.perf_counter()
+    oracle.build_rows(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, rows)
+    dt = max(time.perf_counter() - t, 1e-6)
+    R = int(min(n, max(64, 0.4 * seconds / dt * rows.size)))
+    rows = np.sort(rng.choice(n, size=R, replace=False))
+    t = time.perf_counter()
+    blk = oracle.build_rows(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, rows)
+    t_build_rows = time.perf_counter() - t
+    x = rng.standard_normal(n)
+    oracle.matvec(blk, x)
+    reps, t_mv = 0, 0.0
+    t0 = time.perf_counter()
+    while True:
+        oracle.matvec(blk, x)
+        reps += 1
+        t_mv = time.perf_counter() - t0
+        if t_mv > 0.4 * seconds or reps >= 200:
+            break
+    t_build = t_build_rows * n / R
+    t_gemv = t_mv / reps * n / R
+    ng = n_gemv(iters, P.restart)
+    est = t_build + ng * t_gemv
+    desc = (f"oracle_build_rows on {R} of {n} rows ({t_build_rows:.2f} s) and {reps} oracle GEMVs on that {R}x{n} block "
+            f"({t_mv:.2f} s); step = n/R * build + {ng} GEMVs (the GPU run's count) * n/R * block GEMV; "
+            f"Gram-Schmidt O(n*iters) not included")
+    return est, desc, cores, {"build_s": t_build, "gemv_s": t_gemv, "gemvs": ng}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the box's host cores, same config/metric/unit (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from paper_2108_01786_b200 import inputs
+    P = inputs.make_config(args.config)
+    n = P.n
+    iters_nominal = {1: 18, 2: 33, 3: 74, 4: 127, 5: 158}[args.config]  # the oracle's own counts (tests)
+    per = max(2.0, min(args.cpu_seconds, 120.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        oracle_sample(P, iters_nominal, per)
+    ests = []
+    for _ in range(args.steps):
+        est, desc, cores, parts = oracle_sample(P, iters_nominal, per)
+        ests.append(est)
+    est = float(np.mean(ests))
+    val = n * n / est / 1e9
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": est * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(P, args, iters_nominal),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0,
+            "build": {"gentries_per_s": n * n / parts["build_s"] / 1e9, "ms": parts["build_s"] * 1e3},
+            "gmres": {"ms": parts["gemv_s"] * parts["gemvs"] * 1e3, "iters": iters_nominal}}
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(P, args, iters):
+    g = P.geometry
+    return {"workload": f"BASELINE.json configs[{P.config - 1}]: {P.name}", "n": int(g.n),
+            "counts": [int(c) for c in g.counts], "restart": int(P.restart), "tol": P.tol,
+            "operator": "matrix-free" if args.matrix_free else "dense",
+            "matrix_bytes": 0 if args.matrix_free else int(8 * g.n * g.n),
+            "l2_policy": "inputs larger than L2 (matrix 17x L2); no flush needed" if 8 * g.n * g.n > 2.5e8
+            else "matrix fits L2 (126 MB): L2-resident GEMV, reported as such",
+            "replicas": int(args.gpus)}
+
+
+# ---------------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------------
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+    import torch
+    import torch.distributed as dist
+    from paper_2108_01786_b200 import bie, inputs, build as _build
+
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a B200: the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        _build.build_library()
+    if world > 1:
+        dist.barrier()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(v: float) -> float:
+        if world == 1:
+            return v
+        t = torch.tensor([v], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t[0])
+
+    P = inputs.make_config(args.config)
+    g, n = P.geometry, P.n
+    ctx = bie.Context(local)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    z, dz, d2z, b = dev(g.zeta), dev(g.dzeta), dev(g.d2zeta), dev(P.rhs[0])
+    A = None if args.matrix_free else torch.empty((n, n + (n & 1)), dtype=torch.float64, device="cuda")
+    x = torch.empty(n + (n & 1), dtype=torch.float64, device="cuda")[:n]
+    ws = torch.empty(ctx.bie_gmres_workspace_bytes(n, P.restart), dtype=torch.uint8, device="cuda")
+    oi = torch.zeros(2, dtype=torch.int32, device="cuda")
+    of = torch.zeros(1, dtype=torch.float64, device="cuda")
+
+    def step(ev=None):
+        if ev: ev[0].record()
+        if A is None:
+            ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z)          # 1 launch
+        else:
+            ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A)              # 2 launches: node prep + tile kernel
+        if ev: ev[1].record()
+        ctx.bie_gmres(A, b, x, P.tol, P.restart, P.max_iters, ws, oi, of)  # 1 cooperative launch
+        if ev: ev[2].record()
+    launches_per_step = 2 if A is None else 3
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    iters, status, relres = int(oi[0]), int(oi[1]), float(of[0])
+    if status != 0 or not (relres <= 1e-12):
+        raise SystemExit(f"bench: GMRES did not converge (status {status}, relres {relres})")
+
+    # FP64 pipe rate of this GPU, now (roofline denominator of the build)
+    probe_out = torch.zeros(1, dtype=torch.float64, device="cuda")
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ctx.bie_probe_dfma(1 << 15, probe_out)
+    torch.cuda.synchronize()
+    e0.record(); total_fma = ctx.bie_probe_dfma(1 << 17, probe_out); e1.record()
+    torch.cuda.synchronize()
+    dfma_per_s = total_fma / (e0.elapsed_time(e1) * 1e-3)
+
+    # ---- timed region: K steps, device time, max over ranks ------------------------------------------
+    K = args.steps
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    barrier()
+    t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_start.record()
+    for k in range(K):
+        step(evs[k])
+    t_end.record()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = max_over_ranks(t_start.elapsed_time(t_end))
+    build_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
+    gmres_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
+    ms_per_step = total_ms / K
+    value = world * n * n / (ms_per_step * 1e-3) / 1e9
+
+    # ---- end to end through bie_solve_host, pinned host buffers ---------------------------------------------
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    hz, hdz, hd2z, hb = pin(g.zeta.view(np.float64)), pin(g.dzeta.view(np.float64)), pin(g.d2zeta.view(np.float64)), pin(P.rhs[0])
+    hx = torch.empty(n, dtype=torch.float64).pin_memory()
+    del A
+    torch.cuda.empty_cache()
+    sws = torch.empty(ctx.bie_solve_workspace_bytes(n, P.restart, args.matrix_free), dtype=torch.uint8, device="cuda")
+    for _ in range(2):
+        ctx.bie_solve_host(g.counts, g.kinds, hz, hdz, hd2z, hb, hx, P.tol, P.restart, P.max_iters, sws, args.matrix_free)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(K):
+        e_it, e_rr, e_st = ctx.bie_solve_host(g.counts, g.kinds, hz, hdz, hd2z, hb, hx, P.tol, P.restart, P.max_iters,
+                                              sws, args.matrix_free)
+    torch.cuda.synchronize()
+    e2e_s = max_over_ranks((time.perf_counter() - t0) / K)
+    h2d = 3 * 16 * n + 8 * n
+    d2h = 8 * n + 8 + 8
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- rooflines -------------------------------------------------------------------------------------------
+    peak, peak_src = hbm_peak()
+    ng = n_gemv(iters, P.restart)
+    if args.matrix_free:
+        roof = {"bound": "alu", "kernel": "bie_gmres_kernel<matrix-free>",
+                "achieved": ng * n * n * FP64_INSTR_PER_ENTRY / (gmres_ms * 1e-3) / 1e12, "peak": dfma_per_s / 1e12,
+                "unit": "T FP64 instr/s", "traffic": None,
+                "peak_source": "bie_probe_dfma in this run (nominal 148 SM x 64 lanes x 1.965 GHz = 18.6)"}
+    else:
+        roof = {"bound": "hbm", "kernel": "bie_gmres_kernel (persistent; GEMV phases dominate)",
+                "achieved": ng * 8.0 * n * n / (gmres_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                "traffic": TRAFFIC_BYTES.get(args.config), "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": ng * 8 * n * n, "gemvs_per_launch": ng}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof_build = None
+    if not args.matrix_free:
+        ach = n * n * FP64_INSTR_PER_ENTRY / (build_ms * 1e-3)
+        roof_build = {"bound": "alu", "kernel": "bie_build_kernel (+ node prep)", "achieved": ach / 1e12,
+                      "peak": dfma_per_s / 1e12, "unit": "T FP64 instr/s", "frac": ach / dfma_per_s,
+                      "peak_source": "bie_probe_dfma in this run (nominal 148 SM x 64 lanes x 1.965 GHz = 18.6)",
+                      "fp64_instr_per_entry": FP64_INSTR_PER_ENTRY,
+                      "hbm_write_gbs": 8.0 * n * n / (build_ms * 1e-3) / 1e9, "hbm_write_frac": 8.0 * n * n / (build_ms * 1e-3) / 1e9 / peak}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": workload_config(P, args, iters),
+            "build": None if args.matrix_free else {"gentries_per_s": n * n / (build_ms * 1e-3) / 1e9, "ms": build_ms},
+            "gmres": {"ms": gmres_ms, "iters": iters, "relres_true": relres, "us_per_iter": gmres_ms * 1e3 / max(iters, 1)},
+            "e2e": {"value": world * n * n / e2e_s / 1e9, "unit": UNIT, "ms_per_step": e2e_s * 1e3,
+                    "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "api": "bie_solve_host", "iters": e_it},
+            "gpu_launches": launches_per_step * K,
+            "roofline": roof, "roofline_build": roof_build, "clocks": clocks,
+            "fp64_probe_tflops": 2 * dfma_per_s / 1e12}
+    if not args.no_cpu_baseline:
+        est, desc, cores, parts = oracle_sample(P, iters, args.cpu_seconds)
+        line["cpu_baseline"] = {"value": n * n / est / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+                                "ms_per_step": est * 1e3, "build_gentries_per_s": n * n / parts["build_s"] / 1e9,
+                                "gmres_ms": parts["gemv_s"] * parts["gemvs"] * 1e3}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

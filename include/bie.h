@@ -133,11 +133,13 @@ int bie_matvec_free(bie_ctx* ctx, int n, const double* x, double* y, void* strea
  * workspace: dev, at least bie_gmres_workspace_bytes(n, restart) bytes, contents undefined afterwards.
  * Returns BIE_OK immediately after the launch (convergence status is in *iters_out vs max_iters, and in
  * status_out if not NULL: dev int32, 0 converged / 1 max_iters / 2 breakdown (h_{j+1,j} == 0, converged)).
+ * res_hist (dev, max_iters + 1 doubles, may be NULL): res_hist[i] = recurrence residual |g_{i+1}| / ||b|| after
+ * i steps (res_hist[0] = 1), the quantity behind the paper's i_max statistics.
  */
 size_t bie_gmres_workspace_bytes(int n, int restart);
 int bie_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, const double* rhs,
               double tol, int restart, int max_iters,
-              double* x, int32_t* iters_out, double* relres_out, int32_t* status_out,
+              double* x, int32_t* iters_out, double* relres_out, int32_t* status_out, double* res_hist,
               void* workspace, size_t workspace_bytes, void* stream);
 
 /* ---------------------------------------------------------------------------------------------------

@@ -66,7 +66,7 @@ def lib() -> ctypes.CDLL:
         L.bie_gmres_workspace_bytes.restype = sz
         L.bie_gmres_workspace_bytes.argtypes = [i32, i32]
         L.bie_gmres.restype = i32
-        L.bie_gmres.argtypes = [vp, i32, vp, i64, vp, dbl, i32, i32, vp, vp, vp, vp, vp, sz, vp]
+        L.bie_gmres.argtypes = [vp, i32, vp, i64, vp, dbl, i32, i32, vp, vp, vp, vp, vp, vp, sz, vp]
         L.bie_solve_workspace_bytes.restype = sz
         L.bie_solve_workspace_bytes.argtypes = [i32, i32, i32]
         L.bie_solve_host.restype = i32
@@ -183,9 +183,9 @@ class Context:
         return int(lib().bie_gmres_workspace_bytes(int(n), int(restart)))
 
     def bie_gmres(self, A, rhs, x, tol: float, restart: int, max_iters: int, workspace, out_i32, out_f64,
-                  lda: Optional[int] = None):
+                  lda: Optional[int] = None, res_hist=None):
         """Asynchronous.  A = None selects the matrix-free operator.  out_i32: CUDA int32[2] <- (iters, status);
-        out_f64: CUDA float64[1] <- true relative residual."""
+        out_f64: CUDA float64[1] <- true relative residual; res_hist: optional CUDA float64[max_iters+1]."""
         import torch
         n = rhs.numel()
         if A is None:
@@ -198,7 +198,9 @@ class Context:
         ws_bytes = workspace.numel() * workspace.element_size()
         _check(lib().bie_gmres(self._h, n, pA, lda, _dev_f64(rhs, n), float(tol), int(restart), int(max_iters),
                                _dev_f64(x, n), out_i32.data_ptr(), _dev_f64(out_f64, 1),
-                               out_i32.data_ptr() + 4, workspace.data_ptr(), ws_bytes, _stream()), "bie_gmres")
+                               out_i32.data_ptr() + 4,
+                               None if res_hist is None else _dev_f64(res_hist, int(max_iters) + 1),
+                               workspace.data_ptr(), ws_bytes, _stream()), "bie_gmres")
         return x
 
     # ---- end to end with host buffers ------------------------------------------------------------------

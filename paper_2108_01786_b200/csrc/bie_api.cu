@@ -123,12 +123,12 @@ size_t bie_gmres_workspace_bytes(int n, int restart) { return bie_gmres_ws_bytes
 
 int bie_gmres(bie_ctx* c, int n, const double* A, int64_t lda, const double* rhs, double tol, int restart,
               int max_iters, double* x, int32_t* iters_out, double* relres_out, int32_t* status_out,
-              void* workspace, size_t workspace_bytes, void* stream)
+              double* res_hist, void* workspace, size_t workspace_bytes, void* stream)
 {
     if (!c) return BIE_ERR_NULL;
     BIE_CUDA(cudaSetDevice(c->device));
     return bie_launch_gmres(c, n, A, lda, rhs, tol, restart, max_iters, x, iters_out, relres_out, status_out,
-                            workspace, workspace_bytes, (cudaStream_t)stream);
+                            res_hist, workspace, workspace_bytes, (cudaStream_t)stream);
 }
 
 // ---- end-to-end with host buffers --------------------------------------------------------------------
@@ -184,7 +184,7 @@ int bie_solve_host(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* 
         rc = bie_launch_build(c, dA, (int64_t)nld, 0, st);
         if (rc != BIE_OK) return rc;
     }
-    rc = bie_launch_gmres(c, n, dA, (int64_t)nld, drhs, tol, restart, max_iters, dx, dint, drel, dint + 1, gws,
+    rc = bie_launch_gmres(c, n, dA, (int64_t)nld, drhs, tol, restart, max_iters, dx, dint, drel, dint + 1, nullptr, gws,
                           gws_bytes, st);
     if (rc != BIE_OK) return rc;
     BIE_CUDA(cudaMemcpyAsync(x, dx, 8 * (size_t)n, cudaMemcpyDeviceToHost, st));

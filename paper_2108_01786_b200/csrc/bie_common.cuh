@@ -88,7 +88,7 @@ int bie_launch_matvec(bie_ctx* ctx, int n, const double* A, int64_t lda, const d
 int bie_launch_matvec_free(bie_ctx* ctx, const double* x, double* y, cudaStream_t st);
 int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, const double* rhs, double tol,
                      int restart, int max_iters, double* x, int32_t* iters_out, double* relres_out,
-                     int32_t* status_out, void* ws, size_t ws_bytes, cudaStream_t st);
+                     int32_t* status_out, double* res_hist, void* ws, size_t ws_bytes, cudaStream_t st);
 size_t bie_gmres_ws_bytes(int n, int restart);
 int bie_launch_probe_dfma(bie_ctx* ctx, int64_t fma_per_thread, double* out, int64_t* total_fma, cudaStream_t st);
 

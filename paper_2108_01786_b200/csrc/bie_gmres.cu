@@ -32,6 +32,7 @@ struct GmresArgs {
     int32_t* iters_out;
     double* relres_out;
     int32_t* status_out;
+    double* res_hist;  // [max_iters+1] recurrence residual / ||b|| after each step, or NULL
     double* V;     // [(m+1)][nld]
     double* wbuf;  // [nld]
     double* part;  // [3][m+2][G]
@@ -194,6 +195,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
 
     int iters = 0, status = 0;
     bool done = (bn == 0.0);
+    if (a.res_hist && blockIdx.x == 0 && threadIdx.x == 0) a.res_hist[0] = 1.0;
     bool first = true;
     while (!done) {
         // ---- cycle start: r = b - A x ------------------------------------------------------------
@@ -270,6 +272,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
                 for (int i = threadIdx.x; i <= j; i += blockDim.x) a.R[(size_t)j * (m + 1) + i] = hcol[i];
             ++iters;
             k = j + 1;
+            if (a.res_hist && blockIdx.x == 0 && threadIdx.x == 0) a.res_hist[iters] = fabs(g[j + 1]) / bn;
             conv = (fabs(g[j + 1]) <= thresh) || (hn == 0.0);
             if (hn == 0.0 && !(fabs(g[j + 1]) <= thresh)) status = 2;
             __syncthreads();
@@ -395,7 +398,7 @@ static int launch_gmres(const GmresArgs& a, const GmresPlan& pl, cudaStream_t st
 
 int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, const double* rhs, double tol,
                      int restart, int max_iters, double* x, int32_t* iters_out, double* relres_out,
-                     int32_t* status_out, void* ws, size_t ws_bytes, cudaStream_t st)
+                     int32_t* status_out, double* res_hist, void* ws, size_t ws_bytes, cudaStream_t st)
 {
     if (!ctx || !rhs || !x || !ws) return BIE_ERR_NULL;
     if (n < 1 || restart < 1 || max_iters < 0 || !(tol >= 0.0)) return BIE_ERR_ARG;
@@ -415,7 +418,7 @@ int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, const do
     if (base - (uintptr_t)ws + pl.total > ws_bytes) return BIE_ERR_WORKSPACE;
     GmresArgs a;
     a.A = A; a.lda = lda; a.n = n; a.b = rhs; a.tol = tol; a.m = restart; a.max_iters = max_iters;
-    a.x = x; a.iters_out = iters_out; a.relres_out = relres_out; a.status_out = status_out;
+    a.x = x; a.iters_out = iters_out; a.relres_out = relres_out; a.status_out = status_out; a.res_hist = res_hist;
     a.V = (double*)(base + pl.offV);
     a.wbuf = (double*)(base + pl.offW);
     a.part = (double*)(base + pl.offP);
