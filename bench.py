@@ -39,7 +39,7 @@ FP64_INSTR_PER_ENTRY = 19      # FP64-pipe instruct
 HBM_FALLBACK_GBS = 6650.0      # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 # dram__bytes_read.sum + dram__bytes_write.sum of the GMRES kernel, one launch, from the committed ncu capture
 # (profiles/r01_ncu_full_gmres_cfg5.md); None for workloads that were not captured
-TRAFFIC_BYTES = {}
+TRAFFIC_BYTES = {5: 345.81e9}
 
 
 def parse_args():
@@ -301,6 +301,26 @@ def main():
     ms_per_step = total_ms / K
     value = world * n * n / (ms_per_step * 1e-3) / 1e9
 
+    # ---- the stand-alone operator calls (outside the timed region; matvec against HBM) ---------
+    def time_call(fn, reps):
+        fn(); torch.cuda.synchronize()
+        a, c = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(reps):
+            fn()
+        c.record(); torch.cuda.synchronize()
+        return a.elapsed_time(c) / reps
+
+    xv = torch.from_numpy(np.random.default_rng(1).standard_normal(n)).cuda()
+    yv = torch.empty(n + (n & 1), dtype=torch.float64, device="cuda")[:n]
+    matvec = {}
+    if A is not None:
+        mv_ms = time_call(lambda: ctx.bie_matvec(A, xv, yv), 50)
+        matvec["dense"] = {"ms": mv_ms, "gbs": 8.0 * n * n / (mv_ms * 1e-3) / 1e9}
+    mf_ms = time_call(lambda: ctx.bie_matvec_free(xv, yv), 20)
+    matvec["matrix_free"] = {"ms": mf_ms, "gentries_per_s": n * n / (mf_ms * 1e-3) / 1e9,
+                             "fp64_frac": n * n * FP64_INSTR_PER_ENTRY / (mf_ms * 1e-3) / dfma_per_s}
+
     # ---- end to end through bie_solve_host, pinned host buffers ---------------------------------------------
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     hz, hdz, hd2z, hb = pin(g.zeta.view(np.float64)), pin(g.dzeta.view(np.float64)), pin(g.d2zeta.view(np.float64)), pin(P.rhs[0])
@@ -356,7 +376,7 @@ def main():
             "e2e": {"value": world * n * n / e2e_s / 1e9, "unit": UNIT, "ms_per_step": e2e_s * 1e3,
                     "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "api": "bie_solve_host", "iters": e_it},
             "gpu_launches": launches_per_step * K,
-            "roofline": roof, "roofline_build": roof_build, "clocks": clocks,
+            "roofline": roof, "roofline_build": roof_build, "matvec": matvec, "clocks": clocks,
             "fp64_probe_tflops": 2 * dfma_per_s / 1e12}
     if not args.no_cpu_baseline:
         est, desc, cores, parts = oracle_sample(P, iters, args.cpu_seconds)
