@@ -35,7 +35,7 @@ if ROOT not in sys.path:
 
 METRIC = "matrix build Gentries/s and GMRES solve ms (FP64); % of FP64 / HBM roofline"
 UNIT = "Gentries/s"
-FP64_INSTR_PER_ENTRY = 19      # FP64-pipe instructions per matrix entry (SASS count)
+FP64_INSTR_PER_ENTRY = 13      # FP64-pipe instructions per matrix entry (SASS count)
 HBM_FALLBACK_GBS = 6650.0      # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 # dram__bytes_read.sum + dram__bytes_write.sum of the GMRES kernel, one launch, from the committed ncu capture
 # (profiles/r01_ncu_full_gmres_cfg5.md); None for workloads that were not captured

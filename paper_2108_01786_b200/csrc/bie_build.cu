@@ -2,79 +2,82 @@
 //
 // Tiling.  A CTA of 128 threads owns a tile of T target rows x 256 source columns.  Each thread keeps the
 // per-node factors of TWO adjacent source columns in registers and walks down the T target rows, whose
-// factors (S, C, P, N) sit in shared memory and are read as warp-wide broadcasts.  A warp therefore writes,
+// factors (E_t, M_t) sit in shared memory and are read as warp-wide broadcasts.  A warp therefore writes,
 // per target row, 32 x 16 B = 512 contiguous bytes of that row (128-bit coalesced stores, full 128 B lines).
 //
-// Per pair (fast path): 19 FP64-pipe instructions + 1 MUFU, no transcendental (bie_common.cuh).
-// The walk over the target rows is split into segments of constant target component, so that the
-// Re/Im selection of Eq. (3.10) and the -1/M_k of E_k become two
-// per-segment register coefficients (u, v) and one fused constant em:
-//     entry = (u * nr + v * ni) * r - em,      c = q * cot(w/2),  cot = (nr - i ni) r
-//     Im c  ->  (u, v) = ( qi, -qr)      [k = 0, j = 0]  and  [k >= 1, j >= 1]
-//     Re c  ->  (u, v) = ( qr,  qi)      [k = 0, j >= 1]
-//    -Re c  ->  (u, v) = (-qr, -qi)      [k >= 1, j = 0]
-// Pairs closer than |w|^2 < BIE_NEAR_TAU (which includes s == t) take the near path: Laurent series of
-// cot from the coordinate differences, or the precomputed diagonal entry when s == t.
+// Per entry (fast path): 13 FP64-pipe instructions + 1 MUFU + 1 integer compare, no transcendental
+// (bie_common.cuh).  The walk over the target rows is split into segments of constant target component, so
+// that the Re/Im selection of Eq. (3.10) and the -1/M_k of E_k become two
+// per-segment register coefficients (alpha, beta) and one fused constant em:
+//     entry = (alpha X + beta Y) / den - em
+//     Im c  ->  (alpha, beta) = (-2 qi,  qr)     [k = 0, j = 0]  and  [k >= 1, j >= 1]
+//     Re c  ->  (alpha, beta) = (-2 qr, -qi)     [k = 0, j >= 1]
+//    -Re c  ->  (alpha, beta) = ( 2 qr,  qi)     [k >= 1, j = 0]
+// The inner loop has no branch: it only ORs a "near" flag (den < thr_s, which includes s == t).  After every
+// BUILD_RB rows the warp votes; if any lane saw a near pair, those rows are revisited and the near entries are
+// overwritten with the Laurent-series value, or with the precomputed diagonal entry when s == t.
 #include "bie_common.cuh"
 
 #define BUILD_THREADS 128
 #define BUILD_COLS 2
 #define BUILD_TILE_W (BUILD_THREADS * BUILD_COLS)
+#define BUILD_RB 4
 
-struct SrcRegs {
-    double S2, C2, P, N;  // 2 sin(x_s/2), 2 cos(x_s/2), e^{y_s/2}, e^{-y_s/2}
-    double qr, qi;
-    double u, v, em;  // per-segment coefficients
+struct SrcCol {
+    double er, ei, m;   // E_s, M_s
+    int thi;            // high word of thr_s
+    double a, b, em;    // per-segment coefficients
 };
 
-__device__ __forceinline__ double bie_pair_entry(const SrcRegs& s, const double2 sc, const double2 pn,
-                                                 const NodeTable& nt, int sidx, int tidx)
+__device__ __forceinline__ double bie_entry_fast(const SrcCol& s, const double2 te, const double tm, int& flag)
 {
-    // 2 sin a = (2 S_s) C_t - (2 C_s) S_t ; 2 cos a = (2 C_s) C_t + (2 S_s) S_t
-    const double sa = fma(s.S2, sc.y, -(s.C2 * sc.x));
-    const double ca = fma(s.C2, sc.y, s.S2 * sc.x);
-    const double ep = s.P * pn.y, en = s.N * pn.x;
-    const double D = ep - en, G = ep + en;
-    double nr = sa * ca, ni = D * G;
-    const double den = fma(D, D, sa * sa);
-    double r = bie_rcp(den);
-    if (den < BIE_NEAR_TAU) {
-        if (sidx == tidx) return nt.DIAG[tidx];
-        double cr, ci;
-        bie_cot_half_near(nt.X[sidx] - nt.X[tidx], nt.Y[sidx] - nt.Y[tidx], &cr, &ci);
-        nr = cr; ni = -ci; r = 1.0;
-    }
-    return fma(fma(s.v, ni, s.u * nr), r, -s.em);
+    const double dr = s.er - te.x, di = s.ei - te.y;
+    const double den = fma(dr, dr, di * di);
+    const double X = fma(te.y, s.er, -(te.x * s.ei));
+    const double Y = s.m - tm;
+    const double val = fma(s.b, Y, s.a * X);
+    flag |= (__double2hiint(den) < s.thi) ? 1 : 0;
+    return fma(val, bie_rcp3(den), -s.em);
+}
+
+// exact value of a near entry (rare): Laurent series from the coordinate differences, or the diagonal limit
+static __device__ __noinline__ double bie_entry_near(const double2* __restrict__ DG, const double2* __restrict__ XY,
+                                                     double sa, double sb, double sem, int sidx, int tidx)
+{
+    if (sidx == tidx) return DG[tidx].x;
+    const double2 zs = XY[sidx], zt = XY[tidx];
+    double cr, ci;
+    bie_cot_half_near(zs.x - zt.x, zs.y - zt.y, &cr, &ci);
+    // entry = alpha X/den + beta Y/den with cot = (-2X + iY)/den
+    return fma(sb, ci, -0.5 * sa * cr) - sem;
 }
 
 __global__ void __launch_bounds__(BUILD_THREADS)
 bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long lda, int T, int only0)
 {
-    extern __shared__ __align__(16) double2 sm[];  // [T] (S_t, C_t) then [T] (P_t, N_t)
+    extern __shared__ __align__(16) double2 sm[];  // [T] E_t then [T] (M_t, -)
     const int n = nt.n;
     const int c0 = blockIdx.x * BUILD_TILE_W;
     const int t0 = blockIdx.y * T;
     const int t1 = min(t0 + T, n);
     if (only0 && t0 >= ct.off[1] && c0 >= ct.off[1]) return;  // a4: solid-solid tiles stay
-    double2* sSC = sm;
-    double2* sPN = sm + T;
+    double2* sE = sm;
+    double* sM = reinterpret_cast<double*>(sm + T);
     for (int i = threadIdx.x; i < t1 - t0; i += BUILD_THREADS) {
-        sSC[i] = make_double2(nt.S[t0 + i], nt.C[t0 + i]);
-        sPN[i] = make_double2(nt.P[t0 + i], nt.N[t0 + i]);
+        sE[i] = nt.E[t0 + i];
+        sM[i] = nt.MT[t0 + i].x;
     }
     const int s0 = c0 + BUILD_COLS * threadIdx.x;  // < npad by construction
-    SrcRegs src[BUILD_COLS];
+    SrcCol src[BUILD_COLS];
+    double sqr[BUILD_COLS], sqi[BUILD_COLS], sem[BUILD_COLS];
     int scomp[BUILD_COLS];
-    double sem[BUILD_COLS];
 #pragma unroll
     for (int c = 0; c < BUILD_COLS; ++c) {
-        src[c].S2 = 2.0 * nt.S[s0 + c];
-        src[c].C2 = 2.0 * nt.C[s0 + c];
-        src[c].P = nt.P[s0 + c];
-        src[c].N = nt.N[s0 + c];
-        src[c].qr = nt.QR[s0 + c];
-        src[c].qi = nt.QI[s0 + c];
-        sem[c] = nt.EM[s0 + c];
+        const double2 e = nt.E[s0 + c], mt = nt.MT[s0 + c], q = nt.Q[s0 + c];
+        src[c].er = e.x; src[c].ei = e.y; src[c].m = mt.x;
+        src[c].thi = __double2hiint(mt.y);
+        sqr[c] = q.x; sqi[c] = q.y;
+        sem[c] = nt.DG[s0 + c].y;
         scomp[c] = nt.COMP[s0 + c];
     }
     __syncthreads();
@@ -86,19 +89,41 @@ bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long l
 #pragma unroll
         for (int c = 0; c < BUILD_COLS; ++c) {
             const bool src0 = (scomp[c] == 0), tgt0 = (k == 0);
-            if (src0 == tgt0) { src[c].u = src[c].qi; src[c].v = -src[c].qr; }        // Im c
-            else if (tgt0)    { src[c].u = src[c].qr; src[c].v = src[c].qi; }         // Re c   (G_0j)
-            else              { src[c].u = -src[c].qr; src[c].v = -src[c].qi; }       // -Re c  (-G_k0)
+            if (src0 == tgt0) { src[c].a = -2.0 * sqi[c]; src[c].b = sqr[c]; }       // Im c
+            else if (tgt0)    { src[c].a = -2.0 * sqr[c]; src[c].b = -sqi[c]; }      // Re c   (G_0j)
+            else              { src[c].a = 2.0 * sqr[c];  src[c].b = sqi[c]; }       // -Re c  (-G_k0)
             src[c].em = (scomp[c] == k) ? sem[c] : 0.0;
         }
-        double* row = A + (long long)a * lda + s0;
-#pragma unroll 2
-        for (int t = a; t < b; ++t, row += lda) {
-            const double2 sc = sSC[t - t0], pn = sPN[t - t0];
-            const double e0 = bie_pair_entry(src[0], sc, pn, nt, s0, t);
-            const double e1 = bie_pair_entry(src[1], sc, pn, nt, s0 + 1, t);
-            if (full) *reinterpret_cast<double2*>(row) = make_double2(e0, e1);
-            else if (part) row[0] = e0;
+        for (int tb = a; tb < b; tb += BUILD_RB) {
+            int flag = 0;
+            double* row = A + (long long)tb * lda + s0;
+#pragma unroll
+            for (int r = 0; r < BUILD_RB; ++r) {
+                const int t = min(tb + r, b - 1);  // the tail repeats the last row (same values, same address)
+                const double2 te = sE[t - t0];
+                const double tm = sM[t - t0];
+                const double e0 = bie_entry_fast(src[0], te, tm, flag);
+                const double e1 = bie_entry_fast(src[1], te, tm, flag);
+                double* p = row + (long long)(t - tb) * lda;
+                if (full) *reinterpret_cast<double2*>(p) = make_double2(e0, e1);
+                else if (part) p[0] = e0;
+            }
+            if (__any_sync(0xffffffffu, flag)) {
+                if (flag) {
+                    const int te_ = min(tb + BUILD_RB, b);
+                    for (int t = tb; t < te_; ++t) {
+                        const double2 te = sE[t - t0];
+#pragma unroll
+                        for (int c = 0; c < BUILD_COLS; ++c) {
+                            if (s0 + c >= n) continue;
+                            const double dr = src[c].er - te.x, di = src[c].ei - te.y;
+                            const double den = fma(dr, dr, di * di);
+                            if (__double2hiint(den) < src[c].thi)
+                                A[(long long)t * lda + s0 + c] = bie_entry_near(nt.DG, nt.XY, src[c].a, src[c].b, src[c].em, s0 + c, t);
+                        }
+                    }
+                }
+            }
         }
     }
 }
@@ -115,8 +140,8 @@ int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int only_comp0, cudaS
     int T = 128;
     while (T > 8 && (long long)gx * ((n + T - 1) / T) < 4LL * ctx->sm_count) T >>= 1;
     dim3 grid(gx, (n + T - 1) / T);
-    bie_build_kernel<<<grid, BUILD_THREADS, sizeof(double2) * 2 * T, st>>>(nt, ctx->comps, A, (long long)lda, T,
-                                                                        only_comp0);
+    bie_build_kernel<<<grid, BUILD_THREADS, (sizeof(double2) + sizeof(double)) * T + 16, st>>>(nt, ctx->comps, A, (long long)lda, T,
+                                                                                            only_comp0);
     BIE_CUDA(cudaGetLastError());
     return BIE_OK;
 }

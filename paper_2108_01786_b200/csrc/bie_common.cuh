@@ -1,17 +1,18 @@
 // bie_common.cuh -- shared declarations of the CUDA path (sm_100a only).  No oracle code is shared.
 //
-// Pair arithmetic.  For a source node s and a target node t,
-//   w = zeta_s - zeta_t = x + i y,  a = x/2,  b = y/2,
-// the complex cotangent of Eq. (3.4) is assembled from PER-NODE factors, with no
-// transcendental per pair:
-//   S = sin(x_node/2), C = cos(x_node/2), P = exp(y_node/2), N = exp(-y_node/2)
-//   sin a = S_s C_t - C_s S_t,   cos a = C_s C_t + S_s S_t
-//   e^{b} = P_s N_t,  e^{-b} = N_s P_t,   D = e^b - e^-b = 2 sinh b,  G = e^b + e^-b = 2 cosh b
-//   cot(w/2) = (sin a cos a - i sinh b cosh b)/(sin^2 a + sinh^2 b)
-//            = (4 sin a cos a - i D G) / (4 sin^2 a + D^2)
-// The assembled sin a and D cancel for |w| -> 0 (relative error about eps/|w|); pairs with
-// 4 sin^2 a + D^2 < BIE_NEAR_TAU take the near path: differences first, x reduced by 2 pi, then the
-// Laurent series of cot (bie_cot_half_near), which is accurate to rounding there.
+// Pair arithmetic (DESIGN.md section 5 "Pair arithmetic").  The periodised Cauchy kernel of Eq. (3.4)
+// for a source node s and a target node t, w = zeta_s - zeta_t, is evaluated from ONE complex
+// exponential per NODE, E = e^{i zeta} = e^{-(y - y_ref)} (cos x + i sin x), M = |E|^2, with no transcendental
+// per pair:
+//     cot(w/2) = i (e^{iw} + 1)/(e^{iw} - 1) = i (E_s + E_t) conj(E_s - E_t) / |E_s - E_t|^2
+//              = ( -2 X + i Y ) / den,    X = Im(E_t conj E_s),  Y = M_s - M_t,  den = |E_s - E_t|^2 .
+// With the source weight q_s = zeta'_s/(2 M_j) the entry is (alpha X + beta Y)/den:
+//     Im{q cot} : (alpha, beta) = (-2 qi,  qr)     Re{q cot} : (-2 qr, -qi)     -Re{q cot} : (2 qr, qi)
+// i.e. 13 FP64-pipe instructions per pair including the reciprocal (bie_rcp3).  E_s - E_t cancels for
+// |w| -> 0 (relative error about 10 eps/|w|, entry error about 20 eps |q_s|/|w|^2); pairs with
+// den < thr_s = tau_s M_s, tau_s = BIE_NEAR_C |q_s| (clamped), are "near": they are recomputed from the
+// coordinate differences with the Laurent series of cot (bie_cot_half_near), accurate to rounding, and the
+// pair s == t takes the analytic diagonal limit.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -19,25 +20,22 @@
 
 #define BIE_MAX_COMP 64
 #define BIE_NODE_PAD 256              // node tables are padded to a multiple of the build tile width
-#define BIE_NEAR_TAU 1.0e-3           // |w|^2 below which the near path is taken (|w| < 0.0316)
+#define BIE_NEAR_C 0.25               // tau_s = BIE_NEAR_C |q_s|  (fast-path entry error <= ~1e-14)
+#define BIE_NEAR_TAU_MIN 1.0e-9
+#define BIE_NEAR_TAU_MAX 1.0e-2       // |w| < 0.1: Laurent truncation 2|w/2|^9/93555 < 1e-16
 
-// SoA node table.  All double arrays have length npad.
+// Node table, arrays of double2 of length npad.
 struct NodeTable {
-    const double* S;     // sin(x/2)
-    const double* C;     // cos(x/2)
-    const double* P;     // exp(y/2)
-    const double* N;     // exp(-y/2)
-    const double* QR;    // Re zeta' / (2 M_j)   (source weight)
-    const double* QI;    // Im zeta' / (2 M_j)
-    const double* X;     // Re zeta
-    const double* Y;     // Im zeta
-    const double* DIAG;  // complete diagonal entry: Im{zeta''/(2 zeta')}/M_k -+ 1/2 - EM
-    const double* EM;    // [obstacle, variant A] / M_k, else 0   (E_m = M_m^{-1} e e^T)
+    const double2* E;    // (Re, Im) of e^{i zeta} scaled by e^{y_ref}
+    const double2* MT;   // (M = |E|^2, thr = tau_s M)
+    const double2* Q;    // zeta' / (2 M_j)   (source weight)
+    const double2* XY;   // (Re zeta, Im zeta)  (near path)
+    const double2* DG;   // (complete diagonal entry Im{zeta''/(2 zeta')}/M_k -+ 1/2 - em,  em = [obstacle, variant A]/M_k)
     const int* COMP;     // component index of the node (padding: -1)
     int n;
     int npad;
 };
-#define BIE_NODE_ARRAYS 10
+#define BIE_NODE_ARRAYS 10            // doubles per node in node_buf
 
 // component offsets, by value into kernels (<= 260 bytes)
 struct CompTable {
@@ -96,20 +94,19 @@ int bie_launch_probe_dfma(bie_ctx* ctx, int64_t fma_per_thread, double* out, int
 // device helpers
 // ---------------------------------------------------------------------------------------------------
 #ifdef __CUDACC__
-// 1/d for d > 0 in normal range: MUFU.RCP64H seed + two Newton steps (4 DFMA); within about 1 ulp, which
-// is all an entry needs (no IEEE division sequence, no slow-path branch).  d = 0 gives inf/NaN: callers
-// overwrite those pairs (s == t) afterwards.
-__device__ __forceinline__ double bie_rcp(double d) {
+// 1/d for d > 0 in normal range: MUFU.RCP64H seed (relative error < 2^-19.9, measured over 2^24 arguments on
+// B200) + one cubic refinement r0 (1 + e + e^2), e = 1 - d r0: error e^3 < 2^-59 plus rounding, 2 ulp at most.
+// Three DFMA, no IEEE division sequence, no slow-path branch.  d = 0 gives inf/NaN: those pairs are near pairs
+// and never use the value.
+__device__ __forceinline__ double bie_rcp3(double d) {
     double r;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
-    double e = fma(-d, r, 1.0);
-    r = fma(r, e, r);
-    e = fma(-d, r, 1.0);
-    r = fma(r, e, r);
-    return r;
+    const double e = fma(-d, r, 1.0);
+    const double t = fma(e, e, e);
+    return fma(r, t, r);
 }
 
-// Near path: cot(w/2) for |w mod 2 pi| < about 0.05, from the differences x = x_s - x_t, y = y_s - y_t.
+// Near path: cot(w/2) for |w mod 2 pi| < 0.1, from the differences x = x_s - x_t, y = y_s - y_t.
 // x is reduced to (-pi, pi] with a two-word 2 pi (the kernel is 2 pi-periodic in x: the sum over images
 // of Eq. (3.4)), then with z = w/2
 //   cot z = 1/z - z (1/3 + z^2 (1/45 + z^2 (2/945 + z^2/4725)))      (truncation < 1e-20 |z| for |z| < 0.03)

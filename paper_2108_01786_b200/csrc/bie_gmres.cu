@@ -96,11 +96,7 @@ __device__ __forceinline__ void cta_apply(const GmresArgs& a, int r0, int r1, co
                                           double* xs, double* gpart, double* y_local)
 {
     if (FREE) {
-        bie_cta_matvec_free(a.nt, a.ct, r0, r1, xin, gpart, y_local);
-        if (scale != 1.0) {
-            for (int r = threadIdx.x; r < r1 - r0; r += blockDim.x) y_local[r] *= scale;
-            __syncthreads();
-        }
+        bie_cta_matvec_free(a.nt, a.ct, r0, r1, xin, scale, gpart, y_local);
     } else if (XS) {
         const int n2 = a.n >> 1;
         for (int i = threadIdx.x; i < n2; i += blockDim.x) {
@@ -173,7 +169,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
     double* g = sn + m;                   // [m+1]
     double* red = g + (m + 1);            // [34]
     double* gpart = red + 34 + ((m & 1) ? 0 : 1);  // GEMV partials or matrix-free scratch (16-byte aligned)
-    double* xs = gpart + (FREE ? free_scratch_doubles(a.rows_per_cta)
+    double* xs = gpart + (FREE ? free_scratch_doubles(GM_THREADS)
                                : ((gemv_part_doubles(a.rows_per_cta, n, a.chunk) + 1) & ~1));
     double* part1 = a.part;
     double* part2 = a.part + (size_t)(m + 2) * G;
@@ -351,7 +347,7 @@ static int gmres_plan(int n, int restart, int sm_count, int max_smem, int l2_byt
     pl->nld = (n + 1) & ~1;
     const int rows2 = (pl->rows_per_cta + 1) & ~1;
     size_t base = 2 * (size_t)rows2 + 2 * (size_t)(m + 2) + 2 * (size_t)m + (size_t)(m + 1) + 34 + 1;
-    base += free_op ? (size_t)free_scratch_doubles(pl->rows_per_cta)
+    base += free_op ? (size_t)free_scratch_doubles(GM_THREADS)
                     : (size_t)((gemv_part_doubles(pl->rows_per_cta, n, pl->chunk) + 1) & ~1);
     base *= sizeof(double);
     pl->xs = !free_op && base + sizeof(double) * ((size_t)n + 2) <= (size_t)max_smem;

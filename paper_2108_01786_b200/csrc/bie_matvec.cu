@@ -78,7 +78,7 @@ bie_matvec_free_kernel(NodeTable nt, CompTable ct, int rows_per_cta, const doubl
     if (r0 >= r1) return;
     double* y_local = smem;
     double* scratch = y_local + ((rows_per_cta + 1) & ~1);
-    bie_cta_matvec_free(nt, ct, r0, r1, x, scratch, y_local);
+    bie_cta_matvec_free(nt, ct, r0, r1, x, 1.0, scratch, y_local);
     for (int r = threadIdx.x; r < r1 - r0; r += blockDim.x) y[r0 + r] = y_local[r];
 }
 
@@ -90,7 +90,7 @@ int bie_launch_matvec_free(bie_ctx* ctx, const double* x, double* y, cudaStream_
     const int n = ctx->n;
     const int G = ctx->sm_count;
     const int rows_per_cta = (n + G - 1) / G;
-    const size_t smem = sizeof(double) * (((rows_per_cta + 1) & ~1) + free_scratch_doubles(rows_per_cta));
+    const size_t smem = sizeof(double) * (((rows_per_cta + 1) & ~1) + free_scratch_doubles(FREE_THREADS));
     if (smem > (size_t)ctx->max_smem_optin) return BIE_ERR_ARG;
     BIE_CUDA(cudaFuncSetAttribute(bie_matvec_free_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int grid = (n + rows_per_cta - 1) / rows_per_cta;

@@ -1,9 +1,11 @@
 // bie_nodes.cu -- SURVEY 8(a) row a1: per-node factors of the pair arithmetic (see bie_common.cuh).
 //
 // One thread per node.  The only transcendentals of the whole matrix build are evaluated here, O(n) of
-// them: sincos(x/2), exp(+-y/2).  Also the source weight q = zeta'/(2 M_j), the complete
-// diagonal entry from the limit K_jj(a,a) = Im{zeta''/(2 zeta')} with the -+1/2 of
-// Eq. (3.10) and the -1/M_m of E_m.
+// them: sincos(x) and exp(-(y - y_ref)), giving E = e^{i zeta} up to the common factor e^{-y_ref}
+// (y_ref = Im zeta[0]; cot((zeta_s - zeta_t)/2) only sees ratios E_s/E_t).  Also the source weight
+// q = zeta'/(2 M_j), the near threshold thr = tau_s |E|^2, and the complete diagonal entry from the
+// limit K_jj(a,a) = Im{zeta''/(2 zeta')} with the -+1/2 of Eq. (3.10) and the
+// -1/M_m of E_m.
 #include "bie_common.cuh"
 
 struct PrepArgs {
@@ -14,44 +16,42 @@ struct PrepArgs {
 __global__ void __launch_bounds__(256)
 bie_prepare_nodes_kernel(PrepArgs pa, int n, int npad, int variant,
                          const double2* __restrict__ zeta, const double2* __restrict__ dzeta,
-                         const double2* __restrict__ d2zeta, double* __restrict__ buf, int* __restrict__ comp)
+                         const double2* __restrict__ d2zeta, double2* __restrict__ buf, int* __restrict__ comp)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= npad) return;
-    double* S = buf;
-    double* C = buf + (size_t)npad;
-    double* P = buf + 2 * (size_t)npad;
-    double* N = buf + 3 * (size_t)npad;
-    double* QR = buf + 4 * (size_t)npad;
-    double* QI = buf + 5 * (size_t)npad;
-    double* X = buf + 6 * (size_t)npad;
-    double* Y = buf + 7 * (size_t)npad;
-    double* DG = buf + 8 * (size_t)npad;
-    double* EM = buf + 9 * (size_t)npad;
-    if (i >= n) {  // padding: benign values, never stored to A
-        S[i] = 0.0; C[i] = 1.0; P[i] = 1.0; N[i] = 1.0; QR[i] = 0.0; QI[i] = 0.0;
-        X[i] = 0.0; Y[i] = 1.0e3; DG[i] = 0.0; EM[i] = 0.0; comp[i] = -1;
+    double2* E = buf;
+    double2* MT = buf + (size_t)npad;
+    double2* Q = buf + 2 * (size_t)npad;
+    double2* XY = buf + 3 * (size_t)npad;
+    double2* DG = buf + 4 * (size_t)npad;
+    if (i >= n) {  // padding: zero weight, never near (thr = 0), never stored to A
+        E[i] = make_double2(0.0, 0.0); MT[i] = make_double2(0.0, 0.0); Q[i] = make_double2(0.0, 0.0);
+        XY[i] = make_double2(0.0, 1.0e3); DG[i] = make_double2(0.0, 0.0); comp[i] = -1;
         return;
     }
     int k = 0;
     while (k + 1 < pa.comps.ncomp && i >= pa.comps.off[k + 1]) ++k;
     const double M = (double)(pa.comps.off[k + 1] - pa.comps.off[k]);
     const double2 z = zeta[i], dz = dzeta[i], d2 = d2zeta[i];
+    const double yref = zeta[0].y;
     double s, c;
-    sincos(0.5 * z.x, &s, &c);
-    S[i] = s; C[i] = c;
-    P[i] = exp(0.5 * z.y);
-    N[i] = exp(-0.5 * z.y);
-    QR[i] = dz.x / (2.0 * M);
-    QI[i] = dz.y / (2.0 * M);
-    X[i] = z.x; Y[i] = z.y;
+    sincos(z.x, &s, &c);
+    const double m = exp(-(z.y - yref));
+    E[i] = make_double2(m * c, m * s);
+    const double qr = dz.x / (2.0 * M), qi = dz.y / (2.0 * M);
+    Q[i] = make_double2(qr, qi);
+    double tau = BIE_NEAR_C * sqrt(qr * qr + qi * qi);
+    tau = fmin(fmax(tau, BIE_NEAR_TAU_MIN), BIE_NEAR_TAU_MAX);
+    MT[i] = make_double2(m * m, tau * m * m);
+    XY[i] = z;
     // Im{ zeta'' / (2 zeta' M) }
     const double den = dz.x * dz.x + dz.y * dz.y;
     double d = (d2.y * dz.x - d2.x * dz.y) / den / (2.0 * M);
     const double em = (variant == BIE_VARIANT_A && pa.kinds[k] == BIE_KIND_OBSTACLE) ? 1.0 / M : 0.0;
     d += (k == 0) ? -0.5 : 0.5;
     d -= em;
-    DG[i] = d; EM[i] = em;
+    DG[i] = make_double2(d, em);
     comp[i] = k;
 }
 
@@ -59,16 +59,12 @@ NodeTable bie_node_table(const bie_ctx* ctx)
 {
     NodeTable t;
     const size_t np = (size_t)bie_npad(ctx->n);
-    t.S = ctx->node_buf;
-    t.C = ctx->node_buf + np;
-    t.P = ctx->node_buf + 2 * np;
-    t.N = ctx->node_buf + 3 * np;
-    t.QR = ctx->node_buf + 4 * np;
-    t.QI = ctx->node_buf + 5 * np;
-    t.X = ctx->node_buf + 6 * np;
-    t.Y = ctx->node_buf + 7 * np;
-    t.DIAG = ctx->node_buf + 8 * np;
-    t.EM = ctx->node_buf + 9 * np;
+    const double2* b = reinterpret_cast<const double2*>(ctx->node_buf);
+    t.E = b;
+    t.MT = b + np;
+    t.Q = b + 2 * np;
+    t.XY = b + 3 * np;
+    t.DG = b + 4 * np;
     t.COMP = ctx->comp_buf;
     t.n = ctx->n;
     t.npad = (int)np;
@@ -118,7 +114,7 @@ int bie_prepare_nodes(bie_ctx* ctx, int ncomp, const int32_t* counts, const int3
     ctx->have_geom = 1;
     bie_prepare_nodes_kernel<<<(npad + 255) / 256, 256, 0, st>>>(
         pa, (int)n, npad, variant, (const double2*)zeta, (const double2*)dzeta, (const double2*)d2zeta,
-        ctx->node_buf, ctx->comp_buf);
+        (double2*)ctx->node_buf, ctx->comp_buf);
     BIE_CUDA(cudaGetLastError());
     return BIE_OK;
 }
