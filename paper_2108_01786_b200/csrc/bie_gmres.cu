@@ -42,6 +42,7 @@ struct GmresArgs {
     int nld;
     int rows_per_cta;
     int chunk;
+    int VS;        // Krylov vectors 0..VS-1 keep this CTA's rows in shared memory; the others in V (global, L2)
     NodeTable nt;
     CompTable ct;
 };
@@ -116,36 +117,95 @@ __device__ __forceinline__ void cta_apply(const GmresArgs& a, int r0, int r1, co
     }
 }
 
+// This CTA's rows of Krylov vector i: in shared memory for i < VS, else in the global basis (L2-resident).
+struct Basis {
+    double* Vs;      // shared, [VS][rows2]
+    double* Vg;      // global, a.V + r0, vector stride nld
+    int VS, rows2;
+    long long nld;
+};
+
+// t[r] = sum_{i < cnt} coef[i] * v_i[r] for this CTA's rows, using every thread: the threads form `groups`
+// groups of rp threads; group g takes the vectors i = g, g + groups, ...; the group sums are added in fixed
+// order.  red2: shared, >= blockDim.x + rows2 doubles.  Result in red2[0 .. rows) after the closing barrier.
+__device__ __forceinline__ void basis_combine(const Basis& B, int rows, int cnt, const double* coef, double* red2)
+{
+    int rp = (rows + 31) & ~31;
+    if (rp > (int)blockDim.x) rp = blockDim.x;
+    const int groups = blockDim.x / rp;
+    const int g = threadIdx.x / rp, lr = threadIdx.x - g * rp;
+    const int cs_ = min(cnt, B.VS);
+    if (g < groups) {
+        for (int r = lr; r < rows; r += rp) {
+            double s0 = 0.0, s1 = 0.0;
+            int i = g;
+            const double* vs = B.Vs + r;
+            for (; i + groups < cs_; i += 2 * groups) {
+                s0 = fma(coef[i], vs[(size_t)i * B.rows2], s0);
+                s1 = fma(coef[i + groups], vs[(size_t)(i + groups) * B.rows2], s1);
+            }
+            for (; i < cs_; i += groups) s0 = fma(coef[i], vs[(size_t)i * B.rows2], s0);
+            const double* vg = B.Vg + r;
+#pragma unroll 4
+            for (; i < cnt; i += groups) s1 = fma(coef[i], __ldcg(vg + (size_t)i * B.nld), s1);
+            red2[g * rp + r] = s0 + s1;   // rows <= rp unless groups == 1
+        }
+    }
+    __syncthreads();
+    if (groups > 1) {
+        double t = 0.0;
+        const int r = threadIdx.x;
+        if (r < rows)
+            for (int q = 0; q < groups; ++q) t += red2[q * rp + r];
+        __syncthreads();
+        if (r < rows) red2[r] = t;
+        __syncthreads();
+    }
+}
+
 // one classical Gram-Schmidt pass against v_0..v_j: hloc[i] (+)= <v_i, w>, w -= sum_i <v_i, w> v_i
-__device__ __forceinline__ void cgs_pass(const GmresArgs& a, int r0, int rows, int j, double* part_slot,
-                                         double* w_local, double* hloc, double* hacc, bool accumulate,
+__device__ __forceinline__ void cgs_pass(const GmresArgs& a, const Basis& B, int rows, int j, double* part_slot,
+                                         double* w_local, double* hloc, double* hacc, bool accumulate, double* red2,
                                          unsigned int& target)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
     const int G = gridDim.x;
     for (int i = warp; i <= j; i += nwarp) {
-        const double* vi = a.V + (size_t)i * a.nld + r0;
         double s = 0.0;
-        for (int r = lane; r < rows; r += 32) s = fma(vi[r], w_local[r], s);
+        if (i < B.VS) {
+            const double* vi = B.Vs + (size_t)i * B.rows2;
+            for (int r = lane; r < rows; r += 32) s = fma(vi[r], w_local[r], s);
+        } else {
+            const double* vi = B.Vg + (size_t)i * B.nld;
+            for (int r = lane; r < rows; r += 32) s = fma(__ldcg(vi + r), w_local[r], s);
+        }
         s = bie_warp_sum(s);
         if (lane == 0) part_slot[(size_t)i * G + blockIdx.x] = s;
     }
     grid_barrier(a.sync, target);
-    for (int i = warp; i <= j; i += nwarp) {
-        const double h = warp_sum_partials(part_slot + (size_t)i * G, G);
-        if (lane == 0) {
-            hloc[i] = h;
-            hacc[i] = accumulate ? hacc[i] + h : h;
+    // fixed-order sums of the G per-CTA partials; the loads of up to four vectors are in flight together
+    for (int i0 = warp; i0 <= j; i0 += 4 * nwarp) {
+        double s[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int i = i0 + q * nwarp;
+            s[q] = 0.0;
+            if (i <= j)
+                for (int c = lane; c < G; c += 32) s[q] += __ldcg(part_slot + (size_t)i * G + c);
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int i = i0 + q * nwarp;
+            const double h = bie_warp_sum(s[q]);
+            if (i <= j && lane == 0) {
+                hloc[i] = h;
+                hacc[i] = accumulate ? hacc[i] + h : h;
+            }
         }
     }
     __syncthreads();
-    for (int r = threadIdx.x; r < rows; r += blockDim.x) {
-        double s = 0.0;
-        const double* v = a.V + r0 + r;
-#pragma unroll 4
-        for (int i = 0; i <= j; ++i) s = fma(hloc[i], v[(size_t)i * a.nld], s);
-        w_local[r] -= s;
-    }
+    basis_combine(B, rows, j + 1, hloc, red2);
+    for (int r = threadIdx.x; r < rows; r += blockDim.x) w_local[r] -= red2[r];
     __syncthreads();
 }
 
@@ -171,6 +231,10 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
     double* gpart = red + 34 + ((m & 1) ? 0 : 1);  // GEMV partials or matrix-free scratch (16-byte aligned)
     double* xs = gpart + (FREE ? free_scratch_doubles(GM_THREADS)
                                : ((gemv_part_doubles(a.rows_per_cta, n, a.chunk) + 1) & ~1));
+    double* red2 = xs + ((FREE || !XS) ? 0 : ((n + 2) & ~1));   // [blockDim + rows2]
+    Basis B;
+    B.Vs = red2 + GM_THREADS + rows2;                          // [VS][rows2]
+    B.Vg = a.V + r0; B.VS = a.VS; B.rows2 = rows2; B.nld = a.nld;
     double* part1 = a.part;
     double* part2 = a.part + (size_t)(m + 2) * G;
     double* part3 = a.part + 2 * (size_t)(m + 2) * G;
@@ -216,7 +280,10 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
         if (beta <= thresh) break;                         // converged (status 0)
         if (iters >= a.max_iters) { status = BIE_MAX_ITERS; break; }
         double inv = 1.0 / beta;
-        for (int r = threadIdx.x; r < rows; r += blockDim.x) a.V[r0 + r] = w_local[r] * inv;
+        {
+            double* v0 = (0 < B.VS) ? B.Vs : B.Vg;
+            for (int r = threadIdx.x; r < rows; r += blockDim.x) v0[r] = w_local[r] * inv;
+        }
         if (threadIdx.x == 0) g[0] = beta;
         __syncthreads();
 
@@ -229,8 +296,8 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
             for (int r = threadIdx.x; r < rows; r += blockDim.x) w_local[r] = y_local[r];
             __syncthreads();
             // a7: CGS2
-            cgs_pass(a, r0, rows, j, part1, w_local, hloc, hcol, false, target);
-            cgs_pass(a, r0, rows, j, part2, w_local, hloc, hcol, true, target);
+            cgs_pass(a, B, rows, j, part1, w_local, hloc, hcol, false, red2, target);
+            cgs_pass(a, B, rows, j, part2, w_local, hloc, hcol, true, red2, target);
             p = 0.0;
             for (int r = threadIdx.x; r < rows; r += blockDim.x) {
                 const double v = w_local[r];
@@ -243,7 +310,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
             const double hn = sqrt(warp_sum_partials(part3, G));
             inv = (hn != 0.0) ? 1.0 / hn : 0.0;
             {
-                double* vn = a.V + (size_t)(j + 1) * a.nld + r0;
+                double* vn = (j + 1 < B.VS) ? B.Vs + (size_t)(j + 1) * rows2 : B.Vg + (size_t)(j + 1) * a.nld;
                 for (int r = threadIdx.x; r < rows; r += blockDim.x) vn[r] = w_local[r] * inv;
             }
             // a8: Givens rotations on column j, new rotation, recurrence residual
@@ -292,12 +359,8 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
         grid_barrier(a.sync, target);
         for (int i = threadIdx.x; i < k; i += blockDim.x) hloc[i] = __ldcg(a.yv + i);
         __syncthreads();
-        for (int r = threadIdx.x; r < rows; r += blockDim.x) {
-            double s = 0.0;
-            const double* v = a.V + r0 + r;
-            for (int i = 0; i < k; ++i) s = fma(hloc[i], v[(size_t)i * a.nld], s);
-            a.x[r0 + r] += s;
-        }
+        basis_combine(B, rows, k, hloc, red2);
+        for (int r = threadIdx.x; r < rows; r += blockDim.x) a.x[r0 + r] += red2[r];
         grid_barrier(a.sync, target);  // x complete (next residual / final residual read all of it)
         if (conv) break;
         if (iters >= a.max_iters) { status = BIE_MAX_ITERS; break; }
@@ -330,7 +393,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
 static inline size_t al256(size_t b) { return (b + 255) & ~(size_t)255; }
 
 struct GmresPlan {
-    int G, rows_per_cta, chunk, nld;
+    int G, rows_per_cta, chunk, nld, VS;
     bool xs, stream;
     size_t smem;
     size_t offV, offW, offP, offR, offY, total;
@@ -350,9 +413,17 @@ static int gmres_plan(int n, int restart, int sm_count, int max_smem, int l2_byt
     base += free_op ? (size_t)free_scratch_doubles(GM_THREADS)
                     : (size_t)((gemv_part_doubles(pl->rows_per_cta, n, pl->chunk) + 1) & ~1);
     base *= sizeof(double);
+    base += sizeof(double) * ((size_t)GM_THREADS + rows2);  // red2
     pl->xs = !free_op && base + sizeof(double) * ((size_t)n + 2) <= (size_t)max_smem;
     pl->smem = base + (pl->xs ? sizeof(double) * ((size_t)n + 2) : 0);
     if (pl->smem > (size_t)max_smem) return BIE_ERR_ARG;
+    // the rest of the shared memory holds this CTA's rows of as many Krylov vectors as fit
+    // (dense operator: the streaming loads of A need the L1 as their landing buffer, 16 warps x 4 KB in flight,
+    // so the shared-memory carve-out stops at 164 KB; measured: 408 us per step with 227 KB against 338 us)
+    const size_t cap = free_op ? (size_t)max_smem : (size_t)(163 * 1024 < max_smem ? 163 * 1024 : max_smem);
+    pl->VS = pl->smem < cap ? (int)((cap - pl->smem) / (sizeof(double) * rows2)) : 0;
+    if (pl->VS > m + 1) pl->VS = m + 1;
+    pl->smem += sizeof(double) * (size_t)pl->VS * rows2;
     if (free_op && pl->rows_per_cta > 2 * FREE_THREADS) return BIE_ERR_ARG;
     pl->stream = !free_op && (double)n * (double)lda * 8.0 > 0.6 * (double)l2_bytes;
     size_t o = 0;
@@ -421,7 +492,7 @@ int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, const do
     a.R = (double*)(base + pl.offR);
     a.yv = (double*)(base + pl.offY);
     a.sync = ctx->sync_buf;
-    a.nld = pl.nld; a.rows_per_cta = pl.rows_per_cta; a.chunk = pl.chunk;
+    a.nld = pl.nld; a.rows_per_cta = pl.rows_per_cta; a.chunk = pl.chunk; a.VS = pl.VS;
     if (free_op) { a.nt = bie_node_table(ctx); a.ct = ctx->comps; }
     else { memset(&a.nt, 0, sizeof(a.nt)); memset(&a.ct, 0, sizeof(a.ct)); }
     BIE_CUDA(cudaMemsetAsync(ctx->sync_buf, 0, sizeof(unsigned int), st));
