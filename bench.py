@@ -214,33 +214,22 @@ def main():
         run_reference(args)
         return
     import torch
-    import torch.distributed as dist
-    from paper_2108_01786_b200 import bie, inputs, build as _build
+    from paper_2108_01786_b200 import bie, inputs, ranks, build as _build
 
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a B200: the CUDA path has no CPU fallback")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    R = ranks.from_env("nccl")      # replicas only: NCCL serves the timing barrier and the max, nothing else
+    rank, local, world = R.rank, R.local_rank, R.world
     if rank == 0:
         _build.build_library()
-    if world > 1:
-        dist.barrier()
+    ranks.barrier(R)
 
     def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+        ranks.barrier(R, torch.cuda.synchronize)
 
     def max_over_ranks(v: float) -> float:
-        if world == 1:
-            return v
-        t = torch.tensor([v], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t[0])
+        return ranks.max_over_ranks(R, v)
 
     P = inputs.make_config(args.config)
     g, n = P.geometry, P.n
@@ -341,8 +330,7 @@ def main():
     d2h = 8 * n + 8 + 8
 
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
+        ranks.finish(R)
         return
 
     # ---- rooflines -------------------------------------------------------------------------------------------
@@ -384,8 +372,7 @@ def main():
                                 "ms_per_step": est * 1e3, "build_gentries_per_s": n * n / parts["build_s"] / 1e9,
                                 "gmres_ms": parts["gemv_s"] * parts["gemvs"] * 1e3}
     print(json.dumps(line), flush=True)
-    if world > 1:
-        dist.destroy_process_group()
+    ranks.finish(R)
 
 
 if __name__ == "__main__":
