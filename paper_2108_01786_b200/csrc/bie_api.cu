@@ -24,8 +24,10 @@ int bie_create(bie_ctx** out, int device)
     c->l2_bytes = prop.l2CacheSize;
     c->coop_ok = prop.cooperativeLaunch;
     c->max_smem_optin = (int)prop.sharedMemPerBlockOptin;
-    c->node_buf = nullptr; c->comp_buf = nullptr; c->cap = 0; c->have_geom = 0; c->n = 0;
+    c->node_buf = nullptr; c->comp_buf = nullptr; c->free_buf = nullptr; c->cap = 0; c->have_geom = 0; c->n = 0;
     c->sync_buf = nullptr; c->pinned_i = nullptr; c->pinned_d = nullptr;
+    c->near_ptr = nullptr; c->near_col = nullptr; c->near_val = nullptr; c->near_valid = 0;
+    c->taubar = nullptr; c->near_overflow = nullptr;
     if (cudaMalloc((void**)&c->sync_buf, 256) != cudaSuccess ||
         cudaMallocHost((void**)&c->pinned_i, 4 * sizeof(int32_t)) != cudaSuccess ||
         cudaMallocHost((void**)&c->pinned_d, 4 * sizeof(double)) != cudaSuccess) {
@@ -35,6 +37,9 @@ int bie_create(bie_ctx** out, int device)
         delete c;
         return bie_cuda_err(le == cudaSuccess ? cudaErrorMemoryAllocation : le);
     }
+    // the tail of the 256-byte block holds two device scalars
+    c->taubar = reinterpret_cast<double*>(reinterpret_cast<char*>(c->sync_buf) + 64);
+    c->near_overflow = reinterpret_cast<int*>(reinterpret_cast<char*>(c->sync_buf) + 128);
     *out = c;
     return BIE_OK;
 }
@@ -45,6 +50,10 @@ int bie_destroy(bie_ctx* c)
     cudaSetDevice(c->device);
     if (c->node_buf) cudaFree(c->node_buf);
     if (c->comp_buf) cudaFree(c->comp_buf);
+    if (c->free_buf) cudaFree(c->free_buf);
+    if (c->near_ptr) cudaFree(c->near_ptr);
+    if (c->near_col) cudaFree(c->near_col);
+    if (c->near_val) cudaFree(c->near_val);
     if (c->sync_buf) cudaFree(c->sync_buf);
     if (c->pinned_i) cudaFreeHost(c->pinned_i);
     if (c->pinned_d) cudaFreeHost(c->pinned_d);

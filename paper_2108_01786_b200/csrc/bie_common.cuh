@@ -23,6 +23,7 @@
 #define BIE_NEAR_C 0.25               // tau_s = BIE_NEAR_C |q_s|  (fast-path entry error <= ~1e-14)
 #define BIE_NEAR_TAU_MIN 1.0e-9
 #define BIE_NEAR_TAU_MAX 1.0e-2       // |w| < 0.1: Laurent truncation 2|w/2|^9/93555 < 1e-16
+#define BIE_NEAR_PER_NODE 48          // capacity of the CSR near matrix of the matrix-free operator, entries per node
 
 // Node table, arrays of double2 of length npad.
 struct NodeTable {
@@ -52,6 +53,13 @@ struct bie_ctx {
     // node-table storage (device), capacity in nodes
     double* node_buf;
     int* comp_buf;
+    double* free_buf;        // matrix-free operator: per-matvec source tables [8][cap] + partial sums (bie_free.cuh)
+    double* taubar;          // device scalar: max_s tau_s of the current geometry (bie_near.cu)
+    int* near_ptr;           // CSR near matrix (bie_near.cu): [8 cap + 1] offsets of the (row, segment) lists
+    int* near_col;           // [BIE_NEAR_PER_NODE cap]
+    double* near_val;        // [BIE_NEAR_PER_NODE cap]
+    int* near_overflow;      // device flag: the near matrix did not fit (the operator then returns NaN)
+    int near_valid;          // near matrix built for the current geometry
     unsigned int* sync_buf;  // grid-barrier counter
     int cap;
     // current geometry (host copies)
@@ -76,6 +84,12 @@ static inline int bie_cuda_err(cudaError_t e) { return e == cudaSuccess ? BIE_OK
 
 static inline int bie_npad(int n) { return (n + BIE_NODE_PAD - 1) / BIE_NODE_PAD * BIE_NODE_PAD; }
 NodeTable bie_node_table(const bie_ctx* ctx);
+struct FreePlan;
+// doubles of ctx->free_buf for a node capacity `cap`; work split of the matrix-free operator over `grid` CTAs
+size_t bie_free_buf_doubles(int cap);
+int bie_free_plan(const bie_ctx* ctx, int grid, FreePlan* fp);
+size_t bie_near_cap(int npad);
+int bie_ensure_near(bie_ctx* ctx, cudaStream_t st);
 
 // internal entry points (one per .cu)
 int bie_prepare_nodes(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds,
@@ -127,6 +141,26 @@ __device__ __forceinline__ void bie_cot_half_near(double x, double y, double* re
     // 1/z - z p
     *re = zr * inv - fma(zr, pr, -zi * pi);
     *im = -zi * inv - fma(zr, pi, zi * pr);
+}
+
+// ---- grid barrier (cooperative launch guarantees co-residency) -------------------------------------
+__device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p)
+{
+    unsigned int v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void grid_barrier(unsigned int* ctr, unsigned int& target)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        target += gridDim.x;
+        __threadfence();
+        atomicAdd(ctr, 1u);
+        while (ld_acquire_u32(ctr) < target) { }
+        __threadfence();
+    }
+    __syncthreads();
 }
 
 __device__ __forceinline__ double bie_warp_sum(double v) {

@@ -1,251 +1,222 @@
 // bie_free.cuh -- matrix-free form of SURVEY 8(a) row a6: y_t = sum_s A[t][s] x_s with the entries of
 // Eq. (3.16) recomputed on the fly from the node tables; no matrix traffic at all.
-// Device functions for a TEAM of warps of one CTA (all of it in bie_matvec_free and in the matrix-free GMRES;
-// half of it in the hybrid GMRES, where the other half streams stored columns from HBM).
+// Device functions shared by bie_matvec_free (bie_matvec.cu) and the matrix-free GMRES (bie_gmres.cu).
 //
-// Mapping.  The CTA owns the targets [r0, r1).  A thread keeps TWO targets in registers (E_t, M_t and class) and
-// runs over a share of the sources, which are staged tile by tile in shared memory and read as warp-wide
-// broadcasts; the running sums stay in registers, so there is no reduction in the inner loop.  The team's
-// threads form NG source groups of TG threads (TG = target slots / 2, a power of two >= 32); group g takes the
-// g-th part of every source tile; the NG partial sums per target are added in fixed order at the end.
-// The source's weight, the Re/Im selection of Eq. (3.10) and x_s are folded into two coefficient pairs per
-// source, (alpha, beta) x_s for targets on Gamma_0 and for targets on solids (see bie_common.cuh).
-// Per pair: 13 FP64-pipe instructions.  The inner loop is branch-free: near pairs (den < thr_s, including
-// s == t) are left out by predication and only flagged; after every FREE_SB sources the warp votes and, if
-// needed, revisits those sources for the near pairs alone (Laurent series / diagonal limit).
-// The rank-one E_k is applied as -(1/M_k) sum_{s in k} x_s after the pair loop.
+// Arithmetic.  With E = e^{i zeta} per node (bie_common.cuh), X = Im(E_t conj E_s), Y = M_s - M_t and the
+// block coefficients (alpha, beta) of Eq. (3.10), the product of an entry with x_s is
+//     A[t][s] x_s = (alpha X + beta Y) x_s / den
+//                 = ( Ei_t P_s - Er_t Q_s + R_s - M_t B_s ) / den,          den = |E_s - E_t|^2,
+//     P_s = alpha x_s Er_s,  Q_s = alpha x_s Ei_s,  R_s = beta x_s M_s,  B_s = beta x_s,
+// so everything that depends on the source alone is folded, once per matvec and per source (O(n)), into two
+// double2 (P,Q), (R,B) per target class (class 0: target on Gamma_0, class 1: target on a solid; the class fixes
+// the Re/Im/sign selection of Eq. (3.10)).  Per pair that leaves 11 FP64-pipe instructions:
+// 2 sub, 2 for den, 3 FMA for the numerator, 3 FMA refining MUFU.RCP64H (bie_rcp3), 1 FMA accumulating.
+//
+// Work split.  The rows are cut into row blocks of FREE_ROWS = 128 targets of one class; the (row block x source)
+// rectangle list is laid out linearly and cut into gridDim.x equal slabs, one per CTA, so every SM has the same
+// number of pairs whatever n is.  A CTA's slab touches one or two row blocks ("parts"); for each part the 16
+// warps share the part's sources, every lane keeps FREE_NT = 4 targets of the block in registers and runs over
+// its warp's sources, which the warp stages 32 at a time in its own shared-memory buffer (no CTA-wide barrier in
+// the pair loop) and reads as warp-wide broadcasts.  The 16 warp sums are added in fixed order and go to a
+// partial buffer in global memory (L2); after a grid barrier the owner of a row adds the (at most three)
+// partials of its row block, again in fixed order: the result is deterministic.
+//
+// Near pairs.  den < taubar M_t (den/M_t = |e^{iw} - 1|^2 ~ |w|^2; this includes s == t) marks a pair as near:
+// it is left out of the fast sum by predication, and its exact entry (Laurent series of cot, or the analytic
+// diagonal limit PAPER.md:L265) comes from the sparse near matrix that bie_near.cu builds once per geometry;
+// the owner of a row adds  sum_k val[k] x[col[k]]  when it gathers the partials.  The rank-one E_k
+// is applied there too, as -(1/M_k) sum_{s in k} x_s.
 #pragma once
 #include "bie_common.cuh"
 
 #define FREE_THREADS 512
-#define FREE_SB 32   // sources between near votes
+#define FREE_WARPS (FREE_THREADS / 32)
+#define FREE_NT 4
+#define FREE_ROWS (32 * FREE_NT)
+#define FREE_STAGE_DOUBLES (FREE_WARPS * 2 * 3 * 32 * 2)
 
-struct FreeTeam {
-    int tid;   // 0 .. nthr-1
-    int nthr;  // multiple of 32; source tile = nthr sources (one per thread)
-    int bar;   // named barrier id used by this team (0 = the whole CTA)
-};
-__device__ __forceinline__ void team_sync(const FreeTeam& tm)
-{
-    asm volatile("bar.sync %0, %1;" ::"r"(tm.bar), "r"(tm.nthr) : "memory");
-}
-
-__host__ __device__ inline int free_tg(int rows, int nthr)
-{
-    int tg = 32;
-    while (tg < nthr && 2 * tg < rows) tg <<= 1;
-    return tg;
-}
-// doubles of scratch for a team of nthr threads: 2 tile buffers x 4 double2 arrays x nthr, group partials
-// [2][nthr], component sums
-__host__ __device__ inline int free_scratch_doubles(int nthr) { return 2 * 8 * nthr + 2 * nthr + BIE_MAX_COMP + 2; }
-
-struct FreeSrc {  // what one thread loads for one source of the next tile
-    double2 e, mt, q;
-    double x;
-    int comp;
+// host-computed description of the work split (by value into the kernels)
+struct FreePlan {
+    int M0;          // rows of class 0 = nodes of component 0
+    int NB0, NB;     // row blocks of class 0, all row blocks
+    int UB;          // units (of 2 sources) per row block = npad / 2
+    long long U;     // NB * UB
+    int Geff;        // CTAs that take a slab (<= gridDim.x)
+    double2* T;      // [4][npad]: (P,Q) class 0, (R,B) class 0, (P,Q) class 1, (R,B) class 1
+    double* PB;      // [(NB + Geff)][FREE_ROWS] partial sums, part id = row block + CTA
+    const double* taubar;     // device scalar: near threshold relative to M_t (bie_near.cu)
+    const int* near_ptr;      // CSR near matrix: offsets of the (row, segment) lists, row t = [ptr[8t], ptr[8t+8])
+    const int* near_col;
+    const double* near_val;
+    const int* near_overflow; // != 0: the near matrix did not fit; the operator returns NaN
 };
 
-__device__ __forceinline__ FreeSrc free_load_src(const NodeTable& nt, const double* __restrict__ x, double scale,
-                                                 int s, int s_end)
+// doubles of shared scratch: warp staging buffers [16][2 stages][3][32] double2, warp sums [16][128], component sums
+__host__ __device__ inline int free_scratch_doubles(int /*nthr*/)
 {
-    FreeSrc f;
-    if (s < s_end) {
-        f.e = nt.E[s]; f.mt = nt.MT[s]; f.q = nt.Q[s]; f.comp = nt.COMP[s];
-        f.x = __ldcg(x + s) * scale;
-    } else {  // beyond the range: zero weight (contributes exactly 0), never near (thr = 0)
-        f.e = make_double2(0.0, 0.0); f.mt = make_double2(0.0, 0.0); f.q = make_double2(0.0, 0.0);
-        f.x = 0.0; f.comp = -1;
+    return FREE_STAGE_DOUBLES + FREE_WARPS * FREE_ROWS + BIE_MAX_COMP + 2;
+}
+
+__device__ __forceinline__ long long free_slab_start(const FreePlan& fp, int c)
+{
+    return (long long)c * fp.U / fp.Geff;
+}
+__device__ __forceinline__ int free_block_row0(const FreePlan& fp, int b)
+{
+    return b < fp.NB0 ? b * FREE_ROWS : fp.M0 + (b - fp.NB0) * FREE_ROWS;
+}
+__device__ __forceinline__ int free_block_rows(const FreePlan& fp, int b, int n)
+{
+    const int r0 = free_block_row0(fp, b);
+    const int end = b < fp.NB0 ? fp.M0 : n;
+    return min(FREE_ROWS, end - r0);
+}
+
+// ---- step 1: per-source tables for the vector v (rows [r0, r1) of this CTA; v indexed from r0) ------------
+__device__ __forceinline__ void free_write_tables(const NodeTable& nt, const FreePlan& fp, int r0, int r1,
+                                                  const double* v /* shared or global, v[s - r0] */)
+{
+    const int np = nt.npad;
+    for (int s = r0 + threadIdx.x; s < r1; s += blockDim.x) {
+        const double2 e = nt.E[s], q = nt.Q[s];
+        const double M = nt.MT[s].x;
+        const double x = v[s - r0];
+        const bool src0 = (nt.COMP[s] == 0);
+        // (alpha, beta): Im c -> (-2 qi, qr), Re c -> (-2 qr, -qi), -Re c -> (2 qr, qi)   (bie_common.cuh)
+        double a0, b0, a1, b1;
+        if (src0) { a0 = -2.0 * q.y; b0 = q.x;  a1 = 2.0 * q.x;  b1 = q.y; }   // K_00 ; -G_k0
+        else      { a0 = -2.0 * q.x; b0 = -q.y; a1 = -2.0 * q.y; b1 = q.x; }   // G_0j ; K_kj
+        a0 *= x; b0 *= x; a1 *= x; b1 *= x;
+        fp.T[s]          = make_double2(a0 * e.x, a0 * e.y);
+        fp.T[np + s]     = make_double2(b0 * M, b0);
+        fp.T[2 * np + s] = make_double2(a1 * e.x, a1 * e.y);
+        fp.T[3 * np + s] = make_double2(b1 * M, b1);
     }
-    return f;
 }
 
-__device__ __forceinline__ void free_store_src(const FreeSrc& f, double2* buf, int nthr, int i)
+// ---- step 2: this CTA's slab of the (row block x source) list -> partial sums in fp.PB --------------------
+// scratch: shared, free_scratch_doubles() doubles, 16-byte aligned.  All threads of the CTA must call.
+__device__ __forceinline__ void free_parts(const NodeTable& nt, const FreePlan& fp, double* scratch)
 {
-    const double ur = f.q.x * f.x, ui = f.q.y * f.x;
-    buf[i] = f.e;
-    buf[nthr + i] = f.mt;
-    if (f.comp == 0) {
-        buf[2 * nthr + i] = make_double2(-2.0 * ui, ur);   // target on Gamma_0: Im c
-        buf[3 * nthr + i] = make_double2(2.0 * ur, ui);    // target on a solid: -Re c
-    } else {
-        buf[2 * nthr + i] = make_double2(-2.0 * ur, -ui);  // target on Gamma_0: Re c
-        buf[3 * nthr + i] = make_double2(-2.0 * ui, ur);   // target on a solid: Im c
-    }
-}
-
-struct FreeState {
-    double er[2], ei[2], m[2], acc[2];
-    int idx[2], cls[2];  // cls: 0 target on Gamma_0, 1 on a solid
-    int TG, NG, slot, grp;
-};
-
-__device__ __forceinline__ void free_begin(FreeState& st, const NodeTable& nt, int r0, int r1, const FreeTeam& tm)
-{
-    const int rows = r1 - r0;
-    st.TG = free_tg(rows, tm.nthr);
-    st.NG = tm.nthr / st.TG;
-    st.slot = tm.tid & (st.TG - 1);
-    st.grp = tm.tid / st.TG;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int c = blockIdx.x;
+    if (c >= fp.Geff) return;
+    double2* stage = reinterpret_cast<double2*>(scratch) + warp * (2 * 3 * 32);  // [2][3][32] double2 of this warp
+    double* wsum = scratch + FREE_STAGE_DOUBLES;                                  // [16][128]
+    const int np = nt.npad;
+    const double taubar = __ldg(fp.taubar);
+    long long u0 = free_slab_start(fp, c);
+    const long long u1 = free_slab_start(fp, c + 1);
+    int b = (int)(u0 / fp.UB);
+    while (u0 < u1) {
+        const long long ub = (long long)b * fp.UB;
+        const long long ue = min(u1, ub + fp.UB);
+        const int sa = 2 * (int)(u0 - ub), sb = 2 * (int)(ue - ub);  // sources [sa, sb) of row block b
+        const int cls = b < fp.NB0 ? 0 : 1;
+        const int row0 = free_block_row0(fp, b);
+        const int rows = free_block_rows(fp, b, nt.n);
+        // this lane's targets
+        double ter[FREE_NT], tei[FREE_NT], tm[FREE_NT], acc[FREE_NT];
+        int thi[FREE_NT];
 #pragma unroll
-    for (int q = 0; q < 2; ++q) {
-        const int loc = st.slot + q * st.TG;
-        const int i = r0 + min(loc, rows - 1);  // inactive slots shadow the last target; result dropped
-        const double2 e = nt.E[i];
-        st.er[q] = e.x; st.ei[q] = e.y; st.m[q] = nt.MT[i].x;
-        st.acc[q] = 0.0; st.idx[q] = i; st.cls[q] = (nt.COMP[i] == 0) ? 0 : 1;
-    }
-}
-
-// near pairs of the sources [jb, je) of the current tile, for one thread's two targets (rare path): returns the
-// two sums of their exact contributions.  Everything by value, so that the caller's state stays in registers.
-static __device__ __noinline__ double2 free_near_fix(const double2* __restrict__ DG, const double2* __restrict__ XY,
-                                                     const double* __restrict__ x, double scale, const double2* cur,
-                                                     int nthr, int jb, int je, int sbase, double er0, double ei0,
-                                                     double er1, double ei1, int idx0, int idx1, int cls0, int cls1)
-{
-    double add[2] = {0.0, 0.0};
-    const double ter[2] = {er0, er1}, tei[2] = {ei0, ei1};
-    const int tidx[2] = {idx0, idx1}, tcls[2] = {cls0, cls1};
-    for (int j = jb; j < je; ++j) {
-        const double2 e = cur[j];
-        const int thi = __double2hiint(cur[nthr + j].y);
-#pragma unroll
-        for (int q = 0; q < 2; ++q) {
-            const double dr = e.x - ter[q], di = e.y - tei[q];
-            const double den = fma(dr, dr, di * di);
-            if (__double2hiint(den) < thi) {
-                const int sidx = sbase + j;
-                if (sidx == tidx[q]) {  // diagonal entry without its -E part (that is in the component sum)
-                    const double2 dg = DG[sidx];
-                    add[q] = fma(dg.x + dg.y, __ldcg(x + sidx) * scale, add[q]);
-                } else {
-                    const double2 zs = XY[sidx], zt = XY[tidx[q]];
-                    double cr, ci;
-                    bie_cot_half_near(zs.x - zt.x, zs.y - zt.y, &cr, &ci);
-                    const double2 ab = cur[(2 + tcls[q]) * nthr + j];
-                    add[q] += fma(ab.y, ci, -0.5 * ab.x * cr);
-                }
-            }
+        for (int i = 0; i < FREE_NT; ++i) {
+            const int t = row0 + min(lane + 32 * i, rows - 1);  // inactive slots shadow the last row; result dropped
+            const double2 e = nt.E[t];
+            ter[i] = e.x; tei[i] = e.y; tm[i] = nt.MT[t].x; acc[i] = 0.0;
+            thi[i] = __double2hiint(taubar * tm[i]);
         }
-    }
-    return make_double2(add[0], add[1]);
-}
-
-// adds the contribution of the sources [c_lo, c_hi) (x scaled by `scale`) to the running sums.
-// scratch: shared, free_scratch_doubles(nthr) doubles, 16-byte aligned.  All threads of the team must call.
-__device__ __forceinline__ void free_chunk(FreeState& st, const NodeTable& nt, int c_lo, int c_hi,
-                                           const double* __restrict__ x, double scale, double* scratch,
-                                           const FreeTeam& tm)
-{
-    const int nthr = tm.nthr;
-    double2* const tile0 = reinterpret_cast<double2*>(scratch);  // two buffers of 4 nthr double2 each
-    const int per = nthr / st.NG;  // sources of a tile per group (= TG >= 32, a multiple of FREE_SB)
-    const int ntile = (c_hi - c_lo + nthr - 1) / nthr;
-    if (ntile <= 0) return;
-    FreeSrc nxt = free_load_src(nt, x, scale, c_lo + tm.tid, c_hi);
-    team_sync(tm);  // previous users of the tile buffers are done
-    free_store_src(nxt, tile0, nthr, tm.tid);
-    team_sync(tm);
-    const unsigned thr_lane_any = 0xffffffffu;
-    for (int it = 0; it < ntile; ++it) {
-        const double2* cur = tile0 + (it & 1) * 4 * nthr;
-        if (it + 1 < ntile) nxt = free_load_src(nt, x, scale, c_lo + (it + 1) * nthr + tm.tid, c_hi);
-        const double2* sE = cur;
-        const double2* sMT = cur + nthr;
-        const double2* ab0 = cur + (2 + st.cls[0]) * nthr;
-        const double2* ab1 = cur + (2 + st.cls[1]) * nthr;
-        const int sb = st.grp * per;
-        for (int jb = sb; jb < sb + per; jb += FREE_SB) {
-            int flag = 0;
+        // this warp's share of the sources, in units of 2
+        const int units = (sb - sa) >> 1;
+        const int wa = sa + 2 * (int)((long long)units * warp / FREE_WARPS);
+        const int wb = sa + 2 * (int)((long long)units * (warp + 1) / FREE_WARPS);
+        const double2* TE = nt.E;
+        const double2* TPQ = fp.T + (size_t)(2 * cls) * np;
+        const double2* TRB = fp.T + (size_t)(2 * cls + 1) * np;
+        const double2 zero2 = make_double2(0.0, 0.0);
+        double2 ne = zero2, npq = zero2, nrb = zero2;
+        if (wa + lane < wb) { const int s = wa + lane; ne = TE[s]; npq = __ldcg(TPQ + s); nrb = __ldcg(TRB + s); }
+        int buf = 0;
+        for (int base = wa; base < wb; base += 32, buf ^= 1) {
+            double2* sg = stage + buf * 96;
+            sg[lane] = ne; sg[32 + lane] = npq; sg[64 + lane] = nrb;   // the other buffer may still be read
+            __syncwarp();
+            {   // prefetch the next chunk
+                const int s = base + 32 + lane;
+                ne = zero2; npq = zero2; nrb = zero2;
+                if (s < wb) { ne = TE[s]; npq = __ldcg(TPQ + s); nrb = __ldcg(TRB + s); }
+            }
+            const int cnt = min(32, wb - base);   // even
 #pragma unroll 2
-            for (int j = jb; j < jb + FREE_SB; ++j) {
-                const double2 e = sE[j], mt = sMT[j];
-                const int thi = __double2hiint(mt.y);
-                {
-                    const double2 ab = ab0[j];
-                    const double dr = e.x - st.er[0], di = e.y - st.ei[0];
+            for (int j = 0; j < cnt; ++j) {
+                const double2 e = sg[j], pq = sg[32 + j], rb = sg[64 + j];
+#pragma unroll
+                for (int i = 0; i < FREE_NT; ++i) {
+                    const double dr = e.x - ter[i], di = e.y - tei[i];
                     const double den = fma(dr, dr, di * di);
-                    const double X = fma(st.ei[0], e.x, -(st.er[0] * e.y));
-                    const double Y = mt.x - st.m[0];
-                    const double val = fma(ab.y, Y, ab.x * X);
+                    double val = fma(tei[i], pq.x, rb.x);
+                    val = fma(-ter[i], pq.y, val);
+                    val = fma(-tm[i], rb.y, val);
                     const double r = bie_rcp3(den);
-                    const bool near = __double2hiint(den) < thi;
-                    flag |= near ? 1 : 0;
-                    if (!near) st.acc[0] = fma(val, r, st.acc[0]);
-                }
-                {
-                    const double2 ab = ab1[j];
-                    const double dr = e.x - st.er[1], di = e.y - st.ei[1];
-                    const double den = fma(dr, dr, di * di);
-                    const double X = fma(st.ei[1], e.x, -(st.er[1] * e.y));
-                    const double Y = mt.x - st.m[1];
-                    const double val = fma(ab.y, Y, ab.x * X);
-                    const double r = bie_rcp3(den);
-                    const bool near = __double2hiint(den) < thi;
-                    flag |= near ? 1 : 0;
-                    if (!near) st.acc[1] = fma(val, r, st.acc[1]);
-                }
-            }
-            if (__any_sync(thr_lane_any, flag)) {
-                if (flag) {
-                    const double2 d = free_near_fix(nt.DG, nt.XY, x, scale, cur, nthr, jb, jb + FREE_SB, c_lo + it * nthr,
-                                                    st.er[0], st.ei[0], st.er[1], st.ei[1], st.idx[0], st.idx[1],
-                                                    st.cls[0], st.cls[1]);
-                    st.acc[0] += d.x; st.acc[1] += d.y;
+                    if (!(__double2hiint(den) < thi[i])) acc[i] = fma(val, r, acc[i]);
                 }
             }
         }
-        if (it + 1 < ntile) free_store_src(nxt, tile0 + ((it + 1) & 1) * 4 * nthr, nthr, tm.tid);
-        team_sync(tm);
+        // the 16 warp sums, added in fixed order
+#pragma unroll
+        for (int i = 0; i < FREE_NT; ++i) wsum[warp * FREE_ROWS + lane + 32 * i] = acc[i];
+        __syncthreads();
+        if (threadIdx.x < FREE_ROWS) {
+            double s = 0.0;
+#pragma unroll
+            for (int w = 0; w < FREE_WARPS; ++w) s += wsum[w * FREE_ROWS + threadIdx.x];
+            fp.PB[(size_t)(b + c) * FREE_ROWS + threadIdx.x] = s;
+        }
+        __syncthreads();
+        u0 = ue;
+        ++b;
     }
 }
 
-// y_local[t - r0] = running sums + E_k term over the sources [c_lo, c_hi) that were processed.
-// All threads of the team must call; ends with a team_sync.
-__device__ __forceinline__ void free_end(FreeState& st, const NodeTable& nt, const CompTable& ct, int r0, int r1,
-                                         int c_lo, int c_hi, const double* __restrict__ x, double scale,
-                                         double* scratch, double* y_local, bool accumulate, const FreeTeam& tm)
+// ---- step 3 (after a grid barrier): y_local[t - r0] = scale * (partials + near entries - E_k term) ---------
+// xsrc: the vector of step 1 (global, complete).  All threads of the CTA must call; ends with __syncthreads.
+__device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable& ct, const FreePlan& fp, int r0, int r1,
+                                            const double* __restrict__ xsrc, double scale, double* scratch,
+                                            double* y_local)
 {
-    const int nthr = tm.nthr;
-    const int rows = r1 - r0;
-    double* gpart = scratch + 2 * 8 * nthr;  // [2][nthr]
-    double* csum = gpart + 2 * nthr;         // [ncomp]
-    // component sums of x over the processed range (fixed order: one warp per component, lanes strided)
-    {
-        const int lane = tm.tid & 31, warp = tm.tid >> 5;
-        for (int k = warp; k < ct.ncomp; k += nthr / 32) {
-            const int a = max(ct.off[k], c_lo), b = min(ct.off[k + 1], c_hi);
+    double* csum = scratch + FREE_STAGE_DOUBLES + FREE_WARPS * FREE_ROWS;  // [ncomp]
+    {   // component sums of x, for the components that own one of this CTA's rows; fixed order
+        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+        for (int k = warp; k < ct.ncomp; k += nwarp) {
             double s = 0.0;
-            for (int i = a + lane; i < b; i += 32) s += __ldcg(x + i);
+            if (ct.off[k] < r1 && ct.off[k + 1] > r0)
+                for (int i = ct.off[k] + lane; i < ct.off[k + 1]; i += 32) s += __ldcg(xsrc + i);
             s = bie_warp_sum(s);
-            if (lane == 0) csum[k] = s * scale;
+            if (lane == 0) csum[k] = s;
         }
     }
-#pragma unroll
-    for (int q = 0; q < 2; ++q) gpart[q * nthr + tm.tid] = st.acc[q];
-    team_sync(tm);
-    for (int loc = tm.tid; loc < rows; loc += nthr) {
-        const int q = loc / st.TG, sl = loc - q * st.TG;
+    __syncthreads();
+    const bool bad = (__ldcg(fp.near_overflow) != 0);
+    for (int t = r0 + threadIdx.x; t < r1; t += blockDim.x) {
+        int b, off;
+        if (t < fp.M0) { b = t / FREE_ROWS; off = t - b * FREE_ROWS; }
+        else { const int d = t - fp.M0; b = d / FREE_ROWS; off = d - b * FREE_ROWS; b += fp.NB0; }
+        const long long X0 = (long long)b * fp.UB, X1 = X0 + fp.UB;
+        int c_lo = (int)(((X0 + 1) * fp.Geff + fp.U - 1) / fp.U) - 1;
+        int c_hi = (int)((X1 * fp.Geff + fp.U - 1) / fp.U) - 1;
+        c_lo = max(c_lo, 0); c_hi = min(c_hi, fp.Geff - 1);
         double s = 0.0;
-        for (int g = 0; g < st.NG; ++g) s += gpart[q * nthr + g * st.TG + sl];
-        const int t = r0 + loc;
+        for (int c = c_lo; c <= c_hi; ++c) {
+            const long long a = max(free_slab_start(fp, c), X0), e = min(free_slab_start(fp, c + 1), X1);
+            if (a < e) s += __ldcg(fp.PB + (size_t)(b + c) * FREE_ROWS + off);
+        }
+        // near pairs: exact entries from the CSR near matrix
+        const int p0 = fp.near_ptr[8 * (size_t)t], p1 = fp.near_ptr[8 * (size_t)t + 8];
+        double sn = 0.0;
+        for (int p = p0; p < p1; ++p) sn = fma(fp.near_val[p], __ldcg(xsrc + fp.near_col[p]), sn);
+        s += sn;
         const int k = nt.COMP[t];
         s = fma(-nt.DG[t].y, csum[k], s);
-        y_local[loc] = accumulate ? y_local[loc] + s : s;
+        y_local[t - r0] = bad ? __longlong_as_double(0x7ff8000000000000LL) : s * scale;
     }
-    team_sync(tm);
-}
-
-// whole operator for a CTA (team = all threads): y_local[t - r0] = sum_s A[t][s] (scale x[s]), t in [r0, r1)
-__device__ __forceinline__ void bie_cta_matvec_free(const NodeTable& nt, const CompTable& ct, int r0, int r1,
-                                                    const double* __restrict__ x, double scale, double* scratch,
-                                                    double* y_local)
-{
-    FreeTeam tm;
-    tm.tid = threadIdx.x; tm.nthr = blockDim.x; tm.bar = 0;
-    FreeState st;
-    free_begin(st, nt, r0, r1, tm);
-    free_chunk(st, nt, 0, nt.n, x, scale, scratch, tm);
-    free_end(st, nt, ct, r0, r1, 0, nt.n, x, scale, scratch, y_local, false, tm);
+    __syncthreads();
 }

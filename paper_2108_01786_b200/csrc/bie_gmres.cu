@@ -45,27 +45,8 @@ struct GmresArgs {
     int VS;        // Krylov vectors 0..VS-1 keep this CTA's rows in shared memory; the others in V (global, L2)
     NodeTable nt;
     CompTable ct;
+    FreePlan fp;
 };
-
-// ---- grid barrier (cooperative launch guarantees co-residency) -------------------------------------
-__device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p)
-{
-    unsigned int v;
-    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void grid_barrier(unsigned int* ctr, unsigned int& target)
-{
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        target += gridDim.x;
-        __threadfence();
-        atomicAdd(ctr, 1u);
-        while (ld_acquire_u32(ctr) < target) { }
-        __threadfence();
-    }
-    __syncthreads();
-}
 
 // sum over the CTA; result to all threads.  red: shared, >= 33 doubles
 __device__ __forceinline__ double block_sum(double v, double* red)
@@ -94,10 +75,19 @@ __device__ __forceinline__ double warp_sum_partials(const double* p, int G)
 
 template <bool STREAM, bool XS, bool FREE>
 __device__ __forceinline__ void cta_apply(const GmresArgs& a, int r0, int r1, const double* xin, double scale,
-                                          double* xs, double* gpart, double* y_local)
+                                          double* xs, double* gpart, double* y_local, bool tables_ready,
+                                          unsigned int& target)
 {
     if (FREE) {
-        bie_cta_matvec_free(a.nt, a.ct, r0, r1, xin, scale, gpart, y_local);
+        // xin is complete in global memory; its per-source tables either were written by the row owners before
+        // the last grid barrier (tables_ready) or are written here
+        if (!tables_ready) {
+            free_write_tables(a.nt, a.fp, r0, r1, xin + r0);
+            grid_barrier(a.sync, target);
+        }
+        free_parts(a.nt, a.fp, gpart);
+        grid_barrier(a.sync, target);
+        free_gather(a.nt, a.ct, a.fp, r0, r1, xin, scale, gpart, y_local);
     } else if (XS) {
         const int n2 = a.n >> 1;
         for (int i = threadIdx.x; i < n2; i += blockDim.x) {
@@ -263,7 +253,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
             for (int r = threadIdx.x; r < rows; r += blockDim.x) w_local[r] = a.b[r0 + r];
             first = false;
         } else {
-            cta_apply<STREAM, XS, FREE>(a, r0, r1, a.x, 1.0, xs, gpart, y_local);
+            cta_apply<STREAM, XS, FREE>(a, r0, r1, a.x, 1.0, xs, gpart, y_local, false, target);
             for (int r = threadIdx.x; r < rows; r += blockDim.x) w_local[r] = a.b[r0 + r] - y_local[r];
         }
         __syncthreads();
@@ -273,6 +263,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
             p = fma(v, v, p);
             a.wbuf[r0 + r] = v;
         }
+        if (FREE) free_write_tables(a.nt, a.fp, r0, r1, w_local);
         p = block_sum(p, red);
         if (threadIdx.x == 0) part3[blockIdx.x] = p;
         grid_barrier(a.sync, target);
@@ -292,7 +283,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
         bool conv = false;
         for (int j = 0; j < m; ++j) {
             // a6: w = A v_j, with v_j = wbuf * inv
-            cta_apply<STREAM, XS, FREE>(a, r0, r1, a.wbuf, inv, xs, gpart, y_local);
+            cta_apply<STREAM, XS, FREE>(a, r0, r1, a.wbuf, inv, xs, gpart, y_local, true, target);
             for (int r = threadIdx.x; r < rows; r += blockDim.x) w_local[r] = y_local[r];
             __syncthreads();
             // a7: CGS2
@@ -304,6 +295,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
                 p = fma(v, v, p);
                 a.wbuf[r0 + r] = v;
             }
+            if (FREE) free_write_tables(a.nt, a.fp, r0, r1, w_local);
             p = block_sum(p, red);
             if (threadIdx.x == 0) part3[blockIdx.x] = p;
             grid_barrier(a.sync, target);
@@ -369,7 +361,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
     // ---- a10: outputs; true residual ||b - A x|| / ||b|| (reported only) -----------------------------
     double relres = 0.0;
     if (a.relres_out && bn != 0.0) {
-        cta_apply<STREAM, XS, FREE>(a, r0, r1, a.x, 1.0, xs, gpart, y_local);
+        cta_apply<STREAM, XS, FREE>(a, r0, r1, a.x, 1.0, xs, gpart, y_local, false, target);
         p = 0.0;
         for (int r = threadIdx.x; r < rows; r += blockDim.x) {
             const double v = a.b[r0 + r] - y_local[r];
@@ -404,7 +396,6 @@ static int gmres_plan(int n, int restart, int sm_count, int max_smem, int l2_byt
 {
     const int m = restart;
     pl->rows_per_cta = (n + sm_count - 1) / sm_count;
-    if (free_op && pl->rows_per_cta < 64) pl->rows_per_cta = 64 < n ? 64 : n;  // keep the lanes busy
     pl->G = (n + pl->rows_per_cta - 1) / pl->rows_per_cta;
     pl->chunk = gemv_chunk(pl->rows_per_cta, n, GM_THREADS / 32);
     pl->nld = (n + 1) & ~1;
@@ -424,7 +415,6 @@ static int gmres_plan(int n, int restart, int sm_count, int max_smem, int l2_byt
     pl->VS = pl->smem < cap ? (int)((cap - pl->smem) / (sizeof(double) * rows2)) : 0;
     if (pl->VS > m + 1) pl->VS = m + 1;
     pl->smem += sizeof(double) * (size_t)pl->VS * rows2;
-    if (free_op && pl->rows_per_cta > 2 * FREE_THREADS) return BIE_ERR_ARG;
     pl->stream = !free_op && (double)n * (double)lda * 8.0 > 0.6 * (double)l2_bytes;
     size_t o = 0;
     pl->offV = o; o += al256(sizeof(double) * (size_t)(m + 1) * pl->nld);
@@ -493,8 +483,14 @@ int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, const do
     a.yv = (double*)(base + pl.offY);
     a.sync = ctx->sync_buf;
     a.nld = pl.nld; a.rows_per_cta = pl.rows_per_cta; a.chunk = pl.chunk; a.VS = pl.VS;
-    if (free_op) { a.nt = bie_node_table(ctx); a.ct = ctx->comps; }
-    else { memset(&a.nt, 0, sizeof(a.nt)); memset(&a.ct, 0, sizeof(a.ct)); }
+    memset(&a.nt, 0, sizeof(a.nt)); memset(&a.ct, 0, sizeof(a.ct)); memset(&a.fp, 0, sizeof(a.fp));
+    if (free_op) {
+        a.nt = bie_node_table(ctx); a.ct = ctx->comps;
+        rc = bie_ensure_near(ctx, st);
+        if (rc != BIE_OK) return rc;
+        rc = bie_free_plan(ctx, pl.G, &a.fp);
+        if (rc != BIE_OK) return rc;
+    }
     BIE_CUDA(cudaMemsetAsync(ctx->sync_buf, 0, sizeof(unsigned int), st));
     if (free_op) return launch_gmres<false, false, true>(a, pl, st);
     if (pl.stream) return pl.xs ? launch_gmres<true, true, false>(a, pl, st) : launch_gmres<true, false, false>(a, pl, st);

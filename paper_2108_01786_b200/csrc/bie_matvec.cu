@@ -65,20 +65,24 @@ int bie_launch_matvec(bie_ctx* ctx, int n, const double* A, int64_t lda, const d
 }
 
 // ---------------------------------------------------------------------------------------------------
-// matrix-free
+// matrix-free: one cooperative launch, three phases separated by grid barriers (bie_free.cuh)
 // ---------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(FREE_THREADS, 1)
-bie_matvec_free_kernel(NodeTable nt, CompTable ct, int rows_per_cta, const double* __restrict__ x,
-                       double* __restrict__ y)
+bie_matvec_free_kernel(NodeTable nt, CompTable ct, FreePlan fp, int rows_per_cta, const double* __restrict__ x,
+                       double* __restrict__ y, unsigned int* sync)
 {
     extern __shared__ __align__(16) double smem[];
     const int n = nt.n;
-    const int r0 = blockIdx.x * rows_per_cta;
+    const int r0 = min(blockIdx.x * rows_per_cta, n);
     const int r1 = min(r0 + rows_per_cta, n);
-    if (r0 >= r1) return;
-    double* y_local = smem;
-    double* scratch = y_local + ((rows_per_cta + 1) & ~1);
-    bie_cta_matvec_free(nt, ct, r0, r1, x, 1.0, scratch, y_local);
+    double* scratch = smem;
+    double* y_local = scratch + free_scratch_doubles(FREE_THREADS);
+    unsigned int target = 0;
+    free_write_tables(nt, fp, r0, r1, x + r0);
+    grid_barrier(sync, target);
+    free_parts(nt, fp, scratch);
+    grid_barrier(sync, target);
+    free_gather(nt, ct, fp, r0, r1, x, 1.0, scratch, y_local);
     for (int r = threadIdx.x; r < r1 - r0; r += blockDim.x) y[r0 + r] = y_local[r];
 }
 
@@ -87,14 +91,24 @@ int bie_launch_matvec_free(bie_ctx* ctx, const double* x, double* y, cudaStream_
     if (!ctx || !x || !y) return BIE_ERR_NULL;
     if (!ctx->have_geom) return BIE_ERR_GEOMETRY;
     if ((((uintptr_t)x) | ((uintptr_t)y)) & 15u) return BIE_ERR_LAYOUT;
+    if (!ctx->coop_ok || ctx->sm_count > 256) return BIE_ERR_DEVICE;
     const int n = ctx->n;
     const int G = ctx->sm_count;
     const int rows_per_cta = (n + G - 1) / G;
-    const size_t smem = sizeof(double) * (((rows_per_cta + 1) & ~1) + free_scratch_doubles(FREE_THREADS));
+    const size_t smem = sizeof(double) * (size_t)(free_scratch_doubles(FREE_THREADS) + ((rows_per_cta + 1) & ~1));
     if (smem > (size_t)ctx->max_smem_optin) return BIE_ERR_ARG;
+    FreePlan fp;
+    int rc = bie_ensure_near(ctx, st);
+    if (rc != BIE_OK) return rc;
+    rc = bie_free_plan(ctx, G, &fp);
+    if (rc != BIE_OK) return rc;
     BIE_CUDA(cudaFuncSetAttribute(bie_matvec_free_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    const int grid = (n + rows_per_cta - 1) / rows_per_cta;
-    bie_matvec_free_kernel<<<grid, FREE_THREADS, smem, st>>>(bie_node_table(ctx), ctx->comps, rows_per_cta, x, y);
-    BIE_CUDA(cudaGetLastError());
+    BIE_CUDA(cudaMemsetAsync(ctx->sync_buf, 0, sizeof(unsigned int), st));
+    NodeTable nt = bie_node_table(ctx);
+    CompTable ct = ctx->comps;
+    int rpc = rows_per_cta;
+    unsigned int* sync = ctx->sync_buf;
+    void* params[] = {(void*)&nt, (void*)&ct, (void*)&fp, (void*)&rpc, (void*)&x, (void*)&y, (void*)&sync};
+    BIE_CUDA(cudaLaunchCooperativeKernel((const void*)bie_matvec_free_kernel, dim3(G), dim3(FREE_THREADS), params, smem, st));
     return BIE_OK;
 }

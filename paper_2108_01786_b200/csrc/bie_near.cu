@@ -1,0 +1,127 @@
+// bie_near.cu -- near-pair correction of the matrix-free operator (bie_free.cuh), built once per geometry.
+//
+// The fast pair arithmetic (one exponential per node, bie_common.cuh) cancels for |w| = |zeta_s - zeta_t| -> 0.
+// A pair is NEAR when den = |E_s - E_t|^2 < taubar M_t, i.e. |e^{iw} - 1|^2 < taubar ~ |w|^2, with
+// taubar = max_s clamp(BIE_NEAR_C |q_s|) one number per geometry (<= 1e-2, so that |w| < 0.11 and the Laurent
+// series of bie_cot_half_near is exact to rounding).  The pair loop of the operator leaves near pairs out by
+// predication; their exact matrix entries -- Laurent series of cot for s != t, the analytic diagonal limit
+// K_jj(a,a) = Im{zeta''/(2 zeta')} with the -+1/2 of Eq. (3.10) for s == t, both WITHOUT the
+// rank-one -E_k of PAPER.md:L324, which the operator applies through component sums -- are stored here as a
+// sparse matrix in CSR form (a handful of entries per row: the neighbours on the same curve and whatever
+// other curve comes closer than sqrt(taubar)), and added as  y_t += sum_k val[k] x[col[k]]  when the operator
+// gathers its partial sums.  Classification uses exactly the expression of the pair loop, so both agree bit
+// for bit.  Three launches per geometry: count, exclusive scan, fill (the first and last scan all n^2 pairs
+// with 4 FP64 instructions each).
+#include "bie_common.cuh"
+
+#define NEAR_THREADS 128
+#define NEAR_SEG 8          // source segments per target row: (row, segment) lists are contiguous in CSR order
+#define NEAR_TILE 512
+
+template <bool FILL>
+__global__ void __launch_bounds__(NEAR_THREADS)
+bie_near_kernel(NodeTable nt, const double* __restrict__ taubar, int* __restrict__ cnt /* [n][NEAR_SEG] counts or offsets */,
+                int* __restrict__ col, double* __restrict__ val, int cap, int* __restrict__ overflow)
+{
+    __shared__ double2 sE[NEAR_TILE];
+    const int n = nt.n;
+    const int t = blockIdx.x * NEAR_THREADS + threadIdx.x;
+    const int seg = blockIdx.y;
+    const int per = (nt.npad / NEAR_SEG + 1) & ~1;
+    const int s_lo = seg * per, s_hi = min(s_lo + per, n);
+    const int tt = min(t, n - 1);
+    const double2 te = nt.E[tt];
+    const int thi = __double2hiint(taubar[0] * nt.MT[tt].x);
+    const bool tgt0 = (nt.COMP[tt] == 0);
+    int k = 0, base = 0;
+    if (FILL && t < n) base = cnt[(size_t)t * NEAR_SEG + seg];
+    for (int s0 = s_lo; s0 < s_hi; s0 += NEAR_TILE) {
+        __syncthreads();
+        for (int i = threadIdx.x; i < NEAR_TILE; i += NEAR_THREADS)
+            sE[i] = (s0 + i < s_hi) ? nt.E[s0 + i] : make_double2(0.0, 0.0);  // E = 0 is never near (den = M_t)
+        __syncthreads();
+        const int m = min(NEAR_TILE, s_hi - s0);
+#pragma unroll 4
+        for (int j = 0; j < m; ++j) {
+            const double2 e = sE[j];
+            const double dr = e.x - te.x, di = e.y - te.y;
+            const double den = fma(dr, dr, di * di);
+            if (__double2hiint(den) < thi) {
+                if (FILL && t < n) {
+                    const int s = s0 + j;
+                    const int p = base + k;
+                    if (p < cap) {
+                        double v;
+                        if (s == t) {
+                            const double2 dg = nt.DG[t];
+                            v = dg.x + dg.y;   // complete diagonal entry without its -E_k part
+                        } else {
+                            const double2 zs = nt.XY[s], zt = nt.XY[t], q = nt.Q[s];
+                            double cr, ci;
+                            bie_cot_half_near(zs.x - zt.x, zs.y - zt.y, &cr, &ci);
+                            const bool src0 = (nt.COMP[s] == 0);
+                            double al, be;   // block coefficients of Eq. (3.10) (bie_common.cuh)
+                            if (src0 == tgt0) { al = -2.0 * q.y; be = q.x; }        // Im c
+                            else if (tgt0)    { al = -2.0 * q.x; be = -q.y; }       // Re c   (G_0j)
+                            else              { al = 2.0 * q.x;  be = q.y; }        // -Re c  (-G_k0)
+                            v = fma(be, ci, -0.5 * al * cr);   // cot = (-2X + iY)/den
+                        }
+                        col[p] = s;
+                        val[p] = v;
+                    } else {
+                        *overflow = 1;
+                    }
+                }
+                ++k;
+            }
+        }
+    }
+    if (!FILL && t < n) cnt[(size_t)t * NEAR_SEG + seg] = k;
+}
+
+// exclusive prefix sum of N ints in place, total to a[N]; one CTA
+__global__ void __launch_bounds__(1024) bie_near_scan_kernel(int* __restrict__ a, int N)
+{
+    __shared__ int sums[1024];
+    const int per = (N + 1023) / 1024;
+    const int lo = min(threadIdx.x * per, N), hi = min(lo + per, N);
+    int s = 0;
+    for (int i = lo; i < hi; ++i) s += a[i];
+    sums[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = 1; o < 1024; o <<= 1) {   // Hillis-Steele inclusive scan
+        const int v = (threadIdx.x >= o) ? sums[threadIdx.x - o] : 0;
+        __syncthreads();
+        sums[threadIdx.x] += v;
+        __syncthreads();
+    }
+    int run = sums[threadIdx.x] - s;
+    for (int i = lo; i < hi; ++i) {
+        const int v = a[i];
+        a[i] = run;
+        run += v;
+    }
+    if (threadIdx.x == 1023) a[N] = sums[1023];
+}
+
+size_t bie_near_cap(int npad) { return (size_t)BIE_NEAR_PER_NODE * (size_t)npad; }
+
+// builds the CSR near matrix of the ctx's current geometry if it is not there yet (lazy: the dense path never
+// needs it)
+int bie_ensure_near(bie_ctx* ctx, cudaStream_t st)
+{
+    if (!ctx->have_geom) return BIE_ERR_GEOMETRY;
+    if (ctx->near_valid) return BIE_OK;
+    const NodeTable nt = bie_node_table(ctx);
+    const int n = ctx->n;
+    const int cap = (int)bie_near_cap(nt.npad);
+    dim3 grid((n + NEAR_THREADS - 1) / NEAR_THREADS, NEAR_SEG);
+    BIE_CUDA(cudaMemsetAsync(ctx->near_overflow, 0, sizeof(int), st));
+    bie_near_kernel<false><<<grid, NEAR_THREADS, 0, st>>>(nt, ctx->taubar, ctx->near_ptr, nullptr, nullptr, cap, ctx->near_overflow);
+    bie_near_scan_kernel<<<1, 1024, 0, st>>>(ctx->near_ptr, n * NEAR_SEG);
+    bie_near_kernel<true><<<grid, NEAR_THREADS, 0, st>>>(nt, ctx->taubar, ctx->near_ptr, ctx->near_col, ctx->near_val, cap,
+                                                        ctx->near_overflow);
+    BIE_CUDA(cudaGetLastError());
+    ctx->near_valid = 1;
+    return BIE_OK;
+}

@@ -7,6 +7,7 @@
 // limit K_jj(a,a) = Im{zeta''/(2 zeta')} with the -+1/2 of Eq. (3.10) and the
 // -1/M_m of E_m.
 #include "bie_common.cuh"
+#include "bie_free.cuh"
 
 struct PrepArgs {
     CompTable comps;
@@ -16,7 +17,8 @@ struct PrepArgs {
 __global__ void __launch_bounds__(256)
 bie_prepare_nodes_kernel(PrepArgs pa, int n, int npad, int variant,
                          const double2* __restrict__ zeta, const double2* __restrict__ dzeta,
-                         const double2* __restrict__ d2zeta, double2* __restrict__ buf, int* __restrict__ comp)
+                         const double2* __restrict__ d2zeta, double2* __restrict__ buf, int* __restrict__ comp,
+                         double2* __restrict__ T, double* __restrict__ taubar)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= npad) return;
@@ -28,6 +30,8 @@ bie_prepare_nodes_kernel(PrepArgs pa, int n, int npad, int variant,
     if (i >= n) {  // padding: zero weight, never near (thr = 0), never stored to A
         E[i] = make_double2(0.0, 0.0); MT[i] = make_double2(0.0, 0.0); Q[i] = make_double2(0.0, 0.0);
         XY[i] = make_double2(0.0, 1.0e3); DG[i] = make_double2(0.0, 0.0); comp[i] = -1;
+        // padding sources of the matrix-free tables: zero weight for every vector
+        for (int a = 0; a < 4; ++a) T[(size_t)a * npad + i] = make_double2(0.0, 0.0);
         return;
     }
     int k = 0;
@@ -44,6 +48,8 @@ bie_prepare_nodes_kernel(PrepArgs pa, int n, int npad, int variant,
     double tau = BIE_NEAR_C * sqrt(qr * qr + qi * qi);
     tau = fmin(fmax(tau, BIE_NEAR_TAU_MIN), BIE_NEAR_TAU_MAX);
     MT[i] = make_double2(m * m, tau * m * m);
+    // taubar = max_s tau_s (positive doubles order like their bit patterns)
+    atomicMax(reinterpret_cast<unsigned long long*>(taubar), (unsigned long long)__double_as_longlong(tau));
     XY[i] = z;
     // Im{ zeta'' / (2 zeta' M) }
     const double den = dz.x * dz.x + dz.y * dz.y;
@@ -94,9 +100,18 @@ int bie_prepare_nodes(bie_ctx* ctx, int ncomp, const int32_t* counts, const int3
         // grow the ctx's node storage (the only allocation outside bie_create; O(n) bytes)
         if (ctx->node_buf) cudaFree(ctx->node_buf);
         if (ctx->comp_buf) cudaFree(ctx->comp_buf);
-        ctx->node_buf = nullptr; ctx->comp_buf = nullptr; ctx->cap = 0;
+        if (ctx->free_buf) cudaFree(ctx->free_buf);
+        if (ctx->near_ptr) cudaFree(ctx->near_ptr);
+        if (ctx->near_col) cudaFree(ctx->near_col);
+        if (ctx->near_val) cudaFree(ctx->near_val);
+        ctx->node_buf = nullptr; ctx->comp_buf = nullptr; ctx->free_buf = nullptr; ctx->cap = 0;
+        ctx->near_ptr = nullptr; ctx->near_col = nullptr; ctx->near_val = nullptr;
         BIE_CUDA(cudaMalloc((void**)&ctx->node_buf, sizeof(double) * BIE_NODE_ARRAYS * (size_t)npad));
         BIE_CUDA(cudaMalloc((void**)&ctx->comp_buf, sizeof(int) * (size_t)npad));
+        BIE_CUDA(cudaMalloc((void**)&ctx->free_buf, sizeof(double) * bie_free_buf_doubles(npad)));
+        BIE_CUDA(cudaMalloc((void**)&ctx->near_ptr, sizeof(int) * (8 * (size_t)npad + 1)));
+        BIE_CUDA(cudaMalloc((void**)&ctx->near_col, sizeof(int) * bie_near_cap(npad)));
+        BIE_CUDA(cudaMalloc((void**)&ctx->near_val, sizeof(double) * bie_near_cap(npad)));
         ctx->cap = npad;
     }
     PrepArgs pa;
@@ -112,9 +127,36 @@ int bie_prepare_nodes(bie_ctx* ctx, int ncomp, const int32_t* counts, const int3
     for (int c = 0; c < ncomp; ++c) { ctx->counts[c] = counts[c]; ctx->kinds[c] = kinds[c]; }
     ctx->comps = pa.comps;
     ctx->have_geom = 1;
+    ctx->near_valid = 0;
+    BIE_CUDA(cudaMemsetAsync(ctx->taubar, 0, sizeof(double), st));
     bie_prepare_nodes_kernel<<<(npad + 255) / 256, 256, 0, st>>>(
         pa, (int)n, npad, variant, (const double2*)zeta, (const double2*)dzeta, (const double2*)d2zeta,
-        (double2*)ctx->node_buf, ctx->comp_buf);
+        (double2*)ctx->node_buf, ctx->comp_buf, (double2*)ctx->free_buf, ctx->taubar);
     BIE_CUDA(cudaGetLastError());
+    return BIE_OK;
+}
+
+// ---- matrix-free operator: storage and work split (bie_free.cuh) ------------------------------------------
+size_t bie_free_buf_doubles(int cap)
+{
+    // tables [4][cap] double2, then partial sums for (row blocks + CTAs) parts of FREE_ROWS rows
+    return 8 * (size_t)cap + ((size_t)cap / FREE_ROWS + 2 + 256) * FREE_ROWS;
+}
+
+int bie_free_plan(const bie_ctx* ctx, int grid, FreePlan* fp)
+{
+    if (!ctx->have_geom || grid < 1 || grid > 256) return BIE_ERR_GEOMETRY;
+    const int n = ctx->n, npad = bie_npad(n);
+    fp->M0 = ctx->counts[0];
+    fp->NB0 = (fp->M0 + FREE_ROWS - 1) / FREE_ROWS;
+    fp->NB = fp->NB0 + (n - fp->M0 + FREE_ROWS - 1) / FREE_ROWS;
+    fp->UB = npad / 2;
+    fp->U = (long long)fp->NB * fp->UB;
+    fp->Geff = (long long)grid < fp->U ? grid : (int)fp->U;
+    fp->T = reinterpret_cast<double2*>(ctx->free_buf);
+    fp->PB = ctx->free_buf + 8 * (size_t)npad;
+    fp->taubar = ctx->taubar;
+    fp->near_ptr = ctx->near_ptr; fp->near_col = ctx->near_col; fp->near_val = ctx->near_val;
+    fp->near_overflow = ctx->near_overflow;
     return BIE_OK;
 }
