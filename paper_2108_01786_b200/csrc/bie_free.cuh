@@ -184,14 +184,24 @@ __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable
                                             double* y_local)
 {
     double* csum = scratch + FREE_STAGE_DOUBLES + FREE_WARPS * FREE_ROWS;  // [ncomp]
-    {   // component sums of x, for the components that own one of this CTA's rows; fixed order
+    double* wred = scratch + FREE_STAGE_DOUBLES;   // [nwarp] (the warp-sum area is free again)
+    {   // sum of x over each OBSTACLE component (em != 0) that owns one of this CTA's rows: all warps share the
+        // component, lanes strided, warp sums added in fixed order -- every CTA gets the same bits
         const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
-        for (int k = warp; k < ct.ncomp; k += nwarp) {
+        for (int k = 0; k < ct.ncomp; ++k) {
+            if (!(ct.off[k] < r1 && ct.off[k + 1] > r0)) continue;      // CTA-uniform
+            if (nt.DG[ct.off[k]].y == 0.0) { if (threadIdx.x == 0) csum[k] = 0.0; continue; }
             double s = 0.0;
-            if (ct.off[k] < r1 && ct.off[k + 1] > r0)
-                for (int i = ct.off[k] + lane; i < ct.off[k + 1]; i += 32) s += __ldcg(xsrc + i);
+            for (int i = ct.off[k] + threadIdx.x; i < ct.off[k + 1]; i += blockDim.x) s += __ldcg(xsrc + i);
             s = bie_warp_sum(s);
-            if (lane == 0) csum[k] = s;
+            if (lane == 0) wred[warp] = s;
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                double tsum = 0.0;
+                for (int w = 0; w < nwarp; ++w) tsum += wred[w];
+                csum[k] = tsum;
+            }
+            __syncthreads();
         }
     }
     __syncthreads();

@@ -73,6 +73,16 @@ __device__ __forceinline__ double warp_sum_partials(const double* p, int G)
     return bie_warp_sum(s);
 }
 
+#ifdef BIE_PHASE_TIMING
+#include <cstdio>
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define PT_DECL unsigned long long pt_t0 = gtime(), pt_acc[8] = {0,0,0,0,0,0,0,0};
+#define PT(i) { const unsigned long long pt_t1 = gtime(); pt_acc[i] += pt_t1 - pt_t0; pt_t0 = pt_t1; }
+#else
+#define PT_DECL
+#define PT(i)
+#endif
+
 template <bool STREAM, bool XS, bool FREE>
 __device__ __forceinline__ void cta_apply(const GmresArgs& a, int r0, int r1, const double* xin, double scale,
                                           double* xs, double* gpart, double* y_local, bool tables_ready,
@@ -281,14 +291,28 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
         // ---- Arnoldi steps ------------------------------------------------------------------------
         int k = 0;
         bool conv = false;
+        PT_DECL
         for (int j = 0; j < m; ++j) {
+            PT(7)
             // a6: w = A v_j, with v_j = wbuf * inv
+#ifdef BIE_PHASE_TIMING
+            if (FREE) {
+                free_parts(a.nt, a.fp, gpart);
+                PT(0)
+                grid_barrier(a.sync, target);
+                PT(1)
+                free_gather(a.nt, a.ct, a.fp, r0, r1, a.wbuf, inv, gpart, y_local);
+                PT(2)
+            } else
+#endif
             cta_apply<STREAM, XS, FREE>(a, r0, r1, a.wbuf, inv, xs, gpart, y_local, true, target);
             for (int r = threadIdx.x; r < rows; r += blockDim.x) w_local[r] = y_local[r];
             __syncthreads();
+            PT(3)
             // a7: CGS2
             cgs_pass(a, B, rows, j, part1, w_local, hloc, hcol, false, red2, target);
             cgs_pass(a, B, rows, j, part2, w_local, hloc, hcol, true, red2, target);
+            PT(4)
             p = 0.0;
             for (int r = threadIdx.x; r < rows; r += blockDim.x) {
                 const double v = w_local[r];
@@ -300,6 +324,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
             if (threadIdx.x == 0) part3[blockIdx.x] = p;
             grid_barrier(a.sync, target);
             const double hn = sqrt(warp_sum_partials(part3, G));
+            PT(5)
             inv = (hn != 0.0) ? 1.0 / hn : 0.0;
             {
                 double* vn = (j + 1 < B.VS) ? B.Vs + (size_t)(j + 1) * rows2 : B.Vg + (size_t)(j + 1) * a.nld;
@@ -331,8 +356,15 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
             conv = (fabs(g[j + 1]) <= thresh) || (hn == 0.0);
             if (hn == 0.0 && !(fabs(g[j + 1]) <= thresh)) status = 2;
             __syncthreads();
+            PT(6)
             if (conv || iters >= a.max_iters) break;
         }
+#ifdef BIE_PHASE_TIMING
+        if (threadIdx.x == 0 && (blockIdx.x == 0 || blockIdx.x == 77 || blockIdx.x == 147))
+            printf("cta %d k=%d us/iter: parts %.1f bar %.1f gather %.1f copy %.1f cgs2 %.1f norm %.1f givens %.1f\n", blockIdx.x, k,
+                   pt_acc[0] * 1e-3 / k, pt_acc[1] * 1e-3 / k, pt_acc[2] * 1e-3 / k, pt_acc[3] * 1e-3 / k, pt_acc[4] * 1e-3 / k,
+                   pt_acc[5] * 1e-3 / k, pt_acc[6] * 1e-3 / k);
+#endif
         // ---- a9: y = R^{-1} g (CTA 0), x += V y ---------------------------------------------------
         if (blockIdx.x == 0) {
             __syncthreads();
