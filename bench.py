@@ -35,7 +35,8 @@ if ROOT not in sys.path:
 
 METRIC = "matrix build Gentries/s and GMRES solve ms (FP64); % of FP64 / HBM roofline"
 UNIT = "Gentries/s"
-FP64_INSTR_PER_ENTRY = 13      # FP64-pipe instructions per matrix entry (SASS count)
+FP64_INSTR_PER_ENTRY = 13      # FP64-pipe instructions per stored matrix entry (SASS count)
+FP64_INSTR_PER_PAIR_FREE = 11  # matrix-free operator: FP64-pipe instructions per pair incl. the accumulation (bie_free.cuh)
 HBM_FALLBACK_GBS = 6650.0      # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 # dram__bytes_read.sum + dram__bytes_write.sum of the GMRES kernel, one launch, from the committed ncu capture
 # (profiles/r01_ncu_full_gmres_cfg5.md); None for workloads that were not captured
@@ -49,10 +50,17 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--matrix-free", action="store_true", help="solve with the matrix-free operator (no dense build)")
+    ap.add_argument("--operator", default="auto", choices=["auto", "dense", "free"],
+                    help="dense: bie_build + GMRES on the stored matrix; free: matrix-free GMRES (entries recomputed on the "
+                         "fly, no matrix); auto (default): both are timed during warm-up and the faster one is the timed step")
+    ap.add_argument("--matrix-free", action="store_true", help="same as --operator free")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="budget of the oracle sample")
-    return ap.parse_args()
+    a = ap.parse_args()
+    if a.matrix_free:
+        a.operator = "free"
+    a.matrix_free = (a.operator == "free")
+    return a
 
 
 def hbm_peak():
@@ -198,7 +206,7 @@ def workload_config(P, args, iters):
     g = P.geometry
     return {"workload": f"BASELINE.json configs[{P.config - 1}]: {P.name}", "n": int(g.n),
             "counts": [int(c) for c in g.counts], "restart": int(P.restart), "tol": P.tol,
-            "operator": "matrix-free" if args.matrix_free else "dense",
+            "operator": ("matrix-free" if args.matrix_free else "dense") + (" (chosen by measurement)" if args.operator == "auto" else ""),
             "matrix_bytes": 0 if args.matrix_free else int(8 * g.n * g.n),
             "l2_policy": "inputs larger than L2 (matrix 17x L2); no flush needed" if 8 * g.n * g.n > 2.5e8
             else "matrix fits L2 (126 MB): L2-resident GEMV, reported as such",
@@ -236,22 +244,46 @@ def main():
     ctx = bie.Context(local)
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
     z, dz, d2z, b = dev(g.zeta), dev(g.dzeta), dev(g.d2zeta), dev(P.rhs[0])
-    A = None if args.matrix_free else torch.empty((n, n + (n & 1)), dtype=torch.float64, device="cuda")
+    # the stored matrix is also needed for the stand-alone dense GEMV timing, whichever operator the step uses
+    A = torch.empty((n, n + (n & 1)), dtype=torch.float64, device="cuda")
     x = torch.empty(n + (n & 1), dtype=torch.float64, device="cuda")[:n]
     ws = torch.empty(ctx.bie_gmres_workspace_bytes(n, P.restart), dtype=torch.uint8, device="cuda")
     oi = torch.zeros(2, dtype=torch.int32, device="cuda")
     of = torch.zeros(1, dtype=torch.float64, device="cuda")
 
-    def step(ev=None):
+    def step_dense(ev=None):
         if ev: ev[0].record()
-        if A is None:
-            ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z)          # 1 launch
-        else:
-            ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A)              # 2 launches: node prep + tile kernel
+        ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A)                  # 2 launches: node prep + tile kernel
         if ev: ev[1].record()
         ctx.bie_gmres(A, b, x, P.tol, P.restart, P.max_iters, ws, oi, of)  # 1 cooperative launch
         if ev: ev[2].record()
-    launches_per_step = 2 if A is None else 3
+
+    def step_free(ev=None):
+        if ev: ev[0].record()
+        ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z)              # 1 launch: node prep
+        if ev: ev[1].record()
+        ctx.bie_gmres(None, b, x, P.tol, P.restart, P.max_iters, ws, oi, of)  # near matrix (3) + 1 cooperative launch
+        if ev: ev[2].record()
+
+    def time_steps(fn, k):
+        torch.cuda.synchronize()
+        a_, c_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a_.record()
+        for _ in range(k):
+            fn()
+        c_.record(); torch.cuda.synchronize()
+        return a_.elapsed_time(c_) / k
+
+    # operator choice by measurement (north_star: "matrix-free fused rebuild+matvec variant chosen by measurement")
+    choice_ms = {}
+    if args.operator == "auto":
+        step_dense(); step_free()
+        choice_ms = {"dense": time_steps(step_dense, 2), "free": time_steps(step_free, 2)}
+        ops = torch.tensor([choice_ms["dense"], choice_ms["free"]], dtype=torch.float64)
+        use_free = bool(max_over_ranks(float(ops[1])) < max_over_ranks(float(ops[0])))
+        args.matrix_free = use_free
+    step = step_free if args.matrix_free else step_dense
+    launches_per_step = 5 if args.matrix_free else 3
 
     for _ in range(max(args.warmup, 3)):
         step()
@@ -303,12 +335,14 @@ def main():
     xv = torch.from_numpy(np.random.default_rng(1).standard_normal(n)).cuda()
     yv = torch.empty(n + (n & 1), dtype=torch.float64, device="cuda")[:n]
     matvec = {}
-    if A is not None:
-        mv_ms = time_call(lambda: ctx.bie_matvec(A, xv, yv), 50)
-        matvec["dense"] = {"ms": mv_ms, "gbs": 8.0 * n * n / (mv_ms * 1e-3) / 1e9}
+    prep_ms = build_ms
+    if args.matrix_free:   # the dense build is not part of this step: time it on its own (stand-alone calls, warm)
+        build_ms = time_call(lambda: ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A), 20)
+    mv_ms = time_call(lambda: ctx.bie_matvec(A, xv, yv), 50)
+    matvec["dense"] = {"ms": mv_ms, "gbs": 8.0 * n * n / (mv_ms * 1e-3) / 1e9, "hbm_frac": 8.0 * n * n / (mv_ms * 1e-3) / 1e9 / hbm_peak()[0]}
     mf_ms = time_call(lambda: ctx.bie_matvec_free(xv, yv), 20)
     matvec["matrix_free"] = {"ms": mf_ms, "gentries_per_s": n * n / (mf_ms * 1e-3) / 1e9,
-                             "fp64_frac": n * n * FP64_INSTR_PER_ENTRY / (mf_ms * 1e-3) / dfma_per_s}
+                             "fp64_frac": n * n * FP64_INSTR_PER_PAIR_FREE / (mf_ms * 1e-3) / dfma_per_s}
 
     # ---- end to end through bie_solve_host, pinned host buffers ---------------------------------------------
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
@@ -337,9 +371,10 @@ def main():
     peak, peak_src = hbm_peak()
     ng = n_gemv(iters, P.restart)
     if args.matrix_free:
-        roof = {"bound": "alu", "kernel": "bie_gmres_kernel<matrix-free>",
-                "achieved": ng * n * n * FP64_INSTR_PER_ENTRY / (gmres_ms * 1e-3) / 1e12, "peak": dfma_per_s / 1e12,
-                "unit": "T FP64 instr/s", "traffic": None,
+        roof = {"bound": "alu", "kernel": "bie_gmres_kernel<matrix-free> (persistent; pair loops dominate)",
+                "achieved": ng * n * n * FP64_INSTR_PER_PAIR_FREE / (gmres_ms * 1e-3) / 1e12, "peak": dfma_per_s / 1e12,
+                "unit": "T FP64 instr/s", "traffic": None, "fp64_instr_per_pair": FP64_INSTR_PER_PAIR_FREE,
+                "pairs_per_launch": ng * n * n, "operator_applications_per_launch": ng,
                 "peak_source": "bie_probe_dfma in this run (nominal 148 SM x 64 lanes x 1.965 GHz = 18.6)"}
     else:
         roof = {"bound": "hbm", "kernel": "bie_gmres_kernel (persistent; GEMV phases dominate)",
@@ -348,7 +383,7 @@ def main():
                 "algorithmic_bytes_per_launch": ng * 8 * n * n, "gemvs_per_launch": ng}
     roof["frac"] = roof["achieved"] / roof["peak"]
     roof_build = None
-    if not args.matrix_free:
+    if True:
         ach = n * n * FP64_INSTR_PER_ENTRY / (build_ms * 1e-3)
         roof_build = {"bound": "alu", "kernel": "bie_build_kernel (+ node prep)", "achieved": ach / 1e12,
                       "peak": dfma_per_s / 1e12, "unit": "T FP64 instr/s", "frac": ach / dfma_per_s,
@@ -359,13 +394,17 @@ def main():
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic", "config": workload_config(P, args, iters),
-            "build": None if args.matrix_free else {"gentries_per_s": n * n / (build_ms * 1e-3) / 1e9, "ms": build_ms},
+            "build": {"gentries_per_s": n * n / (build_ms * 1e-3) / 1e9, "ms": build_ms,
+                      "in_step": not args.matrix_free,
+                      "note": "stand-alone bie_build calls outside the timed region (the matrix-free step stores no matrix; "
+                              "its geometry preparation took %.4f ms per step)" % prep_ms if args.matrix_free else "inside the timed step"},
             "gmres": {"ms": gmres_ms, "iters": iters, "relres_true": relres, "us_per_iter": gmres_ms * 1e3 / max(iters, 1)},
             "e2e": {"value": world * n * n / e2e_s / 1e9, "unit": UNIT, "ms_per_step": e2e_s * 1e3,
                     "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "api": "bie_solve_host", "iters": e_it},
             "gpu_launches": launches_per_step * K,
             "roofline": roof, "roofline_build": roof_build, "matvec": matvec, "clocks": clocks,
-            "fp64_probe_tflops": 2 * dfma_per_s / 1e12}
+            "fp64_probe_tflops": 2 * dfma_per_s / 1e12,
+            "operator_choice_ms_per_step": choice_ms or None}
     if not args.no_cpu_baseline:
         est, desc, cores, parts = oracle_sample(P, iters, args.cpu_seconds)
         line["cpu_baseline"] = {"value": n * n / est / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
