@@ -50,16 +50,16 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--operator", default="auto", choices=["auto", "dense", "free"],
+    ap.add_argument("--operator", default="auto", choices=["auto", "dense", "free", "hybrid"],
                     help="dense: bie_build + GMRES on the stored matrix; free: matrix-free GMRES (entries recomputed on the "
-                         "fly, no matrix); auto (default): both are timed during warm-up and the faster one is the timed step")
+                         "fly, no matrix); hybrid: a slab of bie_hybrid_cols(n) columns stored and streamed while the other "
+                         "sources are recomputed; auto (default): all are timed during warm-up and the fastest is the timed step")
     ap.add_argument("--matrix-free", action="store_true", help="same as --operator free")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="budget of the oracle sample")
     a = ap.parse_args()
     if a.matrix_free:
         a.operator = "free"
-    a.matrix_free = (a.operator == "free")
     return a
 
 
@@ -180,6 +180,7 @@ def run_reference(args):
     from paper_2108_01786_b200 import inputs
     P = inputs.make_config(args.config)
     n = P.n
+    args.op, args.stored_cols = "dense", n     # the oracle stores the matrix
     iters_nominal = {1: 18, 2: 33, 3: 74, 4: 127, 5: 158}[args.config]  # the oracle's own counts (tests)
     per = max(2.0, min(args.cpu_seconds, 120.0 / max(1, args.steps + args.warmup)))
     for _ in range(args.warmup):
@@ -206,8 +207,9 @@ def workload_config(P, args, iters):
     g = P.geometry
     return {"workload": f"BASELINE.json configs[{P.config - 1}]: {P.name}", "n": int(g.n),
             "counts": [int(c) for c in g.counts], "restart": int(P.restart), "tol": P.tol,
-            "operator": ("matrix-free" if args.matrix_free else "dense") + (" (chosen by measurement)" if args.operator == "auto" else ""),
-            "matrix_bytes": 0 if args.matrix_free else int(8 * g.n * g.n),
+            "operator": {"dense": "dense", "free": "matrix-free", "hybrid": "hybrid (stored slab + recomputed sources)"}[args.op]
+                        + (" (chosen by measurement)" if args.operator == "auto" else ""),
+            "matrix_bytes": int(8 * g.n * args.stored_cols), "stored_columns": int(args.stored_cols),
             "l2_policy": "inputs larger than L2 (matrix 17x L2); no flush needed" if 8 * g.n * g.n > 2.5e8
             else "matrix fits L2 (126 MB): L2-resident GEMV, reported as such",
             "replicas": int(args.gpus)}
@@ -265,6 +267,15 @@ def main():
         ctx.bie_gmres(None, b, x, P.tol, P.restart, P.max_iters, ws, oi, of)  # near matrix (3) + 1 cooperative launch
         if ev: ev[2].record()
 
+    nd = ctx.bie_hybrid_cols(n)
+
+    def step_hybrid(ev=None):
+        if ev: ev[0].record()
+        ctx.bie_build_cols(g.counts, g.kinds, z, dz, d2z, nd, A)        # 2 launches: node prep + slab tiles
+        if ev: ev[1].record()
+        ctx.bie_gmres_hybrid(A, nd, b, x, P.tol, P.restart, P.max_iters, ws, oi, of)  # near matrix (3) + 1 cooperative launch
+        if ev: ev[2].record()
+
     def time_steps(fn, k):
         torch.cuda.synchronize()
         a_, c_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -275,15 +286,24 @@ def main():
         return a_.elapsed_time(c_) / k
 
     # operator choice by measurement (north_star: "matrix-free fused rebuild+matvec variant chosen by measurement")
+    steps = {"dense": step_dense, "free": step_free}
+    if nd > 0:
+        steps["hybrid"] = step_hybrid
     choice_ms = {}
-    if args.operator == "auto":
-        step_dense(); step_free()
-        choice_ms = {"dense": time_steps(step_dense, 2), "free": time_steps(step_free, 2)}
-        ops = torch.tensor([choice_ms["dense"], choice_ms["free"]], dtype=torch.float64)
-        use_free = bool(max_over_ranks(float(ops[1])) < max_over_ranks(float(ops[0])))
-        args.matrix_free = use_free
-    step = step_free if args.matrix_free else step_dense
-    launches_per_step = 5 if args.matrix_free else 3
+    op = args.operator
+    if op == "hybrid" and nd == 0:
+        raise SystemExit("bench: n is too small for the hybrid operator")
+    if op == "auto":
+        for name, fn in steps.items():
+            fn()
+            choice_ms[name] = max_over_ranks(time_steps(fn, 2))
+        op = min(choice_ms, key=choice_ms.get)
+    step = steps[op]
+    args.op = op
+    args.stored_cols = {"dense": n, "free": 0, "hybrid": nd}[op]
+    args.matrix_free = (op == "free")
+    launches_per_step = {"dense": 3, "free": 5, "hybrid": 6}[op]
+    solve_mode = {"dense": 0, "free": 1, "hybrid": 2}[op]
 
     for _ in range(max(args.warmup, 3)):
         step()
@@ -336,7 +356,7 @@ def main():
     yv = torch.empty(n + (n & 1), dtype=torch.float64, device="cuda")[:n]
     matvec = {}
     prep_ms = build_ms
-    if args.matrix_free:   # the dense build is not part of this step: time it on its own (stand-alone calls, warm)
+    if args.op != "dense":   # the full dense build is not part of this step: time it on its own (stand-alone calls, warm)
         build_ms = time_call(lambda: ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A), 20)
     mv_ms = time_call(lambda: ctx.bie_matvec(A, xv, yv), 50)
     matvec["dense"] = {"ms": mv_ms, "gbs": 8.0 * n * n / (mv_ms * 1e-3) / 1e9, "hbm_frac": 8.0 * n * n / (mv_ms * 1e-3) / 1e9 / hbm_peak()[0]}
@@ -350,14 +370,14 @@ def main():
     hx = torch.empty(n, dtype=torch.float64).pin_memory()
     del A
     torch.cuda.empty_cache()
-    sws = torch.empty(ctx.bie_solve_workspace_bytes(n, P.restart, args.matrix_free), dtype=torch.uint8, device="cuda")
+    sws = torch.empty(ctx.bie_solve_workspace_bytes(n, P.restart, solve_mode), dtype=torch.uint8, device="cuda")
     for _ in range(2):
-        ctx.bie_solve_host(g.counts, g.kinds, hz, hdz, hd2z, hb, hx, P.tol, P.restart, P.max_iters, sws, args.matrix_free)
+        ctx.bie_solve_host(g.counts, g.kinds, hz, hdz, hd2z, hb, hx, P.tol, P.restart, P.max_iters, sws, solve_mode)
     barrier()
     t0 = time.perf_counter()
     for _ in range(K):
         e_it, e_rr, e_st = ctx.bie_solve_host(g.counts, g.kinds, hz, hdz, hd2z, hb, hx, P.tol, P.restart, P.max_iters,
-                                              sws, args.matrix_free)
+                                              sws, solve_mode)
     torch.cuda.synchronize()
     e2e_s = max_over_ranks((time.perf_counter() - t0) / K)
     h2d = 3 * 16 * n + 8 * n
@@ -370,12 +390,19 @@ def main():
     # ---- rooflines -------------------------------------------------------------------------------------------
     peak, peak_src = hbm_peak()
     ng = n_gemv(iters, P.restart)
-    if args.matrix_free:
-        roof = {"bound": "alu", "kernel": "bie_gmres_kernel<matrix-free> (persistent; pair loops dominate)",
-                "achieved": ng * n * n * FP64_INSTR_PER_PAIR_FREE / (gmres_ms * 1e-3) / 1e12, "peak": dfma_per_s / 1e12,
+    if args.op != "dense":
+        sc = args.stored_cols          # 0 (matrix-free) or the slab width (hybrid)
+        pairs = ng * n * (n - sc)
+        instr = pairs * FP64_INSTR_PER_PAIR_FREE + ng * n * sc          # + one DFMA per streamed slab entry
+        roof = {"bound": "alu", "kernel": "bie_gmres_kernel<%s> (persistent; pair loops dominate)" % args.op,
+                "achieved": instr / (gmres_ms * 1e-3) / 1e12, "peak": dfma_per_s / 1e12,
                 "unit": "T FP64 instr/s", "traffic": None, "fp64_instr_per_pair": FP64_INSTR_PER_PAIR_FREE,
-                "pairs_per_launch": ng * n * n, "operator_applications_per_launch": ng,
+                "pairs_per_launch": pairs, "operator_applications_per_launch": ng,
                 "peak_source": "bie_probe_dfma in this run (nominal 148 SM x 64 lanes x 1.965 GHz = 18.6)"}
+        if sc:   # the slab is streamed from HBM by the other warps at the same time
+            gbs = ng * 8.0 * n * sc / (gmres_ms * 1e-3) / 1e9
+            roof["hbm_concurrent"] = {"achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
+                                      "algorithmic_bytes_per_launch": ng * 8 * n * sc, "peak_source": peak_src}
     else:
         roof = {"bound": "hbm", "kernel": "bie_gmres_kernel (persistent; GEMV phases dominate)",
                 "achieved": ng * 8.0 * n * n / (gmres_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
@@ -395,9 +422,11 @@ def main():
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic", "config": workload_config(P, args, iters),
             "build": {"gentries_per_s": n * n / (build_ms * 1e-3) / 1e9, "ms": build_ms,
-                      "in_step": not args.matrix_free,
-                      "note": "stand-alone bie_build calls outside the timed region (the matrix-free step stores no matrix; "
-                              "its geometry preparation took %.4f ms per step)" % prep_ms if args.matrix_free else "inside the timed step"},
+                      "in_step": args.op == "dense",
+                      "note": "inside the timed step" if args.op == "dense" else
+                              "full bie_build, stand-alone calls outside the timed region; inside the step the %s operator "
+                              "spent %.4f ms on its own preparation (node tables%s)"
+                              % (args.op, prep_ms, " + slab of %d columns" % args.stored_cols if args.stored_cols else "")},
             "gmres": {"ms": gmres_ms, "iters": iters, "relres_true": relres, "us_per_iter": gmres_ms * 1e3 / max(iters, 1)},
             "e2e": {"value": world * n * n / e2e_s / 1e9, "unit": UNIT, "ms_per_step": e2e_s * 1e3,
                     "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "api": "bie_solve_host", "iters": e_it},

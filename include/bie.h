@@ -53,6 +53,11 @@ extern "C" {
 #define BIE_KIND_BOTTOM 1
 #define BIE_KIND_OBSTACLE 2
 
+/* operator of bie_solve_host (its `matrix_free` argument) */
+#define BIE_OP_DENSE 0  /* whole matrix stored, GEMV from HBM                                            */
+#define BIE_OP_FREE 1   /* nothing stored, entries recomputed on the fly                                 */
+#define BIE_OP_HYBRID 2 /* first bie_hybrid_cols(n) columns stored, the other sources recomputed         */
+
 /* bie_build `variant` */
 #define BIE_VARIANT_A 0 /* Eq. (3.16): 1/2 I + K_mm - E_m on obstacle diagonal blocks  */
 #define BIE_VARIANT_B 1 /* the uncorrected operator B of Eq. (3.10), for invariants    */
@@ -102,6 +107,20 @@ int bie_build_update(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32
                      const double* zeta, const double* dzeta, const double* d2zeta,
                      int variant, double* A, int64_t lda, void* stream);
 
+/* Hybrid operator (north_star: "matrix-free fused rebuild+matvec variant chosen by measurement").  The dense
+ * GEMV is HBM-bound and leaves the FP64 pipe idle, the matrix-free operator is FP64-bound and leaves HBM idle;
+ * the hybrid operator does both at once: the first ncols columns of the matrix are stored (a slab, n x ncols,
+ * row-major with leading dimension lda >= ncols, lda even) and streamed by some warps of every CTA while the
+ * other warps recompute the entries of the remaining sources from the node tables.
+ * bie_build_cols: as bie_build, but only the columns [0, ncols) of every row are written (1 <= ncols <= n).
+ * bie_hybrid_cols: the slab width the library recommends for n on a B200 (even; 0 = too small, use bie_gmres).
+ * bie_set_hybrid_free_warps: tuning knob, warps per CTA (of 16) on the pair loops (default 8). */
+int bie_build_cols(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds,
+                   const double* zeta, const double* dzeta, const double* d2zeta,
+                   int variant, int ncols, double* A, int64_t lda, void* stream);
+int bie_hybrid_cols(bie_ctx* ctx, int n);
+int bie_set_hybrid_free_warps(bie_ctx* ctx, int free_warps);
+
 /* Prepares the node tables of a geometry in the ctx without writing a matrix (for the matrix-free
  * operator).  Same geometry arguments as bie_build. */
 int bie_set_geometry(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds,
@@ -142,13 +161,21 @@ int bie_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, const double* r
               double* x, int32_t* iters_out, double* relres_out, int32_t* status_out, double* res_hist,
               void* workspace, size_t workspace_bytes, void* stream);
 
+/* Same solve with the hybrid operator: A is the slab written by bie_build_cols for the ctx's current geometry,
+ * ncols_dense its width (even, 2 <= ncols_dense < n), lda >= ncols_dense.  Everything else as bie_gmres. */
+int bie_gmres_hybrid(bie_ctx* ctx, int n, const double* A, int64_t lda, int ncols_dense, const double* rhs,
+                     double tol, int restart, int max_iters,
+                     double* x, int32_t* iters_out, double* relres_out, int32_t* status_out, double* res_hist,
+                     void* workspace, size_t workspace_bytes, void* stream);
+
 /* ---------------------------------------------------------------------------------------------------
  * End-to-end call with HOST buffers (what bench.py's "e2e" times): copies the node data and rhs to the
  * device, builds A, solves, copies x / iters / relres back and SYNCHRONISES the stream before returning.
  * zeta, dzeta, d2zeta, rhs, x: host (pinned memory makes the copies asynchronous).  dev_workspace: dev, at
  * least bie_solve_workspace_bytes(n, restart) bytes (holds node data, A with lda = n rounded up to even,
- * rhs, x and the GMRES workspace).  matrix_free != 0 skips the dense matrix and solves with the
- * matrix-free operator.  Returns BIE_OK, BIE_MAX_ITERS or an error.
+ * rhs, x and the GMRES workspace).  matrix_free selects the operator: BIE_OP_DENSE (0), BIE_OP_FREE (1: no
+ * matrix is stored) or BIE_OP_HYBRID (2: a slab of bie_hybrid_cols(n) columns is stored).  Returns BIE_OK,
+ * BIE_MAX_ITERS or an error.
  */
 size_t bie_solve_workspace_bytes(int n, int restart, int matrix_free);
 int bie_solve_host(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds,

@@ -22,9 +22,11 @@ _lib: Optional[ctypes.CDLL] = None
 # the symbols include/bie.h declares
 EXPORTS = ("bie_create", "bie_destroy", "bie_strerror", "bie_device_info", "bie_build", "bie_build_update",
            "bie_set_geometry", "bie_matvec", "bie_matvec_free", "bie_gmres_workspace_bytes", "bie_gmres",
-           "bie_solve_workspace_bytes", "bie_solve_host", "bie_probe_dfma")
+           "bie_solve_workspace_bytes", "bie_solve_host", "bie_probe_dfma", "bie_build_cols", "bie_hybrid_cols",
+           "bie_set_hybrid_free_warps", "bie_gmres_hybrid")
 
 BIE_OK, BIE_MAX_ITERS = 0, 1
+OP_DENSE, OP_FREE, OP_HYBRID = 0, 1, 2
 VARIANT_A, VARIANT_B = 0, 1
 
 
@@ -72,6 +74,14 @@ def lib() -> ctypes.CDLL:
         L.bie_solve_host.restype = i32
         L.bie_solve_host.argtypes = [vp, i32, ip, ip, vp, vp, vp, vp, dbl, i32, i32, i32, vp, ip,
                                      ctypes.POINTER(dbl), vp, sz, vp]
+        L.bie_build_cols.restype = i32
+        L.bie_build_cols.argtypes = geo + [i32, vp, i64, vp]
+        L.bie_hybrid_cols.restype = i32
+        L.bie_hybrid_cols.argtypes = [vp, i32]
+        L.bie_set_hybrid_free_warps.restype = i32
+        L.bie_set_hybrid_free_warps.argtypes = [vp, i32]
+        L.bie_gmres_hybrid.restype = i32
+        L.bie_gmres_hybrid.argtypes = [vp, i32, vp, i64, i32, vp, dbl, i32, i32, vp, vp, vp, vp, vp, vp, sz, vp]
         L.bie_probe_dfma.restype = i32
         L.bie_probe_dfma.argtypes = [vp, i64, vp, ctypes.POINTER(i64), vp]
         _lib = L
@@ -160,6 +170,22 @@ class Context:
         _check(lib().bie_build_update(*args, A.data_ptr(), lda, _stream()), "bie_build_update")
         return A
 
+    def bie_build_cols(self, counts, kinds, zeta, dzeta, d2zeta, ncols: int, A, variant: int = VARIANT_A,
+                       lda: Optional[int] = None):
+        """A (CUDA float64, n x lda row-major, lda >= ncols) <- columns [0, ncols) of the matrix of Eq. (3.16):
+        the stored slab of the hybrid operator."""
+        n, args, keep = self._geo(counts, kinds, zeta, dzeta, d2zeta, variant)
+        lda = int(lda if lda is not None else A.stride(0))
+        _dev_f64(A, (n - 1) * lda + int(ncols))
+        _check(lib().bie_build_cols(*args, int(ncols), A.data_ptr(), lda, _stream()), "bie_build_cols")
+        return A
+
+    def bie_hybrid_cols(self, n: int) -> int:
+        return int(lib().bie_hybrid_cols(self._h, int(n)))
+
+    def bie_set_hybrid_free_warps(self, free_warps: int):
+        _check(lib().bie_set_hybrid_free_warps(self._h, int(free_warps)), "bie_set_hybrid_free_warps")
+
     def bie_set_geometry(self, counts, kinds, zeta, dzeta, d2zeta, variant: int = VARIANT_A):
         n, args, keep = self._geo(counts, kinds, zeta, dzeta, d2zeta, variant)
         _check(lib().bie_set_geometry(*args, _stream()), "bie_set_geometry")
@@ -203,13 +229,30 @@ class Context:
                                workspace.data_ptr(), ws_bytes, _stream()), "bie_gmres")
         return x
 
+    def bie_gmres_hybrid(self, A, ncols_dense: int, rhs, x, tol: float, restart: int, max_iters: int, workspace,
+                         out_i32, out_f64, lda: Optional[int] = None, res_hist=None):
+        """Asynchronous.  A: the slab written by bie_build_cols (n x lda, lda >= ncols_dense).  Outputs as bie_gmres."""
+        import torch
+        n = rhs.numel()
+        lda = int(lda if lda is not None else A.stride(0))
+        pA = _dev_f64(A, (n - 1) * lda + int(ncols_dense))
+        assert out_i32.is_cuda and out_i32.dtype == torch.int32 and out_i32.numel() >= 2
+        assert workspace.is_cuda and workspace.is_contiguous()
+        ws_bytes = workspace.numel() * workspace.element_size()
+        _check(lib().bie_gmres_hybrid(self._h, n, pA, lda, int(ncols_dense), _dev_f64(rhs, n), float(tol), int(restart),
+                                      int(max_iters), _dev_f64(x, n), out_i32.data_ptr(), _dev_f64(out_f64, 1),
+                                      out_i32.data_ptr() + 4,
+                                      None if res_hist is None else _dev_f64(res_hist, int(max_iters) + 1),
+                                      workspace.data_ptr(), ws_bytes, _stream()), "bie_gmres_hybrid")
+        return x
+
     # ---- end to end with host buffers ------------------------------------------------------------------
     @staticmethod
-    def bie_solve_workspace_bytes(n: int, restart: int, matrix_free: bool = False) -> int:
-        return int(lib().bie_solve_workspace_bytes(int(n), int(restart), int(bool(matrix_free))))
+    def bie_solve_workspace_bytes(n: int, restart: int, matrix_free=False) -> int:
+        return int(lib().bie_solve_workspace_bytes(int(n), int(restart), int(matrix_free)))
 
     def bie_solve_host(self, counts, kinds, zeta, dzeta, d2zeta, rhs, x, tol: float, restart: int, max_iters: int,
-                       dev_workspace, matrix_free: bool = False) -> Tuple[int, float, int]:
+                       dev_workspace, matrix_free=False) -> Tuple[int, float, int]:
         """Host (ideally pinned) CPU tensors / numpy arrays in, density x (host) out; synchronises.
         -> (iters, relres_true, status)"""
         counts, kinds = _i32(counts), _i32(kinds)
@@ -226,7 +269,7 @@ class Context:
         ws_bytes = dev_workspace.numel() * dev_workspace.element_size()
         rc = lib().bie_solve_host(self._h, int(counts.size), _ip(counts), _ip(kinds), hp(zeta, 16 * n),
                                   hp(dzeta, 16 * n), hp(d2zeta, 16 * n), hp(rhs, 8 * n), float(tol), int(restart),
-                                  int(max_iters), int(bool(matrix_free)), hp(x, 8 * n), ctypes.byref(iters),
+                                  int(max_iters), int(matrix_free), hp(x, 8 * n), ctypes.byref(iters),
                                   ctypes.byref(relres), dev_workspace.data_ptr(), ws_bytes, _stream())
         _check(rc, "bie_solve_host", ok=(BIE_OK, BIE_MAX_ITERS))
         return int(iters.value), float(relres.value), int(rc)

@@ -27,6 +27,7 @@ int bie_create(bie_ctx** out, int device)
     c->node_buf = nullptr; c->comp_buf = nullptr; c->free_buf = nullptr; c->cap = 0; c->have_geom = 0; c->n = 0;
     c->sync_buf = nullptr; c->pinned_i = nullptr; c->pinned_d = nullptr;
     c->near_ptr = nullptr; c->near_col = nullptr; c->near_val = nullptr; c->near_valid = 0;
+    c->hybrid_free_warps = BIE_HYBRID_FREE_WARPS;
     c->taubar = nullptr; c->near_overflow = nullptr;
     if (cudaMalloc((void**)&c->sync_buf, 256) != cudaSuccess ||
         cudaMallocHost((void**)&c->pinned_i, 4 * sizeof(int32_t)) != cudaSuccess ||
@@ -100,7 +101,7 @@ int bie_build(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* kinds
     BIE_CUDA(cudaSetDevice(c->device));
     int rc = bie_prepare_nodes(c, ncomp, counts, kinds, zeta, dzeta, d2zeta, variant, (cudaStream_t)stream);
     if (rc != BIE_OK) return rc;
-    return bie_launch_build(c, A, lda, 0, (cudaStream_t)stream);
+    return bie_launch_build(c, A, lda, c->n, 0, (cudaStream_t)stream);
 }
 
 int bie_build_update(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* kinds, const double* zeta,
@@ -110,7 +111,36 @@ int bie_build_update(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t
     BIE_CUDA(cudaSetDevice(c->device));
     int rc = bie_prepare_nodes(c, ncomp, counts, kinds, zeta, dzeta, d2zeta, variant, (cudaStream_t)stream);
     if (rc != BIE_OK) return rc;
-    return bie_launch_build(c, A, lda, 1, (cudaStream_t)stream);
+    return bie_launch_build(c, A, lda, c->n, 1, (cudaStream_t)stream);
+}
+
+int bie_build_cols(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* kinds, const double* zeta,
+                   const double* dzeta, const double* d2zeta, int variant, int ncols, double* A, int64_t lda, void* stream)
+{
+    if (!c || !A) return BIE_ERR_NULL;
+    BIE_CUDA(cudaSetDevice(c->device));
+    int rc = bie_prepare_nodes(c, ncomp, counts, kinds, zeta, dzeta, d2zeta, variant, (cudaStream_t)stream);
+    if (rc != BIE_OK) return rc;
+    return bie_launch_build(c, A, lda, ncols, 0, (cudaStream_t)stream);
+}
+
+int bie_hybrid_cols(bie_ctx* c, int n)
+{
+    if (!c || n < 4) return 0;
+    // the slab's share of the columns that makes the streaming warps and the pair-loop warps finish together on a
+    // B200 (measured); a multiple of 64 so that slab rows are whole 512-byte lines
+    int nd = (int)((double)n * BIE_HYBRID_DENSE_FRACTION) & ~63;
+    if (nd < 64) nd = 0;            // too small to be worth two teams: use bie_gmres
+    if (nd > n - 2) nd = (n - 2) & ~1;
+    return nd;
+}
+
+int bie_set_hybrid_free_warps(bie_ctx* c, int free_warps)
+{
+    if (!c) return BIE_ERR_NULL;
+    if (free_warps < 1 || free_warps > 15) return BIE_ERR_ARG;
+    c->hybrid_free_warps = free_warps;
+    return BIE_OK;
 }
 
 int bie_matvec(bie_ctx* c, int n, const double* A, int64_t lda, const double* x, double* y, void* stream)
@@ -136,22 +166,48 @@ int bie_gmres(bie_ctx* c, int n, const double* A, int64_t lda, const double* rhs
 {
     if (!c) return BIE_ERR_NULL;
     BIE_CUDA(cudaSetDevice(c->device));
-    return bie_launch_gmres(c, n, A, lda, rhs, tol, restart, max_iters, x, iters_out, relres_out, status_out,
+    return bie_launch_gmres(c, n, A, lda, 0, rhs, tol, restart, max_iters, x, iters_out, relres_out, status_out,
                             res_hist, workspace, workspace_bytes, (cudaStream_t)stream);
+}
+
+int bie_gmres_hybrid(bie_ctx* c, int n, const double* A, int64_t lda, int ncols_dense, const double* rhs, double tol,
+                     int restart, int max_iters, double* x, int32_t* iters_out, double* relres_out,
+                     int32_t* status_out, double* res_hist, void* workspace, size_t workspace_bytes, void* stream)
+{
+    if (!c) return BIE_ERR_NULL;
+    if (!A) return BIE_ERR_NULL;
+    if (ncols_dense < 2) return BIE_ERR_ARG;
+    BIE_CUDA(cudaSetDevice(c->device));
+    return bie_launch_gmres(c, n, A, lda, ncols_dense, rhs, tol, restart, max_iters, x, iters_out, relres_out,
+                            status_out, res_hist, workspace, workspace_bytes, (cudaStream_t)stream);
 }
 
 // ---- end-to-end with host buffers --------------------------------------------------------------------
 static inline size_t up256(size_t b) { return (b + 255) & ~(size_t)255; }
 
+// slab width of bie_solve_host's stored part for an operator mode (0: n, 1: none, 2: bie_hybrid_cols)
+static int solve_cols(int n, int op)
+{
+    if (op == BIE_OP_FREE) return 0;
+    if (op == BIE_OP_HYBRID) {
+        int nd = (int)((double)n * BIE_HYBRID_DENSE_FRACTION) & ~63;
+        if (nd < 64) return 0;
+        if (nd > n - 2) nd = (n - 2) & ~1;
+        return nd;
+    }
+    return n;
+}
+
 size_t bie_solve_workspace_bytes(int n, int restart, int matrix_free)
 {
     if (n < 1 || restart < 1) return 0;
-    const size_t nld = ((size_t)n + 1) & ~(size_t)1;
+    const size_t nld = ((size_t)solve_cols(n, matrix_free) + 1) & ~(size_t)1;
+    const size_t nvec = ((size_t)n + 1) & ~(size_t)1;
     size_t o = 256;
     o += 3 * up256(16 * (size_t)n);          // zeta, dzeta, d2zeta
-    o += 2 * up256(8 * nld);                 // rhs, x
+    o += 2 * up256(8 * nvec);                // rhs, x
     o += up256(64);                          // iters, status, relres
-    if (!matrix_free) o += up256(8 * nld * (size_t)n);
+    if (nld) o += up256(8 * nld * (size_t)n);
     o += bie_gmres_ws_bytes(n, restart);
     return o;
 }
@@ -166,21 +222,23 @@ int bie_solve_host(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* 
     long long nn = 0;
     for (int k = 0; k < ncomp; ++k) { if (counts[k] < 1) return BIE_ERR_GEOMETRY; nn += counts[k]; }
     if (nn > (1 << 30)) return BIE_ERR_GEOMETRY;
-    if (restart < 1) return BIE_ERR_ARG;
+    if (restart < 1 || matrix_free < 0 || matrix_free > 2) return BIE_ERR_ARG;
     const int n = (int)nn;
     if (bie_solve_workspace_bytes(n, restart, matrix_free) > dev_workspace_bytes) return BIE_ERR_WORKSPACE;
+    const int ncols = solve_cols(n, matrix_free);      // stored columns: n (dense), 0 (matrix-free), slab (hybrid)
     BIE_CUDA(cudaSetDevice(c->device));
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t nld = ((size_t)n + 1) & ~(size_t)1;
+    const size_t nld = ((size_t)ncols + 1) & ~(size_t)1;
+    const size_t nvec = ((size_t)n + 1) & ~(size_t)1;
     char* p = (char*)(((uintptr_t)dev_workspace + 255) & ~(uintptr_t)255);
     double* dz0 = (double*)p; p += up256(16 * (size_t)n);
     double* dz1 = (double*)p; p += up256(16 * (size_t)n);
     double* dz2 = (double*)p; p += up256(16 * (size_t)n);
-    double* drhs = (double*)p; p += up256(8 * nld);
-    double* dx = (double*)p; p += up256(8 * nld);
+    double* drhs = (double*)p; p += up256(8 * nvec);
+    double* dx = (double*)p; p += up256(8 * nvec);
     int32_t* dint = (int32_t*)p; double* drel = (double*)(p + 16); p += up256(64);
     double* dA = nullptr;
-    if (!matrix_free) { dA = (double*)p; p += up256(8 * nld * (size_t)n); }
+    if (ncols) { dA = (double*)p; p += up256(8 * nld * (size_t)n); }
     void* gws = p;
     const size_t gws_bytes = bie_gmres_ws_bytes(n, restart);
     BIE_CUDA(cudaMemcpyAsync(dz0, zeta, 16 * (size_t)n, cudaMemcpyHostToDevice, st));
@@ -189,12 +247,12 @@ int bie_solve_host(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* 
     BIE_CUDA(cudaMemcpyAsync(drhs, rhs, 8 * (size_t)n, cudaMemcpyHostToDevice, st));
     int rc = bie_prepare_nodes(c, ncomp, counts, kinds, dz0, dz1, dz2, BIE_VARIANT_A, st);
     if (rc != BIE_OK) return rc;
-    if (!matrix_free) {
-        rc = bie_launch_build(c, dA, (int64_t)nld, 0, st);
+    if (ncols) {
+        rc = bie_launch_build(c, dA, (int64_t)nld, ncols, 0, st);
         if (rc != BIE_OK) return rc;
     }
-    rc = bie_launch_gmres(c, n, dA, (int64_t)nld, drhs, tol, restart, max_iters, dx, dint, drel, dint + 1, nullptr, gws,
-                          gws_bytes, st);
+    rc = bie_launch_gmres(c, n, dA, (int64_t)nld, ncols < n ? ncols : 0, drhs, tol, restart, max_iters, dx, dint, drel,
+                          dint + 1, nullptr, gws, gws_bytes, st);
     if (rc != BIE_OK) return rc;
     BIE_CUDA(cudaMemcpyAsync(x, dx, 8 * (size_t)n, cudaMemcpyDeviceToHost, st));
     BIE_CUDA(cudaMemcpyAsync(c->pinned_i, dint, 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, st));

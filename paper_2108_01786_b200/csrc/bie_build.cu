@@ -53,7 +53,7 @@ static __device__ __noinline__ double bie_entry_near(const double2* __restrict__
 }
 
 __global__ void __launch_bounds__(BUILD_THREADS)
-bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long lda, int T, int only0)
+bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long lda, int T, int only0, int ncols)
 {
     extern __shared__ __align__(16) double2 sm[];  // [T] E_t then [T] (M_t, -)
     const int n = nt.n;
@@ -81,8 +81,8 @@ bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long l
         scomp[c] = nt.COMP[s0 + c];
     }
     __syncthreads();
-    const bool full = (s0 + 1 < n);
-    const bool part = (s0 < n);
+    const bool full = (s0 + 1 < ncols);   // ncols = n, or the width of the hybrid operator's slab
+    const bool part = (s0 < ncols);
     for (int k = 0; k < ct.ncomp; ++k) {
         const int a = max(t0, ct.off[k]), b = min(t1, ct.off[k + 1]);
         if (a >= b) continue;
@@ -115,7 +115,7 @@ bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long l
                         const double2 te = sE[t - t0];
 #pragma unroll
                         for (int c = 0; c < BUILD_COLS; ++c) {
-                            if (s0 + c >= n) continue;
+                            if (s0 + c >= ncols) continue;
                             const double dr = src[c].er - te.x, di = src[c].ei - te.y;
                             const double den = fma(dr, dr, di * di);
                             if (__double2hiint(den) < src[c].thi)
@@ -128,20 +128,22 @@ bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long l
     }
 }
 
-int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int only_comp0, cudaStream_t st)
+// ncols: the first ncols columns of every row are written (ncols = n: the whole matrix)
+int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int ncols, int only_comp0, cudaStream_t st)
 {
     if (!ctx || !A) return BIE_ERR_NULL;
     if (!ctx->have_geom) return BIE_ERR_GEOMETRY;
     const int n = ctx->n;
-    if (lda < n || (lda & 1) || (((uintptr_t)A) & 15u)) return BIE_ERR_LAYOUT;
+    if (ncols < 1 || ncols > n) return BIE_ERR_ARG;
+    if (lda < ncols || (lda & 1) || (((uintptr_t)A) & 15u)) return BIE_ERR_LAYOUT;
     const NodeTable nt = bie_node_table(ctx);
-    const int gx = nt.npad / BUILD_TILE_W;
+    const int gx = (ncols + BUILD_TILE_W - 1) / BUILD_TILE_W;
     // rows per CTA: 128 when that still gives every SM several CTAs, else smaller
     int T = 128;
     while (T > 8 && (long long)gx * ((n + T - 1) / T) < 4LL * ctx->sm_count) T >>= 1;
     dim3 grid(gx, (n + T - 1) / T);
     bie_build_kernel<<<grid, BUILD_THREADS, (sizeof(double2) + sizeof(double)) * T + 16, st>>>(nt, ctx->comps, A, (long long)lda, T,
-                                                                                            only_comp0);
+                                                                                            only_comp0, ncols);
     BIE_CUDA(cudaGetLastError());
     return BIE_OK;
 }

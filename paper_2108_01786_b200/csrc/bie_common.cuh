@@ -23,6 +23,8 @@
 #define BIE_NEAR_C 0.25               // tau_s = BIE_NEAR_C |q_s|  (fast-path entry error <= ~1e-14)
 #define BIE_NEAR_TAU_MIN 1.0e-9
 #define BIE_NEAR_TAU_MAX 1.0e-2       // |w| < 0.1: Laurent truncation 2|w/2|^9/93555 < 1e-16
+#define BIE_HYBRID_FREE_WARPS 8        // hybrid operator: warps of a CTA on the pair loops (of 16)
+#define BIE_HYBRID_DENSE_FRACTION 0.42 // hybrid operator: share of the columns kept as a stored slab
 #define BIE_NEAR_PER_NODE 48          // capacity of the CSR near matrix of the matrix-free operator, entries per node
 
 // Node table, arrays of double2 of length npad.
@@ -60,6 +62,7 @@ struct bie_ctx {
     double* near_val;        // [BIE_NEAR_PER_NODE cap]
     int* near_overflow;      // device flag: the near matrix did not fit (the operator then returns NaN)
     int near_valid;          // near matrix built for the current geometry
+    int hybrid_free_warps;   // hybrid operator: warps per CTA on the pair loops (the other 16 - this stream the slab)
     unsigned int* sync_buf;  // grid-barrier counter
     int cap;
     // current geometry (host copies)
@@ -87,7 +90,7 @@ NodeTable bie_node_table(const bie_ctx* ctx);
 struct FreePlan;
 // doubles of ctx->free_buf for a node capacity `cap`; work split of the matrix-free operator over `grid` CTAs
 size_t bie_free_buf_doubles(int cap);
-int bie_free_plan(const bie_ctx* ctx, int grid, FreePlan* fp);
+int bie_free_plan(const bie_ctx* ctx, int grid, int s_off, FreePlan* fp);
 size_t bie_near_cap(int npad);
 int bie_ensure_near(bie_ctx* ctx, cudaStream_t st);
 
@@ -95,10 +98,10 @@ int bie_ensure_near(bie_ctx* ctx, cudaStream_t st);
 int bie_prepare_nodes(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds,
                       const double* zeta, const double* dzeta, const double* d2zeta, int variant,
                       cudaStream_t st);
-int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int only_comp0, cudaStream_t st);
+int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int ncols, int only_comp0, cudaStream_t st);
 int bie_launch_matvec(bie_ctx* ctx, int n, const double* A, int64_t lda, const double* x, double* y, cudaStream_t st);
 int bie_launch_matvec_free(bie_ctx* ctx, const double* x, double* y, cudaStream_t st);
-int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, const double* rhs, double tol,
+int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, int nd, const double* rhs, double tol,
                      int restart, int max_iters, double* x, int32_t* iters_out, double* relres_out,
                      int32_t* status_out, double* res_hist, void* ws, size_t ws_bytes, cudaStream_t st);
 size_t bie_gmres_ws_bytes(int n, int restart);
@@ -161,6 +164,30 @@ __device__ __forceinline__ void grid_barrier(unsigned int* ctr, unsigned int& ta
         __threadfence();
     }
     __syncthreads();
+}
+
+// a team = a contiguous group of warps of one CTA with its own named barrier (the whole CTA: barrier 0)
+struct Team {
+    int tid, nthr;     // thread index within the team, threads of the team (multiple of 32)
+    int warp, nwarp;   // warp index within the team, warps of the team
+    int bar;           // named barrier id
+};
+__device__ __forceinline__ void team_sync(const Team& t)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(t.bar), "r"(t.nthr) : "memory");
+}
+__device__ __forceinline__ Team cta_team()
+{
+    Team t;
+    t.tid = threadIdx.x; t.nthr = blockDim.x; t.warp = threadIdx.x >> 5; t.nwarp = blockDim.x >> 5; t.bar = 0;
+    return t;
+}
+// warps [w0, w0 + nw) of the CTA as a team using barrier `bar` (1..15); call only from those warps
+__device__ __forceinline__ Team sub_team(int w0, int nw, int bar)
+{
+    Team t;
+    t.tid = threadIdx.x - 32 * w0; t.nthr = 32 * nw; t.warp = (threadIdx.x >> 5) - w0; t.nwarp = nw; t.bar = bar;
+    return t;
 }
 
 __device__ __forceinline__ double bie_warp_sum(double v) {

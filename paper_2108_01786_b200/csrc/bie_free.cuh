@@ -39,9 +39,10 @@
 struct FreePlan {
     int M0;          // rows of class 0 = nodes of component 0
     int NB0, NB;     // row blocks of class 0, all row blocks
-    int UB;          // units (of 2 sources) per row block = npad / 2
+    int UB;          // units (of 2 sources) per row block = (npad - s_off) / 2
     long long U;     // NB * UB
     int Geff;        // CTAs that take a slab (<= gridDim.x)
+    int s_off;       // first source of the operator (0; the hybrid operator reads the sources below it from its slab)
     double2* T;      // [4][npad]: (P,Q) class 0, (R,B) class 0, (P,Q) class 1, (R,B) class 1
     double* PB;      // [(NB + Geff)][FREE_ROWS] partial sums, part id = row block + CTA
     const double* taubar;     // device scalar: near threshold relative to M_t (bie_near.cu)
@@ -95,10 +96,10 @@ __device__ __forceinline__ void free_write_tables(const NodeTable& nt, const Fre
 }
 
 // ---- step 2: this CTA's slab of the (row block x source) list -> partial sums in fp.PB --------------------
-// scratch: shared, free_scratch_doubles() doubles, 16-byte aligned.  All threads of the CTA must call.
-__device__ __forceinline__ void free_parts(const NodeTable& nt, const FreePlan& fp, double* scratch)
+// scratch: shared, free_scratch_doubles() doubles, 16-byte aligned.  All threads of the team must call.
+__device__ __forceinline__ void free_parts(const NodeTable& nt, const FreePlan& fp, double* scratch, const Team& team)
 {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int lane = team.tid & 31, warp = team.warp;
     const int c = blockIdx.x;
     if (c >= fp.Geff) return;
     double2* stage = reinterpret_cast<double2*>(scratch) + warp * (2 * 3 * 32);  // [2][3][32] double2 of this warp
@@ -111,7 +112,7 @@ __device__ __forceinline__ void free_parts(const NodeTable& nt, const FreePlan& 
     while (u0 < u1) {
         const long long ub = (long long)b * fp.UB;
         const long long ue = min(u1, ub + fp.UB);
-        const int sa = 2 * (int)(u0 - ub), sb = 2 * (int)(ue - ub);  // sources [sa, sb) of row block b
+        const int sa = fp.s_off + 2 * (int)(u0 - ub), sb = fp.s_off + 2 * (int)(ue - ub);  // sources [sa, sb) of row block b
         const int cls = b < fp.NB0 ? 0 : 1;
         const int row0 = free_block_row0(fp, b);
         const int rows = free_block_rows(fp, b, nt.n);
@@ -127,8 +128,8 @@ __device__ __forceinline__ void free_parts(const NodeTable& nt, const FreePlan& 
         }
         // this warp's share of the sources, in units of 2
         const int units = (sb - sa) >> 1;
-        const int wa = sa + 2 * (int)((long long)units * warp / FREE_WARPS);
-        const int wb = sa + 2 * (int)((long long)units * (warp + 1) / FREE_WARPS);
+        const int wa = sa + 2 * (int)((long long)units * warp / team.nwarp);
+        const int wb = sa + 2 * (int)((long long)units * (warp + 1) / team.nwarp);
         const double2* TE = nt.E;
         const double2* TPQ = fp.T + (size_t)(2 * cls) * np;
         const double2* TRB = fp.T + (size_t)(2 * cls + 1) * np;
@@ -161,17 +162,16 @@ __device__ __forceinline__ void free_parts(const NodeTable& nt, const FreePlan& 
                 }
             }
         }
-        // the 16 warp sums, added in fixed order
+        // the warp sums, added in fixed order
 #pragma unroll
         for (int i = 0; i < FREE_NT; ++i) wsum[warp * FREE_ROWS + lane + 32 * i] = acc[i];
-        __syncthreads();
-        if (threadIdx.x < FREE_ROWS) {
+        team_sync(team);
+        for (int r = team.tid; r < FREE_ROWS; r += team.nthr) {
             double s = 0.0;
-#pragma unroll
-            for (int w = 0; w < FREE_WARPS; ++w) s += wsum[w * FREE_ROWS + threadIdx.x];
-            fp.PB[(size_t)(b + c) * FREE_ROWS + threadIdx.x] = s;
+            for (int w = 0; w < team.nwarp; ++w) s += wsum[w * FREE_ROWS + r];
+            fp.PB[(size_t)(b + c) * FREE_ROWS + r] = s;
         }
-        __syncthreads();
+        team_sync(team);
         u0 = ue;
         ++b;
     }
@@ -192,7 +192,7 @@ __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable
             if (!(ct.off[k] < r1 && ct.off[k + 1] > r0)) continue;      // CTA-uniform
             if (nt.DG[ct.off[k]].y == 0.0) { if (threadIdx.x == 0) csum[k] = 0.0; continue; }
             double s = 0.0;
-            for (int i = ct.off[k] + threadIdx.x; i < ct.off[k + 1]; i += blockDim.x) s += __ldcg(xsrc + i);
+            for (int i = max(ct.off[k], fp.s_off) + threadIdx.x; i < ct.off[k + 1]; i += blockDim.x) s += __ldcg(xsrc + i);
             s = bie_warp_sum(s);
             if (lane == 0) wred[warp] = s;
             __syncthreads();
@@ -222,7 +222,10 @@ __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable
         // near pairs: exact entries from the CSR near matrix
         const int p0 = fp.near_ptr[8 * (size_t)t], p1 = fp.near_ptr[8 * (size_t)t + 8];
         double sn = 0.0;
-        for (int p = p0; p < p1; ++p) sn = fma(fp.near_val[p], __ldcg(xsrc + fp.near_col[p]), sn);
+        for (int p = p0; p < p1; ++p) {
+            const int cix = fp.near_col[p];
+            if (cix >= fp.s_off) sn = fma(fp.near_val[p], __ldcg(xsrc + cix), sn);
+        }
         s += sn;
         const int k = nt.COMP[t];
         s = fma(-nt.DG[t].y, csum[k], s);

@@ -20,6 +20,9 @@ __host__ __device__ inline int gemv_chunk(int rows_per_cta, int n, int nwarp)
     int chunk = 2048;
     const int npair = (rows_per_cta + 1) >> 1;
     while (chunk > 128 && npair * ((n + chunk - 1) / chunk) < 2 * nwarp) chunk >>= 1;
+    // equal chunks: a short last chunk would always land on the same warps (units go round-robin)
+    const int nch = (n + chunk - 1) / chunk;
+    chunk = ((n + nch - 1) / nch + 63) & ~63;
     return chunk;
 }
 
@@ -39,13 +42,14 @@ __host__ __device__ inline int gemv_part_doubles(int rows_per_cta, int n, int ch
 }
 
 // y_local[r - r0] = sum_c A[r][c] * x[c] for r in [r0, r1).  xs: x in shared memory (XS = true) or global.
-// part: shared scratch of gemv_part_doubles() doubles.  All threads of the CTA must call; ends with the
-// results in y_local (shared) after a __syncthreads().
-template <bool STREAM, bool XS>
+// part: shared scratch of gemv_part_doubles() doubles.  All threads of the team must call; ends with the
+// results in y_local (shared) after a team barrier.  n = number of columns used (the hybrid operator passes
+// the width of its stored slab).
+template <bool STREAM, bool XS, int UNROLL = GEMV_UNROLL>
 __device__ __forceinline__ void bie_cta_gemv(const double* __restrict__ A, long long lda, int n, int r0, int r1, int chunk,
-                                             const double* xs, double* part, double* y_local)
+                                             const double* xs, double* part, double* y_local, const Team& tm)
 {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    const int lane = tm.tid & 31, warp = tm.warp, nwarp = tm.nwarp;
     const int rows = r1 - r0;
     const int rows2 = (rows + 1) & ~1;
     const int npair = rows2 >> 1;
@@ -63,15 +67,15 @@ __device__ __forceinline__ void bie_cta_gemv(const double* __restrict__ A, long 
         const int cend = min(cbeg + (chunk >> 1), n2);
         double acc0 = 0.0, acc1 = 0.0;
         int c = cbeg + lane;
-        for (; c + 32 * (GEMV_UNROLL - 1) < cend; c += 32 * GEMV_UNROLL) {
-            double2 v0[GEMV_UNROLL], v1[GEMV_UNROLL];
+        for (; c + 32 * (UNROLL - 1) < cend; c += 32 * UNROLL) {
+            double2 v0[UNROLL], v1[UNROLL];
 #pragma unroll
-            for (int i = 0; i < GEMV_UNROLL; ++i) {
+            for (int i = 0; i < UNROLL; ++i) {
                 v0[i] = gemv_ld<STREAM>(a0 + c + 32 * i);
                 v1[i] = gemv_ld<STREAM>(a1 + c + 32 * i);
             }
 #pragma unroll
-            for (int i = 0; i < GEMV_UNROLL; ++i) {
+            for (int i = 0; i < UNROLL; ++i) {
                 double2 xv;
                 if (XS) xv = reinterpret_cast<const double2*>(xs)[c + 32 * i];
                 else xv = __ldcg(reinterpret_cast<const double2*>(xs) + c + 32 * i);
@@ -99,11 +103,11 @@ __device__ __forceinline__ void bie_cta_gemv(const double* __restrict__ A, long 
             part[ch * rows2 + 2 * p + 1] = acc1;
         }
     }
-    __syncthreads();
-    for (int r = threadIdx.x; r < rows; r += blockDim.x) {
+    team_sync(tm);
+    for (int r = tm.tid; r < rows; r += tm.nthr) {
         double s = 0.0;
         for (int ch = 0; ch < nch; ++ch) s += part[ch * rows2 + r];
         y_local[r] = s;
     }
-    __syncthreads();
+    team_sync(tm);
 }

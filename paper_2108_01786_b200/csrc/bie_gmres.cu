@@ -19,6 +19,9 @@
 #include "bie_free.cuh"
 
 #define GM_THREADS 512
+#ifndef HYB_GEMV_UNROLL
+#define HYB_GEMV_UNROLL 8   // hybrid operator: 2 rows x 8 LDG.128 per lane in flight in each streaming warp
+#endif
 
 struct GmresArgs {
     const double* A;
@@ -43,6 +46,8 @@ struct GmresArgs {
     int rows_per_cta;
     int chunk;
     int VS;        // Krylov vectors 0..VS-1 keep this CTA's rows in shared memory; the others in V (global, L2)
+    int nd;        // hybrid operator: columns [0, nd) come from the stored slab A, sources [nd, n) are recomputed
+    int nwf;       // hybrid operator: warps 0..nwf-1 run the pair loops, the others stream the slab
     NodeTable nt;
     CompTable ct;
     FreePlan fp;
@@ -83,21 +88,61 @@ __device__ __forceinline__ unsigned long long gtime() { unsigned long long t; as
 #define PT(i)
 #endif
 
-template <bool STREAM, bool XS, bool FREE>
+// MODE: 0 = stored matrix (GEMV, HBM-bound), 1 = matrix-free (pair loops, FP64-bound), 2 = hybrid: the first a.nd
+// columns are read from the stored slab by the streaming warps WHILE the other warps recompute the remaining
+// sources -- the HBM pipe and the FP64 pipe of every SM work at the same time.
+template <bool STREAM, bool XS, int MODE>
 __device__ __forceinline__ void cta_apply(const GmresArgs& a, int r0, int r1, const double* xin, double scale,
-                                          double* xs, double* gpart, double* y_local, bool tables_ready,
-                                          unsigned int& target)
+                                          double* xs, double* gpart, double* gpart2, double* ydense, double* y_local,
+                                          bool tables_ready, unsigned int& target)
 {
-    if (FREE) {
+    if (MODE != 0) {
         // xin is complete in global memory; its per-source tables either were written by the row owners before
         // the last grid barrier (tables_ready) or are written here
         if (!tables_ready) {
             free_write_tables(a.nt, a.fp, r0, r1, xin + r0);
             grid_barrier(a.sync, target);
         }
-        free_parts(a.nt, a.fp, gpart);
+        if (MODE == 1) {
+            free_parts(a.nt, a.fp, gpart, cta_team());
+        } else {
+            const int warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+#ifdef BIE_PHASE_TIMING
+            __shared__ unsigned long long hy_acc[3];
+            if (threadIdx.x == 0 && target <= 2 * gridDim.x) { hy_acc[0] = hy_acc[1] = hy_acc[2] = 0; }
+            const unsigned long long hy_t0 = gtime();
+#endif
+            if (warp < a.nwf) {
+                free_parts(a.nt, a.fp, gpart, sub_team(0, a.nwf, 1));
+#ifdef BIE_PHASE_TIMING
+                if (threadIdx.x == 0) hy_acc[0] += gtime() - hy_t0;
+#endif
+            } else {
+                const Team st = sub_team(a.nwf, nwarp - a.nwf, 2);
+                const int nd2 = a.nd >> 1;   // nd is even
+                for (int i = st.tid; i < nd2; i += st.nthr)
+                    reinterpret_cast<double2*>(xs)[i] = __ldcg(reinterpret_cast<const double2*>(xin) + i);
+                team_sync(st);
+                bie_cta_gemv<STREAM, true, HYB_GEMV_UNROLL>(a.A, a.lda, a.nd, r0, r1, a.chunk, xs, gpart2, ydense, st);
+#ifdef BIE_PHASE_TIMING
+                if (st.tid == 0) hy_acc[1] += gtime() - hy_t0;
+#endif
+            }
+            __syncthreads();
+#ifdef BIE_PHASE_TIMING
+            if (threadIdx.x == 0) {
+                hy_acc[2] += 1;
+                if (hy_acc[2] == 40 && (blockIdx.x == 0 || blockIdx.x == 100))
+                    printf("cta %d hybrid us/apply: pair loops %.1f, slab stream %.1f\n", blockIdx.x, hy_acc[0] * 1e-3 / 40, hy_acc[1] * 1e-3 / 40);
+            }
+#endif
+        }
         grid_barrier(a.sync, target);
         free_gather(a.nt, a.ct, a.fp, r0, r1, xin, scale, gpart, y_local);
+        if (MODE == 2) {
+            for (int r = threadIdx.x; r < r1 - r0; r += blockDim.x) y_local[r] = fma(scale, ydense[r], y_local[r]);
+            __syncthreads();
+        }
     } else if (XS) {
         const int n2 = a.n >> 1;
         for (int i = threadIdx.x; i < n2; i += blockDim.x) {
@@ -107,9 +152,9 @@ __device__ __forceinline__ void cta_apply(const GmresArgs& a, int r0, int r1, co
         }
         if ((a.n & 1) && threadIdx.x == 0) xs[a.n - 1] = __ldcg(xin + a.n - 1) * scale;
         __syncthreads();
-        bie_cta_gemv<STREAM, true>(a.A, a.lda, a.n, r0, r1, a.chunk, xs, gpart, y_local);
+        bie_cta_gemv<STREAM, true>(a.A, a.lda, a.n, r0, r1, a.chunk, xs, gpart, y_local, cta_team());
     } else {
-        bie_cta_gemv<STREAM, false>(a.A, a.lda, a.n, r0, r1, a.chunk, xin, gpart, y_local);
+        bie_cta_gemv<STREAM, false>(a.A, a.lda, a.n, r0, r1, a.chunk, xin, gpart, y_local, cta_team());
         if (scale != 1.0) {
             for (int r = threadIdx.x; r < r1 - r0; r += blockDim.x) y_local[r] *= scale;
             __syncthreads();
@@ -209,9 +254,10 @@ __device__ __forceinline__ void cgs_pass(const GmresArgs& a, const Basis& B, int
     __syncthreads();
 }
 
-template <bool STREAM, bool XS, bool FREE>
+template <bool STREAM, bool XS, int MODE>
 __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArgs a)
 {
+    constexpr bool FREE = (MODE != 0);
     extern __shared__ __align__(16) double smem[];
     const int G = gridDim.x;
     const int n = a.n, m = a.m;
@@ -229,9 +275,11 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
     double* g = sn + m;                   // [m+1]
     double* red = g + (m + 1);            // [34]
     double* gpart = red + 34 + ((m & 1) ? 0 : 1);  // GEMV partials or matrix-free scratch (16-byte aligned)
-    double* xs = gpart + (FREE ? free_scratch_doubles(GM_THREADS)
-                               : ((gemv_part_doubles(a.rows_per_cta, n, a.chunk) + 1) & ~1));
-    double* red2 = xs + ((FREE || !XS) ? 0 : ((n + 2) & ~1));   // [blockDim + rows2]
+    // hybrid: GEMV partials of the slab and its result, after the matrix-free scratch
+    double* gpart2 = gpart + (FREE ? free_scratch_doubles(GM_THREADS) : 0);
+    double* ydense = gpart2 + ((MODE == 1) ? 0 : ((gemv_part_doubles(a.rows_per_cta, MODE == 2 ? a.nd : n, a.chunk) + 1) & ~1));
+    double* xs = ydense + ((MODE == 2) ? rows2 : 0);
+    double* red2 = xs + ((MODE == 2) ? ((a.nd + 2) & ~1) : ((FREE || !XS) ? 0 : ((n + 2) & ~1)));   // [blockDim + rows2]
     Basis B;
     B.Vs = red2 + GM_THREADS + rows2;                          // [VS][rows2]
     B.Vg = a.V + r0; B.VS = a.VS; B.rows2 = rows2; B.nld = a.nld;
@@ -263,7 +311,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
             for (int r = threadIdx.x; r < rows; r += blockDim.x) w_local[r] = a.b[r0 + r];
             first = false;
         } else {
-            cta_apply<STREAM, XS, FREE>(a, r0, r1, a.x, 1.0, xs, gpart, y_local, false, target);
+            cta_apply<STREAM, XS, MODE>(a, r0, r1, a.x, 1.0, xs, gpart, gpart2, ydense, y_local, false, target);
             for (int r = threadIdx.x; r < rows; r += blockDim.x) w_local[r] = a.b[r0 + r] - y_local[r];
         }
         __syncthreads();
@@ -296,8 +344,8 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
             PT(7)
             // a6: w = A v_j, with v_j = wbuf * inv
 #ifdef BIE_PHASE_TIMING
-            if (FREE) {
-                free_parts(a.nt, a.fp, gpart);
+            if (MODE == 1) {
+                free_parts(a.nt, a.fp, gpart, cta_team());
                 PT(0)
                 grid_barrier(a.sync, target);
                 PT(1)
@@ -305,7 +353,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
                 PT(2)
             } else
 #endif
-            cta_apply<STREAM, XS, FREE>(a, r0, r1, a.wbuf, inv, xs, gpart, y_local, true, target);
+            cta_apply<STREAM, XS, MODE>(a, r0, r1, a.wbuf, inv, xs, gpart, gpart2, ydense, y_local, true, target);
             for (int r = threadIdx.x; r < rows; r += blockDim.x) w_local[r] = y_local[r];
             __syncthreads();
             PT(3)
@@ -393,7 +441,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
     // ---- a10: outputs; true residual ||b - A x|| / ||b|| (reported only) -----------------------------
     double relres = 0.0;
     if (a.relres_out && bn != 0.0) {
-        cta_apply<STREAM, XS, FREE>(a, r0, r1, a.x, 1.0, xs, gpart, y_local, false, target);
+        cta_apply<STREAM, XS, MODE>(a, r0, r1, a.x, 1.0, xs, gpart, gpart2, ydense, y_local, false, target);
         p = 0.0;
         for (int r = threadIdx.x; r < rows; r += blockDim.x) {
             const double v = a.b[r0 + r] - y_local[r];
@@ -423,31 +471,35 @@ struct GmresPlan {
     size_t offV, offW, offP, offR, offY, total;
 };
 
-static int gmres_plan(int n, int restart, int sm_count, int max_smem, int l2_bytes, long long lda, bool free_op,
-                      GmresPlan* pl)
+// mode: 0 stored matrix, 1 matrix-free, 2 hybrid (slab of nd columns streamed by 16 - nwf warps)
+static int gmres_plan(int n, int restart, int sm_count, int max_smem, int l2_bytes, long long lda, int mode, int nd,
+                      int nwf, GmresPlan* pl)
 {
     const int m = restart;
+    const bool free_op = (mode != 0);
     pl->rows_per_cta = (n + sm_count - 1) / sm_count;
     pl->G = (n + pl->rows_per_cta - 1) / pl->rows_per_cta;
-    pl->chunk = gemv_chunk(pl->rows_per_cta, n, GM_THREADS / 32);
+    pl->chunk = mode == 2 ? gemv_chunk(pl->rows_per_cta, nd, GM_THREADS / 32 - nwf)
+                          : gemv_chunk(pl->rows_per_cta, n, GM_THREADS / 32);
     pl->nld = (n + 1) & ~1;
     const int rows2 = (pl->rows_per_cta + 1) & ~1;
     size_t base = 2 * (size_t)rows2 + 2 * (size_t)(m + 2) + 2 * (size_t)m + (size_t)(m + 1) + 34 + 1;
-    base += free_op ? (size_t)free_scratch_doubles(GM_THREADS)
-                    : (size_t)((gemv_part_doubles(pl->rows_per_cta, n, pl->chunk) + 1) & ~1);
+    if (free_op) base += (size_t)free_scratch_doubles(GM_THREADS);
+    if (mode != 1) base += (size_t)((gemv_part_doubles(pl->rows_per_cta, mode == 2 ? nd : n, pl->chunk) + 1) & ~1);
+    if (mode == 2) base += (size_t)rows2 + (size_t)((nd + 2) & ~1);   // slab result, x of the slab's columns
     base *= sizeof(double);
     base += sizeof(double) * ((size_t)GM_THREADS + rows2);  // red2
-    pl->xs = !free_op && base + sizeof(double) * ((size_t)n + 2) <= (size_t)max_smem;
-    pl->smem = base + (pl->xs ? sizeof(double) * ((size_t)n + 2) : 0);
+    pl->xs = mode == 2 || (!free_op && base + sizeof(double) * ((size_t)n + 2) <= (size_t)max_smem);
+    pl->smem = base + ((pl->xs && mode == 0) ? sizeof(double) * ((size_t)n + 2) : 0);
     if (pl->smem > (size_t)max_smem) return BIE_ERR_ARG;
     // the rest of the shared memory holds this CTA's rows of as many Krylov vectors as fit
     // (dense operator: the streaming loads of A need the L1 as their landing buffer, 16 warps x 4 KB in flight,
     // so the shared-memory carve-out stops at 164 KB; measured: 408 us per step with 227 KB against 338 us)
-    const size_t cap = free_op ? (size_t)max_smem : (size_t)(163 * 1024 < max_smem ? 163 * 1024 : max_smem);
+    const size_t cap = mode == 1 ? (size_t)max_smem : (size_t)(163 * 1024 < max_smem ? 163 * 1024 : max_smem);
     pl->VS = pl->smem < cap ? (int)((cap - pl->smem) / (sizeof(double) * rows2)) : 0;
     if (pl->VS > m + 1) pl->VS = m + 1;
     pl->smem += sizeof(double) * (size_t)pl->VS * rows2;
-    pl->stream = !free_op && (double)n * (double)lda * 8.0 > 0.6 * (double)l2_bytes;
+    pl->stream = mode != 1 && (double)n * (double)(mode == 2 ? nd : lda) * 8.0 > 0.6 * (double)l2_bytes;
     size_t o = 0;
     pl->offV = o; o += al256(sizeof(double) * (size_t)(m + 1) * pl->nld);
     pl->offW = o; o += al256(sizeof(double) * (size_t)pl->nld);
@@ -475,32 +527,35 @@ size_t bie_gmres_ws_bytes(int n, int restart)
     return o + 256;
 }
 
-template <bool STREAM, bool XS, bool FREE>
+template <bool STREAM, bool XS, int MODE>
 static int launch_gmres(const GmresArgs& a, const GmresPlan& pl, cudaStream_t st)
 {
-    auto k = bie_gmres_kernel<STREAM, XS, FREE>;
+    auto k = bie_gmres_kernel<STREAM, XS, MODE>;
     BIE_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
     void* params[] = {(void*)&a};
     BIE_CUDA(cudaLaunchCooperativeKernel((const void*)k, dim3(pl.G), dim3(GM_THREADS), params, pl.smem, st));
     return BIE_OK;
 }
 
-int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, const double* rhs, double tol,
+// nd == 0: stored matrix (A != NULL) or matrix-free (A == NULL); 0 < nd < n (even): hybrid, A holds the columns [0, nd)
+int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, int nd, const double* rhs, double tol,
                      int restart, int max_iters, double* x, int32_t* iters_out, double* relres_out,
                      int32_t* status_out, double* res_hist, void* ws, size_t ws_bytes, cudaStream_t st)
 {
     if (!ctx || !rhs || !x || !ws) return BIE_ERR_NULL;
     if (n < 1 || restart < 1 || max_iters < 0 || !(tol >= 0.0)) return BIE_ERR_ARG;
-    const bool free_op = (A == nullptr);
-    if (free_op) {
-        if (!ctx->have_geom || ctx->n != n) return BIE_ERR_GEOMETRY;
-    } else if (lda < n || (lda & 1) || (((uintptr_t)A) & 15u)) return BIE_ERR_LAYOUT;
+    if (nd < 0 || nd >= n || (nd & 1) || (nd > 0 && !A)) return nd > 0 && !A ? BIE_ERR_NULL : BIE_ERR_ARG;
+    const int mode = nd > 0 ? 2 : (A == nullptr ? 1 : 0);
+    const bool free_op = (mode != 0);
+    if (free_op && (!ctx->have_geom || ctx->n != n)) return BIE_ERR_GEOMETRY;
+    if (mode != 1 && (lda < (mode == 2 ? nd : n) || (lda & 1) || (((uintptr_t)A) & 15u))) return BIE_ERR_LAYOUT;
     if ((((uintptr_t)rhs) | ((uintptr_t)x)) & 15u) return BIE_ERR_LAYOUT;
     if (!ctx->coop_ok) return BIE_ERR_DEVICE;
     if (ctx->sm_count > 256) return BIE_ERR_DEVICE;
     if (restart > n) restart = n;  // the Krylov space cannot exceed n
     GmresPlan pl;
-    int rc = gmres_plan(n, restart, ctx->sm_count, ctx->max_smem_optin, ctx->l2_bytes, free_op ? n : lda, free_op, &pl);
+    const int nwf = ctx->hybrid_free_warps;
+    int rc = gmres_plan(n, restart, ctx->sm_count, ctx->max_smem_optin, ctx->l2_bytes, free_op ? n : lda, mode, nd, nwf, &pl);
     if (rc != BIE_OK) return rc;
     // align the caller's workspace to 256 bytes
     uintptr_t base = ((uintptr_t)ws + 255) & ~(uintptr_t)255;
@@ -515,16 +570,18 @@ int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, const do
     a.yv = (double*)(base + pl.offY);
     a.sync = ctx->sync_buf;
     a.nld = pl.nld; a.rows_per_cta = pl.rows_per_cta; a.chunk = pl.chunk; a.VS = pl.VS;
+    a.nd = nd; a.nwf = nwf;
     memset(&a.nt, 0, sizeof(a.nt)); memset(&a.ct, 0, sizeof(a.ct)); memset(&a.fp, 0, sizeof(a.fp));
     if (free_op) {
         a.nt = bie_node_table(ctx); a.ct = ctx->comps;
         rc = bie_ensure_near(ctx, st);
         if (rc != BIE_OK) return rc;
-        rc = bie_free_plan(ctx, pl.G, &a.fp);
+        rc = bie_free_plan(ctx, pl.G, nd, &a.fp);
         if (rc != BIE_OK) return rc;
     }
     BIE_CUDA(cudaMemsetAsync(ctx->sync_buf, 0, sizeof(unsigned int), st));
-    if (free_op) return launch_gmres<false, false, true>(a, pl, st);
-    if (pl.stream) return pl.xs ? launch_gmres<true, true, false>(a, pl, st) : launch_gmres<true, false, false>(a, pl, st);
-    return pl.xs ? launch_gmres<false, true, false>(a, pl, st) : launch_gmres<false, false, false>(a, pl, st);
+    if (mode == 1) return launch_gmres<false, false, 1>(a, pl, st);
+    if (mode == 2) return pl.stream ? launch_gmres<true, true, 2>(a, pl, st) : launch_gmres<false, true, 2>(a, pl, st);
+    if (pl.stream) return pl.xs ? launch_gmres<true, true, 0>(a, pl, st) : launch_gmres<true, false, 0>(a, pl, st);
+    return pl.xs ? launch_gmres<false, true, 0>(a, pl, st) : launch_gmres<false, false, 0>(a, pl, st);
 }

@@ -26,7 +26,7 @@ bie_matvec_kernel(const double* __restrict__ A, long long lda, int n, int rows_p
         if ((n & 1) && threadIdx.x == 0) xs[n - 1] = x[n - 1];
         __syncthreads();
     }
-    bie_cta_gemv<STREAM, XS>(A, lda, n, r0, r1, chunk, XS ? xs : x, part, y_local);
+    bie_cta_gemv<STREAM, XS>(A, lda, n, r0, r1, chunk, XS ? xs : x, part, y_local, cta_team());
     for (int r = threadIdx.x; r < r1 - r0; r += blockDim.x) y[r0 + r] = y_local[r];
 }
 
@@ -80,7 +80,7 @@ bie_matvec_free_kernel(NodeTable nt, CompTable ct, FreePlan fp, int rows_per_cta
     unsigned int target = 0;
     free_write_tables(nt, fp, r0, r1, x + r0);
     grid_barrier(sync, target);
-    free_parts(nt, fp, scratch);
+    free_parts(nt, fp, scratch, cta_team());
     grid_barrier(sync, target);
     free_gather(nt, ct, fp, r0, r1, x, 1.0, scratch, y_local);
     for (int r = threadIdx.x; r < r1 - r0; r += blockDim.x) y[r0 + r] = y_local[r];
@@ -100,7 +100,7 @@ int bie_launch_matvec_free(bie_ctx* ctx, const double* x, double* y, cudaStream_
     FreePlan fp;
     int rc = bie_ensure_near(ctx, st);
     if (rc != BIE_OK) return rc;
-    rc = bie_free_plan(ctx, G, &fp);
+    rc = bie_free_plan(ctx, G, 0, &fp);
     if (rc != BIE_OK) return rc;
     BIE_CUDA(cudaFuncSetAttribute(bie_matvec_free_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     BIE_CUDA(cudaMemsetAsync(ctx->sync_buf, 0, sizeof(unsigned int), st));

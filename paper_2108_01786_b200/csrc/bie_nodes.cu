@@ -143,16 +143,19 @@ size_t bie_free_buf_doubles(int cap)
     return 8 * (size_t)cap + ((size_t)cap / FREE_ROWS + 2 + 256) * FREE_ROWS;
 }
 
-int bie_free_plan(const bie_ctx* ctx, int grid, FreePlan* fp)
+int bie_free_plan(const bie_ctx* ctx, int grid, int s_off, FreePlan* fp)
 {
     if (!ctx->have_geom || grid < 1 || grid > 256) return BIE_ERR_GEOMETRY;
+    if (s_off < 0 || (s_off & 1) || s_off > ctx->n) return BIE_ERR_ARG;
     const int n = ctx->n, npad = bie_npad(n);
     fp->M0 = ctx->counts[0];
     fp->NB0 = (fp->M0 + FREE_ROWS - 1) / FREE_ROWS;
     fp->NB = fp->NB0 + (n - fp->M0 + FREE_ROWS - 1) / FREE_ROWS;
-    fp->UB = npad / 2;
+    fp->s_off = s_off;
+    fp->UB = (npad - s_off) / 2;
     fp->U = (long long)fp->NB * fp->UB;
     fp->Geff = (long long)grid < fp->U ? grid : (int)fp->U;
+    if (fp->Geff < 1) fp->Geff = 1;
     fp->T = reinterpret_cast<double2*>(ctx->free_buf);
     fp->PB = ctx->free_buf + 8 * (size_t)npad;
     fp->taubar = ctx->taubar;

@@ -288,6 +288,69 @@ def test_gmres_matrix_free_parity(ctx, c):
     assert rr <= 10 * P.tol
 
 
+def gpu_gmres_hybrid(ctx, g, nd, b, tol, restart, max_iters=1000, lda=None):
+    """slab of nd columns written by bie_build_cols (the rest of the allocation is poisoned: it must never be read)"""
+    from paper_2108_01786_b200 import bie
+    n = b.size
+    lda = lda or (nd + (nd & 1))
+    z, dz, d2z = geo_dev(g)
+    A = torch.full((n, lda), float("nan"), dtype=torch.float64, device="cuda")
+    ctx.bie_build_cols(g.counts, g.kinds, z, dz, d2z, nd, A, lda=lda)
+    ws = torch.empty(bie.Context.bie_gmres_workspace_bytes(n, restart), dtype=torch.uint8, device="cuda")
+    oi = torch.full((2,), -7, dtype=torch.int32, device="cuda")
+    of = torch.full((1,), -7.0, dtype=torch.float64, device="cuda")
+    x = torch.empty(n + (n & 1), dtype=torch.float64, device="cuda")
+    ctx.bie_gmres_hybrid(A, nd, dev(b), x[:n], tol, restart, max_iters, ws, oi, of, lda=lda)
+    torch.cuda.synchronize()
+    return x[:n].cpu().numpy(), int(oi[0]), float(of[0]), int(oi[1]), A
+
+
+def test_build_cols_writes_only_the_slab(ctx):
+    g = cfg(2).geometry
+    n, nd, lda = g.n, 778, 900
+    z, dz, d2z = geo_dev(g)
+    A = torch.full((n, lda), -7.0, dtype=torch.float64, device="cuda")
+    ctx.bie_build_cols(g.counts, g.kinds, z, dz, d2z, nd, A, lda=lda)
+    Ah = A.cpu().numpy()
+    Ao = oracle_build(g)
+    assert rel_max(Ah[:, :nd], Ao[:, :nd]) <= TOL_ENTRY
+    assert np.all(Ah[:, nd:] == -7.0)
+
+
+@pytest.mark.parametrize("c,nd", [(1, 128), (2, 0), (2, 2), (2, 1030), (2, 2046), (3, 0), (5, 0)])
+def test_gmres_hybrid_parity(ctx, c, nd):
+    """hybrid operator (stored slab of nd columns + recomputed sources): same solution, same iteration band;
+    nd = 0 takes the library's own split (bie_hybrid_cols)"""
+    P = cfg(c)
+    g, b = P.geometry, P.rhs[0]
+    nd = nd or ctx.bie_hybrid_cols(g.n)
+    assert 0 < nd < g.n and nd % 2 == 0
+    Ao = oracle_build(g)
+    xo, ito, _, _, _ = oracle.gmres(Ao, b, P.tol, P.restart, P.max_iters)
+    x, it, rr, st, A = gpu_gmres_hybrid(ctx, g, nd, b, P.tol, P.restart, P.max_iters)
+    lo, hi = iteration_band(Ao, b, P.tol, P.restart, P.max_iters)
+    assert st == 0 and lo - 1 <= it <= hi + 1, (it, ito, lo, hi)
+    assert np.linalg.norm(x - xo) / np.linalg.norm(xo) <= TOL_X
+    assert rr <= 10 * P.tol
+    r = b - oracle.matvec(Ao, x)
+    assert np.linalg.norm(r) / np.linalg.norm(b) <= 10 * P.tol
+    del A
+
+
+def test_gmres_hybrid_free_warps_knob(ctx):
+    P = cfg(2)
+    g, b = P.geometry, P.rhs[0]
+    Ao = oracle_build(g)
+    xo, ito, _, _, _ = oracle.gmres(Ao, b, P.tol, P.restart, P.max_iters)
+    try:
+        for w in (1, 4, 12, 15):
+            ctx.bie_set_hybrid_free_warps(w)
+            x, it, rr, st, A = gpu_gmres_hybrid(ctx, g, 1024, b, P.tol, P.restart, P.max_iters)
+            assert st == 0 and abs(it - ito) <= 1 and np.linalg.norm(x - xo) / np.linalg.norm(xo) <= TOL_X
+    finally:
+        ctx.bie_set_hybrid_free_warps(8)
+
+
 def test_gmres_restart_and_iteration_cap(ctx):
     """small restart forces several cycles; iteration counts still agree; max_iters is honoured"""
     P = cfg(2)
@@ -332,7 +395,7 @@ def test_solve_host_end_to_end(ctx):
     g, b = P.geometry, P.rhs[0]
     Ao = oracle_build(g)
     xo, ito, _, _, _ = oracle.gmres(Ao, b, P.tol, P.restart, P.max_iters)
-    for mf in (False, True):
+    for mf in (0, 1, 2):   # BIE_OP_DENSE, BIE_OP_FREE, BIE_OP_HYBRID
         ws = torch.empty(bie.Context.bie_solve_workspace_bytes(g.n, P.restart, mf), dtype=torch.uint8, device="cuda")
         x = np.empty(g.n)
         it, rr, st = ctx.bie_solve_host(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, b, x, P.tol, P.restart,
