@@ -79,14 +79,22 @@ bie_near_kernel(NodeTable nt, const double* __restrict__ taubar, int* __restrict
     if (!FILL && t < n) cnt[(size_t)t * NEAR_SEG + seg] = k;
 }
 
-// exclusive prefix sum of N ints in place, total to a[N]; one CTA
+// exclusive prefix sum of N ints in place (N a multiple of 4, a 16-byte aligned), total to a[N]; one CTA.
+// Thread i owns a contiguous run of int4; the loads of a run are independent and unrolled (the run is read twice,
+// from L2).
 __global__ void __launch_bounds__(1024) bie_near_scan_kernel(int* __restrict__ a, int N)
 {
     __shared__ int sums[1024];
-    const int per = (N + 1023) / 1024;
-    const int lo = min(threadIdx.x * per, N), hi = min(lo + per, N);
+    int4* a4 = reinterpret_cast<int4*>(a);
+    const int N4 = N >> 2;
+    const int per = (N4 + 1023) / 1024;
+    const int lo = min((int)threadIdx.x * per, N4), hi = min(lo + per, N4);
     int s = 0;
-    for (int i = lo; i < hi; ++i) s += a[i];
+#pragma unroll 8
+    for (int i = lo; i < hi; ++i) {
+        const int4 v = __ldcg(a4 + i);
+        s += (v.x + v.y) + (v.z + v.w);
+    }
     sums[threadIdx.x] = s;
     __syncthreads();
     for (int o = 1; o < 1024; o <<= 1) {   // Hillis-Steele inclusive scan
@@ -96,10 +104,13 @@ __global__ void __launch_bounds__(1024) bie_near_scan_kernel(int* __restrict__ a
         __syncthreads();
     }
     int run = sums[threadIdx.x] - s;
+#pragma unroll 8
     for (int i = lo; i < hi; ++i) {
-        const int v = a[i];
-        a[i] = run;
-        run += v;
+        const int4 v = __ldcg(a4 + i);
+        int4 o;
+        o.x = run; o.y = o.x + v.x; o.z = o.y + v.y; o.w = o.z + v.z;
+        run = o.w + v.w;
+        a4[i] = o;
     }
     if (threadIdx.x == 1023) a[N] = sums[1023];
 }
