@@ -40,7 +40,7 @@ FP64_INSTR_PER_PAIR_FREE = 11  # matrix-free operator: FP64-pipe instructions pe
 HBM_FALLBACK_GBS = 6650.0      # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 # dram__bytes_read.sum + dram__bytes_write.sum of the GMRES kernel, one launch, from the committed ncu capture
 # (profiles/r01_ncu_full_gmres_cfg5.md); None for workloads that were not captured
-TRAFFIC_BYTES = {5: 345.81e9}
+TRAFFIC_BYTES = {(5, "dense"): 341.50e9, (5, "hybrid"): 142.79e9}   # profiles/r01b_, r01c_ncu_full_cfg5.md
 
 
 def parse_args():
@@ -396,7 +396,8 @@ def main():
         instr = pairs * FP64_INSTR_PER_PAIR_FREE + ng * n * sc          # + one DFMA per streamed slab entry
         roof = {"bound": "alu", "kernel": "bie_gmres_kernel<%s> (persistent; pair loops dominate)" % args.op,
                 "achieved": instr / (gmres_ms * 1e-3) / 1e12, "peak": dfma_per_s / 1e12,
-                "unit": "T FP64 instr/s", "traffic": None, "fp64_instr_per_pair": FP64_INSTR_PER_PAIR_FREE,
+                "unit": "T FP64 instr/s", "traffic": TRAFFIC_BYTES.get((args.config, args.op)),
+                "fp64_instr_per_pair": FP64_INSTR_PER_PAIR_FREE,
                 "pairs_per_launch": pairs, "operator_applications_per_launch": ng,
                 "peak_source": "bie_probe_dfma in this run (nominal 148 SM x 64 lanes x 1.965 GHz = 18.6)"}
         if sc:   # the slab is streamed from HBM by the other warps at the same time
@@ -406,7 +407,7 @@ def main():
     else:
         roof = {"bound": "hbm", "kernel": "bie_gmres_kernel (persistent; GEMV phases dominate)",
                 "achieved": ng * 8.0 * n * n / (gmres_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
-                "traffic": TRAFFIC_BYTES.get(args.config), "peak_source": peak_src,
+                "traffic": TRAFFIC_BYTES.get((args.config, args.op)), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": ng * 8 * n * n, "gemvs_per_launch": ng}
     roof["frac"] = roof["achieved"] / roof["peak"]
     roof_build = None
