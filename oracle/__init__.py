@@ -83,7 +83,8 @@ def _c128_as_f64(z: np.ndarray) -> np.ndarray:
 
 def build_matrix(counts, kinds, zeta, dzeta, d2zeta, variant: int = 0,
                  out: Optional[np.ndarray] = None) -> np.ndarray:
-    """Matrix of Eq. (3.16) (variant 0) or the uncorrected operator B of Eq. (3.10) (variant 1)."""
+    """Matrix of Eq. (3.16) (variant 0), the uncorrected operator B of Eq. (3.10) (variant 1), or the vortex-sheet
+    system matrix of Eqs. (4.14) + (4.17) built from the adjoint matrices of Eq. (4.7) (variant 2)."""
     counts = np.ascontiguousarray(counts, dtype=np.int32)
     kinds = np.ascontiguousarray(kinds, dtype=np.int32)
     n = int(counts.sum())

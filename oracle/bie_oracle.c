@@ -14,6 +14,8 @@
  *                     Table 1, the diagonal limit, the block
  *                     structure of Eq. (3.10), the trapezoid weights 1/M_j
  *                      and E_m = M_m^{-1} e e^T.
+ *                     variant 2: the vortex-sheet system of Eqs. (4.14) + (4.17) with the adjoint
+ *                     matrices K+, G+ of Eq. (4.7); its solid-solid block is Eq. (4.5).
  *   oracle_matvec     y = A x, the plain definition (long-double accumulation).
  *   oracle_gmres      restarted GMRES(m) of Saad & Schultz (ref. [38] cited at PAPER.md:L855), modified
  *                     Gram-Schmidt + Givens rotations, x0 = 0, stop when the recurrence residual
@@ -22,7 +24,9 @@
  * Pins (tests/test_oracle_pins.py, run with -m "not gpu"): P1 cot vs 40-digit mpmath and vs the image
  * sum (3.4); P2 block row sums from Eq. (6.3); P3 analytic-function reproduction; P4 spectral
  * convergence; P5 adaptive quadrature of the kernel; P6 flat/flat closed-form solution; P7 GMRES vs
- * LAPACK dgesv.  Nothing here is "parity unpinned".
+ * LAPACK dgesv; P8 (variant 2) the dagger relation S = D B^T D^-1 + J against the pinned B, the Fourier
+ * closed form of the flat-bottom auxiliary system, adaptive quadrature of Eq. (4.6).  Nothing here is
+ * "parity unpinned".
  *
  * Readings of the paper where it is silent or garbled are listed in DESIGN.md ("Readings").
  */
@@ -105,6 +109,54 @@ static void oracle_row(long t, long n, const int *comp, const int *counts, const
     }
 }
 
+/* One row (node t = (k,m)) of the VORTEX-SHEET system matrix S: rows on Gamma_0 are Eq. (4.14),
+ * rows on solids Eq. (4.17); its trailing block (rows and columns on solids) is the matrix of
+ * the auxiliary system (4.5).  The adjoint operators of Eq. (4.6) are collocated
+ * with the matrices of Eq. (4.7):
+ *      (K+_jk)_ml = K_jk(alpha_jl, alpha_km) / M_j,    (G+_jk)_ml = G_jk(alpha_jl, alpha_km) / M_j,
+ * row m on Gamma_k, column l on Gamma_j.  With Table 1, K_jk(a,b) + i G..: the kernel's target is
+ * its FIRST index, so  K_jk(alpha_jl, alpha_km) = Im c,  G_jk(alpha_jl, alpha_km) = Re c  with
+ *      c = zeta'_k[m]/2 * cot((zeta_k[m] - zeta_j[l])/2)        (weight zeta' of the ROW node, argument row - column)
+ * and for (k,m) == (j,l) the limit K_kk(a,a) = Im{zeta''_k/(2 zeta'_k)}.  Entry, divided by M_j:
+ *      k = 0,  j = 0  :  Im c + 1/2 delta        (1/2 I + K+_00,   Eq. 4.14)
+ *      k = 0,  j >= 1 : -Re c                    (-G+_j0,          Eq. 4.14)
+ *      k >= 1, j = 0  :  Re c                    (G+_0k,           Eq. 4.17)
+ *      k >= 1, j >= 1 :  Im c - 1/2 delta        (-1/2 I + K+_jk,  Eq. 4.5 / 4.17)                                  */
+static void oracle_row_dagger(long t, long n, const int *comp, const int *counts,
+                              const double *zeta, const double *dzeta, const double *d2zeta, double *row)
+{
+    const int k = comp[t];
+    const double ztr = zeta[2 * t], zti = zeta[2 * t + 1];
+    const double ur = 0.5 * dzeta[2 * t], ui = 0.5 * dzeta[2 * t + 1]; /* zeta'_k[m] / 2 */
+    for (long s = 0; s < n; ++s) {
+        const int j = comp[s];
+        const double Mj = (double)counts[j];
+        double cre, cim;
+        if (s == t) {
+            double ar = d2zeta[2 * s], ai = d2zeta[2 * s + 1];
+            double br = dzeta[2 * s], bi = dzeta[2 * s + 1];
+            double den = br * br + bi * bi;
+            cre = 0.0; /* never used: G blocks have k != j */
+            cim = (ai * br - ar * bi) / den / 2.0;
+        } else {
+            double cr, ci;
+            oracle_cot_half(ztr - zeta[2 * s], zti - zeta[2 * s + 1], &cr, &ci);
+            cre = ur * cr - ui * ci;
+            cim = ur * ci + ui * cr;
+        }
+        double e;
+        if (k == 0 && j == 0)
+            e = cim / Mj + (s == t ? 0.5 : 0.0);
+        else if (k == 0)
+            e = -cre / Mj;
+        else if (j == 0)
+            e = cre / Mj;
+        else
+            e = cim / Mj - (s == t ? 0.5 : 0.0);
+        row[s] = e;
+    }
+}
+
 /* Matrix of Eq. (3.16).
  *
  * components: c = 0..ncomp-1 with counts[c] = M_c nodes alpha_{cl} = 2 pi l / M_c,
@@ -118,7 +170,8 @@ static void oracle_row(long t, long n, const int *comp, const int *counts, const
  *         k = 0, j >= 1:  Re c                      (G_0j)
  *         k >= 1, j = 0: -Re c                      (-G_k0)
  *         k >= 1, j >= 1: Im c + 1/2 delta - [k = j is an obstacle]/M_k   (1/2 I + K_kj - E_k)
- * variant 0: as above; variant 1: without the E_k term (the operator B of Eq. (3.10)).
+ * variant 0: as above; variant 1: without the E_k term (the operator B of Eq. (3.10)); variant 2: the vortex-sheet
+ * system matrix of Eqs. (4.14) + (4.17) documented at oracle_row_dagger.
  * A is row-major n x n with leading dimension lda >= n.  Returns 0, or <0 on bad arguments. */
 int oracle_build(int ncomp, const int *counts, const int *kinds,
                  const double *zeta, const double *dzeta, const double *d2zeta,
@@ -141,8 +194,10 @@ int oracle_build(int ncomp, const int *counts, const int *kinds,
             for (int l = 0; l < counts[c]; ++l) comp[p++] = c;
     }
 #pragma omp parallel for schedule(static)
-    for (long t = 0; t < n; ++t)
-        oracle_row(t, n, comp, counts, kinds, zeta, dzeta, d2zeta, variant, A + t * lda);
+    for (long t = 0; t < n; ++t) {
+        if (variant == 2) oracle_row_dagger(t, n, comp, counts, zeta, dzeta, d2zeta, A + t * lda);
+        else oracle_row(t, n, comp, counts, kinds, zeta, dzeta, d2zeta, variant, A + t * lda);
+    }
     free(comp);
     return 0;
 }
@@ -171,8 +226,10 @@ int oracle_build_rows(int ncomp, const int *counts, const int *kinds,
             for (int l = 0; l < counts[c]; ++l) comp[p++] = c;
     }
 #pragma omp parallel for schedule(static)
-    for (long i = 0; i < nrows; ++i)
-        oracle_row(rows[i], n, comp, counts, kinds, zeta, dzeta, d2zeta, variant, out + i * n);
+    for (long i = 0; i < nrows; ++i) {
+        if (variant == 2) oracle_row_dagger(rows[i], n, comp, counts, zeta, dzeta, d2zeta, out + i * n);
+        else oracle_row(rows[i], n, comp, counts, kinds, zeta, dzeta, d2zeta, variant, out + i * n);
+    }
     free(comp);
     return 0;
 }

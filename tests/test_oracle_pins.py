@@ -397,3 +397,125 @@ def test_config_iteration_counts_in_paper_range():
         A = _build(P.geometry)
         x, iters, relres, hist, status = oracle.gmres(A, P.rhs[0], P.tol, P.restart, P.max_iters)
         assert status == 0 and lo <= iters <= hi and relres < 2e-13
+
+
+# --------------------------------------------------------------------------------------------
+# P8  vortex-sheet system (variant 2): adjoint matrices of Eq. (4.7), systems (4.5) and (4.14) + (4.17)
+# --------------------------------------------------------------------------------------------
+def _comp_of(geo):
+    return np.repeat(np.arange(len(geo.counts)), geo.counts)
+
+
+@pytest.mark.parametrize("which", ["config1", "ragged"])
+def test_p8_dagger_relation_against_the_pinned_B(which):
+    """Eq. (4.7): (K+_jk)_ml = (M_k/M_j) K_jk,lm, same for G+.  Hence the matrix S of (4.14) + (4.17),
+    which the oracle builds entry by entry from K_jk(alpha_jl, alpha_km)/M_j, must equal D B^T D^-1 + J with B the
+    operator of Eq. (3.10) (pinned by P1-P6), D = diag(M of the node's component) and J = +1 on Gamma_0 rows
+    (1/2 I + K+_00 against (-1/2 I + K_00)^T), -1 on solid rows.  A wrong weight (1/M_k for 1/M_j), a wrong sign of the
+    cot argument, a swapped Re/Im or a zeta' taken from the column node each break it at O(1)."""
+    geo = inputs.make_config(1).geometry if which == "config1" else inputs.small_problem(37, 29, [19, 23]).geometry
+    B = _build(geo, variant=1)
+    S = _build(geo, variant=2)
+    comp = _comp_of(geo)
+    D = np.asarray(geo.counts, dtype=float)[comp]
+    J = np.where(comp == 0, 1.0, -1.0)
+    R = D[:, None] * B.T / D[None, :] + np.diag(J)
+    assert np.max(np.abs(S - R)) < 5e-15
+    # and it is NOT the plain transpose when the components have different M (the re-normalisation matters)
+    assert np.max(np.abs(S - (B.T + np.diag(J)))) > 1e-3
+
+
+def test_p8_flat_bottom_auxiliary_system_closed_form():
+    """N = 1, flat surface zeta_0 = a over a flat bottom zeta_1 = a - iH: K+_11 = 0, so Eq. (4.5) is
+    -1/2 gamma_1 = -G+_01 gamma_0.  From cot(z/2) = i (1 + 2 sum_k e^{-ikz}) for Im z < 0:
+    G_01(beta, alpha) = Re{1/2 cot((alpha - beta - iH)/2)} = sum_k e^{-kH} sin k(alpha - beta), hence
+    G+_01 cos(p.) = 1/2 e^{-pH} sin(p.), G+_01 sin(p.) = -1/2 e^{-pH} cos(p.), and gamma_1 = e^{-pH} sin(p a) for
+    gamma_0 = cos(p a).  Also K+_00 = 0 and G+_10 = the mirror image (row on Gamma_0 lies ABOVE the source)."""
+    M0, M1, H, p = 64, 48, 1.3, 3
+    geo = inputs.flat_flat(M0, M1, H)
+    S = _build(geo, variant=2)
+    a0 = 2 * np.pi * np.arange(M0) / M0
+    a1 = 2 * np.pi * np.arange(M1) / M1
+    G01 = S[M0:, :M0]                     # rows on the bottom, columns on Gamma_0
+    assert np.max(np.abs(G01 @ np.cos(p * a0) - 0.5 * np.exp(-p * H) * np.sin(p * a1))) < 1e-14
+    assert np.max(np.abs(G01 @ np.sin(p * a0) + 0.5 * np.exp(-p * H) * np.cos(p * a1))) < 1e-14
+    assert np.max(np.abs(S[:M0, :M0] - 0.5 * np.eye(M0))) < 1e-15      # 1/2 I + K+_00, K+_00 = 0
+    assert np.max(np.abs(S[M0:, M0:] + 0.5 * np.eye(M1))) < 1e-15      # -1/2 I + K+_11, K+_11 = 0
+    # -G+_10: the bottom seen from above, Im z > 0: cot(z/2) = -i (1 + 2 sum e^{ikz}), Re{1/2 cot((a - b + iH)/2)} =
+    # sum_k e^{-kH} sin k(a - b) again, so G+_10 cos(p.) = 1/2 e^{-pH} sin(p.) and the block -G+_10 gives minus that
+    mG10 = S[:M0, M0:]
+    assert np.max(np.abs(mG10 @ np.cos(p * a1) + 0.5 * np.exp(-p * H) * np.sin(p * a0))) < 1e-14
+    # the auxiliary system (4.5), solved by the oracle's GMRES
+    aux = S[M0:, M0:]
+    rhs = -G01 @ np.cos(p * a0)
+    x, iters, relres, hist, status = oracle.gmres(np.ascontiguousarray(aux), rhs, 1e-14, 50, 200)
+    assert status == 0 and np.max(np.abs(x - np.exp(-p * H) * np.sin(p * a1))) < 1e-13
+
+
+def test_p8_adjoint_rows_against_adaptive_quadrature():
+    """Eq. (4.6): (K*_jk gamma_j)(alpha) = (1/2pi) int K_jk(beta, alpha) gamma_j(beta) d beta and the same
+    with G, by Gauss-Kronrod on analytic curves; K_jk(beta, alpha) = Im{zeta'_k(alpha)/2 cot((zeta_k(alpha) - zeta_j(beta))/2)}
+    written from Table 1 with numpy's tan, limit Im{zeta''/(2 zeta')} at beta = alpha; against (row of S) . samples."""
+    from scipy.integrate import quad
+
+    M0, M1, M2 = 64, 48, 40
+    c0 = lambda a: a + 1j * (0.1 * np.cos(a) + 0.03 * np.sin(2 * a))
+    d0 = lambda a: 1 + 1j * (-0.1 * np.sin(a) + 0.06 * np.cos(2 * a))
+    e0 = lambda a: 1j * (-0.1 * np.cos(a) - 0.12 * np.sin(2 * a))
+    c1 = lambda a: a + 1j * (-1.5 + 0.2 * np.cos(a))
+    d1 = lambda a: 1 + 1j * (-0.2 * np.sin(a))
+    e1 = lambda a: 1j * (-0.2 * np.cos(a))
+    rot, zc, q, bb = np.exp(0.4j), 3.0 - 0.7j, 0.35, 0.2
+    c2 = lambda a: zc + rot * (q * np.cos(a) - 1j * bb * np.sin(a))
+    d2 = lambda a: rot * (-q * np.sin(a) - 1j * bb * np.cos(a))
+    e2 = lambda a: rot * (-q * np.cos(a) + 1j * bb * np.sin(a))
+    curves = [(c0, d0, e0, M0), (c1, d1, e1, M1), (c2, d2, e2, M2)]
+    parts = []
+    for c, d, e, M in curves:
+        a = 2 * np.pi * np.arange(M) / M
+        parts.append((c(a), d(a), e(a)))
+    geo = inputs.assemble(parts, [0, 1, 2])
+    S = _build(geo, variant=2)
+    gam = lambda b: 0.7 + 0.5 * np.cos(b) - 0.25 * np.sin(3 * b)
+
+    def kern(k, j, a, b):
+        """entry pattern of row block k (point alpha on Gamma_k), column block j (density on Gamma_j)"""
+        ck, dk, ek, cj = curves[k][0], curves[k][1], curves[k][2], curves[j][0]
+        if k == j and abs(b - a) < 1e-9:
+            c = ek(a) / (2 * dk(a))
+        else:
+            c = 0.5 * dk(a) / np.tan(0.5 * (ck(a) - cj(b)))
+        if k == 0 and j == 0:
+            return c.imag          # K*_00   (Eq. 4.14)
+        if k == 0:
+            return -c.real         # -G*_j0  (Eq. 4.14)
+        if j == 0:
+            return c.real          # G*_0k   (Eq. 4.17)
+        return c.imag              # K*_jk   (Eq. 4.5 / 4.17)
+
+    for (k, m) in [(0, 5), (1, 17), (2, 3), (2, 21), (0, 40)]:
+        a = 2 * np.pi * m / curves[k][3]
+        row = geo.component(k).start + m
+        for j in range(3):
+            val, _ = quad(lambda b: kern(k, j, a, b) * gam(b) / (2 * np.pi), 0, 2 * np.pi,
+                          points=[a] if k == j and a > 0 else None, epsabs=1e-13, epsrel=1e-13, limit=400)
+            sj = geo.component(j)
+            bj = 2 * np.pi * np.arange(curves[j][3]) / curves[j][3]
+            num = S[row, sj] @ gam(bj)
+            if k == j:  # remove the +-1/2 identity
+                num -= (0.5 if k == 0 else -0.5) * gam(a)
+            assert abs(num - val) < 2e-11, (k, m, j, num, val)
+
+
+def test_p8_auxiliary_system_is_well_conditioned_and_converges_like_the_paper():
+    """Eq. (4.5) "is well-conditioned once enough grid points are used"; the paper's GMRES needs 20-32
+    iterations on it.  Plausibility band only."""
+    P = inputs.make_config(2)
+    g = P.geometry
+    S = _build(g, variant=2)
+    M0 = g.counts[0]
+    aux = np.ascontiguousarray(S[M0:, M0:])
+    assert np.linalg.cond(aux) < 50
+    rhs = np.cos(np.arange(aux.shape[0]) * 0.01) + 0.3
+    x, iters, relres, hist, status = oracle.gmres(aux, rhs, 1e-13, 50, 500)
+    assert status == 0 and 8 <= iters <= 60 and relres < 1e-12
