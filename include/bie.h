@@ -61,6 +61,15 @@ extern "C" {
 /* bie_build `variant` */
 #define BIE_VARIANT_A 0 /* Eq. (3.16): 1/2 I + K_mm - E_m on obstacle diagonal blocks  */
 #define BIE_VARIANT_B 1 /* the uncorrected operator B of Eq. (3.10), for invariants    */
+#define BIE_VARIANT_VORTEX 2 /* vortex-sheet system S of Eqs. (4.14) + (4.17), built from the
+                                adjoint matrices of Eq. (4.7):  c+ = zeta'_k[m]/(2 M_j) cot((zeta_k[m] - zeta_j[l])/2)
+                                  k = 0,  j = 0  :  Im c+ + 1/2 [s==t]     (1/2 I + K+_00)
+                                  k = 0,  j >= 1 : -Re c+                  (-G+_j0)
+                                  k >= 1, j = 0  :  Re c+                  (G+_0k)
+                                  k >= 1, j >= 1 :  Im c+ - 1/2 [s==t]     (-1/2 I + K+_jk)
+                                Its trailing block (rows and columns on solids: A + M_0 lda + M_0, size n - M_0, M_0 even)
+                                is the auxiliary system (4.5); bie_gmres takes it as it is.
+                                Dense only: the matrix-free / hybrid operators apply to variants A and B. */
 
 typedef struct bie_ctx bie_ctx;
 

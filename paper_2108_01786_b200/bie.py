@@ -27,7 +27,7 @@ EXPORTS = ("bie_create", "bie_destroy", "bie_strerror", "bie_device_info", "bie_
 
 BIE_OK, BIE_MAX_ITERS = 0, 1
 OP_DENSE, OP_FREE, OP_HYBRID = 0, 1, 2
-VARIANT_A, VARIANT_B = 0, 1
+VARIANT_A, VARIANT_B, VARIANT_VORTEX = 0, 1, 2
 
 
 class BieError(RuntimeError):

@@ -128,6 +128,114 @@ bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long l
     }
 }
 
+// ---------------------------------------------------------------------------------------------------
+// Vortex-sheet variant (BIE_VARIANT_VORTEX): the matrix S of Eqs. (4.14) + (4.17) from
+// the adjoint matrices of Eq. (4.7), (K+_jk)_ml = K_jk(alpha_jl, alpha_km)/M_j.  Entry of row
+// t = (k,m), column s = (j,l):   c+ = zeta'_t/(2 M_j) cot((zeta_t - zeta_s)/2) = -(u_t/M_j)(-2X + iY)/den,
+// u_t = zeta'_t/2, i.e. the weight comes from the ROW node and only 1/M_j from the column.  With m_s = 1/M_j folded
+// into the source's factors (X' = m_s X, Y' = m_s (M_s - M_t)) the entry is (A_t X' + B_t Y')/den with
+//     Im c+ -> (A, B) = (2 u_i, -u_r)   [k = 0, j = 0: 1/2 I + K+_00]  and  [k, j >= 1: -1/2 I + K+_jk]
+//    -Re c+ -> (-2 u_r, -u_i)           [k = 0, j >= 1: -G+_j0]
+//     Re c+ -> ( 2 u_r,  u_i)           [k >= 1, j = 0:  G+_0k]
+// again 13 FP64-pipe instructions per entry; (A, B) sit in shared memory per target row, one pair for columns
+// on Gamma_0 and one for columns on solids.  Same tiling, near-pair handling and stores as bie_build_kernel.
+struct SrcColD {
+    double er, ei;        // E_s
+    double ser, sei, sm;  // m_s E_s, m_s M_s
+    double ms;            // 1 / M_j
+    int thi;
+};
+
+__device__ __forceinline__ double bie_entry_fast_dagger(const SrcColD& s, const double2 te, const double tm,
+                                                        const double2 ab, int& flag)
+{
+    const double dr = s.er - te.x, di = s.ei - te.y;
+    const double den = fma(dr, dr, di * di);
+    const double X = fma(te.y, s.ser, -(te.x * s.sei));
+    const double Y = fma(-s.ms, tm, s.sm);
+    const double val = fma(ab.y, Y, ab.x * X);
+    flag |= (__double2hiint(den) < s.thi) ? 1 : 0;
+    return val * bie_rcp3(den);
+}
+
+__global__ void __launch_bounds__(BUILD_THREADS)
+bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long lda, int T, int only0, int ncols)
+{
+    extern __shared__ __align__(16) double2 sm[];  // [T] E_t, [T] (A,B) for columns on Gamma_0, [T] (A,B) for solids, [T] M_t
+    const int n = nt.n;
+    const int c0 = blockIdx.x * BUILD_TILE_W;
+    const int t0 = blockIdx.y * T;
+    const int t1 = min(t0 + T, n);
+    if (only0 && t0 >= ct.off[1] && c0 >= ct.off[1]) return;
+    double2* sE = sm;
+    double2* sAB0 = sm + T;
+    double2* sAB1 = sm + 2 * T;
+    double* sM = reinterpret_cast<double*>(sm + 3 * T);
+    for (int i = threadIdx.x; i < t1 - t0; i += BUILD_THREADS) {
+        const int t = t0 + i;
+        const int k = nt.COMP[t];
+        const double Mk = (double)(ct.off[k + 1] - ct.off[k]);
+        const double2 q = nt.Q[t];
+        const double ur = q.x * Mk, ui = q.y * Mk;   // zeta'_t / 2
+        sE[i] = nt.E[t];
+        sM[i] = nt.MT[t].x;
+        const double2 im = make_double2(2.0 * ui, -ur);
+        if (k == 0) { sAB0[i] = im; sAB1[i] = make_double2(-2.0 * ur, -ui); }   // K+_00 ; -G+_j0
+        else        { sAB0[i] = make_double2(2.0 * ur, ui); sAB1[i] = im; }      // G+_0k ; K+_jk
+    }
+    const int s0 = c0 + BUILD_COLS * threadIdx.x;  // < npad by construction
+    SrcColD src[BUILD_COLS];
+    const double2* sAB[BUILD_COLS];
+#pragma unroll
+    for (int c = 0; c < BUILD_COLS; ++c) {
+        const double2 e = nt.E[s0 + c], mt = nt.MT[s0 + c];
+        const int j = nt.COMP[s0 + c];
+        const double ms = (j >= 0) ? 1.0 / (double)(ct.off[j + 1] - ct.off[j]) : 0.0;
+        src[c].er = e.x; src[c].ei = e.y;
+        src[c].ser = ms * e.x; src[c].sei = ms * e.y; src[c].sm = ms * mt.x; src[c].ms = ms;
+        src[c].thi = __double2hiint(mt.y);
+        sAB[c] = (j == 0) ? sAB0 : sAB1;
+    }
+    __syncthreads();
+    const bool full = (s0 + 1 < ncols);
+    const bool part = (s0 < ncols);
+    for (int tb = t0; tb < t1; tb += BUILD_RB) {
+        int flag = 0;
+        double* row = A + (long long)tb * lda + s0;
+#pragma unroll
+        for (int r = 0; r < BUILD_RB; ++r) {
+            const int t = min(tb + r, t1 - 1);  // the tail repeats the last row (same values, same address)
+            const double2 te = sE[t - t0];
+            const double tm = sM[t - t0];
+            const double e0 = bie_entry_fast_dagger(src[0], te, tm, sAB[0][t - t0], flag);
+            const double e1 = bie_entry_fast_dagger(src[1], te, tm, sAB[1][t - t0], flag);
+            double* p = row + (long long)(t - tb) * lda;
+            if (full) *reinterpret_cast<double2*>(p) = make_double2(e0, e1);
+            else if (part) p[0] = e0;
+        }
+        if (__any_sync(0xffffffffu, flag)) {
+            if (flag) {
+                const int te_ = min(tb + BUILD_RB, t1);
+                for (int t = tb; t < te_; ++t) {
+                    const double2 te = sE[t - t0];
+#pragma unroll
+                    for (int c = 0; c < BUILD_COLS; ++c) {
+                        if (s0 + c >= ncols) continue;
+                        const double dr = src[c].er - te.x, di = src[c].ei - te.y;
+                        const double den = fma(dr, dr, di * di);
+                        if (__double2hiint(den) < src[c].thi) {
+                            const double2 ab = sAB[c][t - t0];
+                            // (A X' + B Y')/den with cot = (-2X + iY)/den; the diagonal entry is prepared per node
+                            A[(long long)t * lda + s0 + c] =
+                                bie_entry_near(nt.DG, nt.XY, src[c].ms * ab.x, src[c].ms * ab.y, 0.0, s0 + c, t);
+                        }
+                    }
+                }
+            }
+        }
+    }
+}
+
 // ncols: the first ncols columns of every row are written (ncols = n: the whole matrix)
 int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int ncols, int only_comp0, cudaStream_t st)
 {
@@ -142,6 +250,12 @@ int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int ncols, int only_c
     int T = 128;
     while (T > 8 && (long long)gx * ((n + T - 1) / T) < 4LL * ctx->sm_count) T >>= 1;
     dim3 grid(gx, (n + T - 1) / T);
+    if (ctx->variant == BIE_VARIANT_VORTEX) {
+        bie_build_dagger_kernel<<<grid, BUILD_THREADS, (3 * sizeof(double2) + sizeof(double)) * T + 16, st>>>(
+            nt, ctx->comps, A, (long long)lda, T, only_comp0, ncols);
+        BIE_CUDA(cudaGetLastError());
+        return BIE_OK;
+    }
     bie_build_kernel<<<grid, BUILD_THREADS, (sizeof(double2) + sizeof(double)) * T + 16, st>>>(nt, ctx->comps, A, (long long)lda, T,
                                                                                             only_comp0, ncols);
     BIE_CUDA(cudaGetLastError());

@@ -548,6 +548,7 @@ int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, int nd, 
     const int mode = nd > 0 ? 2 : (A == nullptr ? 1 : 0);
     const bool free_op = (mode != 0);
     if (free_op && (!ctx->have_geom || ctx->n != n)) return BIE_ERR_GEOMETRY;
+    if (free_op && ctx->variant == BIE_VARIANT_VORTEX) return BIE_ERR_ARG;   // dense only (include/bie.h)
     if (mode != 1 && (lda < (mode == 2 ? nd : n) || (lda & 1) || (((uintptr_t)A) & 15u))) return BIE_ERR_LAYOUT;
     if ((((uintptr_t)rhs) | ((uintptr_t)x)) & 15u) return BIE_ERR_LAYOUT;
     if (!ctx->coop_ok) return BIE_ERR_DEVICE;

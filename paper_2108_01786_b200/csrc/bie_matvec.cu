@@ -90,6 +90,7 @@ int bie_launch_matvec_free(bie_ctx* ctx, const double* x, double* y, cudaStream_
 {
     if (!ctx || !x || !y) return BIE_ERR_NULL;
     if (!ctx->have_geom) return BIE_ERR_GEOMETRY;
+    if (ctx->variant == BIE_VARIANT_VORTEX) return BIE_ERR_ARG;   // dense only (include/bie.h)
     if ((((uintptr_t)x) | ((uintptr_t)y)) & 15u) return BIE_ERR_LAYOUT;
     if (!ctx->coop_ok || ctx->sm_count > 256) return BIE_ERR_DEVICE;
     const int n = ctx->n;

@@ -55,7 +55,9 @@ bie_prepare_nodes_kernel(PrepArgs pa, int n, int npad, int variant,
     const double den = dz.x * dz.x + dz.y * dz.y;
     double d = (d2.y * dz.x - d2.x * dz.y) / den / (2.0 * M);
     const double em = (variant == BIE_VARIANT_A && pa.kinds[k] == BIE_KIND_OBSTACLE) ? 1.0 / M : 0.0;
-    d += (k == 0) ? -0.5 : 0.5;
+    // -1/2 I + K_00, 1/2 I + K_kk (Eq. 3.10); the vortex-sheet system has 1/2 I + K+_00, -1/2 I + K+_kk (Eqs. 4.14, 4.5)
+    if (variant == BIE_VARIANT_VORTEX) d += (k == 0) ? 0.5 : -0.5;
+    else d += (k == 0) ? -0.5 : 0.5;
     d -= em;
     DG[i] = make_double2(d, em);
     comp[i] = k;
@@ -83,7 +85,7 @@ int bie_prepare_nodes(bie_ctx* ctx, int ncomp, const int32_t* counts, const int3
 {
     if (!ctx || !counts || !kinds || !zeta || !dzeta || !d2zeta) return BIE_ERR_NULL;
     if (ncomp < 1 || ncomp > BIE_MAX_COMP) return BIE_ERR_GEOMETRY;
-    if (variant != BIE_VARIANT_A && variant != BIE_VARIANT_B) return BIE_ERR_ARG;
+    if (variant != BIE_VARIANT_A && variant != BIE_VARIANT_B && variant != BIE_VARIANT_VORTEX) return BIE_ERR_ARG;
     long long n = 0;
     int nbottom = 0;
     for (int c = 0; c < ncomp; ++c) {

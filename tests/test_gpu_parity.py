@@ -224,6 +224,83 @@ def test_matvec_free_ragged(ctx, shape):
 
 
 # ------------------------------------------------------------------------------------------------
+# (a') vortex-sheet variant: S of Eqs. (4.14) + (4.17), adjoint matrices of Eq. (4.7)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("c", [1, 2, 3])
+def test_build_vortex_parity_full_matrix(ctx, c):
+    g = cfg(c).geometry
+    S = gpu_build(ctx, g, variant=2).cpu().numpy()[:, :g.n]
+    So = oracle_build(g, variant=2)
+    assert rel_max(S, So) <= TOL_ENTRY
+    assert np.array_equal(np.sign(np.diag(S)), np.where(np.arange(g.n) < g.counts[0], 1.0, -1.0))
+
+
+@pytest.mark.parametrize("shape", [(37, 29, [19, 23]), (5, 3, []), (1, 1, [1]), (300, 171, [33, 2, 129])])
+def test_build_vortex_ragged_sizes(ctx, shape):
+    g = inputs.small_problem(*shape).geometry
+    S = gpu_build(ctx, g, variant=2).cpu().numpy()[:, :g.n]
+    assert rel_max(S, oracle_build(g, variant=2)) <= TOL_ENTRY
+
+
+@pytest.mark.parametrize("c", [4, 5])
+def test_build_vortex_full_size_sampled_rows(ctx, c):
+    g = cfg(c).geometry
+    rng = np.random.default_rng(40 + c)
+    rows = _sample_rows(g, rng)
+    S = gpu_build(ctx, g, variant=2)
+    Sg = S[torch.from_numpy(rows).cuda()].cpu().numpy()[:, :g.n]
+    So = oracle.build_rows(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, rows, variant=2)
+    assert rel_max(Sg, So) <= TOL_ENTRY
+    del S
+
+
+def test_vortex_auxiliary_system_solve(ctx):
+    """Eq. (4.5): the solid-solid block of S, solved in place (pointer offset M_0 lda + M_0) for gamma_1..gamma_N with
+    the right-hand side -G+_0k gamma_0 (the block S[M_0:, :M_0]); and the full system (4.14) + (4.17)."""
+    from paper_2108_01786_b200 import bie
+    P = cfg(2)
+    g = P.geometry
+    n, M0 = g.n, int(g.counts[0])
+    So = oracle_build(g, variant=2)
+    S = gpu_build(ctx, g, variant=2)
+    a0 = 2 * np.pi * np.arange(M0) / M0
+    gamma0 = 1.0 + 0.3 * np.cos(a0) - 0.2 * np.sin(2 * a0)
+    rhs = -So[M0:, :M0] @ gamma0
+    aux_o = np.ascontiguousarray(So[M0:, M0:])
+    xo, ito, _, _, sto = oracle.gmres(aux_o, rhs, 1e-13, 50, 500)
+    assert sto == 0
+    ns = n - M0
+    ws = torch.empty(bie.Context.bie_gmres_workspace_bytes(ns, 50), dtype=torch.uint8, device="cuda")
+    oi = torch.full((2,), -7, dtype=torch.int32, device="cuda")
+    of = torch.full((1,), -7.0, dtype=torch.float64, device="cuda")
+    x = torch.empty(ns, dtype=torch.float64, device="cuda")
+    lda = S.stride(0)
+    sub = S.view(-1)[M0 * lda + M0:]          # the block starts at row M_0, column M_0; same leading dimension
+    ctx.bie_gmres(sub, dev(rhs), x, 1e-13, 50, 500, ws, oi, of, lda=lda)
+    torch.cuda.synchronize()
+    assert int(oi[1]) == 0 and abs(int(oi[0]) - ito) <= 1 and float(of[0]) <= 1e-12
+    assert np.linalg.norm(x.cpu().numpy() - xo) / np.linalg.norm(xo) <= TOL_X
+    # full system with a smooth right-hand side
+    b = P.rhs[0]
+    xo, ito, _, _, sto = oracle.gmres(So, b, P.tol, P.restart, P.max_iters)
+    xg, it, rr, st = gpu_gmres(ctx, S, b, P.tol, P.restart, P.max_iters)
+    assert sto == 0 and st == 0 and abs(it - ito) <= 1 and rr <= 10 * P.tol
+    assert np.linalg.norm(xg - xo) / np.linalg.norm(xo) <= TOL_X
+
+
+def test_vortex_variant_is_dense_only(ctx):
+    from paper_2108_01786_b200 import bie
+    g = cfg(1).geometry
+    z, dz, d2z = geo_dev(g)
+    ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z, variant=2)
+    x = torch.zeros(g.n, dtype=torch.float64, device="cuda")
+    with pytest.raises(bie.BieError) as e:
+        ctx.bie_matvec_free(x, torch.empty_like(x))
+    assert e.value.code == -6
+    ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z)
+
+
+# ------------------------------------------------------------------------------------------------
 # (c) GMRES
 # ------------------------------------------------------------------------------------------------
 def iteration_band(Ao, b, tol, restart, max_iters, delta=0.25):
