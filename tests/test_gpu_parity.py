@@ -428,6 +428,29 @@ def test_gmres_hybrid_free_warps_knob(ctx):
         ctx.bie_set_hybrid_free_warps(8)
 
 
+def test_config4_sequence_of_four_stages(ctx):
+    """BASELINE.json configs[3]: 4 Runge-Kutta-like stages, Gamma_0 perturbed by 1e-3 per stage.  Stage 0 is a full
+    build, stages 1-3 rebuild only the blocks touching Gamma_0 (a4, bie_build_update); every stage is solved from
+    x0 = 0 and compared with the oracle's solution of ITS matrix of that stage."""
+    P = cfg(4)
+    A = None
+    for s, (g, b) in enumerate(zip(P.stages, P.rhs)):
+        z, dz, d2z = geo_dev(g)
+        if s == 0:
+            A = gpu_build(ctx, g)
+        else:
+            ctx.bie_build_update(g.counts, g.kinds, z, dz, d2z, A)
+        Ao = oracle_build(g)
+        xo, ito, _, _, sto = oracle.gmres(Ao, b, P.tol, P.restart, P.max_iters)
+        x, it, rr, st = gpu_gmres(ctx, A, b, P.tol, P.restart, P.max_iters)
+        lo, hi = iteration_band(Ao, b, P.tol, P.restart, P.max_iters)
+        assert sto == 0 and st == 0 and lo - 1 <= it <= hi + 1, (s, it, ito, lo, hi)
+        assert np.linalg.norm(x - xo) / np.linalg.norm(xo) <= TOL_X, s
+        assert rr <= 10 * P.tol
+        del Ao
+    del A
+
+
 def test_gmres_restart_and_iteration_cap(ctx):
     """small restart forces several cycles; iteration counts still agree; max_iters is honoured"""
     P = cfg(2)
