@@ -44,6 +44,9 @@ def lib() -> ctypes.CDLL:
         L.oracle_build_rows.restype = ctypes.c_int
         L.oracle_build_rows.argtypes = [ctypes.c_int, ip, ip, dp, dp, dp, ctypes.c_int, ctypes.c_long,
                                         ctypes.POINTER(ctypes.c_long), dp]
+        L.oracle_normal_velocity_sums.restype = ctypes.c_int
+        L.oracle_normal_velocity_sums.argtypes = [ctypes.c_int, ip, dp, dp, dp, dp, ctypes.c_long,
+                                                  ctypes.POINTER(ctypes.c_long), dp]
         L.oracle_matvec.argtypes = [ctypes.c_long, dp, ctypes.c_long, dp, dp]
         L.oracle_matvec_rect.argtypes = [ctypes.c_long, ctypes.c_long, dp, ctypes.c_long, dp, dp]
         L.oracle_gmres.restype = ctypes.c_int
@@ -112,6 +115,37 @@ def build_rows(counts, kinds, zeta, dzeta, d2zeta, rows, variant: int = 0) -> np
     if rc != 0:
         raise ValueError(f"oracle_build_rows failed: {rc}")
     return out
+
+
+def hilbert(f: np.ndarray) -> np.ndarray:
+    """Periodic Hilbert transform of Eq. (3.22) on equispaced samples, by the FFT with the symbol
+    -i sgn(k); the Nyquist mode of an even-length sample has no sign and is dropped."""
+    f = np.asarray(f, dtype=np.float64)
+    M = f.size
+    k = np.fft.fftfreq(M, d=1.0 / M)
+    sym = -1j * np.sign(k)
+    if M % 2 == 0:
+        sym[M // 2] = 0.0
+    return np.real(np.fft.ifft(sym * np.fft.fft(f)))
+
+
+def normal_velocity(counts, zeta, dzeta, d2zeta, domega, rows=None) -> np.ndarray:
+    """s_alpha * dphi~/dn on Gamma_0 at the listed nodes (default: all) from the derivatives omega' of the densities:
+    the sum of Eq. (3.19) over the solids and Eq. (3.24),
+        -1/2 H omega'_0  -  G+_00 omega'_0  +  sum_j K+_j0 omega'_j,
+    WITHOUT the phi_mv term (3.17).  Hilbert transform by FFT, the integrals by the trapezoidal rule."""
+    counts = np.ascontiguousarray(counts, dtype=np.int32)
+    n, M0 = int(counts.sum()), int(counts[0])
+    z, dz, d2z = _c128_as_f64(zeta), _c128_as_f64(dzeta), _c128_as_f64(d2zeta)
+    w = np.ascontiguousarray(domega, dtype=np.float64)
+    assert w.size == n
+    rows = np.arange(M0, dtype=np.int64) if rows is None else np.ascontiguousarray(rows, dtype=np.int64)
+    out = np.empty(rows.size, dtype=np.float64)
+    rc = lib().oracle_normal_velocity_sums(int(counts.size), _ip(counts), _dp(z), _dp(dz), _dp(d2z), _dp(w), rows.size,
+                                           rows.ctypes.data_as(ctypes.POINTER(ctypes.c_long)), _dp(out))
+    if rc != 0:
+        raise ValueError(f"oracle_normal_velocity_sums failed: {rc}")
+    return out - 0.5 * hilbert(w[:M0])[rows]
 
 
 def matvec(A: np.ndarray, x: np.ndarray) -> np.ndarray:

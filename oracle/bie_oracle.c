@@ -16,6 +16,8 @@
  *                      and E_m = M_m^{-1} e e^T.
  *                     variant 2: the vortex-sheet system of Eqs. (4.14) + (4.17) with the adjoint
  *                     matrices K+, G+ of Eq. (4.7); its solid-solid block is Eq. (4.5).
+ *   oracle_normal_velocity_sums   the trapezoid sums of Eqs. (3.19) and (3.24) for the normal velocity on
+ *                     Gamma_0 (Section 3.4); the FFT Hilbert transform is added in Python.
  *   oracle_matvec     y = A x, the plain definition (long-double accumulation).
  *   oracle_gmres      restarted GMRES(m) of Saad & Schultz (ref. [38] cited at PAPER.md:L855), modified
  *                     Gram-Schmidt + Givens rotations, x0 = 0, stop when the recurrence residual
@@ -32,6 +34,7 @@
  */
 #include <math.h>
 #include <stdlib.h>
+#define ORACLE_PI 3.14159265358979323846264338327950288
 #include <string.h>
 #ifdef _OPENMP
 #include <omp.h>
@@ -231,6 +234,59 @@ int oracle_build_rows(int ncomp, const int *counts, const int *kinds,
         else oracle_row(rows[i], n, comp, counts, kinds, zeta, dzeta, d2zeta, variant, out + i * n);
     }
     free(comp);
+    return 0;
+}
+
+/* NEXT-2: the trapezoid sums of the normal velocity on the free surface, Section 3.4, for the
+ * listed nodes m of Gamma_0 (component 0).  With w = omega' (the derivatives of the densities, all components
+ * concatenated) the function returns, per listed node,
+ *      out = - (1/M_0) sum_l G_00(alpha_l, alpha_m) w_0[l]  +  sum_{j>=1} (1/M_j) sum_l K_j0(alpha_jl, alpha_m) w_j[l],
+ * i.e. the integral of Eq. (3.24) and the integrals of Eq. (3.19) on the
+ * trapezoidal rule ("which we evaluate with spectral accuracy using the trapezoidal rule").  The
+ * integration variable is in the FIRST slot of the kernels: with Table 1
+ *      K_j0(beta, alpha) = Im{ zeta'_0(alpha)/2 cot((zeta_0(alpha) - zeta_j(beta))/2) },
+ *      G_00(beta, alpha) = Re{ zeta'_0(alpha)/2 cot((zeta_0(alpha) - zeta_0(beta))/2) } - 1/2 cot((alpha - beta)/2),
+ * and G_00(alpha, alpha) = Re{zeta''_0/(2 zeta'_0)} (the bracket of Eq. (3.23) tends to -zeta''/(2 zeta')).
+ * The Hilbert-transform term -1/2 H omega'_0 of Eq. (3.24) and the phi_mv term (3.17) are NOT included here: the
+ * caller adds them (FFT, symbol -i sgn k).  Returns 0, or < 0 on bad arguments. */
+int oracle_normal_velocity_sums(int ncomp, const int *counts, const double *zeta, const double *dzeta,
+                                const double *d2zeta, const double *w, long nrows, const long *rows, double *out)
+{
+    if (ncomp < 1 || !counts || !zeta || !dzeta || !d2zeta || !w || !rows || !out) return -1;
+    long n = 0;
+    for (int c = 0; c < ncomp; ++c) { if (counts[c] < 1) return -2; n += counts[c]; }
+    const long M0 = counts[0];
+    for (long i = 0; i < nrows; ++i) if (rows[i] < 0 || rows[i] >= M0) return -3;
+#pragma omp parallel for schedule(static)
+    for (long i = 0; i < nrows; ++i) {
+        const long m = rows[i];
+        const double ur = 0.5 * dzeta[2 * m], ui = 0.5 * dzeta[2 * m + 1]; /* zeta'_0(alpha_m)/2 */
+        const double alpha_m = 2.0 * ORACLE_PI * (double)m / (double)M0;
+        long double acc = 0.0L;
+        long s = 0;
+        for (int j = 0; j < ncomp; ++j) {
+            const double Mj = (double)counts[j];
+            for (long l = 0; l < counts[j]; ++l, ++s) {
+                double e;
+                if (s == m) { /* j = 0, beta = alpha: G_00(alpha, alpha) */
+                    double ar = d2zeta[2 * s], ai = d2zeta[2 * s + 1], br = dzeta[2 * s], bi = dzeta[2 * s + 1];
+                    e = -((ar * br + ai * bi) / (br * br + bi * bi)) / 2.0;
+                } else {
+                    double cr, ci;
+                    oracle_cot_half(zeta[2 * m] - zeta[2 * s], zeta[2 * m + 1] - zeta[2 * s + 1], &cr, &ci);
+                    const double cre = ur * cr - ui * ci, cim = ur * ci + ui * cr;
+                    if (j == 0) {
+                        const double beta_l = 2.0 * ORACLE_PI * (double)l / (double)M0;
+                        e = -(cre - 0.5 / tan(0.5 * (alpha_m - beta_l)));
+                    } else {
+                        e = cim;
+                    }
+                }
+                acc += (long double)(e / Mj) * (long double)w[s];
+            }
+        }
+        out[i] = (double)acc;
+    }
     return 0;
 }
 

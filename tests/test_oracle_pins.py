@@ -519,3 +519,77 @@ def test_p8_auxiliary_system_is_well_conditioned_and_converges_like_the_paper():
     rhs = np.cos(np.arange(aux.shape[0]) * 0.01) + 0.3
     x, iters, relres, hist, status = oracle.gmres(aux, rhs, 1e-13, 50, 500)
     assert status == 0 and 8 <= iters <= 60 and relres < 1e-12
+
+
+# --------------------------------------------------------------------------------------------
+# P9  normal velocity on the free surface (NEXT-2): Eqs. (3.19) + (3.24), Section 3.4
+# --------------------------------------------------------------------------------------------
+def _spectral_derivative(f):
+    M = f.size
+    k = np.fft.fftfreq(M, d=1.0 / M)
+    if M % 2 == 0:
+        k[M // 2] = 0.0
+    return np.real(np.fft.ifft(1j * k * np.fft.fft(f)))
+
+
+def test_p9_hilbert_transform_symbol():
+    """Eq. (3.22) (PAPER.md:L357): H cos(k.) = sin(k.), H sin(k.) = -cos(k.), H 1 = 0 (symbol -i sgn k, PAPER.md:L365);
+    and against the principal-value integral itself by the alternating-point trapezoid rule."""
+    for M in (64, 45):
+        a = 2 * np.pi * np.arange(M) / M
+        for k in (1, 3, 11):
+            assert np.max(np.abs(oracle.hilbert(np.cos(k * a)) - np.sin(k * a))) < 1e-13
+            assert np.max(np.abs(oracle.hilbert(np.sin(k * a)) + np.cos(k * a))) < 1e-13
+        assert np.max(np.abs(oracle.hilbert(np.ones(M)))) < 1e-15
+    M = 64
+    a = 2 * np.pi * np.arange(M) / M
+    f = np.exp(np.cos(a)) * np.sin(2 * a)
+    m = 5
+    odd = (np.arange(M) - m) % 2 == 1    # PV integral (1/pi) int 1/2 cot((a_m - b)/2) f(b) db on the staggered points
+    pv = (2.0 / M) * np.sum(f[odd] / np.tan(0.5 * (a[m] - a[odd])))
+    assert abs(oracle.hilbert(f)[m] - pv) < 1e-12
+
+
+def test_p9_flat_surface_closed_forms():
+    """zeta_0 = a: G_00 (regularised) vanishes identically, so Eq. (3.24) is -1/2 H omega'_0; flat bottom at -H:
+    K_10(beta, alpha) = Im{1/2 cot((alpha - beta + iH)/2)} = -1/2 - sum_k e^{-kH} cos k(alpha - beta), hence
+    K+_10 cos(p.) = -1/2 e^{-pH} cos(p.) and K+_10 1 = -1/2 (Fourier series of cot in the upper half plane)."""
+    M0, M1, H, p = 64, 48, 1.3, 3
+    geo = inputs.flat_flat(M0, M1, H)
+    a0 = 2 * np.pi * np.arange(M0) / M0
+    a1 = 2 * np.pi * np.arange(M1) / M1
+    w = np.concatenate([np.sin(2 * a0), np.zeros(M1)])
+    u = oracle.normal_velocity(geo.counts, geo.zeta, geo.dzeta, geo.d2zeta, w)
+    assert np.max(np.abs(u - 0.5 * np.cos(2 * a0))) < 1e-14           # -1/2 H sin(2.) = +1/2 cos(2.)
+    w = np.concatenate([np.zeros(M0), np.cos(p * a1) + 0.7])
+    u = oracle.normal_velocity(geo.counts, geo.zeta, geo.dzeta, geo.d2zeta, w)
+    assert np.max(np.abs(u - (-0.5 * np.exp(-p * H) * np.cos(p * a0) - 0.35))) < 1e-14
+
+
+def test_p9_normal_velocity_of_a_known_potential_flow():
+    """End-to-end pin of Section 3.4 (signs, the side of the Plemelj limit, the first-slot convention of K_j0(beta, alpha),
+    the regularisation of G_00 and its diagonal, the weights 1/M_j): for f analytic in the fluid, solve (3.16) with
+    b_0 = Re f, b_k = Im f (pin P3: then sum_j Phi_j = f, i.e. phi~ = Re f in the fluid), differentiate the densities
+    spectrally, and compare  s_alpha d phi~/dn = Re{ f'(zeta_0) i zeta_0' }  (first line of Eq. (3.19))
+    with the oracle's normal velocity.  Converges spectrally: checked at two resolutions."""
+    def fprime(z):
+        csc2 = lambda w: 1.0 / np.sin(w) ** 2
+        return (1j * np.exp(1j * z) - 0.15 * csc2(0.5 * (z - (1.0 + 0.6j)))
+                - 0.5 * (0.1 + 0.04j) * csc2(0.5 * (z - (-1.0j))) - 0.05j * csc2(0.5 * (z - (2.0 - 2.6j))))
+
+    errs = []
+    for scale in (1, 2):
+        g = inputs.small_problem(96 * scale, 96 * scale, [64 * scale], seed=3).geometry
+        # derivative of _f_poles, checked against a centred difference first
+        z0 = 0.7 - 0.9j
+        assert abs((_f_poles(z0 + 1e-6) - _f_poles(z0 - 1e-6)) / 2e-6 - fprime(z0)) < 1e-8
+        b = inputs.rhs_analytic(g, _f_poles)
+        A = _build(g)
+        x, iters, relres, hist, status = oracle.gmres(A, b, 1e-14, 80, 600)
+        assert status == 0
+        dom = np.concatenate([_spectral_derivative(x[g.component(k)]) for k in range(g.counts.size)])
+        u = oracle.normal_velocity(g.counts, g.zeta, g.dzeta, g.d2zeta, dom)
+        s0 = g.component(0)
+        exact = np.real(fprime(g.zeta[s0]) * 1j * g.dzeta[s0])
+        errs.append(np.max(np.abs(u - exact)) / np.max(np.abs(exact)))
+    assert errs[1] < 1e-9 and errs[1] < errs[0] * 1e-2 or errs[0] < 1e-11, errs
