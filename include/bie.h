@@ -144,6 +144,29 @@ int bie_set_geometry(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32
 int bie_matvec(bie_ctx* ctx, int n, const double* A, int64_t lda, const double* x, double* y, void* stream);
 int bie_matvec_free(bie_ctx* ctx, int n, const double* x, double* y, void* stream);
 
+/* y (nrows) = A (nrows x ncols, row-major, lda >= ncols even) x (ncols): the same HBM-bound kernel on a rectangular block. */
+int bie_matvec_rect(bie_ctx* ctx, int nrows, int ncols, const double* A, int64_t lda, const double* x, double* y,
+                    void* stream);
+
+/* ---------------------------------------------------------------------------------------------------
+ * (b') Normal velocity on the free surface after the solve, Section 3.4, SURVEY 8(f) NEXT-2.
+ * Writes the M_0 x n matrix Nmat (row-major, lda >= n even) with
+ *      s_alpha d phi~/dn (alpha_m) = sum_s Nmat[m][s] omega'[s]
+ *                                  = -1/2 H omega'_0 - G+_00 omega'_0 + sum_{j>=1} K+_j0 omega'_j     (Eqs. 3.24 + 3.19),
+ * omega' = the derivatives of the densities (all components concatenated; the caller differentiates, e.g. by FFT).
+ * Row m on Gamma_0, column (j,l):  c+ = zeta'_0[m]/(2 M_j) cot((zeta_0[m] - zeta_j[l])/2)   (integration variable in
+ * the first slot of the kernels):
+ *      j >= 1 :  Im c+                                                         (K_j0(alpha_jl, alpha_m)/M_j)
+ *      j = 0  : -Re c+ + kappa_{m-l},  diagonal -Re{zeta''_0/(2 zeta'_0)}/M_0   (-G_00(alpha_l, alpha_m)/M_0 - 1/2 H)
+ * where kappa_d carries the regulariser 1/2 cot((alpha - beta)/2) of G_00 (Table 1) and -1/2 of the
+ * Hilbert transform of Eq. (3.22) in its exact discrete form (symbol -i sgn k, Nyquist mode dropped):
+ *      kappa_d = (-1)^d cot(pi d/M_0)/(2 M_0)  (M_0 even),   (-1)^d/(2 M_0 sin(pi d/M_0))  (M_0 odd),   kappa_0 = 0.
+ * The phi_mv term (3.17) is pointwise input data and is not included.  Apply with bie_matvec_rect(M_0, n, ...).
+ * The call replaces the ctx's node tables (call bie_set_geometry / bie_build again before a matrix-free solve). */
+int bie_build_normal_velocity(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds,
+                              const double* zeta, const double* dzeta, const double* d2zeta,
+                              double* Nmat, int64_t lda, void* stream);
+
 /* ---------------------------------------------------------------------------------------------------
  * (c) Restarted GMRES(restart), SURVEY 8(a) rows a5-a10 (Saad & Schultz, ref. [38] cited at
  * PAPER.md:L855), unpreconditioned, x0 = 0, on the system as stored:

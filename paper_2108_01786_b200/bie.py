@@ -23,7 +23,7 @@ _lib: Optional[ctypes.CDLL] = None
 EXPORTS = ("bie_create", "bie_destroy", "bie_strerror", "bie_device_info", "bie_build", "bie_build_update",
            "bie_set_geometry", "bie_matvec", "bie_matvec_free", "bie_gmres_workspace_bytes", "bie_gmres",
            "bie_solve_workspace_bytes", "bie_solve_host", "bie_probe_dfma", "bie_build_cols", "bie_hybrid_cols",
-           "bie_set_hybrid_free_warps", "bie_gmres_hybrid")
+           "bie_set_hybrid_free_warps", "bie_gmres_hybrid", "bie_matvec_rect", "bie_build_normal_velocity")
 
 BIE_OK, BIE_MAX_ITERS = 0, 1
 OP_DENSE, OP_FREE, OP_HYBRID = 0, 1, 2
@@ -82,6 +82,10 @@ def lib() -> ctypes.CDLL:
         L.bie_set_hybrid_free_warps.argtypes = [vp, i32]
         L.bie_gmres_hybrid.restype = i32
         L.bie_gmres_hybrid.argtypes = [vp, i32, vp, i64, i32, vp, dbl, i32, i32, vp, vp, vp, vp, vp, vp, sz, vp]
+        L.bie_matvec_rect.restype = i32
+        L.bie_matvec_rect.argtypes = [vp, i32, i32, vp, i64, vp, vp, vp]
+        L.bie_build_normal_velocity.restype = i32
+        L.bie_build_normal_velocity.argtypes = geo[:-1] + [vp, i64, vp]
         L.bie_probe_dfma.restype = i32
         L.bie_probe_dfma.argtypes = [vp, i64, vp, ctypes.POINTER(i64), vp]
         _lib = L
@@ -197,6 +201,23 @@ class Context:
         _check(lib().bie_matvec(self._h, n, _dev_f64(A, (n - 1) * lda + n), lda, _dev_f64(x, n), _dev_f64(y, n),
                                 _stream()), "bie_matvec")
         return y
+
+    def bie_matvec_rect(self, A, x, y, lda: Optional[int] = None):
+        """y (nrows = y.numel()) = A (nrows x ncols, ncols = x.numel()) x"""
+        nrows, ncols = y.numel(), x.numel()
+        lda = int(lda if lda is not None else A.stride(0))
+        _check(lib().bie_matvec_rect(self._h, nrows, ncols, _dev_f64(A, (nrows - 1) * lda + ncols), lda, _dev_f64(x, ncols),
+                                     _dev_f64(y, nrows), _stream()), "bie_matvec_rect")
+        return y
+
+    def bie_build_normal_velocity(self, counts, kinds, zeta, dzeta, d2zeta, Nmat, lda: Optional[int] = None):
+        """Nmat (CUDA float64, M_0 x lda, lda >= n) <- the normal-velocity operator of Section 3.4 (Eqs. 3.19 + 3.24)."""
+        n, args, keep = self._geo(counts, kinds, zeta, dzeta, d2zeta, 0)
+        M0 = int(keep[0][0])
+        lda = int(lda if lda is not None else Nmat.stride(0))
+        _dev_f64(Nmat, (M0 - 1) * lda + n)
+        _check(lib().bie_build_normal_velocity(*args[:-1], Nmat.data_ptr(), lda, _stream()), "bie_build_normal_velocity")
+        return Nmat
 
     def bie_matvec_free(self, x, y):
         n = x.numel()

@@ -28,7 +28,7 @@ int bie_create(bie_ctx** out, int device)
     c->sync_buf = nullptr; c->pinned_i = nullptr; c->pinned_d = nullptr;
     c->near_ptr = nullptr; c->near_col = nullptr; c->near_val = nullptr; c->near_valid = 0;
     c->hybrid_free_warps = BIE_HYBRID_FREE_WARPS;
-    c->taubar = nullptr; c->near_overflow = nullptr;
+    c->taubar = nullptr; c->near_overflow = nullptr; c->kappa = nullptr;
     if (cudaMalloc((void**)&c->sync_buf, 256) != cudaSuccess ||
         cudaMallocHost((void**)&c->pinned_i, 4 * sizeof(int32_t)) != cudaSuccess ||
         cudaMallocHost((void**)&c->pinned_d, 4 * sizeof(double)) != cudaSuccess) {
@@ -55,6 +55,7 @@ int bie_destroy(bie_ctx* c)
     if (c->near_ptr) cudaFree(c->near_ptr);
     if (c->near_col) cudaFree(c->near_col);
     if (c->near_val) cudaFree(c->near_val);
+    if (c->kappa) cudaFree(c->kappa);
     if (c->sync_buf) cudaFree(c->sync_buf);
     if (c->pinned_i) cudaFreeHost(c->pinned_i);
     if (c->pinned_d) cudaFreeHost(c->pinned_d);
@@ -90,6 +91,7 @@ int bie_set_geometry(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t
                      const double* dzeta, const double* d2zeta, int variant, void* stream)
 {
     if (!c) return BIE_ERR_NULL;
+    if (variant < BIE_VARIANT_A || variant > BIE_VARIANT_VORTEX) return BIE_ERR_ARG;
     BIE_CUDA(cudaSetDevice(c->device));
     return bie_prepare_nodes(c, ncomp, counts, kinds, zeta, dzeta, d2zeta, variant, (cudaStream_t)stream);
 }
@@ -97,6 +99,7 @@ int bie_set_geometry(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t
 int bie_build(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* kinds, const double* zeta,
               const double* dzeta, const double* d2zeta, int variant, double* A, int64_t lda, void* stream)
 {
+    if (variant < BIE_VARIANT_A || variant > BIE_VARIANT_VORTEX) return BIE_ERR_ARG;
     if (!c || !A) return BIE_ERR_NULL;
     BIE_CUDA(cudaSetDevice(c->device));
     int rc = bie_prepare_nodes(c, ncomp, counts, kinds, zeta, dzeta, d2zeta, variant, (cudaStream_t)stream);
@@ -107,6 +110,7 @@ int bie_build(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* kinds
 int bie_build_update(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* kinds, const double* zeta,
                      const double* dzeta, const double* d2zeta, int variant, double* A, int64_t lda, void* stream)
 {
+    if (variant < BIE_VARIANT_A || variant > BIE_VARIANT_VORTEX) return BIE_ERR_ARG;
     if (!c || !A) return BIE_ERR_NULL;
     BIE_CUDA(cudaSetDevice(c->device));
     int rc = bie_prepare_nodes(c, ncomp, counts, kinds, zeta, dzeta, d2zeta, variant, (cudaStream_t)stream);
@@ -117,6 +121,7 @@ int bie_build_update(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t
 int bie_build_cols(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* kinds, const double* zeta,
                    const double* dzeta, const double* d2zeta, int variant, int ncols, double* A, int64_t lda, void* stream)
 {
+    if (variant < BIE_VARIANT_A || variant > BIE_VARIANT_VORTEX) return BIE_ERR_ARG;
     if (!c || !A) return BIE_ERR_NULL;
     BIE_CUDA(cudaSetDevice(c->device));
     int rc = bie_prepare_nodes(c, ncomp, counts, kinds, zeta, dzeta, d2zeta, variant, (cudaStream_t)stream);
@@ -147,7 +152,26 @@ int bie_matvec(bie_ctx* c, int n, const double* A, int64_t lda, const double* x,
 {
     if (!c) return BIE_ERR_NULL;
     BIE_CUDA(cudaSetDevice(c->device));
-    return bie_launch_matvec(c, n, A, lda, x, y, (cudaStream_t)stream);
+    return bie_launch_matvec(c, n, n, A, lda, x, y, (cudaStream_t)stream);
+}
+
+int bie_matvec_rect(bie_ctx* c, int nrows, int ncols, const double* A, int64_t lda, const double* x, double* y,
+                    void* stream)
+{
+    if (!c) return BIE_ERR_NULL;
+    BIE_CUDA(cudaSetDevice(c->device));
+    return bie_launch_matvec(c, nrows, ncols, A, lda, x, y, (cudaStream_t)stream);
+}
+
+int bie_build_normal_velocity(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* kinds, const double* zeta,
+                              const double* dzeta, const double* d2zeta, double* Nmat, int64_t lda, void* stream)
+{
+    if (!c || !Nmat) return BIE_ERR_NULL;
+    BIE_CUDA(cudaSetDevice(c->device));
+    int rc = bie_prepare_nodes(c, ncomp, counts, kinds, zeta, dzeta, d2zeta, BIE_VARIANT_NORMAL_INTERNAL,
+                               (cudaStream_t)stream);
+    if (rc != BIE_OK) return rc;
+    return bie_launch_build(c, Nmat, lda, c->n, 0, (cudaStream_t)stream);
 }
 
 int bie_matvec_free(bie_ctx* c, int n, const double* x, double* y, void* stream)

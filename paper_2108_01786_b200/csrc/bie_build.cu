@@ -159,13 +159,14 @@ __device__ __forceinline__ double bie_entry_fast_dagger(const SrcColD& s, const 
 }
 
 __global__ void __launch_bounds__(BUILD_THREADS)
-bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long lda, int T, int only0, int ncols)
+bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long lda, int T, int only0, int ncols,
+                        const double* __restrict__ kappa /* NULL: vortex-sheet S; else the normal-velocity operator */)
 {
     extern __shared__ __align__(16) double2 sm[];  // [T] E_t, [T] (A,B) for columns on Gamma_0, [T] (A,B) for solids, [T] M_t
     const int n = nt.n;
     const int c0 = blockIdx.x * BUILD_TILE_W;
     const int t0 = blockIdx.y * T;
-    const int t1 = min(t0 + T, n);
+    const int t1 = min(t0 + T, kappa ? ct.off[1] : n);   // the normal-velocity operator has rows on Gamma_0 only
     if (only0 && t0 >= ct.off[1] && c0 >= ct.off[1]) return;
     double2* sE = sm;
     double2* sAB0 = sm + T;
@@ -180,12 +181,14 @@ bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long
         sE[i] = nt.E[t];
         sM[i] = nt.MT[t].x;
         const double2 im = make_double2(2.0 * ui, -ur);
-        if (k == 0) { sAB0[i] = im; sAB1[i] = make_double2(-2.0 * ur, -ui); }   // K+_00 ; -G+_j0
-        else        { sAB0[i] = make_double2(2.0 * ur, ui); sAB1[i] = im; }      // G+_0k ; K+_jk
+        if (kappa)       { sAB0[i] = make_double2(-2.0 * ur, -ui); sAB1[i] = im; }  // -G+_00 (3.24) ; K+_j0 (3.19)
+        else if (k == 0) { sAB0[i] = im; sAB1[i] = make_double2(-2.0 * ur, -ui); }  // K+_00 ; -G+_j0
+        else             { sAB0[i] = make_double2(2.0 * ur, ui); sAB1[i] = im; }     // G+_0k ; K+_jk
     }
     const int s0 = c0 + BUILD_COLS * threadIdx.x;  // < npad by construction
     SrcColD src[BUILD_COLS];
     const double2* sAB[BUILD_COLS];
+    bool kap[BUILD_COLS];
 #pragma unroll
     for (int c = 0; c < BUILD_COLS; ++c) {
         const double2 e = nt.E[s0 + c], mt = nt.MT[s0 + c];
@@ -195,7 +198,9 @@ bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long
         src[c].ser = ms * e.x; src[c].sei = ms * e.y; src[c].sm = ms * mt.x; src[c].ms = ms;
         src[c].thi = __double2hiint(mt.y);
         sAB[c] = (j == 0) ? sAB0 : sAB1;
+        kap[c] = (kappa != nullptr && j == 0);
     }
+    const int M0 = ct.off[1];
     __syncthreads();
     const bool full = (s0 + 1 < ncols);
     const bool part = (s0 < ncols);
@@ -207,8 +212,10 @@ bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long
             const int t = min(tb + r, t1 - 1);  // the tail repeats the last row (same values, same address)
             const double2 te = sE[t - t0];
             const double tm = sM[t - t0];
-            const double e0 = bie_entry_fast_dagger(src[0], te, tm, sAB[0][t - t0], flag);
-            const double e1 = bie_entry_fast_dagger(src[1], te, tm, sAB[1][t - t0], flag);
+            double e0 = bie_entry_fast_dagger(src[0], te, tm, sAB[0][t - t0], flag);
+            double e1 = bie_entry_fast_dagger(src[1], te, tm, sAB[1][t - t0], flag);
+            if (kap[0]) { const int d = t - s0;     e0 += __ldg(kappa + (d < 0 ? d + M0 : d)); }
+            if (kap[1]) { const int d = t - s0 - 1; e1 += __ldg(kappa + (d < 0 ? d + M0 : d)); }
             double* p = row + (long long)(t - tb) * lda;
             if (full) *reinterpret_cast<double2*>(p) = make_double2(e0, e1);
             else if (part) p[0] = e0;
@@ -226,8 +233,9 @@ bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long
                         if (__double2hiint(den) < src[c].thi) {
                             const double2 ab = sAB[c][t - t0];
                             // (A X' + B Y')/den with cot = (-2X + iY)/den; the diagonal entry is prepared per node
-                            A[(long long)t * lda + s0 + c] =
-                                bie_entry_near(nt.DG, nt.XY, src[c].ms * ab.x, src[c].ms * ab.y, 0.0, s0 + c, t);
+                            double v = bie_entry_near(nt.DG, nt.XY, src[c].ms * ab.x, src[c].ms * ab.y, 0.0, s0 + c, t);
+                            if (kap[c]) { const int d = t - s0 - c; v += __ldg(kappa + (d < 0 ? d + M0 : d)); }
+                            A[(long long)t * lda + s0 + c] = v;
                         }
                     }
                 }
@@ -247,12 +255,18 @@ int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int ncols, int only_c
     const NodeTable nt = bie_node_table(ctx);
     const int gx = (ncols + BUILD_TILE_W - 1) / BUILD_TILE_W;
     // rows per CTA: 128 when that still gives every SM several CTAs, else smaller
+    int nt_rows = n;
     int T = 128;
     while (T > 8 && (long long)gx * ((n + T - 1) / T) < 4LL * ctx->sm_count) T >>= 1;
-    dim3 grid(gx, (n + T - 1) / T);
-    if (ctx->variant == BIE_VARIANT_VORTEX) {
+    if (ctx->variant == BIE_VARIANT_NORMAL_INTERNAL) {   // M_0 x n: rows on Gamma_0 only
+        const int M0 = ctx->counts[0];
+        nt_rows = M0;
+    }
+    dim3 grid(gx, (nt_rows + T - 1) / T);
+    if (ctx->variant == BIE_VARIANT_VORTEX || ctx->variant == BIE_VARIANT_NORMAL_INTERNAL) {
         bie_build_dagger_kernel<<<grid, BUILD_THREADS, (3 * sizeof(double2) + sizeof(double)) * T + 16, st>>>(
-            nt, ctx->comps, A, (long long)lda, T, only_comp0, ncols);
+            nt, ctx->comps, A, (long long)lda, T, only_comp0, ncols,
+            ctx->variant == BIE_VARIANT_NORMAL_INTERNAL ? ctx->kappa : nullptr);
         BIE_CUDA(cudaGetLastError());
         return BIE_OK;
     }

@@ -19,6 +19,7 @@
 #include "../../include/bie.h"
 
 #define BIE_MAX_COMP 64
+#define BIE_VARIANT_NORMAL_INTERNAL 3  // node tables for bie_build_normal_velocity (not a bie_build variant)
 #define BIE_NODE_PAD 256              // node tables are padded to a multiple of the build tile width
 #define BIE_NEAR_C 0.25               // tau_s = BIE_NEAR_C |q_s|  (fast-path entry error <= ~1e-14)
 #define BIE_NEAR_TAU_MIN 1.0e-9
@@ -62,6 +63,7 @@ struct bie_ctx {
     double* near_val;        // [BIE_NEAR_PER_NODE cap]
     int* near_overflow;      // device flag: the near matrix did not fit (the operator then returns NaN)
     int near_valid;          // near matrix built for the current geometry
+    double* kappa;           // [cap] real-cot table of the normal-velocity operator (bie_build_normal_velocity)
     int hybrid_free_warps;   // hybrid operator: warps per CTA on the pair loops (the other 16 - this stream the slab)
     unsigned int* sync_buf;  // grid-barrier counter
     int cap;
@@ -99,7 +101,8 @@ int bie_prepare_nodes(bie_ctx* ctx, int ncomp, const int32_t* counts, const int3
                       const double* zeta, const double* dzeta, const double* d2zeta, int variant,
                       cudaStream_t st);
 int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int ncols, int only_comp0, cudaStream_t st);
-int bie_launch_matvec(bie_ctx* ctx, int n, const double* A, int64_t lda, const double* x, double* y, cudaStream_t st);
+int bie_launch_matvec(bie_ctx* ctx, int nrows, int n, const double* A, int64_t lda, const double* x, double* y,
+                      cudaStream_t st);
 int bie_launch_matvec_free(bie_ctx* ctx, const double* x, double* y, cudaStream_t st);
 int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, int nd, const double* rhs, double tol,
                      int restart, int max_iters, double* x, int32_t* iters_out, double* relres_out,

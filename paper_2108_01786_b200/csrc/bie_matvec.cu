@@ -9,12 +9,12 @@
 
 template <bool STREAM, bool XS>
 __global__ void __launch_bounds__(MV_THREADS, 1)
-bie_matvec_kernel(const double* __restrict__ A, long long lda, int n, int rows_per_cta, int chunk,
+bie_matvec_kernel(const double* __restrict__ A, long long lda, int nrows, int n, int rows_per_cta, int chunk,
                   const double* __restrict__ x, double* __restrict__ y)
 {
     extern __shared__ __align__(16) double smem[];
     const int r0 = blockIdx.x * rows_per_cta;
-    const int r1 = min(r0 + rows_per_cta, n);
+    const int r1 = min(r0 + rows_per_cta, nrows);
     if (r0 >= r1) return;
     double* y_local = smem;
     double* part = y_local + ((rows_per_cta + 1) & ~1);
@@ -31,25 +31,27 @@ bie_matvec_kernel(const double* __restrict__ A, long long lda, int n, int rows_p
 }
 
 template <bool STREAM, bool XS>
-static int launch_mv(bie_ctx* ctx, int n, const double* A, int64_t lda, const double* x, double* y,
+static int launch_mv(bie_ctx* ctx, int nrows, int n, const double* A, int64_t lda, const double* x, double* y,
                      int rows_per_cta, int chunk, size_t smem, cudaStream_t st)
 {
     auto k = bie_matvec_kernel<STREAM, XS>;
     BIE_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    const int grid = (n + rows_per_cta - 1) / rows_per_cta;
-    k<<<grid, MV_THREADS, smem, st>>>(A, (long long)lda, n, rows_per_cta, chunk, x, y);
+    const int grid = (nrows + rows_per_cta - 1) / rows_per_cta;
+    k<<<grid, MV_THREADS, smem, st>>>(A, (long long)lda, nrows, n, rows_per_cta, chunk, x, y);
     BIE_CUDA(cudaGetLastError());
     (void)ctx;
     return BIE_OK;
 }
 
-int bie_launch_matvec(bie_ctx* ctx, int n, const double* A, int64_t lda, const double* x, double* y, cudaStream_t st)
+// y (nrows) = A (nrows x n, row-major, lda) x (n)
+int bie_launch_matvec(bie_ctx* ctx, int nrows, int n, const double* A, int64_t lda, const double* x, double* y,
+                      cudaStream_t st)
 {
     if (!ctx || !A || !x || !y) return BIE_ERR_NULL;
-    if (n < 1) return BIE_ERR_ARG;
+    if (n < 1 || nrows < 1) return BIE_ERR_ARG;
     if (lda < n || (lda & 1) || ((((uintptr_t)A) | ((uintptr_t)x) | ((uintptr_t)y)) & 15u)) return BIE_ERR_LAYOUT;
     const int G = ctx->sm_count;
-    const int rows_per_cta = (n + G - 1) / G;
+    const int rows_per_cta = (nrows + G - 1) / G;
     const int chunk = gemv_chunk(rows_per_cta, n, MV_THREADS / 32);
     const size_t base = sizeof(double) * (((rows_per_cta + 1) & ~1) + gemv_part_doubles(rows_per_cta, n, chunk));
     const bool xs = base + sizeof(double) * ((size_t)n + 2) <= (size_t)ctx->max_smem_optin;
@@ -57,11 +59,11 @@ int bie_launch_matvec(bie_ctx* ctx, int n, const double* A, int64_t lda, const d
     if (smem > (size_t)ctx->max_smem_optin) return BIE_ERR_ARG;
     // matrices that cannot stay in L2 are streamed (evict-first) so that they do not displace x, y and
     // the Krylov basis; smaller ones are read with the default policy and stay L2-resident between calls
-    const bool stream = (double)n * (double)lda * 8.0 > 0.6 * (double)ctx->l2_bytes;
-    if (stream) return xs ? launch_mv<true, true>(ctx, n, A, lda, x, y, rows_per_cta, chunk, smem, st)
-                          : launch_mv<true, false>(ctx, n, A, lda, x, y, rows_per_cta, chunk, smem, st);
-    return xs ? launch_mv<false, true>(ctx, n, A, lda, x, y, rows_per_cta, chunk, smem, st)
-              : launch_mv<false, false>(ctx, n, A, lda, x, y, rows_per_cta, chunk, smem, st);
+    const bool stream = (double)nrows * (double)lda * 8.0 > 0.6 * (double)ctx->l2_bytes;
+    if (stream) return xs ? launch_mv<true, true>(ctx, nrows, n, A, lda, x, y, rows_per_cta, chunk, smem, st)
+                          : launch_mv<true, false>(ctx, nrows, n, A, lda, x, y, rows_per_cta, chunk, smem, st);
+    return xs ? launch_mv<false, true>(ctx, nrows, n, A, lda, x, y, rows_per_cta, chunk, smem, st)
+              : launch_mv<false, false>(ctx, nrows, n, A, lda, x, y, rows_per_cta, chunk, smem, st);
 }
 
 // ---------------------------------------------------------------------------------------------------

@@ -18,7 +18,7 @@ __global__ void __launch_bounds__(256)
 bie_prepare_nodes_kernel(PrepArgs pa, int n, int npad, int variant,
                          const double2* __restrict__ zeta, const double2* __restrict__ dzeta,
                          const double2* __restrict__ d2zeta, double2* __restrict__ buf, int* __restrict__ comp,
-                         double2* __restrict__ T, double* __restrict__ taubar)
+                         double2* __restrict__ T, double* __restrict__ taubar, double* __restrict__ kappa)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= npad) return;
@@ -56,7 +56,23 @@ bie_prepare_nodes_kernel(PrepArgs pa, int n, int npad, int variant,
     double d = (d2.y * dz.x - d2.x * dz.y) / den / (2.0 * M);
     const double em = (variant == BIE_VARIANT_A && pa.kinds[k] == BIE_KIND_OBSTACLE) ? 1.0 / M : 0.0;
     // -1/2 I + K_00, 1/2 I + K_kk (Eq. 3.10); the vortex-sheet system has 1/2 I + K+_00, -1/2 I + K+_kk (Eqs. 4.14, 4.5)
-    if (variant == BIE_VARIANT_VORTEX) d += (k == 0) ? 0.5 : -0.5;
+    if (variant == BIE_VARIANT_NORMAL_INTERNAL) {
+        // normal-velocity operator (Section 3.4): diagonal -G_00(a,a)/M_0 = -Re{zeta''/(2 zeta')}/M_0,
+        // and the real-cot table kappa_d, d = m - l mod M_0, that carries the regulariser of G_00 and
+        // -1/2 of the discrete Hilbert transform (symbol -i sgn k) together:
+        //   M_0 even: (-1)^d cot(pi d/M_0)/(2 M_0)      M_0 odd: (-1)^d / (2 M_0 sin(pi d/M_0))      kappa_0 = 0
+        d = -(d2.x * dz.x + d2.y * dz.y) / den / (2.0 * M);
+        if (k == 0) {
+            double kv = 0.0;
+            if (i > 0) {
+                const int M0 = pa.comps.off[1];
+                const double sgn = (i & 1) ? -1.0 : 1.0;
+                const double sp = sinpi((double)i / M), cp = cospi((double)i / M);
+                kv = (M0 & 1) ? sgn / (2.0 * M * sp) : sgn * cp / (2.0 * M * sp);
+            }
+            kappa[i] = kv;
+        }
+    } else if (variant == BIE_VARIANT_VORTEX) d += (k == 0) ? 0.5 : -0.5;
     else d += (k == 0) ? -0.5 : 0.5;
     d -= em;
     DG[i] = make_double2(d, em);
@@ -85,7 +101,8 @@ int bie_prepare_nodes(bie_ctx* ctx, int ncomp, const int32_t* counts, const int3
 {
     if (!ctx || !counts || !kinds || !zeta || !dzeta || !d2zeta) return BIE_ERR_NULL;
     if (ncomp < 1 || ncomp > BIE_MAX_COMP) return BIE_ERR_GEOMETRY;
-    if (variant != BIE_VARIANT_A && variant != BIE_VARIANT_B && variant != BIE_VARIANT_VORTEX) return BIE_ERR_ARG;
+    if (variant != BIE_VARIANT_A && variant != BIE_VARIANT_B && variant != BIE_VARIANT_VORTEX &&
+        variant != BIE_VARIANT_NORMAL_INTERNAL) return BIE_ERR_ARG;
     long long n = 0;
     int nbottom = 0;
     for (int c = 0; c < ncomp; ++c) {
@@ -106,6 +123,8 @@ int bie_prepare_nodes(bie_ctx* ctx, int ncomp, const int32_t* counts, const int3
         if (ctx->near_ptr) cudaFree(ctx->near_ptr);
         if (ctx->near_col) cudaFree(ctx->near_col);
         if (ctx->near_val) cudaFree(ctx->near_val);
+        if (ctx->kappa) cudaFree(ctx->kappa);
+        ctx->kappa = nullptr;
         ctx->node_buf = nullptr; ctx->comp_buf = nullptr; ctx->free_buf = nullptr; ctx->cap = 0;
         ctx->near_ptr = nullptr; ctx->near_col = nullptr; ctx->near_val = nullptr;
         BIE_CUDA(cudaMalloc((void**)&ctx->node_buf, sizeof(double) * BIE_NODE_ARRAYS * (size_t)npad));
@@ -114,6 +133,7 @@ int bie_prepare_nodes(bie_ctx* ctx, int ncomp, const int32_t* counts, const int3
         BIE_CUDA(cudaMalloc((void**)&ctx->near_ptr, sizeof(int) * (8 * (size_t)npad + 1)));
         BIE_CUDA(cudaMalloc((void**)&ctx->near_col, sizeof(int) * bie_near_cap(npad)));
         BIE_CUDA(cudaMalloc((void**)&ctx->near_val, sizeof(double) * bie_near_cap(npad)));
+        BIE_CUDA(cudaMalloc((void**)&ctx->kappa, sizeof(double) * (size_t)npad));
         ctx->cap = npad;
     }
     PrepArgs pa;
@@ -133,7 +153,7 @@ int bie_prepare_nodes(bie_ctx* ctx, int ncomp, const int32_t* counts, const int3
     BIE_CUDA(cudaMemsetAsync(ctx->taubar, 0, sizeof(double), st));
     bie_prepare_nodes_kernel<<<(npad + 255) / 256, 256, 0, st>>>(
         pa, (int)n, npad, variant, (const double2*)zeta, (const double2*)dzeta, (const double2*)d2zeta,
-        (double2*)ctx->node_buf, ctx->comp_buf, (double2*)ctx->free_buf, ctx->taubar);
+        (double2*)ctx->node_buf, ctx->comp_buf, (double2*)ctx->free_buf, ctx->taubar, ctx->kappa);
     BIE_CUDA(cudaGetLastError());
     return BIE_OK;
 }

@@ -301,6 +301,82 @@ def test_vortex_variant_is_dense_only(ctx):
 
 
 # ------------------------------------------------------------------------------------------------
+# (b') normal velocity on Gamma_0 (Section 3.4, NEXT-2): matrix of Eqs. (3.19) + (3.24), applied with bie_matvec_rect
+# ------------------------------------------------------------------------------------------------
+def _domega(g, seed):
+    """a smooth omega' per component (zero mean, as a derivative has)"""
+    rng = np.random.default_rng(seed)
+    parts = []
+    for M in g.counts:
+        a = 2 * np.pi * np.arange(M) / M
+        f = sum(rng.standard_normal() * np.cos(k * a + rng.uniform(0, 6.28)) / k for k in range(1, 9))
+        parts.append(f)
+    return np.concatenate(parts)
+
+
+def gpu_normal_velocity(ctx, g, w):
+    n, M0 = g.n, int(g.counts[0])
+    lda = n + (n & 1)
+    N = torch.empty((M0, lda), dtype=torch.float64, device="cuda")
+    z, dz, d2z = geo_dev(g)
+    ctx.bie_build_normal_velocity(g.counts, g.kinds, z, dz, d2z, N)
+    y = torch.empty(M0 + (M0 & 1), dtype=torch.float64, device="cuda")[:M0]
+    ctx.bie_matvec_rect(N, dev(w), y)
+    torch.cuda.synchronize()
+    return y.cpu().numpy(), N
+
+
+@pytest.mark.parametrize("c", [1, 2, 3])
+def test_normal_velocity_parity(ctx, c):
+    g = cfg(c).geometry
+    w = _domega(g, 50 + c)
+    u, N = gpu_normal_velocity(ctx, g, w)
+    uo = oracle.normal_velocity(g.counts, g.zeta, g.dzeta, g.d2zeta, w)
+    assert float(np.max(np.abs(u - uo))) <= 1e-12 * max(1.0, float(np.max(np.abs(uo))))
+    # the matrix entries themselves: unit vectors through the oracle (a few columns of each block, and the diagonal)
+    M0 = int(g.counts[0])
+    Nh = N[:, :g.n].cpu().numpy()
+    for s in [0, 1, M0 // 2, M0 - 1, M0, M0 + 3, g.n - 1]:
+        e = np.zeros(g.n); e[s] = 1.0
+        col = oracle.normal_velocity(g.counts, g.zeta, g.dzeta, g.d2zeta, e)
+        assert float(np.max(np.abs(Nh[:, s] - col))) <= TOL_ENTRY, s
+
+
+@pytest.mark.parametrize("shape", [(37, 29, [19, 23]), (5, 3, []), (2, 1, [1]), (64, 64, [64]), (301, 171, [33, 2, 129])])
+def test_normal_velocity_ragged_and_odd_sizes(ctx, shape):
+    """odd M_0 takes the 1/sin form of the discrete Hilbert kernel"""
+    g = inputs.small_problem(*shape).geometry
+    w = _domega(g, 7)
+    u, N = gpu_normal_velocity(ctx, g, w)
+    uo = oracle.normal_velocity(g.counts, g.zeta, g.dzeta, g.d2zeta, w)
+    assert float(np.max(np.abs(u - uo))) <= 1e-12 * max(1.0, float(np.max(np.abs(uo))))
+
+
+@pytest.mark.parametrize("c", [4, 5])
+def test_normal_velocity_full_size_sampled_rows(ctx, c):
+    g = cfg(c).geometry
+    w = _domega(g, 60 + c)
+    u, N = gpu_normal_velocity(ctx, g, w)
+    M0 = int(g.counts[0])
+    rows = np.unique(np.concatenate([np.random.default_rng(c).integers(0, M0, size=48), [0, 1, M0 - 1]])).astype(np.int64)
+    uo = oracle.normal_velocity(g.counts, g.zeta, g.dzeta, g.d2zeta, w, rows=rows)
+    assert float(np.max(np.abs(u[rows] - uo))) <= 1e-12 * max(1.0, float(np.max(np.abs(uo))))
+    assert np.all(np.isfinite(u))
+    del N
+
+
+def test_matvec_rect_matches_the_oracle(ctx):
+    rng = np.random.default_rng(3)
+    for (nr, nc, lda) in [(1, 2, 2), (7, 130, 132), (300, 64, 64), (129, 1001, 1002)]:
+        A = rng.standard_normal((nr, lda))
+        x = rng.standard_normal(nc)
+        y = torch.empty(nr + (nr & 1), dtype=torch.float64, device="cuda")[:nr]
+        ctx.bie_matvec_rect(dev(A), dev(x), y, lda=lda)
+        yo = oracle.matvec(np.ascontiguousarray(A[:, :nc]), x)
+        assert rel_max(y.cpu().numpy(), yo) <= 1e-13
+
+
+# ------------------------------------------------------------------------------------------------
 # (c) GMRES
 # ------------------------------------------------------------------------------------------------
 def iteration_band(Ao, b, tol, restart, max_iters, delta=0.25):
