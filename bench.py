@@ -375,6 +375,26 @@ def main():
     matvec["matrix_free"] = {"ms": mf_ms, "gentries_per_s": n * n / (mf_ms * 1e-3) / 1e9,
                              "fp64_frac": n * n * FP64_INSTR_PER_PAIR_FREE / (mf_ms * 1e-3) / dfma_per_s}
 
+    # ---- SURVEY 8(f) NEXT rows built so far, stand-alone calls outside the timed region ----------------------------
+    next_rows = {}
+    vx_ms = time_call(lambda: ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A, variant=2), 10)
+    next_rows["vortex_sheet_matrix"] = {"call": "bie_build(variant=BIE_VARIANT_VORTEX)", "ms": vx_ms,
+                                        "gentries_per_s": n * n / (vx_ms * 1e-3) / 1e9,
+                                        "fp64_frac": n * n * FP64_INSTR_PER_ENTRY / (vx_ms * 1e-3) / dfma_per_s,
+                                        "hbm_write_frac": 8.0 * n * n / (vx_ms * 1e-3) / 1e9 / hbm_peak()[0]}
+    M0 = int(g.counts[0])
+    Nm = A.view(-1)[: M0 * A.stride(0)].view(M0, A.stride(0))       # the first M_0 rows of the same allocation
+    wv = torch.from_numpy(np.random.default_rng(2).standard_normal(n)).cuda()
+    uv = torch.empty(M0 + (M0 & 1), dtype=torch.float64, device="cuda")[:M0]
+    nb_ms = time_call(lambda: ctx.bie_build_normal_velocity(g.counts, g.kinds, z, dz, d2z, Nm), 10)
+    na_ms = time_call(lambda: ctx.bie_matvec_rect(Nm, wv, uv), 20)
+    next_rows["normal_velocity"] = {"call": "bie_build_normal_velocity + bie_matvec_rect", "rows": M0, "cols": n,
+                                    "build_ms": nb_ms, "build_gentries_per_s": M0 * n / (nb_ms * 1e-3) / 1e9,
+                                    "build_hbm_write_frac": 8.0 * M0 * n / (nb_ms * 1e-3) / 1e9 / hbm_peak()[0],
+                                    "apply_ms": na_ms, "apply_gbs": 8.0 * M0 * n / (na_ms * 1e-3) / 1e9,
+                                    "apply_hbm_frac": 8.0 * M0 * n / (na_ms * 1e-3) / 1e9 / hbm_peak()[0]}
+    del Nm
+
     # ---- end to end through bie_solve_host, pinned host buffers ---------------------------------------------
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     hz, hdz, hd2z, hb = pin(g.zeta.view(np.float64)), pin(g.dzeta.view(np.float64)), pin(g.d2zeta.view(np.float64)), pin(P.rhs[0])
@@ -447,7 +467,7 @@ def main():
             "gpu_launches": launches_per_step * K,
             "roofline": roof, "roofline_build": roof_build, "matvec": matvec, "clocks": clocks,
             "fp64_probe_tflops": 2 * dfma_per_s / 1e12,
-            "operator_choice_ms_per_step": choice_ms or None}
+            "operator_choice_ms_per_step": choice_ms or None, "next_rows": next_rows}
     if not args.no_cpu_baseline:
         est, desc, cores, parts = oracle_sample(P, iters, args.cpu_seconds)
         line["cpu_baseline"] = {"value": n * n / est / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
