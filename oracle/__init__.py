@@ -44,6 +44,8 @@ def lib() -> ctypes.CDLL:
         L.oracle_build_rows.restype = ctypes.c_int
         L.oracle_build_rows.argtypes = [ctypes.c_int, ip, ip, dp, dp, dp, ctypes.c_int, ctypes.c_long,
                                         ctypes.POINTER(ctypes.c_long), dp]
+        L.oracle_add_cyl_columns.restype = ctypes.c_int
+        L.oracle_add_cyl_columns.argtypes = [ctypes.c_int, ip, ip, dp, dp, dp, ctypes.c_long]
         L.oracle_normal_velocity_sums.restype = ctypes.c_int
         L.oracle_normal_velocity_sums.argtypes = [ctypes.c_int, ip, dp, dp, dp, dp, ctypes.c_long,
                                                   ctypes.POINTER(ctypes.c_long), dp]
@@ -115,6 +117,22 @@ def build_rows(counts, kinds, zeta, dzeta, d2zeta, rows, variant: int = 0) -> np
     if rc != 0:
         raise ValueError(f"oracle_build_rows failed: {rc}")
     return out
+
+
+def build_matrix_appendix_b(counts, kinds, zeta, dzeta, d2zeta, centers) -> np.ndarray:
+    """Matrix of Eq. (B.2): the operator B of Eq. (3.10) plus the columns phi_cyl/psi_cyl(zeta - z_m) <1_m, .>
+    (stream function prescribed on the solids; a_m = <1_m, omega> unknown).  centers: one complex z_m per obstacle."""
+    A = build_matrix(counts, kinds, zeta, dzeta, d2zeta, variant=1)
+    counts = np.ascontiguousarray(counts, dtype=np.int32)
+    kinds = np.ascontiguousarray(kinds, dtype=np.int32)
+    zc = np.ascontiguousarray(np.asarray(centers, dtype=np.complex128).reshape(-1))
+    assert zc.size == int(np.sum(kinds == 2))
+    zcf = zc.view(np.float64) if zc.size else np.zeros(2)
+    rc = lib().oracle_add_cyl_columns(int(counts.size), _ip(counts), _ip(kinds), _dp(_c128_as_f64(zeta)), _dp(zcf), _dp(A),
+                                      A.shape[1])
+    if rc != 0:
+        raise ValueError(f"oracle_add_cyl_columns failed: {rc}")
+    return A
 
 
 def hilbert(f: np.ndarray) -> np.ndarray:

@@ -16,6 +16,8 @@
  *                      and E_m = M_m^{-1} e e^T.
  *                     variant 2: the vortex-sheet system of Eqs. (4.14) + (4.17) with the adjoint
  *                     matrices K+, G+ of Eq. (4.7); its solid-solid block is Eq. (4.5).
+ *   oracle_add_cyl_columns   the rank-(N-1) correction of Appendix B, Eq. (B.2): stream function
+ *                     prescribed on the solids, circulations unknown.
  *   oracle_normal_velocity_sums   the trapezoid sums of Eqs. (3.19) and (3.24) for the normal velocity on
  *                     Gamma_0 (Section 3.4); the FFT Hilbert transform is added in Python.
  *   oracle_matvec     y = A x, the plain definition (long-double accumulation).
@@ -234,6 +236,42 @@ int oracle_build_rows(int ncomp, const int *counts, const int *kinds,
         else oracle_row(rows[i], n, comp, counts, kinds, zeta, dzeta, d2zeta, variant, out + i * n);
     }
     free(comp);
+    return 0;
+}
+
+/* NEXT-4, Appendix B: the variant in which the stream function is prescribed on the solids and
+ * the circulation parameters a_m = <1_m, omega> are unknowns.  Eq. (B.2):
+ *      A omega = B omega + sum_{m >= 2} c_m <1_m, omega>,    c_m = ( phi_cyl(zeta_0 - z_m), psi_cyl(zeta_1 - z_m), ..., psi_cyl(zeta_N - z_m) ),
+ * Phi_cyl(z) = -i log(1 - e^{iz}) (Eq. (3.2)), phi_cyl = Re Phi_cyl = arg(1 - e^{iz}), psi_cyl = Im Phi_cyl =
+ * -log|1 - e^{iz}|; z_m = a point inside obstacle m.  On the trapezoidal rule <1_m, omega> = (1/M_m) sum_l
+ * omega_m[l], so the correction adds c_m[t]/M_m to every column of obstacle m, in every row t.
+ * This function ADDS that correction to a matrix A that holds B (oracle_build with variant 1).  centers: interleaved
+ * (re, im), one per component with kinds[c] == 2, in component order.  Returns 0, or < 0 on bad arguments. */
+int oracle_add_cyl_columns(int ncomp, const int *counts, const int *kinds, const double *zeta, const double *centers,
+                           double *A, long lda)
+{
+    if (ncomp < 1 || !counts || !kinds || !zeta || !A) return -1;
+    long n = 0;
+    for (int c = 0; c < ncomp; ++c) { if (counts[c] < 1) return -2; n += counts[c]; }
+    if (lda < n) return -3;
+    long off = 0;
+    int o = 0;
+    for (int m = 0; m < ncomp; off += counts[m], ++m) {
+        if (kinds[m] != 2) continue;
+        if (!centers) return -1;
+        const double zr = centers[2 * o], zi = centers[2 * o + 1];
+        ++o;
+        const double Mm = (double)counts[m];
+#pragma omp parallel for schedule(static)
+        for (long t = 0; t < n; ++t) {
+            /* w = 1 - e^{i(zeta_t - z_m)} */
+            const double x = zeta[2 * t] - zr, y = zeta[2 * t + 1] - zi;
+            const double ex = exp(-y);
+            const double wr = 1.0 - ex * cos(x), wi = -ex * sin(x);
+            const double c = (t < counts[0]) ? atan2(wi, wr) : -0.5 * log(wr * wr + wi * wi);
+            for (long l = 0; l < counts[m]; ++l) A[t * lda + off + l] += c / Mm;
+        }
+    }
     return 0;
 }
 

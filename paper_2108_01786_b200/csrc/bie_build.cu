@@ -254,16 +254,30 @@ int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int ncols, int only_c
     if (lda < ncols || (lda & 1) || (((uintptr_t)A) & 15u)) return BIE_ERR_LAYOUT;
     const NodeTable nt = bie_node_table(ctx);
     const int gx = (ncols + BUILD_TILE_W - 1) / BUILD_TILE_W;
-    // rows per CTA: 128 when that still gives every SM several CTAs, else smaller
     int nt_rows = n;
+    if (ctx->variant == BIE_VARIANT_NORMAL_INTERNAL) nt_rows = ctx->counts[0];   // M_0 x n: rows on Gamma_0 only
+    const bool dagger = (ctx->variant == BIE_VARIANT_VORTEX || ctx->variant == BIE_VARIANT_NORMAL_INTERNAL);
+    // rows per CTA: 128 when that still gives every SM several CTAs, else smaller ...
     int T = 128;
-    while (T > 8 && (long long)gx * ((n + T - 1) / T) < 4LL * ctx->sm_count) T >>= 1;
-    if (ctx->variant == BIE_VARIANT_NORMAL_INTERNAL) {   // M_0 x n: rows on Gamma_0 only
-        const int M0 = ctx->counts[0];
-        nt_rows = M0;
+    while (T > 8 && (long long)gx * ((nt_rows + T - 1) / T) < 4LL * ctx->sm_count) T >>= 1;
+    // ... and, for grids of several waves, the T in [96, 256] that fills whole waves of resident CTAs: the tail wave
+    // of the default (8192 CTAs = 11.07 waves of 740 at n = 16384) cost 16 % (profiles/r01b_ncu_full_cfg5.md)
+    {
+        int occ = 0;
+        if (dagger) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bie_build_dagger_kernel, BUILD_THREADS, 7 * 8 * 256 + 16);
+        else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bie_build_kernel, BUILD_THREADS, 3 * 8 * 256 + 16);
+        const long long wave = (long long)ctx->sm_count * (occ > 0 ? occ : 1);
+        if ((long long)gx * ((nt_rows + 127) / 128) >= 2 * wave) {
+            double best = 0.0;
+            for (int t = 96; t <= 256; t += BUILD_RB) {
+                const long long gy = (nt_rows + t - 1) / t, ctas = (long long)gx * gy;
+                const double eff = (double)ctas / (double)(((ctas + wave - 1) / wave) * wave) * (double)nt_rows / (double)(gy * t);
+                if (eff > best + 1e-9) { best = eff; T = t; }
+            }
+        }
     }
     dim3 grid(gx, (nt_rows + T - 1) / T);
-    if (ctx->variant == BIE_VARIANT_VORTEX || ctx->variant == BIE_VARIANT_NORMAL_INTERNAL) {
+    if (dagger) {
         bie_build_dagger_kernel<<<grid, BUILD_THREADS, (3 * sizeof(double2) + sizeof(double)) * T + 16, st>>>(
             nt, ctx->comps, A, (long long)lda, T, only_comp0, ncols,
             ctx->variant == BIE_VARIANT_NORMAL_INTERNAL ? ctx->kappa : nullptr);

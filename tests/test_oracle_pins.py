@@ -593,3 +593,64 @@ def test_p9_normal_velocity_of_a_known_potential_flow():
         exact = np.real(fprime(g.zeta[s0]) * 1j * g.dzeta[s0])
         errs.append(np.max(np.abs(u - exact)) / np.max(np.abs(exact)))
     assert errs[1] < 1e-9 and errs[1] < errs[0] * 1e-2 or errs[0] < 1e-11, errs
+
+
+# --------------------------------------------------------------------------------------------
+# P10  Appendix B (NEXT-4): stream function prescribed on the solids, circulations a_m = <1_m, omega> unknown
+# --------------------------------------------------------------------------------------------
+def _appendix_b_case():
+    g = inputs.small_problem(96, 80, [48, 56], seed=5).geometry
+    cents = [np.mean(g.zeta[g.component(k)]) for k in (2, 3)]    # a point inside each obstacle
+    return g, cents
+
+
+def test_p10_columns_are_the_boundary_values_of_phi_cyl():
+    """The correction columns of Eq. (B.2) against Phi_cyl(z) = -i log(1 - e^{iz}) (Eq. 3.2)
+    evaluated with numpy's complex log: rows on Gamma_0 take Re, rows on solids Im; weight 1/M_m; nothing outside the
+    obstacle column blocks changes; and psi_cyl agrees with the form -log|1 - e^{iz}| used for right-hand sides."""
+    g, cents = _appendix_b_case()
+    B = _build(g, variant=1)
+    AB = oracle.build_matrix_appendix_b(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, cents)
+    D = AB - B
+    s0, s1 = g.component(0), g.component(1)
+    assert np.max(np.abs(D[:, s0])) == 0.0 and np.max(np.abs(D[:, s1])) == 0.0
+    for o, k in enumerate((2, 3)):
+        sk = g.component(k)
+        Phi = -1j * np.log(1.0 - np.exp(1j * (g.zeta - cents[o])))
+        col = np.where(np.arange(g.n) < g.counts[0], Phi.real, Phi.imag) / g.counts[k]
+        assert np.max(np.abs(D[:, sk] - col[:, None])) < 1e-15
+        assert np.max(np.abs(Phi.imag - inputs.psi_cyl(g.zeta - cents[o]))) < 1e-14
+
+
+def test_p10_appendix_b_solution_from_the_pinned_system():
+    """Consistency with the pinned system (3.16).  Solve A omega_A = b of (3.15) for GIVEN circulations a_m (PAPER.md:L297);
+    then psi|_m = <1_m, omega_A>.  Prescribe exactly these psi|_m in Appendix B: b_0 = phi - V_1 xi,
+    b_k = psi|_k - V_1 eta_k.  Because ker B = span{1_m}, the unique solution of (B.2) is
+    omega_B = omega_A + sum_m (a_m - psi|_m) 1_m, and it returns the circulations: <1_m, omega_B> = a_m."""
+    g, cents = _appendix_b_case()
+    V1, a = 0.8, [0.6, -0.35]
+    rng = np.random.default_rng(9)
+    a0 = 2 * np.pi * np.arange(g.counts[0]) / g.counts[0]
+    phi_t = 0.2 * np.cos(a0) + 0.1 * np.sin(3 * a0)                      # phi~ on Gamma_0
+    bA = inputs.rhs_physical(g, V1, a, cents, phi_tilde=phi_t)
+    A = _build(g)
+    wA, it, rr, _, st = oracle.gmres(A, bA, 1e-14, 80, 600)
+    assert st == 0
+    psi = [np.mean(wA[g.component(k)]) for k in (2, 3)]
+    # Appendix-B right-hand side: phi = phi~ + phi_mv on Gamma_0, so phi - V1 xi = phi~ + sum a_m phi_cyl(zeta_0 - z_m)
+    s0 = g.component(0)
+    bB = np.zeros(g.n)
+    bB[s0] = phi_t + sum(am * (-1j * np.log(1.0 - np.exp(1j * (g.zeta[s0] - zm)))).real for am, zm in zip(a, cents))
+    for k in range(1, g.counts.size):
+        sk = g.component(k)
+        pk = 0.0 if k == 1 else psi[k - 2]
+        bB[sk] = pk - V1 * g.zeta[sk].imag
+    AB = oracle.build_matrix_appendix_b(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, cents)
+    assert np.linalg.cond(AB) < 1e3
+    wB, it, rr, _, st = oracle.gmres(AB, bB, 1e-14, 80, 600)
+    assert st == 0
+    expect = wA.copy()
+    for o, k in enumerate((2, 3)):
+        expect[g.component(k)] += a[o] - psi[o]
+        assert abs(np.mean(wB[g.component(k)]) - a[o]) < 1e-12          # the circulations come back
+    assert np.max(np.abs(wB - expect)) < 1e-11
