@@ -382,6 +382,13 @@ def main():
                                         "gentries_per_s": n * n / (vx_ms * 1e-3) / 1e9,
                                         "fp64_frac": n * n * FP64_INSTR_PER_ENTRY / (vx_ms * 1e-3) / dfma_per_s,
                                         "hbm_write_frac": 8.0 * n * n / (vx_ms * 1e-3) / 1e9 / hbm_peak()[0]}
+    if P.centers:
+        ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A, variant=1)
+        cyl_ms = time_call(lambda: ctx.bie_add_cyl_columns(g.counts, g.kinds, z, P.centers, A), 10)
+        nobs_cols = int(sum(int(cn) for cn, kd in zip(g.counts, g.kinds) if kd == 2))
+        next_rows["appendix_b_columns"] = {"call": "bie_add_cyl_columns (in place on the variant-B matrix)", "ms": cyl_ms,
+                                           "entries": n * nobs_cols, "gbs": 16.0 * n * nobs_cols / (cyl_ms * 1e-3) / 1e9,
+                                           "hbm_frac": 16.0 * n * nobs_cols / (cyl_ms * 1e-3) / 1e9 / hbm_peak()[0]}
     M0 = int(g.counts[0])
     Nm = A.view(-1)[: M0 * A.stride(0)].view(M0, A.stride(0))       # the first M_0 rows of the same allocation
     wv = torch.from_numpy(np.random.default_rng(2).standard_normal(n)).cuda()

@@ -144,6 +144,16 @@ int bie_set_geometry(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32
 int bie_matvec(bie_ctx* ctx, int n, const double* A, int64_t lda, const double* x, double* y, void* stream);
 int bie_matvec_free(bie_ctx* ctx, int n, const double* x, double* y, void* stream);
 
+/* stream function prescribed on the solids, circulation parameters
+ * a_m = <1_m, omega> unknown.  Adds, in place, the rank-(N-1) correction of Eq. (B.2) to a matrix A that holds
+ * the operator B (bie_build with BIE_VARIANT_B):  A[t][s] += c_m[t]/M_m for every column s of obstacle m, with
+ * c_m[t] = phi_cyl(zeta_t - z_m) = arg(1 - e^{i(zeta_t - z_m)}) for rows on Gamma_0 and psi_cyl = -log|1 - e^{i(zeta_t - z_m)}|
+ * for rows on solids (Phi_cyl = -i log(1 - e^{iz}), Eq. (3.2)).  centers: HOST, interleaved (re, im), one
+ * point z_m inside each obstacle, in component order; zeta: dev as in bie_build; A: dev, n x lda.
+ * The right-hand side of the variant is b_0 = phi - V_1 xi, b_k = psi|_k - V_1 eta_k; solve with bie_gmres. */
+int bie_add_cyl_columns(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds, const double* zeta,
+                        const double* centers, double* A, int64_t lda, void* stream);
+
 /* y (nrows) = A (nrows x ncols, row-major, lda >= ncols even) x (ncols): the same HBM-bound kernel on a rectangular block. */
 int bie_matvec_rect(bie_ctx* ctx, int nrows, int ncols, const double* A, int64_t lda, const double* x, double* y,
                     void* stream);

@@ -23,7 +23,8 @@ _lib: Optional[ctypes.CDLL] = None
 EXPORTS = ("bie_create", "bie_destroy", "bie_strerror", "bie_device_info", "bie_build", "bie_build_update",
            "bie_set_geometry", "bie_matvec", "bie_matvec_free", "bie_gmres_workspace_bytes", "bie_gmres",
            "bie_solve_workspace_bytes", "bie_solve_host", "bie_probe_dfma", "bie_build_cols", "bie_hybrid_cols",
-           "bie_set_hybrid_free_warps", "bie_gmres_hybrid", "bie_matvec_rect", "bie_build_normal_velocity")
+           "bie_set_hybrid_free_warps", "bie_gmres_hybrid", "bie_matvec_rect", "bie_build_normal_velocity",
+           "bie_add_cyl_columns")
 
 BIE_OK, BIE_MAX_ITERS = 0, 1
 OP_DENSE, OP_FREE, OP_HYBRID = 0, 1, 2
@@ -86,6 +87,8 @@ def lib() -> ctypes.CDLL:
         L.bie_matvec_rect.argtypes = [vp, i32, i32, vp, i64, vp, vp, vp]
         L.bie_build_normal_velocity.restype = i32
         L.bie_build_normal_velocity.argtypes = geo[:-1] + [vp, i64, vp]
+        L.bie_add_cyl_columns.restype = i32
+        L.bie_add_cyl_columns.argtypes = [vp, i32, ip, ip, vp, ctypes.POINTER(dbl), vp, i64, vp]
         L.bie_probe_dfma.restype = i32
         L.bie_probe_dfma.argtypes = [vp, i64, vp, ctypes.POINTER(i64), vp]
         _lib = L
@@ -218,6 +221,19 @@ class Context:
         _dev_f64(Nmat, (M0 - 1) * lda + n)
         _check(lib().bie_build_normal_velocity(*args[:-1], Nmat.data_ptr(), lda, _stream()), "bie_build_normal_velocity")
         return Nmat
+
+    def bie_add_cyl_columns(self, counts, kinds, zeta, centers, A, lda: Optional[int] = None):
+        """A (holding the operator B, variant 1) += the correction columns of Appendix B, Eq. (B.2); centers: one complex
+        point per obstacle (host)."""
+        counts, kinds = _i32(counts), _i32(kinds)
+        n = int(counts.sum())
+        zc = np.ascontiguousarray(np.asarray(centers, dtype=np.complex128).reshape(-1))
+        zf = zc.view(np.float64) if zc.size else np.zeros(2)
+        lda = int(lda if lda is not None else A.stride(0))
+        _check(lib().bie_add_cyl_columns(self._h, int(counts.size), _ip(counts), _ip(kinds), _dev_c128(zeta, n),
+                                         zf.ctypes.data_as(ctypes.POINTER(ctypes.c_double)),
+                                         _dev_f64(A, (n - 1) * lda + n), lda, _stream()), "bie_add_cyl_columns")
+        return A
 
     def bie_matvec_free(self, x, y):
         n = x.numel()

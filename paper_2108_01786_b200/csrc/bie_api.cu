@@ -155,6 +155,14 @@ int bie_matvec(bie_ctx* c, int n, const double* A, int64_t lda, const double* x,
     return bie_launch_matvec(c, n, n, A, lda, x, y, (cudaStream_t)stream);
 }
 
+int bie_add_cyl_columns(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* kinds, const double* zeta,
+                        const double* centers, double* A, int64_t lda, void* stream)
+{
+    if (!c) return BIE_ERR_NULL;
+    BIE_CUDA(cudaSetDevice(c->device));
+    return bie_launch_add_cyl_columns(c, ncomp, counts, kinds, zeta, centers, A, lda, (cudaStream_t)stream);
+}
+
 int bie_matvec_rect(bie_ctx* c, int nrows, int ncols, const double* A, int64_t lda, const double* x, double* y,
                     void* stream)
 {

@@ -365,6 +365,63 @@ def test_normal_velocity_full_size_sampled_rows(ctx, c):
     del N
 
 
+@pytest.mark.parametrize("c", [1, 3, 5])
+def test_appendix_b_matrix_parity(ctx, c):
+    """NEXT-4: B + the correction columns of Eq. (B.2); full matrix for configs 1 and 3, sampled rows at config 5"""
+    P = cfg(c)
+    g = P.geometry
+    A = gpu_build(ctx, g, variant=1)
+    z, _, _ = geo_dev(g)
+    ctx.bie_add_cyl_columns(g.counts, g.kinds, z, P.centers, A)
+    torch.cuda.synchronize()
+    if c < 5:
+        Ao = oracle.build_matrix_appendix_b(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, P.centers)
+        assert rel_max(A.cpu().numpy()[:, :g.n], Ao) <= TOL_ENTRY
+    else:
+        rows = _sample_rows(g, np.random.default_rng(c), k=32)
+        Ag = A[torch.from_numpy(rows).cuda(), :g.n].cpu().numpy()
+        Ao = oracle.build_rows(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, rows, variant=1)
+        off = g.offsets
+        for o, k in enumerate(range(2, g.counts.size)):
+            Phi = -1j * np.log(1.0 - np.exp(1j * (g.zeta[rows] - P.centers[o])))
+            col = np.where(rows < g.counts[0], Phi.real, Phi.imag) / g.counts[k]
+            Ao[:, off[k]:off[k + 1]] += col[:, None]
+        assert float(np.max(np.abs(Ag - Ao))) <= TOL_ENTRY * float(np.max(np.abs(Ao)))
+    del A
+
+
+def test_appendix_b_solve_returns_the_circulations(ctx):
+    """the consistency argument of pin P10 on the GPU: solve (3.16) for given a_m, prescribe the resulting psi|_m, solve the
+    Appendix-B system, get omega_A + sum (a_m - psi|_m) 1_m and the circulations back"""
+    g = inputs.small_problem(96, 80, [48, 56], seed=5).geometry
+    cents = [np.mean(g.zeta[g.component(k)]) for k in (2, 3)]
+    V1, a = 0.8, [0.6, -0.35]
+    a0 = 2 * np.pi * np.arange(g.counts[0]) / g.counts[0]
+    phi_t = 0.2 * np.cos(a0) + 0.1 * np.sin(3 * a0)
+    bA = inputs.rhs_physical(g, V1, a, cents, phi_tilde=phi_t)
+    A = gpu_build(ctx, g)
+    wA, it, rr, st = gpu_gmres(ctx, A, bA, 1e-14, 80, 600)
+    assert st == 0
+    psi = [np.mean(wA[g.component(k)]) for k in (2, 3)]
+    s0 = g.component(0)
+    bB = np.zeros(g.n)
+    bB[s0] = phi_t + sum(am * (-1j * np.log(1.0 - np.exp(1j * (g.zeta[s0] - zm)))).real for am, zm in zip(a, cents))
+    for k in range(1, g.counts.size):
+        sk = g.component(k)
+        bB[sk] = (0.0 if k == 1 else psi[k - 2]) - V1 * g.zeta[sk].imag
+    AB = gpu_build(ctx, g, variant=1)
+    z, _, _ = geo_dev(g)
+    ctx.bie_add_cyl_columns(g.counts, g.kinds, z, cents, AB)
+    wB, it, rr, st = gpu_gmres(ctx, AB, bB, 1e-14, 80, 600)
+    assert st == 0
+    ABo = oracle.build_matrix_appendix_b(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, cents)
+    wo, ito, _, _, sto = oracle.gmres(ABo, bB, 1e-14, 80, 600)
+    assert sto == 0 and abs(it - ito) <= 1
+    assert np.linalg.norm(wB - wo) / np.linalg.norm(wo) <= TOL_X
+    for o, k in enumerate((2, 3)):
+        assert abs(np.mean(wB[g.component(k)]) - a[o]) < 1e-11
+
+
 def test_matvec_rect_matches_the_oracle(ctx):
     rng = np.random.default_rng(3)
     for (nr, nc, lda) in [(1, 2, 2), (7, 130, 132), (300, 64, 64), (129, 1001, 1002)]:
