@@ -44,6 +44,8 @@ def lib() -> ctypes.CDLL:
         L.oracle_build_rows.restype = ctypes.c_int
         L.oracle_build_rows.argtypes = [ctypes.c_int, ip, ip, dp, dp, dp, ctypes.c_int, ctypes.c_long,
                                         ctypes.POINTER(ctypes.c_long), dp]
+        L.oracle_cauchy_eval.restype = ctypes.c_int
+        L.oracle_cauchy_eval.argtypes = [ctypes.c_int, ip, ip, dp, dp, ctypes.c_int, dp, ctypes.c_long, dp, dp]
         L.oracle_add_cyl_columns.restype = ctypes.c_int
         L.oracle_add_cyl_columns.argtypes = [ctypes.c_int, ip, ip, dp, dp, dp, ctypes.c_long]
         L.oracle_normal_velocity_sums.restype = ctypes.c_int
@@ -133,6 +135,24 @@ def build_matrix_appendix_b(counts, kinds, zeta, dzeta, d2zeta, centers) -> np.n
     if rc != 0:
         raise ValueError(f"oracle_add_cyl_columns failed: {rc}")
     return A
+
+
+def cauchy_eval(counts, kinds, zeta, dzeta, fvals, zpts) -> np.ndarray:
+    """Eq. (F.4) / (5.5): values at the points zpts (complex, in the closed fluid region) of nf functions analytic in the
+    fluid, from their boundary values fvals (nf x n complex) -> (nf x npts complex)."""
+    counts = np.ascontiguousarray(counts, dtype=np.int32)
+    kinds = np.ascontiguousarray(kinds, dtype=np.int32)
+    n = int(counts.sum())
+    f = np.ascontiguousarray(np.atleast_2d(np.asarray(fvals, dtype=np.complex128)))
+    zp = np.ascontiguousarray(np.asarray(zpts, dtype=np.complex128).reshape(-1))
+    assert f.shape[1] == n
+    out = np.empty((f.shape[0], zp.size), dtype=np.complex128)
+    rc = lib().oracle_cauchy_eval(int(counts.size), _ip(counts), _ip(kinds), _dp(_c128_as_f64(zeta)), _dp(_c128_as_f64(dzeta)),
+                                  int(f.shape[0]), _dp(f.view(np.float64)), zp.size, _dp(zp.view(np.float64)),
+                                  _dp(out.view(np.float64)))
+    if rc != 0:
+        raise ValueError(f"oracle_cauchy_eval failed: {rc}")
+    return out
 
 
 def hilbert(f: np.ndarray) -> np.ndarray:

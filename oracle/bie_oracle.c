@@ -16,6 +16,8 @@
  *                      and E_m = M_m^{-1} e e^T.
  *                     variant 2: the vortex-sheet system of Eqs. (4.14) + (4.17) with the adjoint
  *                     matrices K+, G+ of Eq. (4.7); its solid-solid block is Eq. (4.5).
+ *   oracle_cauchy_eval   Eq. (F.4) / (5.5): a function analytic in the fluid from its boundary
+ *                     values, spectrally accurate up to the boundary.
  *   oracle_add_cyl_columns   the rank-(N-1) correction of Appendix B, Eq. (B.2): stream function
  *                     prescribed on the solids, circulations unknown.
  *   oracle_normal_velocity_sums   the trapezoid sums of Eqs. (3.19) and (3.24) for the normal velocity on
@@ -273,6 +275,60 @@ int oracle_add_cyl_columns(int ncomp, const int *counts, const int *kinds, const
         }
     }
     return 0;
+}
+
+/* NEXT-3, Section 5.1 / Appendix F: evaluation of a function analytic in the fluid from
+ * its boundary values, spectrally accurate up to the boundary (Helsing & Ojala, periodic version).  Eq. (F.4) / (5.5):
+ *      f(z) ~ sum_km lambda~_km(z) f(zeta_k(alpha_m)) / sum_km lambda~_km(z),
+ *      lambda~_km(z) = (sigma_k / M_k) * 1/2 cot((zeta_k(alpha_m) - z)/2) * zeta'_k(alpha_m),
+ * with sigma_0 = -1 and sigma_k = +1 for the solids: Gamma_0 is parameterised with the fluid on its RIGHT, so it
+ * enters the boundary integral of (F.1) with the opposite orientation (reading R18; (F.3)/(F.4) do not print it).
+ * "If z coincides with zeta_k(alpha_m), we set f(z) = f(zeta_k(alpha_m))".
+ * f: nf functions, [nf][n] complex interleaved; zpts: npts complex; out: [nf][npts] complex.  Returns 0 or < 0. */
+int oracle_cauchy_eval(int ncomp, const int *counts, const int *kinds, const double *zeta, const double *dzeta,
+                       int nf, const double *f, long npts, const double *zpts, double *out)
+{
+    if (ncomp < 1 || !counts || !kinds || !zeta || !dzeta || !f || !zpts || !out || nf < 1) return -1;
+    long n = 0;
+    for (int c = 0; c < ncomp; ++c) { if (counts[c] < 1) return -2; n += counts[c]; }
+#pragma omp parallel for schedule(static)
+    for (long p = 0; p < npts; ++p) {
+        const double zr = zpts[2 * p], zi = zpts[2 * p + 1];
+        long double Dr = 0.0L, Di = 0.0L;
+        long double Nr[8], Ni[8];
+        for (int q = 0; q < nf && q < 8; ++q) { Nr[q] = 0.0L; Ni[q] = 0.0L; }
+        long hit = -1;
+        long s = 0;
+        for (int k = 0; k < ncomp && hit < 0; ++k) {
+            const double wgt = (kinds[k] == 0 ? -1.0 : 1.0) / (double)counts[k];
+            for (long m = 0; m < counts[k]; ++m, ++s) {
+                const double x = zeta[2 * s] - zr, y = zeta[2 * s + 1] - zi;
+                const double sx = sin(0.5 * x), sh = sinh(0.5 * y);
+                if (sx * sx + sh * sh == 0.0) { hit = s; break; }
+                double cr, ci;
+                oracle_cot_half(x, y, &cr, &ci);
+                /* lambda~ = wgt * 1/2 * cot * zeta' */
+                const double lr = 0.5 * wgt * (cr * dzeta[2 * s] - ci * dzeta[2 * s + 1]);
+                const double li = 0.5 * wgt * (cr * dzeta[2 * s + 1] + ci * dzeta[2 * s]);
+                Dr += lr; Di += li;
+                for (int q = 0; q < nf && q < 8; ++q) {
+                    const double fr = f[2 * ((long)q * n + s)], fi = f[2 * ((long)q * n + s) + 1];
+                    Nr[q] += (long double)lr * fr - (long double)li * fi;
+                    Ni[q] += (long double)lr * fi + (long double)li * fr;
+                }
+            }
+        }
+        for (int q = 0; q < nf && q < 8; ++q) {
+            double *o = out + 2 * ((long)q * npts + p);
+            if (hit >= 0) { o[0] = f[2 * ((long)q * n + hit)]; o[1] = f[2 * ((long)q * n + hit) + 1]; }
+            else {
+                const long double d2 = Dr * Dr + Di * Di;
+                o[0] = (double)((Nr[q] * Dr + Ni[q] * Di) / d2);
+                o[1] = (double)((Ni[q] * Dr - Nr[q] * Di) / d2);
+            }
+        }
+    }
+    return nf > 8 ? -5 : 0;
 }
 
 /* NEXT-2: the trapezoid sums of the normal velocity on the free surface, Section 3.4, for the

@@ -654,3 +654,55 @@ def test_p10_appendix_b_solution_from_the_pinned_system():
         expect[g.component(k)] += a[o] - psi[o]
         assert abs(np.mean(wB[g.component(k)]) - a[o]) < 1e-12          # the circulations come back
     assert np.max(np.abs(wB - expect)) < 1e-11
+
+
+# --------------------------------------------------------------------------------------------
+# P11  evaluation of Cauchy integrals near boundaries (NEXT-3): Eq. (F.4) / (5.5)
+# --------------------------------------------------------------------------------------------
+def _near_boundary_points(g):
+    """interior points, points at distance 1e-2 ... 1e-9 from the boundaries along the inward normal, and two nodes"""
+    pts = list(_interior_points())
+    for k, m, sign in [(0, 7, 1.0), (1, 11, 1.0), (2, 5, 1.0), (0, 200, 1.0)]:
+        s = g.component(k).start + m
+        nrm = 1j * g.dzeta[s] / abs(g.dzeta[s])          # left normal of the parameterisation
+        inward = -nrm if k == 0 else nrm                   # fluid is to the RIGHT of Gamma_0, to the left of solids
+        for d in (1e-2, 1e-4, 1e-6, 1e-9):
+            pts.append(g.zeta[s] + d * inward)
+    return np.array(pts)
+
+
+def test_p11_reproduces_an_analytic_function_up_to_the_boundary():
+    """f analytic in the fluid (poles outside): Eq. (F.4) returns f(z) with spectral accuracy at interior points AND at
+    points 1e-2 ... 1e-9 away from the boundary, where the plain trapezoid rule for (F.1) has O(1) error (PAPER.md:L569,
+    L1162).  The sign sigma_0 = -1 on Gamma_0 is essential: with +1 the denominator of (F.4) vanishes (reading R18)."""
+    g = inputs.make_config(1).geometry
+    f = np.vstack([_f_poles(g.zeta), np.exp(2j * g.zeta), np.ones(g.n)])
+    zp = _near_boundary_points(g)
+    out = oracle.cauchy_eval(g.counts, g.kinds, g.zeta, g.dzeta, f, zp)
+    assert np.max(np.abs(out[0] - _f_poles(zp))) < 5e-12
+    assert np.max(np.abs(out[1] - np.exp(2j * zp))) < 5e-12
+    assert np.max(np.abs(out[2] - 1.0)) < 1e-15                 # the weights lambda_km sum to one
+    # the plain trapezoid rule of (F.1) at a point 1e-4 from Gamma_0 is useless; (F.4) is not
+    z = zp[len(_interior_points()) + 1]
+    plain = 0.0
+    for k in range(3):
+        sk = g.component(k)
+        sig = -1.0 if k == 0 else 1.0
+        plain += sig / g.counts[k] * np.sum(0.5 / np.tan(0.5 * (g.zeta[sk] - z)) * g.dzeta[sk] * f[0, sk]) / 1j
+    assert abs(plain - _f_poles(z)) > 1e-2
+    # wrong orientation of Gamma_0: denominator ~ 0
+    D = sum((1.0 / g.counts[k]) * np.sum(0.5 / np.tan(0.5 * (g.zeta[g.component(k)] - zp[0])) * g.dzeta[g.component(k)])
+            for k in range(3))
+    assert abs(D) < 1e-12
+
+
+def test_p11_coincidence_and_periodicity():
+    g = inputs.make_config(1).geometry
+    f = _f_poles(g.zeta)[None, :]
+    s = [3, g.component(1).start + 9, g.component(2).start + 40]
+    out = oracle.cauchy_eval(g.counts, g.kinds, g.zeta, g.dzeta, f, g.zeta[s])
+    assert np.array_equal(out[0], f[0, s])                        # PAPER.md:L573
+    zp = _interior_points()
+    a = oracle.cauchy_eval(g.counts, g.kinds, g.zeta, g.dzeta, f, zp)
+    b = oracle.cauchy_eval(g.counts, g.kinds, g.zeta, g.dzeta, f, zp + 2 * np.pi)
+    assert np.max(np.abs(a - b)) < 1e-13                          # sum over periodic images, Eq. (3.4)
