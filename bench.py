@@ -389,6 +389,21 @@ def main():
         next_rows["appendix_b_columns"] = {"call": "bie_add_cyl_columns (in place on the variant-B matrix)", "ms": cyl_ms,
                                            "entries": n * nobs_cols, "gbs": 16.0 * n * nobs_cols / (cyl_ms * 1e-3) / 1e9,
                                            "hbm_frac": 16.0 * n * nobs_cols / (cyl_ms * 1e-3) / 1e9 / hbm_peak()[0]}
+    # NEXT-3: 2 functions (Phi', Phi_t of Eq. 5.3) at 65 536 points below the free surface
+    npts_e = 65536
+    rng_e = np.random.default_rng(3)
+    ie = rng_e.integers(0, int(g.counts[0]), size=npts_e)
+    zp_e = dev(g.zeta[ie] - 1j * rng_e.uniform(0.01, 0.3, size=npts_e))
+    f_e = dev(np.vstack([np.exp(1j * g.zeta), np.exp(2j * g.zeta)]))
+    zc_e, dzc_e = dev(g.zeta), dev(g.dzeta)
+    out_e = torch.empty((2, npts_e), dtype=torch.complex128, device="cuda")
+    ev_ms = time_call(lambda: ctx.bie_cauchy_eval(g.counts, g.kinds, zc_e, dzc_e, f_e, zp_e, out=out_e), 5)
+    ev_instr = 12 + 4 * 3     # FP64-pipe instructions per pair: cot (12) + denominator and two numerators (4 each)
+    next_rows["cauchy_eval_near_boundary"] = {"call": "bie_cauchy_eval (nf = 2)", "points": npts_e, "sources": n, "ms": ev_ms,
+                                              "gpairs_per_s": npts_e * n / (ev_ms * 1e-3) / 1e9,
+                                              "fp64_instr_per_pair": ev_instr,
+                                              "fp64_frac": npts_e * n * ev_instr / (ev_ms * 1e-3) / dfma_per_s}
+    del zp_e, f_e, out_e
     M0 = int(g.counts[0])
     Nm = A.view(-1)[: M0 * A.stride(0)].view(M0, A.stride(0))       # the first M_0 rows of the same allocation
     wv = torch.from_numpy(np.random.default_rng(2).standard_normal(n)).cuda()

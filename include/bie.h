@@ -154,6 +154,18 @@ int bie_matvec_free(bie_ctx* ctx, int n, const double* x, double* y, void* strea
 int bie_add_cyl_columns(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds, const double* zeta,
                         const double* centers, double* A, int64_t lda, void* stream);
 
+/* values in the closed fluid region of nf
+ * (1..4) functions analytic in the fluid, from their boundary values, spectrally accurate up to the boundary:
+ *      f(z) = sum_s lambda~_s(z) f_s / sum_s lambda~_s(z),   lambda~_s(z) = (sigma_k/M_k) 1/2 cot((zeta_s - z)/2) zeta'_s     (Eq. F.4 / 5.5)
+ * with sigma_0 = -1 on Gamma_0 (parameterised with the fluid on its right) and +1 on the solids; a point that
+ * coincides with a node (modulo the period) gets that node's value.  E.g. f = Phi' and Phi_t for the velocity
+ * and pressure fields of Eq. (5.3)-(5.4).  zeta, dzeta: dev, as in bie_build (d2zeta is not needed); fvals: dev, [nf][n] complex
+ * interleaved; zpts: dev, npts complex; out: dev, [nf][npts] complex; workspace: dev, bie_cauchy_eval_workspace_bytes(). */
+size_t bie_cauchy_eval_workspace_bytes(bie_ctx* ctx, int nf, int npts);
+int bie_cauchy_eval(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds,
+                    const double* zeta, const double* dzeta, int nf, const double* fvals,
+                    int npts, const double* zpts, double* out, void* workspace, size_t workspace_bytes, void* stream);
+
 /* y (nrows) = A (nrows x ncols, row-major, lda >= ncols even) x (ncols): the same HBM-bound kernel on a rectangular block. */
 int bie_matvec_rect(bie_ctx* ctx, int nrows, int ncols, const double* A, int64_t lda, const double* x, double* y,
                     void* stream);

@@ -24,7 +24,7 @@ EXPORTS = ("bie_create", "bie_destroy", "bie_strerror", "bie_device_info", "bie_
            "bie_set_geometry", "bie_matvec", "bie_matvec_free", "bie_gmres_workspace_bytes", "bie_gmres",
            "bie_solve_workspace_bytes", "bie_solve_host", "bie_probe_dfma", "bie_build_cols", "bie_hybrid_cols",
            "bie_set_hybrid_free_warps", "bie_gmres_hybrid", "bie_matvec_rect", "bie_build_normal_velocity",
-           "bie_add_cyl_columns")
+           "bie_add_cyl_columns", "bie_cauchy_eval_workspace_bytes", "bie_cauchy_eval")
 
 BIE_OK, BIE_MAX_ITERS = 0, 1
 OP_DENSE, OP_FREE, OP_HYBRID = 0, 1, 2
@@ -89,6 +89,10 @@ def lib() -> ctypes.CDLL:
         L.bie_build_normal_velocity.argtypes = geo[:-1] + [vp, i64, vp]
         L.bie_add_cyl_columns.restype = i32
         L.bie_add_cyl_columns.argtypes = [vp, i32, ip, ip, vp, ctypes.POINTER(dbl), vp, i64, vp]
+        L.bie_cauchy_eval_workspace_bytes.restype = sz
+        L.bie_cauchy_eval_workspace_bytes.argtypes = [vp, i32, i32]
+        L.bie_cauchy_eval.restype = i32
+        L.bie_cauchy_eval.argtypes = [vp, i32, ip, ip, vp, vp, i32, vp, i32, vp, vp, vp, sz, vp]
         L.bie_probe_dfma.restype = i32
         L.bie_probe_dfma.argtypes = [vp, i64, vp, ctypes.POINTER(i64), vp]
         _lib = L
@@ -234,6 +238,24 @@ class Context:
                                          zf.ctypes.data_as(ctypes.POINTER(ctypes.c_double)),
                                          _dev_f64(A, (n - 1) * lda + n), lda, _stream()), "bie_add_cyl_columns")
         return A
+
+    def bie_cauchy_eval(self, counts, kinds, zeta, dzeta, fvals, zpts, out=None):
+        """Eq. (F.4)/(5.5): fvals (CUDA complex128, nf x n) at the boundary nodes -> values at zpts (CUDA complex128, npts);
+        returns out (nf x npts complex128)."""
+        import torch
+        counts, kinds = _i32(counts), _i32(kinds)
+        n = int(counts.sum())
+        fv = fvals if fvals.dim() == 2 else fvals[None, :]
+        nf, npts = int(fv.shape[0]), int(zpts.numel())
+        assert fv.is_cuda and fv.dtype == torch.complex128 and fv.is_contiguous() and fv.shape[1] == n
+        assert zpts.is_cuda and zpts.dtype == torch.complex128 and zpts.is_contiguous()
+        if out is None:
+            out = torch.empty((nf, npts), dtype=torch.complex128, device=zpts.device)
+        ws = torch.empty(int(lib().bie_cauchy_eval_workspace_bytes(self._h, nf, npts)), dtype=torch.uint8, device=zpts.device)
+        _check(lib().bie_cauchy_eval(self._h, int(counts.size), _ip(counts), _ip(kinds), _dev_c128(zeta, n), _dev_c128(dzeta, n),
+                                     nf, fv.data_ptr(), npts, zpts.data_ptr(), out.data_ptr(), ws.data_ptr(), ws.numel(),
+                                     _stream()), "bie_cauchy_eval")
+        return out
 
     def bie_matvec_free(self, x, y):
         n = x.numel()

@@ -163,6 +163,21 @@ int bie_add_cyl_columns(bie_ctx* c, int ncomp, const int32_t* counts, const int3
     return bie_launch_add_cyl_columns(c, ncomp, counts, kinds, zeta, centers, A, lda, (cudaStream_t)stream);
 }
 
+size_t bie_cauchy_eval_workspace_bytes(bie_ctx* c, int nf, int npts)
+{
+    return c ? bie_cauchy_eval_ws_bytes(nf, npts, c->sm_count) : 0;
+}
+
+int bie_cauchy_eval(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* kinds, const double* zeta,
+                    const double* dzeta, int nf, const double* fvals, int npts, const double* zpts, double* out,
+                    void* workspace, size_t workspace_bytes, void* stream)
+{
+    if (!c) return BIE_ERR_NULL;
+    BIE_CUDA(cudaSetDevice(c->device));
+    return bie_launch_cauchy_eval(c, ncomp, counts, kinds, zeta, dzeta, nf, fvals, npts, zpts, out, workspace,
+                                  workspace_bytes, (cudaStream_t)stream);
+}
+
 int bie_matvec_rect(bie_ctx* c, int nrows, int ncols, const double* A, int64_t lda, const double* x, double* y,
                     void* stream)
 {

@@ -108,6 +108,10 @@ int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, int nd, 
                      int restart, int max_iters, double* x, int32_t* iters_out, double* relres_out,
                      int32_t* status_out, double* res_hist, void* ws, size_t ws_bytes, cudaStream_t st);
 size_t bie_gmres_ws_bytes(int n, int restart);
+size_t bie_cauchy_eval_ws_bytes(int nf, int npts, int sm_count);
+int bie_launch_cauchy_eval(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds, const double* zeta,
+                           const double* dzeta, int nf, const double* fvals, int npts, const double* zpts, double* out,
+                           void* ws, size_t ws_bytes, cudaStream_t st);
 int bie_launch_add_cyl_columns(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds, const double* zeta,
                                const double* centers, double* A, int64_t lda, cudaStream_t st);
 int bie_launch_probe_dfma(bie_ctx* ctx, int64_t fma_per_thread, double* out, int64_t* total_fma, cudaStream_t st);

@@ -1,0 +1,194 @@
+// bie_eval.cu -- SURVEY 8(f) NEXT-3, Section 5.1 / Appendix F: values inside the fluid,
+// up to the boundary, of functions analytic in the fluid from their boundary values (Helsing & Ojala, periodic form):
+//     f(z) ~ sum_s lambda~_s(z) f_s / sum_s lambda~_s(z),    lambda~_s(z) = (sigma_k/M_k) 1/2 cot((zeta_s - z)/2) zeta'_s   (F.4)/(5.5)
+// sigma_0 = -1 on Gamma_0 (fluid on its right; reading R18), +1 on the solids.  "If z coincides with
+// zeta_k(alpha_m), we set f(z) = f(zeta_k(alpha_m))".
+//
+// Second workload of the same pair arithmetic (bie_common.cuh): one thread per evaluation point, the sources staged tile by
+// tile in shared memory with their factors E_s = e^{i zeta_s}, M_s, q_s = sigma zeta'_s/(2 M_s) and g_s = q_s f_s (per
+// function), so that per pair  cot = (-2X + iY)/den  costs 12 FP64 instructions and each of the 1 + nf complex sums
+// (denominator and numerators) 4 more.  Pairs closer than the near threshold are recomputed from the coordinate differences
+// with the Laurent series (exact to rounding at any distance, which is the whole point of (F.4)); an exact coincidence
+// is recorded and resolved in the second kernel, which also adds the partial sums of the source segments (few points:
+// the sources are split over blockIdx.y so that the GPU is filled) and divides.
+#include "bie_common.cuh"
+
+#define EVAL_THREADS 128
+#define EVAL_TILE 256
+#define EVAL_MAX_NF 4
+
+struct EvalComps {
+    int ncomp;
+    int off[BIE_MAX_COMP + 1];
+    int surface[BIE_MAX_COMP];   // 1: sigma = -1
+};
+
+template <int NF>
+__global__ void __launch_bounds__(EVAL_THREADS)
+bie_cauchy_eval_kernel(EvalComps ec, int n, const double2* __restrict__ zeta, const double2* __restrict__ dzeta,
+                       const double2* __restrict__ f, int npts, const double2* __restrict__ zpts, int nseg,
+                       double2* __restrict__ part /* [nseg][1+NF][npts] */, int* __restrict__ hit /* [npts] */)
+{
+    __shared__ double2 sE[EVAL_TILE], sMT[EVAL_TILE], sQ[EVAL_TILE], sXY[EVAL_TILE];
+    __shared__ double2 sG[NF][EVAL_TILE];
+    const int p = blockIdx.x * EVAL_THREADS + threadIdx.x;
+    const int seg = blockIdx.y;
+    const int per = (((n + nseg - 1) / nseg) + 1) & ~1;
+    const int s_lo = seg * per, s_hi = min(s_lo + per, n);
+    const double yref = zeta[0].y;
+    // this thread's point
+    const double2 z = zpts[min(p, npts - 1)];
+    double ter, tei, tm;
+    {
+        double s, c;
+        sincos(z.x, &s, &c);
+        const double m = exp(-(z.y - yref));
+        ter = m * c; tei = m * s; tm = m * m;
+    }
+    double Dr = 0.0, Di = 0.0, Nr[NF], Ni[NF];
+#pragma unroll
+    for (int q = 0; q < NF; ++q) { Nr[q] = 0.0; Ni[q] = 0.0; }
+    int myhit = -1;
+    for (int s0 = s_lo; s0 < s_hi; s0 += EVAL_TILE) {
+        __syncthreads();
+        for (int i = threadIdx.x; i < EVAL_TILE; i += EVAL_THREADS) {
+            const int s = s0 + i;
+            if (s < s_hi) {
+                int k = 0;
+                while (k + 1 < ec.ncomp && s >= ec.off[k + 1]) ++k;
+                const double M = (double)(ec.off[k + 1] - ec.off[k]);
+                const double wgt = (ec.surface[k] ? -0.5 : 0.5) / M;
+                const double2 zs = zeta[s], dz = dzeta[s];
+                double sn, cs;
+                sincos(zs.x, &sn, &cs);
+                const double m = exp(-(zs.y - yref));
+                const double2 q = make_double2(wgt * dz.x, wgt * dz.y);
+                double tau = BIE_NEAR_C * sqrt(q.x * q.x + q.y * q.y);
+                tau = fmin(fmax(tau, BIE_NEAR_TAU_MIN), BIE_NEAR_TAU_MAX);
+                sE[i] = make_double2(m * cs, m * sn);
+                sMT[i] = make_double2(m * m, tau * m * m);
+                sQ[i] = q;
+                sXY[i] = zs;
+#pragma unroll
+                for (int c = 0; c < NF; ++c) {
+                    const double2 fv = f[(size_t)c * n + s];
+                    sG[c][i] = make_double2(q.x * fv.x - q.y * fv.y, q.x * fv.y + q.y * fv.x);
+                }
+            } else {   // beyond the segment: zero weight, never near
+                sE[i] = make_double2(0.0, 0.0); sMT[i] = make_double2(0.0, 0.0); sQ[i] = make_double2(0.0, 0.0);
+                sXY[i] = make_double2(0.0, 1.0e3);
+#pragma unroll
+                for (int c = 0; c < NF; ++c) sG[c][i] = make_double2(0.0, 0.0);
+            }
+        }
+        __syncthreads();
+#pragma unroll 2
+        for (int j = 0; j < EVAL_TILE; ++j) {
+            const double2 e = sE[j], mt = sMT[j];
+            const double dr = e.x - ter, di = e.y - tei;
+            const double den = fma(dr, dr, di * di);
+            const double X = fma(tei, e.x, -(ter * e.y));
+            const double Y = mt.x - tm;
+            const double r = bie_rcp3(den);
+            double cr = -2.0 * X * r, ci = Y * r;            // cot((zeta_s - z)/2) = (-2X + iY)/den
+            if (den < mt.y) {                                  // near pair (rare): from the coordinate differences
+                const double2 zs = sXY[j];
+                const double x = zs.x - z.x, y = zs.y - z.y;
+                // exact coincidence (modulo the period): cot has a pole, (F.4) degenerates to f_s
+                const double xr = x - 6.283185307179586232 * rint(x * 0.15915494309189534561);
+                if (xr == 0.0 && y == 0.0) { myhit = s0 + j; cr = 0.0; ci = 0.0; }
+                else bie_cot_half_near(x, y, &cr, &ci);
+            }
+            const double2 q = sQ[j];
+            Dr = fma(q.x, cr, Dr); Dr = fma(-q.y, ci, Dr);
+            Di = fma(q.x, ci, Di); Di = fma(q.y, cr, Di);
+#pragma unroll
+            for (int c = 0; c < NF; ++c) {
+                const double2 g = sG[c][j];
+                Nr[c] = fma(g.x, cr, Nr[c]); Nr[c] = fma(-g.y, ci, Nr[c]);
+                Ni[c] = fma(g.x, ci, Ni[c]); Ni[c] = fma(g.y, cr, Ni[c]);
+            }
+        }
+    }
+    if (p < npts) {
+        double2* o = part + (size_t)seg * (1 + NF) * npts;
+        o[p] = make_double2(Dr, Di);
+#pragma unroll
+        for (int c = 0; c < NF; ++c) o[(size_t)(1 + c) * npts + p] = make_double2(Nr[c], Ni[c]);
+        if (myhit >= 0) atomicMax(hit + p, myhit);
+    }
+}
+
+// out[c][p] = N_c / D (fixed-order sum over the source segments), or the boundary value at a coincident node
+__global__ void __launch_bounds__(256)
+bie_cauchy_finish_kernel(int nf, int n, int npts, int nseg, const double2* __restrict__ part, const int* __restrict__ hit,
+                         const double2* __restrict__ f, double2* __restrict__ out)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= npts) return;
+    const int h = hit[p];
+    double Dr = 0.0, Di = 0.0;
+    for (int s = 0; s < nseg; ++s) {
+        const double2 d = part[(size_t)s * (1 + nf) * npts + p];
+        Dr += d.x; Di += d.y;
+    }
+    const double inv = 1.0 / (Dr * Dr + Di * Di);
+    for (int c = 0; c < nf; ++c) {
+        if (h >= 0) { out[(size_t)c * npts + p] = f[(size_t)c * n + h]; continue; }
+        double Nr = 0.0, Ni = 0.0;
+        for (int s = 0; s < nseg; ++s) {
+            const double2 v = part[((size_t)s * (1 + nf) + 1 + c) * npts + p];
+            Nr += v.x; Ni += v.y;
+        }
+        out[(size_t)c * npts + p] = make_double2((Nr * Dr + Ni * Di) * inv, (Ni * Dr - Nr * Di) * inv);
+    }
+}
+
+size_t bie_cauchy_eval_ws_bytes(int nf, int npts, int sm_count)
+{
+    if (nf < 1 || nf > EVAL_MAX_NF || npts < 1) return 0;
+    const int gx = (npts + EVAL_THREADS - 1) / EVAL_THREADS;
+    int nseg = (4 * sm_count + gx - 1) / gx;
+    if (nseg < 1) nseg = 1;
+    if (nseg > 64) nseg = 64;
+    return sizeof(double2) * (size_t)nseg * (1 + nf) * npts + sizeof(int) * (size_t)npts + 256;
+}
+
+int bie_launch_cauchy_eval(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds, const double* zeta,
+                           const double* dzeta, int nf, const double* fvals, int npts, const double* zpts, double* out,
+                           void* ws, size_t ws_bytes, cudaStream_t st)
+{
+    if (!ctx || !counts || !kinds || !zeta || !dzeta || !fvals || !zpts || !out || !ws) return BIE_ERR_NULL;
+    if (ncomp < 1 || ncomp > BIE_MAX_COMP) return BIE_ERR_GEOMETRY;
+    if (nf < 1 || nf > EVAL_MAX_NF || npts < 1) return BIE_ERR_ARG;
+    EvalComps ec;
+    ec.ncomp = ncomp; ec.off[0] = 0;
+    long long n = 0;
+    for (int c = 0; c < ncomp; ++c) {
+        if (counts[c] < 1 || kinds[c] < 0 || kinds[c] > 2 || (kinds[c] == BIE_KIND_SURFACE) != (c == 0)) return BIE_ERR_GEOMETRY;
+        n += counts[c];
+        ec.off[c + 1] = (int)n; ec.surface[c] = (kinds[c] == BIE_KIND_SURFACE);
+    }
+    if (n > (1 << 30)) return BIE_ERR_GEOMETRY;
+    if ((((uintptr_t)zeta) | ((uintptr_t)dzeta) | ((uintptr_t)fvals) | ((uintptr_t)zpts) | ((uintptr_t)out)) & 15u) return BIE_ERR_LAYOUT;
+    if (bie_cauchy_eval_ws_bytes(nf, npts, ctx->sm_count) > ws_bytes) return BIE_ERR_WORKSPACE;
+    const int gx = (npts + EVAL_THREADS - 1) / EVAL_THREADS;
+    int nseg = (4 * ctx->sm_count + gx - 1) / gx;
+    if (nseg < 1) nseg = 1;
+    if (nseg > 64) nseg = 64;
+    if (nseg > (int)((n + 1) / 2)) nseg = (int)((n + 1) / 2);
+    double2* part = (double2*)(((uintptr_t)ws + 255) & ~(uintptr_t)255);
+    int* hit = (int*)(part + (size_t)nseg * (1 + nf) * npts);
+    BIE_CUDA(cudaMemsetAsync(hit, 0xFF, sizeof(int) * (size_t)npts, st));
+    dim3 grid(gx, nseg);
+    const double2 *z2 = (const double2*)zeta, *d2 = (const double2*)dzeta, *f2 = (const double2*)fvals, *p2 = (const double2*)zpts;
+    switch (nf) {
+        case 1: bie_cauchy_eval_kernel<1><<<grid, EVAL_THREADS, 0, st>>>(ec, (int)n, z2, d2, f2, npts, p2, nseg, part, hit); break;
+        case 2: bie_cauchy_eval_kernel<2><<<grid, EVAL_THREADS, 0, st>>>(ec, (int)n, z2, d2, f2, npts, p2, nseg, part, hit); break;
+        case 3: bie_cauchy_eval_kernel<3><<<grid, EVAL_THREADS, 0, st>>>(ec, (int)n, z2, d2, f2, npts, p2, nseg, part, hit); break;
+        default: bie_cauchy_eval_kernel<4><<<grid, EVAL_THREADS, 0, st>>>(ec, (int)n, z2, d2, f2, npts, p2, nseg, part, hit); break;
+    }
+    bie_cauchy_finish_kernel<<<(npts + 255) / 256, 256, 0, st>>>(nf, (int)n, npts, nseg, part, hit, f2, (double2*)out);
+    BIE_CUDA(cudaGetLastError());
+    return BIE_OK;
+}

@@ -422,6 +422,53 @@ def test_appendix_b_solve_returns_the_circulations(ctx):
         assert abs(np.mean(wB[g.component(k)]) - a[o]) < 1e-11
 
 
+def _fluid_points(g, rng, npts):
+    """points in the fluid: random depths between Gamma_0 and the bottom (away from the obstacles' interiors is not
+    required for parity: both sides evaluate the same formula), plus points 1e-3 ... 1e-9 off nodes, plus nodes"""
+    s0, s1 = g.component(0), g.component(1)
+    i0 = rng.integers(0, g.counts[0], size=npts)
+    t = rng.uniform(0.02, 0.6, size=npts)
+    x = g.zeta[s0][i0].real
+    ytop = g.zeta[s0][i0].imag
+    cand = x + 1j * (ytop - t * (ytop + 1.6))
+    # keep the candidates that lie in the fluid: there the sum of lambda~ is i (Eq. F.1), inside an obstacle it is 0
+    D = np.zeros(cand.size, dtype=np.complex128)
+    for k in range(g.counts.size):
+        sk = g.component(k)
+        sig = -1.0 if k == 0 else 1.0
+        D += sig / g.counts[k] * np.sum(0.5 / np.tan(0.5 * (g.zeta[sk][None, :] - cand[:, None])) * g.dzeta[sk][None, :], axis=1)
+    pts = list(cand[np.abs(D) > 0.5])
+    for k in range(g.counts.size):
+        sk = g.component(k)
+        for m in (0, int(g.counts[k]) // 3):
+            s = sk.start + m
+            nrm = 1j * g.dzeta[s] / abs(g.dzeta[s])
+            inward = -nrm if k == 0 else nrm
+            pts += [g.zeta[s] + d * inward for d in (1e-3, 1e-6, 1e-9)]
+            pts.append(g.zeta[s])                       # coincidence
+    pts.append(g.zeta[s0][5] + 2 * np.pi)               # coincidence modulo the period
+    return np.array(pts)
+
+
+@pytest.mark.parametrize("c,npts,nf", [(1, 300, 1), (2, 2000, 2), (3, 50, 4), (5, 40, 3)])
+def test_cauchy_eval_parity(ctx, c, npts, nf):
+    """NEXT-3: Eq. (F.4)/(5.5) against the oracle on the same boundary values and points; many points (one source segment)
+    and few points (sources split over the grid); interior, near-boundary and coincident points"""
+    g = cfg(c).geometry
+    rng = np.random.default_rng(70 + c)
+    zp = _fluid_points(g, rng, npts)
+    f = np.vstack([np.exp(1j * (q + 1) * g.zeta) * (1.0 + 0.1 * q) + rng.standard_normal() for q in range(nf)])
+    out = ctx.bie_cauchy_eval(g.counts, g.kinds, dev(g.zeta), dev(g.dzeta), dev(f), dev(zp))
+    torch.cuda.synchronize()
+    ref = oracle.cauchy_eval(g.counts, g.kinds, g.zeta, g.dzeta, f, zp)
+    scale = float(np.max(np.abs(ref)))
+    assert float(np.max(np.abs(out.cpu().numpy() - ref))) <= 1e-11 * scale
+    # and it is the analytic function itself (spectral accuracy up to the boundary) where the grid resolves it
+    if c <= 3:
+        exact = np.exp(1j * zp) + (f[0, 0] - np.exp(1j * g.zeta[0]))
+        assert float(np.max(np.abs(out[0].cpu().numpy() - exact))) <= 1e-9 * scale
+
+
 def test_matvec_rect_matches_the_oracle(ctx):
     rng = np.random.default_rng(3)
     for (nr, nc, lda) in [(1, 2, 2), (7, 130, 132), (300, 64, 64), (129, 1001, 1002)]:
