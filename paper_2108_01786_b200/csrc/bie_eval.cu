@@ -158,9 +158,9 @@ int bie_launch_cauchy_eval(bie_ctx* ctx, int ncomp, const int32_t* counts, const
                            const double* dzeta, int nf, const double* fvals, int npts, const double* zpts, double* out,
                            void* ws, size_t ws_bytes, cudaStream_t st)
 {
+    if (nf < 1 || nf > EVAL_MAX_NF || npts < 1) return BIE_ERR_ARG;
     if (!ctx || !counts || !kinds || !zeta || !dzeta || !fvals || !zpts || !out || !ws) return BIE_ERR_NULL;
     if (ncomp < 1 || ncomp > BIE_MAX_COMP) return BIE_ERR_GEOMETRY;
-    if (nf < 1 || nf > EVAL_MAX_NF || npts < 1) return BIE_ERR_ARG;
     EvalComps ec;
     ec.ncomp = ncomp; ec.off[0] = 0;
     long long n = 0;

@@ -704,6 +704,48 @@ def test_error_codes(ctx):
     assert e.value.code == -4
 
 
+def test_error_codes_of_the_operator_and_next_calls(ctx):
+    import ctypes
+    from paper_2108_01786_b200 import bie
+    g = cfg(1).geometry
+    n = g.n
+    z, dz, d2z = geo_dev(g)
+    A = torch.empty((n, n), dtype=torch.float64, device="cuda")
+    ws = torch.empty(bie.Context.bie_gmres_workspace_bytes(n, 50), dtype=torch.uint8, device="cuda")
+    oi = torch.zeros(2, dtype=torch.int32, device="cuda")
+    of = torch.zeros(1, dtype=torch.float64, device="cuda")
+    b = torch.ones(n, dtype=torch.float64, device="cuda")
+    x = torch.empty_like(b)
+    ctx.bie_build_cols(g.counts, g.kinds, z, dz, d2z, 128, A)
+    for nd, code in [(127, -6), (n, -6), (0, -6)]:                    # odd, whole matrix, none
+        with pytest.raises(bie.BieError) as e:
+            ctx.bie_gmres_hybrid(A, nd, b, x, 1e-13, 50, 10, ws, oi, of)
+        assert e.value.code == code, nd
+    with pytest.raises(bie.BieError) as e:                             # empty slab
+        ctx.bie_build_cols(g.counts, g.kinds, z, dz, d2z, 0, A)
+    assert e.value.code == -6
+    with pytest.raises(bie.BieError) as e:                             # the internal node-table variant is not public
+        ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A, variant=3)
+    assert e.value.code == -6
+    with pytest.raises(bie.BieError) as e:
+        ctx.bie_set_hybrid_free_warps(16)
+    assert e.value.code == -6
+    assert ctx.bie_hybrid_cols(2) == 0 and ctx.bie_hybrid_cols(100) == 0 and ctx.bie_hybrid_cols(16384) == 6848
+    # Appendix B without centres for a geometry that has an obstacle; Cauchy evaluation with too many functions
+    rc = bie.lib().bie_add_cyl_columns(ctx._h, 3, bie._ip(bie._i32(g.counts)), bie._ip(bie._i32(g.kinds)), z.data_ptr(), None,
+                                       A.data_ptr(), n, None)
+    assert rc == -1
+    f = torch.zeros((5, n), dtype=torch.complex128, device="cuda")
+    with pytest.raises(bie.BieError) as e:
+        ctx.bie_cauchy_eval(g.counts, g.kinds, z, dz, f, z[:4].clone())
+    assert e.value.code == -6
+    # after a matrix-free-incompatible call sequence the context still works
+    ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A)
+    ctx.bie_gmres(None, b, x, 1e-13, 50, 100, ws, oi, of)
+    torch.cuda.synchronize()
+    assert int(oi[1]) == 0
+
+
 def test_probe_dfma_runs(ctx):
     out = torch.zeros(1, dtype=torch.float64, device="cuda")
     total = ctx.bie_probe_dfma(1 << 12, out)
