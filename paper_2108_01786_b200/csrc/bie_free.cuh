@@ -222,7 +222,7 @@ __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable
         // near pairs: exact entries from the CSR near matrix
         const int p0 = fp.near_ptr[8 * (size_t)t], p1 = fp.near_ptr[8 * (size_t)t + 8];
         double sn = 0.0;
-        for (int p = p0; p < p1; ++p) {
+        for (int p = p0; p < p1 && !bad; ++p) {   // (on overflow the offsets run past the arrays)
             const int cix = fp.near_col[p];
             if (cix >= fp.s_off) sn = fma(fp.near_val[p], __ldcg(xsrc + cix), sn);
         }

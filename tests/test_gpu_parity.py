@@ -223,6 +223,58 @@ def test_matvec_free_ragged(ctx, shape):
         assert rel_max(y[:g.n].cpu().numpy(), oracle.matvec(Ao, x)) <= 1e-12
 
 
+def _geometry_with_an_obstacle_close_to_the_surface(gap):
+    """flat-ish surface, flat bottom and one ellipse whose top is `gap` below the surface: near pairs ACROSS components"""
+    M0, M1, M2 = 512, 256, 384
+    eta = inputs.Series(np.array([1.0]), np.array([0.01 + 0.0j]))     # eta = 0.02 cos(alpha): lowest point -0.02 at pi
+    top = -0.02 - gap
+    parts = [inputs.graph_curve(M0, 0.0, eta), inputs.graph_curve(M1, -2.0, None),
+             inputs.ellipse_curve(M2, complex(np.pi, top - 0.2), 0.5, 0.2, 0.0)]
+    return inputs.assemble(parts, [0, 1, 2])
+
+
+@pytest.mark.parametrize("gap", [0.02, 0.004])
+def test_operators_with_near_pairs_across_components(ctx, gap):
+    """the near matrix of the matrix-free operator must catch pairs of DIFFERENT curves that come closer than
+    sqrt(taubar) (here an obstacle 0.02 / 0.004 under the free surface, node spacing 0.012): dense build, matrix-free
+    matvec and hybrid solve against the oracle"""
+    g = _geometry_with_an_obstacle_close_to_the_surface(gap)
+    n = g.n
+    Ao = oracle_build(g)
+    A = gpu_build(ctx, g)
+    assert rel_max(A.cpu().numpy()[:, :n], Ao) <= TOL_ENTRY
+    x = _x(n, 5)
+    y = torch.empty(n, dtype=torch.float64, device="cuda")
+    ctx.bie_matvec_free(dev(x), y)
+    assert rel_max(y.cpu().numpy(), oracle.matvec(Ao, x)) <= 1e-12
+    b = inputs.rhs_analytic(g, lambda z: np.exp(1j * z))
+    xo, ito, _, _, sto = oracle.gmres(Ao, b, 1e-13, 50, 2000)
+    xg, it, rr, st, S = gpu_gmres_hybrid(ctx, g, 448, b, 1e-13, 50, 2000)
+    assert sto == 0 and st == 0 and abs(it - ito) <= max(1, ito // 50)
+    assert np.linalg.norm(xg - xo) / np.linalg.norm(xo) <= TOL_X * max(1.0, np.linalg.cond(Ao) / 100.0)
+
+
+def test_near_matrix_overflow_is_loud(ctx):
+    """a 4-node obstacle next to an 8192-node surface pushes taubar to its cap (|w| < 0.1): every surface row then has
+    more near pairs than the CSR near matrix holds per node; the matrix-free operator must answer NaN, not a wrong
+    number (the dense path is unaffected)"""
+    M0 = 8192
+    parts = [inputs.graph_curve(M0, 0.0, None), inputs.graph_curve(64, -2.0, None),
+             inputs.ellipse_curve(4, complex(3.0, -1.0), 0.3, 0.2, 0.0)]
+    g = inputs.assemble(parts, [0, 1, 2])
+    z, dz, d2z = geo_dev(g)
+    ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z)
+    x = torch.ones(g.n, dtype=torch.float64, device="cuda")
+    y = torch.zeros(g.n, dtype=torch.float64, device="cuda")
+    ctx.bie_matvec_free(x, y)
+    torch.cuda.synchronize()
+    assert bool(torch.isnan(y).all())
+    A = gpu_build(ctx, g)
+    assert bool(torch.isfinite(A[:, :g.n]).all())
+    ctx.bie_matvec(A, x, y)
+    assert bool(torch.isfinite(y).all())
+
+
 # ------------------------------------------------------------------------------------------------
 # (a') vortex-sheet variant: S of Eqs. (4.14) + (4.17), adjoint matrices of Eq. (4.7)
 # ------------------------------------------------------------------------------------------------
