@@ -4,7 +4,8 @@
 // The paper ran the GEMV on the GPU and shipped every Krylov vector over PCIe to orthogonalise on the CPU
 // (PAPER.md:L857).  Here nothing leaves the device: one CTA per SM owns a contiguous block R of rows of A and,
 // with it, the same rows of every Krylov vector.  Per Arnoldi step
-//     w[R]  = A[R,:] v_j                     (bie_cta_gemv, HBM-bound; or bie_cta_matvec_free)
+//     w[R]  = A[R,:] v_j                     (bie_cta_gemv, HBM-bound; or the matrix-free pair loops of bie_free.cuh,
+//                                             FP64-bound, + one grid barrier; or both at once: hybrid operator)
 //     h    += V_j^T w ; w -= V_j h           twice (CGS2): local dots over R, one grid barrier, fixed-order sum
 //     h_{j+1,j} = ||w||                      local sum of squares, one grid barrier
 // i.e. three grid barriers per step.  v_{j+1} is never broadcast normalised: the unnormalised w goes to a
