@@ -521,6 +521,35 @@ def test_cauchy_eval_parity(ctx, c, npts, nf):
         assert float(np.max(np.abs(out[0].cpu().numpy() - exact))) <= 1e-9 * scale
 
 
+def test_stage_chain_against_a_known_potential_flow(ctx):
+    """One right-hand-side evaluation of the velocity-potential method on the GPU, against ANALYTIC truth (not the oracle):
+    build (3.16) -> GMRES -> densities -> spectral derivative -> normal-velocity operator (3.19) + (3.24).  For f analytic in
+    the fluid with b_0 = Re f, b_k = Im f the result must be s_alpha d phi/dn = Re{f'(zeta_0) i zeta_0'} (pin P9)."""
+    cot = lambda w: 1.0 / np.tan(w)
+    csc2 = lambda w: 1.0 / np.sin(w) ** 2
+    f = lambda z: (np.exp(1j * z) + 0.3 * cot(0.5 * (z - (1.0 + 0.6j))) + (0.1 + 0.04j) * cot(0.5 * (z - (-1.0j)))
+                   + 0.1j * cot(0.5 * (z - (2.0 - 2.6j))))
+    fp = lambda z: (1j * np.exp(1j * z) - 0.15 * csc2(0.5 * (z - (1.0 + 0.6j))) - 0.5 * (0.1 + 0.04j) * csc2(0.5 * (z - (-1.0j)))
+                    - 0.05j * csc2(0.5 * (z - (2.0 - 2.6j))))
+    g = inputs.small_problem(192, 192, [128], seed=3).geometry
+    b = inputs.rhs_analytic(g, f)
+    for op in ("dense", "free"):
+        A = gpu_build(ctx, g)
+        x, it, rr, st = gpu_gmres(ctx, A if op == "dense" else None, b, 1e-14, 80, 600)
+        assert st == 0
+        dom = []
+        for k in range(g.counts.size):
+            w = x[g.component(k)]
+            kk = np.fft.fftfreq(w.size, d=1.0 / w.size)
+            if w.size % 2 == 0:
+                kk[w.size // 2] = 0.0
+            dom.append(np.real(np.fft.ifft(1j * kk * np.fft.fft(w))))
+        u, N = gpu_normal_velocity(ctx, g, np.concatenate(dom))
+        s0 = g.component(0)
+        exact = np.real(fp(g.zeta[s0]) * 1j * g.dzeta[s0])
+        assert float(np.max(np.abs(u - exact))) <= 1e-9 * float(np.max(np.abs(exact))), op
+
+
 def test_matvec_rect_matches_the_oracle(ctx):
     rng = np.random.default_rng(3)
     for (nr, nc, lda) in [(1, 2, 2), (7, 130, 132), (300, 64, 64), (129, 1001, 1002)]:
