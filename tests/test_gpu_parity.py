@@ -521,6 +521,37 @@ def test_cauchy_eval_parity(ctx, c, npts, nf):
         assert float(np.max(np.abs(out[0].cpu().numpy() - exact))) <= 1e-9 * scale
 
 
+def test_matrix_free_and_hybrid_with_the_uncorrected_operator(ctx):
+    """variant B (no E_k term): the matrix-free operator must not apply the rank-one correction, the hybrid slab must not
+    contain it; B is singular (ker B = span{1_m}), so compare operator applications, not solves"""
+    g = cfg(2).geometry
+    n = g.n
+    Bo = oracle_build(g, variant=1)
+    z, dz, d2z = geo_dev(g)
+    ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z, variant=1)
+    x = _x(n, 21)
+    y = torch.empty(n, dtype=torch.float64, device="cuda")
+    ctx.bie_matvec_free(dev(x), y)
+    assert rel_max(y.cpu().numpy(), oracle.matvec(Bo, x)) <= 1e-12
+    ones = np.zeros(n); ones[g.component(2)] = 1.0
+    ctx.bie_matvec_free(dev(ones), y)
+    assert float(y.abs().max()) <= 1e-12           # B 1_m = 0 (pin P2), through the matrix-free operator
+    # hybrid: one Arnoldi step exposes the operator: x_1 = (b, Ab)/(Ab, Ab) Ab ... compare with the dense GMRES after 3 steps
+    b = _x(n, 22)
+    xd, itd, rrd, std_ = gpu_gmres(ctx, gpu_build(ctx, g, variant=1), b, 1e-13, 50, 3)
+    nd = 1024
+    A = torch.full((n, nd), float("nan"), dtype=torch.float64, device="cuda")
+    ctx.bie_build_cols(g.counts, g.kinds, z, dz, d2z, nd, A, variant=1)
+    from paper_2108_01786_b200 import bie
+    ws = torch.empty(bie.Context.bie_gmres_workspace_bytes(n, 50), dtype=torch.uint8, device="cuda")
+    oi = torch.zeros(2, dtype=torch.int32, device="cuda"); of = torch.zeros(1, dtype=torch.float64, device="cuda")
+    xh = torch.empty(n, dtype=torch.float64, device="cuda")
+    ctx.bie_gmres_hybrid(A, nd, dev(b), xh, 1e-13, 50, 3, ws, oi, of)
+    torch.cuda.synchronize()
+    assert int(oi[0]) == 3 and np.linalg.norm(xh.cpu().numpy() - xd) <= 1e-11 * np.linalg.norm(xd)
+    assert abs(float(of[0]) - rrd) <= 1e-10 * rrd
+
+
 def test_stage_chain_against_a_known_potential_flow(ctx):
     """One right-hand-side evaluation of the velocity-potential method on the GPU, against ANALYTIC truth (not the oracle):
     build (3.16) -> GMRES -> densities -> spectral derivative -> normal-velocity operator (3.19) + (3.24).  For f analytic in
