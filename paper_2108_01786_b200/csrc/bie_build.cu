@@ -201,6 +201,7 @@ bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long
         kap[c] = (kappa != nullptr && j == 0);
     }
     const int M0 = ct.off[1];
+    const bool same_cls = (sAB[0] == sAB[1]);
     __syncthreads();
     const bool full = (s0 + 1 < ncols);
     const bool part = (s0 < ncols);
@@ -212,8 +213,10 @@ bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long
             const int t = min(tb + r, t1 - 1);  // the tail repeats the last row (same values, same address)
             const double2 te = sE[t - t0];
             const double tm = sM[t - t0];
-            double e0 = bie_entry_fast_dagger(src[0], te, tm, sAB[0][t - t0], flag);
-            double e1 = bie_entry_fast_dagger(src[1], te, tm, sAB[1][t - t0], flag);
+            const double2 ab0 = sAB[0][t - t0];
+            const double2 ab1 = same_cls ? ab0 : sAB[1][t - t0];   // both columns on the same side of M_0, almost always
+            double e0 = bie_entry_fast_dagger(src[0], te, tm, ab0, flag);
+            double e1 = bie_entry_fast_dagger(src[1], te, tm, ab1, flag);
             if (kap[0]) { const int d = t - s0;     e0 += __ldg(kappa + (d < 0 ? d + M0 : d)); }
             if (kap[1]) { const int d = t - s0 - 1; e1 += __ldg(kappa + (d < 0 ? d + M0 : d)); }
             double* p = row + (long long)(t - tb) * lda;
