@@ -369,6 +369,11 @@ def main():
     prep_ms = build_ms
     if args.op != "dense":   # the full dense build is not part of this step: time it on its own (stand-alone calls, warm)
         build_ms = time_call(lambda: ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A), 20)
+    # a4: partial rebuild (only the blocks touching Gamma_0), stand-alone, on the matrix just built
+    ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A)
+    upd_ms = time_call(lambda: ctx.bie_build_update(g.counts, g.kinds, z, dz, d2z, A), 20)
+    M0_ = int(g.counts[0])
+    upd_entries = n * n - (n - M0_) * (n - M0_)
     mv_ms = time_call(lambda: ctx.bie_matvec(A, xv, yv), 50)
     matvec["dense"] = {"ms": mv_ms, "gbs": 8.0 * n * n / (mv_ms * 1e-3) / 1e9, "hbm_frac": 8.0 * n * n / (mv_ms * 1e-3) / 1e9 / hbm_peak()[0]}
     mf_ms = time_call(lambda: ctx.bie_matvec_free(xv, yv), 20)
@@ -482,6 +487,8 @@ def main():
                               "full bie_build, stand-alone calls outside the timed region; inside the step the %s operator "
                               "spent %.4f ms on its own preparation (node tables%s)"
                               % (args.op, prep_ms, " + slab of %d columns" % args.stored_cols if args.stored_cols else "")},
+            "build_update": {"ms": upd_ms, "entries": upd_entries, "gentries_per_s": upd_entries / (upd_ms * 1e-3) / 1e9,
+                             "share_of_matrix": upd_entries / float(n * n)},
             "gmres": {"ms": gmres_ms, "iters": iters, "relres_true": relres, "us_per_iter": gmres_ms * 1e3 / max(iters * nstage, 1),
                       "stages": nstage, "note": "ms covers all stages of the step (incl. their rebuilds after the first); iters is the last stage's"},
             "e2e": {"value": world * n * n / e2e_s / 1e9, "unit": UNIT, "ms_per_step": e2e_s * 1e3,
