@@ -521,6 +521,29 @@ def test_cauchy_eval_parity(ctx, c, npts, nf):
         assert float(np.max(np.abs(out[0].cpu().numpy() - exact))) <= 1e-9 * scale
 
 
+def test_matrix_free_at_the_papers_largest_size(ctx):
+    """n = 20224 (the paper's largest problem): more row blocks than SMs, so a CTA's slab of the matrix-free
+    operator spans several row blocks; sampled rows against the oracle, and dense vs matrix-free on the GPU"""
+    g = inputs.small_problem(10112, 5056, [2528, 2528], seed=11).geometry
+    n = g.n
+    assert n == 20224
+    x = _x(n, 31)
+    z, dz, d2z = geo_dev(g)
+    ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z)
+    y = torch.empty(n, dtype=torch.float64, device="cuda")
+    ctx.bie_matvec_free(dev(x), y)
+    rows = _sample_rows(g, np.random.default_rng(12), k=40)
+    Ao = oracle.build_rows(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, rows)
+    yo = oracle.matvec(Ao, x)
+    yg = y.cpu().numpy()
+    assert float(np.max(np.abs(yg[rows] - yo))) <= 1e-12 * max(1.0, float(np.max(np.abs(yo))))
+    A = gpu_build(ctx, g)
+    yd = torch.empty(n, dtype=torch.float64, device="cuda")
+    ctx.bie_matvec(A, dev(x), yd)
+    assert float((y - yd).abs().max()) <= 1e-12 * max(1.0, float(yd.abs().max()))
+    del A
+
+
 def test_matrix_free_and_hybrid_with_the_uncorrected_operator(ctx):
     """variant B (no E_k term): the matrix-free operator must not apply the rank-one correction, the hybrid slab must not
     contain it; B is singular (ker B = span{1_m}), so compare operator applications, not solves"""
