@@ -387,6 +387,10 @@ def main():
                                         "gentries_per_s": n * n / (vx_ms * 1e-3) / 1e9,
                                         "fp64_frac": n * n * FP64_INSTR_PER_ENTRY / (vx_ms * 1e-3) / dfma_per_s,
                                         "hbm_write_frac": 8.0 * n * n / (vx_ms * 1e-3) / 1e9 / hbm_peak()[0]}
+    ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z, variant=2)
+    vmf_ms = time_call(lambda: ctx.bie_matvec_free(xv, yv), 20)
+    next_rows["vortex_sheet_matrix"]["matrix_free_matvec_ms"] = vmf_ms
+    next_rows["vortex_sheet_matrix"]["matrix_free_fp64_frac"] = n * n * 13 / (vmf_ms * 1e-3) / dfma_per_s
     if P.centers:
         ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A, variant=1)
         cyl_ms = time_call(lambda: ctx.bie_add_cyl_columns(g.counts, g.kinds, z, P.centers, A), 10)

@@ -69,7 +69,7 @@ extern "C" {
                                   k >= 1, j >= 1 :  Im c+ - 1/2 [s==t]     (-1/2 I + K+_jk)
                                 Its trailing block (rows and columns on solids: A + M_0 lda + M_0, size n - M_0, M_0 even)
                                 is the auxiliary system (4.5); bie_gmres takes it as it is.
-                                Dense only: the matrix-free / hybrid operators apply to variants A and B. */
+                                The matrix-free and hybrid operators also serve the full S (13 FP64 instructions per pair). */
 
 typedef struct bie_ctx bie_ctx;
 

@@ -42,6 +42,7 @@ struct FreePlan {
     int UB;          // units (of 2 sources) per row block = (npad - s_off) / 2
     long long U;     // NB * UB
     int Geff;        // CTAs that take a slab (<= gridDim.x)
+    int vortex;      // 1: the vortex-sheet matrix S (BIE_VARIANT_VORTEX) instead of Eq. (3.16); see free_parts
     int s_off;       // first source of the operator (0; the hybrid operator reads the sources below it from its slab)
     double2* T;      // [4][npad]: (P,Q) class 0, (R,B) class 0, (P,Q) class 1, (R,B) class 1
     double* PB;      // [(NB + Geff)][FREE_ROWS] partial sums, part id = row block + CTA
@@ -74,14 +75,21 @@ __device__ __forceinline__ int free_block_rows(const FreePlan& fp, int b, int n)
 }
 
 // ---- step 1: per-source tables for the vector v (rows [r0, r1) of this CTA; v indexed from r0) ------------
-__device__ __forceinline__ void free_write_tables(const NodeTable& nt, const FreePlan& fp, int r0, int r1,
-                                                  const double* v /* shared or global, v[s - r0] */)
+__device__ __forceinline__ void free_write_tables(const NodeTable& nt, const CompTable& ct, const FreePlan& fp, int r0,
+                                                  int r1, const double* v /* shared or global, v[s - r0] */)
 {
     const int np = nt.npad;
     for (int s = r0 + threadIdx.x; s < r1; s += blockDim.x) {
         const double2 e = nt.E[s], q = nt.Q[s];
         const double M = nt.MT[s].x;
         const double x = v[s - r0];
+        if (fp.vortex) {   // S: the source only carries mu_s = x_s / M_j (the weight zeta' belongs to the ROW, Eq. 4.7)
+            const int j = nt.COMP[s];
+            const double mu = x / (double)(ct.off[j + 1] - ct.off[j]);
+            fp.T[s]      = make_double2(mu * e.x, mu * e.y);
+            fp.T[np + s] = make_double2(mu * M, mu);
+            continue;
+        }
         const bool src0 = (nt.COMP[s] == 0);
         // (alpha, beta): Im c -> (-2 qi, qr), Re c -> (-2 qr, -qi), -Re c -> (2 qr, qi)   (bie_common.cuh)
         double a0, b0, a1, b1;
@@ -97,7 +105,13 @@ __device__ __forceinline__ void free_write_tables(const NodeTable& nt, const Fre
 
 // ---- step 2: this CTA's slab of the (row block x source) list -> partial sums in fp.PB --------------------
 // scratch: shared, free_scratch_doubles() doubles, 16-byte aligned.  All threads of the team must call.
-__device__ __forceinline__ void free_parts(const NodeTable& nt, const FreePlan& fp, double* scratch, const Team& team)
+// VORTEX: the matrix S of Eqs. (4.14) + (4.17) (bie_build.cu, "Vortex-sheet variant"): entry x_s = (A_t X' + B_t Y')/den with
+// X' = Ei_t P_s - Er_t Q_s, Y' = R_s - M_t B_s from the class-independent tables (P,Q) = mu_s E_s, (R,B) = mu_s (M_s, 1), and the
+// row's (A_t, B_t) = (2u_i, -u_r) / +-(2u_r, u_i), u_t = zeta'_t/2, which depend on whether the SOURCE lies on Gamma_0: the
+// warp's source range is cut at M_0.  13 FP64-pipe instructions per pair.
+template <bool VORTEX>
+__device__ __forceinline__ void free_parts_impl(const NodeTable& nt, const CompTable& ct, const FreePlan& fp, double* scratch,
+                                                const Team& team)
 {
     const int lane = team.tid & 31, warp = team.warp;
     const int c = blockIdx.x;
@@ -126,17 +140,35 @@ __device__ __forceinline__ void free_parts(const NodeTable& nt, const FreePlan& 
             ter[i] = e.x; tei[i] = e.y; tm[i] = nt.MT[t].x; acc[i] = 0.0;
             thi[i] = __double2hiint(taubar * tm[i]);
         }
+        double ca[2][FREE_NT], cb[2][FREE_NT];   // VORTEX: (A_t, B_t) for sources on Gamma_0 [0] and on solids [1]
+        if (VORTEX) {
+#pragma unroll
+            for (int i = 0; i < FREE_NT; ++i) {
+                const int t = row0 + min(lane + 32 * i, rows - 1);
+                const int k = nt.COMP[t];
+                const double Mk = (double)(ct.off[k + 1] - ct.off[k]);
+                const double2 q = nt.Q[t];
+                const double ur = q.x * Mk, ui = q.y * Mk;
+                if (cls == 0) { ca[0][i] = 2.0 * ui; cb[0][i] = -ur; ca[1][i] = -2.0 * ur; cb[1][i] = -ui; }   // K+_00 ; -G+_j0
+                else          { ca[0][i] = 2.0 * ur; cb[0][i] = ui;  ca[1][i] = 2.0 * ui;  cb[1][i] = -ur; }   // G+_0k ; K+_jk
+            }
+        }
         // this warp's share of the sources, in units of 2
         const int units = (sb - sa) >> 1;
-        const int wa = sa + 2 * (int)((long long)units * warp / team.nwarp);
-        const int wb = sa + 2 * (int)((long long)units * (warp + 1) / team.nwarp);
+        const int wa_all = sa + 2 * (int)((long long)units * warp / team.nwarp);
+        const int wb_all = sa + 2 * (int)((long long)units * (warp + 1) / team.nwarp);
         const double2* TE = nt.E;
-        const double2* TPQ = fp.T + (size_t)(2 * cls) * np;
-        const double2* TRB = fp.T + (size_t)(2 * cls + 1) * np;
+        const double2* TPQ = fp.T + (VORTEX ? (size_t)0 : (size_t)(2 * cls) * np);
+        const double2* TRB = fp.T + (VORTEX ? (size_t)np : (size_t)(2 * cls + 1) * np);
         const double2 zero2 = make_double2(0.0, 0.0);
+        for (int sgm = 0; sgm < (VORTEX ? 2 : 1); ++sgm) {
+        // VORTEX: sources on Gamma_0 first, then the solids (different row coefficients); else the whole range at once
+        const int wa = VORTEX ? (sgm == 0 ? wa_all : max(wa_all, fp.M0)) : wa_all;
+        const int wb = VORTEX ? (sgm == 0 ? min(wb_all, fp.M0) : wb_all) : wb_all;
         double2 ne = zero2, npq = zero2, nrb = zero2;
         if (wa + lane < wb) { const int s = wa + lane; ne = TE[s]; npq = __ldcg(TPQ + s); nrb = __ldcg(TRB + s); }
         int buf = 0;
+        __syncwarp();
         for (int base = wa; base < wb; base += 32, buf ^= 1) {
             double2* sg = stage + buf * 96;
             sg[lane] = ne; sg[32 + lane] = npq; sg[64 + lane] = nrb;   // the other buffer may still be read
@@ -154,13 +186,21 @@ __device__ __forceinline__ void free_parts(const NodeTable& nt, const FreePlan& 
                 for (int i = 0; i < FREE_NT; ++i) {
                     const double dr = e.x - ter[i], di = e.y - tei[i];
                     const double den = fma(dr, dr, di * di);
-                    double val = fma(tei[i], pq.x, rb.x);
-                    val = fma(-ter[i], pq.y, val);
-                    val = fma(-tm[i], rb.y, val);
+                    double val;
+                    if (VORTEX) {
+                        const double X = fma(tei[i], pq.x, -(ter[i] * pq.y));
+                        const double Y = fma(-tm[i], rb.y, rb.x);
+                        val = fma(cb[sgm][i], Y, ca[sgm][i] * X);
+                    } else {
+                        val = fma(tei[i], pq.x, rb.x);
+                        val = fma(-ter[i], pq.y, val);
+                        val = fma(-tm[i], rb.y, val);
+                    }
                     const double r = bie_rcp3(den);
                     if (!(__double2hiint(den) < thi[i])) acc[i] = fma(val, r, acc[i]);
                 }
             }
+        }
         }
         // the warp sums, added in fixed order
 #pragma unroll
@@ -175,6 +215,13 @@ __device__ __forceinline__ void free_parts(const NodeTable& nt, const FreePlan& 
         u0 = ue;
         ++b;
     }
+}
+
+__device__ __forceinline__ void free_parts(const NodeTable& nt, const CompTable& ct, const FreePlan& fp, double* scratch,
+                                           const Team& team)
+{
+    if (fp.vortex) free_parts_impl<true>(nt, ct, fp, scratch, team);
+    else free_parts_impl<false>(nt, ct, fp, scratch, team);
 }
 
 // ---- step 3 (after a grid barrier): y_local[t - r0] = scale * (partials + near entries - E_k term) ---------

@@ -101,11 +101,11 @@ __device__ __forceinline__ void cta_apply(const GmresArgs& a, int r0, int r1, co
         // xin is complete in global memory; its per-source tables either were written by the row owners before
         // the last grid barrier (tables_ready) or are written here
         if (!tables_ready) {
-            free_write_tables(a.nt, a.fp, r0, r1, xin + r0);
+            free_write_tables(a.nt, a.ct, a.fp, r0, r1, xin + r0);
             grid_barrier(a.sync, target);
         }
         if (MODE == 1) {
-            free_parts(a.nt, a.fp, gpart, cta_team());
+            free_parts(a.nt, a.ct, a.fp, gpart, cta_team());
         } else {
             const int warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
 #ifdef BIE_PHASE_TIMING
@@ -114,7 +114,7 @@ __device__ __forceinline__ void cta_apply(const GmresArgs& a, int r0, int r1, co
             const unsigned long long hy_t0 = gtime();
 #endif
             if (warp < a.nwf) {
-                free_parts(a.nt, a.fp, gpart, sub_team(0, a.nwf, 1));
+                free_parts(a.nt, a.ct, a.fp, gpart, sub_team(0, a.nwf, 1));
 #ifdef BIE_PHASE_TIMING
                 if (threadIdx.x == 0) hy_acc[0] += gtime() - hy_t0;
 #endif
@@ -322,7 +322,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
             p = fma(v, v, p);
             a.wbuf[r0 + r] = v;
         }
-        if (FREE) free_write_tables(a.nt, a.fp, r0, r1, w_local);
+        if (FREE) free_write_tables(a.nt, a.ct, a.fp, r0, r1, w_local);
         p = block_sum(p, red);
         if (threadIdx.x == 0) part3[blockIdx.x] = p;
         grid_barrier(a.sync, target);
@@ -346,7 +346,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
             // a6: w = A v_j, with v_j = wbuf * inv
 #ifdef BIE_PHASE_TIMING
             if (MODE == 1) {
-                free_parts(a.nt, a.fp, gpart, cta_team());
+                free_parts(a.nt, a.ct, a.fp, gpart, cta_team());
                 PT(0)
                 grid_barrier(a.sync, target);
                 PT(1)
@@ -368,7 +368,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
                 p = fma(v, v, p);
                 a.wbuf[r0 + r] = v;
             }
-            if (FREE) free_write_tables(a.nt, a.fp, r0, r1, w_local);
+            if (FREE) free_write_tables(a.nt, a.ct, a.fp, r0, r1, w_local);
             p = block_sum(p, red);
             if (threadIdx.x == 0) part3[blockIdx.x] = p;
             grid_barrier(a.sync, target);
@@ -549,7 +549,6 @@ int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, int nd, 
     const int mode = nd > 0 ? 2 : (A == nullptr ? 1 : 0);
     const bool free_op = (mode != 0);
     if (free_op && (!ctx->have_geom || ctx->n != n)) return BIE_ERR_GEOMETRY;
-    if (free_op && ctx->variant == BIE_VARIANT_VORTEX) return BIE_ERR_ARG;   // dense only (include/bie.h)
     if (mode != 1 && (lda < (mode == 2 ? nd : n) || (lda & 1) || (((uintptr_t)A) & 15u))) return BIE_ERR_LAYOUT;
     if ((((uintptr_t)rhs) | ((uintptr_t)x)) & 15u) return BIE_ERR_LAYOUT;
     if (!ctx->coop_ok) return BIE_ERR_DEVICE;

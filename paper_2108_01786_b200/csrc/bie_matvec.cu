@@ -80,9 +80,9 @@ bie_matvec_free_kernel(NodeTable nt, CompTable ct, FreePlan fp, int rows_per_cta
     double* scratch = smem;
     double* y_local = scratch + free_scratch_doubles(FREE_THREADS);
     unsigned int target = 0;
-    free_write_tables(nt, fp, r0, r1, x + r0);
+    free_write_tables(nt, ct, fp, r0, r1, x + r0);
     grid_barrier(sync, target);
-    free_parts(nt, fp, scratch, cta_team());
+    free_parts(nt, ct, fp, scratch, cta_team());
     grid_barrier(sync, target);
     free_gather(nt, ct, fp, r0, r1, x, 1.0, scratch, y_local);
     for (int r = threadIdx.x; r < r1 - r0; r += blockDim.x) y[r0 + r] = y_local[r];
@@ -92,7 +92,6 @@ int bie_launch_matvec_free(bie_ctx* ctx, const double* x, double* y, cudaStream_
 {
     if (!ctx || !x || !y) return BIE_ERR_NULL;
     if (!ctx->have_geom) return BIE_ERR_GEOMETRY;
-    if (ctx->variant == BIE_VARIANT_VORTEX) return BIE_ERR_ARG;   // dense only (include/bie.h)
     if ((((uintptr_t)x) | ((uintptr_t)y)) & 15u) return BIE_ERR_LAYOUT;
     if (!ctx->coop_ok || ctx->sm_count > 256) return BIE_ERR_DEVICE;
     const int n = ctx->n;

@@ -20,7 +20,7 @@
 
 template <bool FILL>
 __global__ void __launch_bounds__(NEAR_THREADS)
-bie_near_kernel(NodeTable nt, const double* __restrict__ taubar, int* __restrict__ cnt /* [n][NEAR_SEG] counts or offsets */,
+bie_near_kernel(NodeTable nt, CompTable ct, int vortex, const double* __restrict__ taubar, int* __restrict__ cnt /* [n][NEAR_SEG] counts or offsets */,
                 int* __restrict__ col, double* __restrict__ val, int cap, int* __restrict__ overflow)
 {
     __shared__ double2 sE[NEAR_TILE];
@@ -59,11 +59,22 @@ bie_near_kernel(NodeTable nt, const double* __restrict__ taubar, int* __restrict
                             const double2 zs = nt.XY[s], zt = nt.XY[t], q = nt.Q[s];
                             double cr, ci;
                             bie_cot_half_near(zs.x - zt.x, zs.y - zt.y, &cr, &ci);
-                            const bool src0 = (nt.COMP[s] == 0);
-                            double al, be;   // block coefficients of Eq. (3.10) (bie_common.cuh)
-                            if (src0 == tgt0) { al = -2.0 * q.y; be = q.x; }        // Im c
-                            else if (tgt0)    { al = -2.0 * q.x; be = -q.y; }       // Re c   (G_0j)
-                            else              { al = 2.0 * q.x;  be = q.y; }        // -Re c  (-G_k0)
+                            const int j = nt.COMP[s];
+                            const bool src0 = (j == 0);
+                            double al, be;
+                            if (vortex) {   // S of Eqs. (4.14) + (4.17): weight zeta'_t/2 of the ROW, 1/M_j of the column
+                                const int k = nt.COMP[t];
+                                const double2 qt = nt.Q[t];
+                                const double Mk = (double)(ct.off[k + 1] - ct.off[k]), ms = 1.0 / (double)(ct.off[j + 1] - ct.off[j]);
+                                const double ur = qt.x * Mk * ms, ui = qt.y * Mk * ms;
+                                if (src0 == tgt0) { al = 2.0 * ui;  be = -ur; }      // Im c+
+                                else if (tgt0)    { al = -2.0 * ur; be = -ui; }      // -Re c+ (-G+_j0)
+                                else              { al = 2.0 * ur;  be = ui; }       // Re c+  (G+_0k)
+                            } else {        // block coefficients of Eq. (3.10) (bie_common.cuh)
+                                if (src0 == tgt0) { al = -2.0 * q.y; be = q.x; }        // Im c
+                                else if (tgt0)    { al = -2.0 * q.x; be = -q.y; }       // Re c   (G_0j)
+                                else              { al = 2.0 * q.x;  be = q.y; }        // -Re c  (-G_k0)
+                            }
                             v = fma(be, ci, -0.5 * al * cr);   // cot = (-2X + iY)/den
                         }
                         col[p] = s;
@@ -126,11 +137,12 @@ int bie_ensure_near(bie_ctx* ctx, cudaStream_t st)
     const NodeTable nt = bie_node_table(ctx);
     const int n = ctx->n;
     const int cap = (int)bie_near_cap(nt.npad);
+    const int vx = (ctx->variant == BIE_VARIANT_VORTEX) ? 1 : 0;
     dim3 grid((n + NEAR_THREADS - 1) / NEAR_THREADS, NEAR_SEG);
     BIE_CUDA(cudaMemsetAsync(ctx->near_overflow, 0, sizeof(int), st));
-    bie_near_kernel<false><<<grid, NEAR_THREADS, 0, st>>>(nt, ctx->taubar, ctx->near_ptr, nullptr, nullptr, cap, ctx->near_overflow);
+    bie_near_kernel<false><<<grid, NEAR_THREADS, 0, st>>>(nt, ctx->comps, vx, ctx->taubar, ctx->near_ptr, nullptr, nullptr, cap, ctx->near_overflow);
     bie_near_scan_kernel<<<1, 1024, 0, st>>>(ctx->near_ptr, n * NEAR_SEG);
-    bie_near_kernel<true><<<grid, NEAR_THREADS, 0, st>>>(nt, ctx->taubar, ctx->near_ptr, ctx->near_col, ctx->near_val, cap,
+    bie_near_kernel<true><<<grid, NEAR_THREADS, 0, st>>>(nt, ctx->comps, vx, ctx->taubar, ctx->near_ptr, ctx->near_col, ctx->near_val, cap,
                                                         ctx->near_overflow);
     BIE_CUDA(cudaGetLastError());
     ctx->near_valid = 1;

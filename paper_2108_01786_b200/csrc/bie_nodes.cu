@@ -168,11 +168,13 @@ size_t bie_free_buf_doubles(int cap)
 int bie_free_plan(const bie_ctx* ctx, int grid, int s_off, FreePlan* fp)
 {
     if (!ctx->have_geom || grid < 1 || grid > 256) return BIE_ERR_GEOMETRY;
+    if (ctx->variant == BIE_VARIANT_NORMAL_INTERNAL) return BIE_ERR_GEOMETRY;   // node tables of another operator
     if (s_off < 0 || (s_off & 1) || s_off > ctx->n) return BIE_ERR_ARG;
     const int n = ctx->n, npad = bie_npad(n);
     fp->M0 = ctx->counts[0];
     fp->NB0 = (fp->M0 + FREE_ROWS - 1) / FREE_ROWS;
     fp->NB = fp->NB0 + (n - fp->M0 + FREE_ROWS - 1) / FREE_ROWS;
+    fp->vortex = (ctx->variant == BIE_VARIANT_VORTEX) ? 1 : 0;
     fp->s_off = s_off;
     fp->UB = (npad - s_off) / 2;
     fp->U = (long long)fp->NB * fp->UB;

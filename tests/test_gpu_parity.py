@@ -340,15 +340,60 @@ def test_vortex_auxiliary_system_solve(ctx):
     assert np.linalg.norm(xg - xo) / np.linalg.norm(xo) <= TOL_X
 
 
-def test_vortex_variant_is_dense_only(ctx):
+@pytest.mark.parametrize("c", [1, 2, 3])
+def test_vortex_matrix_free_and_hybrid(ctx, c):
+    """the vortex-sheet matrix S through the matrix-free operator (13 instructions per pair, row coefficients cut at M_0)
+    and through the hybrid operator: operator application and full solve against the oracle"""
+    from paper_2108_01786_b200 import bie
+    P = cfg(c)
+    g, b = P.geometry, P.rhs[0]
+    n = g.n
+    So = oracle_build(g, variant=2)
+    z, dz, d2z = geo_dev(g)
+    ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z, variant=2)
+    x = _x(n, 80 + c)
+    y = torch.empty(n, dtype=torch.float64, device="cuda")
+    ctx.bie_matvec_free(dev(x), y)
+    assert rel_max(y.cpu().numpy(), oracle.matvec(So, x)) <= 1e-12
+    xo, ito, _, _, sto = oracle.gmres(So, b, P.tol, P.restart, P.max_iters)
+    xg, it, rr, st = gpu_gmres(ctx, None, b, P.tol, P.restart, P.max_iters)
+    assert sto == 0 and st == 0 and abs(it - ito) <= 1 and rr <= 10 * P.tol
+    assert np.linalg.norm(xg - xo) / np.linalg.norm(xo) <= TOL_X
+    nd = ctx.bie_hybrid_cols(n)
+    A = torch.full((n, nd), float("nan"), dtype=torch.float64, device="cuda")
+    ctx.bie_build_cols(g.counts, g.kinds, z, dz, d2z, nd, A, variant=2)
+    ws = torch.empty(bie.Context.bie_gmres_workspace_bytes(n, P.restart), dtype=torch.uint8, device="cuda")
+    oi = torch.zeros(2, dtype=torch.int32, device="cuda"); of = torch.zeros(1, dtype=torch.float64, device="cuda")
+    xh = torch.empty(n, dtype=torch.float64, device="cuda")
+    ctx.bie_gmres_hybrid(A, nd, dev(b), xh, P.tol, P.restart, P.max_iters, ws, oi, of)
+    torch.cuda.synchronize()
+    assert int(oi[1]) == 0 and abs(int(oi[0]) - ito) <= 1
+    assert np.linalg.norm(xh.cpu().numpy() - xo) / np.linalg.norm(xo) <= TOL_X
+    ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z)
+
+
+def test_vortex_matrix_free_ragged(ctx):
+    g = inputs.small_problem(301, 171, [33, 2, 129]).geometry
+    So = oracle_build(g, variant=2)
+    z, dz, d2z = geo_dev(g)
+    ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z, variant=2)
+    x = _x(g.n, 3)
+    y = torch.empty(g.n + (g.n & 1), dtype=torch.float64, device="cuda")[:g.n]
+    ctx.bie_matvec_free(dev(x), y)
+    assert rel_max(y.cpu().numpy(), oracle.matvec(So, x)) <= 1e-12
+    ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z)
+
+
+def test_normal_velocity_tables_do_not_serve_the_matrix_free_operator(ctx):
     from paper_2108_01786_b200 import bie
     g = cfg(1).geometry
     z, dz, d2z = geo_dev(g)
-    ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z, variant=2)
+    N = torch.empty((int(g.counts[0]), g.n), dtype=torch.float64, device="cuda")
+    ctx.bie_build_normal_velocity(g.counts, g.kinds, z, dz, d2z, N)
     x = torch.zeros(g.n, dtype=torch.float64, device="cuda")
     with pytest.raises(bie.BieError) as e:
         ctx.bie_matvec_free(x, torch.empty_like(x))
-    assert e.value.code == -6
+    assert e.value.code == -2
     ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z)
 
 
