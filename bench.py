@@ -36,7 +36,9 @@ if ROOT not in sys.path:
 METRIC = "matrix build Gentries/s and GMRES solve ms (FP64); % of FP64 / HBM roofline"
 UNIT = "Gentries/s"
 FP64_INSTR_PER_ENTRY = 13      # FP64-pipe instructions per stored matrix entry (SASS count)
-FP64_INSTR_PER_PAIR_FREE = 11  # matrix-free operator: FP64-pipe instructions per pair incl. the accumulation (bie_free.cuh)
+FP64_INSTR_PER_PAIR_FREE = 11  # one-directional pair loops (hybrid operator): FP64-pipe instructions per entry (bie_free.cuh)
+FP64_INSTR_PER_ENTRY_SYM = 7.7  # symmetric pair loops (whole-matrix matrix-free operator, bie_free_sym.cuh): 15 per pair of
+                                # entries + 9 DADD of the lane reduction per 32 pairs, i.e. 7.64 per entry; own blocks 11
 HBM_FALLBACK_GBS = 6650.0      # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 # dram__bytes_read.sum + dram__bytes_write.sum of the GMRES kernel, one launch, from the committed ncu capture
 # (profiles/r01_ncu_full_gmres_cfg5.md); None for workloads that were not captured
@@ -378,7 +380,8 @@ def main():
     matvec["dense"] = {"ms": mv_ms, "gbs": 8.0 * n * n / (mv_ms * 1e-3) / 1e9, "hbm_frac": 8.0 * n * n / (mv_ms * 1e-3) / 1e9 / hbm_peak()[0]}
     mf_ms = time_call(lambda: ctx.bie_matvec_free(xv, yv), 20)
     matvec["matrix_free"] = {"ms": mf_ms, "gentries_per_s": n * n / (mf_ms * 1e-3) / 1e9,
-                             "fp64_frac": n * n * FP64_INSTR_PER_PAIR_FREE / (mf_ms * 1e-3) / dfma_per_s}
+                             "fp64_instr_per_entry": FP64_INSTR_PER_ENTRY_SYM,
+                             "fp64_frac": n * n * FP64_INSTR_PER_ENTRY_SYM / (mf_ms * 1e-3) / dfma_per_s}
 
     # ---- SURVEY 8(f) NEXT rows built so far, stand-alone calls outside the timed region ----------------------------
     next_rows = {}
@@ -456,11 +459,12 @@ def main():
     if args.op != "dense":
         sc = args.stored_cols          # 0 (matrix-free) or the slab width (hybrid)
         pairs = ng * n * (n - sc)
-        instr = pairs * FP64_INSTR_PER_PAIR_FREE + ng * n * sc          # + one DFMA per streamed slab entry
+        per_entry = FP64_INSTR_PER_PAIR_FREE if sc else FP64_INSTR_PER_ENTRY_SYM   # hybrid: one-directional loops
+        instr = pairs * per_entry + ng * n * sc          # + one DFMA per streamed slab entry
         roof = {"bound": "alu", "kernel": "bie_gmres_kernel<%s> (persistent; pair loops dominate)" % args.op,
                 "achieved": instr / (gmres_ms * 1e-3) / 1e12, "peak": dfma_per_s / 1e12,
                 "unit": "T FP64 instr/s", "traffic": TRAFFIC_BYTES.get((args.config, args.op)),
-                "fp64_instr_per_pair": FP64_INSTR_PER_PAIR_FREE,
+                "fp64_instr_per_entry": per_entry,
                 "pairs_per_launch": pairs, "operator_applications_per_launch": ng,
                 "peak_source": "bie_probe_dfma in this run (nominal 148 SM x 64 lanes x 1.965 GHz = 18.6)"}
         if sc:   # the slab is streamed from HBM by the other warps at the same time

@@ -24,7 +24,7 @@ EXPORTS = ("bie_create", "bie_destroy", "bie_strerror", "bie_device_info", "bie_
            "bie_set_geometry", "bie_matvec", "bie_matvec_free", "bie_gmres_workspace_bytes", "bie_gmres",
            "bie_solve_workspace_bytes", "bie_solve_host", "bie_probe_dfma", "bie_build_cols", "bie_hybrid_cols",
            "bie_set_hybrid_free_warps", "bie_gmres_hybrid", "bie_matvec_rect", "bie_build_normal_velocity",
-           "bie_add_cyl_columns", "bie_cauchy_eval_workspace_bytes", "bie_cauchy_eval")
+           "bie_add_cyl_columns", "bie_cauchy_eval_workspace_bytes", "bie_cauchy_eval", "bie_set_symmetric")
 
 BIE_OK, BIE_MAX_ITERS = 0, 1
 OP_DENSE, OP_FREE, OP_HYBRID = 0, 1, 2
@@ -93,6 +93,8 @@ def lib() -> ctypes.CDLL:
         L.bie_cauchy_eval_workspace_bytes.argtypes = [vp, i32, i32]
         L.bie_cauchy_eval.restype = i32
         L.bie_cauchy_eval.argtypes = [vp, i32, ip, ip, vp, vp, i32, vp, i32, vp, vp, vp, sz, vp]
+        L.bie_set_symmetric.restype = i32
+        L.bie_set_symmetric.argtypes = [vp, i32]
         L.bie_probe_dfma.restype = i32
         L.bie_probe_dfma.argtypes = [vp, i64, vp, ctypes.POINTER(i64), vp]
         _lib = L
@@ -256,6 +258,9 @@ class Context:
                                      nf, fv.data_ptr(), npts, zpts.data_ptr(), out.data_ptr(), ws.data_ptr(), ws.numel(),
                                      _stream()), "bie_cauchy_eval")
         return out
+
+    def bie_set_symmetric(self, on: bool):
+        _check(lib().bie_set_symmetric(self._h, int(bool(on))), "bie_set_symmetric")
 
     def bie_matvec_free(self, x, y):
         n = x.numel()

@@ -1,6 +1,7 @@
 // bie_api.cu -- the extern "C" boundary declared in include/bie.h: argument checks, ctx life cycle, the
 // host-buffer end-to-end call and the DFMA roofline probe.  All arithmetic of the method is in the kernels
 // of bie_nodes.cu / bie_build.cu / bie_matvec.cu / bie_gmres.cu.
+#include <cstdlib>
 #include <new>
 #include "bie_common.cuh"
 
@@ -29,6 +30,8 @@ int bie_create(bie_ctx** out, int device)
     c->near_ptr = nullptr; c->near_col = nullptr; c->near_val = nullptr; c->near_valid = 0;
     c->hybrid_free_warps = BIE_HYBRID_FREE_WARPS;
     c->taubar = nullptr; c->near_overflow = nullptr; c->kappa = nullptr;
+    c->pc_buf = nullptr; c->pc_cap = 0;
+    c->use_sym = 1;   // bie_set_symmetric
     if (cudaMalloc((void**)&c->sync_buf, 256) != cudaSuccess ||
         cudaMallocHost((void**)&c->pinned_i, 4 * sizeof(int32_t)) != cudaSuccess ||
         cudaMallocHost((void**)&c->pinned_d, 4 * sizeof(double)) != cudaSuccess) {
@@ -56,6 +59,7 @@ int bie_destroy(bie_ctx* c)
     if (c->near_col) cudaFree(c->near_col);
     if (c->near_val) cudaFree(c->near_val);
     if (c->kappa) cudaFree(c->kappa);
+    if (c->pc_buf) cudaFree(c->pc_buf);
     if (c->sync_buf) cudaFree(c->sync_buf);
     if (c->pinned_i) cudaFreeHost(c->pinned_i);
     if (c->pinned_d) cudaFreeHost(c->pinned_d);
@@ -138,6 +142,13 @@ int bie_hybrid_cols(bie_ctx* c, int n)
     if (nd < 64) nd = 0;            // too small to be worth two teams: use bie_gmres
     if (nd > n - 2) nd = (n - 2) & ~1;
     return nd;
+}
+
+int bie_set_symmetric(bie_ctx* c, int on)
+{
+    if (!c) return BIE_ERR_NULL;
+    c->use_sym = on ? 1 : 0;
+    return BIE_OK;
 }
 
 int bie_set_hybrid_free_warps(bie_ctx* c, int free_warps)

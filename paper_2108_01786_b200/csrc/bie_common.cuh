@@ -63,6 +63,9 @@ struct bie_ctx {
     double* near_val;        // [BIE_NEAR_PER_NODE cap]
     int* near_overflow;      // device flag: the near matrix did not fit (the operator then returns NaN)
     int near_valid;          // near matrix built for the current geometry
+    double* pc_buf;          // symmetric matrix-free operator: reverse partials [row blocks][npad] (bie_free_sym.cuh)
+    size_t pc_cap;           // doubles allocated in pc_buf
+    int use_sym;             // use the symmetric work split for the whole-matrix matrix-free operator
     double* kappa;           // [cap] real-cot table of the normal-velocity operator (bie_build_normal_velocity)
     int hybrid_free_warps;   // hybrid operator: warps per CTA on the pair loops (the other 16 - this stream the slab)
     unsigned int* sync_buf;  // grid-barrier counter
@@ -92,7 +95,7 @@ NodeTable bie_node_table(const bie_ctx* ctx);
 struct FreePlan;
 // doubles of ctx->free_buf for a node capacity `cap`; work split of the matrix-free operator over `grid` CTAs
 size_t bie_free_buf_doubles(int cap);
-int bie_free_plan(const bie_ctx* ctx, int grid, int s_off, FreePlan* fp);
+int bie_free_plan(const bie_ctx* ctx, int grid, int s_off, FreePlan* fp, cudaStream_t st);
 size_t bie_near_cap(int npad);
 int bie_ensure_near(bie_ctx* ctx, cudaStream_t st);
 

@@ -33,7 +33,7 @@
 #define FREE_WARPS (FREE_THREADS / 32)
 #define FREE_NT 4
 #define FREE_ROWS (32 * FREE_NT)
-#define FREE_STAGE_DOUBLES (FREE_WARPS * 2 * 3 * 32 * 2)
+#define FREE_STAGE_DOUBLES (FREE_WARPS * 2 * 4 * 32 * 2)   // room for the 4 staged arrays of bie_free_sym.cuh; 3 are used here
 
 // host-computed description of the work split (by value into the kernels)
 struct FreePlan {
@@ -42,6 +42,11 @@ struct FreePlan {
     int UB;          // units (of 2 sources) per row block = (npad - s_off) / 2
     long long U;     // NB * UB
     int Geff;        // CTAs that take a slab (<= gridDim.x)
+    int sym;         // 1: symmetric (oddness) work split of bie_free_sym.cuh: U = sources of the triangular list, PC valid
+    double* PC;      // sym: [NB][npad] reverse partial sums (row block I, source s)
+    const long long* sym_cum;   // sym: [NB + 1] sources before position k of the (permuted) triangular list
+    const int* sym_perm;        // sym: [NB] row block at position k
+    const int* sym_pos;         // sym: [NB] position of row block b
     int vortex;      // 1: the vortex-sheet matrix S (BIE_VARIANT_VORTEX) instead of Eq. (3.16); see free_parts
     int s_off;       // first source of the operator (0; the hybrid operator reads the sources below it from its slab)
     double2* T;      // [4][npad]: (P,Q) class 0, (R,B) class 0, (P,Q) class 1, (R,B) class 1
@@ -217,10 +222,13 @@ __device__ __forceinline__ void free_parts_impl(const NodeTable& nt, const CompT
     }
 }
 
+__device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePlan& fp, double* scratch);
+
 __device__ __forceinline__ void free_parts(const NodeTable& nt, const CompTable& ct, const FreePlan& fp, double* scratch,
                                            const Team& team)
 {
-    if (fp.vortex) free_parts_impl<true>(nt, ct, fp, scratch, team);
+    if (fp.sym) free_parts_sym(nt, fp, scratch);           // whole CTA (the plan sets sym only for s_off == 0, variants A/B)
+    else if (fp.vortex) free_parts_impl<true>(nt, ct, fp, scratch, team);
     else free_parts_impl<false>(nt, ct, fp, scratch, team);
 }
 
@@ -252,20 +260,52 @@ __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable
         }
     }
     __syncthreads();
+    // symmetric work split: row t of block J also receives sum_{I < J} PC[I][t].  These are up to NB - 1 loads per row, each
+    // from another L2 line: four threads share a row (I = q, q + 4, ...; eight loads in flight each) and the four partial
+    // sums are added in fixed order.  rsum lives in the staging area (free again).
+    double* rsum = scratch;   // [rows]
+    if (fp.sym) {
+        double* rpart = scratch + ((r1 - r0 + 1) & ~1);   // [4][rows]
+        const int rows = r1 - r0;
+        for (int w = threadIdx.x; w < 4 * rows; w += blockDim.x) {
+            const int q = w / rows, lr = w - q * rows;
+            const int t = r0 + lr;
+            const int b = t < fp.M0 ? t / FREE_ROWS : fp.NB0 + (t - fp.M0) / FREE_ROWS;
+            const double* pc = fp.PC + t;
+            double a0 = 0.0, a1 = 0.0;
+            int I = q;
+            for (; I + 28 < b; I += 32) {
+                double v[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) v[k] = __ldcg(pc + (size_t)(I + 4 * k) * nt.npad);
+#pragma unroll
+                for (int k = 0; k < 8; k += 2) { a0 += v[k]; a1 += v[k + 1]; }
+            }
+            for (; I < b; I += 4) a0 += __ldcg(pc + (size_t)I * nt.npad);
+            rpart[q * rows + lr] = a0 + a1;
+        }
+        __syncthreads();
+        for (int lr = threadIdx.x; lr < rows; lr += blockDim.x)
+            rsum[lr] = (rpart[lr] + rpart[rows + lr]) + (rpart[2 * rows + lr] + rpart[3 * rows + lr]);
+        __syncthreads();
+    }
     const bool bad = (__ldcg(fp.near_overflow) != 0);
     for (int t = r0 + threadIdx.x; t < r1; t += blockDim.x) {
         int b, off;
         if (t < fp.M0) { b = t / FREE_ROWS; off = t - b * FREE_ROWS; }
         else { const int d = t - fp.M0; b = d / FREE_ROWS; off = d - b * FREE_ROWS; b += fp.NB0; }
-        const long long X0 = (long long)b * fp.UB, X1 = X0 + fp.UB;
+        const int kpos = fp.sym ? __ldg(fp.sym_pos + b) : b;   // position of the block in the work list
+        const long long X0 = fp.sym ? __ldg(fp.sym_cum + kpos) : (long long)b * fp.UB;
+        const long long X1 = fp.sym ? __ldg(fp.sym_cum + kpos + 1) : X0 + fp.UB;
         int c_lo = (int)(((X0 + 1) * fp.Geff + fp.U - 1) / fp.U) - 1;
         int c_hi = (int)((X1 * fp.Geff + fp.U - 1) / fp.U) - 1;
         c_lo = max(c_lo, 0); c_hi = min(c_hi, fp.Geff - 1);
         double s = 0.0;
         for (int c = c_lo; c <= c_hi; ++c) {
             const long long a = max(free_slab_start(fp, c), X0), e = min(free_slab_start(fp, c + 1), X1);
-            if (a < e) s += __ldcg(fp.PB + (size_t)(b + c) * FREE_ROWS + off);
+            if (a < e) s += __ldcg(fp.PB + (size_t)(kpos + c) * FREE_ROWS + off);
         }
+        if (fp.sym) s += rsum[t - r0];   // reverse partials of the earlier row blocks (summed above)
         // near pairs: exact entries from the CSR near matrix
         const int p0 = fp.near_ptr[8 * (size_t)t], p1 = fp.near_ptr[8 * (size_t)t + 8];
         double sn = 0.0;
@@ -280,3 +320,5 @@ __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable
     }
     __syncthreads();
 }
+
+#include "bie_free_sym.cuh"   // free_parts_sym (declared above)

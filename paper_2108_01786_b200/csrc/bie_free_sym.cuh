@@ -1,0 +1,197 @@
+// bie_free_sym.cuh -- the matrix-free operator of bie_free.cuh using the ODDNESS of the kernel:
+//     cot((zeta_s - zeta_t)/2) = -cot((zeta_t - zeta_s)/2),
+// so den = |E_s - E_t|^2, its reciprocal and the differences E_s - E_t serve the entry (t,s) AND the entry (s,t) of
+// Eq. (3.16) (SURVEY section 7 "oddness").  Per pair of entries: 2 sub + 2 den + 3 rcp shared, 3 + 1 FMA for each direction:
+// 15 FP64-pipe instructions for two entries instead of 22, plus the lane reduction of the reverse sums.
+//
+// Work split.  Row block I (FREE_ROWS rows of one class) x the sources s >= row0(I): the block's own rows one-directionally
+// (all their pairs are inside), the later sources symmetrically -- forward A[t][s] x_s into the lane's register sums as in
+// bie_free.cuh, reverse A[s][t] x_t summed over the 128 targets of the block into a per-(row block, source) partial
+// PC[I][s] in L2.  The triangular list is cut into equal slabs of sources, one per CTA.  The owner of row t (block J)
+// gathers the forward partials of J and  sum_{I < J} PC[I][t]  in fixed order: deterministic.
+// Reverse sums of 8 consecutive sources are reduced over the lanes together by a transposing butterfly (9 shuffles).
+// Near pairs: forward skipped when den < taubar M_t, reverse when den < taubar M_s -- the row-based rule of bie_near.cu,
+// whose CSR matrix supplies both.
+#pragma once
+#include "bie_free.cuh"
+
+#define SYM_BATCH 8
+
+// The triangular list is laid out in the order perm[0], perm[1], ... = 0, NB-1, 1, NB-2, ... (long and short source lists
+// alternate, so that every CTA's slab holds one or two long parts and at most a few short ones); cum[k] = sources before
+// position k.  Host-computed tables in device memory (FreePlan::sym_cum / sym_perm / sym_pos).
+__device__ __forceinline__ int sym_find_pos(const FreePlan& fp, long long u)
+{
+    int lo = 0, hi = fp.NB - 1;   // largest k with cum[k] <= u
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (__ldg(fp.sym_cum + mid) <= u) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
+
+// the lanes hold rev[0..7] = their partial reverse sums for 8 sources; afterwards every lane holds in its return value
+// the warp total of source (lane >> 2)
+__device__ __forceinline__ double sym_butterfly(double (&rev)[SYM_BATCH], int lane)
+{
+#pragma unroll
+    for (int h = 4, m = 16; h >= 1; h >>= 1, m >>= 1) {
+        const bool up = (lane & m) != 0;
+#pragma unroll
+        for (int q = 0; q < h; ++q) {
+            const double send = up ? rev[q] : rev[q + h];
+            const double keep = up ? rev[q + h] : rev[q];
+            rev[q] = keep + __shfl_xor_sync(0xffffffffu, send, m);
+        }
+    }
+    double v = rev[0];
+    v += __shfl_xor_sync(0xffffffffu, v, 2);
+    v += __shfl_xor_sync(0xffffffffu, v, 1);
+    return v;
+}
+
+#define SYM_STAGE_DOUBLES (FREE_WARPS * 2 * 4 * 32 * 2)   // [16 warps][2 buffers][4 arrays][32] double2
+
+// this CTA's slab of the triangular (row block x later sources) list -> forward partials in fp.PB, reverse partials in fp.PC.
+// scratch: shared, >= SYM_STAGE_DOUBLES + FREE_WARPS * FREE_ROWS doubles.  All threads of the CTA must call.
+__device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePlan& fp, double* scratch)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    const int c = blockIdx.x;
+    if (c >= fp.Geff) return;
+    double2* stage = reinterpret_cast<double2*>(scratch) + warp * (2 * 4 * 32);
+    double* wsum = scratch + SYM_STAGE_DOUBLES;
+    const int np = nt.npad;
+    const double taubar = __ldg(fp.taubar);
+    long long u0 = (long long)c * fp.U / fp.Geff;
+    const long long u1 = (long long)(c + 1) * fp.U / fp.Geff;
+    int k = sym_find_pos(fp, u0);
+    const double2 zero2 = make_double2(0.0, 0.0);
+    while (u0 < u1) {
+        const int b = __ldg(fp.sym_perm + k);
+        const long long ub = __ldg(fp.sym_cum + k);
+        const long long ue = min(u1, __ldg(fp.sym_cum + k + 1));
+        const int cls = b < fp.NB0 ? 0 : 1;
+        const int row0 = free_block_row0(fp, b);
+        const int rows = free_block_rows(fp, b, nt.n);
+        const int sa = row0 + (int)(u0 - ub), sb = row0 + (int)(ue - ub);   // sources [sa, sb), all >= row0
+        double ter[FREE_NT], tei[FREE_NT], tm[FREE_NT], acc[FREE_NT];
+        int thi[FREE_NT];
+        bool live[FREE_NT];
+#pragma unroll
+        for (int i = 0; i < FREE_NT; ++i) {
+            live[i] = (lane + 32 * i < rows);
+            const int t = row0 + min(lane + 32 * i, rows - 1);   // inactive slots shadow the last row; forward result dropped
+            const double2 e = nt.E[t];
+            ter[i] = e.x; tei[i] = e.y; tm[i] = nt.MT[t].x; acc[i] = 0.0;
+            thi[i] = __double2hiint(taubar * tm[i]);
+        }
+        const int span = sb - sa;
+        const int wa_all = sa + (int)((long long)span * warp / nwarp);
+        const int wb_all = sa + (int)((long long)span * (warp + 1) / nwarp);
+        const int d_end = row0 + rows;                       // end of the block's own rows
+        const int c_end = (cls == 0) ? fp.M0 : np;           // end of the sources of the block's own class
+        const double2* TPQ = fp.T + (size_t)(2 * cls) * np;      // forward tables: the class of the block's rows
+        const double2* TRB = fp.T + (size_t)(2 * cls + 1) * np;
+        for (int sgm = 0; sgm < 3; ++sgm) {
+            // 0: own rows (one direction); 1: later sources of the same class; 2: sources on solids below a Gamma_0 block
+            const int lo = sgm == 0 ? row0 : (sgm == 1 ? d_end : c_end);
+            const int hi = sgm == 0 ? d_end : (sgm == 1 ? c_end : np);
+            const int wa = max(wa_all, lo), wb = min(wb_all, hi);
+            if (wa >= wb) continue;                          // warp-uniform
+            const bool rev = (sgm != 0);
+            const int rcls = (sgm == 2) ? 1 : cls;           // class of the ROWS of the reverse entries (= of these sources)
+            double tp[FREE_NT], tq[FREE_NT], tr[FREE_NT], tb[FREE_NT];
+#pragma unroll
+            for (int i = 0; i < FREE_NT; ++i) {
+                tp[i] = tq[i] = tr[i] = tb[i] = 0.0;
+                if (rev && live[i]) {                        // this target as a SOURCE of rows of class rcls
+                    const int t = row0 + lane + 32 * i;
+                    const double2 pq = __ldcg(fp.T + (size_t)(2 * rcls) * np + t), rb = __ldcg(fp.T + (size_t)(2 * rcls + 1) * np + t);
+                    tp[i] = pq.x; tq[i] = pq.y; tr[i] = rb.x; tb[i] = rb.y;
+                }
+            }
+            double2 ne = zero2, npq = zero2, nrb = zero2, nmt = zero2;
+            if (wa + lane < wb) {
+                const int s = wa + lane;
+                ne = nt.E[s]; npq = __ldcg(TPQ + s); nrb = __ldcg(TRB + s);
+                const double M = nt.MT[s].x; nmt = make_double2(M, taubar * M);
+            }
+            int buf = 0;
+            __syncwarp();
+            for (int base = wa; base < wb; base += 32, buf ^= 1) {
+                double2* sg = stage + buf * 128;
+                sg[lane] = ne; sg[32 + lane] = npq; sg[64 + lane] = nrb; sg[96 + lane] = nmt;
+                __syncwarp();
+                {
+                    const int s = base + 32 + lane;
+                    ne = zero2; npq = zero2; nrb = zero2; nmt = zero2;
+                    if (s < wb) {
+                        ne = nt.E[s]; npq = __ldcg(TPQ + s); nrb = __ldcg(TRB + s);
+                        const double M = nt.MT[s].x; nmt = make_double2(M, taubar * M);
+                    }
+                }
+                const int cnt = min(32, wb - base);
+                if (!rev) {
+#pragma unroll 2
+                    for (int j = 0; j < cnt; ++j) {
+                        const double2 e = sg[j], pq = sg[32 + j], rb = sg[64 + j];
+#pragma unroll
+                        for (int i = 0; i < FREE_NT; ++i) {
+                            const double dr = e.x - ter[i], di = e.y - tei[i];
+                            const double den = fma(dr, dr, di * di);
+                            double val = fma(tei[i], pq.x, rb.x);
+                            val = fma(-ter[i], pq.y, val);
+                            val = fma(-tm[i], rb.y, val);
+                            const double r = bie_rcp3(den);
+                            if (!(__double2hiint(den) < thi[i])) acc[i] = fma(val, r, acc[i]);
+                        }
+                    }
+                } else {
+                    for (int j0 = 0; j0 < cnt; j0 += SYM_BATCH) {   // sources beyond cnt are zero sources; not written
+                        double rv[SYM_BATCH];
+#pragma unroll
+                        for (int u = 0; u < SYM_BATCH; ++u) {
+                            const int j = j0 + u;
+                            const double2 e = sg[j], pq = sg[32 + j], rb = sg[64 + j], mt = sg[96 + j];
+                            const int thj = __double2hiint(mt.y);
+                            double s_rev = 0.0;
+#pragma unroll
+                            for (int i = 0; i < FREE_NT; ++i) {
+                                const double dr = e.x - ter[i], di = e.y - tei[i];
+                                const double den = fma(dr, dr, di * di);
+                                double val = fma(tei[i], pq.x, rb.x);
+                                val = fma(-ter[i], pq.y, val);
+                                val = fma(-tm[i], rb.y, val);
+                                const double r = bie_rcp3(den);
+                                const int dh = __double2hiint(den);
+                                if (!(dh < thi[i])) acc[i] = fma(val, r, acc[i]);
+                                // reverse entry A[s][t] x_t: row s (E_s, M_s), source t (its tables for the class of s)
+                                double vr = fma(e.y, tp[i], tr[i]);
+                                vr = fma(-e.x, tq[i], vr);
+                                vr = fma(-mt.x, tb[i], vr);
+                                if (!(dh < thj)) s_rev = fma(vr, r, s_rev);
+                            }
+                            rv[u] = s_rev;
+                        }
+                        const double tot = sym_butterfly(rv, lane);
+                        const int j = j0 + (lane >> 2);
+                        if ((lane & 3) == 0 && j < cnt) fp.PC[(size_t)b * np + base + j] = tot;
+                    }
+                }
+            }
+        }
+        // the warp sums of the forward direction, added in fixed order
+#pragma unroll
+        for (int i = 0; i < FREE_NT; ++i) wsum[warp * FREE_ROWS + lane + 32 * i] = acc[i];
+        __syncthreads();
+        for (int r = threadIdx.x; r < FREE_ROWS; r += blockDim.x) {
+            double s = 0.0;
+            for (int w = 0; w < nwarp; ++w) s += wsum[w * FREE_ROWS + r];
+            fp.PB[(size_t)(k + c) * FREE_ROWS + r] = s;
+        }
+        __syncthreads();
+        u0 = ue;
+        ++k;
+    }
+}

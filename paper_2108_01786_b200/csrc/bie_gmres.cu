@@ -577,7 +577,7 @@ int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, int nd, 
         a.nt = bie_node_table(ctx); a.ct = ctx->comps;
         rc = bie_ensure_near(ctx, st);
         if (rc != BIE_OK) return rc;
-        rc = bie_free_plan(ctx, pl.G, nd, &a.fp);
+        rc = bie_free_plan(ctx, pl.G, nd, &a.fp, st);
         if (rc != BIE_OK) return rc;
     }
     BIE_CUDA(cudaMemsetAsync(ctx->sync_buf, 0, sizeof(unsigned int), st));

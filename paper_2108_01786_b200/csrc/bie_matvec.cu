@@ -102,7 +102,7 @@ int bie_launch_matvec_free(bie_ctx* ctx, const double* x, double* y, cudaStream_
     FreePlan fp;
     int rc = bie_ensure_near(ctx, st);
     if (rc != BIE_OK) return rc;
-    rc = bie_free_plan(ctx, G, 0, &fp);
+    rc = bie_free_plan(ctx, G, 0, &fp, st);
     if (rc != BIE_OK) return rc;
     BIE_CUDA(cudaFuncSetAttribute(bie_matvec_free_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     BIE_CUDA(cudaMemsetAsync(ctx->sync_buf, 0, sizeof(unsigned int), st));

@@ -7,6 +7,8 @@
 // limit K_jj(a,a) = Im{zeta''/(2 zeta')} with the -+1/2 of Eq. (3.10) and the
 // -1/M_m of E_m.
 #include "bie_common.cuh"
+#include <cstdlib>
+#include <vector>
 #include "bie_free.cuh"
 
 struct PrepArgs {
@@ -165,7 +167,7 @@ size_t bie_free_buf_doubles(int cap)
     return 8 * (size_t)cap + ((size_t)cap / FREE_ROWS + 2 + 256) * FREE_ROWS;
 }
 
-int bie_free_plan(const bie_ctx* ctx, int grid, int s_off, FreePlan* fp)
+int bie_free_plan(const bie_ctx* ctx, int grid, int s_off, FreePlan* fp, cudaStream_t st)
 {
     if (!ctx->have_geom || grid < 1 || grid > 256) return BIE_ERR_GEOMETRY;
     if (ctx->variant == BIE_VARIANT_NORMAL_INTERNAL) return BIE_ERR_GEOMETRY;   // node tables of another operator
@@ -178,6 +180,40 @@ int bie_free_plan(const bie_ctx* ctx, int grid, int s_off, FreePlan* fp)
     fp->s_off = s_off;
     fp->UB = (npad - s_off) / 2;
     fp->U = (long long)fp->NB * fp->UB;
+    // symmetric work split (bie_free_sym.cuh): whole operator only, Eq. (3.16) variants, and while the reverse partials
+    // [NB][npad] stay small
+    fp->sym = 0; fp->PC = nullptr; fp->sym_cum = nullptr; fp->sym_perm = nullptr; fp->sym_pos = nullptr;
+    if (ctx->use_sym && s_off == 0 && !fp->vortex && npad <= 65536) {
+        const size_t need = (size_t)fp->NB * (size_t)npad;
+        bie_ctx* c = const_cast<bie_ctx*>(ctx);
+        if (need > c->pc_cap) {
+            if (c->pc_buf) cudaFree(c->pc_buf);
+            c->pc_buf = nullptr; c->pc_cap = 0;
+            if (cudaMalloc((void**)&c->pc_buf, sizeof(double) * need + 16 * (size_t)(fp->NB + 2)) != cudaSuccess) return BIE_ERR_CUDA_BASE - (int)cudaErrorMemoryAllocation;
+            c->pc_cap = need;
+        }
+        // work list: blocks in the order 0, NB-1, 1, NB-2, ... ; tables behind the partials
+        const int NB = fp->NB;
+        std::vector<long long> cum(NB + 1);
+        std::vector<int> perm(NB), pos(NB);
+        for (int k = 0; k < NB; ++k) perm[k] = (k & 1) ? NB - 1 - (k >> 1) : (k >> 1);
+        cum[0] = 0;
+        for (int k = 0; k < NB; ++k) {
+            const int b = perm[k];
+            pos[b] = k;
+            const int row0 = b < fp->NB0 ? b * FREE_ROWS : fp->M0 + (b - fp->NB0) * FREE_ROWS;
+            cum[k + 1] = cum[k] + (npad - row0);
+        }
+        const long long U = cum[NB];
+        char* tab = reinterpret_cast<char*>(c->pc_buf + need);
+        cudaMemcpyAsync(tab, cum.data(), sizeof(long long) * (NB + 1), cudaMemcpyHostToDevice, st);
+        cudaMemcpyAsync(tab + sizeof(long long) * (NB + 1), perm.data(), sizeof(int) * NB, cudaMemcpyHostToDevice, st);
+        cudaMemcpyAsync(tab + sizeof(long long) * (NB + 1) + sizeof(int) * NB, pos.data(), sizeof(int) * NB, cudaMemcpyHostToDevice, st);
+        fp->sym_cum = reinterpret_cast<const long long*>(tab);
+        fp->sym_perm = reinterpret_cast<const int*>(tab + sizeof(long long) * (NB + 1));
+        fp->sym_pos = fp->sym_perm + NB;
+        fp->sym = 1; fp->PC = c->pc_buf; fp->U = U;
+    }
     fp->Geff = (long long)grid < fp->U ? grid : (int)fp->U;
     if (fp->Geff < 1) fp->Geff = 1;
     fp->T = reinterpret_cast<double2*>(ctx->free_buf);

@@ -566,6 +566,35 @@ def test_cauchy_eval_parity(ctx, c, npts, nf):
         assert float(np.max(np.abs(out[0].cpu().numpy() - exact))) <= 1e-9 * scale
 
 
+@pytest.mark.parametrize("shape", [None, (37, 29, [19, 23]), (300, 171, [33, 2, 129]), (5, 3, [])])
+def test_matrix_free_one_directional_and_symmetric_agree(ctx, shape):
+    """bie_set_symmetric: the symmetric (oddness) work split and the one-directional pair loops are the same operator"""
+    g = cfg(3).geometry if shape is None else inputs.small_problem(*shape).geometry
+    n = g.n
+    Ao = oracle_build(g)
+    x = _x(n, 41)
+    yo = oracle.matvec(Ao, x)
+    z, dz, d2z = geo_dev(g)
+    ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z)
+    ys = []
+    try:
+        for on in (True, False):
+            ctx.bie_set_symmetric(on)
+            y = torch.empty(n + (n & 1), dtype=torch.float64, device="cuda")[:n]
+            ctx.bie_matvec_free(dev(x), y)
+            ys.append(y.cpu().numpy())
+            assert rel_max(ys[-1], yo) <= 1e-12, on
+        b = inputs.rhs_analytic(g, lambda zz: np.exp(1j * zz))
+        ctx.bie_set_symmetric(False)
+        x0, it0, rr0, st0 = gpu_gmres(ctx, None, b, 1e-13, 50, 1000)
+        ctx.bie_set_symmetric(True)
+        x1, it1, rr1, st1 = gpu_gmres(ctx, None, b, 1e-13, 50, 1000)
+        assert st0 == 0 and st1 == 0 and abs(it0 - it1) <= 1
+        assert np.linalg.norm(x0 - x1) <= 1e-10 * np.linalg.norm(x0)
+    finally:
+        ctx.bie_set_symmetric(True)
+
+
 def test_matrix_free_at_the_papers_largest_size(ctx):
     """n = 20224 (the paper's largest problem): more row blocks than SMs, so a CTA's slab of the matrix-free
     operator spans several row blocks; sampled rows against the oracle, and dense vs matrix-free on the GPU"""
