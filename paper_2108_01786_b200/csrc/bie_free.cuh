@@ -61,7 +61,7 @@ struct FreePlan {
 // doubles of shared scratch: warp staging buffers [16][2 stages][3][32] double2, warp sums [16][128], component sums
 __host__ __device__ inline int free_scratch_doubles(int /*nthr*/)
 {
-    return FREE_STAGE_DOUBLES + FREE_WARPS * FREE_ROWS + BIE_MAX_COMP + 2;
+    return FREE_STAGE_DOUBLES + FREE_WARPS * FREE_ROWS + BIE_MAX_COMP + 2 + FREE_WARPS * 8 * 33;   // + bie_free_sym.cuh columns
 }
 
 __device__ __forceinline__ long long free_slab_start(const FreePlan& fp, int c)

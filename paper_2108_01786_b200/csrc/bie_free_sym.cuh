@@ -9,7 +9,8 @@
 // bie_free.cuh, reverse A[s][t] x_t summed over the 128 targets of the block into a per-(row block, source) partial
 // PC[I][s] in L2.  The triangular list is cut into equal slabs of sources, one per CTA.  The owner of row t (block J)
 // gathers the forward partials of J and  sum_{I < J} PC[I][t]  in fixed order: deterministic.
-// Reverse sums of 8 consecutive sources are reduced over the lanes together by a transposing butterfly (9 shuffles).
+// Reverse sums of 8 consecutive sources are reduced over the lanes through lane-private shared-memory slots (a transposing
+// shuffle butterfly, sym_butterfly below, is kept for reference: its 9 dependent steps made the loop 3 % slower).
 // Near pairs: forward skipped when den < taubar M_t, reverse when den < taubar M_s -- the row-based rule of bie_near.cu,
 // whose CSR matrix supplies both.
 #pragma once
@@ -51,6 +52,8 @@ __device__ __forceinline__ double sym_butterfly(double (&rev)[SYM_BATCH], int la
 }
 
 #define SYM_STAGE_DOUBLES (FREE_WARPS * 2 * 4 * 32 * 2)   // [16 warps][2 buffers][4 arrays][32] double2
+#define SYM_COL_STRIDE 33                                  // [SYM_BATCH][33] doubles per warp: lane-private slots, no bank conflicts
+#define SYM_COL_DOUBLES (FREE_WARPS * SYM_BATCH * SYM_COL_STRIDE)
 
 // this CTA's slab of the triangular (row block x later sources) list -> forward partials in fp.PB, reverse partials in fp.PC.
 // scratch: shared, >= SYM_STAGE_DOUBLES + FREE_WARPS * FREE_ROWS doubles.  All threads of the CTA must call.
@@ -61,6 +64,7 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
     if (c >= fp.Geff) return;
     double2* stage = reinterpret_cast<double2*>(scratch) + warp * (2 * 4 * 32);
     double* wsum = scratch + SYM_STAGE_DOUBLES;
+    double* col = wsum + FREE_WARPS * FREE_ROWS + warp * (SYM_BATCH * SYM_COL_STRIDE);   // this warp's reverse sums of a batch
     const int np = nt.npad;
     const double taubar = __ldg(fp.taubar);
     long long u0 = (long long)c * fp.U / fp.Geff;
@@ -149,13 +153,12 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
                     }
                 } else {
                     for (int j0 = 0; j0 < cnt; j0 += SYM_BATCH) {   // sources beyond cnt are zero sources; not written
-                        double rv[SYM_BATCH];
 #pragma unroll
                         for (int u = 0; u < SYM_BATCH; ++u) {
                             const int j = j0 + u;
                             const double2 e = sg[j], pq = sg[32 + j], rb = sg[64 + j], mt = sg[96 + j];
                             const int thj = __double2hiint(mt.y);
-                            double s_rev = 0.0;
+                            double s_rev0 = 0.0, s_rev1 = 0.0;
 #pragma unroll
                             for (int i = 0; i < FREE_NT; ++i) {
                                 const double dr = e.x - ter[i], di = e.y - tei[i];
@@ -170,13 +173,22 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
                                 double vr = fma(e.y, tp[i], tr[i]);
                                 vr = fma(-e.x, tq[i], vr);
                                 vr = fma(-mt.x, tb[i], vr);
-                                if (!(dh < thj)) s_rev = fma(vr, r, s_rev);
+                                if (!(dh < thj)) { if (i & 1) s_rev1 = fma(vr, r, s_rev1); else s_rev0 = fma(vr, r, s_rev0); }
                             }
-                            rv[u] = s_rev;
+                            col[u * SYM_COL_STRIDE + lane] = s_rev0 + s_rev1;
                         }
-                        const double tot = sym_butterfly(rv, lane);
-                        const int j = j0 + (lane >> 2);
-                        if ((lane & 3) == 0 && j < cnt) fp.PC[(size_t)b * np + base + j] = tot;
+                        // lane reduction of the 8 reverse sums through shared memory: lane l adds the slots 8 (l & 3) .. + 7 of
+                        // source l >> 2, two shuffles finish (fixed order)
+                        __syncwarp();
+                        {
+                            const double* cp = col + (lane >> 2) * SYM_COL_STRIDE + 8 * (lane & 3);
+                            double v = ((cp[0] + cp[1]) + (cp[2] + cp[3])) + ((cp[4] + cp[5]) + (cp[6] + cp[7]));
+                            v += __shfl_xor_sync(0xffffffffu, v, 2);
+                            v += __shfl_xor_sync(0xffffffffu, v, 1);
+                            const int j = j0 + (lane >> 2);
+                            if ((lane & 3) == 0 && j < cnt) fp.PC[(size_t)b * np + base + j] = v;
+                        }
+                        __syncwarp();
                     }
                 }
             }
