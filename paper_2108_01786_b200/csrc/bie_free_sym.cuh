@@ -10,7 +10,7 @@
 // PC[I][s] in L2.  The triangular list is cut into equal slabs of sources, one per CTA.  The owner of row t (block J)
 // gathers the forward partials of J and  sum_{I < J} PC[I][t]  in fixed order: deterministic.
 // Reverse sums of 8 consecutive sources are reduced over the lanes through lane-private shared-memory slots (a transposing
-// shuffle butterfly, sym_butterfly below, is kept for reference: its 9 dependent steps made the loop 3 % slower).
+// shuffle butterfly was 3 % slower: its 9 dependent steps stall the warp).
 // Near pairs: forward skipped when den < taubar M_t, reverse when den < taubar M_s -- the row-based rule of bie_near.cu,
 // whose CSR matrix supplies both.
 #pragma once
@@ -29,26 +29,6 @@ __device__ __forceinline__ int sym_find_pos(const FreePlan& fp, long long u)
         if (__ldg(fp.sym_cum + mid) <= u) lo = mid; else hi = mid - 1;
     }
     return lo;
-}
-
-// the lanes hold rev[0..7] = their partial reverse sums for 8 sources; afterwards every lane holds in its return value
-// the warp total of source (lane >> 2)
-__device__ __forceinline__ double sym_butterfly(double (&rev)[SYM_BATCH], int lane)
-{
-#pragma unroll
-    for (int h = 4, m = 16; h >= 1; h >>= 1, m >>= 1) {
-        const bool up = (lane & m) != 0;
-#pragma unroll
-        for (int q = 0; q < h; ++q) {
-            const double send = up ? rev[q] : rev[q + h];
-            const double keep = up ? rev[q + h] : rev[q];
-            rev[q] = keep + __shfl_xor_sync(0xffffffffu, send, m);
-        }
-    }
-    double v = rev[0];
-    v += __shfl_xor_sync(0xffffffffu, v, 2);
-    v += __shfl_xor_sync(0xffffffffu, v, 1);
-    return v;
 }
 
 #define SYM_STAGE_DOUBLES (FREE_WARPS * 2 * 4 * 32 * 2)   // [16 warps][2 buffers][4 arrays][32] double2
