@@ -146,7 +146,9 @@ int bie_matvec_free(bie_ctx* ctx, int n, const double* x, double* y, void* strea
 /* The whole-matrix matrix-free operator (bie_matvec_free, bie_gmres with A == NULL; variants A and B, n <= 65536) uses the
  * oddness of the kernel, cot((zeta_s - zeta_t)/2) = -cot((zeta_t - zeta_s)/2): one evaluation of the pair serves the entries
  * (t,s) and (s,t) (15 FP64 instructions for two entries instead of 22).  on = 0 switches back to the one-directional pair
- * loops (default: on).  Same results to rounding; both are deterministic. */
+ * loops, on = 1 is the default, on = 2 also uses the symmetric loops inside the hybrid operator when the slab width is a
+ * row-block boundary (a multiple of 128 up to M_0, or M_0 + a multiple of 128) -- measured slower there on a B200, kept
+ * for measurement.  Same results to rounding; all are deterministic. */
 int bie_set_symmetric(bie_ctx* ctx, int on);
 
 /* stream function prescribed on the solids, circulation parameters

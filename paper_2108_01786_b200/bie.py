@@ -259,8 +259,10 @@ class Context:
                                      _stream()), "bie_cauchy_eval")
         return out
 
-    def bie_set_symmetric(self, on: bool):
-        _check(lib().bie_set_symmetric(self._h, int(bool(on))), "bie_set_symmetric")
+    def bie_set_symmetric(self, on):
+        """0: one-directional pair loops; 1 (default): symmetric loops in the whole-matrix matrix-free operator; 2: also in
+        the hybrid operator"""
+        _check(lib().bie_set_symmetric(self._h, int(on)), "bie_set_symmetric")
 
     def bie_matvec_free(self, x, y):
         n = x.numel()

@@ -137,9 +137,9 @@ int bie_hybrid_cols(bie_ctx* c, int n)
 {
     if (!c || n < 4) return 0;
     // the slab's share of the columns that makes the streaming warps and the pair-loop warps finish together on a
-    // B200 (measured); a multiple of 64 so that slab rows are whole 512-byte lines
-    int nd = (int)((double)n * BIE_HYBRID_DENSE_FRACTION) & ~63;
-    if (nd < 64) nd = 0;            // too small to be worth two teams: use bie_gmres
+    // B200 (measured); a multiple of 128 = a row-block boundary of the pair loops
+    int nd = (int)((double)n * BIE_HYBRID_DENSE_FRACTION) & ~127;   // a row-block boundary of the pair loops (128 rows)
+    if (nd < 128) nd = 0;           // too small to be worth two teams: use bie_gmres
     if (nd > n - 2) nd = (n - 2) & ~1;
     return nd;
 }
@@ -147,7 +147,8 @@ int bie_hybrid_cols(bie_ctx* c, int n)
 int bie_set_symmetric(bie_ctx* c, int on)
 {
     if (!c) return BIE_ERR_NULL;
-    c->use_sym = on ? 1 : 0;
+    if (on < 0 || on > 2) return BIE_ERR_ARG;
+    c->use_sym = on;
     return BIE_OK;
 }
 
@@ -248,8 +249,8 @@ static int solve_cols(int n, int op)
 {
     if (op == BIE_OP_FREE) return 0;
     if (op == BIE_OP_HYBRID) {
-        int nd = (int)((double)n * BIE_HYBRID_DENSE_FRACTION) & ~63;
-        if (nd < 64) return 0;
+        int nd = (int)((double)n * BIE_HYBRID_DENSE_FRACTION) & ~127;
+        if (nd < 128) return 0;
         if (nd > n - 2) nd = (n - 2) & ~1;
         return nd;
     }

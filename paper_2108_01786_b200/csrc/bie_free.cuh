@@ -47,6 +47,7 @@ struct FreePlan {
     const long long* sym_cum;   // sym: [NB + 1] sources before position k of the (permuted) triangular list
     const int* sym_perm;        // sym: [NB] row block at position k
     const int* sym_pos;         // sym: [NB] position of row block b
+    int sym_first;              // sym: first row block of the triangle (0; hybrid: the block that starts at s_off)
     int vortex;      // 1: the vortex-sheet matrix S (BIE_VARIANT_VORTEX) instead of Eq. (3.16); see free_parts
     int s_off;       // first source of the operator (0; the hybrid operator reads the sources below it from its slab)
     double2* T;      // [4][npad]: (P,Q) class 0, (R,B) class 0, (P,Q) class 1, (R,B) class 1
@@ -222,12 +223,12 @@ __device__ __forceinline__ void free_parts_impl(const NodeTable& nt, const CompT
     }
 }
 
-__device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePlan& fp, double* scratch);
+__device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePlan& fp, double* scratch, const Team& team);
 
 __device__ __forceinline__ void free_parts(const NodeTable& nt, const CompTable& ct, const FreePlan& fp, double* scratch,
                                            const Team& team)
 {
-    if (fp.sym) free_parts_sym(nt, fp, scratch);           // whole CTA (the plan sets sym only for s_off == 0, variants A/B)
+    if (fp.sym) free_parts_sym(nt, fp, scratch, team);     // variants A/B; s_off = 0 or a row-block boundary
     else if (fp.vortex) free_parts_impl<true>(nt, ct, fp, scratch, team);
     else free_parts_impl<false>(nt, ct, fp, scratch, team);
 }
@@ -273,7 +274,7 @@ __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable
             const int b = t < fp.M0 ? t / FREE_ROWS : fp.NB0 + (t - fp.M0) / FREE_ROWS;
             const double* pc = fp.PC + t;
             double a0 = 0.0, a1 = 0.0;
-            int I = q;
+            int I = fp.sym_first + q;
             for (; I + 28 < b; I += 32) {
                 double v[8];
 #pragma unroll

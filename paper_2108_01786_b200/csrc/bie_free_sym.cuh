@@ -36,10 +36,12 @@ __device__ __forceinline__ int sym_find_pos(const FreePlan& fp, long long u)
 #define SYM_COL_DOUBLES (FREE_WARPS * SYM_BATCH * SYM_COL_STRIDE)
 
 // this CTA's slab of the triangular (row block x later sources) list -> forward partials in fp.PB, reverse partials in fp.PC.
-// scratch: shared, >= SYM_STAGE_DOUBLES + FREE_WARPS * FREE_ROWS doubles.  All threads of the CTA must call.
-__device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePlan& fp, double* scratch)
+// scratch: shared, free_scratch_doubles() doubles.  All threads of the team must call.
+// Hybrid operator (fp.s_off > 0, a row-block boundary): row blocks below s_off take the sources [s_off, npad) one-directionally
+// (their mirror entries are in the stored slab); the row blocks from s_off on form the triangle.
+__device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePlan& fp, double* scratch, const Team& team)
 {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    const int lane = team.tid & 31, warp = team.warp, nwarp = team.nwarp;
     const int c = blockIdx.x;
     if (c >= fp.Geff) return;
     double2* stage = reinterpret_cast<double2*>(scratch) + warp * (2 * 4 * 32);
@@ -58,7 +60,9 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
         const int cls = b < fp.NB0 ? 0 : 1;
         const int row0 = free_block_row0(fp, b);
         const int rows = free_block_rows(fp, b, nt.n);
-        const int sa = row0 + (int)(u0 - ub), sb = row0 + (int)(ue - ub);   // sources [sa, sb), all >= row0
+        const bool below = (row0 + rows <= fp.s_off);        // hybrid: a row block of the slab's columns
+        const int src0 = below ? fp.s_off : row0;
+        const int sa = src0 + (int)(u0 - ub), sb = src0 + (int)(ue - ub);   // sources [sa, sb), all >= src0
         double ter[FREE_NT], tei[FREE_NT], tm[FREE_NT], acc[FREE_NT];
         int thi[FREE_NT];
         bool live[FREE_NT];
@@ -73,13 +77,13 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
         const int span = sb - sa;
         const int wa_all = sa + (int)((long long)span * warp / nwarp);
         const int wb_all = sa + (int)((long long)span * (warp + 1) / nwarp);
-        const int d_end = row0 + rows;                       // end of the block's own rows
-        const int c_end = (cls == 0) ? fp.M0 : np;           // end of the sources of the block's own class
+        const int d_end = below ? np : row0 + rows;           // end of the one-directional sources (the block's own rows)
+        const int c_end = below ? np : ((cls == 0) ? fp.M0 : np);   // end of the sources of the block's own class
         const double2* TPQ = fp.T + (size_t)(2 * cls) * np;      // forward tables: the class of the block's rows
         const double2* TRB = fp.T + (size_t)(2 * cls + 1) * np;
         for (int sgm = 0; sgm < 3; ++sgm) {
             // 0: own rows (one direction); 1: later sources of the same class; 2: sources on solids below a Gamma_0 block
-            const int lo = sgm == 0 ? row0 : (sgm == 1 ? d_end : c_end);
+            const int lo = sgm == 0 ? src0 : (sgm == 1 ? d_end : c_end);
             const int hi = sgm == 0 ? d_end : (sgm == 1 ? c_end : np);
             const int wa = max(wa_all, lo), wb = min(wb_all, hi);
             if (wa >= wb) continue;                          // warp-uniform
@@ -176,13 +180,13 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
         // the warp sums of the forward direction, added in fixed order
 #pragma unroll
         for (int i = 0; i < FREE_NT; ++i) wsum[warp * FREE_ROWS + lane + 32 * i] = acc[i];
-        __syncthreads();
-        for (int r = threadIdx.x; r < FREE_ROWS; r += blockDim.x) {
+        team_sync(team);
+        for (int r = team.tid; r < FREE_ROWS; r += team.nthr) {
             double s = 0.0;
             for (int w = 0; w < nwarp; ++w) s += wsum[w * FREE_ROWS + r];
             fp.PB[(size_t)(k + c) * FREE_ROWS + r] = s;
         }
-        __syncthreads();
+        team_sync(team);
         u0 = ue;
         ++k;
     }

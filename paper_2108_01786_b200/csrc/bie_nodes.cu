@@ -183,7 +183,12 @@ int bie_free_plan(const bie_ctx* ctx, int grid, int s_off, FreePlan* fp, cudaStr
     // symmetric work split (bie_free_sym.cuh): whole operator only, Eq. (3.16) variants, and while the reverse partials
     // [NB][npad] stay small
     fp->sym = 0; fp->PC = nullptr; fp->sym_cum = nullptr; fp->sym_perm = nullptr; fp->sym_pos = nullptr;
-    if (ctx->use_sym && s_off == 0 && !fp->vortex && npad <= 65536) {
+    // hybrid operator: s_off must be a row-block boundary (row blocks are cut per class: 128 b, then M_0 + 128 b)
+    const bool boundary = s_off == 0 || (s_off <= fp->M0 ? (s_off % FREE_ROWS == 0 || s_off == fp->M0)
+                                                          : ((s_off - fp->M0) % FREE_ROWS == 0));
+    fp->sym_first = 0;
+    // (in the hybrid operator only on request, use_sym == 2: with 8 pair-loop warps it is slower, 289 against 200 us per step)
+    if (ctx->use_sym && (s_off == 0 || ctx->use_sym == 2) && boundary && !fp->vortex && npad <= 65536) {
         const size_t need = (size_t)fp->NB * (size_t)npad;
         bie_ctx* c = const_cast<bie_ctx*>(ctx);
         if (need > c->pc_cap) {
@@ -196,13 +201,20 @@ int bie_free_plan(const bie_ctx* ctx, int grid, int s_off, FreePlan* fp, cudaStr
         const int NB = fp->NB;
         std::vector<long long> cum(NB + 1);
         std::vector<int> perm(NB), pos(NB);
+        // blocks in the order of decreasing length of their source lists (blocks below s_off: npad - s_off each, then the
+        // triangle), taken alternately from both ends: 0, NB-1, 1, NB-2, ...
+        auto row0_of = [&](int b) { return b < fp->NB0 ? b * FREE_ROWS : fp->M0 + (b - fp->NB0) * FREE_ROWS; };
+        auto rows_of = [&](int b) { const int r0 = row0_of(b), end = b < fp->NB0 ? fp->M0 : n; return end - r0 < FREE_ROWS ? end - r0 : FREE_ROWS; };
+        int first = 0;
+        while (first < NB && row0_of(first) + rows_of(first) <= s_off) ++first;
+        fp->sym_first = first;
         for (int k = 0; k < NB; ++k) perm[k] = (k & 1) ? NB - 1 - (k >> 1) : (k >> 1);
         cum[0] = 0;
         for (int k = 0; k < NB; ++k) {
             const int b = perm[k];
             pos[b] = k;
-            const int row0 = b < fp->NB0 ? b * FREE_ROWS : fp->M0 + (b - fp->NB0) * FREE_ROWS;
-            cum[k + 1] = cum[k] + (npad - row0);
+            const int src0 = b < first ? s_off : row0_of(b);
+            cum[k + 1] = cum[k] + (npad - src0);
         }
         const long long U = cum[NB];
         char* tab = reinterpret_cast<char*>(c->pc_buf + need);

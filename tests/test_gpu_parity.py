@@ -578,21 +578,21 @@ def test_matrix_free_one_directional_and_symmetric_agree(ctx, shape):
     ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z)
     ys = []
     try:
-        for on in (True, False):
+        for on in (1, 0):
             ctx.bie_set_symmetric(on)
             y = torch.empty(n + (n & 1), dtype=torch.float64, device="cuda")[:n]
             ctx.bie_matvec_free(dev(x), y)
             ys.append(y.cpu().numpy())
             assert rel_max(ys[-1], yo) <= 1e-12, on
         b = inputs.rhs_analytic(g, lambda zz: np.exp(1j * zz))
-        ctx.bie_set_symmetric(False)
+        ctx.bie_set_symmetric(0)
         x0, it0, rr0, st0 = gpu_gmres(ctx, None, b, 1e-13, 50, 1000)
-        ctx.bie_set_symmetric(True)
+        ctx.bie_set_symmetric(1)
         x1, it1, rr1, st1 = gpu_gmres(ctx, None, b, 1e-13, 50, 1000)
         assert st0 == 0 and st1 == 0 and abs(it0 - it1) <= 1
         assert np.linalg.norm(x0 - x1) <= 1e-10 * np.linalg.norm(x0)
     finally:
-        ctx.bie_set_symmetric(True)
+        ctx.bie_set_symmetric(1)
 
 
 def test_matrix_free_at_the_papers_largest_size(ctx):
@@ -783,7 +783,7 @@ def test_build_cols_writes_only_the_slab(ctx):
     assert np.all(Ah[:, nd:] == -7.0)
 
 
-@pytest.mark.parametrize("c,nd", [(1, 128), (2, 0), (2, 2), (2, 1030), (2, 2046), (3, 0), (5, 0)])
+@pytest.mark.parametrize("c,nd", [(1, 128), (2, 0), (2, 2), (2, 1030), (2, 1024), (2, 1280), (2, 2046), (3, 0), (3, 2048), (3, 2560), (5, 0)])
 def test_gmres_hybrid_parity(ctx, c, nd):
     """hybrid operator (stored slab of nd columns + recomputed sources): same solution, same iteration band;
     nd = 0 takes the library's own split (bie_hybrid_cols)"""
@@ -801,6 +801,25 @@ def test_gmres_hybrid_parity(ctx, c, nd):
     r = b - oracle.matvec(Ao, x)
     assert np.linalg.norm(r) / np.linalg.norm(b) <= 10 * P.tol
     del A
+
+
+@pytest.mark.parametrize("c,nd", [(2, 1024), (2, 1280), (3, 2048), (3, 2560), (1, 256)])
+def test_gmres_hybrid_with_symmetric_pair_loops(ctx, c, nd):
+    """bie_set_symmetric(2): the triangle of the hybrid operator's recomputed part (rows and sources >= nd) through the
+    symmetric loops; nd on a row-block boundary of Gamma_0 (1024, 2048, 256) and of the solids (M_0 + 256, M_0 + 512)"""
+    P = cfg(c)
+    g, b = P.geometry, P.rhs[0]
+    Ao = oracle_build(g)
+    xo, ito, _, _, _ = oracle.gmres(Ao, b, P.tol, P.restart, P.max_iters)
+    try:
+        ctx.bie_set_symmetric(2)
+        x, it, rr, st, A = gpu_gmres_hybrid(ctx, g, nd, b, P.tol, P.restart, P.max_iters)
+    finally:
+        ctx.bie_set_symmetric(1)
+    lo, hi = iteration_band(Ao, b, P.tol, P.restart, P.max_iters)
+    assert st == 0 and lo - 1 <= it <= hi + 1, (it, ito, lo, hi)
+    assert np.linalg.norm(x - xo) / np.linalg.norm(xo) <= TOL_X
+    assert rr <= 10 * P.tol
 
 
 def test_gmres_hybrid_free_warps_knob(ctx):
@@ -939,7 +958,7 @@ def test_error_codes_of_the_operator_and_next_calls(ctx):
     with pytest.raises(bie.BieError) as e:
         ctx.bie_set_hybrid_free_warps(16)
     assert e.value.code == -6
-    assert ctx.bie_hybrid_cols(2) == 0 and ctx.bie_hybrid_cols(100) == 0 and ctx.bie_hybrid_cols(16384) == 6848
+    assert ctx.bie_hybrid_cols(2) == 0 and ctx.bie_hybrid_cols(100) == 0 and ctx.bie_hybrid_cols(16384) == 6784
     # Appendix B without centres for a geometry that has an obstacle; Cauchy evaluation with too many functions
     rc = bie.lib().bie_add_cyl_columns(ctx._h, 3, bie._ip(bie._i32(g.counts)), bie._ip(bie._i32(g.kinds)), z.data_ptr(), None,
                                        A.data_ptr(), n, None)
