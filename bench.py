@@ -42,7 +42,7 @@ FP64_INSTR_PER_ENTRY_SYM = 7.7  # symmetric pair loops (whole-matrix matrix-free
 HBM_FALLBACK_GBS = 6650.0      # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 # dram__bytes_read.sum + dram__bytes_write.sum of the GMRES kernel, one launch, from the committed ncu capture
 # (profiles/r01_ncu_full_gmres_cfg5.md); None for workloads that were not captured
-TRAFFIC_BYTES = {(5, "dense"): 341.50e9, (5, "hybrid"): 142.79e9}   # profiles/r01b_, r01c_ncu_full_cfg5.md
+TRAFFIC_BYTES = {(5, "dense"): 341.50e9, (5, "hybrid"): 142.37e9}   # profiles/r01b_ncu_full_cfg5.md, r01e_launches_cfg5.md
 
 
 def parse_args():
