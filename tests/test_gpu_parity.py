@@ -595,6 +595,20 @@ def test_matrix_free_one_directional_and_symmetric_agree(ctx, shape):
         ctx.bie_set_symmetric(1)
 
 
+@pytest.mark.parametrize("shape", [(5, 3, []), (2, 1, [1]), (37, 29, [19, 23]), (130, 127, [129])])
+def test_gmres_matrix_free_tiny_and_ragged(ctx, shape):
+    """matrix-free GMRES when there are fewer rows than SMs, odd sizes, blocks of one row"""
+    P = inputs.small_problem(*shape)
+    g, b = P.geometry, P.rhs[0]
+    Ao = oracle_build(g)
+    xo, ito, _, _, sto = oracle.gmres(Ao, b, 1e-13, 50, 500)
+    z, dz, d2z = geo_dev(g)
+    ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z)
+    x, it, rr, st = gpu_gmres(ctx, None, b, 1e-13, 50, 500)
+    assert sto == 0 and st == 0 and abs(it - ito) <= 1, (it, ito)
+    assert np.linalg.norm(x - xo) <= 1e-10 * max(np.linalg.norm(xo), 1e-300) * max(1.0, np.linalg.cond(Ao) / 100)
+
+
 def test_matrix_free_at_the_papers_largest_size(ctx):
     """n = 20224 (the paper's largest problem): more row blocks than SMs, so a CTA's slab of the matrix-free
     operator spans several row blocks; sampled rows against the oracle, and dense vs matrix-free on the GPU"""
