@@ -90,6 +90,17 @@ static inline int bie_cuda_err(cudaError_t e) { return e == cudaSuccess ? BIE_OK
         if (e__ != cudaSuccess) return bie_cuda_err(e__); \
     } while (0)
 
+// row pairs per CTA block that a streaming GEMV keeps L2-resident (bie_gemv.cuh): about 60 % of the L2 (measured flat from
+// 30 % to 60 %, worse above), less the bytes the caller keeps there anyway (Krylov basis), spread over the CTAs' row blocks
+static inline int bie_gemv_resident_pairs(int l2_bytes, int nrows, long long lda, int rows_per_cta, size_t other_bytes)
+{
+    const double budget = 0.6 * (double)l2_bytes - (double)other_bytes;
+    if (budget <= 0.0 || nrows < 1) return 0;
+    const double frac = budget / ((double)nrows * (double)lda * 8.0);
+    if (frac >= 1.0) return (rows_per_cta + 1) / 2;
+    return (int)(frac * rows_per_cta) / 2;
+}
+
 static inline int bie_npad(int n) { return (n + BIE_NODE_PAD - 1) / BIE_NODE_PAD * BIE_NODE_PAD; }
 NodeTable bie_node_table(const bie_ctx* ctx);
 struct FreePlan;

@@ -49,6 +49,7 @@ struct GmresArgs {
     int VS;        // Krylov vectors 0..VS-1 keep this CTA's rows in shared memory; the others in V (global, L2)
     int nd;        // hybrid operator: columns [0, nd) come from the stored slab A, sources [nd, n) are recomputed
     int nwf;       // hybrid operator: warps 0..nwf-1 run the pair loops, the others stream the slab
+    int res_pairs; // streaming GEMV: leading row pairs of every CTA block kept L2-resident (bie_gemv.cuh)
     NodeTable nt;
     CompTable ct;
     FreePlan fp;
@@ -153,9 +154,9 @@ __device__ __forceinline__ void cta_apply(const GmresArgs& a, int r0, int r1, co
         }
         if ((a.n & 1) && threadIdx.x == 0) xs[a.n - 1] = __ldcg(xin + a.n - 1) * scale;
         __syncthreads();
-        bie_cta_gemv<STREAM, true>(a.A, a.lda, a.n, r0, r1, a.chunk, xs, gpart, y_local, cta_team());
+        bie_cta_gemv<STREAM, true>(a.A, a.lda, a.n, r0, r1, a.chunk, xs, gpart, y_local, cta_team(), a.res_pairs);
     } else {
-        bie_cta_gemv<STREAM, false>(a.A, a.lda, a.n, r0, r1, a.chunk, xin, gpart, y_local, cta_team());
+        bie_cta_gemv<STREAM, false>(a.A, a.lda, a.n, r0, r1, a.chunk, xin, gpart, y_local, cta_team(), a.res_pairs);
         if (scale != 1.0) {
             for (int r = threadIdx.x; r < r1 - r0; r += blockDim.x) y_local[r] *= scale;
             __syncthreads();
@@ -572,6 +573,8 @@ int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, int nd, 
     a.sync = ctx->sync_buf;
     a.nld = pl.nld; a.rows_per_cta = pl.rows_per_cta; a.chunk = pl.chunk; a.VS = pl.VS;
     a.nd = nd; a.nwf = nwf;
+    a.res_pairs = (mode == 0 && pl.stream)
+        ? bie_gemv_resident_pairs(ctx->l2_bytes, n, (long long)lda, pl.rows_per_cta, sizeof(double) * (size_t)(restart + 2) * pl.nld) : 0;
     memset(&a.nt, 0, sizeof(a.nt)); memset(&a.ct, 0, sizeof(a.ct)); memset(&a.fp, 0, sizeof(a.fp));
     if (free_op) {
         a.nt = bie_node_table(ctx); a.ct = ctx->comps;

@@ -9,7 +9,7 @@
 
 template <bool STREAM, bool XS>
 __global__ void __launch_bounds__(MV_THREADS, 1)
-bie_matvec_kernel(const double* __restrict__ A, long long lda, int nrows, int n, int rows_per_cta, int chunk,
+bie_matvec_kernel(const double* __restrict__ A, long long lda, int nrows, int n, int rows_per_cta, int chunk, int res_pairs,
                   const double* __restrict__ x, double* __restrict__ y)
 {
     extern __shared__ __align__(16) double smem[];
@@ -26,18 +26,18 @@ bie_matvec_kernel(const double* __restrict__ A, long long lda, int nrows, int n,
         if ((n & 1) && threadIdx.x == 0) xs[n - 1] = x[n - 1];
         __syncthreads();
     }
-    bie_cta_gemv<STREAM, XS>(A, lda, n, r0, r1, chunk, XS ? xs : x, part, y_local, cta_team());
+    bie_cta_gemv<STREAM, XS>(A, lda, n, r0, r1, chunk, XS ? xs : x, part, y_local, cta_team(), res_pairs);
     for (int r = threadIdx.x; r < r1 - r0; r += blockDim.x) y[r0 + r] = y_local[r];
 }
 
 template <bool STREAM, bool XS>
 static int launch_mv(bie_ctx* ctx, int nrows, int n, const double* A, int64_t lda, const double* x, double* y,
-                     int rows_per_cta, int chunk, size_t smem, cudaStream_t st)
+                     int rows_per_cta, int chunk, int res_pairs, size_t smem, cudaStream_t st)
 {
     auto k = bie_matvec_kernel<STREAM, XS>;
     BIE_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int grid = (nrows + rows_per_cta - 1) / rows_per_cta;
-    k<<<grid, MV_THREADS, smem, st>>>(A, (long long)lda, nrows, n, rows_per_cta, chunk, x, y);
+    k<<<grid, MV_THREADS, smem, st>>>(A, (long long)lda, nrows, n, rows_per_cta, chunk, res_pairs, x, y);
     BIE_CUDA(cudaGetLastError());
     (void)ctx;
     return BIE_OK;
@@ -60,10 +60,11 @@ int bie_launch_matvec(bie_ctx* ctx, int nrows, int n, const double* A, int64_t l
     // matrices that cannot stay in L2 are streamed (evict-first) so that they do not displace x, y and
     // the Krylov basis; smaller ones are read with the default policy and stay L2-resident between calls
     const bool stream = (double)nrows * (double)lda * 8.0 > 0.6 * (double)ctx->l2_bytes;
-    if (stream) return xs ? launch_mv<true, true>(ctx, nrows, n, A, lda, x, y, rows_per_cta, chunk, smem, st)
-                          : launch_mv<true, false>(ctx, nrows, n, A, lda, x, y, rows_per_cta, chunk, smem, st);
-    return xs ? launch_mv<false, true>(ctx, nrows, n, A, lda, x, y, rows_per_cta, chunk, smem, st)
-              : launch_mv<false, false>(ctx, nrows, n, A, lda, x, y, rows_per_cta, chunk, smem, st);
+    const int res_pairs = stream ? bie_gemv_resident_pairs(ctx->l2_bytes, nrows, (long long)lda, rows_per_cta, 0) : 0;
+    if (stream) return xs ? launch_mv<true, true>(ctx, nrows, n, A, lda, x, y, rows_per_cta, chunk, res_pairs, smem, st)
+                          : launch_mv<true, false>(ctx, nrows, n, A, lda, x, y, rows_per_cta, chunk, res_pairs, smem, st);
+    return xs ? launch_mv<false, true>(ctx, nrows, n, A, lda, x, y, rows_per_cta, chunk, res_pairs, smem, st)
+              : launch_mv<false, false>(ctx, nrows, n, A, lda, x, y, rows_per_cta, chunk, res_pairs, smem, st);
 }
 
 // ---------------------------------------------------------------------------------------------------
