@@ -30,6 +30,10 @@
 #include "bie_common.cuh"
 
 #define FREE_THREADS 512
+#ifndef FREE_SRC_UNROLL_N
+#define FREE_SRC_UNROLL_N 2
+#endif
+constexpr int FREE_SRC_UNROLL = FREE_SRC_UNROLL_N;   // sources per unrolled step of the pair loop
 #define FREE_WARPS (FREE_THREADS / 32)
 #define FREE_NT 4
 #define FREE_ROWS (32 * FREE_NT)
@@ -185,7 +189,7 @@ __device__ __forceinline__ void free_parts_impl(const NodeTable& nt, const CompT
                 if (s < wb) { ne = TE[s]; npq = __ldcg(TPQ + s); nrb = __ldcg(TRB + s); }
             }
             const int cnt = min(32, wb - base);   // even
-#pragma unroll 2
+#pragma unroll FREE_SRC_UNROLL
             for (int j = 0; j < cnt; ++j) {
                 const double2 e = sg[j], pq = sg[32 + j], rb = sg[64 + j];
 #pragma unroll

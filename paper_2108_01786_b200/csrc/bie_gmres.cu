@@ -19,7 +19,9 @@
 #include "bie_gemv.cuh"
 #include "bie_free.cuh"
 
+#ifndef GM_THREADS
 #define GM_THREADS 512
+#endif
 #ifndef HYB_GEMV_UNROLL
 #define HYB_GEMV_UNROLL 8   // hybrid operator: 2 rows x 8 LDG.128 per lane in flight in each streaming warp
 #endif
