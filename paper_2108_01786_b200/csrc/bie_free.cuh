@@ -119,6 +119,12 @@ __device__ __forceinline__ void free_write_tables(const NodeTable& nt, const Com
 // X' = Ei_t P_s - Er_t Q_s, Y' = R_s - M_t B_s from the class-independent tables (P,Q) = mu_s E_s, (R,B) = mu_s (M_s, 1), and the
 // row's (A_t, B_t) = (2u_i, -u_r) / +-(2u_r, u_i), u_t = zeta'_t/2, which depend on whether the SOURCE lies on Gamma_0: the
 // warp's source range is cut at M_0.  13 FP64-pipe instructions per pair.
+__device__ __forceinline__ void free_cp_async16(void* dst_shared, const void* src_global, unsigned src_bytes)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_shared);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(d), "l"(src_global), "r"(src_bytes) : "memory");
+}
+
 template <bool VORTEX>
 __device__ __forceinline__ void free_parts_impl(const NodeTable& nt, const CompTable& ct, const FreePlan& fp, double* scratch,
                                                 const Team& team)
@@ -175,19 +181,26 @@ __device__ __forceinline__ void free_parts_impl(const NodeTable& nt, const CompT
         // VORTEX: sources on Gamma_0 first, then the solids (different row coefficients); else the whole range at once
         const int wa = VORTEX ? (sgm == 0 ? wa_all : max(wa_all, fp.M0)) : wa_all;
         const int wb = VORTEX ? (sgm == 0 ? min(wb_all, fp.M0) : wb_all) : wb_all;
-        double2 ne = zero2, npq = zero2, nrb = zero2;
-        if (wa + lane < wb) { const int s = wa + lane; ne = TE[s]; npq = __ldcg(TPQ + s); nrb = __ldcg(TRB + s); }
+        // warp-private double buffer filled by cp.async (L2 only: the tables change between applications), zero-filled past wb
+        auto issue = [&](int base_, int bufi) {
+            const int s = base_ + lane;
+            const bool ok = s < wb;
+            const int sc = ok ? s : wa;
+            const unsigned sz = ok ? 16u : 0u;
+            double2* sg = stage + bufi * 96;
+            free_cp_async16(sg + lane, TE + sc, sz);
+            free_cp_async16(sg + 32 + lane, TPQ + sc, sz);
+            free_cp_async16(sg + 64 + lane, TRB + sc, sz);
+            asm volatile("cp.async.commit_group;" ::: "memory");
+        };
         int buf = 0;
         __syncwarp();
+        if (wa < wb) issue(wa, 0);
         for (int base = wa; base < wb; base += 32, buf ^= 1) {
-            double2* sg = stage + buf * 96;
-            sg[lane] = ne; sg[32 + lane] = npq; sg[64 + lane] = nrb;   // the other buffer may still be read
-            __syncwarp();
-            {   // prefetch the next chunk
-                const int s = base + 32 + lane;
-                ne = zero2; npq = zero2; nrb = zero2;
-                if (s < wb) { ne = TE[s]; npq = __ldcg(TPQ + s); nrb = __ldcg(TRB + s); }
-            }
+            const double2* sg = stage + buf * 96;
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+            __syncwarp();                                   // chunk landed for all lanes; the other buffer is no longer read
+            if (base + 32 < wb) issue(base + 32, buf ^ 1);
             const int cnt = min(32, wb - base);   // even
 #pragma unroll FREE_SRC_UNROLL
             for (int j = 0; j < cnt; ++j) {
