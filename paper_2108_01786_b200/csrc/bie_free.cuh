@@ -63,10 +63,17 @@ struct FreePlan {
     const int* near_overflow; // != 0: the near matrix did not fit; the operator returns NaN
 };
 
-// doubles of shared scratch: warp staging buffers [16][2 stages][3][32] double2, warp sums [16][128], component sums
+// doubles of shared scratch, in this order: warp sums [16][128], component sums [BIE_MAX_COMP + 2], warp staging buffers
+// [16][2 stages][4][32] double2 (3 of the 4 arrays used by the one-directional loops), reverse-sum slots of bie_free_sym.cuh
+#define FREE_HEAD_DOUBLES (FREE_WARPS * FREE_ROWS + ((BIE_MAX_COMP + 2 + 1) & ~1))
 __host__ __device__ inline int free_scratch_doubles(int /*nthr*/)
 {
-    return FREE_STAGE_DOUBLES + FREE_WARPS * FREE_ROWS + BIE_MAX_COMP + 2 + FREE_WARPS * 8 * 33;   // + bie_free_sym.cuh columns
+    return FREE_HEAD_DOUBLES + FREE_STAGE_DOUBLES + FREE_WARPS * 8 * 33;
+}
+// what the one-directional loops (no bie_free_sym.cuh) need: the staging buffers hold 3 arrays
+__host__ __device__ inline int free_scratch_doubles_onedir()
+{
+    return FREE_HEAD_DOUBLES + FREE_WARPS * 2 * 3 * 32 * 2;
 }
 
 __device__ __forceinline__ long long free_slab_start(const FreePlan& fp, int c)
@@ -132,8 +139,8 @@ __device__ __forceinline__ void free_parts_impl(const NodeTable& nt, const CompT
     const int lane = team.tid & 31, warp = team.warp;
     const int c = blockIdx.x;
     if (c >= fp.Geff) return;
-    double2* stage = reinterpret_cast<double2*>(scratch) + warp * (2 * 3 * 32);  // [2][3][32] double2 of this warp
-    double* wsum = scratch + FREE_STAGE_DOUBLES;                                  // [16][128]
+    double* wsum = scratch;                                                       // [16][128]
+    double2* stage = reinterpret_cast<double2*>(scratch + FREE_HEAD_DOUBLES) + warp * (2 * 3 * 32);  // [2][3][32] double2 of this warp
     const int np = nt.npad;
     const double taubar = __ldg(fp.taubar);
     long long u0 = free_slab_start(fp, c);
@@ -256,8 +263,8 @@ __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable
                                             const double* __restrict__ xsrc, double scale, double* scratch,
                                             double* y_local)
 {
-    double* csum = scratch + FREE_STAGE_DOUBLES + FREE_WARPS * FREE_ROWS;  // [ncomp]
-    double* wred = scratch + FREE_STAGE_DOUBLES;   // [nwarp] (the warp-sum area is free again)
+    double* csum = scratch + FREE_WARPS * FREE_ROWS;  // [ncomp]
+    double* wred = scratch;   // [nwarp] (the warp-sum area is free again)
     {   // sum of x over each OBSTACLE component (em != 0) that owns one of this CTA's rows: all warps share the
         // component, lanes strided, warp sums added in fixed order -- every CTA gets the same bits
         const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
@@ -280,10 +287,10 @@ __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable
     __syncthreads();
     // symmetric work split: row t of block J also receives sum_{I < J} PC[I][t].  These are up to NB - 1 loads per row, each
     // from another L2 line: four threads share a row (I = q, q + 4, ...; eight loads in flight each) and the four partial
-    // sums are added in fixed order.  rsum lives in the staging area (free again).
-    double* rsum = scratch;   // [rows]
+    // sums are added in fixed order.  rsum lives in the staging area (free again; fp.sym => the full scratch).
+    double* rsum = scratch + FREE_HEAD_DOUBLES;   // [rows]
     if (fp.sym) {
-        double* rpart = scratch + ((r1 - r0 + 1) & ~1);   // [4][rows]
+        double* rpart = rsum + ((r1 - r0 + 1) & ~1);   // [4][rows]
         const int rows = r1 - r0;
         for (int w = threadIdx.x; w < 4 * rows; w += blockDim.x) {
             const int q = w / rows, lr = w - q * rows;

@@ -44,9 +44,9 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
     const int lane = team.tid & 31, warp = team.warp, nwarp = team.nwarp;
     const int c = blockIdx.x;
     if (c >= fp.Geff) return;
-    double2* stage = reinterpret_cast<double2*>(scratch) + warp * (2 * 4 * 32);
-    double* wsum = scratch + SYM_STAGE_DOUBLES;
-    double* col = wsum + FREE_WARPS * FREE_ROWS + warp * (SYM_BATCH * SYM_COL_STRIDE);   // this warp's reverse sums of a batch
+    double* wsum = scratch;
+    double2* stage = reinterpret_cast<double2*>(scratch + FREE_HEAD_DOUBLES) + warp * (2 * 4 * 32);
+    double* col = scratch + FREE_HEAD_DOUBLES + SYM_STAGE_DOUBLES + warp * (SYM_BATCH * SYM_COL_STRIDE);   // this warp's reverse sums of a batch
     const int np = nt.npad;
     const double taubar = __ldg(fp.taubar);
     long long u0 = (long long)c * fp.U / fp.Geff;

@@ -52,6 +52,7 @@ struct GmresArgs {
     int nd;        // hybrid operator: columns [0, nd) come from the stored slab A, sources [nd, n) are recomputed
     int nwf;       // hybrid operator: warps 0..nwf-1 run the pair loops, the others stream the slab
     int res_pairs; // streaming GEMV: leading row pairs of every CTA block kept L2-resident (bie_gemv.cuh)
+    int scratch_doubles;  // matrix-free scratch in shared memory (full, or the smaller one of the one-directional loops)
     NodeTable nt;
     CompTable ct;
     FreePlan fp;
@@ -280,7 +281,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
     double* red = g + (m + 1);            // [34]
     double* gpart = red + 34 + ((m & 1) ? 0 : 1);  // GEMV partials or matrix-free scratch (16-byte aligned)
     // hybrid: GEMV partials of the slab and its result, after the matrix-free scratch
-    double* gpart2 = gpart + (FREE ? free_scratch_doubles(GM_THREADS) : 0);
+    double* gpart2 = gpart + (FREE ? a.scratch_doubles : 0);
     double* ydense = gpart2 + ((MODE == 1) ? 0 : ((gemv_part_doubles(a.rows_per_cta, MODE == 2 ? a.nd : n, a.chunk) + 1) & ~1));
     double* xs = ydense + ((MODE == 2) ? rows2 : 0);
     double* red2 = xs + ((MODE == 2) ? ((a.nd + 2) & ~1) : ((FREE || !XS) ? 0 : ((n + 2) & ~1)));   // [blockDim + rows2]
@@ -469,7 +470,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
 static inline size_t al256(size_t b) { return (b + 255) & ~(size_t)255; }
 
 struct GmresPlan {
-    int G, rows_per_cta, chunk, nld, VS;
+    int G, rows_per_cta, chunk, nld, VS, scratch_doubles;
     bool xs, stream;
     size_t smem;
     size_t offV, offW, offP, offR, offY, total;
@@ -477,7 +478,7 @@ struct GmresPlan {
 
 // mode: 0 stored matrix, 1 matrix-free, 2 hybrid (slab of nd columns streamed by 16 - nwf warps)
 static int gmres_plan(int n, int restart, int sm_count, int max_smem, int l2_bytes, long long lda, int mode, int nd,
-                      int nwf, GmresPlan* pl)
+                      int nwf, bool sym_possible, GmresPlan* pl)
 {
     const int m = restart;
     const bool free_op = (mode != 0);
@@ -486,9 +487,10 @@ static int gmres_plan(int n, int restart, int sm_count, int max_smem, int l2_byt
     pl->chunk = mode == 2 ? gemv_chunk(pl->rows_per_cta, nd, GM_THREADS / 32 - nwf)
                           : gemv_chunk(pl->rows_per_cta, n, GM_THREADS / 32);
     pl->nld = (n + 1) & ~1;
+    pl->scratch_doubles = free_op ? (sym_possible ? free_scratch_doubles(GM_THREADS) : free_scratch_doubles_onedir()) : 0;
     const int rows2 = (pl->rows_per_cta + 1) & ~1;
     size_t base = 2 * (size_t)rows2 + 2 * (size_t)(m + 2) + 2 * (size_t)m + (size_t)(m + 1) + 34 + 1;
-    if (free_op) base += (size_t)free_scratch_doubles(GM_THREADS);
+    if (free_op) base += (size_t)pl->scratch_doubles;
     if (mode != 1) base += (size_t)((gemv_part_doubles(pl->rows_per_cta, mode == 2 ? nd : n, pl->chunk) + 1) & ~1);
     if (mode == 2) base += (size_t)rows2 + (size_t)((nd + 2) & ~1);   // slab result, x of the slab's columns
     base *= sizeof(double);
@@ -559,7 +561,9 @@ int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, int nd, 
     if (restart > n) restart = n;  // the Krylov space cannot exceed n
     GmresPlan pl;
     const int nwf = ctx->hybrid_free_warps;
-    int rc = gmres_plan(n, restart, ctx->sm_count, ctx->max_smem_optin, ctx->l2_bytes, free_op ? n : lda, mode, nd, nwf, &pl);
+    // the symmetric loops (bie_free_sym.cuh) need the larger scratch; bie_free_plan decides later whether they run
+    const bool sym_possible = (mode == 1 && ctx->use_sym != 0) || (mode == 2 && ctx->use_sym == 2);
+    int rc = gmres_plan(n, restart, ctx->sm_count, ctx->max_smem_optin, ctx->l2_bytes, free_op ? n : lda, mode, nd, nwf, sym_possible, &pl);
     if (rc != BIE_OK) return rc;
     // align the caller's workspace to 256 bytes
     uintptr_t base = ((uintptr_t)ws + 255) & ~(uintptr_t)255;
@@ -574,7 +578,7 @@ int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, int nd, 
     a.yv = (double*)(base + pl.offY);
     a.sync = ctx->sync_buf;
     a.nld = pl.nld; a.rows_per_cta = pl.rows_per_cta; a.chunk = pl.chunk; a.VS = pl.VS;
-    a.nd = nd; a.nwf = nwf;
+    a.nd = nd; a.nwf = nwf; a.scratch_doubles = pl.scratch_doubles;
     a.res_pairs = (mode == 0 && pl.stream)
         ? bie_gemv_resident_pairs(ctx->l2_bytes, n, (long long)lda, pl.rows_per_cta, sizeof(double) * (size_t)(restart + 2) * pl.nld) : 0;
     memset(&a.nt, 0, sizeof(a.nt)); memset(&a.ct, 0, sizeof(a.ct)); memset(&a.fp, 0, sizeof(a.fp));
