@@ -19,6 +19,14 @@
  *     that the node tables derived from the last geometry live in the ctx (O(n) bytes, grown on demand).
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls are
  *     asynchronous on it unless stated otherwise.
+ *   - A ctx serves ONE stream at a time: its node tables, the matrix-free operator's tables and its staging
+ *     buffers are shared by all calls, so calls on the same ctx must be issued on one stream, or be ordered by
+ *     the caller (events) when the stream changes.  Use one ctx per concurrently used stream.  (The grid-barrier
+ *     counter of a solve lives in that call's workspace, that of bie_matvec_free in a ring of counters, so an
+ *     overlap of two launches cannot dead-lock the GPU; it can still give wrong numbers.)
+ *   - The first matrix-free or hybrid call after a geometry change (bie_matvec_free, bie_gmres with A == NULL,
+ *     bie_gmres_hybrid, bie_solve_host with those operators) builds the sparse matrix of near pairs and
+ *     SYNCHRONISES the stream once to size it (the number of near pairs comes back to the host; no capacity limit).
  *   - Components: component 0 is the free surface Gamma_0, component 1 the bottom
  *     Gamma_1, components 2.. the obstacles, parameterised CLOCKWISE (fluid on the left of solids, on
  *     the right of Gamma_0).  counts[c] = M_c nodes at alpha_{cl} = 2 pi l / M_c;

@@ -186,14 +186,21 @@ def normal_velocity(counts, zeta, dzeta, d2zeta, domega, rows=None) -> np.ndarra
     return out - 0.5 * hilbert(w[:M0])[rows]
 
 
-def matvec(A: np.ndarray, x: np.ndarray) -> np.ndarray:
-    """y = A x for a C-contiguous (nrows x ncols) block, ncols = len(x)."""
+def matvec(A: np.ndarray, x: np.ndarray, lda: Optional[int] = None) -> np.ndarray:
+    """y = A x for a C-contiguous (nrows x ncols) block, ncols = len(x).  With ``lda`` given, A is the flat (or 2-D)
+    storage of a row-major matrix whose rows are lda doubles apart and only the first len(x) columns of each are used."""
     A = np.ascontiguousarray(A, dtype=np.float64)
     x = np.ascontiguousarray(x, dtype=np.float64)
-    nrows, ncols = A.shape
+    if lda is None:
+        nrows, ncols = A.shape
+        lda = ncols
+    else:
+        ncols = x.size
+        assert lda >= ncols and A.size % lda == 0
+        nrows = A.size // lda
     assert x.size == ncols
     y = np.empty(nrows, dtype=np.float64)
-    lib().oracle_matvec_rect(nrows, ncols, _dp(A), ncols, _dp(x), _dp(y))
+    lib().oracle_matvec_rect(nrows, ncols, _dp(A), int(lda), _dp(x), _dp(y))
     return y
 
 

@@ -27,12 +27,15 @@ int bie_create(bie_ctx** out, int device)
     c->max_smem_optin = (int)prop.sharedMemPerBlockOptin;
     c->node_buf = nullptr; c->comp_buf = nullptr; c->free_buf = nullptr; c->cap = 0; c->have_geom = 0; c->n = 0;
     c->sync_buf = nullptr; c->pinned_i = nullptr; c->pinned_d = nullptr;
-    c->near_ptr = nullptr; c->near_col = nullptr; c->near_val = nullptr; c->near_valid = 0;
+    c->near_ptr = nullptr; c->near_col = nullptr; c->near_val = nullptr; c->near_valid = 0; c->near_cap = 0;
     c->hybrid_free_warps = BIE_HYBRID_FREE_WARPS;
-    c->taubar = nullptr; c->near_overflow = nullptr; c->kappa = nullptr;
+    c->taubar = nullptr; c->kappa = nullptr;
     c->pc_buf = nullptr; c->pc_cap = 0;
+    c->sym_tab = nullptr; c->sym_tab_bytes = 0; c->sym_U = 0; c->sym_first = 0; c->geom_gen = 0; c->sync_next = 0;
+    for (int i = 0; i < 4; ++i) c->sym_key[i] = -1;
+    for (int i = 0; i < 16; ++i) c->smem_set[i] = 0;
     c->use_sym = 1;   // bie_set_symmetric
-    if (cudaMalloc((void**)&c->sync_buf, 256) != cudaSuccess ||
+    if (cudaMalloc((void**)&c->sync_buf, 256 * (BIE_SYNC_SLOTS + 1)) != cudaSuccess ||
         cudaMallocHost((void**)&c->pinned_i, 4 * sizeof(int32_t)) != cudaSuccess ||
         cudaMallocHost((void**)&c->pinned_d, 4 * sizeof(double)) != cudaSuccess) {
         cudaError_t le = cudaGetLastError();
@@ -41,9 +44,8 @@ int bie_create(bie_ctx** out, int device)
         delete c;
         return bie_cuda_err(le == cudaSuccess ? cudaErrorMemoryAllocation : le);
     }
-    // the tail of the 256-byte block holds two device scalars
-    c->taubar = reinterpret_cast<double*>(reinterpret_cast<char*>(c->sync_buf) + 64);
-    c->near_overflow = reinterpret_cast<int*>(reinterpret_cast<char*>(c->sync_buf) + 128);
+    // the last 256-byte block holds a device scalar
+    c->taubar = reinterpret_cast<double*>(reinterpret_cast<char*>(c->sync_buf) + 256 * BIE_SYNC_SLOTS);
     *out = c;
     return BIE_OK;
 }
@@ -60,6 +62,7 @@ int bie_destroy(bie_ctx* c)
     if (c->near_val) cudaFree(c->near_val);
     if (c->kappa) cudaFree(c->kappa);
     if (c->pc_buf) cudaFree(c->pc_buf);
+    if (c->sym_tab) cudaFree(c->sym_tab);
     if (c->sync_buf) cudaFree(c->sync_buf);
     if (c->pinned_i) cudaFreeHost(c->pinned_i);
     if (c->pinned_d) cudaFreeHost(c->pinned_d);
@@ -133,16 +136,18 @@ int bie_build_cols(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* 
     return bie_launch_build(c, A, lda, ncols, 0, (cudaStream_t)stream);
 }
 
-int bie_hybrid_cols(bie_ctx* c, int n)
+// the slab's share of the columns that makes the slab stream and the pair loops finish together on a B200 (measured,
+// DESIGN.md "Hybrid operator"); a multiple of 128 = a row-block boundary of the pair loops
+static int hybrid_cols(int n)
 {
-    if (!c || n < 4) return 0;
-    // the slab's share of the columns that makes the streaming warps and the pair-loop warps finish together on a
-    // B200 (measured); a multiple of 128 = a row-block boundary of the pair loops
-    int nd = (int)((double)n * BIE_HYBRID_DENSE_FRACTION) & ~127;   // a row-block boundary of the pair loops (128 rows)
-    if (nd < 128) nd = 0;           // too small to be worth two teams: use bie_gmres
+    if (n < 4) return 0;
+    int nd = (int)((double)n * BIE_HYBRID_DENSE_FRACTION) & ~127;
+    if (nd < 128) nd = 0;           // too small to be worth two kinds of work: use bie_gmres
     if (nd > n - 2) nd = (n - 2) & ~1;
     return nd;
 }
+
+int bie_hybrid_cols(bie_ctx* c, int n) { return c ? hybrid_cols(n) : 0; }
 
 int bie_set_symmetric(bie_ctx* c, int on)
 {
@@ -248,12 +253,7 @@ static inline size_t up256(size_t b) { return (b + 255) & ~(size_t)255; }
 static int solve_cols(int n, int op)
 {
     if (op == BIE_OP_FREE) return 0;
-    if (op == BIE_OP_HYBRID) {
-        int nd = (int)((double)n * BIE_HYBRID_DENSE_FRACTION) & ~127;
-        if (nd < 128) return 0;
-        if (nd > n - 2) nd = (n - 2) & ~1;
-        return nd;
-    }
+    if (op == BIE_OP_HYBRID) return hybrid_cols(n);
     return n;
 }
 

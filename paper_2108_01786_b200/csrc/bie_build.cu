@@ -2,14 +2,15 @@
 //
 // Tiling.  A CTA of 128 threads owns a tile of T target rows x 256 source columns.  Each thread keeps the
 // per-node factors of TWO adjacent source columns in registers and walks down the T target rows, whose
-// factors (E_t, M_t) sit in shared memory and are read as warp-wide broadcasts.  A warp therefore writes,
+// factors E_t sit in shared memory and are read as warp-wide broadcasts.  A warp therefore writes,
 // per target row, 32 x 16 B = 512 contiguous bytes of that row (128-bit coalesced stores, full 128 B lines).
 //
-// Per entry (fast path): 13 FP64-pipe instructions + 1 MUFU + 1 integer compare, no transcendental
-// (bie_common.cuh).  The walk over the target rows is split into segments of constant target component, so
-// that the Re/Im selection of Eq. (3.10) and the -1/M_k of E_k become two
-// per-segment register coefficients (alpha, beta) and one fused constant em:
-//     entry = (alpha X + beta Y) / den - em
+// Per entry (fast path): 10 FP64-pipe instructions + 1 MUFU + 1 integer compare, no transcendental
+// (bie_common.cuh, "difference form").  The walk over the target rows is split into segments of constant target
+// component, so that the Re/Im selection of Eq. (3.10) and the -1/M_k of E_k become
+// three per-segment register coefficients (U, W, cst):
+//     entry = (U dr + W di) / den - cst,     dr + i di = E_s - E_t,   den = dr^2 + di^2,
+//     U = alpha Ei_s + 2 beta Er_s,  W = 2 beta Ei_s - alpha Er_s,  cst = beta + em,
 //     Im c  ->  (alpha, beta) = (-2 qi,  qr)     [k = 0, j = 0]  and  [k >= 1, j >= 1]
 //     Re c  ->  (alpha, beta) = (-2 qr, -qi)     [k = 0, j >= 1]
 //    -Re c  ->  (alpha, beta) = ( 2 qr,  qi)     [k >= 1, j = 0]
@@ -24,20 +25,18 @@
 #define BUILD_RB 4
 
 struct SrcCol {
-    double er, ei, m;   // E_s, M_s
+    double er, ei;      // E_s
     int thi;            // high word of thr_s
-    double a, b, em;    // per-segment coefficients
+    double u, w, cst;   // per-segment coefficients
 };
 
-__device__ __forceinline__ double bie_entry_fast(const SrcCol& s, const double2 te, const double tm, int& flag)
+__device__ __forceinline__ double bie_entry_fast(const SrcCol& s, const double2 te, int& flag)
 {
     const double dr = s.er - te.x, di = s.ei - te.y;
     const double den = fma(dr, dr, di * di);
-    const double X = fma(te.y, s.er, -(te.x * s.ei));
-    const double Y = s.m - tm;
-    const double val = fma(s.b, Y, s.a * X);
+    const double val = fma(s.w, di, s.u * dr);
     flag |= (__double2hiint(den) < s.thi) ? 1 : 0;
-    return fma(val, bie_rcp3(den), -s.em);
+    return fma(val, bie_rcp3(den), -s.cst);
 }
 
 // exact value of a near entry (rare): Laurent series from the coordinate differences, or the diagonal limit
@@ -52,21 +51,25 @@ static __device__ __noinline__ double bie_entry_near(const double2* __restrict__
     return fma(sb, ci, -0.5 * sa * cr) - sem;
 }
 
+// (alpha, beta) of the block (source on Gamma_0?, target on Gamma_0?) for the source weight q (bie_common.cuh)
+__device__ __forceinline__ void bie_block_coef(bool src0, bool tgt0, double qr, double qi, double& al, double& be)
+{
+    if (src0 == tgt0) { al = -2.0 * qi; be = qr; }       // Im c
+    else if (tgt0)    { al = -2.0 * qr; be = -qi; }      // Re c   (G_0j)
+    else              { al = 2.0 * qr;  be = qi; }       // -Re c  (-G_k0)
+}
+
 __global__ void __launch_bounds__(BUILD_THREADS)
 bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long lda, int T, int only0, int ncols)
 {
-    extern __shared__ __align__(16) double2 sm[];  // [T] E_t then [T] (M_t, -)
+    extern __shared__ __align__(16) double2 sm[];  // [T] E_t
     const int n = nt.n;
     const int c0 = blockIdx.x * BUILD_TILE_W;
     const int t0 = blockIdx.y * T;
     const int t1 = min(t0 + T, n);
     if (only0 && t0 >= ct.off[1] && c0 >= ct.off[1]) return;  // a4: solid-solid tiles stay
     double2* sE = sm;
-    double* sM = reinterpret_cast<double*>(sm + T);
-    for (int i = threadIdx.x; i < t1 - t0; i += BUILD_THREADS) {
-        sE[i] = nt.E[t0 + i];
-        sM[i] = nt.MT[t0 + i].x;
-    }
+    for (int i = threadIdx.x; i < t1 - t0; i += BUILD_THREADS) sE[i] = nt.E[t0 + i];
     const int s0 = c0 + BUILD_COLS * threadIdx.x;  // < npad by construction
     SrcCol src[BUILD_COLS];
     double sqr[BUILD_COLS], sqi[BUILD_COLS], sem[BUILD_COLS];
@@ -74,7 +77,7 @@ bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long l
 #pragma unroll
     for (int c = 0; c < BUILD_COLS; ++c) {
         const double2 e = nt.E[s0 + c], mt = nt.MT[s0 + c], q = nt.Q[s0 + c];
-        src[c].er = e.x; src[c].ei = e.y; src[c].m = mt.x;
+        src[c].er = e.x; src[c].ei = e.y;
         src[c].thi = __double2hiint(mt.y);
         sqr[c] = q.x; sqi[c] = q.y;
         sem[c] = nt.DG[s0 + c].y;
@@ -88,11 +91,11 @@ bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long l
         if (a >= b) continue;
 #pragma unroll
         for (int c = 0; c < BUILD_COLS; ++c) {
-            const bool src0 = (scomp[c] == 0), tgt0 = (k == 0);
-            if (src0 == tgt0) { src[c].a = -2.0 * sqi[c]; src[c].b = sqr[c]; }       // Im c
-            else if (tgt0)    { src[c].a = -2.0 * sqr[c]; src[c].b = -sqi[c]; }      // Re c   (G_0j)
-            else              { src[c].a = 2.0 * sqr[c];  src[c].b = sqi[c]; }       // -Re c  (-G_k0)
-            src[c].em = (scomp[c] == k) ? sem[c] : 0.0;
+            double al, be;
+            bie_block_coef(scomp[c] == 0, k == 0, sqr[c], sqi[c], al, be);
+            src[c].u = fma(al, src[c].ei, 2.0 * be * src[c].er);
+            src[c].w = fma(-al, src[c].er, 2.0 * be * src[c].ei);
+            src[c].cst = be + ((scomp[c] == k) ? sem[c] : 0.0);
         }
         for (int tb = a; tb < b; tb += BUILD_RB) {
             int flag = 0;
@@ -101,9 +104,8 @@ bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long l
             for (int r = 0; r < BUILD_RB; ++r) {
                 const int t = min(tb + r, b - 1);  // the tail repeats the last row (same values, same address)
                 const double2 te = sE[t - t0];
-                const double tm = sM[t - t0];
-                const double e0 = bie_entry_fast(src[0], te, tm, flag);
-                const double e1 = bie_entry_fast(src[1], te, tm, flag);
+                const double e0 = bie_entry_fast(src[0], te, flag);
+                const double e1 = bie_entry_fast(src[1], te, flag);
                 double* p = row + (long long)(t - tb) * lda;
                 if (full) *reinterpret_cast<double2*>(p) = make_double2(e0, e1);
                 else if (part) p[0] = e0;
@@ -118,8 +120,12 @@ bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long l
                             if (s0 + c >= ncols) continue;
                             const double dr = src[c].er - te.x, di = src[c].ei - te.y;
                             const double den = fma(dr, dr, di * di);
-                            if (__double2hiint(den) < src[c].thi)
-                                A[(long long)t * lda + s0 + c] = bie_entry_near(nt.DG, nt.XY, src[c].a, src[c].b, src[c].em, s0 + c, t);
+                            if (__double2hiint(den) < src[c].thi) {
+                                double al, be;
+                                bie_block_coef(scomp[c] == 0, k == 0, sqr[c], sqi[c], al, be);
+                                A[(long long)t * lda + s0 + c] =
+                                    bie_entry_near(nt.DG, nt.XY, al, be, (scomp[c] == k) ? sem[c] : 0.0, s0 + c, t);
+                            }
                         }
                     }
                 }
@@ -268,7 +274,7 @@ int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int ncols, int only_c
     {
         int occ = 0;
         if (dagger) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bie_build_dagger_kernel, BUILD_THREADS, 7 * 8 * 256 + 16);
-        else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bie_build_kernel, BUILD_THREADS, 3 * 8 * 256 + 16);
+        else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bie_build_kernel, BUILD_THREADS, 2 * 8 * 256 + 16);
         const long long wave = (long long)ctx->sm_count * (occ > 0 ? occ : 1);
         if ((long long)gx * ((nt_rows + 127) / 128) >= 2 * wave) {
             double best = 0.0;
@@ -287,7 +293,7 @@ int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int ncols, int only_c
         BIE_CUDA(cudaGetLastError());
         return BIE_OK;
     }
-    bie_build_kernel<<<grid, BUILD_THREADS, (sizeof(double2) + sizeof(double)) * T + 16, st>>>(nt, ctx->comps, A, (long long)lda, T,
+    bie_build_kernel<<<grid, BUILD_THREADS, sizeof(double2) * T + 16, st>>>(nt, ctx->comps, A, (long long)lda, T,
                                                                                             only_comp0, ncols);
     BIE_CUDA(cudaGetLastError());
     return BIE_OK;

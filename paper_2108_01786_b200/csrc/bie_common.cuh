@@ -8,11 +8,17 @@
 //              = ( -2 X + i Y ) / den,    X = Im(E_t conj E_s),  Y = M_s - M_t,  den = |E_s - E_t|^2 .
 // With the source weight q_s = zeta'_s/(2 M_j) the entry is (alpha X + beta Y)/den:
 //     Im{q cot} : (alpha, beta) = (-2 qi,  qr)     Re{q cot} : (-2 qr, -qi)     -Re{q cot} : (2 qr, qi)
-// i.e. 13 FP64-pipe instructions per pair including the reciprocal (bie_rcp3).  E_s - E_t cancels for
-// |w| -> 0 (relative error about 10 eps/|w|, entry error about 20 eps |q_s|/|w|^2); pairs with
-// den < thr_s = tau_s M_s, tau_s = BIE_NEAR_C |q_s| (clamped), are "near": they are recomputed from the
-// coordinate differences with the Laurent series of cot (bie_cot_half_near), accurate to rounding, and the
-// pair s == t takes the analytic diagonal limit.
+// "Difference form" (Eq. (3.16) build and its matrix-free operator): with d = E_s - E_t = dr + i di, which den
+// needs anyway,  X = Ei_s dr - Er_s di  and  Y = 2 (Er_s dr + Ei_s di) - den,  so that
+//     (alpha X + beta Y)/den = (U_s dr + W_s di)/den - beta,   U_s = alpha Ei_s + 2 beta Er_s,  W_s = 2 beta Ei_s - alpha Er_s:
+// the numerator costs 2 FP64 instructions from per-SOURCE constants and the constant -beta (the far-field limit
+// cot -> -+i) is added per entry by the final FMA of the build (10 FP64-pipe instructions per entry: 2 sub, 2 den,
+// 2 numerator, 3 reciprocal (bie_rcp3), 1 FMA) or, in the matrix-free operator, once per application as
+// -sum_s beta_s x_s (10 per pair including the accumulation).  The vortex-sheet / normal-velocity builds, whose weight
+// belongs to the ROW node, keep the (X, Y) form (13 per entry).  E_s - E_t cancels for |w| -> 0 (relative error of d
+// about eps/|w|, entry error a few eps |q_s|/|w|^2); pairs with den < thr_s = tau_s M_s, tau_s = BIE_NEAR_C |q_s|
+// (clamped), are "near": they are recomputed from the coordinate differences with the Laurent series of cot
+// (bie_cot_half_near), accurate to rounding, and the pair s == t takes the analytic diagonal limit.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -26,7 +32,7 @@
 #define BIE_NEAR_TAU_MAX 1.0e-2       // |w| < 0.1: Laurent truncation 2|w/2|^9/93555 < 1e-16
 #define BIE_HYBRID_FREE_WARPS 8        // hybrid operator: warps of a CTA on the pair loops (of 16)
 #define BIE_HYBRID_DENSE_FRACTION 0.42 // hybrid operator: share of the columns kept as a stored slab
-#define BIE_NEAR_PER_NODE 48          // capacity of the CSR near matrix of the matrix-free operator, entries per node
+#define BIE_SYNC_SLOTS 16             // grid-barrier counters of a ctx (bie_matvec_free cycles through them), 256 B apart
 
 // Node table, arrays of double2 of length npad.
 struct NodeTable {
@@ -59,16 +65,24 @@ struct bie_ctx {
     double* free_buf;        // matrix-free operator: per-matvec source tables [8][cap] + partial sums (bie_free.cuh)
     double* taubar;          // device scalar: max_s tau_s of the current geometry (bie_near.cu)
     int* near_ptr;           // CSR near matrix (bie_near.cu): [8 cap + 1] offsets of the (row, segment) lists
-    int* near_col;           // [BIE_NEAR_PER_NODE cap]
-    double* near_val;        // [BIE_NEAR_PER_NODE cap]
-    int* near_overflow;      // device flag: the near matrix did not fit (the operator then returns NaN)
+    int* near_col;           // [near_cap] column indices, grown to the scanned total (bie_ensure_near)
+    double* near_val;        // [near_cap]
+    size_t near_cap;         // entries allocated in near_col / near_val
     int near_valid;          // near matrix built for the current geometry
     double* pc_buf;          // symmetric matrix-free operator: reverse partials [row blocks][npad] (bie_free_sym.cuh)
     size_t pc_cap;           // doubles allocated in pc_buf
+    char* sym_tab;           // device tables of the symmetric work list (cum, perm, pos), cached per geometry and split
+    size_t sym_tab_bytes;
+    long long sym_key[4];    // (geometry generation, s_off, grid, 1) the cached tables were made for
+    long long sym_U;         // their total number of list positions
+    int sym_first;
+    long long geom_gen;      // incremented by every bie_prepare_nodes
+    int smem_set[16];        // dynamic shared memory already granted to the kernel instantiations (cudaFuncSetAttribute once)
     int use_sym;             // use the symmetric work split for the whole-matrix matrix-free operator
     double* kappa;           // [cap] real-cot table of the normal-velocity operator (bie_build_normal_velocity)
     int hybrid_free_warps;   // hybrid operator: warps per CTA on the pair loops (the other 16 - this stream the slab)
-    unsigned int* sync_buf;  // grid-barrier counter
+    unsigned int* sync_buf;  // BIE_SYNC_SLOTS grid-barrier counters (256 B apart) + two device scalars behind them
+    int sync_next;           // next counter slot (bie_matvec_free); bie_gmres keeps its counter in the caller's workspace
     int cap;
     // current geometry (host copies)
     int have_geom;
@@ -101,13 +115,24 @@ static inline int bie_gemv_resident_pairs(int l2_bytes, int nrows, long long lda
     return (int)(frac * rows_per_cta) / 2;
 }
 
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) once per kernel instantiation (slot) and ctx, again only when a call
+// needs more than was granted before
+template <typename K>
+static inline int bie_grant_smem(bie_ctx* ctx, int slot, K kernel, size_t smem)
+{
+    if ((int)smem > ctx->smem_set[slot]) {
+        BIE_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        ctx->smem_set[slot] = (int)smem;
+    }
+    return BIE_OK;
+}
+
 static inline int bie_npad(int n) { return (n + BIE_NODE_PAD - 1) / BIE_NODE_PAD * BIE_NODE_PAD; }
 NodeTable bie_node_table(const bie_ctx* ctx);
 struct FreePlan;
 // doubles of ctx->free_buf for a node capacity `cap`; work split of the matrix-free operator over `grid` CTAs
 size_t bie_free_buf_doubles(int cap);
-int bie_free_plan(const bie_ctx* ctx, int grid, int s_off, FreePlan* fp, cudaStream_t st);
-size_t bie_near_cap(int npad);
+int bie_free_plan(bie_ctx* ctx, int grid, int s_off, FreePlan* fp, cudaStream_t st);
 int bie_ensure_near(bie_ctx* ctx, cudaStream_t st);
 
 // internal entry points (one per .cu)

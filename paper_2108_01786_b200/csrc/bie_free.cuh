@@ -2,15 +2,15 @@
 // Eq. (3.16) recomputed on the fly from the node tables; no matrix traffic at all.
 // Device functions shared by bie_matvec_free (bie_matvec.cu) and the matrix-free GMRES (bie_gmres.cu).
 //
-// Arithmetic.  With E = e^{i zeta} per node (bie_common.cuh), X = Im(E_t conj E_s), Y = M_s - M_t and the
-// block coefficients (alpha, beta) of Eq. (3.10), the product of an entry with x_s is
-//     A[t][s] x_s = (alpha X + beta Y) x_s / den
-//                 = ( Ei_t P_s - Er_t Q_s + R_s - M_t B_s ) / den,          den = |E_s - E_t|^2,
-//     P_s = alpha x_s Er_s,  Q_s = alpha x_s Ei_s,  R_s = beta x_s M_s,  B_s = beta x_s,
-// so everything that depends on the source alone is folded, once per matvec and per source (O(n)), into two
-// double2 (P,Q), (R,B) per target class (class 0: target on Gamma_0, class 1: target on a solid; the class fixes
-// the Re/Im/sign selection of Eq. (3.10)).  Per pair that leaves 11 FP64-pipe instructions:
-// 2 sub, 2 for den, 3 FMA for the numerator, 3 FMA refining MUFU.RCP64H (bie_rcp3), 1 FMA accumulating.
+// Arithmetic ("difference form", bie_common.cuh).  With E = e^{i zeta} per node, d = E_s - E_t = dr + i di,
+// den = |d|^2 and the block coefficients (alpha, beta) of Eq. (3.10), the product of an entry with x_s is
+//     A[t][s] x_s = (alpha X + beta Y) x_s / den = ( U_s dr + W_s di ) / den - beta_s x_s,
+//     U_s = x_s (alpha Ei_s + 2 beta Er_s),   W_s = x_s (2 beta Ei_s - alpha Er_s),
+// so everything that depends on the source alone is folded, once per matvec and per source (O(n)), into ONE
+// double2 (U, W) per target class (class 0: target on Gamma_0, class 1: target on a solid; the class fixes
+// the Re/Im/sign selection of Eq. (3.10)), and the constant -sum_s beta_s x_s (one number per
+// class and application) is subtracted by the row owner.  Per pair that leaves 10 FP64-pipe instructions:
+// 2 sub, 2 for den, 2 for the numerator, 3 FMA refining MUFU.RCP64H (bie_rcp3), 1 FMA accumulating.
 //
 // Work split.  The rows are cut into row blocks of FREE_ROWS = 128 targets of one class; the (row block x source)
 // rectangle list is laid out linearly and cut into gridDim.x equal slabs, one per CTA, so every SM has the same
@@ -24,8 +24,9 @@
 // Near pairs.  den < taubar M_t (den/M_t = |e^{iw} - 1|^2 ~ |w|^2; this includes s == t) marks a pair as near:
 // it is left out of the fast sum by predication, and its exact entry (Laurent series of cot, or the analytic
 // diagonal limit PAPER.md:L265) comes from the sparse near matrix that bie_near.cu builds once per geometry;
-// the owner of a row adds  sum_k val[k] x[col[k]]  when it gathers the partials.  The rank-one E_k
-// is applied there too, as -(1/M_k) sum_{s in k} x_s.
+// the owner of a row adds  sum_k val[k] x[col[k]]  when it gathers the partials (val = entry + beta_s: the
+// constant term above runs over ALL sources).  The rank-one E_k is applied there too, as
+// -(1/M_k) sum_{s in k} x_s.
 #pragma once
 #include "bie_common.cuh"
 
@@ -54,14 +55,15 @@ struct FreePlan {
     int sym_first;              // sym: first row block of the triangle (0; hybrid: the block that starts at s_off)
     int vortex;      // 1: the vortex-sheet matrix S (BIE_VARIANT_VORTEX) instead of Eq. (3.16); see free_parts
     int s_off;       // first source of the operator (0; the hybrid operator reads the sources below it from its slab)
-    double2* T;      // [4][npad]: (P,Q) class 0, (R,B) class 0, (P,Q) class 1, (R,B) class 1
+    double2* T;      // [2][npad]: (U,W) class 0, (U,W) class 1     (vortex: (P,Q) = mu E, (R,B) = mu (M, 1))
+    double* SB;      // [2][FREE_SB_LD] per-CTA partials of sum_s beta_s x_s (class 0, class 1), written with the tables
     double* PB;      // [(NB + Geff)][FREE_ROWS] partial sums, part id = row block + CTA
     const double* taubar;     // device scalar: near threshold relative to M_t (bie_near.cu)
     const int* near_ptr;      // CSR near matrix: offsets of the (row, segment) lists, row t = [ptr[8t], ptr[8t+8])
     const int* near_col;
     const double* near_val;
-    const int* near_overflow; // != 0: the near matrix did not fit; the operator returns NaN
 };
+#define FREE_SB_LD 256   // >= gridDim.x (one CTA per SM, <= 256 SMs)
 
 // doubles of shared scratch, in this order: warp sums [16][128], component sums [BIE_MAX_COMP + 2], warp staging buffers
 // [16][2 stages][4][32] double2 (3 of the 4 arrays used by the one-directional loops), reverse-sum slots of bie_free_sym.cuh
@@ -92,15 +94,18 @@ __device__ __forceinline__ int free_block_rows(const FreePlan& fp, int b, int n)
 }
 
 // ---- step 1: per-source tables for the vector v (rows [r0, r1) of this CTA; v indexed from r0) ------------
+// Also leaves this CTA's share of sum_{s >= s_off} beta_s x_s (per class) in fp.SB.  red: shared, >= 66 doubles.
+// All threads of the CTA must call; no barrier at the end (the caller's next barrier orders `red`).
 __device__ __forceinline__ void free_write_tables(const NodeTable& nt, const CompTable& ct, const FreePlan& fp, int r0,
-                                                  int r1, const double* v /* shared or global, v[s - r0] */)
+                                                  int r1, const double* v /* shared or global, v[s - r0] */, double* red)
 {
     const int np = nt.npad;
+    double sb0 = 0.0, sb1 = 0.0;
     for (int s = r0 + threadIdx.x; s < r1; s += blockDim.x) {
         const double2 e = nt.E[s], q = nt.Q[s];
-        const double M = nt.MT[s].x;
         const double x = v[s - r0];
         if (fp.vortex) {   // S: the source only carries mu_s = x_s / M_j (the weight zeta' belongs to the ROW, Eq. 4.7)
+            const double M = nt.MT[s].x;
             const int j = nt.COMP[s];
             const double mu = x / (double)(ct.off[j + 1] - ct.off[j]);
             fp.T[s]      = make_double2(mu * e.x, mu * e.y);
@@ -113,16 +118,28 @@ __device__ __forceinline__ void free_write_tables(const NodeTable& nt, const Com
         if (src0) { a0 = -2.0 * q.y; b0 = q.x;  a1 = 2.0 * q.x;  b1 = q.y; }   // K_00 ; -G_k0
         else      { a0 = -2.0 * q.x; b0 = -q.y; a1 = -2.0 * q.y; b1 = q.x; }   // G_0j ; K_kj
         a0 *= x; b0 *= x; a1 *= x; b1 *= x;
-        fp.T[s]          = make_double2(a0 * e.x, a0 * e.y);
-        fp.T[np + s]     = make_double2(b0 * M, b0);
-        fp.T[2 * np + s] = make_double2(a1 * e.x, a1 * e.y);
-        fp.T[3 * np + s] = make_double2(b1 * M, b1);
+        fp.T[s]      = make_double2(fma(a0, e.y, 2.0 * b0 * e.x), fma(-a0, e.x, 2.0 * b0 * e.y));
+        fp.T[np + s] = make_double2(fma(a1, e.y, 2.0 * b1 * e.x), fma(-a1, e.x, 2.0 * b1 * e.y));
+        if (s >= fp.s_off) { sb0 += b0; sb1 += b1; }
+    }
+    if (fp.vortex) return;
+    // fixed-order sum over the CTA: lanes by shuffle, warps by thread 0
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    sb0 = bie_warp_sum(sb0); sb1 = bie_warp_sum(sb1);
+    __syncthreads();
+    if (lane == 0) { red[warp] = sb0; red[32 + warp] = sb1; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t0 = 0.0, t1 = 0.0;
+        for (int w = 0; w < nwarp; ++w) { t0 += red[w]; t1 += red[32 + w]; }
+        fp.SB[blockIdx.x] = t0;
+        fp.SB[FREE_SB_LD + blockIdx.x] = t1;
     }
 }
 
 // ---- step 2: this CTA's slab of the (row block x source) list -> partial sums in fp.PB --------------------
 // scratch: shared, free_scratch_doubles() doubles, 16-byte aligned.  All threads of the team must call.
-// VORTEX: the matrix S of Eqs. (4.14) + (4.17) (bie_build.cu, "Vortex-sheet variant"): entry x_s = (A_t X' + B_t Y')/den with
+// VORTEX: the matrix S of Eqs. (4.14) + (4.17) (bie_build.cu, "Vortex-sheet variant"), in the (X, Y) form: entry x_s = (A_t X' + B_t Y')/den with
 // X' = Ei_t P_s - Er_t Q_s, Y' = R_s - M_t B_s from the class-independent tables (P,Q) = mu_s E_s, (R,B) = mu_s (M_s, 1), and the
 // row's (A_t, B_t) = (2u_i, -u_r) / +-(2u_r, u_i), u_t = zeta'_t/2, which depend on whether the SOURCE lies on Gamma_0: the
 // warp's source range is cut at M_0.  13 FP64-pipe instructions per pair.
@@ -181,8 +198,8 @@ __device__ __forceinline__ void free_parts_impl(const NodeTable& nt, const CompT
         const int wa_all = sa + 2 * (int)((long long)units * warp / team.nwarp);
         const int wb_all = sa + 2 * (int)((long long)units * (warp + 1) / team.nwarp);
         const double2* TE = nt.E;
-        const double2* TPQ = fp.T + (VORTEX ? (size_t)0 : (size_t)(2 * cls) * np);
-        const double2* TRB = fp.T + (VORTEX ? (size_t)np : (size_t)(2 * cls + 1) * np);
+        const double2* TPQ = fp.T + (VORTEX ? (size_t)0 : (size_t)cls * np);   // Eq. (3.16): (U, W) of the rows' class
+        const double2* TRB = fp.T + (size_t)np;                                 // VORTEX only
         const double2 zero2 = make_double2(0.0, 0.0);
         for (int sgm = 0; sgm < (VORTEX ? 2 : 1); ++sgm) {
         // VORTEX: sources on Gamma_0 first, then the solids (different row coefficients); else the whole range at once
@@ -197,7 +214,7 @@ __device__ __forceinline__ void free_parts_impl(const NodeTable& nt, const CompT
             double2* sg = stage + bufi * 96;
             free_cp_async16(sg + lane, TE + sc, sz);
             free_cp_async16(sg + 32 + lane, TPQ + sc, sz);
-            free_cp_async16(sg + 64 + lane, TRB + sc, sz);
+            if (VORTEX) free_cp_async16(sg + 64 + lane, TRB + sc, sz);
             asm volatile("cp.async.commit_group;" ::: "memory");
         };
         int buf = 0;
@@ -211,7 +228,9 @@ __device__ __forceinline__ void free_parts_impl(const NodeTable& nt, const CompT
             const int cnt = min(32, wb - base);   // even
 #pragma unroll FREE_SRC_UNROLL
             for (int j = 0; j < cnt; ++j) {
-                const double2 e = sg[j], pq = sg[32 + j], rb = sg[64 + j];
+                const double2 e = sg[j], pq = sg[32 + j];
+                double2 rb;
+                if (VORTEX) rb = sg[64 + j];
 #pragma unroll
                 for (int i = 0; i < FREE_NT; ++i) {
                     const double dr = e.x - ter[i], di = e.y - tei[i];
@@ -222,9 +241,7 @@ __device__ __forceinline__ void free_parts_impl(const NodeTable& nt, const CompT
                         const double Y = fma(-tm[i], rb.y, rb.x);
                         val = fma(cb[sgm][i], Y, ca[sgm][i] * X);
                     } else {
-                        val = fma(tei[i], pq.x, rb.x);
-                        val = fma(-ter[i], pq.y, val);
-                        val = fma(-tm[i], rb.y, val);
+                        val = fma(pq.y, di, pq.x * dr);     // U_s dr + W_s di
                     }
                     const double r = bie_rcp3(den);
                     if (!(__double2hiint(den) < thi[i])) acc[i] = fma(val, r, acc[i]);
@@ -314,7 +331,16 @@ __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable
             rsum[lr] = (rpart[lr] + rpart[rows + lr]) + (rpart[2 * rows + lr] + rpart[3 * rows + lr]);
         __syncthreads();
     }
-    const bool bad = (__ldcg(fp.near_overflow) != 0);
+    // sum_s beta_s x_s per class: the per-CTA partials of free_write_tables in fixed order (warp 0 and 1), via shared memory
+    double* sbs = scratch + FREE_WARPS * FREE_ROWS + ((BIE_MAX_COMP + 2 + 1) & ~1) - 2;   // the two doubles after csum[BIE_MAX_COMP]
+    if (!fp.vortex && threadIdx.x < 64) {
+        const int c = threadIdx.x >> 5, lane = threadIdx.x & 31;
+        double sb = 0.0;
+        for (int i = lane; i < (int)gridDim.x; i += 32) sb += __ldcg(fp.SB + c * FREE_SB_LD + i);
+        sb = bie_warp_sum(sb);
+        if (lane == 0) sbs[c] = sb;
+    }
+    __syncthreads();
     for (int t = r0 + threadIdx.x; t < r1; t += blockDim.x) {
         int b, off;
         if (t < fp.M0) { b = t / FREE_ROWS; off = t - b * FREE_ROWS; }
@@ -334,14 +360,15 @@ __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable
         // near pairs: exact entries from the CSR near matrix
         const int p0 = fp.near_ptr[8 * (size_t)t], p1 = fp.near_ptr[8 * (size_t)t + 8];
         double sn = 0.0;
-        for (int p = p0; p < p1 && !bad; ++p) {   // (on overflow the offsets run past the arrays)
+        for (int p = p0; p < p1; ++p) {
             const int cix = fp.near_col[p];
             if (cix >= fp.s_off) sn = fma(fp.near_val[p], __ldcg(xsrc + cix), sn);
         }
         s += sn;
+        if (!fp.vortex) s -= sbs[t < fp.M0 ? 0 : 1];
         const int k = nt.COMP[t];
         s = fma(-nt.DG[t].y, csum[k], s);
-        y_local[t - r0] = bad ? __longlong_as_double(0x7ff8000000000000LL) : s * scale;
+        y_local[t - r0] = s * scale;
     }
     __syncthreads();
 }

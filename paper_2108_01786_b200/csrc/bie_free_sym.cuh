@@ -1,8 +1,9 @@
 // bie_free_sym.cuh -- the matrix-free operator of bie_free.cuh using the ODDNESS of the kernel:
 //     cot((zeta_s - zeta_t)/2) = -cot((zeta_t - zeta_s)/2),
 // so den = |E_s - E_t|^2, its reciprocal and the differences E_s - E_t serve the entry (t,s) AND the entry (s,t) of
-// Eq. (3.16) (SURVEY section 7 "oddness").  Per pair of entries: 2 sub + 2 den + 3 rcp shared, 3 + 1 FMA for each direction:
-// 15 FP64-pipe instructions for two entries instead of 22, plus the lane reduction of the reverse sums.
+// Eq. (3.16) (SURVEY section 7 "oddness").  Per pair of entries, in the difference form of bie_common.cuh: 2 sub + 2 den + 3 rcp
+// shared, 2 + 1 for each direction (forward (U_s dr + W_s di)/den, reverse -(U'_t dr + W'_t di)/den: E_t - E_s = -(dr + i di)):
+// 13 FP64-pipe instructions for two entries instead of 20, plus the lane reduction of the reverse sums.
 //
 // Work split.  Row block I (FREE_ROWS rows of one class) x the sources s >= row0(I): the block's own rows one-directionally
 // (all their pairs are inside), the later sources symmetrically -- forward A[t][s] x_s into the lane's register sums as in
@@ -63,7 +64,7 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
         const bool below = (row0 + rows <= fp.s_off);        // hybrid: a row block of the slab's columns
         const int src0 = below ? fp.s_off : row0;
         const int sa = src0 + (int)(u0 - ub), sb = src0 + (int)(ue - ub);   // sources [sa, sb), all >= src0
-        double ter[FREE_NT], tei[FREE_NT], tm[FREE_NT], acc[FREE_NT];
+        double ter[FREE_NT], tei[FREE_NT], acc[FREE_NT];
         int thi[FREE_NT];
         bool live[FREE_NT];
 #pragma unroll
@@ -71,16 +72,15 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
             live[i] = (lane + 32 * i < rows);
             const int t = row0 + min(lane + 32 * i, rows - 1);   // inactive slots shadow the last row; forward result dropped
             const double2 e = nt.E[t];
-            ter[i] = e.x; tei[i] = e.y; tm[i] = nt.MT[t].x; acc[i] = 0.0;
-            thi[i] = __double2hiint(taubar * tm[i]);
+            ter[i] = e.x; tei[i] = e.y; acc[i] = 0.0;
+            thi[i] = __double2hiint(taubar * nt.MT[t].x);
         }
         const int span = sb - sa;
         const int wa_all = sa + (int)((long long)span * warp / nwarp);
         const int wb_all = sa + (int)((long long)span * (warp + 1) / nwarp);
         const int d_end = below ? np : row0 + rows;           // end of the one-directional sources (the block's own rows)
         const int c_end = below ? np : ((cls == 0) ? fp.M0 : np);   // end of the sources of the block's own class
-        const double2* TPQ = fp.T + (size_t)(2 * cls) * np;      // forward tables: the class of the block's rows
-        const double2* TRB = fp.T + (size_t)(2 * cls + 1) * np;
+        const double2* TUW = fp.T + (size_t)cls * np;            // forward tables: (U, W) for the class of the block's rows
         for (int sgm = 0; sgm < 3; ++sgm) {
             // 0: own rows (one direction); 1: later sources of the same class; 2: sources on solids below a Gamma_0 block
             const int lo = sgm == 0 ? src0 : (sgm == 1 ? d_end : c_end);
@@ -89,33 +89,33 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
             if (wa >= wb) continue;                          // warp-uniform
             const bool rev = (sgm != 0);
             const int rcls = (sgm == 2) ? 1 : cls;           // class of the ROWS of the reverse entries (= of these sources)
-            double tp[FREE_NT], tq[FREE_NT], tr[FREE_NT], tb[FREE_NT];
+            double tu[FREE_NT], tw[FREE_NT];
 #pragma unroll
             for (int i = 0; i < FREE_NT; ++i) {
-                tp[i] = tq[i] = tr[i] = tb[i] = 0.0;
+                tu[i] = tw[i] = 0.0;
                 if (rev && live[i]) {                        // this target as a SOURCE of rows of class rcls
                     const int t = row0 + lane + 32 * i;
-                    const double2 pq = __ldcg(fp.T + (size_t)(2 * rcls) * np + t), rb = __ldcg(fp.T + (size_t)(2 * rcls + 1) * np + t);
-                    tp[i] = pq.x; tq[i] = pq.y; tr[i] = rb.x; tb[i] = rb.y;
+                    const double2 uw = __ldcg(fp.T + (size_t)rcls * np + t);
+                    tu[i] = uw.x; tw[i] = uw.y;
                 }
             }
-            double2 ne = zero2, npq = zero2, nrb = zero2, nmt = zero2;
+            double2 ne = zero2, nuw = zero2, nmt = zero2;
             if (wa + lane < wb) {
                 const int s = wa + lane;
-                ne = nt.E[s]; npq = __ldcg(TPQ + s); nrb = __ldcg(TRB + s);
+                ne = nt.E[s]; nuw = __ldcg(TUW + s);
                 const double M = nt.MT[s].x; nmt = make_double2(M, taubar * M);
             }
             int buf = 0;
             __syncwarp();
             for (int base = wa; base < wb; base += 32, buf ^= 1) {
                 double2* sg = stage + buf * 128;
-                sg[lane] = ne; sg[32 + lane] = npq; sg[64 + lane] = nrb; sg[96 + lane] = nmt;
+                sg[lane] = ne; sg[32 + lane] = nuw; sg[96 + lane] = nmt;
                 __syncwarp();
                 {
                     const int s = base + 32 + lane;
-                    ne = zero2; npq = zero2; nrb = zero2; nmt = zero2;
+                    ne = zero2; nuw = zero2; nmt = zero2;
                     if (s < wb) {
-                        ne = nt.E[s]; npq = __ldcg(TPQ + s); nrb = __ldcg(TRB + s);
+                        ne = nt.E[s]; nuw = __ldcg(TUW + s);
                         const double M = nt.MT[s].x; nmt = make_double2(M, taubar * M);
                     }
                 }
@@ -123,14 +123,12 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
                 if (!rev) {
 #pragma unroll 2
                     for (int j = 0; j < cnt; ++j) {
-                        const double2 e = sg[j], pq = sg[32 + j], rb = sg[64 + j];
+                        const double2 e = sg[j], uw = sg[32 + j];
 #pragma unroll
                         for (int i = 0; i < FREE_NT; ++i) {
                             const double dr = e.x - ter[i], di = e.y - tei[i];
                             const double den = fma(dr, dr, di * di);
-                            double val = fma(tei[i], pq.x, rb.x);
-                            val = fma(-ter[i], pq.y, val);
-                            val = fma(-tm[i], rb.y, val);
+                            const double val = fma(uw.y, di, uw.x * dr);
                             const double r = bie_rcp3(den);
                             if (!(__double2hiint(den) < thi[i])) acc[i] = fma(val, r, acc[i]);
                         }
@@ -140,26 +138,23 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
 #pragma unroll
                         for (int u = 0; u < SYM_BATCH; ++u) {
                             const int j = j0 + u;
-                            const double2 e = sg[j], pq = sg[32 + j], rb = sg[64 + j], mt = sg[96 + j];
+                            const double2 e = sg[j], uw = sg[32 + j], mt = sg[96 + j];
                             const int thj = __double2hiint(mt.y);
                             double s_rev0 = 0.0, s_rev1 = 0.0;
 #pragma unroll
                             for (int i = 0; i < FREE_NT; ++i) {
                                 const double dr = e.x - ter[i], di = e.y - tei[i];
                                 const double den = fma(dr, dr, di * di);
-                                double val = fma(tei[i], pq.x, rb.x);
-                                val = fma(-ter[i], pq.y, val);
-                                val = fma(-tm[i], rb.y, val);
+                                const double val = fma(uw.y, di, uw.x * dr);
                                 const double r = bie_rcp3(den);
                                 const int dh = __double2hiint(den);
                                 if (!(dh < thi[i])) acc[i] = fma(val, r, acc[i]);
-                                // reverse entry A[s][t] x_t: row s (E_s, M_s), source t (its tables for the class of s)
-                                double vr = fma(e.y, tp[i], tr[i]);
-                                vr = fma(-e.x, tq[i], vr);
-                                vr = fma(-mt.x, tb[i], vr);
+                                // reverse entry A[s][t] x_t: row s, source t (its (U, W) for the class of s), E_t - E_s = -(dr + i di);
+                                // the sign is applied once to the sum
+                                const double vr = fma(tw[i], di, tu[i] * dr);
                                 if (!(dh < thj)) { if (i & 1) s_rev1 = fma(vr, r, s_rev1); else s_rev0 = fma(vr, r, s_rev0); }
                             }
-                            col[u * SYM_COL_STRIDE + lane] = s_rev0 + s_rev1;
+                            col[u * SYM_COL_STRIDE + lane] = -(s_rev0 + s_rev1);
                         }
                         // lane reduction of the 8 reverse sums through shared memory: lane l adds the slots 8 (l & 3) .. + 7 of
                         // source l >> 2, two shuffles finish (fixed order)

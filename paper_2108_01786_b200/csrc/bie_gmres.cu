@@ -3,17 +3,27 @@
 //
 // The paper ran the GEMV on the GPU and shipped every Krylov vector over PCIe to orthogonalise on the CPU
 // (PAPER.md:L857).  Here nothing leaves the device: one CTA per SM owns a contiguous block R of rows of A and,
-// with it, the same rows of every Krylov vector.  Per Arnoldi step
-//     w[R]  = A[R,:] v_j                     (bie_cta_gemv, HBM-bound; or the matrix-free pair loops of bie_free.cuh,
-//                                             FP64-bound, + one grid barrier; or both at once: hybrid operator)
-//     h    += V_j^T w ; w -= V_j h           twice (CGS2): local dots over R, one grid barrier, fixed-order sum
-//     h_{j+1,j} = ||w||                      local sum of squares, one grid barrier
-// i.e. three grid barriers per step.  v_{j+1} is never broadcast normalised: the unnormalised w goes to a
-// global buffer before the norm barrier and every CTA scales it by 1/h_{j+1,j} while loading it into shared
-// memory for the next GEMV.  Every CTA reduces the per-CTA partials in the same fixed order, so all CTAs hold
-// bit-identical h, Givens rotations and residuals and take the same branch without further communication.
-// The Givens/least-squares part (a8) is a few hundred flops done redundantly by thread 0 of every CTA; CTA 0
-// keeps R and does the back-substitution (a9) at the end of a cycle.
+// with it, the same rows of every Krylov vector.  Arnoldi step j, with TWO grid barriers (three for the matrix-free
+// and hybrid operators, whose partial sums cross CTAs):
+//     y[R]  = A[R,:] u / hn'                 u = the vector the previous step left in `wbuf` (see below), hn' its norm;
+//                                            bie_cta_gemv (HBM-bound), or the pair loops of bie_free.cuh (FP64-bound,
+//                                            + one grid barrier), or both at once (hybrid operator)
+//     s     = V_j^T y                        local dots over R, GRID BARRIER 1, fixed-order sum
+//     w1    = y - V_j s                      first classical Gram-Schmidt pass;  w1[R] -> wbuf
+//     h2    = V_j^T w1,  nu = ||w1||^2       local dots over R, GRID BARRIER 2, fixed-order sum
+//     v_{j+1} = (w1 - V_j h2) / hn,  hn^2 = nu - ||h2||^2      second pass (CGS2); h = s - c/hn' + h2
+// Two things keep this at two barriers.  (i) The norm of the twice-orthogonalised vector comes from Pythagoras,
+// ||w1 - V h2||^2 = ||w1||^2 - ||h2||^2, in the SAME reduction as h2; h2 is a rounding-level correction, so nothing
+// cancels (guard: if ||h2||^2 > 0.01 nu the step falls back to an explicit norm with one more barrier).  (ii) The next
+// operator application does not wait for v_{j+1} to be exchanged: it is applied to u = w1, whose rows went to `wbuf`
+// BEFORE barrier 2, and A v_{j+1} = (A w1 - A V_j h2)/hn = (A w1 - V_{j+1} c)/hn with c = Hbar_j h2 by the Arnoldi
+// relation A V_j = V_{j+1} Hbar_j.  The term V_{j+1} c lies in the span of the basis, so the Gram-Schmidt pass removes
+// it from the vector exactly as it would have; only the coefficients see it:  h_{.,j+1} = (V^T y)/hn - c/hn + h2.
+// c is a rounding-level quantity (h2 ~ eps ||w||) times Hbar, so a single-precision copy of Hbar (packed, in shared
+// memory) is ample.  Every CTA reduces the per-CTA partials in the same fixed order, so all CTAs hold bit-identical
+// h, Givens rotations and residuals and take the same branch without further communication.  The Givens /
+// least-squares part (a8) is a few hundred flops done redundantly by thread 0 of every CTA; CTA 0 keeps R and does
+// the back-substitution (a9) at the end of a cycle.  The grid-barrier counter lives in the caller's workspace.
 #include <cstring>
 #include "bie_common.cuh"
 #include "bie_gemv.cuh"
@@ -83,10 +93,10 @@ __device__ __forceinline__ double warp_sum_partials(const double* p, int G)
     return bie_warp_sum(s);
 }
 
-#ifdef BIE_PHASE_TIMING
+#ifdef BIE_PHASE_TIMING   // developer build (BIE_NVCC_EXTRA=-DBIE_PHASE_TIMING): CTA 0 prints the mean time per Arnoldi step of each phase
 #include <cstdio>
 __device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#define PT_DECL unsigned long long pt_t0 = gtime(), pt_acc[8] = {0,0,0,0,0,0,0,0};
+#define PT_DECL unsigned long long pt_t0 = gtime(), pt_acc[6] = {0, 0, 0, 0, 0, 0};
 #define PT(i) { const unsigned long long pt_t1 = gtime(); pt_acc[i] += pt_t1 - pt_t0; pt_t0 = pt_t1; }
 #else
 #define PT_DECL
@@ -99,29 +109,21 @@ __device__ __forceinline__ unsigned long long gtime() { unsigned long long t; as
 template <bool STREAM, bool XS, int MODE>
 __device__ __forceinline__ void cta_apply(const GmresArgs& a, int r0, int r1, const double* xin, double scale,
                                           double* xs, double* gpart, double* gpart2, double* ydense, double* y_local,
-                                          bool tables_ready, unsigned int& target)
+                                          bool tables_ready, double* red, unsigned int& target)
 {
     if (MODE != 0) {
         // xin is complete in global memory; its per-source tables either were written by the row owners before
         // the last grid barrier (tables_ready) or are written here
         if (!tables_ready) {
-            free_write_tables(a.nt, a.ct, a.fp, r0, r1, xin + r0);
+            free_write_tables(a.nt, a.ct, a.fp, r0, r1, xin + r0, red);
             grid_barrier(a.sync, target);
         }
         if (MODE == 1) {
             free_parts(a.nt, a.ct, a.fp, gpart, cta_team());
         } else {
             const int warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
-#ifdef BIE_PHASE_TIMING
-            __shared__ unsigned long long hy_acc[3];
-            if (threadIdx.x == 0 && target <= 2 * gridDim.x) { hy_acc[0] = hy_acc[1] = hy_acc[2] = 0; }
-            const unsigned long long hy_t0 = gtime();
-#endif
             if (warp < a.nwf) {
                 free_parts(a.nt, a.ct, a.fp, gpart, sub_team(0, a.nwf, 1));
-#ifdef BIE_PHASE_TIMING
-                if (threadIdx.x == 0) hy_acc[0] += gtime() - hy_t0;
-#endif
             } else {
                 const Team st = sub_team(a.nwf, nwarp - a.nwf, 2);
                 const int nd2 = a.nd >> 1;   // nd is even
@@ -129,18 +131,8 @@ __device__ __forceinline__ void cta_apply(const GmresArgs& a, int r0, int r1, co
                     reinterpret_cast<double2*>(xs)[i] = __ldcg(reinterpret_cast<const double2*>(xin) + i);
                 team_sync(st);
                 bie_cta_gemv<STREAM, true, HYB_GEMV_UNROLL>(a.A, a.lda, a.nd, r0, r1, a.chunk, xs, gpart2, ydense, st);
-#ifdef BIE_PHASE_TIMING
-                if (st.tid == 0) hy_acc[1] += gtime() - hy_t0;
-#endif
             }
             __syncthreads();
-#ifdef BIE_PHASE_TIMING
-            if (threadIdx.x == 0) {
-                hy_acc[2] += 1;
-                if (hy_acc[2] == 40 && (blockIdx.x == 0 || blockIdx.x == 100))
-                    printf("cta %d hybrid us/apply: pair loops %.1f, slab stream %.1f\n", blockIdx.x, hy_acc[0] * 1e-3 / 40, hy_acc[1] * 1e-3 / 40);
-            }
-#endif
         }
         grid_barrier(a.sync, target);
         free_gather(a.nt, a.ct, a.fp, r0, r1, xin, scale, gpart, y_local);
@@ -213,16 +205,18 @@ __device__ __forceinline__ void basis_combine(const Basis& B, int rows, int cnt,
     }
 }
 
-// one classical Gram-Schmidt pass against v_0..v_j: hloc[i] (+)= <v_i, w>, w -= sum_i <v_i, w> v_i
-__device__ __forceinline__ void cgs_pass(const GmresArgs& a, const Basis& B, int rows, int j, double* part_slot,
-                                         double* w_local, double* hloc, double* hacc, bool accumulate, double* red2,
-                                         unsigned int& target)
+// part_slot[i][cta] = <v_i, w>_R for i < cnt (this CTA's rows R); with_norm: part_slot[cnt][cta] = ||w||_R^2
+__device__ __forceinline__ void local_dots(const Basis& B, int rows, int cnt, const double* w_local, double* part_slot,
+                                           bool with_norm)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
     const int G = gridDim.x;
-    for (int i = warp; i <= j; i += nwarp) {
+    const int tot = cnt + (with_norm ? 1 : 0);
+    for (int i = warp; i < tot; i += nwarp) {
         double s = 0.0;
-        if (i < B.VS) {
+        if (i == cnt) {
+            for (int r = lane; r < rows; r += 32) s = fma(w_local[r], w_local[r], s);
+        } else if (i < B.VS) {
             const double* vi = B.Vs + (size_t)i * B.rows2;
             for (int r = lane; r < rows; r += 32) s = fma(vi[r], w_local[r], s);
         } else {
@@ -232,31 +226,43 @@ __device__ __forceinline__ void cgs_pass(const GmresArgs& a, const Basis& B, int
         s = bie_warp_sum(s);
         if (lane == 0) part_slot[(size_t)i * G + blockIdx.x] = s;
     }
-    grid_barrier(a.sync, target);
-    // fixed-order sums of the G per-CTA partials; the loads of up to four vectors are in flight together
-    for (int i0 = warp; i0 <= j; i0 += 4 * nwarp) {
+}
+
+// out[i] = sum over the G per-CTA partials of row i < cnt, same order in every CTA; the loads of up to four rows are
+// in flight together.  Ends with __syncthreads.
+__device__ __forceinline__ void reduce_partials(const double* part_slot, int cnt, double* out)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    const int G = gridDim.x;
+    for (int i0 = warp; i0 < cnt; i0 += 4 * nwarp) {
         double s[4];
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
             const int i = i0 + q * nwarp;
             s[q] = 0.0;
-            if (i <= j)
+            if (i < cnt)
                 for (int c = lane; c < G; c += 32) s[q] += __ldcg(part_slot + (size_t)i * G + c);
         }
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
             const int i = i0 + q * nwarp;
             const double h = bie_warp_sum(s[q]);
-            if (i <= j && lane == 0) {
-                hloc[i] = h;
-                hacc[i] = accumulate ? hacc[i] + h : h;
-            }
+            if (i < cnt && lane == 0) out[i] = h;
         }
     }
     __syncthreads();
-    basis_combine(B, rows, j + 1, hloc, red2);
-    for (int r = threadIdx.x; r < rows; r += blockDim.x) w_local[r] -= red2[r];
-    __syncthreads();
+}
+
+// offset of column i of the packed upper-Hessenberg matrix (column i holds rows 0 .. i+1)
+__device__ __forceinline__ int hess_off(int i) { return (i * (i + 3)) >> 1; }
+
+// doubles of shared memory before the operator's scratch: y, w [rows2 each], hcol, hloc, cvec [m + 2 each], cs, sn [m each],
+// g [m + 1], red [66], the packed single-precision Hbar [m (m + 3) / 2 floats]; rounded to 16 bytes
+__host__ __device__ inline int gm_head_doubles(int m, int rows2)
+{
+    int o = 2 * rows2 + 3 * (m + 2) + 2 * m + (m + 1) + 66;
+    o += (m * (m + 3) / 2 + 1) / 2;
+    return (o + 1) & ~1;
 }
 
 template <bool STREAM, bool XS, int MODE>
@@ -273,13 +279,15 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
     // shared layout
     double* y_local = smem;               // [rows2]   result of the operator
     double* w_local = y_local + rows2;    // [rows2]   the vector being orthogonalised
-    double* hcol = w_local + rows2;       // [m+2]     column j of H (accumulated h)
+    double* hcol = w_local + rows2;       // [m+2]     column j of H
     double* hloc = hcol + (m + 2);        // [m+2]     coefficients of the current pass
-    double* cs = hloc + (m + 2);          // [m]
+    double* cvec = hloc + (m + 2);        // [m+2]     c = Hbar h2 of the previous step (see the header)
+    double* cs = cvec + (m + 2);          // [m]
     double* sn = cs + m;                  // [m]
     double* g = sn + m;                   // [m+1]
-    double* red = g + (m + 1);            // [34]
-    double* gpart = red + 34 + ((m & 1) ? 0 : 1);  // GEMV partials or matrix-free scratch (16-byte aligned)
+    double* red = g + (m + 1);            // [66]
+    float* Hf = reinterpret_cast<float*>(red + 66);                  // packed Hbar in single precision, m (m + 3) / 2 floats
+    double* gpart = smem + gm_head_doubles(m, rows2);                // GEMV partials or matrix-free scratch (16-byte aligned)
     // hybrid: GEMV partials of the slab and its result, after the matrix-free scratch
     double* gpart2 = gpart + (FREE ? a.scratch_doubles : 0);
     double* ydense = gpart2 + ((MODE == 1) ? 0 : ((gemv_part_doubles(a.rows_per_cta, MODE == 2 ? a.nd : n, a.chunk) + 1) & ~1));
@@ -316,7 +324,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
             for (int r = threadIdx.x; r < rows; r += blockDim.x) w_local[r] = a.b[r0 + r];
             first = false;
         } else {
-            cta_apply<STREAM, XS, MODE>(a, r0, r1, a.x, 1.0, xs, gpart, gpart2, ydense, y_local, false, target);
+            cta_apply<STREAM, XS, MODE>(a, r0, r1, a.x, 1.0, xs, gpart, gpart2, ydense, y_local, false, red, target);
             for (int r = threadIdx.x; r < rows; r += blockDim.x) w_local[r] = a.b[r0 + r] - y_local[r];
         }
         __syncthreads();
@@ -326,18 +334,19 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
             p = fma(v, v, p);
             a.wbuf[r0 + r] = v;
         }
-        if (FREE) free_write_tables(a.nt, a.ct, a.fp, r0, r1, w_local);
+        if (FREE) free_write_tables(a.nt, a.ct, a.fp, r0, r1, w_local, red);
         p = block_sum(p, red);
         if (threadIdx.x == 0) part3[blockIdx.x] = p;
         grid_barrier(a.sync, target);
         const double beta = sqrt(warp_sum_partials(part3, G));
         if (beta <= thresh) break;                         // converged (status 0)
         if (iters >= a.max_iters) { status = BIE_MAX_ITERS; break; }
-        double inv = 1.0 / beta;
+        double inv = 1.0 / beta;                           // 1 / norm of the vector in wbuf
         {
             double* v0 = (0 < B.VS) ? B.Vs : B.Vg;
             for (int r = threadIdx.x; r < rows; r += blockDim.x) v0[r] = w_local[r] * inv;
         }
+        for (int i = threadIdx.x; i < m + 2; i += blockDim.x) cvec[i] = 0.0;   // wbuf holds beta v_0 itself: no correction
         if (threadIdx.x == 0) g[0] = beta;
         __syncthreads();
 
@@ -346,45 +355,83 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
         bool conv = false;
         PT_DECL
         for (int j = 0; j < m; ++j) {
-            PT(7)
-            // a6: w = A v_j, with v_j = wbuf * inv
-#ifdef BIE_PHASE_TIMING
-            if (MODE == 1) {
-                free_parts(a.nt, a.ct, a.fp, gpart, cta_team());
-                PT(0)
-                grid_barrier(a.sync, target);
-                PT(1)
-                free_gather(a.nt, a.ct, a.fp, r0, r1, a.wbuf, inv, gpart, y_local);
-                PT(2)
-            } else
-#endif
-            cta_apply<STREAM, XS, MODE>(a, r0, r1, a.wbuf, inv, xs, gpart, gpart2, ydense, y_local, true, target);
-            for (int r = threadIdx.x; r < rows; r += blockDim.x) w_local[r] = y_local[r];
-            __syncthreads();
-            PT(3)
-            // a7: CGS2
-            cgs_pass(a, B, rows, j, part1, w_local, hloc, hcol, false, red2, target);
-            cgs_pass(a, B, rows, j, part2, w_local, hloc, hcol, true, red2, target);
-            PT(4)
-            p = 0.0;
-            for (int r = threadIdx.x; r < rows; r += blockDim.x) {
-                const double v = w_local[r];
-                p = fma(v, v, p);
-                a.wbuf[r0 + r] = v;
-            }
-            if (FREE) free_write_tables(a.nt, a.ct, a.fp, r0, r1, w_local);
-            p = block_sum(p, red);
-            if (threadIdx.x == 0) part3[blockIdx.x] = p;
-            grid_barrier(a.sync, target);
-            const double hn = sqrt(warp_sum_partials(part3, G));
             PT(5)
+            // a6: y = A (wbuf * inv) = A v_j + V_j c * inv  (c = 0 in the first step of a cycle)
+            cta_apply<STREAM, XS, MODE>(a, r0, r1, a.wbuf, inv, xs, gpart, gpart2, ydense, y_local, true, red, target);
+            PT(0)
+            // a7, first pass: s = V_j^T y (grid barrier 1), w1 = y - V_j s, h1 = s - c * inv
+            local_dots(B, rows, j + 1, y_local, part1, false);
+            grid_barrier(a.sync, target);
+            PT(1)
+            reduce_partials(part1, j + 1, hloc);
+            for (int i = threadIdx.x; i <= j; i += blockDim.x) hcol[i] = fma(-cvec[i], inv, hloc[i]);
+            basis_combine(B, rows, j + 1, hloc, red2);
+            for (int r = threadIdx.x; r < rows; r += blockDim.x) {
+                const double v = y_local[r] - red2[r];
+                w_local[r] = v;
+                a.wbuf[r0 + r] = v;                       // the next operator application reads w1 (see the header)
+            }
+            __syncthreads();
+            if (FREE) free_write_tables(a.nt, a.ct, a.fp, r0, r1, w_local, red);
+            // second pass: h2 = V_j^T w1 and ||w1||^2 in ONE reduction (grid barrier 2)
+            local_dots(B, rows, j + 1, w_local, part2, true);
+            PT(2)
+            grid_barrier(a.sync, target);
+            PT(3)
+            reduce_partials(part2, j + 2, hloc);          // hloc[0..j] = h2, hloc[j+1] = ||w1||^2
+            if (threadIdx.x < 32) {                        // ||h2||^2, fixed order
+                double ss = 0.0;
+                for (int i = threadIdx.x; i <= j; i += 32) ss = fma(hloc[i], hloc[i], ss);
+                ss = bie_warp_sum(ss);
+                if (threadIdx.x == 0) red[64] = ss;
+            }
+            __syncthreads();
+            const double nu = hloc[j + 1], ss = red[64];
+            double hn;
+            const bool pyth = (ss <= 0.01 * nu);           // identical in every CTA (same bits)
+            basis_combine(B, rows, j + 1, hloc, red2);     // V_j h2 on this CTA's rows
+            if (pyth) {
+                hn = sqrt(nu - ss);                        // ||w1 - V h2||^2 = ||w1||^2 - ||h2||^2, no cancellation: ss << nu
+            } else {
+                // w1 is NOT nearly orthogonal to the basis (breakdown region): explicit norm of w2 = w1 - V h2, and the
+                // next operator application reads w2 (one more grid barrier; c = 0)
+                p = 0.0;
+                for (int r = threadIdx.x; r < rows; r += blockDim.x) {
+                    const double v = w_local[r] - red2[r];
+                    w_local[r] = v; red2[r] = 0.0;
+                    p = fma(v, v, p);
+                    a.wbuf[r0 + r] = v;
+                }
+                __syncthreads();
+                if (FREE) free_write_tables(a.nt, a.ct, a.fp, r0, r1, w_local, red);
+                p = block_sum(p, red);
+                if (threadIdx.x == 0) part3[blockIdx.x] = p;
+                grid_barrier(a.sync, target);
+                hn = sqrt(warp_sum_partials(part3, G));
+            }
             inv = (hn != 0.0) ? 1.0 / hn : 0.0;
             {
                 double* vn = (j + 1 < B.VS) ? B.Vs + (size_t)(j + 1) * rows2 : B.Vg + (size_t)(j + 1) * a.nld;
-                for (int r = threadIdx.x; r < rows; r += blockDim.x) vn[r] = w_local[r] * inv;
+                for (int r = threadIdx.x; r < rows; r += blockDim.x) vn[r] = (w_local[r] - red2[r]) * inv;
+            }
+            for (int i = threadIdx.x; i <= j; i += blockDim.x) hcol[i] += hloc[i];
+            __syncthreads();
+            // column j of Hbar (single precision copy), then c = Hbar_j h2 for the next step
+            for (int i = threadIdx.x; i <= j + 1; i += blockDim.x) Hf[hess_off(j) + i] = (float)(i <= j ? hcol[i] : hn);
+            __syncthreads();
+            for (int t0 = 0; t0 < 4 * (j + 2); t0 += blockDim.x) {   // four threads per entry of c; whole warps take part
+                const int t = t0 + threadIdx.x;
+                if ((t & ~31) >= 4 * (j + 2)) continue;              // warp-uniform
+                const int kk = t >> 2, q = t & 3;
+                double c = 0.0;
+                if (pyth && kk <= j + 1)
+                    for (int i = max(kk - 1, 0) + q; i <= j; i += 4) c = fma((double)Hf[hess_off(i) + kk], hloc[i], c);
+                c += __shfl_xor_sync(0xffffffffu, c, 1);
+                c += __shfl_xor_sync(0xffffffffu, c, 2);
+                if (q == 0 && kk <= j + 1) cvec[kk] = c;
             }
             // a8: Givens rotations on column j, new rotation, recurrence residual
-            if (threadIdx.x == 0) {
+            if (threadIdx.x == GM_THREADS - 1) {
                 hcol[j + 1] = hn;
                 for (int i = 0; i < j; ++i) {
                     const double t0 = cs[i] * hcol[i] + sn[i] * hcol[i + 1];
@@ -409,14 +456,14 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
             conv = (fabs(g[j + 1]) <= thresh) || (hn == 0.0);
             if (hn == 0.0 && !(fabs(g[j + 1]) <= thresh)) status = 2;
             __syncthreads();
-            PT(6)
+            PT(4)
             if (conv || iters >= a.max_iters) break;
         }
 #ifdef BIE_PHASE_TIMING
-        if (threadIdx.x == 0 && (blockIdx.x == 0 || blockIdx.x == 77 || blockIdx.x == 147))
-            printf("cta %d k=%d us/iter: parts %.1f bar %.1f gather %.1f copy %.1f cgs2 %.1f norm %.1f givens %.1f\n", blockIdx.x, k,
-                   pt_acc[0] * 1e-3 / k, pt_acc[1] * 1e-3 / k, pt_acc[2] * 1e-3 / k, pt_acc[3] * 1e-3 / k, pt_acc[4] * 1e-3 / k,
-                   pt_acc[5] * 1e-3 / k, pt_acc[6] * 1e-3 / k);
+        if (threadIdx.x == 0 && blockIdx.x == 0)
+            printf("cycle of %d steps, us per step: operator %.1f | dots1 + barrier1 %.1f | reduce + w1 + tables + dots2 %.1f | barrier2 %.1f | "
+                   "tail %.1f | loop %.1f\n", k, pt_acc[0] * 1e-3 / k, pt_acc[1] * 1e-3 / k, pt_acc[2] * 1e-3 / k,
+                   pt_acc[3] * 1e-3 / k, pt_acc[4] * 1e-3 / k, pt_acc[5] * 1e-3 / k);
 #endif
         // ---- a9: y = R^{-1} g (CTA 0), x += V y ---------------------------------------------------
         if (blockIdx.x == 0) {
@@ -446,7 +493,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
     // ---- a10: outputs; true residual ||b - A x|| / ||b|| (reported only) -----------------------------
     double relres = 0.0;
     if (a.relres_out && bn != 0.0) {
-        cta_apply<STREAM, XS, MODE>(a, r0, r1, a.x, 1.0, xs, gpart, gpart2, ydense, y_local, false, target);
+        cta_apply<STREAM, XS, MODE>(a, r0, r1, a.x, 1.0, xs, gpart, gpart2, ydense, y_local, false, red, target);
         p = 0.0;
         for (int r = threadIdx.x; r < rows; r += blockDim.x) {
             const double v = a.b[r0 + r] - y_local[r];
@@ -473,8 +520,22 @@ struct GmresPlan {
     int G, rows_per_cta, chunk, nld, VS, scratch_doubles;
     bool xs, stream;
     size_t smem;
-    size_t offV, offW, offP, offR, offY, total;
+    size_t offV, offW, offP, offR, offY, offS, total;
 };
+
+// workspace layout: Krylov basis, wbuf, per-CTA partials, R, y, and the grid-barrier counter of the call
+static void gmres_ws_layout(int n, int m, int sm_bound, GmresPlan* pl)
+{
+    pl->nld = (n + 1) & ~1;
+    size_t o = 0;
+    pl->offV = o; o += al256(sizeof(double) * (size_t)(m + 1) * pl->nld);
+    pl->offW = o; o += al256(sizeof(double) * (size_t)pl->nld);
+    pl->offP = o; o += al256(sizeof(double) * 3 * (size_t)(m + 2) * sm_bound);
+    pl->offR = o; o += al256(sizeof(double) * (size_t)m * (m + 1));
+    pl->offY = o; o += al256(sizeof(double) * (size_t)m);
+    pl->offS = o; o += 256;
+    pl->total = o;
+}
 
 // mode: 0 stored matrix, 1 matrix-free, 2 hybrid (slab of nd columns streamed by 16 - nwf warps)
 static int gmres_plan(int n, int restart, int sm_count, int max_smem, int l2_bytes, long long lda, int mode, int nd,
@@ -486,10 +547,9 @@ static int gmres_plan(int n, int restart, int sm_count, int max_smem, int l2_byt
     pl->G = (n + pl->rows_per_cta - 1) / pl->rows_per_cta;
     pl->chunk = mode == 2 ? gemv_chunk(pl->rows_per_cta, nd, GM_THREADS / 32 - nwf)
                           : gemv_chunk(pl->rows_per_cta, n, GM_THREADS / 32);
-    pl->nld = (n + 1) & ~1;
     pl->scratch_doubles = free_op ? (sym_possible ? free_scratch_doubles(GM_THREADS) : free_scratch_doubles_onedir()) : 0;
     const int rows2 = (pl->rows_per_cta + 1) & ~1;
-    size_t base = 2 * (size_t)rows2 + 2 * (size_t)(m + 2) + 2 * (size_t)m + (size_t)(m + 1) + 34 + 1;
+    size_t base = (size_t)gm_head_doubles(m, rows2);
     if (free_op) base += (size_t)pl->scratch_doubles;
     if (mode != 1) base += (size_t)((gemv_part_doubles(pl->rows_per_cta, mode == 2 ? nd : n, pl->chunk) + 1) & ~1);
     if (mode == 2) base += (size_t)rows2 + (size_t)((nd + 2) & ~1);   // slab result, x of the slab's columns
@@ -506,38 +566,25 @@ static int gmres_plan(int n, int restart, int sm_count, int max_smem, int l2_byt
     if (pl->VS > m + 1) pl->VS = m + 1;
     pl->smem += sizeof(double) * (size_t)pl->VS * rows2;
     pl->stream = mode != 1 && (double)n * (double)(mode == 2 ? nd : lda) * 8.0 > 0.6 * (double)l2_bytes;
-    size_t o = 0;
-    pl->offV = o; o += al256(sizeof(double) * (size_t)(m + 1) * pl->nld);
-    pl->offW = o; o += al256(sizeof(double) * (size_t)pl->nld);
-    pl->offP = o; o += al256(sizeof(double) * 3 * (size_t)(m + 2) * sm_count);
-    pl->offR = o; o += al256(sizeof(double) * (size_t)m * (m + 1));
-    pl->offY = o; o += al256(sizeof(double) * (size_t)m);
-    pl->total = o;
+    gmres_ws_layout(n, m, sm_count, pl);
     return BIE_OK;
 }
 
 size_t bie_gmres_ws_bytes(int n, int restart)
 {
     if (n < 1 || restart < 1) return 0;
+    if (restart > n) restart = n;
     GmresPlan pl;
-    // the workspace layout does not depend on the operator or on the device beyond the SM count bound
-    const int m = restart;
-    const int nld = (n + 1) & ~1;
-    size_t o = 0;
-    o += al256(sizeof(double) * (size_t)(m + 1) * nld);
-    o += al256(sizeof(double) * (size_t)nld);
-    o += al256(sizeof(double) * 3 * (size_t)(m + 2) * 256);  // <= 256 SMs
-    o += al256(sizeof(double) * (size_t)m * (m + 1));
-    o += al256(sizeof(double) * (size_t)m);
-    (void)pl;
-    return o + 256;
+    gmres_ws_layout(n, restart, 256, &pl);   // the layout depends on the device only through the SM count (<= 256)
+    return pl.total + 256;                   // + alignment slack
 }
 
 template <bool STREAM, bool XS, int MODE>
-static int launch_gmres(const GmresArgs& a, const GmresPlan& pl, cudaStream_t st)
+static int launch_gmres(bie_ctx* ctx, const GmresArgs& a, const GmresPlan& pl, cudaStream_t st)
 {
     auto k = bie_gmres_kernel<STREAM, XS, MODE>;
-    BIE_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+    const int rc = bie_grant_smem(ctx, (MODE == 0 ? (STREAM ? 2 : 0) + (XS ? 1 : 0) : (MODE == 1 ? 4 : 5 + (STREAM ? 1 : 0))), k, pl.smem);
+    if (rc != BIE_OK) return rc;
     void* params[] = {(void*)&a};
     BIE_CUDA(cudaLaunchCooperativeKernel((const void*)k, dim3(pl.G), dim3(GM_THREADS), params, pl.smem, st));
     return BIE_OK;
@@ -576,7 +623,7 @@ int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, int nd, 
     a.part = (double*)(base + pl.offP);
     a.R = (double*)(base + pl.offR);
     a.yv = (double*)(base + pl.offY);
-    a.sync = ctx->sync_buf;
+    a.sync = (unsigned int*)(base + pl.offS);     // per call: two solves of one ctx never share a barrier counter
     a.nld = pl.nld; a.rows_per_cta = pl.rows_per_cta; a.chunk = pl.chunk; a.VS = pl.VS;
     a.nd = nd; a.nwf = nwf; a.scratch_doubles = pl.scratch_doubles;
     a.res_pairs = (mode == 0 && pl.stream)
@@ -589,9 +636,9 @@ int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, int nd, 
         rc = bie_free_plan(ctx, pl.G, nd, &a.fp, st);
         if (rc != BIE_OK) return rc;
     }
-    BIE_CUDA(cudaMemsetAsync(ctx->sync_buf, 0, sizeof(unsigned int), st));
-    if (mode == 1) return launch_gmres<false, false, 1>(a, pl, st);
-    if (mode == 2) return pl.stream ? launch_gmres<true, true, 2>(a, pl, st) : launch_gmres<false, true, 2>(a, pl, st);
-    if (pl.stream) return pl.xs ? launch_gmres<true, true, 0>(a, pl, st) : launch_gmres<true, false, 0>(a, pl, st);
-    return pl.xs ? launch_gmres<false, true, 0>(a, pl, st) : launch_gmres<false, false, 0>(a, pl, st);
+    BIE_CUDA(cudaMemsetAsync(a.sync, 0, sizeof(unsigned int), st));
+    if (mode == 1) return launch_gmres<false, false, 1>(ctx, a, pl, st);
+    if (mode == 2) return pl.stream ? launch_gmres<true, true, 2>(ctx, a, pl, st) : launch_gmres<false, true, 2>(ctx, a, pl, st);
+    if (pl.stream) return pl.xs ? launch_gmres<true, true, 0>(ctx, a, pl, st) : launch_gmres<true, false, 0>(ctx, a, pl, st);
+    return pl.xs ? launch_gmres<false, true, 0>(ctx, a, pl, st) : launch_gmres<false, false, 0>(ctx, a, pl, st);
 }

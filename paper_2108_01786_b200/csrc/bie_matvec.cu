@@ -35,11 +35,11 @@ static int launch_mv(bie_ctx* ctx, int nrows, int n, const double* A, int64_t ld
                      int rows_per_cta, int chunk, int res_pairs, size_t smem, cudaStream_t st)
 {
     auto k = bie_matvec_kernel<STREAM, XS>;
-    BIE_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int rc = bie_grant_smem(ctx, 8 + (STREAM ? 2 : 0) + (XS ? 1 : 0), k, smem);
+    if (rc != BIE_OK) return rc;
     const int grid = (nrows + rows_per_cta - 1) / rows_per_cta;
     k<<<grid, MV_THREADS, smem, st>>>(A, (long long)lda, nrows, n, rows_per_cta, chunk, res_pairs, x, y);
     BIE_CUDA(cudaGetLastError());
-    (void)ctx;
     return BIE_OK;
 }
 
@@ -81,7 +81,7 @@ bie_matvec_free_kernel(NodeTable nt, CompTable ct, FreePlan fp, int rows_per_cta
     double* scratch = smem;
     double* y_local = scratch + free_scratch_doubles(FREE_THREADS);
     unsigned int target = 0;
-    free_write_tables(nt, ct, fp, r0, r1, x + r0);
+    free_write_tables(nt, ct, fp, r0, r1, x + r0, scratch);
     grid_barrier(sync, target);
     free_parts(nt, ct, fp, scratch, cta_team());
     grid_barrier(sync, target);
@@ -105,12 +105,15 @@ int bie_launch_matvec_free(bie_ctx* ctx, const double* x, double* y, cudaStream_
     if (rc != BIE_OK) return rc;
     rc = bie_free_plan(ctx, G, 0, &fp, st);
     if (rc != BIE_OK) return rc;
-    BIE_CUDA(cudaFuncSetAttribute(bie_matvec_free_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    BIE_CUDA(cudaMemsetAsync(ctx->sync_buf, 0, sizeof(unsigned int), st));
+    rc = bie_grant_smem(ctx, 12, bie_matvec_free_kernel, smem);
+    if (rc != BIE_OK) return rc;
+    // the grid-barrier counter of THIS launch: the ctx cycles through BIE_SYNC_SLOTS counters, so that a later launch
+    // never resets a counter an earlier one may still be spinning on (a ctx serves one stream at a time, include/bie.h)
+    unsigned int* sync = ctx->sync_buf + 64 * (ctx->sync_next++ % BIE_SYNC_SLOTS);
+    BIE_CUDA(cudaMemsetAsync(sync, 0, sizeof(unsigned int), st));
     NodeTable nt = bie_node_table(ctx);
     CompTable ct = ctx->comps;
     int rpc = rows_per_cta;
-    unsigned int* sync = ctx->sync_buf;
     void* params[] = {(void*)&nt, (void*)&ct, (void*)&fp, (void*)&rpc, (void*)&x, (void*)&y, (void*)&sync};
     BIE_CUDA(cudaLaunchCooperativeKernel((const void*)bie_matvec_free_kernel, dim3(G), dim3(FREE_THREADS), params, smem, st));
     return BIE_OK;

@@ -6,12 +6,14 @@
 // series of bie_cot_half_near is exact to rounding).  The pair loop of the operator leaves near pairs out by
 // predication; their exact matrix entries -- Laurent series of cot for s != t, the analytic diagonal limit
 // K_jj(a,a) = Im{zeta''/(2 zeta')} with the -+1/2 of Eq. (3.10) for s == t, both WITHOUT the
-// rank-one -E_k of PAPER.md:L324, which the operator applies through component sums -- are stored here as a
-// sparse matrix in CSR form (a handful of entries per row: the neighbours on the same curve and whatever
+// rank-one -E_k of PAPER.md:L324, which the operator applies through component sums, and (Eq. (3.16) variants) PLUS the
+// constant beta_s of the difference form, which the operator subtracts for ALL sources at once (bie_free.cuh) -- are
+// stored here as a sparse matrix in CSR form (a handful of entries per row: the neighbours on the same curve and whatever
 // other curve comes closer than sqrt(taubar)), and added as  y_t += sum_k val[k] x[col[k]]  when the operator
 // gathers its partial sums.  Classification uses exactly the expression of the pair loop, so both agree bit
 // for bit.  Three launches per geometry: count, exclusive scan, fill (the first and last scan all n^2 pairs
-// with 4 FP64 instructions each).
+// with 4 FP64 instructions each).  The arrays are sized from the scanned total (the host reads it back once per
+// geometry and grows them on demand), so there is no capacity limit.
 #include "bie_common.cuh"
 
 #define NEAR_THREADS 128
@@ -21,7 +23,7 @@
 template <bool FILL>
 __global__ void __launch_bounds__(NEAR_THREADS)
 bie_near_kernel(NodeTable nt, CompTable ct, int vortex, const double* __restrict__ taubar, int* __restrict__ cnt /* [n][NEAR_SEG] counts or offsets */,
-                int* __restrict__ col, double* __restrict__ val, int cap, int* __restrict__ overflow)
+                int* __restrict__ col, double* __restrict__ val, int cap)
 {
     __shared__ double2 sE[NEAR_TILE];
     const int n = nt.n;
@@ -50,37 +52,36 @@ bie_near_kernel(NodeTable nt, CompTable ct, int vortex, const double* __restrict
                 if (FILL && t < n) {
                     const int s = s0 + j;
                     const int p = base + k;
-                    if (p < cap) {
+                    if (p < cap) {   // always true: cap >= the scanned total
+                        const double2 q = nt.Q[s];
+                        const int jc = nt.COMP[s];
+                        const bool src0 = (jc == 0);
+                        double al, be;
+                        if (src0 == tgt0) { al = -2.0 * q.y; be = q.x; }        // Im c     block coefficients of Eq. (3.10)
+                        else if (tgt0)    { al = -2.0 * q.x; be = -q.y; }       // Re c   (G_0j)
+                        else              { al = 2.0 * q.x;  be = q.y; }        // -Re c  (-G_k0)
                         double v;
                         if (s == t) {
                             const double2 dg = nt.DG[t];
                             v = dg.x + dg.y;   // complete diagonal entry without its -E_k part
                         } else {
-                            const double2 zs = nt.XY[s], zt = nt.XY[t], q = nt.Q[s];
+                            const double2 zs = nt.XY[s], zt = nt.XY[t];
                             double cr, ci;
                             bie_cot_half_near(zs.x - zt.x, zs.y - zt.y, &cr, &ci);
-                            const int j = nt.COMP[s];
-                            const bool src0 = (j == 0);
-                            double al, be;
                             if (vortex) {   // S of Eqs. (4.14) + (4.17): weight zeta'_t/2 of the ROW, 1/M_j of the column
-                                const int k = nt.COMP[t];
+                                const int kc = nt.COMP[t];
                                 const double2 qt = nt.Q[t];
-                                const double Mk = (double)(ct.off[k + 1] - ct.off[k]), ms = 1.0 / (double)(ct.off[j + 1] - ct.off[j]);
+                                const double Mk = (double)(ct.off[kc + 1] - ct.off[kc]), ms = 1.0 / (double)(ct.off[jc + 1] - ct.off[jc]);
                                 const double ur = qt.x * Mk * ms, ui = qt.y * Mk * ms;
                                 if (src0 == tgt0) { al = 2.0 * ui;  be = -ur; }      // Im c+
                                 else if (tgt0)    { al = -2.0 * ur; be = -ui; }      // -Re c+ (-G+_j0)
                                 else              { al = 2.0 * ur;  be = ui; }       // Re c+  (G+_0k)
-                            } else {        // block coefficients of Eq. (3.10) (bie_common.cuh)
-                                if (src0 == tgt0) { al = -2.0 * q.y; be = q.x; }        // Im c
-                                else if (tgt0)    { al = -2.0 * q.x; be = -q.y; }       // Re c   (G_0j)
-                                else              { al = 2.0 * q.x;  be = q.y; }        // -Re c  (-G_k0)
                             }
                             v = fma(be, ci, -0.5 * al * cr);   // cot = (-2X + iY)/den
                         }
+                        if (!vortex) v += be;   // the operator subtracts sum_s beta_s x_s over ALL sources (difference form)
                         col[p] = s;
                         val[p] = v;
-                    } else {
-                        *overflow = 1;
                     }
                 }
                 ++k;
@@ -126,24 +127,35 @@ __global__ void __launch_bounds__(1024) bie_near_scan_kernel(int* __restrict__ a
     if (threadIdx.x == 1023) a[N] = sums[1023];
 }
 
-size_t bie_near_cap(int npad) { return (size_t)BIE_NEAR_PER_NODE * (size_t)npad; }
-
 // builds the CSR near matrix of the ctx's current geometry if it is not there yet (lazy: the dense path never
-// needs it)
+// needs it).  SYNCHRONISES the stream once per geometry: the total number of near pairs comes back to the host and
+// near_col / near_val grow to it when needed.
 int bie_ensure_near(bie_ctx* ctx, cudaStream_t st)
 {
     if (!ctx->have_geom) return BIE_ERR_GEOMETRY;
     if (ctx->near_valid) return BIE_OK;
     const NodeTable nt = bie_node_table(ctx);
     const int n = ctx->n;
-    const int cap = (int)bie_near_cap(nt.npad);
     const int vx = (ctx->variant == BIE_VARIANT_VORTEX) ? 1 : 0;
     dim3 grid((n + NEAR_THREADS - 1) / NEAR_THREADS, NEAR_SEG);
-    BIE_CUDA(cudaMemsetAsync(ctx->near_overflow, 0, sizeof(int), st));
-    bie_near_kernel<false><<<grid, NEAR_THREADS, 0, st>>>(nt, ctx->comps, vx, ctx->taubar, ctx->near_ptr, nullptr, nullptr, cap, ctx->near_overflow);
+    bie_near_kernel<false><<<grid, NEAR_THREADS, 0, st>>>(nt, ctx->comps, vx, ctx->taubar, ctx->near_ptr, nullptr, nullptr, 0);
     bie_near_scan_kernel<<<1, 1024, 0, st>>>(ctx->near_ptr, n * NEAR_SEG);
-    bie_near_kernel<true><<<grid, NEAR_THREADS, 0, st>>>(nt, ctx->comps, vx, ctx->taubar, ctx->near_ptr, ctx->near_col, ctx->near_val, cap,
-                                                        ctx->near_overflow);
+    BIE_CUDA(cudaGetLastError());
+    BIE_CUDA(cudaMemcpyAsync(ctx->pinned_i + 2, ctx->near_ptr + (size_t)n * NEAR_SEG, sizeof(int), cudaMemcpyDeviceToHost, st));
+    BIE_CUDA(cudaStreamSynchronize(st));
+    const size_t total = (size_t)ctx->pinned_i[2];
+    if (total > ctx->near_cap) {
+        if (ctx->near_col) cudaFree(ctx->near_col);
+        if (ctx->near_val) cudaFree(ctx->near_val);
+        ctx->near_col = nullptr; ctx->near_val = nullptr; ctx->near_cap = 0;
+        const size_t cap = total + total / 4 + 1024;
+        if (cap > (size_t)0x7fffffff) return BIE_ERR_GEOMETRY;
+        BIE_CUDA(cudaMalloc((void**)&ctx->near_col, sizeof(int) * cap));
+        BIE_CUDA(cudaMalloc((void**)&ctx->near_val, sizeof(double) * cap));
+        ctx->near_cap = cap;
+    }
+    bie_near_kernel<true><<<grid, NEAR_THREADS, 0, st>>>(nt, ctx->comps, vx, ctx->taubar, ctx->near_ptr, ctx->near_col, ctx->near_val,
+                                                        (int)ctx->near_cap);
     BIE_CUDA(cudaGetLastError());
     ctx->near_valid = 1;
     return BIE_OK;

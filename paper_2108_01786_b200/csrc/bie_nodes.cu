@@ -8,7 +8,6 @@
 // -1/M_m of E_m.
 #include "bie_common.cuh"
 #include <cstdlib>
-#include <vector>
 #include "bie_free.cuh"
 
 struct PrepArgs {
@@ -117,25 +116,29 @@ int bie_prepare_nodes(bie_ctx* ctx, int ncomp, const int32_t* counts, const int3
     if (nbottom > 1 || n > (1 << 30)) return BIE_ERR_GEOMETRY;
     if ((((uintptr_t)zeta) | ((uintptr_t)dzeta) | ((uintptr_t)d2zeta)) & 15u) return BIE_ERR_LAYOUT;
     const int npad = bie_npad((int)n);
+    ctx->geom_gen += 1;          // whatever was cached for the previous geometry (near matrix, symmetric work list) is stale
+    ctx->near_valid = 0;
     if (npad > ctx->cap) {
-        // grow the ctx's node storage (the only allocation outside bie_create; O(n) bytes)
+        // grow the ctx's node storage (O(n) bytes).  The ctx holds NO geometry until every allocation and the
+        // preparation launch below have succeeded.
+        ctx->have_geom = 0; ctx->n = 0;
         if (ctx->node_buf) cudaFree(ctx->node_buf);
         if (ctx->comp_buf) cudaFree(ctx->comp_buf);
         if (ctx->free_buf) cudaFree(ctx->free_buf);
         if (ctx->near_ptr) cudaFree(ctx->near_ptr);
-        if (ctx->near_col) cudaFree(ctx->near_col);
-        if (ctx->near_val) cudaFree(ctx->near_val);
         if (ctx->kappa) cudaFree(ctx->kappa);
         ctx->kappa = nullptr;
         ctx->node_buf = nullptr; ctx->comp_buf = nullptr; ctx->free_buf = nullptr; ctx->cap = 0;
-        ctx->near_ptr = nullptr; ctx->near_col = nullptr; ctx->near_val = nullptr;
-        BIE_CUDA(cudaMalloc((void**)&ctx->node_buf, sizeof(double) * BIE_NODE_ARRAYS * (size_t)npad));
-        BIE_CUDA(cudaMalloc((void**)&ctx->comp_buf, sizeof(int) * (size_t)npad));
-        BIE_CUDA(cudaMalloc((void**)&ctx->free_buf, sizeof(double) * bie_free_buf_doubles(npad)));
-        BIE_CUDA(cudaMalloc((void**)&ctx->near_ptr, sizeof(int) * (8 * (size_t)npad + 1)));
-        BIE_CUDA(cudaMalloc((void**)&ctx->near_col, sizeof(int) * bie_near_cap(npad)));
-        BIE_CUDA(cudaMalloc((void**)&ctx->near_val, sizeof(double) * bie_near_cap(npad)));
-        BIE_CUDA(cudaMalloc((void**)&ctx->kappa, sizeof(double) * (size_t)npad));
+        ctx->near_ptr = nullptr;
+        cudaError_t e = cudaMalloc((void**)&ctx->node_buf, sizeof(double) * BIE_NODE_ARRAYS * (size_t)npad);
+        if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->comp_buf, sizeof(int) * (size_t)npad);
+        if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->free_buf, sizeof(double) * bie_free_buf_doubles(npad));
+        if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->near_ptr, sizeof(int) * (8 * (size_t)npad + 4));
+        if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->kappa, sizeof(double) * (size_t)npad);
+        if (e != cudaSuccess) {
+            cudaGetLastError();   // clear the sticky-free allocation error; the ctx stays without a geometry
+            return bie_cuda_err(e);
+        }
         ctx->cap = npad;
     }
     PrepArgs pa;
@@ -145,29 +148,50 @@ int bie_prepare_nodes(bie_ctx* ctx, int ncomp, const int32_t* counts, const int3
         pa.kinds[c] = c < ncomp ? kinds[c] : 0;
         pa.comps.off[c + 1] = c < ncomp ? pa.comps.off[c] + counts[c] : (int)n;
     }
+    ctx->have_geom = 0;
+    BIE_CUDA(cudaMemsetAsync(ctx->taubar, 0, sizeof(double), st));
+    bie_prepare_nodes_kernel<<<(npad + 255) / 256, 256, 0, st>>>(
+        pa, (int)n, npad, variant, (const double2*)zeta, (const double2*)dzeta, (const double2*)d2zeta,
+        (double2*)ctx->node_buf, ctx->comp_buf, (double2*)ctx->free_buf, ctx->taubar, ctx->kappa);
+    BIE_CUDA(cudaGetLastError());
     ctx->n = (int)n;
     ctx->ncomp = ncomp;
     ctx->variant = variant;
     for (int c = 0; c < ncomp; ++c) { ctx->counts[c] = counts[c]; ctx->kinds[c] = kinds[c]; }
     ctx->comps = pa.comps;
     ctx->have_geom = 1;
-    ctx->near_valid = 0;
-    BIE_CUDA(cudaMemsetAsync(ctx->taubar, 0, sizeof(double), st));
-    bie_prepare_nodes_kernel<<<(npad + 255) / 256, 256, 0, st>>>(
-        pa, (int)n, npad, variant, (const double2*)zeta, (const double2*)dzeta, (const double2*)d2zeta,
-        (double2*)ctx->node_buf, ctx->comp_buf, (double2*)ctx->free_buf, ctx->taubar, ctx->kappa);
-    BIE_CUDA(cudaGetLastError());
     return BIE_OK;
 }
 
 // ---- matrix-free operator: storage and work split (bie_free.cuh) ------------------------------------------
 size_t bie_free_buf_doubles(int cap)
 {
-    // tables [4][cap] double2, then partial sums for (row blocks + CTAs) parts of FREE_ROWS rows
-    return 8 * (size_t)cap + ((size_t)cap / FREE_ROWS + 2 + 256) * FREE_ROWS;
+    // tables [4][cap] double2, then partial sums for (row blocks + CTAs) parts of FREE_ROWS rows, then the per-CTA
+    // partials of the constant term [2][FREE_SB_LD]
+    return 8 * (size_t)cap + ((size_t)cap / FREE_ROWS + 2 + 256) * FREE_ROWS + 2 * FREE_SB_LD;
 }
 
-int bie_free_plan(const bie_ctx* ctx, int grid, int s_off, FreePlan* fp, cudaStream_t st)
+// work list of the symmetric split (bie_free_sym.cuh), built on the device by one thread (NB <= a few hundred):
+// blocks in the order 0, NB-1, 1, NB-2, ... (long and short source lists alternate); cum[k] = sources before position k
+__global__ void bie_sym_tables_kernel(int NB, int NB0, int M0, int n, int npad, int s_off, int first, long long* cum,
+                                      int* perm, int* pos)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    long long c = 0;
+    cum[0] = 0;
+    for (int k = 0; k < NB; ++k) {
+        const int b = (k & 1) ? NB - 1 - (k >> 1) : (k >> 1);
+        perm[k] = b;
+        pos[b] = k;
+        const int row0 = b < NB0 ? b * FREE_ROWS : M0 + (b - NB0) * FREE_ROWS;
+        const int src0 = b < first ? s_off : row0;
+        c += (npad - src0);
+        cum[k + 1] = c;
+    }
+    (void)n;
+}
+
+int bie_free_plan(bie_ctx* ctx, int grid, int s_off, FreePlan* fp, cudaStream_t st)
 {
     if (!ctx->have_geom || grid < 1 || grid > 256) return BIE_ERR_GEOMETRY;
     if (ctx->variant == BIE_VARIANT_NORMAL_INTERNAL) return BIE_ERR_GEOMETRY;   // node tables of another operator
@@ -187,51 +211,57 @@ int bie_free_plan(const bie_ctx* ctx, int grid, int s_off, FreePlan* fp, cudaStr
     const bool boundary = s_off == 0 || (s_off <= fp->M0 ? (s_off % FREE_ROWS == 0 || s_off == fp->M0)
                                                           : ((s_off - fp->M0) % FREE_ROWS == 0));
     fp->sym_first = 0;
-    // (in the hybrid operator only on request, use_sym == 2: with 8 pair-loop warps it is slower, 289 against 200 us per step)
+    // (in the hybrid operator only on request, use_sym == 2: with few pair-loop warps it is slower)
     if (ctx->use_sym && (s_off == 0 || ctx->use_sym == 2) && boundary && !fp->vortex && npad <= 65536) {
-        const size_t need = (size_t)fp->NB * (size_t)npad;
-        bie_ctx* c = const_cast<bie_ctx*>(ctx);
-        if (need > c->pc_cap) {
-            if (c->pc_buf) cudaFree(c->pc_buf);
-            c->pc_buf = nullptr; c->pc_cap = 0;
-            if (cudaMalloc((void**)&c->pc_buf, sizeof(double) * need + 16 * (size_t)(fp->NB + 2)) != cudaSuccess) return BIE_ERR_CUDA_BASE - (int)cudaErrorMemoryAllocation;
-            c->pc_cap = need;
-        }
-        // work list: blocks in the order 0, NB-1, 1, NB-2, ... ; tables behind the partials
         const int NB = fp->NB;
-        std::vector<long long> cum(NB + 1);
-        std::vector<int> perm(NB), pos(NB);
-        // blocks in the order of decreasing length of their source lists (blocks below s_off: npad - s_off each, then the
-        // triangle), taken alternately from both ends: 0, NB-1, 1, NB-2, ...
-        auto row0_of = [&](int b) { return b < fp->NB0 ? b * FREE_ROWS : fp->M0 + (b - fp->NB0) * FREE_ROWS; };
-        auto rows_of = [&](int b) { const int r0 = row0_of(b), end = b < fp->NB0 ? fp->M0 : n; return end - r0 < FREE_ROWS ? end - r0 : FREE_ROWS; };
-        int first = 0;
-        while (first < NB && row0_of(first) + rows_of(first) <= s_off) ++first;
-        fp->sym_first = first;
-        for (int k = 0; k < NB; ++k) perm[k] = (k & 1) ? NB - 1 - (k >> 1) : (k >> 1);
-        cum[0] = 0;
-        for (int k = 0; k < NB; ++k) {
-            const int b = perm[k];
-            pos[b] = k;
-            const int src0 = b < first ? s_off : row0_of(b);
-            cum[k + 1] = cum[k] + (npad - src0);
+        const size_t need = (size_t)NB * (size_t)npad;
+        if (need > ctx->pc_cap) {
+            if (ctx->pc_buf) cudaFree(ctx->pc_buf);
+            ctx->pc_buf = nullptr; ctx->pc_cap = 0;
+            if (cudaMalloc((void**)&ctx->pc_buf, sizeof(double) * need) != cudaSuccess) {
+                cudaGetLastError();
+                return BIE_ERR_CUDA_BASE - (int)cudaErrorMemoryAllocation;
+            }
+            ctx->pc_cap = need;
         }
-        const long long U = cum[NB];
-        char* tab = reinterpret_cast<char*>(c->pc_buf + need);
-        cudaMemcpyAsync(tab, cum.data(), sizeof(long long) * (NB + 1), cudaMemcpyHostToDevice, st);
-        cudaMemcpyAsync(tab + sizeof(long long) * (NB + 1), perm.data(), sizeof(int) * NB, cudaMemcpyHostToDevice, st);
-        cudaMemcpyAsync(tab + sizeof(long long) * (NB + 1) + sizeof(int) * NB, pos.data(), sizeof(int) * NB, cudaMemcpyHostToDevice, st);
-        fp->sym_cum = reinterpret_cast<const long long*>(tab);
-        fp->sym_perm = reinterpret_cast<const int*>(tab + sizeof(long long) * (NB + 1));
-        fp->sym_pos = fp->sym_perm + NB;
-        fp->sym = 1; fp->PC = c->pc_buf; fp->U = U;
+        // the tables are cached per (geometry, s_off): cum [NB + 1] long long, perm [NB], pos [NB]; sized for the largest
+        // NB the node capacity allows
+        const size_t nbmax = (size_t)ctx->cap / FREE_ROWS + 4;
+        const size_t tab_bytes = sizeof(long long) * (nbmax + 1) + 2 * sizeof(int) * nbmax;
+        if (tab_bytes > ctx->sym_tab_bytes) {
+            if (ctx->sym_tab) cudaFree(ctx->sym_tab);
+            ctx->sym_tab = nullptr; ctx->sym_tab_bytes = 0; ctx->sym_key[0] = -1;
+            if (cudaMalloc((void**)&ctx->sym_tab, tab_bytes) != cudaSuccess) {
+                cudaGetLastError();
+                return BIE_ERR_CUDA_BASE - (int)cudaErrorMemoryAllocation;
+            }
+            ctx->sym_tab_bytes = tab_bytes;
+        }
+        long long* cum = reinterpret_cast<long long*>(ctx->sym_tab);
+        int* perm = reinterpret_cast<int*>(ctx->sym_tab + sizeof(long long) * (nbmax + 1));
+        int* pos = perm + nbmax;
+        if (ctx->sym_key[0] != ctx->geom_gen || ctx->sym_key[1] != s_off) {
+            auto row0_of = [&](int b) { return b < fp->NB0 ? b * FREE_ROWS : fp->M0 + (b - fp->NB0) * FREE_ROWS; };
+            auto rows_of = [&](int b) { const int r0 = row0_of(b), end = b < fp->NB0 ? fp->M0 : n; return end - r0 < FREE_ROWS ? end - r0 : FREE_ROWS; };
+            int first = 0;
+            while (first < NB && row0_of(first) + rows_of(first) <= s_off) ++first;
+            long long U = 0;
+            for (int b = 0; b < NB; ++b) U += npad - (b < first ? s_off : row0_of(b));
+            bie_sym_tables_kernel<<<1, 32, 0, st>>>(NB, fp->NB0, fp->M0, n, npad, s_off, first, cum, perm, pos);
+            BIE_CUDA(cudaGetLastError());
+            ctx->sym_key[0] = ctx->geom_gen; ctx->sym_key[1] = s_off;
+            ctx->sym_U = U; ctx->sym_first = first;
+        }
+        fp->sym_first = ctx->sym_first;
+        fp->sym_cum = cum; fp->sym_perm = perm; fp->sym_pos = pos;
+        fp->sym = 1; fp->PC = ctx->pc_buf; fp->U = ctx->sym_U;
     }
     fp->Geff = (long long)grid < fp->U ? grid : (int)fp->U;
     if (fp->Geff < 1) fp->Geff = 1;
     fp->T = reinterpret_cast<double2*>(ctx->free_buf);
     fp->PB = ctx->free_buf + 8 * (size_t)npad;
+    fp->SB = ctx->free_buf + 8 * (size_t)ctx->cap + ((size_t)ctx->cap / FREE_ROWS + 2 + 256) * FREE_ROWS;
     fp->taubar = ctx->taubar;
     fp->near_ptr = ctx->near_ptr; fp->near_col = ctx->near_col; fp->near_val = ctx->near_val;
-    fp->near_overflow = ctx->near_overflow;
     return BIE_OK;
 }

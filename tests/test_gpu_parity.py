@@ -3,7 +3,7 @@ element by element on the same seeded inputs.  Tolerances are BASELINE.json's no
 
     matrix entries   max|A_gpu - A_cpu| / max|A_cpu| <= 1e-12          (reading R7: max-norm)
     GMRES solutions  ||x_gpu - x_cpu|| / ||x_cpu||   <= 1e-10 at tol 1e-13
-    iteration counts within +-1
+    iteration counts within +-1   (check_iters below; ONE named exception, config 3, reading R15)
     matvec           max|y_gpu - y_cpu| / max|y_cpu| <= 1e-13          (n eps sqrt-sum bound)
 """
 import numpy as np
@@ -113,19 +113,29 @@ def _sample_rows(g, rng, k=48):
     return np.array(sorted(rows), dtype=np.int64)
 
 
+def _compare_whole_matrix(A, g, variant, chunk=1024):
+    """element by element over the WHOLE matrix: the oracle builds `chunk` rows at a time (oracle.build_rows, pinned against
+    oracle.build_matrix in tests/test_oracle_pins.py), the same rows come back from the GPU; returns (max |diff|, max |A_cpu|)"""
+    n = g.n
+    worst, amax = 0.0, 0.0
+    for r0 in range(0, n, chunk):
+        rows = np.arange(r0, min(r0 + chunk, n), dtype=np.int64)
+        Ao = oracle.build_rows(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, rows, variant=variant)
+        Ag = A[r0:r0 + rows.size, :n].cpu().numpy()
+        assert np.all(np.isfinite(Ag)), r0
+        worst = max(worst, float(np.max(np.abs(Ag - Ao))))
+        amax = max(amax, float(np.max(np.abs(Ao))))
+    return worst, amax
+
+
 @pytest.mark.parametrize("c", [4, 5])
-def test_build_parity_full_size_sampled_rows(ctx, c):
-    """BASELINE.json's large configs in the launch configuration bench.py times: the whole matrix is built on
-    the GPU; sampled rows (random + both ends of every component) are compared element by element."""
+def test_build_parity_full_size_whole_matrix(ctx, c):
+    """BASELINE.json's large configs in the launch configuration bench.py times: the whole matrix is built on the GPU and
+    compared with the oracle element by element -- every tile, every wave and the tail of the grid"""
     g = cfg(c).geometry
     A = gpu_build(ctx, g)
-    rows = _sample_rows(g, np.random.default_rng(c))
-    Ag = A[torch.from_numpy(rows).cuda(), :g.n].cpu().numpy()
-    Ao = oracle.build_rows(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, rows)
-    assert np.all(np.isfinite(Ag))
-    assert float(np.max(np.abs(Ag - Ao))) <= TOL_ENTRY * 0.5  # max|A| >= 0.5 (the +-1/2 diagonal)
-    # property that holds at any size: every finite-entry check on the whole matrix
-    assert bool(torch.isfinite(A[:, :g.n]).all())
+    worst, amax = _compare_whole_matrix(A, g, 0)
+    assert worst / amax <= TOL_ENTRY, (worst, amax)
     del A
 
 
@@ -138,10 +148,8 @@ def test_build_update_only_touches_surface_blocks(ctx):
     z, dz, d2z = geo_dev(g1)
     ctx.bie_build_update(g1.counts, g1.kinds, z, dz, d2z, A)
     torch.cuda.synchronize()
-    rows = _sample_rows(g1, np.random.default_rng(11), k=24)
-    Ag = A[torch.from_numpy(rows).cuda(), :g1.n].cpu().numpy()
-    Ao = oracle.build_rows(g1.counts, g1.kinds, g1.zeta, g1.dzeta, g1.d2zeta, rows)
-    assert float(np.max(np.abs(Ag - Ao))) <= TOL_ENTRY * 0.5
+    worst, amax = _compare_whole_matrix(A, g1, 0)
+    assert worst / amax <= TOL_ENTRY, (worst, amax)
     # and a marker written into a solid-solid entry survives an update (those tiles are not rewritten)
     M0 = int(g1.counts[0])
     A[M0 + 300, M0 + 700] = 123.0
@@ -250,29 +258,42 @@ def test_operators_with_near_pairs_across_components(ctx, gap):
     b = inputs.rhs_analytic(g, lambda z: np.exp(1j * z))
     xo, ito, _, _, sto = oracle.gmres(Ao, b, 1e-13, 50, 2000)
     xg, it, rr, st, S = gpu_gmres_hybrid(ctx, g, 448, b, 1e-13, 50, 2000)
-    assert sto == 0 and st == 0 and abs(it - ito) <= max(1, ito // 50)
+    assert sto == 0 and st == 0
+    check_iters(it, ito, "obstacle %g under the surface" % gap)
     assert np.linalg.norm(xg - xo) / np.linalg.norm(xo) <= TOL_X * max(1.0, np.linalg.cond(Ao) / 100.0)
 
 
-def test_near_matrix_overflow_is_loud(ctx):
+def test_near_matrix_has_no_capacity_limit(ctx):
     """a 4-node obstacle next to an 8192-node surface pushes taubar to its cap (|w| < 0.1): every surface row then has
-    more near pairs than the CSR near matrix holds per node; the matrix-free operator must answer NaN, not a wrong
-    number (the dense path is unaffected)"""
+    about 260 near pairs (node spacing 7.7e-4).  The CSR near matrix is sized from the scanned count, so the matrix-free
+    operator stays exact -- one-directional and symmetric loops, and the hybrid solve -- against the oracle"""
     M0 = 8192
     parts = [inputs.graph_curve(M0, 0.0, None), inputs.graph_curve(64, -2.0, None),
              inputs.ellipse_curve(4, complex(3.0, -1.0), 0.3, 0.2, 0.0)]
     g = inputs.assemble(parts, [0, 1, 2])
+    n = g.n
+    Ao = oracle_build(g)
     z, dz, d2z = geo_dev(g)
-    ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z)
-    x = torch.ones(g.n, dtype=torch.float64, device="cuda")
-    y = torch.zeros(g.n, dtype=torch.float64, device="cuda")
-    ctx.bie_matvec_free(x, y)
-    torch.cuda.synchronize()
-    assert bool(torch.isnan(y).all())
+    xv = _x(n, 9)
+    yo = oracle.matvec(Ao, xv)
+    try:
+        for on in (1, 0):
+            ctx.bie_set_symmetric(on)
+            ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z)
+            y = torch.zeros(n, dtype=torch.float64, device="cuda")
+            ctx.bie_matvec_free(dev(xv), y)
+            torch.cuda.synchronize()
+            assert rel_max(y.cpu().numpy(), yo) <= 1e-12, on
+    finally:
+        ctx.bie_set_symmetric(1)
     A = gpu_build(ctx, g)
-    assert bool(torch.isfinite(A[:, :g.n]).all())
-    ctx.bie_matvec(A, x, y)
-    assert bool(torch.isfinite(y).all())
+    assert rel_max(A[:, :n].cpu().numpy(), Ao) <= TOL_ENTRY
+    b = inputs.rhs_analytic(g, lambda zz: np.exp(1j * zz))
+    xo, ito, _, _, sto = oracle.gmres(Ao, b, 1e-13, 50, 500)
+    xg, it, rr, st, S = gpu_gmres_hybrid(ctx, g, 3456, b, 1e-13, 50, 500)
+    assert sto == 0 and st == 0
+    check_iters(it, ito, "8192-node surface with 260 near pairs per row")
+    assert np.linalg.norm(xg - xo) / np.linalg.norm(xo) <= TOL_X * max(1.0, np.linalg.cond(Ao) / 100.0)
 
 
 # ------------------------------------------------------------------------------------------------
@@ -295,14 +316,11 @@ def test_build_vortex_ragged_sizes(ctx, shape):
 
 
 @pytest.mark.parametrize("c", [4, 5])
-def test_build_vortex_full_size_sampled_rows(ctx, c):
+def test_build_vortex_full_size_whole_matrix(ctx, c):
     g = cfg(c).geometry
-    rng = np.random.default_rng(40 + c)
-    rows = _sample_rows(g, rng)
     S = gpu_build(ctx, g, variant=2)
-    Sg = S[torch.from_numpy(rows).cuda()].cpu().numpy()[:, :g.n]
-    So = oracle.build_rows(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, rows, variant=2)
-    assert rel_max(Sg, So) <= TOL_ENTRY
+    worst, amax = _compare_whole_matrix(S, g, 2)
+    assert worst / amax <= TOL_ENTRY, (worst, amax)
     del S
 
 
@@ -708,14 +726,30 @@ def test_matvec_rect_matches_the_oracle(ctx):
 # ------------------------------------------------------------------------------------------------
 def iteration_band(Ao, b, tol, restart, max_iters, delta=0.25):
     """Iteration counts the ORACLE itself gives when its stopping threshold moves by +-delta (DESIGN.md reading
-    R15): (lo, hi) = first step with recurrence residual <= tol (1 + delta), <= tol (1 - delta).  When the residual
-    crosses tol with a clear margin lo == hi == the oracle's count and the check below is the plain +-1 of the
-    north_star; when it crosses on a plateau (config 3: 1.89e-13, 1.68e-13, 0.983e-13 at steps 72-74, after a
-    restart, where rounding noise is amplified to 10 % of the residual) the count is ill-conditioned and the band
-    says by how much."""
+    R15): (lo, hi) = first step with recurrence residual <= tol (1 + delta), <= tol (1 - delta)."""
     _, hi, _, hist, _ = oracle.gmres(Ao, b, tol * (1.0 - delta), restart, max_iters)
     lo = int(np.argmax(hist <= tol * (1.0 + delta)))
     return lo, hi
+
+
+# The north_star's tolerance on the iteration count is +-1 and that is what every GMRES test asserts, with ONE named
+# exception (DESIGN.md reading R15, where the numbers below are recorded): BASELINE.json configs[2] (n = 4608, restart 50).
+# Its recurrence residual crosses tol = 1e-13 on a plateau after the restart -- oracle: 4.32e-13, 3.34e-13, 1.89e-13,
+# 1.68e-13, 0.983e-13 at steps 70-74, i.e. 1.7 % under tol at step 74 (PAPER.md:L911: the stall after a restart) -- so a
+# relative perturbation of 2 % of the residual (rounding noise of r = b - A x at this level is 10 %) moves the count.
+# Measured on a B200 (round 2): oracle 74; GPU 76 with the dense, matrix-free (both loops) and hybrid operators.  For
+# that problem alone the test takes the counts the ORACLE itself gives for thresholds tol (1 -+ 0.25) -- (74, 76) --
+# widened by the +-1; everywhere else plain +-1.
+PLATEAU_CASES = {"config3"}
+
+
+def check_iters(it, ito, case=None, band=None):
+    if case in PLATEAU_CASES:
+        lo, hi = band()
+        assert lo <= ito <= hi, (ito, lo, hi)
+        assert lo - 1 <= it <= hi + 1, (case, it, ito, lo, hi)
+    else:
+        assert abs(it - ito) <= 1, (case, it, ito)
 
 
 def gpu_gmres(ctx, A, b, tol, restart, max_iters=1000):
@@ -740,11 +774,7 @@ def test_gmres_parity(ctx, c):
     A = gpu_build(ctx, g)  # the GPU's own matrix: the whole hot path
     x, it, rr, st = gpu_gmres(ctx, A, b, P.tol, P.restart, P.max_iters)
     assert st == 0
-    lo, hi = iteration_band(Ao, b, P.tol, P.restart, P.max_iters)
-    assert lo <= ito <= hi
-    assert lo - 1 <= it <= hi + 1, (it, ito, lo, hi)
-    if c in (1, 2):  # single cycle, clear crossing: the plain +-1
-        assert abs(it - ito) <= 1, (it, ito)
+    check_iters(it, ito, "config%d" % c, lambda: iteration_band(Ao, b, P.tol, P.restart, P.max_iters))
     assert np.linalg.norm(x - xo) / np.linalg.norm(xo) <= TOL_X
     assert rr <= 10 * P.tol  # reported true residual (reading R10)
     # and the GPU solution satisfies the ORACLE's system
@@ -753,7 +783,7 @@ def test_gmres_parity(ctx, c):
     del A
 
 
-@pytest.mark.parametrize("c", [1, 2, 5])
+@pytest.mark.parametrize("c", [1, 2, 3, 4, 5])
 def test_gmres_matrix_free_parity(ctx, c):
     P = cfg(c)
     g, b = P.geometry, P.rhs[0]
@@ -762,8 +792,8 @@ def test_gmres_matrix_free_parity(ctx, c):
     z, dz, d2z = geo_dev(g)
     ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z)
     x, it, rr, st = gpu_gmres(ctx, None, b, P.tol, P.restart, P.max_iters)
-    lo, hi = iteration_band(Ao, b, P.tol, P.restart, P.max_iters)
-    assert st == 0 and lo - 1 <= it <= hi + 1, (it, ito, lo, hi)
+    assert st == 0
+    check_iters(it, ito, "config%d" % c, lambda: iteration_band(Ao, b, P.tol, P.restart, P.max_iters))
     assert np.linalg.norm(x - xo) / np.linalg.norm(xo) <= TOL_X
     assert rr <= 10 * P.tol
 
@@ -797,7 +827,7 @@ def test_build_cols_writes_only_the_slab(ctx):
     assert np.all(Ah[:, nd:] == -7.0)
 
 
-@pytest.mark.parametrize("c,nd", [(1, 128), (2, 0), (2, 2), (2, 1030), (2, 1024), (2, 1280), (2, 2046), (3, 0), (3, 2048), (3, 2560), (5, 0)])
+@pytest.mark.parametrize("c,nd", [(1, 128), (2, 0), (2, 2), (2, 1030), (2, 1024), (2, 1280), (2, 2046), (3, 0), (3, 2048), (3, 2560), (4, 0), (5, 0)])
 def test_gmres_hybrid_parity(ctx, c, nd):
     """hybrid operator (stored slab of nd columns + recomputed sources): same solution, same iteration band;
     nd = 0 takes the library's own split (bie_hybrid_cols)"""
@@ -808,8 +838,8 @@ def test_gmres_hybrid_parity(ctx, c, nd):
     Ao = oracle_build(g)
     xo, ito, _, _, _ = oracle.gmres(Ao, b, P.tol, P.restart, P.max_iters)
     x, it, rr, st, A = gpu_gmres_hybrid(ctx, g, nd, b, P.tol, P.restart, P.max_iters)
-    lo, hi = iteration_band(Ao, b, P.tol, P.restart, P.max_iters)
-    assert st == 0 and lo - 1 <= it <= hi + 1, (it, ito, lo, hi)
+    assert st == 0
+    check_iters(it, ito, "config%d" % c, lambda: iteration_band(Ao, b, P.tol, P.restart, P.max_iters))
     assert np.linalg.norm(x - xo) / np.linalg.norm(xo) <= TOL_X
     assert rr <= 10 * P.tol
     r = b - oracle.matvec(Ao, x)
@@ -830,8 +860,8 @@ def test_gmres_hybrid_with_symmetric_pair_loops(ctx, c, nd):
         x, it, rr, st, A = gpu_gmres_hybrid(ctx, g, nd, b, P.tol, P.restart, P.max_iters)
     finally:
         ctx.bie_set_symmetric(1)
-    lo, hi = iteration_band(Ao, b, P.tol, P.restart, P.max_iters)
-    assert st == 0 and lo - 1 <= it <= hi + 1, (it, ito, lo, hi)
+    assert st == 0
+    check_iters(it, ito, "config%d" % c, lambda: iteration_band(Ao, b, P.tol, P.restart, P.max_iters))
     assert np.linalg.norm(x - xo) / np.linalg.norm(xo) <= TOL_X
     assert rr <= 10 * P.tol
 
@@ -865,8 +895,8 @@ def test_config4_sequence_of_four_stages(ctx):
         Ao = oracle_build(g)
         xo, ito, _, _, sto = oracle.gmres(Ao, b, P.tol, P.restart, P.max_iters)
         x, it, rr, st = gpu_gmres(ctx, A, b, P.tol, P.restart, P.max_iters)
-        lo, hi = iteration_band(Ao, b, P.tol, P.restart, P.max_iters)
-        assert sto == 0 and st == 0 and lo - 1 <= it <= hi + 1, (s, it, ito, lo, hi)
+        assert sto == 0 and st == 0
+        check_iters(it, ito, "config4 stage %d" % s)
         assert np.linalg.norm(x - xo) / np.linalg.norm(xo) <= TOL_X, s
         assert rr <= 10 * P.tol
         del Ao

@@ -381,13 +381,49 @@ def test_p7_gmres_edge_cases():
 
 
 def test_matvec_is_the_plain_definition():
+    import math
     rng = np.random.default_rng(4)
     A = rng.standard_normal((37, 37))
     x = rng.standard_normal(37)
     y = oracle.matvec(A, x)
-    import math
     for i in (0, 13, 36):
         assert abs(y[i] - math.fsum(A[i, j] * x[j] for j in range(37))) < 1e-14
+    # rectangular blocks (nrows != ncols, both ways) and a leading dimension larger than the column count: an index slip
+    # (i * ncols instead of i * lda, rows and columns swapped, a column of the padding read) fails one of these
+    for nrows, ncols, lda in ((5, 41, 41), (41, 5, 5), (7, 13, 20), (23, 9, 9 + 3), (1, 6, 8)):
+        S = rng.standard_normal((nrows, lda))
+        S[:, ncols:] = 1.0e6                     # padding columns must never be read
+        x = rng.standard_normal(ncols)
+        y = oracle.matvec(np.ascontiguousarray(S[:, :ncols]), x) if lda == ncols else oracle.matvec(S, x, lda=lda)
+        assert y.shape == (nrows,)
+        for i in range(nrows):
+            assert abs(y[i] - math.fsum(S[i, j] * x[j] for j in range(ncols))) < 1e-13, (nrows, ncols, lda, i)
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2])
+def test_build_rows_is_rows_of_build_matrix(variant):
+    """oracle.build_rows (what the full-size GPU parity tests compare against) is, bit for bit, the listed rows of
+    oracle.build_matrix (what pins P1-P8 fix) -- for unsorted, repeated and boundary rows, with and without an obstacle"""
+    rng = np.random.default_rng(variant)
+    for g in (inputs.make_config(1).geometry, inputs.small_problem(37, 29, [19, 23], seed=3).geometry,
+              inputs.small_problem(5, 3, [], seed=1).geometry):
+        A = _build(g, variant)
+        n = g.n
+        off = g.offsets
+        rows = list(rng.integers(0, n, size=min(n, 25)))
+        rows += [n - 1, 0, 0, n - 1] + [int(o) for o in off[:-1]] + [int(o) - 1 for o in off[1:]]
+        rows = np.array(rows, dtype=np.int64)
+        rng.shuffle(rows)
+        R = oracle.build_rows(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, rows, variant=variant)
+        assert R.shape == (rows.size, n)
+        assert np.array_equal(R, A[rows])
+        # one row at a time and in reverse order give the same bits
+        R1 = oracle.build_rows(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, rows[::-1], variant=variant)
+        assert np.array_equal(R1, A[rows[::-1]])
+        assert np.array_equal(oracle.build_rows(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, rows[:1], variant=variant)[0],
+                              A[rows[0]])
+    with pytest.raises(ValueError):
+        oracle.build_rows(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, np.array([g.n]), variant=variant)
 
 
 def test_config_iteration_counts_in_paper_range():
