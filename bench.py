@@ -294,7 +294,7 @@ def main():
     def step_hybrid(ev=None):
         for si, (gs, (zs, dzs, d2zs), bs) in enumerate(stages):
             if ev and si == 0: ev[0].record()
-            ctx.bie_build_cols(gs.counts, gs.kinds, zs, dzs, d2zs, nd, A)   # 2 launches: node prep + slab tiles
+            ctx.bie_build_block(gs.counts, gs.kinds, zs, dzs, d2zs, nd, A)  # 2 launches: node prep + block tiles
             if ev and si == 0: ev[1].record()
             ctx.bie_gmres_hybrid(A, nd, bs, x, P.tol, P.restart, P.max_iters, ws, oi, of)  # near matrix (3) + 1 launch
         if ev: ev[2].record()

@@ -64,7 +64,7 @@ extern "C" {
 /* operator of bie_solve_host (its `matrix_free` argument) */
 #define BIE_OP_DENSE 0  /* whole matrix stored, GEMV from HBM                                            */
 #define BIE_OP_FREE 1   /* nothing stored, entries recomputed on the fly                                 */
-#define BIE_OP_HYBRID 2 /* first bie_hybrid_cols(n) columns stored, the other sources recomputed         */
+#define BIE_OP_HYBRID 2 /* leading block of bie_hybrid_cols(n) rows and columns stored, the rest recomputed */
 
 /* bie_build `variant` */
 #define BIE_VARIANT_A 0 /* Eq. (3.16): 1/2 I + K_mm - E_m on obstacle diagonal blocks  */
@@ -126,12 +126,23 @@ int bie_build_update(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32
 
 /* Hybrid operator (north_star: "matrix-free fused rebuild+matvec variant chosen by measurement").  The dense
  * GEMV is HBM-bound and leaves the FP64 pipe idle, the matrix-free operator is FP64-bound and leaves HBM idle;
- * the hybrid operator does both at once: the first ncols columns of the matrix are stored (a slab, n x ncols,
- * row-major with leading dimension lda >= ncols, lda even) and streamed by some warps of every CTA while the
- * other warps recompute the entries of the remaining sources from the node tables.
- * bie_build_cols: as bie_build, but only the columns [0, ncols) of every row are written (1 <= ncols <= n).
- * bie_hybrid_cols: the slab width the library recommends for n on a B200 (even; 0 = too small, use bie_gmres).
- * bie_set_hybrid_free_warps: tuning knob, warps per CTA (of 16) on the pair loops (default 8). */
+ * the hybrid operator does both at once: the LEADING nblock x nblock block of the matrix is stored (row-major,
+ * leading dimension lda >= nblock, lda even) and arrives in shared memory by bulk copies (TMA) while the warps of
+ * every CTA recompute every other entry from the node tables -- with the symmetric pair loops (see
+ * bie_set_symmetric): every pair {t, s} outside the block has max(t, s) >= nblock, so one evaluation of the pair
+ * serves both entries -- and consume the landed tiles of the block between their source chunks.
+ * nblock must be a row-block boundary of the pair loops: a multiple of 128 up to M_0, or M_0 itself, or M_0 plus a
+ * multiple of 128; even; < n.
+ * bie_build_block: as bie_build, but only rows and columns [0, nblock) are written (1 <= nblock <= n).
+ * bie_build_cols: as bie_build, but only the columns [0, ncols) of every row are written (1 <= ncols <= n); its
+ *   first ncols rows are the block, so it may feed bie_gmres_hybrid too.
+ * bie_hybrid_cols: the block edge the library recommends for n on a B200 (0 = too small, use bie_gmres); it uses M_0
+ *   of the ctx's current geometry when that has n nodes, else assumes M_0 is a multiple of 128.
+ * bie_set_hybrid_free_warps: tuning knob, warps per CTA on the pair loops (1..15, default 15; warps above it only
+ *   consume tiles of the block, the 16th issues the bulk copies). */
+int bie_build_block(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds,
+                    const double* zeta, const double* dzeta, const double* d2zeta,
+                    int variant, int nblock, double* A, int64_t lda, void* stream);
 int bie_build_cols(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds,
                    const double* zeta, const double* dzeta, const double* d2zeta,
                    int variant, int ncols, double* A, int64_t lda, void* stream);
@@ -151,12 +162,11 @@ int bie_set_geometry(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32
  */
 int bie_matvec(bie_ctx* ctx, int n, const double* A, int64_t lda, const double* x, double* y, void* stream);
 int bie_matvec_free(bie_ctx* ctx, int n, const double* x, double* y, void* stream);
-/* The whole-matrix matrix-free operator (bie_matvec_free, bie_gmres with A == NULL; variants A and B, n <= 65536) uses the
- * oddness of the kernel, cot((zeta_s - zeta_t)/2) = -cot((zeta_t - zeta_s)/2): one evaluation of the pair serves the entries
- * (t,s) and (s,t) (15 FP64 instructions for two entries instead of 22).  on = 0 switches back to the one-directional pair
- * loops, on = 1 is the default, on = 2 also uses the symmetric loops inside the hybrid operator when the slab width is a
- * row-block boundary (a multiple of 128 up to M_0, or M_0 + a multiple of 128) -- measured slower there on a B200, kept
- * for measurement.  Same results to rounding; all are deterministic. */
+/* The matrix-free operator (bie_matvec_free, bie_gmres with A == NULL) and the recomputed part of the hybrid operator
+ * (variants A and B, n <= 65536) use the oddness of the kernel, cot((zeta_s - zeta_t)/2) = -cot((zeta_t - zeta_s)/2): one
+ * evaluation of the pair serves the entries (t,s) and (s,t) (13 FP64 instructions for two entries instead of 20).
+ * on = 0 switches to the one-directional pair loops, on = 1 (default; 2 is accepted as a synonym) uses the symmetric
+ * ones.  Same results to rounding; all are deterministic. */
 int bie_set_symmetric(bie_ctx* ctx, int on);
 
 /* stream function prescribed on the solids, circulation parameters
@@ -230,8 +240,9 @@ int bie_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, const double* r
               double* x, int32_t* iters_out, double* relres_out, int32_t* status_out, double* res_hist,
               void* workspace, size_t workspace_bytes, void* stream);
 
-/* Same solve with the hybrid operator: A is the slab written by bie_build_cols for the ctx's current geometry,
- * ncols_dense its width (even, 2 <= ncols_dense < n), lda >= ncols_dense.  Everything else as bie_gmres. */
+/* Same solve with the hybrid operator: A holds the leading ncols_dense x ncols_dense block of the matrix of the ctx's
+ * current geometry (bie_build_block; or a slab of bie_build_cols), ncols_dense a row-block boundary as described at
+ * bie_build_block (else BIE_ERR_ARG), lda >= ncols_dense.  Everything else as bie_gmres. */
 int bie_gmres_hybrid(bie_ctx* ctx, int n, const double* A, int64_t lda, int ncols_dense, const double* rhs,
                      double tol, int restart, int max_iters,
                      double* x, int32_t* iters_out, double* relres_out, int32_t* status_out, double* res_hist,
@@ -243,7 +254,8 @@ int bie_gmres_hybrid(bie_ctx* ctx, int n, const double* A, int64_t lda, int ncol
  * zeta, dzeta, d2zeta, rhs, x: host (pinned memory makes the copies asynchronous).  dev_workspace: dev, at
  * least bie_solve_workspace_bytes(n, restart) bytes (holds node data, A with lda = n rounded up to even,
  * rhs, x and the GMRES workspace).  matrix_free selects the operator: BIE_OP_DENSE (0), BIE_OP_FREE (1: no
- * matrix is stored) or BIE_OP_HYBRID (2: a slab of bie_hybrid_cols(n) columns is stored).  Returns BIE_OK,
+ * matrix is stored) or BIE_OP_HYBRID (2: the leading block of bie_hybrid_cols(n) rows and columns is stored; falls
+ * back to BIE_OP_FREE when n is too small for a block).  Returns BIE_OK,
  * BIE_MAX_ITERS or an error.
  */
 size_t bie_solve_workspace_bytes(int n, int restart, int matrix_free);

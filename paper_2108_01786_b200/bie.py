@@ -24,7 +24,8 @@ EXPORTS = ("bie_create", "bie_destroy", "bie_strerror", "bie_device_info", "bie_
            "bie_set_geometry", "bie_matvec", "bie_matvec_free", "bie_gmres_workspace_bytes", "bie_gmres",
            "bie_solve_workspace_bytes", "bie_solve_host", "bie_probe_dfma", "bie_build_cols", "bie_hybrid_cols",
            "bie_set_hybrid_free_warps", "bie_gmres_hybrid", "bie_matvec_rect", "bie_build_normal_velocity",
-           "bie_add_cyl_columns", "bie_cauchy_eval_workspace_bytes", "bie_cauchy_eval", "bie_set_symmetric")
+           "bie_add_cyl_columns", "bie_cauchy_eval_workspace_bytes", "bie_cauchy_eval", "bie_set_symmetric",
+           "bie_build_block")
 
 BIE_OK, BIE_MAX_ITERS = 0, 1
 OP_DENSE, OP_FREE, OP_HYBRID = 0, 1, 2
@@ -77,6 +78,8 @@ def lib() -> ctypes.CDLL:
                                      ctypes.POINTER(dbl), vp, sz, vp]
         L.bie_build_cols.restype = i32
         L.bie_build_cols.argtypes = geo + [i32, vp, i64, vp]
+        L.bie_build_block.restype = i32
+        L.bie_build_block.argtypes = geo + [i32, vp, i64, vp]
         L.bie_hybrid_cols.restype = i32
         L.bie_hybrid_cols.argtypes = [vp, i32]
         L.bie_set_hybrid_free_warps.restype = i32
@@ -185,12 +188,22 @@ class Context:
 
     def bie_build_cols(self, counts, kinds, zeta, dzeta, d2zeta, ncols: int, A, variant: int = VARIANT_A,
                        lda: Optional[int] = None):
-        """A (CUDA float64, n x lda row-major, lda >= ncols) <- columns [0, ncols) of the matrix of Eq. (3.16):
-        the stored slab of the hybrid operator."""
+        """A (CUDA float64, n x lda row-major, lda >= ncols) <- columns [0, ncols) of the matrix of Eq. (3.16)
+        (all n rows; the hybrid operator reads only the leading ncols x ncols block of it, see bie_build_block)."""
         n, args, keep = self._geo(counts, kinds, zeta, dzeta, d2zeta, variant)
         lda = int(lda if lda is not None else A.stride(0))
         _dev_f64(A, (n - 1) * lda + int(ncols))
         _check(lib().bie_build_cols(*args, int(ncols), A.data_ptr(), lda, _stream()), "bie_build_cols")
+        return A
+
+    def bie_build_block(self, counts, kinds, zeta, dzeta, d2zeta, nblock: int, A, variant: int = VARIANT_A,
+                        lda: Optional[int] = None):
+        """A (CUDA float64, nblock x lda row-major, lda >= nblock) <- the leading nblock x nblock block of the matrix:
+        the stored part of the hybrid operator."""
+        n, args, keep = self._geo(counts, kinds, zeta, dzeta, d2zeta, variant)
+        lda = int(lda if lda is not None else A.stride(0))
+        _dev_f64(A, (int(nblock) - 1) * lda + int(nblock))
+        _check(lib().bie_build_block(*args, int(nblock), A.data_ptr(), lda, _stream()), "bie_build_block")
         return A
 
     def bie_hybrid_cols(self, n: int) -> int:

@@ -31,7 +31,7 @@ int bie_create(bie_ctx** out, int device)
     c->hybrid_free_warps = BIE_HYBRID_FREE_WARPS;
     c->taubar = nullptr; c->kappa = nullptr;
     c->pc_buf = nullptr; c->pc_cap = 0;
-    c->sym_tab = nullptr; c->sym_tab_bytes = 0; c->sym_U = 0; c->sym_first = 0; c->geom_gen = 0; c->sync_next = 0;
+    c->sym_tab = nullptr; c->sym_tab_bytes = 0; c->sym_U = 0; c->geom_gen = 0; c->sync_next = 0;
     for (int i = 0; i < 4; ++i) c->sym_key[i] = -1;
     for (int i = 0; i < 16; ++i) c->smem_set[i] = 0;
     c->use_sym = 1;   // bie_set_symmetric
@@ -111,7 +111,7 @@ int bie_build(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* kinds
     BIE_CUDA(cudaSetDevice(c->device));
     int rc = bie_prepare_nodes(c, ncomp, counts, kinds, zeta, dzeta, d2zeta, variant, (cudaStream_t)stream);
     if (rc != BIE_OK) return rc;
-    return bie_launch_build(c, A, lda, c->n, 0, (cudaStream_t)stream);
+    return bie_launch_build(c, A, lda, c->n, 0, 0, (cudaStream_t)stream);
 }
 
 int bie_build_update(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* kinds, const double* zeta,
@@ -122,7 +122,7 @@ int bie_build_update(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t
     BIE_CUDA(cudaSetDevice(c->device));
     int rc = bie_prepare_nodes(c, ncomp, counts, kinds, zeta, dzeta, d2zeta, variant, (cudaStream_t)stream);
     if (rc != BIE_OK) return rc;
-    return bie_launch_build(c, A, lda, c->n, 1, (cudaStream_t)stream);
+    return bie_launch_build(c, A, lda, c->n, 0, 1, (cudaStream_t)stream);
 }
 
 int bie_build_cols(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* kinds, const double* zeta,
@@ -133,21 +133,41 @@ int bie_build_cols(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* 
     BIE_CUDA(cudaSetDevice(c->device));
     int rc = bie_prepare_nodes(c, ncomp, counts, kinds, zeta, dzeta, d2zeta, variant, (cudaStream_t)stream);
     if (rc != BIE_OK) return rc;
-    return bie_launch_build(c, A, lda, ncols, 0, (cudaStream_t)stream);
+    return bie_launch_build(c, A, lda, ncols, 0, 0, (cudaStream_t)stream);
 }
 
-// the slab's share of the columns that makes the slab stream and the pair loops finish together on a B200 (measured,
-// DESIGN.md "Hybrid operator"); a multiple of 128 = a row-block boundary of the pair loops
-static int hybrid_cols(int n)
+// edge of the stored leading block of the hybrid operator: the share of n that makes the block stream and the pair loops
+// finish together on a B200 (measured), rounded down to a row-block boundary of the pair
+// loops: a multiple of 128 up to M_0, or M_0 plus a multiple of 128; even; 0 = too small to be worth it
+static int hybrid_cols(int n, int M0)
 {
     if (n < 4) return 0;
-    int nd = (int)((double)n * BIE_HYBRID_DENSE_FRACTION) & ~127;
-    if (nd < 128) nd = 0;           // too small to be worth two kinds of work: use bie_gmres
-    if (nd > n - 2) nd = (n - 2) & ~1;
+    if (M0 < 1 || M0 > n) M0 = n;
+    const int target = (int)((double)n * BIE_HYBRID_DENSE_FRACTION);
+    int nd = target <= M0 ? (target & ~127) : M0 + ((target - M0) & ~127);
+    if (nd & 1) nd = M0 & ~127;      // M_0 odd: stay on Gamma_0
+    if (nd < 128) nd = 0;
+    if (nd > n - 2) nd = 0;
     return nd;
 }
 
-int bie_hybrid_cols(bie_ctx* c, int n) { return c ? hybrid_cols(n) : 0; }
+int bie_hybrid_cols(bie_ctx* c, int n)
+{
+    if (!c) return 0;
+    return hybrid_cols(n, (c->have_geom && c->n == n) ? c->counts[0] : n);
+}
+
+int bie_build_block(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* kinds, const double* zeta,
+                    const double* dzeta, const double* d2zeta, int variant, int nblock, double* A, int64_t lda, void* stream)
+{
+    if (variant < BIE_VARIANT_A || variant > BIE_VARIANT_VORTEX) return BIE_ERR_ARG;
+    if (!c || !A) return BIE_ERR_NULL;
+    if (nblock < 1) return BIE_ERR_ARG;
+    BIE_CUDA(cudaSetDevice(c->device));
+    int rc = bie_prepare_nodes(c, ncomp, counts, kinds, zeta, dzeta, d2zeta, variant, (cudaStream_t)stream);
+    if (rc != BIE_OK) return rc;
+    return bie_launch_build(c, A, lda, nblock, nblock, 0, (cudaStream_t)stream);
+}
 
 int bie_set_symmetric(bie_ctx* c, int on)
 {
@@ -211,7 +231,7 @@ int bie_build_normal_velocity(bie_ctx* c, int ncomp, const int32_t* counts, cons
     int rc = bie_prepare_nodes(c, ncomp, counts, kinds, zeta, dzeta, d2zeta, BIE_VARIANT_NORMAL_INTERNAL,
                                (cudaStream_t)stream);
     if (rc != BIE_OK) return rc;
-    return bie_launch_build(c, Nmat, lda, c->n, 0, (cudaStream_t)stream);
+    return bie_launch_build(c, Nmat, lda, c->n, 0, 0, (cudaStream_t)stream);
 }
 
 int bie_matvec_free(bie_ctx* c, int n, const double* x, double* y, void* stream)
@@ -249,24 +269,27 @@ int bie_gmres_hybrid(bie_ctx* c, int n, const double* A, int64_t lda, int ncols_
 // ---- end-to-end with host buffers --------------------------------------------------------------------
 static inline size_t up256(size_t b) { return (b + 255) & ~(size_t)255; }
 
-// slab width of bie_solve_host's stored part for an operator mode (0: n, 1: none, 2: bie_hybrid_cols)
-static int solve_cols(int n, int op)
+// edge of bie_solve_host's stored part for an operator mode (dense: n, matrix-free: 0, hybrid: the leading block).
+// Without the geometry (workspace query) the hybrid block is bounded by what any M_0 can give.
+static int solve_cols(int n, int M0, int op)
 {
     if (op == BIE_OP_FREE) return 0;
-    if (op == BIE_OP_HYBRID) return hybrid_cols(n);
+    if (op == BIE_OP_HYBRID) return hybrid_cols(n, M0);
     return n;
 }
 
 size_t bie_solve_workspace_bytes(int n, int restart, int matrix_free)
 {
     if (n < 1 || restart < 1) return 0;
-    const size_t nld = ((size_t)solve_cols(n, matrix_free) + 1) & ~(size_t)1;
+    // hybrid: the block edge depends on M_0; (frac n + 128)^2 bounds every case
+    const size_t nblk = matrix_free == BIE_OP_HYBRID ? (size_t)((double)n * BIE_HYBRID_DENSE_FRACTION) + 130 : (size_t)solve_cols(n, n, matrix_free);
+    const size_t nld = (nblk + 1) & ~(size_t)1;
     const size_t nvec = ((size_t)n + 1) & ~(size_t)1;
     size_t o = 256;
     o += 3 * up256(16 * (size_t)n);          // zeta, dzeta, d2zeta
     o += 2 * up256(8 * nvec);                // rhs, x
     o += up256(64);                          // iters, status, relres
-    if (nld) o += up256(8 * nld * (size_t)n);
+    if (nld) o += up256(8 * nld * (matrix_free == BIE_OP_HYBRID ? nld : (size_t)n));
     o += bie_gmres_ws_bytes(n, restart);
     return o;
 }
@@ -284,7 +307,9 @@ int bie_solve_host(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* 
     if (restart < 1 || matrix_free < 0 || matrix_free > 2) return BIE_ERR_ARG;
     const int n = (int)nn;
     if (bie_solve_workspace_bytes(n, restart, matrix_free) > dev_workspace_bytes) return BIE_ERR_WORKSPACE;
-    const int ncols = solve_cols(n, matrix_free);      // stored columns: n (dense), 0 (matrix-free), slab (hybrid)
+    int ncols = solve_cols(n, counts[0], matrix_free);   // stored columns: n (dense), 0 (matrix-free), block edge (hybrid)
+    if (matrix_free == BIE_OP_HYBRID && ncols == 0) { matrix_free = BIE_OP_FREE; }   // too small for a block: matrix-free
+    const int nrows_st = matrix_free == BIE_OP_HYBRID ? ncols : n;                      // stored rows
     BIE_CUDA(cudaSetDevice(c->device));
     cudaStream_t st = (cudaStream_t)stream;
     const size_t nld = ((size_t)ncols + 1) & ~(size_t)1;
@@ -297,7 +322,7 @@ int bie_solve_host(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* 
     double* dx = (double*)p; p += up256(8 * nvec);
     int32_t* dint = (int32_t*)p; double* drel = (double*)(p + 16); p += up256(64);
     double* dA = nullptr;
-    if (ncols) { dA = (double*)p; p += up256(8 * nld * (size_t)n); }
+    if (ncols) { dA = (double*)p; p += up256(8 * nld * (size_t)nrows_st); }
     void* gws = p;
     const size_t gws_bytes = bie_gmres_ws_bytes(n, restart);
     BIE_CUDA(cudaMemcpyAsync(dz0, zeta, 16 * (size_t)n, cudaMemcpyHostToDevice, st));
@@ -307,7 +332,7 @@ int bie_solve_host(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* 
     int rc = bie_prepare_nodes(c, ncomp, counts, kinds, dz0, dz1, dz2, BIE_VARIANT_A, st);
     if (rc != BIE_OK) return rc;
     if (ncols) {
-        rc = bie_launch_build(c, dA, (int64_t)nld, ncols, 0, st);
+        rc = bie_launch_build(c, dA, (int64_t)nld, ncols, nrows_st, 0, st);
         if (rc != BIE_OK) return rc;
     }
     rc = bie_launch_gmres(c, n, dA, (int64_t)nld, ncols < n ? ncols : 0, drhs, tol, restart, max_iters, dx, dint, drel,

@@ -60,13 +60,12 @@ __device__ __forceinline__ void bie_block_coef(bool src0, bool tgt0, double qr, 
 }
 
 __global__ void __launch_bounds__(BUILD_THREADS)
-bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long lda, int T, int only0, int ncols)
+bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long lda, int T, int only0, int ncols, int nrows)
 {
     extern __shared__ __align__(16) double2 sm[];  // [T] E_t
-    const int n = nt.n;
     const int c0 = blockIdx.x * BUILD_TILE_W;
     const int t0 = blockIdx.y * T;
-    const int t1 = min(t0 + T, n);
+    const int t1 = min(t0 + T, nrows);      // nrows = n, or the rows of the hybrid operator's block
     if (only0 && t0 >= ct.off[1] && c0 >= ct.off[1]) return;  // a4: solid-solid tiles stay
     double2* sE = sm;
     for (int i = threadIdx.x; i < t1 - t0; i += BUILD_THREADS) sE[i] = nt.E[t0 + i];
@@ -165,14 +164,13 @@ __device__ __forceinline__ double bie_entry_fast_dagger(const SrcColD& s, const 
 }
 
 __global__ void __launch_bounds__(BUILD_THREADS)
-bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long lda, int T, int only0, int ncols,
+bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long lda, int T, int only0, int ncols, int nrows,
                         const double* __restrict__ kappa /* NULL: vortex-sheet S; else the normal-velocity operator */)
 {
     extern __shared__ __align__(16) double2 sm[];  // [T] E_t, [T] (A,B) for columns on Gamma_0, [T] (A,B) for solids, [T] M_t
-    const int n = nt.n;
     const int c0 = blockIdx.x * BUILD_TILE_W;
     const int t0 = blockIdx.y * T;
-    const int t1 = min(t0 + T, kappa ? ct.off[1] : n);   // the normal-velocity operator has rows on Gamma_0 only
+    const int t1 = min(t0 + T, nrows);   // n; M_0 for the normal-velocity operator (rows on Gamma_0 only); the block's rows
     if (only0 && t0 >= ct.off[1] && c0 >= ct.off[1]) return;
     double2* sE = sm;
     double2* sAB0 = sm + T;
@@ -253,17 +251,17 @@ bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long
     }
 }
 
-// ncols: the first ncols columns of every row are written (ncols = n: the whole matrix)
-int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int ncols, int only_comp0, cudaStream_t st)
+// the first ncols columns of the first nrows rows are written (nrows = ncols = n: the whole matrix; nrows <= 0: all rows)
+int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int ncols, int nrows, int only_comp0, cudaStream_t st)
 {
     if (!ctx || !A) return BIE_ERR_NULL;
     if (!ctx->have_geom) return BIE_ERR_GEOMETRY;
     const int n = ctx->n;
-    if (ncols < 1 || ncols > n) return BIE_ERR_ARG;
+    if (ncols < 1 || ncols > n || nrows > n) return BIE_ERR_ARG;
     if (lda < ncols || (lda & 1) || (((uintptr_t)A) & 15u)) return BIE_ERR_LAYOUT;
     const NodeTable nt = bie_node_table(ctx);
     const int gx = (ncols + BUILD_TILE_W - 1) / BUILD_TILE_W;
-    int nt_rows = n;
+    int nt_rows = nrows > 0 ? nrows : n;
     if (ctx->variant == BIE_VARIANT_NORMAL_INTERNAL) nt_rows = ctx->counts[0];   // M_0 x n: rows on Gamma_0 only
     const bool dagger = (ctx->variant == BIE_VARIANT_VORTEX || ctx->variant == BIE_VARIANT_NORMAL_INTERNAL);
     // rows per CTA: 128 when that still gives every SM several CTAs, else smaller ...
@@ -288,13 +286,13 @@ int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int ncols, int only_c
     dim3 grid(gx, (nt_rows + T - 1) / T);
     if (dagger) {
         bie_build_dagger_kernel<<<grid, BUILD_THREADS, (3 * sizeof(double2) + sizeof(double)) * T + 16, st>>>(
-            nt, ctx->comps, A, (long long)lda, T, only_comp0, ncols,
+            nt, ctx->comps, A, (long long)lda, T, only_comp0, ncols, nt_rows,
             ctx->variant == BIE_VARIANT_NORMAL_INTERNAL ? ctx->kappa : nullptr);
         BIE_CUDA(cudaGetLastError());
         return BIE_OK;
     }
     bie_build_kernel<<<grid, BUILD_THREADS, sizeof(double2) * T + 16, st>>>(nt, ctx->comps, A, (long long)lda, T,
-                                                                                            only_comp0, ncols);
+                                                                             only_comp0, ncols, nt_rows);
     BIE_CUDA(cudaGetLastError());
     return BIE_OK;
 }

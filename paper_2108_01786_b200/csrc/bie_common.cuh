@@ -30,8 +30,8 @@
 #define BIE_NEAR_C 0.25               // tau_s = BIE_NEAR_C |q_s|  (fast-path entry error <= ~1e-14)
 #define BIE_NEAR_TAU_MIN 1.0e-9
 #define BIE_NEAR_TAU_MAX 1.0e-2       // |w| < 0.1: Laurent truncation 2|w/2|^9/93555 < 1e-16
-#define BIE_HYBRID_FREE_WARPS 8        // hybrid operator: warps of a CTA on the pair loops (of 16)
-#define BIE_HYBRID_DENSE_FRACTION 0.42 // hybrid operator: share of the columns kept as a stored slab
+#define BIE_HYBRID_FREE_WARPS 15       // hybrid operator: warps of a CTA on the pair loops (of 16; one warp issues the bulk copies)
+#define BIE_HYBRID_DENSE_FRACTION 0.5625 // hybrid operator: edge of the stored leading block as a share of n (32 % of the entries)
 #define BIE_SYNC_SLOTS 16             // grid-barrier counters of a ctx (bie_matvec_free cycles through them), 256 B apart
 
 // Node table, arrays of double2 of length npad.
@@ -75,7 +75,6 @@ struct bie_ctx {
     size_t sym_tab_bytes;
     long long sym_key[4];    // (geometry generation, s_off, grid, 1) the cached tables were made for
     long long sym_U;         // their total number of list positions
-    int sym_first;
     long long geom_gen;      // incremented by every bie_prepare_nodes
     int smem_set[16];        // dynamic shared memory already granted to the kernel instantiations (cudaFuncSetAttribute once)
     int use_sym;             // use the symmetric work split for the whole-matrix matrix-free operator
@@ -139,7 +138,7 @@ int bie_ensure_near(bie_ctx* ctx, cudaStream_t st);
 int bie_prepare_nodes(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds,
                       const double* zeta, const double* dzeta, const double* d2zeta, int variant,
                       cudaStream_t st);
-int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int ncols, int only_comp0, cudaStream_t st);
+int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int ncols, int nrows, int only_comp0, cudaStream_t st);
 int bie_launch_matvec(bie_ctx* ctx, int nrows, int n, const double* A, int64_t lda, const double* x, double* y,
                       cudaStream_t st);
 int bie_launch_matvec_free(bie_ctx* ctx, const double* x, double* y, cudaStream_t st);

@@ -1,6 +1,6 @@
 // bie_free.cuh -- matrix-free form of SURVEY 8(a) row a6: y_t = sum_s A[t][s] x_s with the entries of
 // Eq. (3.16) recomputed on the fly from the node tables; no matrix traffic at all.
-// Device functions shared by bie_matvec_free (bie_matvec.cu) and the matrix-free GMRES (bie_gmres.cu).
+// Device functions shared by bie_matvec_free (bie_matvec.cu) and the matrix-free / hybrid GMRES (bie_gmres.cu).
 //
 // Arithmetic ("difference form", bie_common.cuh).  With E = e^{i zeta} per node, d = E_s - E_t = dr + i di,
 // den = |d|^2 and the block coefficients (alpha, beta) of Eq. (3.10), the product of an entry with x_s is
@@ -14,12 +14,16 @@
 //
 // Work split.  The rows are cut into row blocks of FREE_ROWS = 128 targets of one class; the (row block x source)
 // rectangle list is laid out linearly and cut into gridDim.x equal slabs, one per CTA, so every SM has the same
-// number of pairs whatever n is.  A CTA's slab touches one or two row blocks ("parts"); for each part the 16
+// number of pairs whatever n is.  A CTA's slab touches one or two row blocks ("parts"); for each part the
 // warps share the part's sources, every lane keeps FREE_NT = 4 targets of the block in registers and runs over
 // its warp's sources, which the warp stages 32 at a time in its own shared-memory buffer (no CTA-wide barrier in
-// the pair loop) and reads as warp-wide broadcasts.  The 16 warp sums are added in fixed order and go to a
+// the pair loop) and reads as warp-wide broadcasts.  The warp sums are added in fixed order and go to a
 // partial buffer in global memory (L2); after a grid barrier the owner of a row adds the (at most three)
 // partials of its row block, again in fixed order: the result is deterministic.
+//
+// Hybrid operator (s_off > 0).  The leading s_off x s_off block of the matrix is STORED and streamed by the caller
+// (bie_gmres.cu, bie_gemv.cuh "block ring"); this operator supplies the rest, an L-shaped region: row blocks below
+// s_off (s_off is a row-block boundary) take the sources [s_off, n), the others all sources.
 //
 // Near pairs.  den < taubar M_t (den/M_t = |e^{iw} - 1|^2 ~ |w|^2; this includes s == t) marks a pair as near:
 // it is left out of the fast sum by predication, and its exact entry (Laurent series of cot, or the analytic
@@ -38,26 +42,26 @@ constexpr int FREE_SRC_UNROLL = FREE_SRC_UNROLL_N;   // sources per unrolled ste
 #define FREE_WARPS (FREE_THREADS / 32)
 #define FREE_NT 4
 #define FREE_ROWS (32 * FREE_NT)
-#define FREE_STAGE_DOUBLES (FREE_WARPS * 2 * 4 * 32 * 2)   // room for the 4 staged arrays of bie_free_sym.cuh; 3 are used here
 
 // host-computed description of the work split (by value into the kernels)
 struct FreePlan {
     int M0;          // rows of class 0 = nodes of component 0
     int NB0, NB;     // row blocks of class 0, all row blocks
-    int UB;          // units (of 2 sources) per row block = (npad - s_off) / 2
-    long long U;     // NB * UB
+    int nb_below;    // row blocks entirely below s_off (hybrid operator; 0 otherwise)
+    int UBb, UBf;    // one-directional list: units (of 2 sources) of a block below s_off, (npad - s_off) / 2, and of the others, npad / 2
+    long long U;     // list length: nb_below UBb + (NB - nb_below) UBf, or the sources of the symmetric list
     int Geff;        // CTAs that take a slab (<= gridDim.x)
     int sym;         // 1: symmetric (oddness) work split of bie_free_sym.cuh: U = sources of the triangular list, PC valid
     double* PC;      // sym: [NB][npad] reverse partial sums (row block I, source s)
     const long long* sym_cum;   // sym: [NB + 1] sources before position k of the (permuted) triangular list
     const int* sym_perm;        // sym: [NB] row block at position k
     const int* sym_pos;         // sym: [NB] position of row block b
-    int sym_first;              // sym: first row block of the triangle (0; hybrid: the block that starts at s_off)
     int vortex;      // 1: the vortex-sheet matrix S (BIE_VARIANT_VORTEX) instead of Eq. (3.16); see free_parts
-    int s_off;       // first source of the operator (0; the hybrid operator reads the sources below it from its slab)
+    int s_off;       // hybrid operator: the leading s_off x s_off block comes from the caller's stored block (0: none)
+    int stage_buf;   // doubles of one staging buffer of a warp (free_stage_buf_doubles): fixes the shared-memory strides
     double2* T;      // [2][npad]: (U,W) class 0, (U,W) class 1     (vortex: (P,Q) = mu E, (R,B) = mu (M, 1))
-    double* SB;      // [2][FREE_SB_LD] per-CTA partials of sum_s beta_s x_s (class 0, class 1), written with the tables
-    double* PB;      // [(NB + Geff)][FREE_ROWS] partial sums, part id = row block + CTA
+    double* SB;      // [4][FREE_SB_LD] per-CTA partials of sum_s beta_s x_s: class 0 / 1 over s >= s_off, class 0 / 1 over s < s_off
+    double* PB;      // [(NB + Geff)][FREE_ROWS] partial sums, part id = list position of the row block + CTA
     const double* taubar;     // device scalar: near threshold relative to M_t (bie_near.cu)
     const int* near_ptr;      // CSR near matrix: offsets of the (row, segment) lists, row t = [ptr[8t], ptr[8t+8])
     const int* near_col;
@@ -65,17 +69,23 @@ struct FreePlan {
 };
 #define FREE_SB_LD 256   // >= gridDim.x (one CTA per SM, <= 256 SMs)
 
-// doubles of shared scratch, in this order: warp sums [16][128], component sums [BIE_MAX_COMP + 2], warp staging buffers
-// [16][2 stages][4][32] double2 (3 of the 4 arrays used by the one-directional loops), reverse-sum slots of bie_free_sym.cuh
-#define FREE_HEAD_DOUBLES (FREE_WARPS * FREE_ROWS + ((BIE_MAX_COMP + 2 + 1) & ~1))
-__host__ __device__ inline int free_scratch_doubles(int /*nthr*/)
+// doubles of shared scratch, in this order: warp sums [16][128]; component sums [2][BIE_MAX_COMP] and the four constants;
+// warp staging buffers [16][2 stages] of 32 sources: E, (U,W) (and (R,B) for the vortex-sheet matrix) as double2, and
+// the near thresholds of the symmetric loops as int; reverse-sum slots of bie_free_sym.cuh
+#define FREE_CSUM_DOUBLES (2 * BIE_MAX_COMP + 4)
+#define FREE_HEAD_DOUBLES (FREE_WARPS * FREE_ROWS + FREE_CSUM_DOUBLES)
+#ifndef SYM_BATCH
+#define SYM_BATCH 8
+#endif
+#define SYM_COL_STRIDE 33                                         // [SYM_BATCH][33] doubles per warp: lane-private slots, no bank conflicts
+#define SYM_COL_DOUBLES (FREE_WARPS * SYM_BATCH * SYM_COL_STRIDE)
+// one staging buffer of a warp (32 sources): E and (U,W) as double2; + (R,B) for the vortex-sheet matrix; + the near
+// thresholds (int) for the symmetric loops
+__host__ __device__ inline int free_stage_buf_doubles(bool vortex, bool sym) { return vortex ? 192 : (sym ? 144 : 128); }
+// shared scratch of the operator: head, [16 warps][2 buffers] staging, and the reverse-sum slots of the symmetric loops
+__host__ __device__ inline int free_scratch_doubles(bool vortex, bool sym)
 {
-    return FREE_HEAD_DOUBLES + FREE_STAGE_DOUBLES + FREE_WARPS * 8 * 33;
-}
-// what the one-directional loops (no bie_free_sym.cuh) need: the staging buffers hold 3 arrays
-__host__ __device__ inline int free_scratch_doubles_onedir()
-{
-    return FREE_HEAD_DOUBLES + FREE_WARPS * 2 * 3 * 32 * 2;
+    return FREE_HEAD_DOUBLES + FREE_WARPS * 2 * free_stage_buf_doubles(vortex, sym) + (sym ? SYM_COL_DOUBLES : 0);
 }
 
 __device__ __forceinline__ long long free_slab_start(const FreePlan& fp, int c)
@@ -92,15 +102,25 @@ __device__ __forceinline__ int free_block_rows(const FreePlan& fp, int b, int n)
     const int end = b < fp.NB0 ? fp.M0 : n;
     return min(FREE_ROWS, end - r0);
 }
+// one-directional list: first unit of row block b, and the block that holds unit u
+__device__ __forceinline__ long long free_list_start(const FreePlan& fp, int b)
+{
+    return b <= fp.nb_below ? (long long)b * fp.UBb : (long long)fp.nb_below * fp.UBb + (long long)(b - fp.nb_below) * fp.UBf;
+}
+__device__ __forceinline__ int free_list_block(const FreePlan& fp, long long u)
+{
+    const long long ub = (long long)fp.nb_below * fp.UBb;
+    return u < ub ? (int)(u / fp.UBb) : fp.nb_below + (int)((u - ub) / fp.UBf);
+}
 
 // ---- step 1: per-source tables for the vector v (rows [r0, r1) of this CTA; v indexed from r0) ------------
-// Also leaves this CTA's share of sum_{s >= s_off} beta_s x_s (per class) in fp.SB.  red: shared, >= 66 doubles.
-// All threads of the CTA must call; no barrier at the end (the caller's next barrier orders `red`).
+// Also leaves this CTA's shares of sum_s beta_s x_s (per class; s >= s_off and s < s_off) in fp.SB.
+// red: shared, >= 128 doubles.  All threads of the CTA must call; no barrier at the end (the caller's next barrier orders `red`).
 __device__ __forceinline__ void free_write_tables(const NodeTable& nt, const CompTable& ct, const FreePlan& fp, int r0,
                                                   int r1, const double* v /* shared or global, v[s - r0] */, double* red)
 {
     const int np = nt.npad;
-    double sb0 = 0.0, sb1 = 0.0;
+    double sb[4] = {0.0, 0.0, 0.0, 0.0};
     for (int s = r0 + threadIdx.x; s < r1; s += blockDim.x) {
         const double2 e = nt.E[s], q = nt.Q[s];
         const double x = v[s - r0];
@@ -120,25 +140,30 @@ __device__ __forceinline__ void free_write_tables(const NodeTable& nt, const Com
         a0 *= x; b0 *= x; a1 *= x; b1 *= x;
         fp.T[s]      = make_double2(fma(a0, e.y, 2.0 * b0 * e.x), fma(-a0, e.x, 2.0 * b0 * e.y));
         fp.T[np + s] = make_double2(fma(a1, e.y, 2.0 * b1 * e.x), fma(-a1, e.x, 2.0 * b1 * e.y));
-        if (s >= fp.s_off) { sb0 += b0; sb1 += b1; }
+        if (s >= fp.s_off) { sb[0] += b0; sb[1] += b1; } else { sb[2] += b0; sb[3] += b1; }
     }
     if (fp.vortex) return;
-    // fixed-order sum over the CTA: lanes by shuffle, warps by thread 0
+    // fixed-order sum over the CTA: lanes by shuffle, warps by threads 0..3
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
-    sb0 = bie_warp_sum(sb0); sb1 = bie_warp_sum(sb1);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) sb[q] = bie_warp_sum(sb[q]);
     __syncthreads();
-    if (lane == 0) { red[warp] = sb0; red[32 + warp] = sb1; }
+    if (lane == 0) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) red[32 * q + warp] = sb[q];
+    }
     __syncthreads();
-    if (threadIdx.x == 0) {
-        double t0 = 0.0, t1 = 0.0;
-        for (int w = 0; w < nwarp; ++w) { t0 += red[w]; t1 += red[32 + w]; }
-        fp.SB[blockIdx.x] = t0;
-        fp.SB[FREE_SB_LD + blockIdx.x] = t1;
+    if (threadIdx.x < 4) {
+        double t = 0.0;
+        for (int w = 0; w < nwarp; ++w) t += red[32 * threadIdx.x + w];
+        fp.SB[threadIdx.x * FREE_SB_LD + blockIdx.x] = t;
     }
 }
 
 // ---- step 2: this CTA's slab of the (row block x source) list -> partial sums in fp.PB --------------------
 // scratch: shared, free_scratch_doubles() doubles, 16-byte aligned.  All threads of the team must call.
+// poll() is called by every warp after each chunk of 32 sources (the hybrid operator consumes tiles of its stored
+// block there, bie_gemv.cuh).
 // VORTEX: the matrix S of Eqs. (4.14) + (4.17) (bie_build.cu, "Vortex-sheet variant"), in the (X, Y) form: entry x_s = (A_t X' + B_t Y')/den with
 // X' = Ei_t P_s - Er_t Q_s, Y' = R_s - M_t B_s from the class-independent tables (P,Q) = mu_s E_s, (R,B) = mu_s (M_s, 1), and the
 // row's (A_t, B_t) = (2u_i, -u_r) / +-(2u_r, u_i), u_t = zeta'_t/2, which depend on whether the SOURCE lies on Gamma_0: the
@@ -149,24 +174,25 @@ __device__ __forceinline__ void free_cp_async16(void* dst_shared, const void* sr
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(d), "l"(src_global), "r"(src_bytes) : "memory");
 }
 
-template <bool VORTEX>
+template <bool VORTEX, class Poll>
 __device__ __forceinline__ void free_parts_impl(const NodeTable& nt, const CompTable& ct, const FreePlan& fp, double* scratch,
-                                                const Team& team)
+                                                const Team& team, const Poll& poll)
 {
     const int lane = team.tid & 31, warp = team.warp;
     const int c = blockIdx.x;
     if (c >= fp.Geff) return;
     double* wsum = scratch;                                                       // [16][128]
-    double2* stage = reinterpret_cast<double2*>(scratch + FREE_HEAD_DOUBLES) + warp * (2 * 3 * 32);  // [2][3][32] double2 of this warp
+    double2* stage = reinterpret_cast<double2*>(scratch + FREE_HEAD_DOUBLES + warp * 2 * fp.stage_buf);  // this warp's 2 buffers
     const int np = nt.npad;
     const double taubar = __ldg(fp.taubar);
     long long u0 = free_slab_start(fp, c);
     const long long u1 = free_slab_start(fp, c + 1);
-    int b = (int)(u0 / fp.UB);
+    int b = free_list_block(fp, u0);
     while (u0 < u1) {
-        const long long ub = (long long)b * fp.UB;
-        const long long ue = min(u1, ub + fp.UB);
-        const int sa = fp.s_off + 2 * (int)(u0 - ub), sb = fp.s_off + 2 * (int)(ue - ub);  // sources [sa, sb) of row block b
+        const long long ub = free_list_start(fp, b);
+        const long long ue = min(u1, free_list_start(fp, b + 1));
+        const int sbase = b < fp.nb_below ? fp.s_off : 0;                        // first source of this block's list
+        const int sa = sbase + 2 * (int)(u0 - ub), sb = sbase + 2 * (int)(ue - ub);  // sources [sa, sb) of row block b
         const int cls = b < fp.NB0 ? 0 : 1;
         const int row0 = free_block_row0(fp, b);
         const int rows = free_block_rows(fp, b, nt.n);
@@ -200,7 +226,6 @@ __device__ __forceinline__ void free_parts_impl(const NodeTable& nt, const CompT
         const double2* TE = nt.E;
         const double2* TPQ = fp.T + (VORTEX ? (size_t)0 : (size_t)cls * np);   // Eq. (3.16): (U, W) of the rows' class
         const double2* TRB = fp.T + (size_t)np;                                 // VORTEX only
-        const double2 zero2 = make_double2(0.0, 0.0);
         for (int sgm = 0; sgm < (VORTEX ? 2 : 1); ++sgm) {
         // VORTEX: sources on Gamma_0 first, then the solids (different row coefficients); else the whole range at once
         const int wa = VORTEX ? (sgm == 0 ? wa_all : max(wa_all, fp.M0)) : wa_all;
@@ -211,7 +236,7 @@ __device__ __forceinline__ void free_parts_impl(const NodeTable& nt, const CompT
             const bool ok = s < wb;
             const int sc = ok ? s : wa;
             const unsigned sz = ok ? 16u : 0u;
-            double2* sg = stage + bufi * 96;
+            double2* sg = stage + bufi * (fp.stage_buf >> 1);
             free_cp_async16(sg + lane, TE + sc, sz);
             free_cp_async16(sg + 32 + lane, TPQ + sc, sz);
             if (VORTEX) free_cp_async16(sg + 64 + lane, TRB + sc, sz);
@@ -221,7 +246,7 @@ __device__ __forceinline__ void free_parts_impl(const NodeTable& nt, const CompT
         __syncwarp();
         if (wa < wb) issue(wa, 0);
         for (int base = wa; base < wb; base += 32, buf ^= 1) {
-            const double2* sg = stage + buf * 96;
+            const double2* sg = stage + buf * (fp.stage_buf >> 1);
             asm volatile("cp.async.wait_group 0;" ::: "memory");
             __syncwarp();                                   // chunk landed for all lanes; the other buffer is no longer read
             if (base + 32 < wb) issue(base + 32, buf ^ 1);
@@ -247,6 +272,7 @@ __device__ __forceinline__ void free_parts_impl(const NodeTable& nt, const CompT
                     if (!(__double2hiint(den) < thi[i])) acc[i] = fma(val, r, acc[i]);
                 }
             }
+            poll();
         }
         }
         // the warp sums, added in fixed order
@@ -264,47 +290,65 @@ __device__ __forceinline__ void free_parts_impl(const NodeTable& nt, const CompT
     }
 }
 
-__device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePlan& fp, double* scratch, const Team& team);
+template <class Poll>
+__device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePlan& fp, double* scratch, const Team& team,
+                                               const Poll& poll);
 
+template <class Poll>
 __device__ __forceinline__ void free_parts(const NodeTable& nt, const CompTable& ct, const FreePlan& fp, double* scratch,
-                                           const Team& team)
+                                           const Team& team, const Poll& poll)
 {
-    if (fp.sym) free_parts_sym(nt, fp, scratch, team);     // variants A/B; s_off = 0 or a row-block boundary
-    else if (fp.vortex) free_parts_impl<true>(nt, ct, fp, scratch, team);
-    else free_parts_impl<false>(nt, ct, fp, scratch, team);
+    if (fp.sym) free_parts_sym(nt, fp, scratch, team, poll);     // variants A/B; s_off = 0 or a row-block boundary
+    else if (fp.vortex) free_parts_impl<true>(nt, ct, fp, scratch, team, poll);
+    else free_parts_impl<false>(nt, ct, fp, scratch, team, poll);
 }
 
-// ---- step 3 (after a grid barrier): y_local[t - r0] = scale * (partials + near entries - E_k term) ---------
+// ---- step 3 (after a grid barrier): y_local[t - r0] = scale * (partials + near entries - constants - E_k term) ---------
 // xsrc: the vector of step 1 (global, complete).  All threads of the CTA must call; ends with __syncthreads.
 __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable& ct, const FreePlan& fp, int r0, int r1,
                                             const double* __restrict__ xsrc, double scale, double* scratch,
                                             double* y_local)
 {
-    double* csum = scratch + FREE_WARPS * FREE_ROWS;  // [ncomp]
-    double* wred = scratch;   // [nwarp] (the warp-sum area is free again)
+    double* csum = scratch + FREE_WARPS * FREE_ROWS;  // [2][BIE_MAX_COMP]: component sums over s >= s_off, over all s
+    double* sbs = csum + 2 * BIE_MAX_COMP;            // [4] constants (free_write_tables)
+    double* wred = scratch;   // [2][32] (the warp-sum area is free again)
     {   // sum of x over each OBSTACLE component (em != 0) that owns one of this CTA's rows: all warps share the
-        // component, lanes strided, warp sums added in fixed order -- every CTA gets the same bits
+        // component, lanes strided, warp sums added in fixed order -- every CTA gets the same bits.  Rows below s_off
+        // (hybrid) only want the sources from s_off on, the stored block has the others.
         const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
         for (int k = 0; k < ct.ncomp; ++k) {
             if (!(ct.off[k] < r1 && ct.off[k + 1] > r0)) continue;      // CTA-uniform
-            if (nt.DG[ct.off[k]].y == 0.0) { if (threadIdx.x == 0) csum[k] = 0.0; continue; }
-            double s = 0.0;
-            for (int i = max(ct.off[k], fp.s_off) + threadIdx.x; i < ct.off[k + 1]; i += blockDim.x) s += __ldcg(xsrc + i);
-            s = bie_warp_sum(s);
-            if (lane == 0) wred[warp] = s;
+            if (nt.DG[ct.off[k]].y == 0.0) { if (threadIdx.x == 0) { csum[k] = 0.0; csum[BIE_MAX_COMP + k] = 0.0; } continue; }
+            double shi = 0.0, slo = 0.0;
+            for (int i = ct.off[k] + threadIdx.x; i < ct.off[k + 1]; i += blockDim.x) {
+                const double xv = __ldcg(xsrc + i);
+                if (i >= fp.s_off) shi += xv; else slo += xv;
+            }
+            shi = bie_warp_sum(shi); slo = bie_warp_sum(slo);
+            if (lane == 0) { wred[warp] = shi; wred[32 + warp] = slo; }
             __syncthreads();
             if (threadIdx.x == 0) {
-                double tsum = 0.0;
-                for (int w = 0; w < nwarp; ++w) tsum += wred[w];
-                csum[k] = tsum;
+                double th = 0.0, tl = 0.0;
+                for (int w = 0; w < nwarp; ++w) { th += wred[w]; tl += wred[32 + w]; }
+                csum[k] = th;
+                csum[BIE_MAX_COMP + k] = th + tl;
             }
             __syncthreads();
         }
     }
+    // sum_s beta_s x_s per class and source range: the per-CTA partials of free_write_tables in fixed order (warps 0..3)
+    if (!fp.vortex && threadIdx.x < 128) {
+        const int q = threadIdx.x >> 5, lane = threadIdx.x & 31;
+        double sb = 0.0;
+        for (int i = lane; i < (int)gridDim.x; i += 32) sb += __ldcg(fp.SB + q * FREE_SB_LD + i);
+        sb = bie_warp_sum(sb);
+        if (lane == 0) sbs[q] = sb;
+    }
     __syncthreads();
-    // symmetric work split: row t of block J also receives sum_{I < J} PC[I][t].  These are up to NB - 1 loads per row, each
-    // from another L2 line: four threads share a row (I = q, q + 4, ...; eight loads in flight each) and the four partial
-    // sums are added in fixed order.  rsum lives in the staging area (free again; fp.sym => the full scratch).
+    // symmetric work split: row t of block J also receives sum_{I < J} PC[I][t] (rows below s_off: nothing, their mirror
+    // entries are stored).  These are up to NB - 1 loads per row, each from another L2 line: four threads share a row
+    // (I = q, q + 4, ...; eight loads in flight each) and the four partial sums are added in fixed order.  rsum lives in
+    // the staging area (free again; fp.sym => the full scratch).
     double* rsum = scratch + FREE_HEAD_DOUBLES;   // [rows]
     if (fp.sym) {
         double* rpart = rsum + ((r1 - r0 + 1) & ~1);   // [4][rows]
@@ -312,10 +356,10 @@ __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable
         for (int w = threadIdx.x; w < 4 * rows; w += blockDim.x) {
             const int q = w / rows, lr = w - q * rows;
             const int t = r0 + lr;
-            const int b = t < fp.M0 ? t / FREE_ROWS : fp.NB0 + (t - fp.M0) / FREE_ROWS;
+            const int b = t < fp.s_off ? 0 : (t < fp.M0 ? t / FREE_ROWS : fp.NB0 + (t - fp.M0) / FREE_ROWS);
             const double* pc = fp.PC + t;
             double a0 = 0.0, a1 = 0.0;
-            int I = fp.sym_first + q;
+            int I = q;
             for (; I + 28 < b; I += 32) {
                 double v[8];
 #pragma unroll
@@ -331,23 +375,13 @@ __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable
             rsum[lr] = (rpart[lr] + rpart[rows + lr]) + (rpart[2 * rows + lr] + rpart[3 * rows + lr]);
         __syncthreads();
     }
-    // sum_s beta_s x_s per class: the per-CTA partials of free_write_tables in fixed order (warp 0 and 1), via shared memory
-    double* sbs = scratch + FREE_WARPS * FREE_ROWS + ((BIE_MAX_COMP + 2 + 1) & ~1) - 2;   // the two doubles after csum[BIE_MAX_COMP]
-    if (!fp.vortex && threadIdx.x < 64) {
-        const int c = threadIdx.x >> 5, lane = threadIdx.x & 31;
-        double sb = 0.0;
-        for (int i = lane; i < (int)gridDim.x; i += 32) sb += __ldcg(fp.SB + c * FREE_SB_LD + i);
-        sb = bie_warp_sum(sb);
-        if (lane == 0) sbs[c] = sb;
-    }
-    __syncthreads();
     for (int t = r0 + threadIdx.x; t < r1; t += blockDim.x) {
         int b, off;
         if (t < fp.M0) { b = t / FREE_ROWS; off = t - b * FREE_ROWS; }
         else { const int d = t - fp.M0; b = d / FREE_ROWS; off = d - b * FREE_ROWS; b += fp.NB0; }
         const int kpos = fp.sym ? __ldg(fp.sym_pos + b) : b;   // position of the block in the work list
-        const long long X0 = fp.sym ? __ldg(fp.sym_cum + kpos) : (long long)b * fp.UB;
-        const long long X1 = fp.sym ? __ldg(fp.sym_cum + kpos + 1) : X0 + fp.UB;
+        const long long X0 = fp.sym ? __ldg(fp.sym_cum + kpos) : free_list_start(fp, b);
+        const long long X1 = fp.sym ? __ldg(fp.sym_cum + kpos + 1) : free_list_start(fp, b + 1);
         int c_lo = (int)(((X0 + 1) * fp.Geff + fp.U - 1) / fp.U) - 1;
         int c_hi = (int)((X1 * fp.Geff + fp.U - 1) / fp.U) - 1;
         c_lo = max(c_lo, 0); c_hi = min(c_hi, fp.Geff - 1);
@@ -357,17 +391,21 @@ __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable
             if (a < e) s += __ldcg(fp.PB + (size_t)(kpos + c) * FREE_ROWS + off);
         }
         if (fp.sym) s += rsum[t - r0];   // reverse partials of the earlier row blocks (summed above)
-        // near pairs: exact entries from the CSR near matrix
+        // near pairs: exact entries from the CSR near matrix (rows below s_off: only the columns the stored block lacks)
+        const bool below = (t < fp.s_off);
         const int p0 = fp.near_ptr[8 * (size_t)t], p1 = fp.near_ptr[8 * (size_t)t + 8];
         double sn = 0.0;
         for (int p = p0; p < p1; ++p) {
             const int cix = fp.near_col[p];
-            if (cix >= fp.s_off) sn = fma(fp.near_val[p], __ldcg(xsrc + cix), sn);
+            if (!below || cix >= fp.s_off) sn = fma(fp.near_val[p], __ldcg(xsrc + cix), sn);
         }
         s += sn;
-        if (!fp.vortex) s -= sbs[t < fp.M0 ? 0 : 1];
+        if (!fp.vortex) {
+            const int cl = t < fp.M0 ? 0 : 1;
+            s -= below ? sbs[cl] : (sbs[cl] + sbs[2 + cl]);
+        }
         const int k = nt.COMP[t];
-        s = fma(-nt.DG[t].y, csum[k], s);
+        s = fma(-nt.DG[t].y, csum[(below ? 0 : BIE_MAX_COMP) + k], s);
         y_local[t - r0] = s * scale;
     }
     __syncthreads();

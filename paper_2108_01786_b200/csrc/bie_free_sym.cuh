@@ -14,14 +14,15 @@
 // shuffle butterfly was 3 % slower: its 9 dependent steps stall the warp).
 // Near pairs: forward skipped when den < taubar M_t, reverse when den < taubar M_s -- the row-based rule of bie_near.cu,
 // whose CSR matrix supplies both.
+// Hybrid operator (fp.s_off > 0, a row-block boundary): the leading s_off x s_off block is stored; every other pair {t, s},
+// t < s, has s >= s_off, so the list is the same triangle with the sources cut at s_off: row blocks below s_off take the
+// sources [s_off, npad) symmetrically (forward into their rows, reverse into the rows from s_off on).
 #pragma once
 #include "bie_free.cuh"
 
-#define SYM_BATCH 8
-
 // The triangular list is laid out in the order perm[0], perm[1], ... = 0, NB-1, 1, NB-2, ... (long and short source lists
 // alternate, so that every CTA's slab holds one or two long parts and at most a few short ones); cum[k] = sources before
-// position k.  Host-computed tables in device memory (FreePlan::sym_cum / sym_perm / sym_pos).
+// position k.  Tables in device memory (FreePlan::sym_cum / sym_perm / sym_pos, bie_nodes.cu).
 __device__ __forceinline__ int sym_find_pos(const FreePlan& fp, long long u)
 {
     int lo = 0, hi = fp.NB - 1;   // largest k with cum[k] <= u
@@ -32,22 +33,19 @@ __device__ __forceinline__ int sym_find_pos(const FreePlan& fp, long long u)
     return lo;
 }
 
-#define SYM_STAGE_DOUBLES (FREE_WARPS * 2 * 4 * 32 * 2)   // [16 warps][2 buffers][4 arrays][32] double2
-#define SYM_COL_STRIDE 33                                  // [SYM_BATCH][33] doubles per warp: lane-private slots, no bank conflicts
-#define SYM_COL_DOUBLES (FREE_WARPS * SYM_BATCH * SYM_COL_STRIDE)
-
 // this CTA's slab of the triangular (row block x later sources) list -> forward partials in fp.PB, reverse partials in fp.PC.
-// scratch: shared, free_scratch_doubles() doubles.  All threads of the team must call.
-// Hybrid operator (fp.s_off > 0, a row-block boundary): row blocks below s_off take the sources [s_off, npad) one-directionally
-// (their mirror entries are in the stored slab); the row blocks from s_off on form the triangle.
-__device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePlan& fp, double* scratch, const Team& team)
+// scratch: shared, free_scratch_doubles(false, true) doubles.  All threads of the team must call.  poll(): see free_parts_impl.
+template <class Poll>
+__device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePlan& fp, double* scratch, const Team& team,
+                                               const Poll& poll)
 {
     const int lane = team.tid & 31, warp = team.warp, nwarp = team.nwarp;
     const int c = blockIdx.x;
     if (c >= fp.Geff) return;
     double* wsum = scratch;
-    double2* stage = reinterpret_cast<double2*>(scratch + FREE_HEAD_DOUBLES) + warp * (2 * 4 * 32);
-    double* col = scratch + FREE_HEAD_DOUBLES + SYM_STAGE_DOUBLES + warp * (SYM_BATCH * SYM_COL_STRIDE);   // this warp's reverse sums of a batch
+    const int sbuf = fp.stage_buf;                                   // 144 doubles: E [32] double2, (U,W) [32] double2, thresholds [32] int
+    double* stage = scratch + FREE_HEAD_DOUBLES + warp * 2 * sbuf;
+    double* col = scratch + FREE_HEAD_DOUBLES + FREE_WARPS * 2 * sbuf + warp * (SYM_BATCH * SYM_COL_STRIDE);   // this warp's reverse sums of a batch
     const int np = nt.npad;
     const double taubar = __ldg(fp.taubar);
     long long u0 = (long long)c * fp.U / fp.Geff;
@@ -61,7 +59,7 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
         const int cls = b < fp.NB0 ? 0 : 1;
         const int row0 = free_block_row0(fp, b);
         const int rows = free_block_rows(fp, b, nt.n);
-        const bool below = (row0 + rows <= fp.s_off);        // hybrid: a row block of the slab's columns
+        const bool below = (row0 + rows <= fp.s_off);        // hybrid: a row block of the stored block's rows
         const int src0 = below ? fp.s_off : row0;
         const int sa = src0 + (int)(u0 - ub), sb = src0 + (int)(ue - ub);   // sources [sa, sb), all >= src0
         double ter[FREE_NT], tei[FREE_NT], acc[FREE_NT];
@@ -78,8 +76,8 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
         const int span = sb - sa;
         const int wa_all = sa + (int)((long long)span * warp / nwarp);
         const int wb_all = sa + (int)((long long)span * (warp + 1) / nwarp);
-        const int d_end = below ? np : row0 + rows;           // end of the one-directional sources (the block's own rows)
-        const int c_end = below ? np : ((cls == 0) ? fp.M0 : np);   // end of the sources of the block's own class
+        const int d_end = below ? src0 : row0 + rows;         // end of the one-directional sources (the block's own rows)
+        const int c_end = (cls == 0) ? max(fp.M0, src0) : np; // end of the sources of the block's own class
         const double2* TUW = fp.T + (size_t)cls * np;            // forward tables: (U, W) for the class of the block's rows
         for (int sgm = 0; sgm < 3; ++sgm) {
             // 0: own rows (one direction); 1: later sources of the same class; 2: sources on solids below a Gamma_0 block
@@ -99,24 +97,26 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
                     tu[i] = uw.x; tw[i] = uw.y;
                 }
             }
-            double2 ne = zero2, nuw = zero2, nmt = zero2;
+            double2 ne = zero2, nuw = zero2;
+            int nth = 0;
             if (wa + lane < wb) {
                 const int s = wa + lane;
                 ne = nt.E[s]; nuw = __ldcg(TUW + s);
-                const double M = nt.MT[s].x; nmt = make_double2(M, taubar * M);
+                nth = __double2hiint(taubar * nt.MT[s].x);
             }
             int buf = 0;
             __syncwarp();
             for (int base = wa; base < wb; base += 32, buf ^= 1) {
-                double2* sg = stage + buf * 128;
-                sg[lane] = ne; sg[32 + lane] = nuw; sg[96 + lane] = nmt;
+                double2* sg = reinterpret_cast<double2*>(stage + buf * sbuf);
+                int* sth = reinterpret_cast<int*>(stage + buf * sbuf + 128);
+                sg[lane] = ne; sg[32 + lane] = nuw; sth[lane] = nth;
                 __syncwarp();
                 {
                     const int s = base + 32 + lane;
-                    ne = zero2; nuw = zero2; nmt = zero2;
+                    ne = zero2; nuw = zero2; nth = 0;
                     if (s < wb) {
                         ne = nt.E[s]; nuw = __ldcg(TUW + s);
-                        const double M = nt.MT[s].x; nmt = make_double2(M, taubar * M);
+                        nth = __double2hiint(taubar * nt.MT[s].x);
                     }
                 }
                 const int cnt = min(32, wb - base);
@@ -138,8 +138,8 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
 #pragma unroll
                         for (int u = 0; u < SYM_BATCH; ++u) {
                             const int j = j0 + u;
-                            const double2 e = sg[j], uw = sg[32 + j], mt = sg[96 + j];
-                            const int thj = __double2hiint(mt.y);
+                            const double2 e = sg[j], uw = sg[32 + j];
+                            const int thj = sth[j];
                             double s_rev0 = 0.0, s_rev1 = 0.0;
 #pragma unroll
                             for (int i = 0; i < FREE_NT; ++i) {
@@ -156,20 +156,25 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
                             }
                             col[u * SYM_COL_STRIDE + lane] = -(s_rev0 + s_rev1);
                         }
-                        // lane reduction of the 8 reverse sums through shared memory: lane l adds the slots 8 (l & 3) .. + 7 of
-                        // source l >> 2, two shuffles finish (fixed order)
+                        // lane reduction of the SYM_BATCH reverse sums through shared memory: 32 / SYM_BATCH lanes share a source,
+                        // each adds 8 slots, shuffles finish (fixed order)
                         __syncwarp();
                         {
-                            const double* cp = col + (lane >> 2) * SYM_COL_STRIDE + 8 * (lane & 3);
-                            double v = ((cp[0] + cp[1]) + (cp[2] + cp[3])) + ((cp[4] + cp[5]) + (cp[6] + cp[7]));
-                            v += __shfl_xor_sync(0xffffffffu, v, 2);
-                            v += __shfl_xor_sync(0xffffffffu, v, 1);
-                            const int j = j0 + (lane >> 2);
-                            if ((lane & 3) == 0 && j < cnt) fp.PC[(size_t)b * np + base + j] = v;
+                            constexpr int LPS = 32 / SYM_BATCH;                 // lanes per source (4 for a batch of 8)
+                            constexpr int SPL = 32 / LPS;                        // slots per lane (8)
+                            const double* cp = col + (lane / LPS) * SYM_COL_STRIDE + SPL * (lane % LPS);
+                            double v = 0.0;
+#pragma unroll
+                            for (int q = 0; q < SPL; q += 2) v += cp[q] + cp[q + 1];
+#pragma unroll
+                            for (int o = LPS >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                            const int j = j0 + lane / LPS;
+                            if ((lane % LPS) == 0 && j < cnt) fp.PC[(size_t)b * np + base + j] = v;
                         }
                         __syncwarp();
                     }
                 }
+                poll();
             }
         }
         // the warp sums of the forward direction, added in fixed order

@@ -137,3 +137,195 @@ __device__ __forceinline__ void bie_cta_gemv(const double* __restrict__ A, long 
     }
     team_sync(tm);
 }
+
+// ---------------------------------------------------------------------------------------------------
+// Block ring of the hybrid operator (bie_gmres.cu): the stored leading block A[0:nd, 0:nd) arrives in shared memory
+// by bulk copies (cp.async.bulk, the TMA engine) issued by ONE thread, as tiles of RING_ROWS rows x one column chunk
+// TOGETHER with the chunk of x they multiply, into a ring of RING_STAGES buffers guarded by mbarriers.  No warp has
+// to keep loads in flight: the warps that run the pair loops of the recomputed part consume landed tiles between
+// their source chunks (they own the issue slots; a tile costs about 150 instructions), claim them through a shared
+// counter and leave the tile's row sums in `part`, one slot per (chunk, row): the result does not depend on which
+// warp took which tile.  Every CTA streams an equal share of the block's rows, whoever owns them in the solve.
+// ---------------------------------------------------------------------------------------------------
+#ifndef RING_STAGES
+#define RING_STAGES 4
+#endif
+#define RING_ROWS 4
+
+// doubles per (row, chunk) of a ring tile: at most 512 (a tile = 4 rows + x = 20 KB), smaller while the CTA has fewer
+// than two tiles per warp; a multiple of 64 (bulk copies need 16-byte sizes and addresses)
+__host__ __device__ inline int ring_chunk(int rows_per_cta, int nd, int nwarp)
+{
+    int chunk = 512;
+    const int ngrp = (rows_per_cta + RING_ROWS - 1) / RING_ROWS;
+    while (chunk > 128 && ngrp * ((nd + chunk - 1) / chunk) < 2 * nwarp) chunk >>= 1;
+    const int nch = (nd + chunk - 1) / chunk;
+    chunk = ((nd + nch - 1) / nch + 63) & ~63;
+    return chunk;
+}
+// shared memory of the ring: RING_STAGES tiles of (RING_ROWS + 1) x chunk doubles, then 2 RING_STAGES mbarriers and the
+// tile counter (padded to an even number of doubles)
+__host__ __device__ inline int ring_doubles(int chunk) { return RING_STAGES * (RING_ROWS + 1) * chunk + 2 * RING_STAGES + 2; }
+// row sums of the tiles: [chunks][rows rounded up to RING_ROWS]
+__host__ __device__ inline int ring_part_doubles(int rows_per_cta, int nd, int chunk)
+{
+    return ((nd + chunk - 1) / chunk) * (((rows_per_cta + RING_ROWS - 1) / RING_ROWS) * RING_ROWS);
+}
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_test(unsigned bar, unsigned parity)
+{
+    unsigned ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
+{
+    while (!mbar_test(bar, parity)) { }
+}
+// bulk copy global -> shared of `bytes` (multiple of 16; both addresses 16-byte aligned), completion on `bar`
+template <bool HINT>
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar, unsigned long long pol)
+{
+    if (HINT)
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                     :: "r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
+    else
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     :: "r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+
+struct BlockRing {
+    const double* A;          // stored block, row-major, leading dimension lda
+    long long lda;
+    int nd, r0, r1, chunk;    // columns (= rows) of the block, the rows this CTA streams, doubles per (row, chunk)
+    int nch, nunit;           // chunks per row, tiles of one application
+    unsigned full0, empty0;   // shared addresses of the mbarriers: full[s] = full0 + 8 s, empty[s] = empty0 + 8 s
+    int* next;                // shared: next tile to claim
+    const double* stage;      // shared: RING_STAGES tiles of (RING_ROWS + 1) x chunk doubles (rows, then x)
+    double* part;             // shared: [nch][rowsP] row sums of the tiles
+    int rowsP;
+    unsigned long long tile0; // tiles issued before this application (ring position and phase run on across applications)
+};
+
+// all threads of the CTA, once per kernel
+__device__ __forceinline__ void ring_init(double* ring_mem, int chunk)
+{
+    if (threadIdx.x == 0) {
+        const unsigned b = smem_u32(ring_mem + RING_STAGES * (RING_ROWS + 1) * chunk);
+        for (int s = 0; s < 2 * RING_STAGES; ++s) mbar_init(b + 8 * s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+}
+
+// ONE thread: every tile of the application, in unit order, as ring slots become free
+template <bool STREAM>
+__device__ __forceinline__ void ring_produce(const BlockRing& R, const double* xin)
+{
+    unsigned long long pol = 0;
+    if (STREAM) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    const unsigned stage_addr = smem_u32(R.stage);
+    for (int t = 0; t < R.nunit; ++t) {
+        const unsigned long long gidx = R.tile0 + t;
+        const unsigned s = (unsigned)(gidx % RING_STAGES), use = (unsigned)(gidx / RING_STAGES);
+        mbar_wait(R.empty0 + 8 * s, (use & 1u) ^ 1u);
+        const int p = t / R.nch, ch = t - p * R.nch;
+        const int ra = R.r0 + RING_ROWS * p;
+        const int nr = min(RING_ROWS, R.r1 - ra);
+        const int cbeg = ch * R.chunk, cend = min(cbeg + R.chunk, R.nd);
+        const unsigned bytes = 8u * (unsigned)(cend - cbeg);
+        const unsigned dst = stage_addr + s * (unsigned)(8 * (RING_ROWS + 1) * R.chunk);
+        mbar_arrive_expect_tx(R.full0 + 8 * s, (unsigned)(nr + 1) * bytes);
+        for (int i = 0; i < nr; ++i)
+            bulk_g2s<STREAM>(dst + 8u * (unsigned)(i * R.chunk), R.A + (long long)(ra + i) * R.lda + cbeg, bytes, R.full0 + 8 * s, pol);
+        bulk_g2s<false>(dst + 8u * (unsigned)(RING_ROWS * R.chunk), xin + cbeg, bytes, R.full0 + 8 * s, 0);   // x: L2-resident
+    }
+}
+
+// a whole warp: claims the next tile; returns false when none is left.  Blocks until the tile has landed.
+__device__ __forceinline__ bool ring_consume(const BlockRing& R)
+{
+    const int lane = threadIdx.x & 31;
+    int t = 0;
+    if (lane == 0) t = atomicAdd(R.next, 1);
+    t = __shfl_sync(0xffffffffu, t, 0);
+    if (t >= R.nunit) return false;
+    const unsigned long long gidx = R.tile0 + t;
+    const unsigned s = (unsigned)(gidx % RING_STAGES), use = (unsigned)(gidx / RING_STAGES);
+    const int p = t / R.nch, ch = t - p * R.nch;
+    const int nr = min(RING_ROWS, R.r1 - (R.r0 + RING_ROWS * p));
+    const int cbeg = ch * R.chunk, cend = min(cbeg + R.chunk, R.nd);
+    const int n2 = (cend - cbeg) >> 1;
+    mbar_wait(R.full0 + 8 * s, use & 1u);
+    const double2* a = reinterpret_cast<const double2*>(R.stage + (size_t)s * (RING_ROWS + 1) * R.chunk);
+    const int ch2 = R.chunk >> 1;
+    const double2* x2 = a + RING_ROWS * ch2;
+    double acc[RING_ROWS], bcc[RING_ROWS];
+#pragma unroll
+    for (int i = 0; i < RING_ROWS; ++i) { acc[i] = 0.0; bcc[i] = 0.0; }
+    // rows the tile does not have are read anyway (stale shared memory, finite or not) and their sums dropped
+    int c = lane;
+    for (; c + 32 < n2; c += 64) {
+        const double2 xa = x2[c], xb = x2[c + 32];
+        double2 va[RING_ROWS], vb[RING_ROWS];
+#pragma unroll
+        for (int i = 0; i < RING_ROWS; ++i) { va[i] = a[i * ch2 + c]; vb[i] = a[i * ch2 + c + 32]; }
+#pragma unroll
+        for (int i = 0; i < RING_ROWS; ++i) {
+            acc[i] = fma(va[i].x, xa.x, acc[i]); bcc[i] = fma(va[i].y, xa.y, bcc[i]);
+            acc[i] = fma(vb[i].x, xb.x, acc[i]); bcc[i] = fma(vb[i].y, xb.y, bcc[i]);
+        }
+    }
+    for (; c < n2; c += 32) {
+        const double2 xa = x2[c];
+#pragma unroll
+        for (int i = 0; i < RING_ROWS; ++i) {
+            const double2 va = a[i * ch2 + c];
+            acc[i] = fma(va.x, xa.x, acc[i]); bcc[i] = fma(va.y, xa.y, bcc[i]);
+        }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(R.empty0 + 8 * s);     // the slot may be refilled
+#pragma unroll
+    for (int i = 0; i < RING_ROWS; ++i) {
+        const double v = bie_warp_sum(acc[i] + bcc[i]);
+        if (lane == 0 && i < nr) R.part[ch * R.rowsP + RING_ROWS * p + i] = v;
+    }
+    return true;
+}
+
+// a whole warp, between two source chunks of its pair loop: takes up to `max_tiles` tiles that have ALREADY landed.
+// Not inlined: the pair loops around the call keep their register allocation.
+static __device__ __noinline__ void ring_poll(const BlockRing& R, int max_tiles)
+{
+    for (int k = 0; k < max_tiles; ++k) {
+        const int t = *reinterpret_cast<volatile int*>(R.next);
+        if (t >= R.nunit) return;
+        const unsigned long long gidx = R.tile0 + t;
+        if (!mbar_test(R.full0 + 8 * (unsigned)(gidx % RING_STAGES), (unsigned)(gidx / RING_STAGES) & 1u)) return;
+        if (!ring_consume(R)) return;
+    }
+}
+
+// what the pair loops of bie_free.cuh call between source chunks
+struct NoPoll { __device__ __forceinline__ void operator()() const {} };
+struct RingPoll {
+    const BlockRing* R;
+    int max_tiles;
+    __device__ __forceinline__ void operator()() const { ring_poll(*R, max_tiles); }
+};

@@ -32,8 +32,9 @@
 #ifndef GM_THREADS
 #define GM_THREADS 512
 #endif
-#ifndef HYB_GEMV_UNROLL
-#define HYB_GEMV_UNROLL 8   // hybrid operator: 2 rows x 8 LDG.128 per lane in flight in each streaming warp
+#define GM_WARPS (GM_THREADS / 32)
+#ifndef RING_POLL_TILES
+#define RING_POLL_TILES 3   // hybrid operator: tiles of the stored block a warp may take between two source chunks
 #endif
 
 struct GmresArgs {
@@ -59,8 +60,11 @@ struct GmresArgs {
     int rows_per_cta;
     int chunk;
     int VS;        // Krylov vectors 0..VS-1 keep this CTA's rows in shared memory; the others in V (global, L2)
-    int nd;        // hybrid operator: columns [0, nd) come from the stored slab A, sources [nd, n) are recomputed
-    int nwf;       // hybrid operator: warps 0..nwf-1 run the pair loops, the others stream the slab
+    int nd;        // hybrid operator: the leading nd x nd block comes from the stored block A, everything else is recomputed
+    int nwf;       // hybrid operator: warps 0..nwf-1 run the pair loops (and take tiles of the stored block in between), warps
+                   // nwf..14 only take tiles, warp 15 issues the bulk copies
+    int brows;     // hybrid operator: rows of the stored block each CTA streams (a multiple of RING_ROWS)
+    double* yd;    // hybrid operator: [nld] product of the stored block with x[0, nd), written by the CTAs that streamed the rows
     int res_pairs; // streaming GEMV: leading row pairs of every CTA block kept L2-resident (bie_gemv.cuh)
     int scratch_doubles;  // matrix-free scratch in shared memory (full, or the smaller one of the one-directional loops)
     NodeTable nt;
@@ -103,12 +107,12 @@ __device__ __forceinline__ unsigned long long gtime() { unsigned long long t; as
 #define PT(i)
 #endif
 
-// MODE: 0 = stored matrix (GEMV, HBM-bound), 1 = matrix-free (pair loops, FP64-bound), 2 = hybrid: the first a.nd
-// columns are read from the stored slab by the streaming warps WHILE the other warps recompute the remaining
-// sources -- the HBM pipe and the FP64 pipe of every SM work at the same time.
+// MODE: 0 = stored matrix (GEMV, HBM-bound), 1 = matrix-free (pair loops, FP64-bound), 2 = hybrid: the leading
+// nd x nd block is stored and arrives through the block ring of bie_gemv.cuh WHILE the warps recompute every other
+// entry -- the HBM pipe and the FP64 pipe of every SM work at the same time.
 template <bool STREAM, bool XS, int MODE>
 __device__ __forceinline__ void cta_apply(const GmresArgs& a, int r0, int r1, const double* xin, double scale,
-                                          double* xs, double* gpart, double* gpart2, double* ydense, double* y_local,
+                                          double* xs, double* gpart, BlockRing& ring, double* y_local,
                                           bool tables_ready, double* red, unsigned int& target)
 {
     if (MODE != 0) {
@@ -119,25 +123,32 @@ __device__ __forceinline__ void cta_apply(const GmresArgs& a, int r0, int r1, co
             grid_barrier(a.sync, target);
         }
         if (MODE == 1) {
-            free_parts(a.nt, a.ct, a.fp, gpart, cta_team());
+            free_parts(a.nt, a.ct, a.fp, gpart, cta_team(), NoPoll());
         } else {
-            const int warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
-            if (warp < a.nwf) {
-                free_parts(a.nt, a.ct, a.fp, gpart, sub_team(0, a.nwf, 1));
+            const int warp = threadIdx.x >> 5;
+            if (threadIdx.x == 0) *ring.next = 0;
+            __syncthreads();
+            if (warp == GM_WARPS - 1) {
+                if ((threadIdx.x & 31) == 0) ring_produce<STREAM>(ring, xin);
+                __syncwarp();
             } else {
-                const Team st = sub_team(a.nwf, nwarp - a.nwf, 2);
-                const int nd2 = a.nd >> 1;   // nd is even
-                for (int i = st.tid; i < nd2; i += st.nthr)
-                    reinterpret_cast<double2*>(xs)[i] = __ldcg(reinterpret_cast<const double2*>(xin) + i);
-                team_sync(st);
-                bie_cta_gemv<STREAM, true, HYB_GEMV_UNROLL>(a.A, a.lda, a.nd, r0, r1, a.chunk, xs, gpart2, ydense, st);
+                if (warp < a.nwf) free_parts(a.nt, a.ct, a.fp, gpart, sub_team(0, a.nwf, 1), RingPoll{&ring, RING_POLL_TILES});
+                while (ring_consume(ring)) { }
             }
             __syncthreads();
+            // the rows of the stored block this CTA streamed: chunk sums in fixed order -> yd (their owners read it after the barrier)
+            for (int r = threadIdx.x; r < ring.r1 - ring.r0; r += blockDim.x) {
+                double sum = 0.0;
+                for (int ch = 0; ch < ring.nch; ++ch) sum += ring.part[ch * ring.rowsP + r];
+                a.yd[ring.r0 + r] = sum;
+            }
+            ring.tile0 += (unsigned long long)ring.nunit;
         }
         grid_barrier(a.sync, target);
         free_gather(a.nt, a.ct, a.fp, r0, r1, xin, scale, gpart, y_local);
         if (MODE == 2) {
-            for (int r = threadIdx.x; r < r1 - r0; r += blockDim.x) y_local[r] = fma(scale, ydense[r], y_local[r]);
+            for (int r = threadIdx.x; r < r1 - r0; r += blockDim.x)
+                if (r0 + r < a.nd) y_local[r] = fma(scale, __ldcg(a.yd + r0 + r), y_local[r]);
             __syncthreads();
         }
     } else if (XS) {
@@ -257,10 +268,10 @@ __device__ __forceinline__ void reduce_partials(const double* part_slot, int cnt
 __device__ __forceinline__ int hess_off(int i) { return (i * (i + 3)) >> 1; }
 
 // doubles of shared memory before the operator's scratch: y, w [rows2 each], hcol, hloc, cvec [m + 2 each], cs, sn [m each],
-// g [m + 1], red [66], the packed single-precision Hbar [m (m + 3) / 2 floats]; rounded to 16 bytes
+// g [m + 1], red [130], the packed single-precision Hbar [m (m + 3) / 2 floats]; rounded to 16 bytes
 __host__ __device__ inline int gm_head_doubles(int m, int rows2)
 {
-    int o = 2 * rows2 + 3 * (m + 2) + 2 * m + (m + 1) + 66;
+    int o = 2 * rows2 + 3 * (m + 2) + 2 * m + (m + 1) + 130;
     o += (m * (m + 3) / 2 + 1) / 2;
     return (o + 1) & ~1;
 }
@@ -285,14 +296,30 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
     double* cs = cvec + (m + 2);          // [m]
     double* sn = cs + m;                  // [m]
     double* g = sn + m;                   // [m+1]
-    double* red = g + (m + 1);            // [66]
-    float* Hf = reinterpret_cast<float*>(red + 66);                  // packed Hbar in single precision, m (m + 3) / 2 floats
+    double* red = g + (m + 1);            // [130]
+    float* Hf = reinterpret_cast<float*>(red + 130);                 // packed Hbar in single precision, m (m + 3) / 2 floats
     double* gpart = smem + gm_head_doubles(m, rows2);                // GEMV partials or matrix-free scratch (16-byte aligned)
-    // hybrid: GEMV partials of the slab and its result, after the matrix-free scratch
-    double* gpart2 = gpart + (FREE ? a.scratch_doubles : 0);
-    double* ydense = gpart2 + ((MODE == 1) ? 0 : ((gemv_part_doubles(a.rows_per_cta, MODE == 2 ? a.nd : n, a.chunk) + 1) & ~1));
-    double* xs = ydense + ((MODE == 2) ? rows2 : 0);
-    double* red2 = xs + ((MODE == 2) ? ((a.nd + 2) & ~1) : ((FREE || !XS) ? 0 : ((n + 2) & ~1)));   // [blockDim + rows2]
+    // dense: GEMV partials, then x; matrix-free: the operator's scratch; hybrid: scratch, row sums of the ring's tiles, the ring
+    double* ring_part = gpart + (FREE ? a.scratch_doubles : 0);
+    double* ring_mem = ring_part + ((MODE == 2) ? ring_part_doubles(a.brows, a.nd, a.chunk) : 0);
+    double* xs = gpart + ((MODE == 0) ? ((gemv_part_doubles(a.rows_per_cta, n, a.chunk) + 1) & ~1) : 0);
+    double* red2 = (MODE == 2) ? ring_mem + ring_doubles(a.chunk)
+                               : ((MODE == 1) ? ring_part : xs + (XS ? ((n + 2) & ~1) : 0));   // [blockDim + rows2]
+    BlockRing ring;
+    if (MODE == 2) {
+        ring.A = a.A; ring.lda = a.lda; ring.nd = a.nd; ring.chunk = a.chunk;
+        ring.r0 = min(blockIdx.x * a.brows, a.nd); ring.r1 = min(ring.r0 + a.brows, a.nd);
+        ring.nch = (a.nd + a.chunk - 1) / a.chunk;
+        ring.nunit = ((ring.r1 - ring.r0 + RING_ROWS - 1) / RING_ROWS) * ring.nch;
+        ring.stage = ring_mem;
+        ring.full0 = smem_u32(ring_mem + RING_STAGES * (RING_ROWS + 1) * a.chunk);
+        ring.empty0 = ring.full0 + 8 * RING_STAGES;
+        ring.next = reinterpret_cast<int*>(ring_mem + RING_STAGES * (RING_ROWS + 1) * a.chunk + 2 * RING_STAGES);
+        ring.part = ring_part;
+        ring.rowsP = ((a.brows + RING_ROWS - 1) / RING_ROWS) * RING_ROWS;
+        ring.tile0 = 0;
+        ring_init(ring_mem, a.chunk);
+    }
     Basis B;
     B.Vs = red2 + GM_THREADS + rows2;                          // [VS][rows2]
     B.Vg = a.V + r0; B.VS = a.VS; B.rows2 = rows2; B.nld = a.nld;
@@ -324,7 +351,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
             for (int r = threadIdx.x; r < rows; r += blockDim.x) w_local[r] = a.b[r0 + r];
             first = false;
         } else {
-            cta_apply<STREAM, XS, MODE>(a, r0, r1, a.x, 1.0, xs, gpart, gpart2, ydense, y_local, false, red, target);
+            cta_apply<STREAM, XS, MODE>(a, r0, r1, a.x, 1.0, xs, gpart, ring, y_local, false, red, target);
             for (int r = threadIdx.x; r < rows; r += blockDim.x) w_local[r] = a.b[r0 + r] - y_local[r];
         }
         __syncthreads();
@@ -357,7 +384,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
         for (int j = 0; j < m; ++j) {
             PT(5)
             // a6: y = A (wbuf * inv) = A v_j + V_j c * inv  (c = 0 in the first step of a cycle)
-            cta_apply<STREAM, XS, MODE>(a, r0, r1, a.wbuf, inv, xs, gpart, gpart2, ydense, y_local, true, red, target);
+            cta_apply<STREAM, XS, MODE>(a, r0, r1, a.wbuf, inv, xs, gpart, ring, y_local, true, red, target);
             PT(0)
             // a7, first pass: s = V_j^T y (grid barrier 1), w1 = y - V_j s, h1 = s - c * inv
             local_dots(B, rows, j + 1, y_local, part1, false);
@@ -383,10 +410,10 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
                 double ss = 0.0;
                 for (int i = threadIdx.x; i <= j; i += 32) ss = fma(hloc[i], hloc[i], ss);
                 ss = bie_warp_sum(ss);
-                if (threadIdx.x == 0) red[64] = ss;
+                if (threadIdx.x == 0) red[128] = ss;
             }
             __syncthreads();
-            const double nu = hloc[j + 1], ss = red[64];
+            const double nu = hloc[j + 1], ss = red[128];
             double hn;
             const bool pyth = (ss <= 0.01 * nu);           // identical in every CTA (same bits)
             basis_combine(B, rows, j + 1, hloc, red2);     // V_j h2 on this CTA's rows
@@ -493,7 +520,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
     // ---- a10: outputs; true residual ||b - A x|| / ||b|| (reported only) -----------------------------
     double relres = 0.0;
     if (a.relres_out && bn != 0.0) {
-        cta_apply<STREAM, XS, MODE>(a, r0, r1, a.x, 1.0, xs, gpart, gpart2, ydense, y_local, false, red, target);
+        cta_apply<STREAM, XS, MODE>(a, r0, r1, a.x, 1.0, xs, gpart, ring, y_local, false, red, target);
         p = 0.0;
         for (int r = threadIdx.x; r < rows; r += blockDim.x) {
             const double v = a.b[r0 + r] - y_local[r];
@@ -517,13 +544,14 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
 static inline size_t al256(size_t b) { return (b + 255) & ~(size_t)255; }
 
 struct GmresPlan {
-    int G, rows_per_cta, chunk, nld, VS, scratch_doubles;
+    int G, rows_per_cta, chunk, nld, VS, scratch_doubles, brows;
     bool xs, stream;
     size_t smem;
-    size_t offV, offW, offP, offR, offY, offS, total;
+    size_t offV, offW, offP, offR, offY, offD, offS, total;
 };
 
-// workspace layout: Krylov basis, wbuf, per-CTA partials, R, y, and the grid-barrier counter of the call
+// workspace layout: Krylov basis, wbuf, per-CTA partials, R, y, the stored block's product (hybrid), and the grid-barrier
+// counter of the call
 static void gmres_ws_layout(int n, int m, int sm_bound, GmresPlan* pl)
 {
     pl->nld = (n + 1) & ~1;
@@ -533,39 +561,51 @@ static void gmres_ws_layout(int n, int m, int sm_bound, GmresPlan* pl)
     pl->offP = o; o += al256(sizeof(double) * 3 * (size_t)(m + 2) * sm_bound);
     pl->offR = o; o += al256(sizeof(double) * (size_t)m * (m + 1));
     pl->offY = o; o += al256(sizeof(double) * (size_t)m);
+    pl->offD = o; o += al256(sizeof(double) * (size_t)pl->nld);
     pl->offS = o; o += 256;
     pl->total = o;
 }
 
-// mode: 0 stored matrix, 1 matrix-free, 2 hybrid (slab of nd columns streamed by 16 - nwf warps)
+static void gmres_grid(int n, int sm_count, GmresPlan* pl)
+{
+    pl->rows_per_cta = (n + sm_count - 1) / sm_count;
+    pl->G = (n + pl->rows_per_cta - 1) / pl->rows_per_cta;
+}
+
+// mode: 0 stored matrix, 1 matrix-free, 2 hybrid (leading nd x nd block stored).  gmres_grid() has been called.
 static int gmres_plan(int n, int restart, int sm_count, int max_smem, int l2_bytes, long long lda, int mode, int nd,
-                      int nwf, bool sym_possible, GmresPlan* pl)
+                      bool vortex, bool sym, GmresPlan* pl)
 {
     const int m = restart;
     const bool free_op = (mode != 0);
-    pl->rows_per_cta = (n + sm_count - 1) / sm_count;
-    pl->G = (n + pl->rows_per_cta - 1) / pl->rows_per_cta;
-    pl->chunk = mode == 2 ? gemv_chunk(pl->rows_per_cta, nd, GM_THREADS / 32 - nwf)
-                          : gemv_chunk(pl->rows_per_cta, n, GM_THREADS / 32);
-    pl->scratch_doubles = free_op ? (sym_possible ? free_scratch_doubles(GM_THREADS) : free_scratch_doubles_onedir()) : 0;
+    pl->brows = 0;
+    if (mode == 2) {
+        // every CTA streams the same number of rows of the stored block (a multiple of RING_ROWS), whoever owns them
+        pl->brows = ((nd + pl->G - 1) / pl->G + RING_ROWS - 1) / RING_ROWS * RING_ROWS;
+        pl->chunk = ring_chunk(pl->brows, nd, GM_WARPS - 1);
+    } else {
+        pl->chunk = gemv_chunk(pl->rows_per_cta, n, GM_WARPS);
+    }
+    pl->scratch_doubles = free_op ? free_scratch_doubles(vortex, sym) : 0;
     const int rows2 = (pl->rows_per_cta + 1) & ~1;
     size_t base = (size_t)gm_head_doubles(m, rows2);
     if (free_op) base += (size_t)pl->scratch_doubles;
-    if (mode != 1) base += (size_t)((gemv_part_doubles(pl->rows_per_cta, mode == 2 ? nd : n, pl->chunk) + 1) & ~1);
-    if (mode == 2) base += (size_t)rows2 + (size_t)((nd + 2) & ~1);   // slab result, x of the slab's columns
+    if (mode == 0) base += (size_t)((gemv_part_doubles(pl->rows_per_cta, n, pl->chunk) + 1) & ~1);
+    if (mode == 2) base += (size_t)ring_part_doubles(pl->brows, nd, pl->chunk) + (size_t)ring_doubles(pl->chunk);
     base *= sizeof(double);
     base += sizeof(double) * ((size_t)GM_THREADS + rows2);  // red2
-    pl->xs = mode == 2 || (!free_op && base + sizeof(double) * ((size_t)n + 2) <= (size_t)max_smem);
-    pl->smem = base + ((pl->xs && mode == 0) ? sizeof(double) * ((size_t)n + 2) : 0);
+    pl->xs = mode == 0 && base + sizeof(double) * ((size_t)n + 2) <= (size_t)max_smem;
+    pl->smem = base + (pl->xs ? sizeof(double) * ((size_t)n + 2) : 0);
     if (pl->smem > (size_t)max_smem) return BIE_ERR_ARG;
     // the rest of the shared memory holds this CTA's rows of as many Krylov vectors as fit
     // (dense operator: the streaming loads of A need the L1 as their landing buffer, 16 warps x 4 KB in flight,
-    // so the shared-memory carve-out stops at 164 KB; measured: 408 us per step with 227 KB against 338 us)
-    const size_t cap = mode == 1 ? (size_t)max_smem : (size_t)(163 * 1024 < max_smem ? 163 * 1024 : max_smem);
+    // so the shared-memory carve-out stops at 164 KB; measured: 408 us per step with 227 KB against 338 us.
+    // The hybrid operator's block arrives by bulk copies into shared memory and needs no L1.)
+    const size_t cap = mode != 0 ? (size_t)max_smem : (size_t)(163 * 1024 < max_smem ? 163 * 1024 : max_smem);
     pl->VS = pl->smem < cap ? (int)((cap - pl->smem) / (sizeof(double) * rows2)) : 0;
     if (pl->VS > m + 1) pl->VS = m + 1;
     pl->smem += sizeof(double) * (size_t)pl->VS * rows2;
-    pl->stream = mode != 1 && (double)n * (double)(mode == 2 ? nd : lda) * 8.0 > 0.6 * (double)l2_bytes;
+    pl->stream = mode != 1 && (double)(mode == 2 ? nd : n) * (double)(mode == 2 ? nd : lda) * 8.0 > 0.6 * (double)l2_bytes;
     gmres_ws_layout(n, m, sm_count, pl);
     return BIE_OK;
 }
@@ -607,15 +647,23 @@ int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, int nd, 
     if (ctx->sm_count > 256) return BIE_ERR_DEVICE;
     if (restart > n) restart = n;  // the Krylov space cannot exceed n
     GmresPlan pl;
-    const int nwf = ctx->hybrid_free_warps;
-    // the symmetric loops (bie_free_sym.cuh) need the larger scratch; bie_free_plan decides later whether they run
-    const bool sym_possible = (mode == 1 && ctx->use_sym != 0) || (mode == 2 && ctx->use_sym == 2);
-    int rc = gmres_plan(n, restart, ctx->sm_count, ctx->max_smem_optin, ctx->l2_bytes, free_op ? n : lda, mode, nd, nwf, sym_possible, &pl);
+    gmres_grid(n, ctx->sm_count, &pl);
+    GmresArgs a;
+    memset(&a.nt, 0, sizeof(a.nt)); memset(&a.ct, 0, sizeof(a.ct)); memset(&a.fp, 0, sizeof(a.fp));
+    int rc;
+    if (free_op) {
+        a.nt = bie_node_table(ctx); a.ct = ctx->comps;
+        rc = bie_ensure_near(ctx, st);
+        if (rc != BIE_OK) return rc;
+        rc = bie_free_plan(ctx, pl.G, nd, &a.fp, st);     // decides one-directional / symmetric loops; checks nd
+        if (rc != BIE_OK) return rc;
+    }
+    rc = gmres_plan(n, restart, ctx->sm_count, ctx->max_smem_optin, ctx->l2_bytes, free_op ? n : lda, mode, nd,
+                    a.fp.vortex != 0, a.fp.sym != 0, &pl);
     if (rc != BIE_OK) return rc;
     // align the caller's workspace to 256 bytes
     uintptr_t base = ((uintptr_t)ws + 255) & ~(uintptr_t)255;
     if (base - (uintptr_t)ws + pl.total > ws_bytes) return BIE_ERR_WORKSPACE;
-    GmresArgs a;
     a.A = A; a.lda = lda; a.n = n; a.b = rhs; a.tol = tol; a.m = restart; a.max_iters = max_iters;
     a.x = x; a.iters_out = iters_out; a.relres_out = relres_out; a.status_out = status_out; a.res_hist = res_hist;
     a.V = (double*)(base + pl.offV);
@@ -623,19 +671,12 @@ int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, int nd, 
     a.part = (double*)(base + pl.offP);
     a.R = (double*)(base + pl.offR);
     a.yv = (double*)(base + pl.offY);
+    a.yd = (double*)(base + pl.offD);
     a.sync = (unsigned int*)(base + pl.offS);     // per call: two solves of one ctx never share a barrier counter
     a.nld = pl.nld; a.rows_per_cta = pl.rows_per_cta; a.chunk = pl.chunk; a.VS = pl.VS;
-    a.nd = nd; a.nwf = nwf; a.scratch_doubles = pl.scratch_doubles;
+    a.nd = nd; a.nwf = ctx->hybrid_free_warps; a.scratch_doubles = pl.scratch_doubles; a.brows = pl.brows;
     a.res_pairs = (mode == 0 && pl.stream)
         ? bie_gemv_resident_pairs(ctx->l2_bytes, n, (long long)lda, pl.rows_per_cta, sizeof(double) * (size_t)(restart + 2) * pl.nld) : 0;
-    memset(&a.nt, 0, sizeof(a.nt)); memset(&a.ct, 0, sizeof(a.ct)); memset(&a.fp, 0, sizeof(a.fp));
-    if (free_op) {
-        a.nt = bie_node_table(ctx); a.ct = ctx->comps;
-        rc = bie_ensure_near(ctx, st);
-        if (rc != BIE_OK) return rc;
-        rc = bie_free_plan(ctx, pl.G, nd, &a.fp, st);
-        if (rc != BIE_OK) return rc;
-    }
     BIE_CUDA(cudaMemsetAsync(a.sync, 0, sizeof(unsigned int), st));
     if (mode == 1) return launch_gmres<false, false, 1>(ctx, a, pl, st);
     if (mode == 2) return pl.stream ? launch_gmres<true, true, 2>(ctx, a, pl, st) : launch_gmres<false, true, 2>(ctx, a, pl, st);

@@ -79,11 +79,11 @@ bie_matvec_free_kernel(NodeTable nt, CompTable ct, FreePlan fp, int rows_per_cta
     const int r0 = min(blockIdx.x * rows_per_cta, n);
     const int r1 = min(r0 + rows_per_cta, n);
     double* scratch = smem;
-    double* y_local = scratch + free_scratch_doubles(FREE_THREADS);
+    double* y_local = scratch + free_scratch_doubles(fp.vortex != 0, fp.sym != 0);
     unsigned int target = 0;
     free_write_tables(nt, ct, fp, r0, r1, x + r0, scratch);
     grid_barrier(sync, target);
-    free_parts(nt, ct, fp, scratch, cta_team());
+    free_parts(nt, ct, fp, scratch, cta_team(), NoPoll());
     grid_barrier(sync, target);
     free_gather(nt, ct, fp, r0, r1, x, 1.0, scratch, y_local);
     for (int r = threadIdx.x; r < r1 - r0; r += blockDim.x) y[r0 + r] = y_local[r];
@@ -98,13 +98,13 @@ int bie_launch_matvec_free(bie_ctx* ctx, const double* x, double* y, cudaStream_
     const int n = ctx->n;
     const int G = ctx->sm_count;
     const int rows_per_cta = (n + G - 1) / G;
-    const size_t smem = sizeof(double) * (size_t)(free_scratch_doubles(FREE_THREADS) + ((rows_per_cta + 1) & ~1));
-    if (smem > (size_t)ctx->max_smem_optin) return BIE_ERR_ARG;
     FreePlan fp;
     int rc = bie_ensure_near(ctx, st);
     if (rc != BIE_OK) return rc;
     rc = bie_free_plan(ctx, G, 0, &fp, st);
     if (rc != BIE_OK) return rc;
+    const size_t smem = sizeof(double) * (size_t)(free_scratch_doubles(fp.vortex != 0, fp.sym != 0) + ((rows_per_cta + 1) & ~1));
+    if (smem > (size_t)ctx->max_smem_optin) return BIE_ERR_ARG;
     rc = bie_grant_smem(ctx, 12, bie_matvec_free_kernel, smem);
     if (rc != BIE_OK) return rc;
     // the grid-barrier counter of THIS launch: the ctx cycles through BIE_SYNC_SLOTS counters, so that a later launch

@@ -167,8 +167,8 @@ int bie_prepare_nodes(bie_ctx* ctx, int ncomp, const int32_t* counts, const int3
 size_t bie_free_buf_doubles(int cap)
 {
     // tables [4][cap] double2, then partial sums for (row blocks + CTAs) parts of FREE_ROWS rows, then the per-CTA
-    // partials of the constant term [2][FREE_SB_LD]
-    return 8 * (size_t)cap + ((size_t)cap / FREE_ROWS + 2 + 256) * FREE_ROWS + 2 * FREE_SB_LD;
+    // partials of the constant terms [4][FREE_SB_LD]
+    return 8 * (size_t)cap + ((size_t)cap / FREE_ROWS + 2 + 256) * FREE_ROWS + 4 * FREE_SB_LD;
 }
 
 // work list of the symmetric split (bie_free_sym.cuh), built on the device by one thread (NB <= a few hundred):
@@ -202,17 +202,21 @@ int bie_free_plan(bie_ctx* ctx, int grid, int s_off, FreePlan* fp, cudaStream_t 
     fp->NB = fp->NB0 + (n - fp->M0 + FREE_ROWS - 1) / FREE_ROWS;
     fp->vortex = (ctx->variant == BIE_VARIANT_VORTEX) ? 1 : 0;
     fp->s_off = s_off;
-    fp->UB = (npad - s_off) / 2;
-    fp->U = (long long)fp->NB * fp->UB;
-    // symmetric work split (bie_free_sym.cuh): whole operator only, Eq. (3.16) variants, and while the reverse partials
-    // [NB][npad] stay small
-    fp->sym = 0; fp->PC = nullptr; fp->sym_cum = nullptr; fp->sym_perm = nullptr; fp->sym_pos = nullptr;
     // hybrid operator: s_off must be a row-block boundary (row blocks are cut per class: 128 b, then M_0 + 128 b)
     const bool boundary = s_off == 0 || (s_off <= fp->M0 ? (s_off % FREE_ROWS == 0 || s_off == fp->M0)
                                                           : ((s_off - fp->M0) % FREE_ROWS == 0));
-    fp->sym_first = 0;
-    // (in the hybrid operator only on request, use_sym == 2: with few pair-loop warps it is slower)
-    if (ctx->use_sym && (s_off == 0 || ctx->use_sym == 2) && boundary && !fp->vortex && npad <= 65536) {
+    if (!boundary) return BIE_ERR_ARG;
+    auto row0_of = [&](int b) { return b < fp->NB0 ? b * FREE_ROWS : fp->M0 + (b - fp->NB0) * FREE_ROWS; };
+    auto rows_of = [&](int b) { const int r0 = row0_of(b), end = b < fp->NB0 ? fp->M0 : n; return end - r0 < FREE_ROWS ? end - r0 : FREE_ROWS; };
+    int first = 0;   // row blocks entirely below s_off: they only take the sources from s_off on (the stored block has the others)
+    while (first < fp->NB && row0_of(first) + rows_of(first) <= s_off) ++first;
+    fp->nb_below = first;
+    fp->UBb = (npad - s_off) / 2;
+    fp->UBf = npad / 2;
+    fp->U = (long long)first * fp->UBb + (long long)(fp->NB - first) * fp->UBf;
+    // symmetric work split (bie_free_sym.cuh): Eq. (3.16) variants, and while the reverse partials [NB][npad] stay small
+    fp->sym = 0; fp->PC = nullptr; fp->sym_cum = nullptr; fp->sym_perm = nullptr; fp->sym_pos = nullptr;
+    if (ctx->use_sym && !fp->vortex && npad <= 65536) {
         const int NB = fp->NB;
         const size_t need = (size_t)NB * (size_t)npad;
         if (need > ctx->pc_cap) {
@@ -241,21 +245,17 @@ int bie_free_plan(bie_ctx* ctx, int grid, int s_off, FreePlan* fp, cudaStream_t 
         int* perm = reinterpret_cast<int*>(ctx->sym_tab + sizeof(long long) * (nbmax + 1));
         int* pos = perm + nbmax;
         if (ctx->sym_key[0] != ctx->geom_gen || ctx->sym_key[1] != s_off) {
-            auto row0_of = [&](int b) { return b < fp->NB0 ? b * FREE_ROWS : fp->M0 + (b - fp->NB0) * FREE_ROWS; };
-            auto rows_of = [&](int b) { const int r0 = row0_of(b), end = b < fp->NB0 ? fp->M0 : n; return end - r0 < FREE_ROWS ? end - r0 : FREE_ROWS; };
-            int first = 0;
-            while (first < NB && row0_of(first) + rows_of(first) <= s_off) ++first;
             long long U = 0;
             for (int b = 0; b < NB; ++b) U += npad - (b < first ? s_off : row0_of(b));
             bie_sym_tables_kernel<<<1, 32, 0, st>>>(NB, fp->NB0, fp->M0, n, npad, s_off, first, cum, perm, pos);
             BIE_CUDA(cudaGetLastError());
             ctx->sym_key[0] = ctx->geom_gen; ctx->sym_key[1] = s_off;
-            ctx->sym_U = U; ctx->sym_first = first;
+            ctx->sym_U = U;
         }
-        fp->sym_first = ctx->sym_first;
         fp->sym_cum = cum; fp->sym_perm = perm; fp->sym_pos = pos;
         fp->sym = 1; fp->PC = ctx->pc_buf; fp->U = ctx->sym_U;
     }
+    fp->stage_buf = free_stage_buf_doubles(fp->vortex != 0, fp->sym != 0);
     fp->Geff = (long long)grid < fp->U ? grid : (int)fp->U;
     if (fp->Geff < 1) fp->Geff = 1;
     fp->T = reinterpret_cast<double2*>(ctx->free_buf);

@@ -257,7 +257,7 @@ def test_operators_with_near_pairs_across_components(ctx, gap):
     assert rel_max(y.cpu().numpy(), oracle.matvec(Ao, x)) <= 1e-12
     b = inputs.rhs_analytic(g, lambda z: np.exp(1j * z))
     xo, ito, _, _, sto = oracle.gmres(Ao, b, 1e-13, 50, 2000)
-    xg, it, rr, st, S = gpu_gmres_hybrid(ctx, g, 448, b, 1e-13, 50, 2000)
+    xg, it, rr, st, S = gpu_gmres_hybrid(ctx, g, 384, b, 1e-13, 50, 2000)
     assert sto == 0 and st == 0
     check_iters(it, ito, "obstacle %g under the surface" % gap)
     assert np.linalg.norm(xg - xo) / np.linalg.norm(xo) <= TOL_X * max(1.0, np.linalg.cond(Ao) / 100.0)
@@ -607,8 +607,15 @@ def test_matrix_free_one_directional_and_symmetric_agree(ctx, shape):
         x0, it0, rr0, st0 = gpu_gmres(ctx, None, b, 1e-13, 50, 1000)
         ctx.bie_set_symmetric(1)
         x1, it1, rr1, st1 = gpu_gmres(ctx, None, b, 1e-13, 50, 1000)
-        assert st0 == 0 and st1 == 0 and abs(it0 - it1) <= 1
+        assert st0 == 0 and st1 == 0
+        # both against the ORACLE's count (the config-3 geometry is the named plateau case: with this right-hand side the
+        # oracle's residuals are 1.37e-13, 1.21e-13, 0.64e-13 at steps 76-78; measured GPU counts 76 and 78)
+        xo, ito, _, _, sto = oracle.gmres(Ao, b, 1e-13, 50, 1000)
+        case = "config3" if shape is None else "small problem %r" % (shape,)
+        for it in (it0, it1):
+            check_iters(it, ito, case, lambda: iteration_band(Ao, b, 1e-13, 50, 1000))
         assert np.linalg.norm(x0 - x1) <= 1e-10 * np.linalg.norm(x0)
+        assert np.linalg.norm(x0 - xo) <= 1e-10 * np.linalg.norm(xo) * max(1.0, np.linalg.cond(Ao) / 100.0)
     finally:
         ctx.bie_set_symmetric(1)
 
@@ -799,13 +806,13 @@ def test_gmres_matrix_free_parity(ctx, c):
 
 
 def gpu_gmres_hybrid(ctx, g, nd, b, tol, restart, max_iters=1000, lda=None):
-    """slab of nd columns written by bie_build_cols (the rest of the allocation is poisoned: it must never be read)"""
+    """leading nd x nd block written by bie_build_block (the rest of the allocation is poisoned: it must never be read)"""
     from paper_2108_01786_b200 import bie
     n = b.size
     lda = lda or (nd + (nd & 1))
     z, dz, d2z = geo_dev(g)
-    A = torch.full((n, lda), float("nan"), dtype=torch.float64, device="cuda")
-    ctx.bie_build_cols(g.counts, g.kinds, z, dz, d2z, nd, A, lda=lda)
+    A = torch.full((nd, lda), float("nan"), dtype=torch.float64, device="cuda")
+    ctx.bie_build_block(g.counts, g.kinds, z, dz, d2z, nd, A, lda=lda)
     ws = torch.empty(bie.Context.bie_gmres_workspace_bytes(n, restart), dtype=torch.uint8, device="cuda")
     oi = torch.full((2,), -7, dtype=torch.int32, device="cuda")
     of = torch.full((1,), -7.0, dtype=torch.float64, device="cuda")
@@ -813,6 +820,18 @@ def gpu_gmres_hybrid(ctx, g, nd, b, tol, restart, max_iters=1000, lda=None):
     ctx.bie_gmres_hybrid(A, nd, dev(b), x[:n], tol, restart, max_iters, ws, oi, of, lda=lda)
     torch.cuda.synchronize()
     return x[:n].cpu().numpy(), int(oi[0]), float(of[0]), int(oi[1]), A
+
+
+def test_build_block_writes_only_the_block(ctx):
+    g = cfg(2).geometry
+    nb, lda = 778, 900
+    z, dz, d2z = geo_dev(g)
+    A = torch.full((nb + 5, lda), -7.0, dtype=torch.float64, device="cuda")
+    ctx.bie_build_block(g.counts, g.kinds, z, dz, d2z, nb, A, lda=lda)
+    Ah = A.cpu().numpy()
+    Ao = oracle_build(g)
+    assert rel_max(Ah[:nb, :nb], Ao[:nb, :nb]) <= TOL_ENTRY
+    assert np.all(Ah[:nb, nb:] == -7.0) and np.all(Ah[nb:] == -7.0)
 
 
 def test_build_cols_writes_only_the_slab(ctx):
@@ -827,10 +846,10 @@ def test_build_cols_writes_only_the_slab(ctx):
     assert np.all(Ah[:, nd:] == -7.0)
 
 
-@pytest.mark.parametrize("c,nd", [(1, 128), (2, 0), (2, 2), (2, 1030), (2, 1024), (2, 1280), (2, 2046), (3, 0), (3, 2048), (3, 2560), (4, 0), (5, 0)])
+@pytest.mark.parametrize("c,nd", [(1, 128), (1, 256), (2, 0), (2, 128), (2, 1024), (2, 1280), (2, 1920), (3, 0), (3, 2048), (3, 2560), (4, 0), (5, 0), (5, 4096)])
 def test_gmres_hybrid_parity(ctx, c, nd):
-    """hybrid operator (stored slab of nd columns + recomputed sources): same solution, same iteration band;
-    nd = 0 takes the library's own split (bie_hybrid_cols)"""
+    """hybrid operator (stored leading nd x nd block + every other entry recomputed): same solution, same iteration
+    count; nd = 0 takes the library's own split (bie_hybrid_cols); nd on Gamma_0, at M_0 and on the solids"""
     P = cfg(c)
     g, b = P.geometry, P.rhs[0]
     nd = nd or ctx.bie_hybrid_cols(g.n)
@@ -848,15 +867,15 @@ def test_gmres_hybrid_parity(ctx, c, nd):
 
 
 @pytest.mark.parametrize("c,nd", [(2, 1024), (2, 1280), (3, 2048), (3, 2560), (1, 256)])
-def test_gmres_hybrid_with_symmetric_pair_loops(ctx, c, nd):
-    """bie_set_symmetric(2): the triangle of the hybrid operator's recomputed part (rows and sources >= nd) through the
-    symmetric loops; nd on a row-block boundary of Gamma_0 (1024, 2048, 256) and of the solids (M_0 + 256, M_0 + 512)"""
+def test_gmres_hybrid_with_one_directional_pair_loops(ctx, c, nd):
+    """bie_set_symmetric(0): the recomputed part of the hybrid operator through the one-directional loops (the default is
+    the symmetric ones); nd on a row-block boundary of Gamma_0 (1024, 2048, 256) and of the solids (M_0 + 256, M_0 + 512)"""
     P = cfg(c)
     g, b = P.geometry, P.rhs[0]
     Ao = oracle_build(g)
     xo, ito, _, _, _ = oracle.gmres(Ao, b, P.tol, P.restart, P.max_iters)
     try:
-        ctx.bie_set_symmetric(2)
+        ctx.bie_set_symmetric(0)
         x, it, rr, st, A = gpu_gmres_hybrid(ctx, g, nd, b, P.tol, P.restart, P.max_iters)
     finally:
         ctx.bie_set_symmetric(1)
@@ -877,7 +896,7 @@ def test_gmres_hybrid_free_warps_knob(ctx):
             x, it, rr, st, A = gpu_gmres_hybrid(ctx, g, 1024, b, P.tol, P.restart, P.max_iters)
             assert st == 0 and abs(it - ito) <= 1 and np.linalg.norm(x - xo) / np.linalg.norm(xo) <= TOL_X
     finally:
-        ctx.bie_set_hybrid_free_warps(8)
+        ctx.bie_set_hybrid_free_warps(15)
 
 
 def test_config4_sequence_of_four_stages(ctx):
@@ -989,7 +1008,7 @@ def test_error_codes_of_the_operator_and_next_calls(ctx):
     b = torch.ones(n, dtype=torch.float64, device="cuda")
     x = torch.empty_like(b)
     ctx.bie_build_cols(g.counts, g.kinds, z, dz, d2z, 128, A)
-    for nd, code in [(127, -6), (n, -6), (0, -6)]:                    # odd, whole matrix, none
+    for nd, code in [(127, -6), (n, -6), (0, -6), (2, -6), (130, -6), (256 + 64, -6)]:   # odd, whole matrix, none, not a row-block boundary
         with pytest.raises(bie.BieError) as e:
             ctx.bie_gmres_hybrid(A, nd, b, x, 1e-13, 50, 10, ws, oi, of)
         assert e.value.code == code, nd
@@ -1002,7 +1021,7 @@ def test_error_codes_of_the_operator_and_next_calls(ctx):
     with pytest.raises(bie.BieError) as e:
         ctx.bie_set_hybrid_free_warps(16)
     assert e.value.code == -6
-    assert ctx.bie_hybrid_cols(2) == 0 and ctx.bie_hybrid_cols(100) == 0 and ctx.bie_hybrid_cols(16384) == 6784
+    assert ctx.bie_hybrid_cols(2) == 0 and ctx.bie_hybrid_cols(100) == 0 and ctx.bie_hybrid_cols(16384) == 9216
     # Appendix B without centres for a geometry that has an obstacle; Cauchy evaluation with too many functions
     rc = bie.lib().bie_add_cyl_columns(ctx._h, 3, bie._ip(bie._i32(g.counts)), bie._ip(bie._i32(g.kinds)), z.data_ptr(), None,
                                        A.data_ptr(), n, None)
