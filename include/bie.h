@@ -126,28 +126,34 @@ int bie_build_update(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32
 
 /* Hybrid operator (north_star: "matrix-free fused rebuild+matvec variant chosen by measurement").  The dense
  * GEMV is HBM-bound and leaves the FP64 pipe idle, the matrix-free operator is FP64-bound and leaves HBM idle;
- * the hybrid operator does both at once: the LEADING nblock x nblock block of the matrix is stored (row-major,
- * leading dimension lda >= nblock, lda even) and arrives in shared memory by bulk copies (TMA) while the warps of
- * every CTA recompute every other entry from the node tables -- with the symmetric pair loops (see
- * bie_set_symmetric): every pair {t, s} outside the block has max(t, s) >= nblock, so one evaluation of the pair
- * serves both entries -- and consume the landed tiles of the block between their source chunks.
- * nblock must be a row-block boundary of the pair loops: a multiple of 128 up to M_0, or M_0 itself, or M_0 plus a
- * multiple of 128; even; < n.
- * bie_build_block: as bie_build, but only rows and columns [0, nblock) are written (1 <= nblock <= n).
- * bie_build_cols: as bie_build, but only the columns [0, ncols) of every row are written (1 <= ncols <= n); its
- *   first ncols rows are the block, so it may feed bie_gmres_hybrid too.
+ * the hybrid operator does both at once: the LEADING nblock x nblock block of the matrix is stored and arrives in
+ * shared memory by bulk copies (TMA) while the warps of every CTA recompute every other entry from the node tables
+ * -- with the symmetric pair loops (see bie_set_symmetric): every pair {t, s} outside the block has
+ * max(t, s) >= nblock, so one evaluation of the pair serves both entries.
+ * The block is kept in a BLOCK FORMAT private to the library: tiles of 4 rows x 512 columns, each tile contiguous
+ * (16 KB, so that ONE bulk copy moves it), rows and columns padded to whole tiles; bie_hybrid_block_bytes(nblock)
+ * is its size.  nblock must be a row-block boundary of the pair loops: a multiple of 128 up to M_0, or M_0 itself,
+ * or M_0 plus a multiple of 128; even; < n.
+ * bie_build_block: the entries of bie_build for rows and columns [0, nblock), written in the block format to A
+ *   (dev, bie_hybrid_block_bytes(nblock) bytes, 16-byte aligned).
+ * bie_build_cols: as bie_build (row-major), but only the columns [0, ncols) of every row are written (1 <= ncols <= n).
  * bie_hybrid_cols: the block edge the library recommends for n on a B200 (0 = too small, use bie_gmres); it uses M_0
  *   of the ctx's current geometry when that has n nodes, else assumes M_0 is a multiple of 128.
- * bie_set_hybrid_free_warps: tuning knob, warps per CTA on the pair loops (1..15, default 15; warps above it only
- *   consume tiles of the block, the 16th issues the bulk copies). */
+ * bie_set_hybrid_free_warps: tuning knob, warps per CTA on the pair loops (1..15; default 12 = the warps of three of the
+ *   SM's four sub-partitions, the fourth hosts the warp that issues the bulk copies and three warps that multiply the
+ *   landed tiles; other values: warps 0..w-1 run the pair loops, the others up to 14 consume tiles, 15 issues). */
+size_t bie_hybrid_block_bytes(int nblock);
 int bie_build_block(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds,
                     const double* zeta, const double* dzeta, const double* d2zeta,
-                    int variant, int nblock, double* A, int64_t lda, void* stream);
+                    int variant, int nblock, double* A, void* stream);
 int bie_build_cols(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t* kinds,
                    const double* zeta, const double* dzeta, const double* d2zeta,
                    int variant, int ncols, double* A, int64_t lda, void* stream);
 int bie_hybrid_cols(bie_ctx* ctx, int n);
 int bie_set_hybrid_free_warps(bie_ctx* ctx, int free_warps);
+/* tuning knob: tiles of the stored block a pair-loop warp may take between two of its source chunks (0..64; 0: only the
+ * warps above bie_set_hybrid_free_warps consume the block) */
+int bie_set_hybrid_poll_tiles(bie_ctx* ctx, int tiles);
 
 /* Prepares the node tables of a geometry in the ctx without writing a matrix (for the matrix-free
  * operator).  Same geometry arguments as bie_build. */
@@ -241,9 +247,9 @@ int bie_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, const double* r
               void* workspace, size_t workspace_bytes, void* stream);
 
 /* Same solve with the hybrid operator: A holds the leading ncols_dense x ncols_dense block of the matrix of the ctx's
- * current geometry (bie_build_block; or a slab of bie_build_cols), ncols_dense a row-block boundary as described at
- * bie_build_block (else BIE_ERR_ARG), lda >= ncols_dense.  Everything else as bie_gmres. */
-int bie_gmres_hybrid(bie_ctx* ctx, int n, const double* A, int64_t lda, int ncols_dense, const double* rhs,
+ * current geometry in the block format (bie_build_block), ncols_dense a row-block boundary as described at
+ * bie_build_block (else BIE_ERR_ARG).  Everything else as bie_gmres. */
+int bie_gmres_hybrid(bie_ctx* ctx, int n, const double* A, int ncols_dense, const double* rhs,
                      double tol, int restart, int max_iters,
                      double* x, int32_t* iters_out, double* relres_out, int32_t* status_out, double* res_hist,
                      void* workspace, size_t workspace_bytes, void* stream);

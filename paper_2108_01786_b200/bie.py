@@ -25,7 +25,7 @@ EXPORTS = ("bie_create", "bie_destroy", "bie_strerror", "bie_device_info", "bie_
            "bie_solve_workspace_bytes", "bie_solve_host", "bie_probe_dfma", "bie_build_cols", "bie_hybrid_cols",
            "bie_set_hybrid_free_warps", "bie_gmres_hybrid", "bie_matvec_rect", "bie_build_normal_velocity",
            "bie_add_cyl_columns", "bie_cauchy_eval_workspace_bytes", "bie_cauchy_eval", "bie_set_symmetric",
-           "bie_build_block")
+           "bie_build_block", "bie_set_hybrid_poll_tiles", "bie_hybrid_block_bytes")
 
 BIE_OK, BIE_MAX_ITERS = 0, 1
 OP_DENSE, OP_FREE, OP_HYBRID = 0, 1, 2
@@ -79,13 +79,17 @@ def lib() -> ctypes.CDLL:
         L.bie_build_cols.restype = i32
         L.bie_build_cols.argtypes = geo + [i32, vp, i64, vp]
         L.bie_build_block.restype = i32
-        L.bie_build_block.argtypes = geo + [i32, vp, i64, vp]
+        L.bie_build_block.argtypes = geo + [i32, vp, vp]
+        L.bie_hybrid_block_bytes.restype = sz
+        L.bie_hybrid_block_bytes.argtypes = [i32]
         L.bie_hybrid_cols.restype = i32
         L.bie_hybrid_cols.argtypes = [vp, i32]
         L.bie_set_hybrid_free_warps.restype = i32
         L.bie_set_hybrid_free_warps.argtypes = [vp, i32]
+        L.bie_set_hybrid_poll_tiles.restype = i32
+        L.bie_set_hybrid_poll_tiles.argtypes = [vp, i32]
         L.bie_gmres_hybrid.restype = i32
-        L.bie_gmres_hybrid.argtypes = [vp, i32, vp, i64, i32, vp, dbl, i32, i32, vp, vp, vp, vp, vp, vp, sz, vp]
+        L.bie_gmres_hybrid.argtypes = [vp, i32, vp, i32, vp, dbl, i32, i32, vp, vp, vp, vp, vp, vp, sz, vp]
         L.bie_matvec_rect.restype = i32
         L.bie_matvec_rect.argtypes = [vp, i32, i32, vp, i64, vp, vp, vp]
         L.bie_build_normal_velocity.restype = i32
@@ -196,14 +200,16 @@ class Context:
         _check(lib().bie_build_cols(*args, int(ncols), A.data_ptr(), lda, _stream()), "bie_build_cols")
         return A
 
-    def bie_build_block(self, counts, kinds, zeta, dzeta, d2zeta, nblock: int, A, variant: int = VARIANT_A,
-                        lda: Optional[int] = None):
-        """A (CUDA float64, nblock x lda row-major, lda >= nblock) <- the leading nblock x nblock block of the matrix:
-        the stored part of the hybrid operator."""
+    @staticmethod
+    def bie_hybrid_block_bytes(nblock: int) -> int:
+        return int(lib().bie_hybrid_block_bytes(int(nblock)))
+
+    def bie_build_block(self, counts, kinds, zeta, dzeta, d2zeta, nblock: int, A, variant: int = VARIANT_A):
+        """A (CUDA float64, bie_hybrid_block_bytes(nblock) bytes) <- the leading nblock x nblock block of the matrix in the
+        library's block format (tiles of 4 x 512, each contiguous): the stored part of the hybrid operator."""
         n, args, keep = self._geo(counts, kinds, zeta, dzeta, d2zeta, variant)
-        lda = int(lda if lda is not None else A.stride(0))
-        _dev_f64(A, (int(nblock) - 1) * lda + int(nblock))
-        _check(lib().bie_build_block(*args, int(nblock), A.data_ptr(), lda, _stream()), "bie_build_block")
+        _dev_f64(A, self.bie_hybrid_block_bytes(nblock) // 8)
+        _check(lib().bie_build_block(*args, int(nblock), A.data_ptr(), _stream()), "bie_build_block")
         return A
 
     def bie_hybrid_cols(self, n: int) -> int:
@@ -211,6 +217,9 @@ class Context:
 
     def bie_set_hybrid_free_warps(self, free_warps: int):
         _check(lib().bie_set_hybrid_free_warps(self._h, int(free_warps)), "bie_set_hybrid_free_warps")
+
+    def bie_set_hybrid_poll_tiles(self, tiles: int):
+        _check(lib().bie_set_hybrid_poll_tiles(self._h, int(tiles)), "bie_set_hybrid_poll_tiles")
 
     def bie_set_geometry(self, counts, kinds, zeta, dzeta, d2zeta, variant: int = VARIANT_A):
         n, args, keep = self._geo(counts, kinds, zeta, dzeta, d2zeta, variant)
@@ -309,16 +318,16 @@ class Context:
         return x
 
     def bie_gmres_hybrid(self, A, ncols_dense: int, rhs, x, tol: float, restart: int, max_iters: int, workspace,
-                         out_i32, out_f64, lda: Optional[int] = None, res_hist=None):
-        """Asynchronous.  A: the slab written by bie_build_cols (n x lda, lda >= ncols_dense).  Outputs as bie_gmres."""
+                         out_i32, out_f64, res_hist=None):
+        """Asynchronous.  A: the leading ncols_dense x ncols_dense block written by bie_build_block (block format).
+        Outputs as bie_gmres."""
         import torch
         n = rhs.numel()
-        lda = int(lda if lda is not None else A.stride(0))
-        pA = _dev_f64(A, (n - 1) * lda + int(ncols_dense))
+        pA = _dev_f64(A, self.bie_hybrid_block_bytes(ncols_dense) // 8)
         assert out_i32.is_cuda and out_i32.dtype == torch.int32 and out_i32.numel() >= 2
         assert workspace.is_cuda and workspace.is_contiguous()
         ws_bytes = workspace.numel() * workspace.element_size()
-        _check(lib().bie_gmres_hybrid(self._h, n, pA, lda, int(ncols_dense), _dev_f64(rhs, n), float(tol), int(restart),
+        _check(lib().bie_gmres_hybrid(self._h, n, pA, int(ncols_dense), _dev_f64(rhs, n), float(tol), int(restart),
                                       int(max_iters), _dev_f64(x, n), out_i32.data_ptr(), _dev_f64(out_f64, 1),
                                       out_i32.data_ptr() + 4,
                                       None if res_hist is None else _dev_f64(res_hist, int(max_iters) + 1),

@@ -29,6 +29,7 @@ int bie_create(bie_ctx** out, int device)
     c->sync_buf = nullptr; c->pinned_i = nullptr; c->pinned_d = nullptr;
     c->near_ptr = nullptr; c->near_col = nullptr; c->near_val = nullptr; c->near_valid = 0; c->near_cap = 0;
     c->hybrid_free_warps = BIE_HYBRID_FREE_WARPS;
+    c->hybrid_poll_tiles = BIE_HYBRID_POLL_TILES;
     c->taubar = nullptr; c->kappa = nullptr;
     c->pc_buf = nullptr; c->pc_cap = 0;
     c->sym_tab = nullptr; c->sym_tab_bytes = 0; c->sym_U = 0; c->geom_gen = 0; c->sync_next = 0;
@@ -157,8 +158,10 @@ int bie_hybrid_cols(bie_ctx* c, int n)
     return hybrid_cols(n, (c->have_geom && c->n == n) ? c->counts[0] : n);
 }
 
+size_t bie_hybrid_block_bytes(int nblock) { return nblock < 1 ? 0 : sizeof(double) * bie_block_doubles(nblock); }
+
 int bie_build_block(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* kinds, const double* zeta,
-                    const double* dzeta, const double* d2zeta, int variant, int nblock, double* A, int64_t lda, void* stream)
+                    const double* dzeta, const double* d2zeta, int variant, int nblock, double* A, void* stream)
 {
     if (variant < BIE_VARIANT_A || variant > BIE_VARIANT_VORTEX) return BIE_ERR_ARG;
     if (!c || !A) return BIE_ERR_NULL;
@@ -166,13 +169,14 @@ int bie_build_block(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t*
     BIE_CUDA(cudaSetDevice(c->device));
     int rc = bie_prepare_nodes(c, ncomp, counts, kinds, zeta, dzeta, d2zeta, variant, (cudaStream_t)stream);
     if (rc != BIE_OK) return rc;
-    return bie_launch_build(c, A, lda, nblock, nblock, 0, (cudaStream_t)stream);
+    return bie_launch_build(c, A, 0 /* block format */, nblock, nblock, 0, (cudaStream_t)stream);
 }
 
 int bie_set_symmetric(bie_ctx* c, int on)
 {
     if (!c) return BIE_ERR_NULL;
     if (on < 0 || on > 2) return BIE_ERR_ARG;
+    if ((c->use_sym != 0) != (on != 0)) c->near_valid = 0;   // the near matrix stores corrections for one or the other
     c->use_sym = on;
     return BIE_OK;
 }
@@ -182,6 +186,14 @@ int bie_set_hybrid_free_warps(bie_ctx* c, int free_warps)
     if (!c) return BIE_ERR_NULL;
     if (free_warps < 1 || free_warps > 15) return BIE_ERR_ARG;
     c->hybrid_free_warps = free_warps;
+    return BIE_OK;
+}
+
+int bie_set_hybrid_poll_tiles(bie_ctx* c, int tiles)
+{
+    if (!c) return BIE_ERR_NULL;
+    if (tiles < 0 || tiles > 64) return BIE_ERR_ARG;
+    c->hybrid_poll_tiles = tiles;
     return BIE_OK;
 }
 
@@ -254,7 +266,7 @@ int bie_gmres(bie_ctx* c, int n, const double* A, int64_t lda, const double* rhs
                             res_hist, workspace, workspace_bytes, (cudaStream_t)stream);
 }
 
-int bie_gmres_hybrid(bie_ctx* c, int n, const double* A, int64_t lda, int ncols_dense, const double* rhs, double tol,
+int bie_gmres_hybrid(bie_ctx* c, int n, const double* A, int ncols_dense, const double* rhs, double tol,
                      int restart, int max_iters, double* x, int32_t* iters_out, double* relres_out,
                      int32_t* status_out, double* res_hist, void* workspace, size_t workspace_bytes, void* stream)
 {
@@ -262,7 +274,7 @@ int bie_gmres_hybrid(bie_ctx* c, int n, const double* A, int64_t lda, int ncols_
     if (!A) return BIE_ERR_NULL;
     if (ncols_dense < 2) return BIE_ERR_ARG;
     BIE_CUDA(cudaSetDevice(c->device));
-    return bie_launch_gmres(c, n, A, lda, ncols_dense, rhs, tol, restart, max_iters, x, iters_out, relres_out,
+    return bie_launch_gmres(c, n, A, 0, ncols_dense, rhs, tol, restart, max_iters, x, iters_out, relres_out,
                             status_out, res_hist, workspace, workspace_bytes, (cudaStream_t)stream);
 }
 
@@ -289,7 +301,7 @@ size_t bie_solve_workspace_bytes(int n, int restart, int matrix_free)
     o += 3 * up256(16 * (size_t)n);          // zeta, dzeta, d2zeta
     o += 2 * up256(8 * nvec);                // rhs, x
     o += up256(64);                          // iters, status, relres
-    if (nld) o += up256(8 * nld * (matrix_free == BIE_OP_HYBRID ? nld : (size_t)n));
+    if (nld) o += up256(matrix_free == BIE_OP_HYBRID ? sizeof(double) * bie_block_doubles((int)nld) : 8 * nld * (size_t)n);
     o += bie_gmres_ws_bytes(n, restart);
     return o;
 }
@@ -322,7 +334,8 @@ int bie_solve_host(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* 
     double* dx = (double*)p; p += up256(8 * nvec);
     int32_t* dint = (int32_t*)p; double* drel = (double*)(p + 16); p += up256(64);
     double* dA = nullptr;
-    if (ncols) { dA = (double*)p; p += up256(8 * nld * (size_t)nrows_st); }
+    const bool blockfmt = (matrix_free == BIE_OP_HYBRID);
+    if (ncols) { dA = (double*)p; p += up256(blockfmt ? sizeof(double) * bie_block_doubles(ncols) : 8 * nld * (size_t)nrows_st); }
     void* gws = p;
     const size_t gws_bytes = bie_gmres_ws_bytes(n, restart);
     BIE_CUDA(cudaMemcpyAsync(dz0, zeta, 16 * (size_t)n, cudaMemcpyHostToDevice, st));
@@ -332,7 +345,7 @@ int bie_solve_host(bie_ctx* c, int ncomp, const int32_t* counts, const int32_t* 
     int rc = bie_prepare_nodes(c, ncomp, counts, kinds, dz0, dz1, dz2, BIE_VARIANT_A, st);
     if (rc != BIE_OK) return rc;
     if (ncols) {
-        rc = bie_launch_build(c, dA, (int64_t)nld, ncols, nrows_st, 0, st);
+        rc = bie_launch_build(c, dA, blockfmt ? 0 : (int64_t)nld, ncols, nrows_st, 0, st);
         if (rc != BIE_OK) return rc;
     }
     rc = bie_launch_gmres(c, n, dA, (int64_t)nld, ncols < n ? ncols : 0, drhs, tol, restart, max_iters, dx, dint, drel,

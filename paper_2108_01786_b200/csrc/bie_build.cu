@@ -83,8 +83,9 @@ bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long l
         scomp[c] = nt.COMP[s0 + c];
     }
     __syncthreads();
-    const bool full = (s0 + 1 < ncols);   // ncols = n, or the width of the hybrid operator's slab
+    const bool full = (s0 + 1 < ncols);   // ncols = n, or the width of the hybrid operator's block
     const bool part = (s0 < ncols);
+    const int nchT = (ncols + BIE_TILE_COLS - 1) / BIE_TILE_COLS;   // block format (lda == 0)
     for (int k = 0; k < ct.ncomp; ++k) {
         const int a = max(t0, ct.off[k]), b = min(t1, ct.off[k + 1]);
         if (a >= b) continue;
@@ -98,14 +99,13 @@ bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long l
         }
         for (int tb = a; tb < b; tb += BUILD_RB) {
             int flag = 0;
-            double* row = A + (long long)tb * lda + s0;
 #pragma unroll
             for (int r = 0; r < BUILD_RB; ++r) {
                 const int t = min(tb + r, b - 1);  // the tail repeats the last row (same values, same address)
                 const double2 te = sE[t - t0];
                 const double e0 = bie_entry_fast(src[0], te, flag);
                 const double e1 = bie_entry_fast(src[1], te, flag);
-                double* p = row + (long long)(t - tb) * lda;
+                double* p = A + bie_entry_off(lda, nchT, t, s0);
                 if (full) *reinterpret_cast<double2*>(p) = make_double2(e0, e1);
                 else if (part) p[0] = e0;
             }
@@ -122,7 +122,7 @@ bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long l
                             if (__double2hiint(den) < src[c].thi) {
                                 double al, be;
                                 bie_block_coef(scomp[c] == 0, k == 0, sqr[c], sqi[c], al, be);
-                                A[(long long)t * lda + s0 + c] =
+                                A[bie_entry_off(lda, nchT, t, s0 + c)] =
                                     bie_entry_near(nt.DG, nt.XY, al, be, (scomp[c] == k) ? sem[c] : 0.0, s0 + c, t);
                             }
                         }
@@ -209,9 +209,9 @@ bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long
     __syncthreads();
     const bool full = (s0 + 1 < ncols);
     const bool part = (s0 < ncols);
+    const int nchT = (ncols + BIE_TILE_COLS - 1) / BIE_TILE_COLS;   // block format (lda == 0)
     for (int tb = t0; tb < t1; tb += BUILD_RB) {
         int flag = 0;
-        double* row = A + (long long)tb * lda + s0;
 #pragma unroll
         for (int r = 0; r < BUILD_RB; ++r) {
             const int t = min(tb + r, t1 - 1);  // the tail repeats the last row (same values, same address)
@@ -223,7 +223,7 @@ bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long
             double e1 = bie_entry_fast_dagger(src[1], te, tm, ab1, flag);
             if (kap[0]) { const int d = t - s0;     e0 += __ldg(kappa + (d < 0 ? d + M0 : d)); }
             if (kap[1]) { const int d = t - s0 - 1; e1 += __ldg(kappa + (d < 0 ? d + M0 : d)); }
-            double* p = row + (long long)(t - tb) * lda;
+            double* p = A + bie_entry_off(lda, nchT, t, s0);
             if (full) *reinterpret_cast<double2*>(p) = make_double2(e0, e1);
             else if (part) p[0] = e0;
         }
@@ -242,7 +242,7 @@ bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long
                             // (A X' + B Y')/den with cot = (-2X + iY)/den; the diagonal entry is prepared per node
                             double v = bie_entry_near(nt.DG, nt.XY, src[c].ms * ab.x, src[c].ms * ab.y, 0.0, s0 + c, t);
                             if (kap[c]) { const int d = t - s0 - c; v += __ldg(kappa + (d < 0 ? d + M0 : d)); }
-                            A[(long long)t * lda + s0 + c] = v;
+                            A[bie_entry_off(lda, nchT, t, s0 + c)] = v;
                         }
                     }
                 }
@@ -258,7 +258,9 @@ int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int ncols, int nrows,
     if (!ctx->have_geom) return BIE_ERR_GEOMETRY;
     const int n = ctx->n;
     if (ncols < 1 || ncols > n || nrows > n) return BIE_ERR_ARG;
-    if (lda < ncols || (lda & 1) || (((uintptr_t)A) & 15u)) return BIE_ERR_LAYOUT;
+    // lda == 0: the block format of the hybrid operator (bie_common.cuh), square blocks only
+    if (lda == 0 ? (nrows != ncols) : (lda < ncols || (lda & 1))) return BIE_ERR_LAYOUT;
+    if (((uintptr_t)A) & 15u) return BIE_ERR_LAYOUT;
     const NodeTable nt = bie_node_table(ctx);
     const int gx = (ncols + BUILD_TILE_W - 1) / BUILD_TILE_W;
     int nt_rows = nrows > 0 ? nrows : n;

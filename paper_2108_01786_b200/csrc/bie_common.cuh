@@ -30,7 +30,8 @@
 #define BIE_NEAR_C 0.25               // tau_s = BIE_NEAR_C |q_s|  (fast-path entry error <= ~1e-14)
 #define BIE_NEAR_TAU_MIN 1.0e-9
 #define BIE_NEAR_TAU_MAX 1.0e-2       // |w| < 0.1: Laurent truncation 2|w/2|^9/93555 < 1e-16
-#define BIE_HYBRID_FREE_WARPS 15       // hybrid operator: warps of a CTA on the pair loops (of 16; one warp issues the bulk copies)
+#define BIE_HYBRID_POLL_TILES 0         // hybrid operator: tiles of the stored block a pair-loop warp may take between two source chunks
+#define BIE_HYBRID_FREE_WARPS 12       // hybrid operator: warps of a CTA on the pair loops (of 16; one warp issues the bulk copies)
 #define BIE_HYBRID_DENSE_FRACTION 0.5625 // hybrid operator: edge of the stored leading block as a share of n (32 % of the entries)
 #define BIE_SYNC_SLOTS 16             // grid-barrier counters of a ctx (bie_matvec_free cycles through them), 256 B apart
 
@@ -79,7 +80,8 @@ struct bie_ctx {
     int smem_set[16];        // dynamic shared memory already granted to the kernel instantiations (cudaFuncSetAttribute once)
     int use_sym;             // use the symmetric work split for the whole-matrix matrix-free operator
     double* kappa;           // [cap] real-cot table of the normal-velocity operator (bie_build_normal_velocity)
-    int hybrid_free_warps;   // hybrid operator: warps per CTA on the pair loops (the other 16 - this stream the slab)
+    int hybrid_free_warps;   // hybrid operator: warps per CTA on the pair loops (warps above it only consume tiles; warp 15 issues the copies)
+    int hybrid_poll_tiles;   // hybrid operator: tiles a pair-loop warp may take between two source chunks (0: it never does)
     unsigned int* sync_buf;  // BIE_SYNC_SLOTS grid-barrier counters (256 B apart) + two device scalars behind them
     int sync_next;           // next counter slot (bie_matvec_free); bie_gmres keeps its counter in the caller's workspace
     int cap;
@@ -126,7 +128,34 @@ static inline int bie_grant_smem(bie_ctx* ctx, int slot, K kernel, size_t smem)
     return BIE_OK;
 }
 
+// Block format of the hybrid operator's stored leading block (bie_build_block -> bie_gmres_hybrid): tiles of
+// BIE_TILE_ROWS rows x BIE_TILE_COLS columns, each tile contiguous (16 KB, row-major inside), tiles in row-major order of
+// (row group, column chunk); rows and columns are padded to whole tiles (the padding is never read).  One tile = ONE
+// bulk copy into shared memory: the TMA engine needs copies of this size to reach HBM speed (4 KB copies: 3.9 TB/s).
+#define BIE_TILE_ROWS 4
+#define BIE_TILE_COLS 512
+static inline size_t bie_block_doubles(int nblock)
+{
+    const size_t ngrp = ((size_t)nblock + BIE_TILE_ROWS - 1) / BIE_TILE_ROWS, nch = ((size_t)nblock + BIE_TILE_COLS - 1) / BIE_TILE_COLS;
+    return ngrp * nch * (BIE_TILE_ROWS * BIE_TILE_COLS);
+}
+#ifdef __CUDACC__
+// offset of entry (t, s): row-major with leading dimension lda, or (lda == 0) the block format with nchT column chunks
+__device__ __forceinline__ long long bie_entry_off(long long lda, int nchT, int t, int s)
+{
+    if (lda) return (long long)t * lda + s;
+    return ((long long)(t / BIE_TILE_ROWS) * nchT + (s / BIE_TILE_COLS)) * (BIE_TILE_ROWS * BIE_TILE_COLS) +
+           (long long)((t % BIE_TILE_ROWS) * BIE_TILE_COLS + (s % BIE_TILE_COLS));
+}
+#endif
+
 static inline int bie_npad(int n) { return (n + BIE_NODE_PAD - 1) / BIE_NODE_PAD * BIE_NODE_PAD; }
+// do the pair loops of the current geometry use the symmetric split (bie_free_sym.cuh)?  Eq. (3.16) variants, and while the
+// reverse partials [row blocks][npad] stay small.  The near matrix is built for one or the other (bie_near.cu).
+static inline bool bie_uses_sym(const bie_ctx* ctx)
+{
+    return ctx->use_sym != 0 && ctx->variant != BIE_VARIANT_VORTEX && bie_npad(ctx->n) <= 65536;
+}
 NodeTable bie_node_table(const bie_ctx* ctx);
 struct FreePlan;
 // doubles of ctx->free_buf for a node capacity `cap`; work split of the matrix-free operator over `grid` CTAs

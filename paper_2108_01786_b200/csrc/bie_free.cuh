@@ -79,9 +79,8 @@ struct FreePlan {
 #endif
 #define SYM_COL_STRIDE 33                                         // [SYM_BATCH][33] doubles per warp: lane-private slots, no bank conflicts
 #define SYM_COL_DOUBLES (FREE_WARPS * SYM_BATCH * SYM_COL_STRIDE)
-// one staging buffer of a warp (32 sources): E and (U,W) as double2; + (R,B) for the vortex-sheet matrix; + the near
-// thresholds (int) for the symmetric loops
-__host__ __device__ inline int free_stage_buf_doubles(bool vortex, bool sym) { return vortex ? 192 : (sym ? 144 : 128); }
+// one staging buffer of a warp (32 sources): E and (U,W) as double2; + (R,B) for the vortex-sheet matrix
+__host__ __device__ inline int free_stage_buf_doubles(bool vortex, bool /*sym*/) { return vortex ? 192 : 128; }
 // shared scratch of the operator: head, [16 warps][2 buffers] staging, and the reverse-sum slots of the symmetric loops
 __host__ __device__ inline int free_scratch_doubles(bool vortex, bool sym)
 {
@@ -245,12 +244,15 @@ __device__ __forceinline__ void free_parts_impl(const NodeTable& nt, const CompT
         int buf = 0;
         __syncwarp();
         if (wa < wb) issue(wa, 0);
-        for (int base = wa; base < wb; base += 32, buf ^= 1) {
+        // the first chunk of warp w is shorter by 2 w sources: the warps reach their poll() calls evenly spread in time instead
+        // of all at once (the ring of the hybrid operator is only a few tiles deep)
+        int len = 32 - 2 * (warp & 15);
+        for (int base = wa; base < wb; base += len, len = 32, buf ^= 1) {
             const double2* sg = stage + buf * (fp.stage_buf >> 1);
             asm volatile("cp.async.wait_group 0;" ::: "memory");
             __syncwarp();                                   // chunk landed for all lanes; the other buffer is no longer read
-            if (base + 32 < wb) issue(base + 32, buf ^ 1);
-            const int cnt = min(32, wb - base);   // even
+            if (base + len < wb) issue(base + len, buf ^ 1);
+            const int cnt = min(len, wb - base);   // even
 #pragma unroll FREE_SRC_UNROLL
             for (int j = 0; j < cnt; ++j) {
                 const double2 e = sg[j], pq = sg[32 + j];

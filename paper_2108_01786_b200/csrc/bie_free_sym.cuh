@@ -12,8 +12,13 @@
 // gathers the forward partials of J and  sum_{I < J} PC[I][t]  in fixed order: deterministic.
 // Reverse sums of 8 consecutive sources are reduced over the lanes through lane-private shared-memory slots (a transposing
 // shuffle butterfly was 3 % slower: its 9 dependent steps stall the warp).
-// Near pairs: forward skipped when den < taubar M_t, reverse when den < taubar M_s -- the row-based rule of bie_near.cu,
-// whose CSR matrix supplies both.
+// Near pairs.  In the block's own rows (which hold the pair s == t, den = 0) a pair with den < taubar M_t is left out by
+// predication, as in bie_free.cuh.  In the symmetric segments there is NO test at all: every pair is summed with the fast
+// arithmetic, and the CSR near matrix of bie_near.cu stores, for the pairs it lists that lie in different row blocks,
+// the CORRECTION exact - fast instead of the exact entry.  Both fast values come from the same rounded E_s - E_t, so they
+// agree to a few ulp and the correction is as accurate as the exact entry; the pair loop loses two compares and four
+// selects per pair and the registers of the thresholds (ncu: the loop was bound by issue slots and latency, not by
+// the FP64 pipe).  Distinct nodes that coincide exactly (a pole of the kernel) give Inf/NaN, as the exact entry would.
 // Hybrid operator (fp.s_off > 0, a row-block boundary): the leading s_off x s_off block is stored; every other pair {t, s},
 // t < s, has s >= s_off, so the list is the same triangle with the sources cut at s_off: row blocks below s_off take the
 // sources [s_off, npad) symmetrically (forward into their rows, reverse into the rows from s_off on).
@@ -43,7 +48,7 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
     const int c = blockIdx.x;
     if (c >= fp.Geff) return;
     double* wsum = scratch;
-    const int sbuf = fp.stage_buf;                                   // 144 doubles: E [32] double2, (U,W) [32] double2, thresholds [32] int
+    const int sbuf = fp.stage_buf;                                   // 128 doubles: E [32] double2, (U,W) [32] double2
     double* stage = scratch + FREE_HEAD_DOUBLES + warp * 2 * sbuf;
     double* col = scratch + FREE_HEAD_DOUBLES + FREE_WARPS * 2 * sbuf + warp * (SYM_BATCH * SYM_COL_STRIDE);   // this warp's reverse sums of a batch
     const int np = nt.npad;
@@ -98,28 +103,28 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
                 }
             }
             double2 ne = zero2, nuw = zero2;
-            int nth = 0;
             if (wa + lane < wb) {
                 const int s = wa + lane;
                 ne = nt.E[s]; nuw = __ldcg(TUW + s);
-                nth = __double2hiint(taubar * nt.MT[s].x);
             }
             int buf = 0;
             __syncwarp();
-            for (int base = wa; base < wb; base += 32, buf ^= 1) {
+            // the first chunk of warp w is shorter by 2 w sources (a multiple of SYM_BATCH would be kinder to the batches, but the
+            // tail batch handles any count): the warps reach their poll() calls evenly spread in time instead of all at once
+            int len = 32 - 2 * (warp & 15);
+            for (int base = wa; base < wb; base += len, len = 32, buf ^= 1) {
                 double2* sg = reinterpret_cast<double2*>(stage + buf * sbuf);
-                int* sth = reinterpret_cast<int*>(stage + buf * sbuf + 128);
-                sg[lane] = ne; sg[32 + lane] = nuw; sth[lane] = nth;
+                {   // lanes beyond this chunk stage zero sources (the batches below run over whole multiples of SYM_BATCH)
+                    const bool in = lane < len;
+                    sg[lane] = in ? ne : zero2; sg[32 + lane] = in ? nuw : zero2;
+                }
                 __syncwarp();
                 {
-                    const int s = base + 32 + lane;
-                    ne = zero2; nuw = zero2; nth = 0;
-                    if (s < wb) {
-                        ne = nt.E[s]; nuw = __ldcg(TUW + s);
-                        nth = __double2hiint(taubar * nt.MT[s].x);
-                    }
+                    const int s = base + len + lane;
+                    ne = zero2; nuw = zero2;
+                    if (s < wb) { ne = nt.E[s]; nuw = __ldcg(TUW + s); }
                 }
-                const int cnt = min(32, wb - base);
+                const int cnt = min(len, wb - base);
                 if (!rev) {
 #pragma unroll 2
                     for (int j = 0; j < cnt; ++j) {
@@ -139,7 +144,6 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
                         for (int u = 0; u < SYM_BATCH; ++u) {
                             const int j = j0 + u;
                             const double2 e = sg[j], uw = sg[32 + j];
-                            const int thj = sth[j];
                             double s_rev0 = 0.0, s_rev1 = 0.0;
 #pragma unroll
                             for (int i = 0; i < FREE_NT; ++i) {
@@ -147,14 +151,13 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
                                 const double den = fma(dr, dr, di * di);
                                 const double val = fma(uw.y, di, uw.x * dr);
                                 const double r = bie_rcp3(den);
-                                const int dh = __double2hiint(den);
-                                if (!(dh < thi[i])) acc[i] = fma(val, r, acc[i]);
+                                acc[i] = fma(val, r, acc[i]);
                                 // reverse entry A[s][t] x_t: row s, source t (its (U, W) for the class of s), E_t - E_s = -(dr + i di);
-                                // the sign is applied once to the sum
+                                // the sign is applied once, after the lane reduction
                                 const double vr = fma(tw[i], di, tu[i] * dr);
-                                if (!(dh < thj)) { if (i & 1) s_rev1 = fma(vr, r, s_rev1); else s_rev0 = fma(vr, r, s_rev0); }
+                                if (i & 1) s_rev1 = fma(vr, r, s_rev1); else s_rev0 = fma(vr, r, s_rev0);
                             }
-                            col[u * SYM_COL_STRIDE + lane] = -(s_rev0 + s_rev1);
+                            col[u * SYM_COL_STRIDE + lane] = s_rev0 + s_rev1;
                         }
                         // lane reduction of the SYM_BATCH reverse sums through shared memory: 32 / SYM_BATCH lanes share a source,
                         // each adds 8 slots, shuffles finish (fixed order)
@@ -169,7 +172,7 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
 #pragma unroll
                             for (int o = LPS >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
                             const int j = j0 + lane / LPS;
-                            if ((lane % LPS) == 0 && j < cnt) fp.PC[(size_t)b * np + base + j] = v;
+                            if ((lane % LPS) == 0 && j < cnt) fp.PC[(size_t)b * np + base + j] = -v;
                         }
                         __syncwarp();
                     }

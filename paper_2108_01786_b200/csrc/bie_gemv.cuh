@@ -150,19 +150,10 @@ __device__ __forceinline__ void bie_cta_gemv(const double* __restrict__ A, long 
 #ifndef RING_STAGES
 #define RING_STAGES 4
 #endif
-#define RING_ROWS 4
+#define RING_ROWS BIE_TILE_ROWS      // a ring tile is a tile of the block format (bie_common.cuh): ONE 16 KB bulk copy
 
-// doubles per (row, chunk) of a ring tile: at most 512 (a tile = 4 rows + x = 20 KB), smaller while the CTA has fewer
-// than two tiles per warp; a multiple of 64 (bulk copies need 16-byte sizes and addresses)
-__host__ __device__ inline int ring_chunk(int rows_per_cta, int nd, int nwarp)
-{
-    int chunk = 512;
-    const int ngrp = (rows_per_cta + RING_ROWS - 1) / RING_ROWS;
-    while (chunk > 128 && ngrp * ((nd + chunk - 1) / chunk) < 2 * nwarp) chunk >>= 1;
-    const int nch = (nd + chunk - 1) / chunk;
-    chunk = ((nd + nch - 1) / nch + 63) & ~63;
-    return chunk;
-}
+// doubles per (row, chunk) of a ring tile = BIE_TILE_COLS
+__host__ __device__ inline int ring_chunk(int /*rows_per_cta*/, int /*nd*/, int /*nwarp*/) { return BIE_TILE_COLS; }
 // shared memory of the ring: RING_STAGES tiles of (RING_ROWS + 1) x chunk doubles, then 2 RING_STAGES mbarriers and the
 // tile counter (padded to an even number of doubles)
 __host__ __device__ inline int ring_doubles(int chunk) { return RING_STAGES * (RING_ROWS + 1) * chunk + 2 * RING_STAGES + 2; }
@@ -192,6 +183,14 @@ __device__ __forceinline__ bool mbar_test(unsigned bar, unsigned parity)
                  : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     return ok != 0;
 }
+// non-blocking probe (try_wait may suspend the thread for a hardware-defined time before it answers "not yet")
+__device__ __forceinline__ bool mbar_probe(unsigned bar, unsigned parity)
+{
+    unsigned ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
+}
 __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
 {
     while (!mbar_test(bar, parity)) { }
@@ -209,12 +208,11 @@ __device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned
 }
 
 struct BlockRing {
-    const double* A;          // stored block, row-major, leading dimension lda
-    long long lda;
+    const double* A;          // stored block in the block format (bie_common.cuh)
     int nd, r0, r1, chunk;    // columns (= rows) of the block, the rows this CTA streams, doubles per (row, chunk)
     int nch, nunit;           // chunks per row, tiles of one application
     unsigned full0, empty0;   // shared addresses of the mbarriers: full[s] = full0 + 8 s, empty[s] = empty0 + 8 s
-    int* next;                // shared: next tile to claim
+    int* next;                // shared: next tile to claim; next[1] = tiles the producer has issued in this application
     const double* stage;      // shared: RING_STAGES tiles of (RING_ROWS + 1) x chunk doubles (rows, then x)
     double* part;             // shared: [nch][rowsP] row sums of the tiles
     int rowsP;
@@ -245,32 +243,31 @@ __device__ __forceinline__ void ring_produce(const BlockRing& R, const double* x
         const unsigned s = (unsigned)(gidx % RING_STAGES), use = (unsigned)(gidx / RING_STAGES);
         mbar_wait(R.empty0 + 8 * s, (use & 1u) ^ 1u);
         const int p = t / R.nch, ch = t - p * R.nch;
-        const int ra = R.r0 + RING_ROWS * p;
-        const int nr = min(RING_ROWS, R.r1 - ra);
         const int cbeg = ch * R.chunk, cend = min(cbeg + R.chunk, R.nd);
-        const unsigned bytes = 8u * (unsigned)(cend - cbeg);
+        const unsigned xbytes = 8u * (unsigned)(cend - cbeg);
+        const unsigned tbytes = 8u * RING_ROWS * BIE_TILE_COLS;
         const unsigned dst = stage_addr + s * (unsigned)(8 * (RING_ROWS + 1) * R.chunk);
-        mbar_arrive_expect_tx(R.full0 + 8 * s, (unsigned)(nr + 1) * bytes);
-        for (int i = 0; i < nr; ++i)
-            bulk_g2s<STREAM>(dst + 8u * (unsigned)(i * R.chunk), R.A + (long long)(ra + i) * R.lda + cbeg, bytes, R.full0 + 8 * s, pol);
-        bulk_g2s<false>(dst + 8u * (unsigned)(RING_ROWS * R.chunk), xin + cbeg, bytes, R.full0 + 8 * s, 0);   // x: L2-resident
+        mbar_arrive_expect_tx(R.full0 + 8 * s, tbytes + xbytes);
+        bulk_g2s<STREAM>(dst, R.A + ((long long)(R.r0 / RING_ROWS + p) * R.nch + ch) * (RING_ROWS * BIE_TILE_COLS), tbytes,
+                         R.full0 + 8 * s, pol);
+        bulk_g2s<false>(dst + tbytes, xin + cbeg, xbytes, R.full0 + 8 * s, 0);   // x: L2-resident
+        // a consumer may wait for tile t only from here on: mbarrier waits tell phases apart by parity alone, and the
+        // previous use of this slot has completed now
+        *reinterpret_cast<volatile int*>(R.next + 1) = t + 1;
     }
 }
 
-// a whole warp: claims the next tile; returns false when none is left.  Blocks until the tile has landed.
-__device__ __forceinline__ bool ring_consume(const BlockRing& R)
+// a whole warp: multiplies tile t (claimed by this warp) with its x chunk as soon as it has landed
+__device__ __forceinline__ void ring_tile(const BlockRing& R, int t)
 {
     const int lane = threadIdx.x & 31;
-    int t = 0;
-    if (lane == 0) t = atomicAdd(R.next, 1);
-    t = __shfl_sync(0xffffffffu, t, 0);
-    if (t >= R.nunit) return false;
     const unsigned long long gidx = R.tile0 + t;
     const unsigned s = (unsigned)(gidx % RING_STAGES), use = (unsigned)(gidx / RING_STAGES);
     const int p = t / R.nch, ch = t - p * R.nch;
     const int nr = min(RING_ROWS, R.r1 - (R.r0 + RING_ROWS * p));
     const int cbeg = ch * R.chunk, cend = min(cbeg + R.chunk, R.nd);
     const int n2 = (cend - cbeg) >> 1;
+    while (*reinterpret_cast<volatile int*>(R.next + 1) <= t) { }     // issued (see ring_produce)
     mbar_wait(R.full0 + 8 * s, use & 1u);
     const double2* a = reinterpret_cast<const double2*>(R.stage + (size_t)s * (RING_ROWS + 1) * R.chunk);
     const int ch2 = R.chunk >> 1;
@@ -280,24 +277,26 @@ __device__ __forceinline__ bool ring_consume(const BlockRing& R)
     for (int i = 0; i < RING_ROWS; ++i) { acc[i] = 0.0; bcc[i] = 0.0; }
     // rows the tile does not have are read anyway (stale shared memory, finite or not) and their sums dropped
     int c = lane;
-    for (; c + 32 < n2; c += 64) {
-        const double2 xa = x2[c], xb = x2[c + 32];
-        double2 va[RING_ROWS], vb[RING_ROWS];
+    if (RING_ROWS <= 4) {
+        for (; c + 32 < n2; c += 64) {
+            const double2 xa = x2[c], xb = x2[c + 32];
+            double2 va[RING_ROWS], vb[RING_ROWS];
 #pragma unroll
-        for (int i = 0; i < RING_ROWS; ++i) { va[i] = a[i * ch2 + c]; vb[i] = a[i * ch2 + c + 32]; }
+            for (int i = 0; i < RING_ROWS; ++i) { va[i] = a[i * ch2 + c]; vb[i] = a[i * ch2 + c + 32]; }
 #pragma unroll
-        for (int i = 0; i < RING_ROWS; ++i) {
-            acc[i] = fma(va[i].x, xa.x, acc[i]); bcc[i] = fma(va[i].y, xa.y, bcc[i]);
-            acc[i] = fma(vb[i].x, xb.x, acc[i]); bcc[i] = fma(vb[i].y, xb.y, bcc[i]);
+            for (int i = 0; i < RING_ROWS; ++i) {
+                acc[i] = fma(va[i].x, xa.x, acc[i]); bcc[i] = fma(va[i].y, xa.y, bcc[i]);
+                acc[i] = fma(vb[i].x, xb.x, acc[i]); bcc[i] = fma(vb[i].y, xb.y, bcc[i]);
+            }
         }
     }
     for (; c < n2; c += 32) {
         const double2 xa = x2[c];
+        double2 va[RING_ROWS];
 #pragma unroll
-        for (int i = 0; i < RING_ROWS; ++i) {
-            const double2 va = a[i * ch2 + c];
-            acc[i] = fma(va.x, xa.x, acc[i]); bcc[i] = fma(va.y, xa.y, bcc[i]);
-        }
+        for (int i = 0; i < RING_ROWS; ++i) va[i] = a[i * ch2 + c];
+#pragma unroll
+        for (int i = 0; i < RING_ROWS; ++i) { acc[i] = fma(va[i].x, xa.x, acc[i]); bcc[i] = fma(va[i].y, xa.y, bcc[i]); }
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(R.empty0 + 8 * s);     // the slot may be refilled
@@ -306,26 +305,47 @@ __device__ __forceinline__ bool ring_consume(const BlockRing& R)
         const double v = bie_warp_sum(acc[i] + bcc[i]);
         if (lane == 0 && i < nr) R.part[ch * R.rowsP + RING_ROWS * p + i] = v;
     }
+}
+
+// a whole warp: claims the next tile and multiplies it; returns false when none is left.  Blocks until the tile has landed.
+__device__ __forceinline__ bool ring_consume(const BlockRing& R)
+{
+    int t = 0;
+    if ((threadIdx.x & 31) == 0) t = atomicAdd(R.next, 1);
+    t = __shfl_sync(0xffffffffu, t, 0);
+    if (t >= R.nunit) return false;
+    ring_tile(R, t);
     return true;
 }
 
-// a whole warp, between two source chunks of its pair loop: takes up to `max_tiles` tiles that have ALREADY landed.
-// Not inlined: the pair loops around the call keep their register allocation.
-static __device__ __noinline__ void ring_poll(const BlockRing& R, int max_tiles)
+// a whole warp: the next unclaimed tile if it has ALREADY landed and this warp wins the claim, else -1 (never blocks:
+// two shared-memory reads, one mbarrier probe, one compare-and-swap)
+__device__ __forceinline__ int ring_try_claim(const BlockRing& R)
 {
-    for (int k = 0; k < max_tiles; ++k) {
-        const int t = *reinterpret_cast<volatile int*>(R.next);
-        if (t >= R.nunit) return;
-        const unsigned long long gidx = R.tile0 + t;
-        if (!mbar_test(R.full0 + 8 * (unsigned)(gidx % RING_STAGES), (unsigned)(gidx / RING_STAGES) & 1u)) return;
-        if (!ring_consume(R)) return;
-    }
+    const int t = *reinterpret_cast<volatile int*>(R.next);
+    if (t >= R.nunit || *reinterpret_cast<volatile int*>(R.next + 1) <= t) return -1;
+    const unsigned long long gidx = R.tile0 + t;
+    if (!mbar_probe(R.full0 + 8 * (unsigned)(gidx % RING_STAGES), (unsigned)(gidx / RING_STAGES) & 1u)) return -1;
+    int won = 0;
+    if ((threadIdx.x & 31) == 0) won = (atomicCAS(R.next, t, t + 1) == t);
+    won = __shfl_sync(0xffffffffu, won, 0);
+    return won ? t : -1;
 }
+// not inlined: the pair loops around the call keep their register allocation
+static __device__ __noinline__ void ring_tile_call(const BlockRing& R, int t) { ring_tile(R, t); }
 
 // what the pair loops of bie_free.cuh call between source chunks
 struct NoPoll { __device__ __forceinline__ void operator()() const {} };
 struct RingPoll {
     const BlockRing* R;
     int max_tiles;
-    __device__ __forceinline__ void operator()() const { ring_poll(*R, max_tiles); }
+    // a whole warp, between two source chunks of its pair loop: takes up to max_tiles tiles that have ALREADY landed
+    __device__ __forceinline__ void operator()() const
+    {
+        for (int k = 0; k < max_tiles; ++k) {
+            const int t = ring_try_claim(*R);
+            if (t < 0) return;
+            ring_tile_call(*R, t);
+        }
+    }
 };

@@ -33,9 +33,6 @@
 #define GM_THREADS 512
 #endif
 #define GM_WARPS (GM_THREADS / 32)
-#ifndef RING_POLL_TILES
-#define RING_POLL_TILES 3   // hybrid operator: tiles of the stored block a warp may take between two source chunks
-#endif
 
 struct GmresArgs {
     const double* A;
@@ -63,6 +60,7 @@ struct GmresArgs {
     int nd;        // hybrid operator: the leading nd x nd block comes from the stored block A, everything else is recomputed
     int nwf;       // hybrid operator: warps 0..nwf-1 run the pair loops (and take tiles of the stored block in between), warps
                    // nwf..14 only take tiles, warp 15 issues the bulk copies
+    int poll_tiles; // hybrid operator: tiles a pair-loop warp may take between two source chunks
     int brows;     // hybrid operator: rows of the stored block each CTA streams (a multiple of RING_ROWS)
     double* yd;    // hybrid operator: [nld] product of the stored block with x[0, nd), written by the CTAs that streamed the rows
     int res_pairs; // streaming GEMV: leading row pairs of every CTA block kept L2-resident (bie_gemv.cuh)
@@ -126,16 +124,52 @@ __device__ __forceinline__ void cta_apply(const GmresArgs& a, int r0, int r1, co
             free_parts(a.nt, a.ct, a.fp, gpart, cta_team(), NoPoll());
         } else {
             const int warp = threadIdx.x >> 5;
-            if (threadIdx.x == 0) *ring.next = 0;
+            if (threadIdx.x == 0) { ring.next[0] = 0; ring.next[1] = 0; }
             __syncthreads();
+#ifdef BIE_PHASE_TIMING
+            __shared__ unsigned long long hy_acc[4];
+            if (threadIdx.x == 0 && ring.tile0 == 0) { hy_acc[0] = hy_acc[1] = hy_acc[2] = hy_acc[3] = 0; }
+            const unsigned long long hy_t0 = gtime();
+#endif
+            // nwf >= 12: the service warps -- the producer (warp 15) and 15 - nwf consumer warps -- all sit on ONE of the SM's
+            // four sub-partitions (warp & 3 == 3: warps 15, 11, 7, 3), so that they do not wait for issue slots behind the
+            // pair-loop warps of the other three.  nwf = 12: the pair loops run on exactly three sub-partitions, four warps
+            // each, as in the matrix-free kernel.  nwf < 12: warps nwf..14 consume, wherever they sit.
+            const bool split = (a.nwf >= 12);
+            const int first_service = 3 + 4 * (a.nwf - 12);                     // split: service warps are first_service, +4, ..., 15
+            const bool service = split ? ((warp & 3) == 3 && warp >= first_service) : (warp >= a.nwf);
             if (warp == GM_WARPS - 1) {
                 if ((threadIdx.x & 31) == 0) ring_produce<STREAM>(ring, xin);
                 __syncwarp();
+#ifdef BIE_PHASE_TIMING
+                if ((threadIdx.x & 31) == 0) hy_acc[2] += gtime() - hy_t0;
+#endif
             } else {
-                if (warp < a.nwf) free_parts(a.nt, a.ct, a.fp, gpart, sub_team(0, a.nwf, 1), RingPoll{&ring, RING_POLL_TILES});
+                if (!service) {
+                    Team tm = sub_team(0, a.nwf, 1);
+                    if (split) {   // index among the pair-loop warps: the service warps below this one do not count
+                        tm.warp = warp - (warp > first_service ? ((warp - first_service + 3) >> 2) : 0);
+                        tm.tid = 32 * tm.warp + (threadIdx.x & 31);
+                    }
+                    free_parts(a.nt, a.ct, a.fp, gpart, tm, RingPoll{&ring, a.poll_tiles});
+                }
+#ifdef BIE_PHASE_TIMING
+                if (threadIdx.x == 0) hy_acc[0] += gtime() - hy_t0;
+#endif
                 while (ring_consume(ring)) { }
+#ifdef BIE_PHASE_TIMING
+                if (threadIdx.x == 0) hy_acc[1] += gtime() - hy_t0;
+#endif
             }
             __syncthreads();
+#ifdef BIE_PHASE_TIMING
+            if (threadIdx.x == 0) {
+                hy_acc[3] += 1;
+                if (hy_acc[3] == 40 && (blockIdx.x == 0 || blockIdx.x == 100))
+                    printf("cta %d hybrid us/apply: pair loops (warp 0) %.1f, + drain %.1f, producer done %.1f\n", blockIdx.x,
+                           hy_acc[0] * 1e-3 / 40, hy_acc[1] * 1e-3 / 40, hy_acc[2] * 1e-3 / 40);
+            }
+#endif
             // the rows of the stored block this CTA streamed: chunk sums in fixed order -> yd (their owners read it after the barrier)
             for (int r = threadIdx.x; r < ring.r1 - ring.r0; r += blockDim.x) {
                 double sum = 0.0;
@@ -307,7 +341,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
                                : ((MODE == 1) ? ring_part : xs + (XS ? ((n + 2) & ~1) : 0));   // [blockDim + rows2]
     BlockRing ring;
     if (MODE == 2) {
-        ring.A = a.A; ring.lda = a.lda; ring.nd = a.nd; ring.chunk = a.chunk;
+        ring.A = a.A; ring.nd = a.nd; ring.chunk = a.chunk;
         ring.r0 = min(blockIdx.x * a.brows, a.nd); ring.r1 = min(ring.r0 + a.brows, a.nd);
         ring.nch = (a.nd + a.chunk - 1) / a.chunk;
         ring.nunit = ((ring.r1 - ring.r0 + RING_ROWS - 1) / RING_ROWS) * ring.nch;
@@ -601,7 +635,10 @@ static int gmres_plan(int n, int restart, int sm_count, int max_smem, int l2_byt
     // (dense operator: the streaming loads of A need the L1 as their landing buffer, 16 warps x 4 KB in flight,
     // so the shared-memory carve-out stops at 164 KB; measured: 408 us per step with 227 KB against 338 us.
     // The hybrid operator's block arrives by bulk copies into shared memory and needs no L1.)
-    const size_t cap = mode != 0 ? (size_t)max_smem : (size_t)(163 * 1024 < max_smem ? 163 * 1024 : max_smem);
+    size_t cap = mode != 0 ? (size_t)max_smem : (size_t)(163 * 1024 < max_smem ? 163 * 1024 : max_smem);
+#ifdef BIE_PHASE_TIMING
+    cap -= 1024;   // the developer build has a few static shared variables
+#endif
     pl->VS = pl->smem < cap ? (int)((cap - pl->smem) / (sizeof(double) * rows2)) : 0;
     if (pl->VS > m + 1) pl->VS = m + 1;
     pl->smem += sizeof(double) * (size_t)pl->VS * rows2;
@@ -641,7 +678,8 @@ int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, int nd, 
     const int mode = nd > 0 ? 2 : (A == nullptr ? 1 : 0);
     const bool free_op = (mode != 0);
     if (free_op && (!ctx->have_geom || ctx->n != n)) return BIE_ERR_GEOMETRY;
-    if (mode != 1 && (lda < (mode == 2 ? nd : n) || (lda & 1) || (((uintptr_t)A) & 15u))) return BIE_ERR_LAYOUT;
+    if (mode == 0 && (lda < n || (lda & 1))) return BIE_ERR_LAYOUT;     // hybrid: A is in the block format, lda is not used
+    if (mode != 1 && (((uintptr_t)A) & 15u)) return BIE_ERR_LAYOUT;
     if ((((uintptr_t)rhs) | ((uintptr_t)x)) & 15u) return BIE_ERR_LAYOUT;
     if (!ctx->coop_ok) return BIE_ERR_DEVICE;
     if (ctx->sm_count > 256) return BIE_ERR_DEVICE;
@@ -674,7 +712,7 @@ int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, int nd, 
     a.yd = (double*)(base + pl.offD);
     a.sync = (unsigned int*)(base + pl.offS);     // per call: two solves of one ctx never share a barrier counter
     a.nld = pl.nld; a.rows_per_cta = pl.rows_per_cta; a.chunk = pl.chunk; a.VS = pl.VS;
-    a.nd = nd; a.nwf = ctx->hybrid_free_warps; a.scratch_doubles = pl.scratch_doubles; a.brows = pl.brows;
+    a.nd = nd; a.nwf = ctx->hybrid_free_warps; a.poll_tiles = ctx->hybrid_poll_tiles; a.scratch_doubles = pl.scratch_doubles; a.brows = pl.brows;
     a.res_pairs = (mode == 0 && pl.stream)
         ? bie_gemv_resident_pairs(ctx->l2_bytes, n, (long long)lda, pl.rows_per_cta, sizeof(double) * (size_t)(restart + 2) * pl.nld) : 0;
     BIE_CUDA(cudaMemsetAsync(a.sync, 0, sizeof(unsigned int), st));

@@ -22,7 +22,8 @@
 
 template <bool FILL>
 __global__ void __launch_bounds__(NEAR_THREADS)
-bie_near_kernel(NodeTable nt, CompTable ct, int vortex, const double* __restrict__ taubar, int* __restrict__ cnt /* [n][NEAR_SEG] counts or offsets */,
+bie_near_kernel(NodeTable nt, CompTable ct, int vortex, int sym /* 1: pairs of different row blocks store exact - fast */,
+                const double* __restrict__ taubar, int* __restrict__ cnt /* [n][NEAR_SEG] counts or offsets */,
                 int* __restrict__ col, double* __restrict__ val, int cap)
 {
     __shared__ double2 sE[NEAR_TILE];
@@ -80,6 +81,18 @@ bie_near_kernel(NodeTable nt, CompTable ct, int vortex, const double* __restrict
                             v = fma(be, ci, -0.5 * al * cr);   // cot = (-2X + iY)/den
                         }
                         if (!vortex) v += be;   // the operator subtracts sum_s beta_s x_s over ALL sources (difference form)
+                        if (sym && s != t) {
+                            // the symmetric pair loops (bie_free_sym.cuh) test nothing outside a row block's own rows: they add the
+                            // FAST value of this pair, and this entry corrects it.  Row blocks: 128 rows, cut per class at M_0.
+                            const int M0 = ct.off[1];
+                            const int bt = t < M0 ? t / 128 : (M0 + 127) / 128 + (t - M0) / 128;
+                            const int bs = s < M0 ? s / 128 : (M0 + 127) / 128 + (s - M0) / 128;
+                            if (bt != bs) {
+                                const double2 es = nt.E[s];
+                                const double u = fma(al, es.y, 2.0 * be * es.x), w = fma(-al, es.x, 2.0 * be * es.y);
+                                v -= fma(w, di, u * dr) * bie_rcp3(den);
+                            }
+                        }
                         col[p] = s;
                         val[p] = v;
                     }
@@ -137,8 +150,9 @@ int bie_ensure_near(bie_ctx* ctx, cudaStream_t st)
     const NodeTable nt = bie_node_table(ctx);
     const int n = ctx->n;
     const int vx = (ctx->variant == BIE_VARIANT_VORTEX) ? 1 : 0;
+    const int sym = bie_uses_sym(ctx) ? 1 : 0;
     dim3 grid((n + NEAR_THREADS - 1) / NEAR_THREADS, NEAR_SEG);
-    bie_near_kernel<false><<<grid, NEAR_THREADS, 0, st>>>(nt, ctx->comps, vx, ctx->taubar, ctx->near_ptr, nullptr, nullptr, 0);
+    bie_near_kernel<false><<<grid, NEAR_THREADS, 0, st>>>(nt, ctx->comps, vx, sym, ctx->taubar, ctx->near_ptr, nullptr, nullptr, 0);
     bie_near_scan_kernel<<<1, 1024, 0, st>>>(ctx->near_ptr, n * NEAR_SEG);
     BIE_CUDA(cudaGetLastError());
     BIE_CUDA(cudaMemcpyAsync(ctx->pinned_i + 2, ctx->near_ptr + (size_t)n * NEAR_SEG, sizeof(int), cudaMemcpyDeviceToHost, st));
@@ -154,7 +168,7 @@ int bie_ensure_near(bie_ctx* ctx, cudaStream_t st)
         BIE_CUDA(cudaMalloc((void**)&ctx->near_val, sizeof(double) * cap));
         ctx->near_cap = cap;
     }
-    bie_near_kernel<true><<<grid, NEAR_THREADS, 0, st>>>(nt, ctx->comps, vx, ctx->taubar, ctx->near_ptr, ctx->near_col, ctx->near_val,
+    bie_near_kernel<true><<<grid, NEAR_THREADS, 0, st>>>(nt, ctx->comps, vx, sym, ctx->taubar, ctx->near_ptr, ctx->near_col, ctx->near_val,
                                                         (int)ctx->near_cap);
     BIE_CUDA(cudaGetLastError());
     ctx->near_valid = 1;

@@ -216,7 +216,7 @@ int bie_free_plan(bie_ctx* ctx, int grid, int s_off, FreePlan* fp, cudaStream_t 
     fp->U = (long long)first * fp->UBb + (long long)(fp->NB - first) * fp->UBf;
     // symmetric work split (bie_free_sym.cuh): Eq. (3.16) variants, and while the reverse partials [NB][npad] stay small
     fp->sym = 0; fp->PC = nullptr; fp->sym_cum = nullptr; fp->sym_perm = nullptr; fp->sym_pos = nullptr;
-    if (ctx->use_sym && !fp->vortex && npad <= 65536) {
+    if (bie_uses_sym(ctx)) {
         const int NB = fp->NB;
         const size_t need = (size_t)NB * (size_t)npad;
         if (need > ctx->pc_cap) {

@@ -378,8 +378,8 @@ def test_vortex_matrix_free_and_hybrid(ctx, c):
     assert sto == 0 and st == 0 and abs(it - ito) <= 1 and rr <= 10 * P.tol
     assert np.linalg.norm(xg - xo) / np.linalg.norm(xo) <= TOL_X
     nd = ctx.bie_hybrid_cols(n)
-    A = torch.full((n, nd), float("nan"), dtype=torch.float64, device="cuda")
-    ctx.bie_build_cols(g.counts, g.kinds, z, dz, d2z, nd, A, variant=2)
+    A = torch.full((bie.Context.bie_hybrid_block_bytes(nd) // 8,), float("nan"), dtype=torch.float64, device="cuda")
+    ctx.bie_build_block(g.counts, g.kinds, z, dz, d2z, nd, A, variant=2)
     ws = torch.empty(bie.Context.bie_gmres_workspace_bytes(n, P.restart), dtype=torch.uint8, device="cuda")
     oi = torch.zeros(2, dtype=torch.int32, device="cuda"); of = torch.zeros(1, dtype=torch.float64, device="cuda")
     xh = torch.empty(n, dtype=torch.float64, device="cuda")
@@ -676,9 +676,9 @@ def test_matrix_free_and_hybrid_with_the_uncorrected_operator(ctx):
     b = _x(n, 22)
     xd, itd, rrd, std_ = gpu_gmres(ctx, gpu_build(ctx, g, variant=1), b, 1e-13, 50, 3)
     nd = 1024
-    A = torch.full((n, nd), float("nan"), dtype=torch.float64, device="cuda")
-    ctx.bie_build_cols(g.counts, g.kinds, z, dz, d2z, nd, A, variant=1)
     from paper_2108_01786_b200 import bie
+    A = torch.full((bie.Context.bie_hybrid_block_bytes(nd) // 8,), float("nan"), dtype=torch.float64, device="cuda")
+    ctx.bie_build_block(g.counts, g.kinds, z, dz, d2z, nd, A, variant=1)
     ws = torch.empty(bie.Context.bie_gmres_workspace_bytes(n, 50), dtype=torch.uint8, device="cuda")
     oi = torch.zeros(2, dtype=torch.int32, device="cuda"); of = torch.zeros(1, dtype=torch.float64, device="cuda")
     xh = torch.empty(n, dtype=torch.float64, device="cuda")
@@ -805,33 +805,42 @@ def test_gmres_matrix_free_parity(ctx, c):
     assert rr <= 10 * P.tol
 
 
-def gpu_gmres_hybrid(ctx, g, nd, b, tol, restart, max_iters=1000, lda=None):
-    """leading nd x nd block written by bie_build_block (the rest of the allocation is poisoned: it must never be read)"""
+def gpu_gmres_hybrid(ctx, g, nd, b, tol, restart, max_iters=1000):
+    """leading nd x nd block written by bie_build_block in the library's block format (the padding of the tiles is poisoned: it
+    must never be read)"""
     from paper_2108_01786_b200 import bie
     n = b.size
-    lda = lda or (nd + (nd & 1))
     z, dz, d2z = geo_dev(g)
-    A = torch.full((nd, lda), float("nan"), dtype=torch.float64, device="cuda")
-    ctx.bie_build_block(g.counts, g.kinds, z, dz, d2z, nd, A, lda=lda)
+    A = torch.full((bie.Context.bie_hybrid_block_bytes(nd) // 8,), float("nan"), dtype=torch.float64, device="cuda")
+    ctx.bie_build_block(g.counts, g.kinds, z, dz, d2z, nd, A)
     ws = torch.empty(bie.Context.bie_gmres_workspace_bytes(n, restart), dtype=torch.uint8, device="cuda")
     oi = torch.full((2,), -7, dtype=torch.int32, device="cuda")
     of = torch.full((1,), -7.0, dtype=torch.float64, device="cuda")
     x = torch.empty(n + (n & 1), dtype=torch.float64, device="cuda")
-    ctx.bie_gmres_hybrid(A, nd, dev(b), x[:n], tol, restart, max_iters, ws, oi, of, lda=lda)
+    ctx.bie_gmres_hybrid(A, nd, dev(b), x[:n], tol, restart, max_iters, ws, oi, of)
     torch.cuda.synchronize()
     return x[:n].cpu().numpy(), int(oi[0]), float(of[0]), int(oi[1]), A
 
 
-def test_build_block_writes_only_the_block(ctx):
+def _untile(T, nb):
+    """the block format of include/bie.h: tiles of 4 rows x 512 columns, each contiguous, in row-major order of the tiles"""
+    ngrp, nch = -(-nb // 4), -(-nb // 512)
+    return T[:ngrp * nch * 2048].reshape(ngrp, nch, 4, 512).transpose(0, 2, 1, 3).reshape(ngrp * 4, nch * 512)[:nb, :nb]
+
+
+@pytest.mark.parametrize("nb", [778, 130, 1024])
+def test_build_block_is_the_leading_block(ctx, nb):
+    from paper_2108_01786_b200 import bie
     g = cfg(2).geometry
-    nb, lda = 778, 900
     z, dz, d2z = geo_dev(g)
-    A = torch.full((nb + 5, lda), -7.0, dtype=torch.float64, device="cuda")
-    ctx.bie_build_block(g.counts, g.kinds, z, dz, d2z, nb, A, lda=lda)
-    Ah = A.cpu().numpy()
-    Ao = oracle_build(g)
-    assert rel_max(Ah[:nb, :nb], Ao[:nb, :nb]) <= TOL_ENTRY
-    assert np.all(Ah[:nb, nb:] == -7.0) and np.all(Ah[nb:] == -7.0)
+    nd = bie.Context.bie_hybrid_block_bytes(nb) // 8
+    A = torch.full((nd + 7,), -7.0, dtype=torch.float64, device="cuda")
+    for variant in (0, 2):
+        ctx.bie_build_block(g.counts, g.kinds, z, dz, d2z, nb, A, variant=variant)
+        Ah = A.cpu().numpy()
+        Ao = oracle_build(g, variant)
+        assert rel_max(_untile(Ah, nb), Ao[:nb, :nb]) <= TOL_ENTRY
+        assert np.all(Ah[nd:] == -7.0)            # nothing behind the block
 
 
 def test_build_cols_writes_only_the_slab(ctx):
@@ -896,7 +905,7 @@ def test_gmres_hybrid_free_warps_knob(ctx):
             x, it, rr, st, A = gpu_gmres_hybrid(ctx, g, 1024, b, P.tol, P.restart, P.max_iters)
             assert st == 0 and abs(it - ito) <= 1 and np.linalg.norm(x - xo) / np.linalg.norm(xo) <= TOL_X
     finally:
-        ctx.bie_set_hybrid_free_warps(15)
+        ctx.bie_set_hybrid_free_warps(12)
 
 
 def test_config4_sequence_of_four_stages(ctx):
@@ -1007,7 +1016,7 @@ def test_error_codes_of_the_operator_and_next_calls(ctx):
     of = torch.zeros(1, dtype=torch.float64, device="cuda")
     b = torch.ones(n, dtype=torch.float64, device="cuda")
     x = torch.empty_like(b)
-    ctx.bie_build_cols(g.counts, g.kinds, z, dz, d2z, 128, A)
+    ctx.bie_build_block(g.counts, g.kinds, z, dz, d2z, 128, A)
     for nd, code in [(127, -6), (n, -6), (0, -6), (2, -6), (130, -6), (256 + 64, -6)]:   # odd, whole matrix, none, not a row-block boundary
         with pytest.raises(bie.BieError) as e:
             ctx.bie_gmres_hybrid(A, nd, b, x, 1e-13, 50, 10, ws, oi, of)
