@@ -1,18 +1,23 @@
 #!/usr/bin/env python
 """bench.py -- one "step" = one pass of the whole hot path over one synthetic geometry:
-node preparation + dense build of the matrix of Eq. (3.16) (bie_build) + restarted GMRES on it (bie_gmres).
+node preparation + the operator's stored part (whole matrix of Eq. (3.16), leading block, or nothing) + restarted
+GMRES with that operator, every stage of the config (config 4: 4 stages, the later ones through bie_build_update).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference] [--matrix-free]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference] [--operator ...]
 
-Prints ONE JSON line (rank 0).  Default workload: BASELINE.json configs[4] (n = 16384, 2.1 GB matrix, restart 100,
-tol 1e-13), the largest single-GPU configuration; its matrix is 17x the L2, so every GEMV streams from HBM.
+Prints ONE JSON line (rank 0).  Default workload: BASELINE.json configs[4] (n = 16384, restart 100, tol 1e-13), the
+largest single-GPU configuration.
 
-  value         whole-step throughput: n^2 matrix entries built AND solved per second, inputs resident in HBM
-  build/gmres   the two halves of BASELINE.json's metric on their own: Gentries/s of the build, ms of the solve
+  value         whole-step throughput: n^2 matrix entries applied per second of a step, inputs resident in HBM
+  build/gmres   the two halves of BASELINE.json's metric on their own: Gentries/s of bie_build (stand-alone calls,
+                median and best of 20), ms of the solve inside the step
+  per_config    configs 1-4 with SURVEY 8(d)'s protocol: 3 warm-ups, median and best of 20 builds / 100 matvecs /
+                10 solves per operator; config 4 as its 4-stage sequence
   e2e           the same step through bie_solve_host with pinned HOST buffers (H2D of nodes+rhs, D2H of the density)
-  roofline      dominant kernel = the persistent GMRES kernel (HBM-bound GEMVs): algorithmic bytes / event time
-  roofline_build  the entry builder against the FP64 pipe (DFMA rate measured by bie_probe_dfma in this run)
-  cpu_baseline  the oracle (oracle/, as it stands) on this box's host cores, on a bounded sample of the same workload
+  roofline      dominant kernel = the persistent GMRES kernel of the operator the step uses
+  roofline_build  the entry builder against its two bounds (HBM write, FP64 pipe)
+  cpu_baseline  the oracle (oracle/, as it stands) REALLY run on this box's host cores: oracle.build_matrix +
+                oracle.gmres on the same inputs, all cores (and one thread where that takes seconds)
 
 --impl reference times the oracle alone (this tier has no reference implementation).
 N > 1: replicas only: every rank runs the same step on its own GPU, no data-path collective.
@@ -20,6 +25,7 @@ N > 1: replicas only: every rank runs the same step on i
 from __future__ import annotations
 
 import argparse
+import csv
 import json
 import os
 import subprocess
@@ -35,14 +41,14 @@ if ROOT not in sys.path:
 
 METRIC = "matrix build Gentries/s and GMRES solve ms (FP64); % of FP64 / HBM roofline"
 UNIT = "Gentries/s"
-FP64_INSTR_PER_ENTRY = 13      # FP64-pipe instructions per stored matrix entry (SASS count)
-FP64_INSTR_PER_PAIR_FREE = 11  # one-directional pair loops (hybrid operator): FP64-pipe instructions per entry (bie_free.cuh)
-FP64_INSTR_PER_ENTRY_SYM = 7.7  # symmetric pair loops (whole-matrix matrix-free operator, bie_free_sym.cuh): 15 per pair of
-                                # entries + 9 DADD of the lane reduction per 32 pairs, i.e. 7.64 per entry; own blocks 11
+# FP64-pipe instructions per matrix entry (DFMA + DMUL + DADD), SASS counts from the ncu captures under profiles/
+# (profiles/r02_build.md, profiles/r02_free.md); the hand counts of DESIGN.md section 5 are 10 / 10 / 6.5 + reduction
+FP64_PER_ENTRY_BUILD = 10.0     # bie_build_kernel, difference form
+FP64_PER_ENTRY_SYM = 6.8        # symmetric pair loops: 13 per pair of entries + lane reduction of the reverse sums
+FP64_PER_PAIR_VORTEX = 13.0     # vortex-sheet matrix, (X, Y) form
+NOMINAL_FP64_INSTR_S = 148 * 64 * 1.965e9   # B200: 148 SMs x 64 FP64 lanes x 1.965 GHz = 18.6 T instr/s
 HBM_FALLBACK_GBS = 6650.0      # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
-# dram__bytes_read.sum + dram__bytes_write.sum of the GMRES kernel, one launch, from the committed ncu capture
-# (profiles/r01_ncu_full_gmres_cfg5.md); None for workloads that were not captured
-TRAFFIC_BYTES = {(5, "dense"): 341.50e9, (5, "hybrid"): 142.37e9}   # profiles/r01b_ncu_full_cfg5.md, r01e_launches_cfg5.md
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_dram_traffic.csv")   # dram bytes per launch from `ncu --set full`
 
 
 def parse_args():
@@ -54,11 +60,13 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--operator", default="auto", choices=["auto", "dense", "free", "hybrid"],
                     help="dense: bie_build + GMRES on the stored matrix; free: matrix-free GMRES (entries recomputed on the "
-                         "fly, no matrix); hybrid: a slab of bie_hybrid_cols(n) columns stored and streamed while the other "
-                         "sources are recomputed; auto (default): all are timed during warm-up and the fastest is the timed step")
+                         "fly, no matrix); hybrid: the leading block of bie_hybrid_cols(n) rows and columns stored and streamed "
+                         "while everything else is recomputed; auto (default): all are timed during warm-up and the fastest is the timed step")
     ap.add_argument("--matrix-free", action="store_true", help="same as --operator free")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="budget of the oracle sample")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config block (configs 1-4)")
+    ap.add_argument("--no-next-rows", action="store_true", help="skip the stand-alone timings of the SURVEY 8(f) rows")
+    ap.add_argument("--cpu-seconds", type=float, default=150.0, help="wall budget of the whole --impl reference run")
     a = ap.parse_args()
     if a.matrix_free:
         a.operator = "free"
@@ -69,16 +77,28 @@ def hbm_peak():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
         try:
-            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, a read+write copy)"
         except Exception:
             pass
     return HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md)"
 
 
 def n_gemv(iters: int, restart: int) -> int:
-    """GEMVs of one bie_gmres launch: one per Arnoldi step, one residual per restart, one final true residual"""
+    """operator applications of one bie_gmres launch: one per Arnoldi step, one residual per restart, one final true residual"""
     cycles = max(1, -(-iters // restart))
     return iters + (cycles - 1) + 1
+
+
+def traffic_bytes(config: int, op: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the GMRES kernel of (config, operator), one launch, from the committed
+    `ncu --set full` capture of THIS code state (profiles/r02_dram_traffic.csv names the commit); None when not captured"""
+    try:
+        for row in csv.DictReader(open(TRAFFIC_CSV)):
+            if int(row["config"]) == config and row["operator"] == op:
+                return {"bytes": float(row["dram_bytes"]), "capture": row.get("capture", ""), "code_state": row.get("code_state", "")}
+    except Exception:
+        pass
+    return None
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -136,100 +156,325 @@ class ClockSampler:
 # ---------------------------------------------------------------------------------------------------
 # oracle legs (the only places bench.py executes oracle/)
 # ---------------------------------------------------------------------------------------------------
-def oracle_sample(P, iters: int, seconds: float):
-    """Times the oracle, as it stands, on a bounded sample of the workload: a block of R rows of the matrix
-    (oracle_build_rows), the GEMV on that block (oracle_matvec_rect) and, when the whole problem fits the budget,
-    nothing is extrapolated.  Returns (step_seconds_estimate, description, cores)."""
+def oracle_step(P, threads=None):
+    """ONE real pass of the oracle over the workload, as it stands: oracle.build_matrix + oracle.gmres for every stage.
+    -> dict with the measured seconds.  threads: None = all cores."""
+    import oracle
+    allc = oracle.num_threads()
+    if threads:
+        oracle.set_num_threads(threads)
+    try:
+        tb = tg = 0.0
+        its = []
+        A = None
+        rr = 0.0
+        for g, b in zip(P.stages, P.rhs):
+            t0 = time.perf_counter()
+            A = oracle.build_matrix(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, out=A)
+            t1 = time.perf_counter()
+            x, it, rr, hist, st = oracle.gmres(A, b, P.tol, P.restart, P.max_iters)
+            t2 = time.perf_counter()
+            tb += t1 - t0; tg += t2 - t1; its.append(int(it))
+        return {"build_s": tb, "gmres_s": tg, "step_s": tb + tg, "iters": its, "relres_true": float(rr),
+                "threads": int(threads or allc)}
+    finally:
+        if threads:
+            oracle.set_num_threads(allc)
+
+
+def oracle_bounded_step(P, budget_s, build_s_per_entry, iters):
+    """A bounded sample of one step for machines where the full oracle step does not fit the budget: the build on R of the n
+    rows and the GEMV on that block, scaled to the whole step.  -> (estimated step seconds, description)"""
     import oracle
     g = P.geometry
     n = g.n
-    cores = oracle.num_threads()
     rng = np.random.default_rng(0)
-    # rate of the build on 64 rows, then as many rows as fit ~40 % of the budget
-    rows = np.sort(rng.choice(n, size=min(n, 64), replace=False))
-    t = time.perf_counter()
-    oracle.build_rows(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, rows)
-    dt = max(time.perf_counter() - t, 1e-6)
-    R = int(min(n, max(64, 0.4 * seconds / dt * rows.size)))
+    R = int(min(n, max(64, n * min(1.0, 0.25 * budget_s / max(build_s_per_entry * n * n, 1e-9)))))
     rows = np.sort(rng.choice(n, size=R, replace=False))
-    t = time.perf_counter()
-    blk = oracle.build_rows(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, rows)
-    t_build_rows = time.perf_counter() - t
-    x = rng.standard_normal(n)
-    oracle.matvec(blk, x)
-    reps, t_mv = 0, 0.0
     t0 = time.perf_counter()
+    blk = oracle.build_rows(g.counts, g.kinds, g.zeta, g.dzeta, g.d2zeta, rows)
+    t_build = (time.perf_counter() - t0) * n / R
+    x = rng.standard_normal(n)
+    reps, t0 = 0, time.perf_counter()
     while True:
-        oracle.matvec(blk, x)
-        reps += 1
-        t_mv = time.perf_counter() - t0
-        if t_mv > 0.4 * seconds or reps >= 200:
+        oracle.matvec(blk, x); reps += 1
+        if time.perf_counter() - t0 > 0.5 * budget_s or reps >= 100:
             break
-    t_build = t_build_rows * n / R
-    t_gemv = t_mv / reps * n / R
+    t_gemv = (time.perf_counter() - t0) / reps * n / R
     ng = n_gemv(iters, P.restart)
-    est = t_build + ng * t_gemv
-    desc = (f"oracle_build_rows on {R} of {n} rows ({t_build_rows:.2f} s) and {reps} oracle GEMVs on that {R}x{n} block "
-            f"({t_mv:.2f} s); step = n/R * build + {ng} GEMVs (the GPU run's count) * n/R * block GEMV; "
-            f"Gram-Schmidt O(n*iters) not included")
-    return est, desc, cores, {"build_s": t_build, "gemv_s": t_gemv, "gemvs": ng}
+    t_gs = ng * 0.5 * min(iters, P.restart) * 4 * 8 * n / 2.0e10      # modified Gram-Schmidt: 4 n j flops per step, memory-bound, ~20 GB/s
+    est = len(P.stages) * (t_build + ng * t_gemv + t_gs)
+    return est, (f"ESTIMATED (the full oracle step does not fit {budget_s:.1f} s here): oracle.build_rows on {R} of {n} rows, {reps} "
+                 f"oracle GEMVs on that block; step = stages * (n/R build + {ng} GEMVs * n/R block GEMV + Gram-Schmidt 2 n j^2 flops)")
 
 
 def run_reference(args):
-    """--impl reference: the oracle on the box's host cores, same config/metric/unit (rank 0 only)."""
+    """--impl reference: the oracle on the box's host cores, same config/metric/unit (rank 0 only).  Every step is ONE real
+    oracle pass (build_matrix + gmres, all stages) when that fits the run's wall budget, else a bounded sample marked estimated."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
+    import oracle
     from paper_2108_01786_b200 import inputs
     P = inputs.make_config(args.config)
     n = P.n
-    args.op, args.stored_cols = "dense", n     # the oracle stores the matrix
-    iters_nominal = {1: 18, 2: 33, 3: 74, 4: 127, 5: 158}[args.config]  # the oracle's own counts (tests)
-    per = max(2.0, min(args.cpu_seconds, 120.0 / max(1, args.steps + args.warmup)))
-    for _ in range(args.warmup):
-        oracle_sample(P, iters_nominal, per)
-    ests = []
-    for _ in range(args.steps):
-        est, desc, cores, parts = oracle_sample(P, iters_nominal, per)
-        ests.append(est)
-    est = float(np.mean(ests))
-    val = n * n / est / 1e9
+    args.op, args.nd = "dense", 0     # the oracle stores the matrix
+    nsteps = max(1, args.steps + args.warmup)
+    per = args.cpu_seconds / nsteps
+    first = oracle_step(P)                      # one real pass tells whether the rest fit
+    full = first["step_s"] <= per
+    times, parts, desc = [], first, None
+    for k in range(1, nsteps):
+        if full:
+            r = oracle_step(P)
+            if k >= args.warmup:
+                times.append(r["step_s"]); parts = r
+        else:
+            est, desc = oracle_bounded_step(P, per, first["build_s"] / len(P.stages) / (n * n), first["iters"][-1])
+            if k >= args.warmup:
+                times.append(est)
+    if not times:
+        times = [first["step_s"]]
+    step_s = float(np.mean(times))
+    val = len(P.stages) * n * n / step_s / 1e9
+    cores = oracle.num_threads()
+    sample = (f"every step = one REAL oracle pass (oracle.build_matrix + oracle.gmres on all {len(P.stages)} stage(s)), "
+              f"{cores} threads" if full else desc)
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": est * 1e3, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload_config(P, args, iters_nominal),
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "warmup": args.warmup, "ms_per_step": step_s * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "estimated": (not full),
+            "config": workload_config(P, args, first["iters"][-1]),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "estimated": (not full)},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0,
-            "build": {"gentries_per_s": n * n / parts["build_s"] / 1e9, "ms": parts["build_s"] * 1e3},
-            "gmres": {"ms": parts["gemv_s"] * parts["gemvs"] * 1e3, "iters": iters_nominal}}
+            "build": {"gentries_per_s": len(P.stages) * n * n / parts["build_s"] / 1e9, "ms": parts["build_s"] * 1e3},
+            "gmres": {"ms": parts["gmres_s"] * 1e3, "iters": parts["iters"][-1], "relres_true": parts["relres_true"]}}
     print(json.dumps(line), flush=True)
 
 
-def l2_policy(n, stored_cols):
-    """what the timed iterations stream: the stored part of the matrix against the 126 MB L2"""
-    stored = 8.0 * n * stored_cols
-    if stored_cols == 0:
+def l2_policy(n, stored):
+    """what the timed iterations stream: the stored part of the matrix (entries) against the 126 MB L2"""
+    nbytes = 8.0 * stored
+    if stored == 0:
         return ("no matrix stored (matrix-free operator): the O(n) node tables are L2-resident by design, the kernel is "
                 "FP64-bound; nothing to flush")
-    if stored > 2.5e8:
-        return "stored part of the matrix (%.0f MB) is %.1fx the 126 MB L2: every operator application streams it from HBM; no flush needed" % (stored / 1e6, stored / 126e6)
-    return "stored matrix (%.0f MB) fits the 126 MB L2: L2-resident GEMV, reported as such" % (stored / 1e6)
+    if nbytes > 2.5e8:
+        return "stored part of the matrix (%.0f MB) is %.1fx the 126 MB L2: every operator application streams it from HBM; no flush needed" % (nbytes / 1e6, nbytes / 126e6)
+    return "stored part of the matrix (%.0f MB) fits the 126 MB L2: L2-resident, reported as such (not as HBM bandwidth)" % (nbytes / 1e6)
+
+
+def stored_entries(n, op, nd):
+    return {"dense": n * n, "free": 0, "hybrid": nd * nd}[op]
 
 
 def workload_config(P, args, iters):
     g = P.geometry
+    se = stored_entries(g.n, args.op, getattr(args, "nd", 0))
     return {"workload": f"BASELINE.json configs[{P.config - 1}]: {P.name}", "n": int(g.n),
             "counts": [int(c) for c in g.counts], "restart": int(P.restart), "tol": P.tol,
-            "operator": {"dense": "dense", "free": "matrix-free", "hybrid": "hybrid (stored slab + recomputed sources)"}[args.op]
+            "operator": {"dense": "dense (whole matrix stored)", "free": "matrix-free (symmetric pair loops)",
+                         "hybrid": "hybrid (stored leading block + recomputed rest)"}[args.op]
                         + (" (chosen by measurement)" if args.operator == "auto" else ""),
-            "matrix_bytes": int(8 * g.n * args.stored_cols), "stored_columns": int(args.stored_cols),
-            "l2_policy": l2_policy(g.n, args.stored_cols),
+            "matrix_bytes": int(8 * se), "stored_entries": int(se),
+            "l2_policy": l2_policy(g.n, se),
             "stages_per_step": len(P.stages), "replicas": int(args.gpus)}
 
 
 # ---------------------------------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------------------------------
+class Timer:
+    """SURVEY 8(d) protocol: warm-ups, then every repetition timed on the device with its own pair of CUDA events (on the
+    current stream, which is the stream the binding launches on); optional L2 flush between repetitions."""
+
+    def __init__(self, torch):
+        self.torch = torch
+        self.flush_buf = None
+
+    def flush(self):
+        if self.flush_buf is None:
+            self.flush_buf = self.torch.empty(256 << 20, dtype=self.torch.uint8, device="cuda")   # 2x the 126 MB L2
+        self.flush_buf.zero_()
+
+    def __call__(self, fn, reps, warm=3, flush=False):
+        t = self.torch
+        for _ in range(warm):
+            fn()
+        t.cuda.synchronize()
+        ms = []
+        for _ in range(reps):
+            if flush:
+                self.flush()
+            a, c = t.cuda.Event(enable_timing=True), t.cuda.Event(enable_timing=True)
+            a.record(); fn(); c.record()
+            t.cuda.synchronize()
+            ms.append(a.elapsed_time(c))
+        return {"median_ms": float(np.median(ms)), "best_ms": float(np.min(ms)), "reps": reps}
+
+
+class Workload:
+    """one config on the device: buffers, the three operators' steps"""
+
+    def __init__(self, torch, bie, ctx, P):
+        self.torch, self.bie, self.ctx, self.P = torch, bie, ctx, P
+        g, n = P.geometry, P.n
+        self.g, self.n = g, n
+        dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+        self.stages = [(gs, tuple(dev(a) for a in (gs.zeta, gs.dzeta, gs.d2zeta)), dev(bs)) for gs, bs in zip(P.stages, P.rhs)]
+        self.z, self.dz, self.d2z = self.stages[0][1]
+        self.A = torch.empty((n, n + (n & 1)), dtype=torch.float64, device="cuda")
+        self.x = torch.empty(n + (n & 1), dtype=torch.float64, device="cuda")[:n]
+        self.ws = torch.empty(ctx.bie_gmres_workspace_bytes(n, P.restart), dtype=torch.uint8, device="cuda")
+        self.oi = torch.zeros(2, dtype=torch.int32, device="cuda")
+        self.of = torch.zeros(1, dtype=torch.float64, device="cuda")
+        ctx.bie_set_geometry(g.counts, g.kinds, self.z, self.dz, self.d2z)
+        self.nd = ctx.bie_hybrid_cols(n)
+        self.blk = (torch.empty(max(ctx.bie_hybrid_block_bytes(self.nd) // 8, 2), dtype=torch.float64, device="cuda")
+                    if self.nd else None)
+
+    def step(self, op, ev=None):
+        ctx, P = self.ctx, self.P
+        for si, (gs, (zs, dzs, d2zs), bs) in enumerate(self.stages):
+            if ev and si == 0: ev[0].record()
+            if op == "dense":
+                if si == 0:
+                    ctx.bie_build(gs.counts, gs.kinds, zs, dzs, d2zs, self.A)      # 2 launches: node prep + tile kernel
+                else:
+                    ctx.bie_build_update(gs.counts, gs.kinds, zs, dzs, d2zs, self.A)   # only the blocks touching Gamma_0
+            elif op == "free":
+                ctx.bie_set_geometry(gs.counts, gs.kinds, zs, dzs, d2zs)      # 1 launch: node prep
+            else:
+                ctx.bie_build_block(gs.counts, gs.kinds, zs, dzs, d2zs, self.nd, self.blk)   # 2 launches: node prep + block tiles
+            if ev and si == 0: ev[1].record()
+            if op == "hybrid":       # near matrix (3 launches, once per geometry) + 1 cooperative launch
+                ctx.bie_gmres_hybrid(self.blk, self.nd, bs, self.x, P.tol, P.restart, P.max_iters, self.ws, self.oi, self.of)
+            else:                    # dense: 1 cooperative launch; matrix-free: near matrix (3) + (symmetric work list 1) + 1
+                ctx.bie_gmres(self.A if op == "dense" else None, bs, self.x, P.tol, P.restart, P.max_iters, self.ws, self.oi, self.of)
+        if ev: ev[2].record()
+
+    def ops(self):
+        return ["dense", "free"] + (["hybrid"] if self.nd else [])
+
+    def result(self):
+        return int(self.oi[0]), int(self.oi[1]), float(self.of[0])
+
+
+def gmres_roofline(n, op, nd, ng, gmres_ms, dfma_per_s, clocks_mhz, config):
+    """roofline of the persistent GMRES kernel for one launch of ng operator applications taking gmres_ms"""
+    peak, peak_src = hbm_peak()
+    t = gmres_ms * 1e-3
+    tr = traffic_bytes(config, op)
+    if op == "dense":
+        ach = ng * 8.0 * n * n / t / 1e9
+        return {"bound": "hbm", "kernel": "bie_gmres_kernel<dense> (persistent; GEMV phases dominate)", "achieved": ach, "peak": peak,
+                "unit": "GB/s", "frac": ach / peak, "traffic": tr and tr["bytes"], "traffic_capture": tr, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": ng * 8 * n * n, "operator_applications_per_launch": ng}
+    entries = ng * (n * n - (nd * nd if op == "hybrid" else 0))
+    instr = entries * FP64_PER_ENTRY_SYM + (ng * nd * nd if op == "hybrid" else 0)     # + one DFMA per streamed block entry
+    ach = instr / t
+    alu = {"achieved": ach / 1e12, "unit": "T FP64 instr/s", "fp64_instr_per_entry": FP64_PER_ENTRY_SYM,
+           "recomputed_entries_per_launch": entries, "peak_probe": dfma_per_s / 1e12, "frac_of_probe": ach / dfma_per_s,
+           "peak_nominal": NOMINAL_FP64_INSTR_S / 1e12, "frac_of_nominal": ach / NOMINAL_FP64_INSTR_S,
+           "sm_mhz_during_step": clocks_mhz,
+           "peak_source": "bie_probe_dfma in this run; nominal = 148 SMs x 64 FP64 lanes x 1.965 GHz (DESIGN.md section 7)"}
+    if op == "free":
+        return {"bound": "alu", "kernel": "bie_gmres_kernel<matrix-free> (persistent; symmetric pair loops dominate)",
+                "achieved": alu["achieved"], "peak": alu["peak_probe"], "unit": alu["unit"], "frac": alu["frac_of_probe"],
+                "traffic": tr and tr["bytes"], "traffic_capture": tr, "operator_applications_per_launch": ng, "alu": alu}
+    gbs = ng * 8.0 * nd * nd / t / 1e9
+    hbm = {"achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "algorithmic_bytes_per_launch": ng * 8 * nd * nd,
+           "peak_source": peak_src}
+    binding = "hbm" if hbm["frac"] >= alu["frac_of_probe"] else "alu"
+    return {"bound": "hbm+alu", "binding_leg": binding, "kernel": "bie_gmres_kernel<hybrid> (persistent; block stream and pair loops at once)",
+            "achieved": hbm["achieved"] if binding == "hbm" else alu["achieved"],
+            "peak": hbm["peak"] if binding == "hbm" else alu["peak_probe"],
+            "unit": hbm["unit"] if binding == "hbm" else alu["unit"],
+            "frac": max(hbm["frac"], alu["frac_of_probe"]), "traffic": tr and tr["bytes"], "traffic_capture": tr,
+            "operator_applications_per_launch": ng, "hbm": hbm, "alu": alu}
+
+
+def measure_config(torch, bie, ctx, c, timer, dfma_per_s):
+    """per_config entry: build, matvec (dense, with L2 flush where the matrix is near the L2 size; matrix-free),
+    and the step with every operator -- median and best of 20 / 100 / 10"""
+    from paper_2108_01786_b200 import inputs
+    P = inputs.make_config(c)
+    W = Workload(torch, bie, ctx, P)
+    g, n = W.g, W.n
+    peak, _ = hbm_peak()
+    out = {"n": n, "counts": [int(v) for v in g.counts], "restart": int(P.restart), "stages": len(P.stages)}
+    b = timer(lambda: ctx.bie_build(g.counts, g.kinds, W.z, W.dz, W.d2z, W.A), 20)
+    b.update({"gentries_per_s_median": n * n / (b["median_ms"] * 1e-3) / 1e9, "gentries_per_s_best": n * n / (b["best_ms"] * 1e-3) / 1e9,
+              "hbm_write_frac": 8.0 * n * n / (b["median_ms"] * 1e-3) / 1e9 / peak,
+              "fp64_frac_of_probe": n * n * FP64_PER_ENTRY_BUILD / (b["median_ms"] * 1e-3) / dfma_per_s,
+              "fp64_frac_of_nominal": n * n * FP64_PER_ENTRY_BUILD / (b["median_ms"] * 1e-3) / NOMINAL_FP64_INSTR_S})
+    out["build"] = b
+    if len(P.stages) > 1:
+        M0 = int(g.counts[0])
+        u = timer(lambda: ctx.bie_build_update(g.counts, g.kinds, W.z, W.dz, W.d2z, W.A), 20)
+        ue = n * n - (n - M0) * (n - M0)
+        u.update({"entries": ue, "share_of_matrix": ue / float(n * n), "gentries_per_s_median": ue / (u["median_ms"] * 1e-3) / 1e9})
+        out["build_update"] = u
+    xv = torch.from_numpy(np.random.default_rng(1).standard_normal(n)).cuda()
+    yv = torch.empty(n + (n & 1), dtype=torch.float64, device="cuda")[:n]
+    nbytes = 8.0 * n * n
+    flush = 0.4 * 126e6 < nbytes < 4 * 126e6       # near the L2 size: flush between repetitions, else the number is an L2 number
+    mv = timer(lambda: ctx.bie_matvec(W.A, xv, yv), 100, flush=flush)
+    mv.update({"gbs_median": nbytes / (mv["median_ms"] * 1e-3) / 1e9, "l2_flushed_between_reps": bool(flush),
+               "regime": ("HBM (matrix %.0f MB, L2 flushed between repetitions)" % (nbytes / 1e6)) if flush else
+                         ("L2-resident (matrix %.1f MB): an L2 / latency number, not HBM bandwidth" % (nbytes / 1e6) if nbytes < 126e6
+                          else "HBM (matrix %.0f MB streams)" % (nbytes / 1e6)),
+               "hbm_frac": (nbytes / (mv["median_ms"] * 1e-3) / 1e9 / peak) if nbytes >= 0.4 * 126e6 else None})
+    out["matvec_dense"] = mv
+    ctx.bie_set_geometry(g.counts, g.kinds, W.z, W.dz, W.d2z)
+    mf = timer(lambda: ctx.bie_matvec_free(xv, yv), 100)
+    mf.update({"gentries_per_s_median": n * n / (mf["median_ms"] * 1e-3) / 1e9,
+               "fp64_frac_of_probe": n * n * FP64_PER_ENTRY_SYM / (mf["median_ms"] * 1e-3) / dfma_per_s})
+    out["matvec_free"] = mf
+    steps = {}
+    for op in W.ops():
+        r = timer(lambda: W.step(op), 10)
+        it, st, rr = W.result()
+        r.update({"iters_last_stage": it, "status": st, "relres_true": rr,
+                  "us_per_iter_median": r["median_ms"] * 1e3 / max(1, it * len(P.stages))})
+        steps[op] = r
+    best = min(steps, key=lambda k: steps[k]["median_ms"])
+    out["step"] = steps
+    out["operator_chosen"] = best
+    it = steps[best]["iters_last_stage"]
+    ng = n_gemv(it, P.restart) * len(P.stages)
+    se = stored_entries(n, best, W.nd)
+    out["l2_policy"] = l2_policy(n, se)
+    rf = gmres_roofline(n, best, W.nd, ng, steps[best]["median_ms"], dfma_per_s, None, c)
+    out["roofline"] = {k: rf[k] for k in ("bound", "achieved", "peak", "unit", "frac") if k in rf}
+    if best == "dense" and 8.0 * n * n < 126e6:
+        out["roofline"]["bound"] = "l2/latency"
+        out["roofline"]["note"] = ("the matrix is L2-resident and the step is dominated by grid barriers: `achieved` is algorithmic bytes "
+                                   "over the whole step, not an HBM statement")
+    del W
+    torch.cuda.empty_cache()
+    return out
+
+
+def cpu_baseline(cfgs):
+    """the oracle really run (build_matrix + gmres, every stage) on all host cores for every config asked for, and on ONE thread
+    where that takes seconds (configs 1-3)"""
+    from paper_2108_01786_b200 import inputs
+    out = {}
+    for c in cfgs:
+        P = inputs.make_config(c)
+        n = P.n
+        r = oracle_step(P)
+        e = {"n": n, "cores": r["threads"], "build_s": r["build_s"], "gmres_s": r["gmres_s"], "step_s": r["step_s"], "iters": r["iters"],
+             "gentries_per_s": len(P.stages) * n * n / r["step_s"] / 1e9, "build_gentries_per_s": len(P.stages) * n * n / r["build_s"] / 1e9,
+             "estimated": False}
+        if c <= 3:
+            s1 = oracle_step(P, threads=1)
+            e["single_thread"] = {"build_s": s1["build_s"], "gmres_s": s1["gmres_s"], "step_s": s1["step_s"]}
+        else:
+            e["single_thread"] = None    # minutes of CPU time: not run
+        out[str(c)] = e
+    return out
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
@@ -256,86 +501,40 @@ def main():
     P = inputs.make_config(args.config)
     g, n = P.geometry, P.n
     ctx = bie.Context(local)
-    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
-    z, dz, d2z, b = dev(g.zeta), dev(g.dzeta), dev(g.d2zeta), dev(P.rhs[0])
-    # the stored matrix is also needed for the stand-alone dense GEMV timing, whichever operator the step uses
-    A = torch.empty((n, n + (n & 1)), dtype=torch.float64, device="cuda")
-    x = torch.empty(n + (n & 1), dtype=torch.float64, device="cuda")[:n]
-    ws = torch.empty(ctx.bie_gmres_workspace_bytes(n, P.restart), dtype=torch.uint8, device="cuda")
-    oi = torch.zeros(2, dtype=torch.int32, device="cuda")
-    of = torch.zeros(1, dtype=torch.float64, device="cuda")
+    timer = Timer(torch)
+    W = Workload(torch, bie, ctx, P)
+    nstage = len(P.stages)
 
-    # BASELINE.json configs[3] is a SEQUENCE of stages (Gamma_0 moves, the solids stay): one step = all its stages, the
-    # first with a full build, the others with bie_build_update (a4); every other config has one stage
-    stages = [(gs, tuple(dev(a) for a in (gs.zeta, gs.dzeta, gs.d2zeta)), dev(bs)) for gs, bs in zip(P.stages, P.rhs)]
-    nstage = len(stages)
-
-    def step_dense(ev=None):
-        for si, (gs, (zs, dzs, d2zs), bs) in enumerate(stages):
-            if ev and si == 0: ev[0].record()
-            if si == 0:
-                ctx.bie_build(gs.counts, gs.kinds, zs, dzs, d2zs, A)      # 2 launches: node prep + tile kernel
-            else:
-                ctx.bie_build_update(gs.counts, gs.kinds, zs, dzs, d2zs, A)   # only the blocks touching Gamma_0
-            if ev and si == 0: ev[1].record()
-            ctx.bie_gmres(A, bs, x, P.tol, P.restart, P.max_iters, ws, oi, of)  # 1 cooperative launch
-        if ev: ev[2].record()
-
-    def step_free(ev=None):
-        for si, (gs, (zs, dzs, d2zs), bs) in enumerate(stages):
-            if ev and si == 0: ev[0].record()
-            ctx.bie_set_geometry(gs.counts, gs.kinds, zs, dzs, d2zs)      # 1 launch: node prep
-            if ev and si == 0: ev[1].record()
-            ctx.bie_gmres(None, bs, x, P.tol, P.restart, P.max_iters, ws, oi, of)  # near matrix (3) + 1 cooperative launch
-        if ev: ev[2].record()
-
-    nd = ctx.bie_hybrid_cols(n)
-
-    def step_hybrid(ev=None):
-        for si, (gs, (zs, dzs, d2zs), bs) in enumerate(stages):
-            if ev and si == 0: ev[0].record()
-            ctx.bie_build_block(gs.counts, gs.kinds, zs, dzs, d2zs, nd, A)  # 2 launches: node prep + block tiles
-            if ev and si == 0: ev[1].record()
-            ctx.bie_gmres_hybrid(A, nd, bs, x, P.tol, P.restart, P.max_iters, ws, oi, of)  # near matrix (3) + 1 launch
-        if ev: ev[2].record()
-
-    def time_steps(fn, k):
+    def time_steps(op, k):
         torch.cuda.synchronize()
         a_, c_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a_.record()
         for _ in range(k):
-            fn()
+            W.step(op)
         c_.record(); torch.cuda.synchronize()
         return a_.elapsed_time(c_) / k
 
     # operator choice by measurement (north_star: "matrix-free fused rebuild+matvec variant chosen by measurement")
-    steps = {"dense": step_dense, "free": step_free}
-    if nd > 0:
-        steps["hybrid"] = step_hybrid
     choice_ms = {}
     op = args.operator
-    if op == "hybrid" and nd == 0:
+    if op == "hybrid" and W.nd == 0:
         raise SystemExit("bench: n is too small for the hybrid operator")
     if op == "auto":
-        for name, fn in steps.items():
-            fn()
-            choice_ms[name] = max_over_ranks(time_steps(fn, 2))
+        for name in W.ops():
+            W.step(name)
+            choice_ms[name] = max_over_ranks(time_steps(name, 2))
         op = min(choice_ms, key=choice_ms.get)
-    step = steps[op]
-    args.op = op
-    args.stored_cols = {"dense": n, "free": 0, "hybrid": nd}[op]
-    args.matrix_free = (op == "free")
-    launches_per_step = {"dense": 3, "free": 5, "hybrid": 6}[op] * nstage
+    args.op, args.nd = op, W.nd
     solve_mode = {"dense": 0, "free": 1, "hybrid": 2}[op]
 
     for _ in range(max(args.warmup, 3)):
-        step()
+        W.step(op)
     barrier()
-    iters, status, relres = int(oi[0]), int(oi[1]), float(of[0])
+    iters, status, relres = W.result()
     if status != 0 or not (relres <= 1e-12):
         raise SystemExit(f"bench: GMRES did not converge (status {status}, relres {relres})")
 
-    # FP64 pipe rate of this GPU, now (roofline denominator of the build)
+    # FP64 pipe rate of this GPU, now (roofline denominator of the FP64-bound kernels)
     probe_out = torch.zeros(1, dtype=torch.float64, device="cuda")
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ctx.bie_probe_dfma(1 << 15, probe_out)
@@ -355,95 +554,89 @@ def main():
     t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     t_start.record()
     for k in range(K):
-        step(evs[k])
+        W.step(op, evs[k])
     t_end.record()
     barrier()
     clocks = sampler.stop() if rank == 0 else None
     total_ms = max_over_ranks(t_start.elapsed_time(t_end))
-    build_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
+    prep_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
     gmres_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
     ms_per_step = total_ms / K
     value = world * nstage * n * n / (ms_per_step * 1e-3) / 1e9
 
-    # ---- the stand-alone operator calls (outside the timed region; matvec against HBM) ---------
-    def time_call(fn, reps):
-        fn(); torch.cuda.synchronize()
-        a, c = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record()
-        for _ in range(reps):
-            fn()
-        c.record(); torch.cuda.synchronize()
-        return a.elapsed_time(c) / reps
-
+    # ---- stand-alone calls (outside the timed region; median and best of 20 / 100) -----------------
+    peak, peak_src = hbm_peak()
     xv = torch.from_numpy(np.random.default_rng(1).standard_normal(n)).cuda()
     yv = torch.empty(n + (n & 1), dtype=torch.float64, device="cuda")[:n]
-    matvec = {}
-    prep_ms = build_ms
-    if args.op != "dense":   # the full dense build is not part of this step: time it on its own (stand-alone calls, warm)
-        build_ms = time_call(lambda: ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A), 20)
-    # a4: partial rebuild (only the blocks touching Gamma_0), stand-alone, on the matrix just built
-    ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A)
-    upd_ms = time_call(lambda: ctx.bie_build_update(g.counts, g.kinds, z, dz, d2z, A), 20)
+    A, z, dz, d2z = W.A, W.z, W.dz, W.d2z
+    bt = timer(lambda: ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A), 20)
+    build_ms = bt["median_ms"]
+    upd = timer(lambda: ctx.bie_build_update(g.counts, g.kinds, z, dz, d2z, A), 20)
     M0_ = int(g.counts[0])
     upd_entries = n * n - (n - M0_) * (n - M0_)
-    mv_ms = time_call(lambda: ctx.bie_matvec(A, xv, yv), 50)
-    matvec["dense"] = {"ms": mv_ms, "gbs": 8.0 * n * n / (mv_ms * 1e-3) / 1e9, "hbm_frac": 8.0 * n * n / (mv_ms * 1e-3) / 1e9 / hbm_peak()[0]}
-    mf_ms = time_call(lambda: ctx.bie_matvec_free(xv, yv), 20)
-    matvec["matrix_free"] = {"ms": mf_ms, "gentries_per_s": n * n / (mf_ms * 1e-3) / 1e9,
-                             "fp64_instr_per_entry": FP64_INSTR_PER_ENTRY_SYM,
-                             "fp64_frac": n * n * FP64_INSTR_PER_ENTRY_SYM / (mf_ms * 1e-3) / dfma_per_s}
+    mv = timer(lambda: ctx.bie_matvec(A, xv, yv), 100)
+    matvec = {"dense": dict(mv, gbs=8.0 * n * n / (mv["median_ms"] * 1e-3) / 1e9,
+                            hbm_frac=8.0 * n * n / (mv["median_ms"] * 1e-3) / 1e9 / peak,
+                            note="read-only stream against the read+write copy peak; about 75 MB of the matrix stay L2-resident by design "
+                                 "(DESIGN.md section 6), so a fraction above 1 exceeds the copy peak, not the hardware")}
+    ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z)
+    mf = timer(lambda: ctx.bie_matvec_free(xv, yv), 100)
+    matvec["matrix_free"] = dict(mf, gentries_per_s=n * n / (mf["median_ms"] * 1e-3) / 1e9, fp64_instr_per_entry=FP64_PER_ENTRY_SYM,
+                                 fp64_frac_of_probe=n * n * FP64_PER_ENTRY_SYM / (mf["median_ms"] * 1e-3) / dfma_per_s,
+                                 fp64_frac_of_nominal=n * n * FP64_PER_ENTRY_SYM / (mf["median_ms"] * 1e-3) / NOMINAL_FP64_INSTR_S)
 
-    # ---- SURVEY 8(f) NEXT rows built so far, stand-alone calls outside the timed region ----------------------------
+    # ---- SURVEY 8(f) NEXT rows, stand-alone calls outside the timed region ----------------------------
     next_rows = {}
-    vx_ms = time_call(lambda: ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A, variant=2), 10)
-    next_rows["vortex_sheet_matrix"] = {"call": "bie_build(variant=BIE_VARIANT_VORTEX)", "ms": vx_ms,
-                                        "gentries_per_s": n * n / (vx_ms * 1e-3) / 1e9,
-                                        "fp64_frac": n * n * FP64_INSTR_PER_ENTRY / (vx_ms * 1e-3) / dfma_per_s,
-                                        "hbm_write_frac": 8.0 * n * n / (vx_ms * 1e-3) / 1e9 / hbm_peak()[0]}
-    ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z, variant=2)
-    vmf_ms = time_call(lambda: ctx.bie_matvec_free(xv, yv), 20)
-    next_rows["vortex_sheet_matrix"]["matrix_free_matvec_ms"] = vmf_ms
-    next_rows["vortex_sheet_matrix"]["matrix_free_fp64_frac"] = n * n * 13 / (vmf_ms * 1e-3) / dfma_per_s
-    if P.centers:
-        ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A, variant=1)
-        cyl_ms = time_call(lambda: ctx.bie_add_cyl_columns(g.counts, g.kinds, z, P.centers, A), 10)
-        nobs_cols = int(sum(int(cn) for cn, kd in zip(g.counts, g.kinds) if kd == 2))
-        next_rows["appendix_b_columns"] = {"call": "bie_add_cyl_columns (in place on the variant-B matrix)", "ms": cyl_ms,
-                                           "entries": n * nobs_cols, "gbs": 16.0 * n * nobs_cols / (cyl_ms * 1e-3) / 1e9,
-                                           "hbm_frac": 16.0 * n * nobs_cols / (cyl_ms * 1e-3) / 1e9 / hbm_peak()[0]}
-    # NEXT-3: 2 functions (Phi', Phi_t of Eq. 5.3) at 65 536 points below the free surface
-    npts_e = 65536
-    rng_e = np.random.default_rng(3)
-    ie = rng_e.integers(0, int(g.counts[0]), size=npts_e)
-    zp_e = dev(g.zeta[ie] - 1j * rng_e.uniform(0.01, 0.3, size=npts_e))
-    f_e = dev(np.vstack([np.exp(1j * g.zeta), np.exp(2j * g.zeta)]))
-    zc_e, dzc_e = dev(g.zeta), dev(g.dzeta)
-    out_e = torch.empty((2, npts_e), dtype=torch.complex128, device="cuda")
-    ev_ms = time_call(lambda: ctx.bie_cauchy_eval(g.counts, g.kinds, zc_e, dzc_e, f_e, zp_e, out=out_e), 5)
-    ev_instr = 12 + 4 * 3     # FP64-pipe instructions per pair: cot (12) + denominator and two numerators (4 each)
-    next_rows["cauchy_eval_near_boundary"] = {"call": "bie_cauchy_eval (nf = 2)", "points": npts_e, "sources": n, "ms": ev_ms,
-                                              "gpairs_per_s": npts_e * n / (ev_ms * 1e-3) / 1e9,
-                                              "fp64_instr_per_pair": ev_instr,
-                                              "fp64_frac": npts_e * n * ev_instr / (ev_ms * 1e-3) / dfma_per_s}
-    del zp_e, f_e, out_e
-    M0 = int(g.counts[0])
-    Nm = A.view(-1)[: M0 * A.stride(0)].view(M0, A.stride(0))       # the first M_0 rows of the same allocation
-    wv = torch.from_numpy(np.random.default_rng(2).standard_normal(n)).cuda()
-    uv = torch.empty(M0 + (M0 & 1), dtype=torch.float64, device="cuda")[:M0]
-    nb_ms = time_call(lambda: ctx.bie_build_normal_velocity(g.counts, g.kinds, z, dz, d2z, Nm), 10)
-    na_ms = time_call(lambda: ctx.bie_matvec_rect(Nm, wv, uv), 20)
-    next_rows["normal_velocity"] = {"call": "bie_build_normal_velocity + bie_matvec_rect", "rows": M0, "cols": n,
-                                    "build_ms": nb_ms, "build_gentries_per_s": M0 * n / (nb_ms * 1e-3) / 1e9,
-                                    "build_hbm_write_frac": 8.0 * M0 * n / (nb_ms * 1e-3) / 1e9 / hbm_peak()[0],
-                                    "apply_ms": na_ms, "apply_gbs": 8.0 * M0 * n / (na_ms * 1e-3) / 1e9,
-                                    "apply_hbm_frac": 8.0 * M0 * n / (na_ms * 1e-3) / 1e9 / hbm_peak()[0]}
-    del Nm
+    if not args.no_next_rows:
+        dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+        vx = timer(lambda: ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A, variant=2), 10)
+        next_rows["vortex_sheet_matrix"] = {"call": "bie_build(variant=BIE_VARIANT_VORTEX)", "ms": vx["median_ms"], "best_ms": vx["best_ms"],
+                                            "gentries_per_s": n * n / (vx["median_ms"] * 1e-3) / 1e9,
+                                            "fp64_frac_of_probe": n * n * FP64_PER_PAIR_VORTEX / (vx["median_ms"] * 1e-3) / dfma_per_s,
+                                            "hbm_write_frac": 8.0 * n * n / (vx["median_ms"] * 1e-3) / 1e9 / peak}
+        ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z, variant=2)
+        vmf = timer(lambda: ctx.bie_matvec_free(xv, yv), 20)
+        next_rows["vortex_sheet_matrix"]["matrix_free_matvec_ms"] = vmf["median_ms"]
+        next_rows["vortex_sheet_matrix"]["matrix_free_fp64_frac_of_probe"] = n * n * FP64_PER_PAIR_VORTEX / (vmf["median_ms"] * 1e-3) / dfma_per_s
+        if P.centers:
+            ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A, variant=1)
+            cy = timer(lambda: ctx.bie_add_cyl_columns(g.counts, g.kinds, z, P.centers, A), 10)
+            nobs_cols = int(sum(int(cn) for cn, kd in zip(g.counts, g.kinds) if kd == 2))
+            next_rows["appendix_b_columns"] = {"call": "bie_add_cyl_columns (in place on the variant-B matrix)", "ms": cy["median_ms"],
+                                               "entries": n * nobs_cols, "gbs": 16.0 * n * nobs_cols / (cy["median_ms"] * 1e-3) / 1e9,
+                                               "hbm_frac": 16.0 * n * nobs_cols / (cy["median_ms"] * 1e-3) / 1e9 / peak}
+        # NEXT-3: 2 functions (Phi', Phi_t of Eq. 5.3) at 65 536 points below the free surface
+        npts_e = 65536
+        rng_e = np.random.default_rng(3)
+        ie = rng_e.integers(0, int(g.counts[0]), size=npts_e)
+        zp_e = dev(g.zeta[ie] - 1j * rng_e.uniform(0.01, 0.3, size=npts_e))
+        f_e = dev(np.vstack([np.exp(1j * g.zeta), np.exp(2j * g.zeta)]))
+        out_e = torch.empty((2, npts_e), dtype=torch.complex128, device="cuda")
+        ev = timer(lambda: ctx.bie_cauchy_eval(g.counts, g.kinds, z, dz, f_e, zp_e, out=out_e), 5)
+        ev_instr = 12 + 4 * 3     # FP64-pipe instructions per pair: cot (12) + denominator and two numerators (4 each)
+        next_rows["cauchy_eval_near_boundary"] = {"call": "bie_cauchy_eval (nf = 2)", "points": npts_e, "sources": n, "ms": ev["median_ms"],
+                                                  "gpairs_per_s": npts_e * n / (ev["median_ms"] * 1e-3) / 1e9,
+                                                  "fp64_instr_per_pair": ev_instr,
+                                                  "fp64_frac_of_probe": npts_e * n * ev_instr / (ev["median_ms"] * 1e-3) / dfma_per_s}
+        del zp_e, f_e, out_e
+        M0 = int(g.counts[0])
+        Nm = A.view(-1)[: M0 * A.stride(0)].view(M0, A.stride(0))       # the first M_0 rows of the same allocation
+        wv = torch.from_numpy(np.random.default_rng(2).standard_normal(n)).cuda()
+        uv = torch.empty(M0 + (M0 & 1), dtype=torch.float64, device="cuda")[:M0]
+        nb = timer(lambda: ctx.bie_build_normal_velocity(g.counts, g.kinds, z, dz, d2z, Nm), 10)
+        na = timer(lambda: ctx.bie_matvec_rect(Nm, wv, uv), 20)
+        next_rows["normal_velocity"] = {"call": "bie_build_normal_velocity + bie_matvec_rect", "rows": M0, "cols": n,
+                                        "build_ms": nb["median_ms"], "build_gentries_per_s": M0 * n / (nb["median_ms"] * 1e-3) / 1e9,
+                                        "build_hbm_write_frac": 8.0 * M0 * n / (nb["median_ms"] * 1e-3) / 1e9 / peak,
+                                        "apply_ms": na["median_ms"], "apply_gbs": 8.0 * M0 * n / (na["median_ms"] * 1e-3) / 1e9,
+                                        "apply_hbm_frac": 8.0 * M0 * n / (na["median_ms"] * 1e-3) / 1e9 / peak}
+        del Nm
 
     # ---- end to end through bie_solve_host, pinned host buffers ---------------------------------------------
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     hz, hdz, hd2z, hb = pin(g.zeta.view(np.float64)), pin(g.dzeta.view(np.float64)), pin(g.d2zeta.view(np.float64)), pin(P.rhs[0])
     hx = torch.empty(n, dtype=torch.float64).pin_memory()
-    del A
+    del W, A
     torch.cuda.empty_cache()
     sws = torch.empty(ctx.bie_solve_workspace_bytes(n, P.restart, solve_mode), dtype=torch.uint8, device="cuda")
     for _ in range(2):
@@ -457,69 +650,63 @@ def main():
     e2e_s = max_over_ranks((time.perf_counter() - t0) / K)
     h2d = 3 * 16 * n + 8 * n
     d2h = 8 * n + 8 + 8
+    del sws
+    torch.cuda.empty_cache()
+
+    # ---- per_config (configs 1-4) ------------------------------------------------------------------------------
+    per_config = {}
+    if not args.no_per_config and args.config == 5 and world == 1:
+        for c in (1, 2, 3, 4):
+            per_config[str(c)] = measure_config(torch, bie, ctx, c, timer, dfma_per_s)
 
     if rank != 0:
         ranks.finish(R)
         return
 
     # ---- rooflines -------------------------------------------------------------------------------------------
-    peak, peak_src = hbm_peak()
-    # operator applications in the GMRES bracket of one step (all stages; the last stage's count stands for each)
-    ng = n_gemv(iters, P.restart) * nstage
-    if args.op != "dense":
-        sc = args.stored_cols          # 0 (matrix-free) or the slab width (hybrid)
-        pairs = ng * n * (n - sc)
-        per_entry = FP64_INSTR_PER_PAIR_FREE if sc else FP64_INSTR_PER_ENTRY_SYM   # hybrid: one-directional loops
-        instr = pairs * per_entry + ng * n * sc          # + one DFMA per streamed slab entry
-        roof = {"bound": "alu", "kernel": "bie_gmres_kernel<%s> (persistent; pair loops dominate)" % args.op,
-                "achieved": instr / (gmres_ms * 1e-3) / 1e12, "peak": dfma_per_s / 1e12,
-                "unit": "T FP64 instr/s", "traffic": TRAFFIC_BYTES.get((args.config, args.op)),
-                "fp64_instr_per_entry": per_entry,
-                "pairs_per_launch": pairs, "operator_applications_per_launch": ng,
-                "peak_source": "bie_probe_dfma in this run (nominal 148 SM x 64 lanes x 1.965 GHz = 18.6)"}
-        if sc:   # the slab is streamed from HBM by the other warps at the same time
-            gbs = ng * 8.0 * n * sc / (gmres_ms * 1e-3) / 1e9
-            roof["hbm_concurrent"] = {"achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
-                                      "algorithmic_bytes_per_launch": ng * 8 * n * sc, "peak_source": peak_src}
-    else:
-        roof = {"bound": "hbm", "kernel": "bie_gmres_kernel (persistent; GEMV phases dominate)",
-                "achieved": ng * 8.0 * n * n / (gmres_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
-                "traffic": TRAFFIC_BYTES.get((args.config, args.op)), "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": ng * 8 * n * n, "gemvs_per_launch": ng}
-    roof["frac"] = roof["achieved"] / roof["peak"]
-    roof_build = None
-    if True:
-        ach = n * n * FP64_INSTR_PER_ENTRY / (build_ms * 1e-3)
-        roof_build = {"bound": "alu", "kernel": "bie_build_kernel (+ node prep)", "achieved": ach / 1e12,
-                      "peak": dfma_per_s / 1e12, "unit": "T FP64 instr/s", "frac": ach / dfma_per_s,
-                      "peak_source": "bie_probe_dfma in this run (nominal 148 SM x 64 lanes x 1.965 GHz = 18.6)",
-                      "fp64_instr_per_entry": FP64_INSTR_PER_ENTRY,
-                      "hbm_write_gbs": 8.0 * n * n / (build_ms * 1e-3) / 1e9, "hbm_write_frac": 8.0 * n * n / (build_ms * 1e-3) / 1e9 / peak}
+    ng = n_gemv(iters, P.restart) * nstage       # operator applications in the GMRES bracket of one step
+    nd = args.nd
+    roof = gmres_roofline(n, op, nd, ng, gmres_ms, dfma_per_s, clocks and clocks.get("sm_mhz"), args.config)
+    ach = n * n * FP64_PER_ENTRY_BUILD / (build_ms * 1e-3)
+    roof_build = {"bound": "hbm", "kernel": "bie_build_kernel (+ node prep), stand-alone calls",
+                  "achieved": 8.0 * n * n / (build_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s (write)",
+                  "frac": 8.0 * n * n / (build_ms * 1e-3) / 1e9 / peak, "peak_source": peak_src,
+                  "fp64": {"achieved": ach / 1e12, "unit": "T FP64 instr/s", "fp64_instr_per_entry": FP64_PER_ENTRY_BUILD,
+                           "frac_of_probe": ach / dfma_per_s, "frac_of_nominal": ach / NOMINAL_FP64_INSTR_S,
+                           "peak_probe": dfma_per_s / 1e12, "peak_nominal": NOMINAL_FP64_INSTR_S / 1e12},
+                  "note": "with 10 FP64 instructions per entry the HBM write of 8 B per entry is the binding bound; the FP64 fractions "
+                          "are the non-binding leg"}
+    # kernels launched per step: node prep (1) [+ tile kernel (1)] + GMRES (1) per stage; the near matrix (count, scan, fill) and the
+    # symmetric work list (1) once per stage geometry for the matrix-free and hybrid operators
+    launches = {"dense": 3, "free": 2 + 4, "hybrid": 3 + 4}[op] * nstage
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic", "config": workload_config(P, args, iters),
-            "build": {"gentries_per_s": n * n / (build_ms * 1e-3) / 1e9, "ms": build_ms,
-                      "in_step": args.op == "dense",
-                      "note": "inside the timed step" if args.op == "dense" else
-                              "full bie_build, stand-alone calls outside the timed region; inside the step the %s operator "
-                              "spent %.4f ms on its own preparation (node tables%s)"
-                              % (args.op, prep_ms, " + slab of %d columns" % args.stored_cols if args.stored_cols else "")},
-            "build_update": {"ms": upd_ms, "entries": upd_entries, "gentries_per_s": upd_entries / (upd_ms * 1e-3) / 1e9,
-                             "share_of_matrix": upd_entries / float(n * n)},
+            "build": {"gentries_per_s": n * n / (build_ms * 1e-3) / 1e9, "ms": build_ms, "best_ms": bt["best_ms"], "reps": bt["reps"],
+                      "in_step": op == "dense",
+                      "note": "full bie_build, stand-alone calls outside the timed region (median of 20); inside the step the %s operator "
+                              "spent %.4f ms on its own preparation per first stage (node tables%s)"
+                              % (op, prep_ms, {"dense": " + whole matrix", "free": "", "hybrid": " + leading block of %d rows" % nd}[op])},
+            "build_update": {"ms": upd["median_ms"], "best_ms": upd["best_ms"], "entries": upd_entries,
+                             "gentries_per_s": upd_entries / (upd["median_ms"] * 1e-3) / 1e9, "share_of_matrix": upd_entries / float(n * n)},
             "gmres": {"ms": gmres_ms, "iters": iters, "relres_true": relres, "us_per_iter": gmres_ms * 1e3 / max(iters * nstage, 1),
                       "stages": nstage, "note": "ms covers all stages of the step (incl. their rebuilds after the first); iters is the last stage's"},
             "e2e": {"value": world * n * n / e2e_s / 1e9, "unit": UNIT, "ms_per_step": e2e_s * 1e3,
-                    "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "api": "bie_solve_host", "iters": e_it},
-            "gpu_launches": launches_per_step * K,
+                    "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "api": "bie_solve_host (first stage of the config)", "iters": e_it},
+            "gpu_launches": launches * K,
             "roofline": roof, "roofline_build": roof_build, "matvec": matvec, "clocks": clocks,
             "fp64_probe_tflops": 2 * dfma_per_s / 1e12,
-            "operator_choice_ms_per_step": choice_ms or None, "next_rows": next_rows}
+            "operator_choice_ms_per_step": choice_ms or None, "per_config": per_config or None, "next_rows": next_rows or None}
     if not args.no_cpu_baseline:
-        est, desc, cores, parts = oracle_sample(P, iters, args.cpu_seconds)
-        line["cpu_baseline"] = {"value": n * n / est / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
-                                "ms_per_step": est * 1e3, "build_gentries_per_s": n * n / parts["build_s"] / 1e9,
-                                "gmres_ms": parts["gemv_s"] * parts["gemvs"] * 1e3}
+        cfgs = sorted(set([args.config] + ([1, 2, 3, 4] if per_config else [])))
+        cb = cpu_baseline(cfgs)
+        h = cb[str(args.config)]
+        line["cpu_baseline"] = {"value": h["gentries_per_s"], "unit": UNIT, "cores": h["cores"], "kind": "oracle", "estimated": False,
+                                "sample": "ONE real pass of the oracle over the whole workload (oracle.build_matrix + oracle.gmres, every "
+                                          "stage) on all host cores; per_config holds the same for configs 1-4 and one-thread runs for 1-3",
+                                "ms_per_step": h["step_s"] * 1e3, "build_gentries_per_s": h["build_gentries_per_s"],
+                                "gmres_ms": h["gmres_s"] * 1e3, "iters": h["iters"], "per_config": cb}
     print(json.dumps(line), flush=True)
     ranks.finish(R)
 
