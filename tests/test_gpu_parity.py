@@ -1016,10 +1016,11 @@ def test_error_codes_of_the_operator_and_next_calls(ctx):
     of = torch.zeros(1, dtype=torch.float64, device="cuda")
     b = torch.ones(n, dtype=torch.float64, device="cuda")
     x = torch.empty_like(b)
-    ctx.bie_build_block(g.counts, g.kinds, z, dz, d2z, 128, A)
+    Ab = torch.empty(bie.Context.bie_hybrid_block_bytes(n) // 8, dtype=torch.float64, device="cuda")   # room for any block edge
+    ctx.bie_build_block(g.counts, g.kinds, z, dz, d2z, 128, Ab)
     for nd, code in [(127, -6), (n, -6), (0, -6), (2, -6), (130, -6), (256 + 64, -6)]:   # odd, whole matrix, none, not a row-block boundary
         with pytest.raises(bie.BieError) as e:
-            ctx.bie_gmres_hybrid(A, nd, b, x, 1e-13, 50, 10, ws, oi, of)
+            ctx.bie_gmres_hybrid(Ab, nd, b, x, 1e-13, 50, 10, ws, oi, of)
         assert e.value.code == code, nd
     with pytest.raises(bie.BieError) as e:                             # empty slab
         ctx.bie_build_cols(g.counts, g.kinds, z, dz, d2z, 0, A)
