@@ -77,6 +77,11 @@ struct FreePlan {
 #ifndef SYM_BATCH
 #define SYM_BATCH 8
 #endif
+#ifndef SYM_PART_PAD
+#define SYM_PART_PAD 256      // symmetric work list: every row block's list is longer by this many VIRTUAL sources (no work): the fixed
+                              // cost of starting a part (target loads, exposed first loads of its segments, warp-sum reduction; measured
+                              // about 5 us = the time of 250-300 sources), so that cutting the list into equal slabs equalises TIME
+#endif
 #define SYM_COL_STRIDE 33                                         // [SYM_BATCH][33] doubles per warp: lane-private slots, no bank conflicts
 #define SYM_COL_DOUBLES (FREE_WARPS * SYM_BATCH * SYM_COL_STRIDE)
 // one staging buffer of a warp (32 sources): E and (U,W) as double2; + (R,B) for the vortex-sheet matrix
@@ -244,10 +249,8 @@ __device__ __forceinline__ void free_parts_impl(const NodeTable& nt, const CompT
         int buf = 0;
         __syncwarp();
         if (wa < wb) issue(wa, 0);
-        // the first chunk of warp w is shorter by 2 w sources: the warps reach their poll() calls evenly spread in time instead
-        // of all at once (the ring of the hybrid operator is only a few tiles deep)
-        int len = 32 - 2 * (warp & 15);
-        for (int base = wa; base < wb; base += len, len = 32, buf ^= 1) {
+        const int len = 32;
+        for (int base = wa; base < wb; base += len, buf ^= 1) {
             const double2* sg = stage + buf * (fp.stage_buf >> 1);
             asm volatile("cp.async.wait_group 0;" ::: "memory");
             __syncwarp();                                   // chunk landed for all lanes; the other buffer is no longer read

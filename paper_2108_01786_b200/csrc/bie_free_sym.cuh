@@ -66,7 +66,8 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
         const int rows = free_block_rows(fp, b, nt.n);
         const bool below = (row0 + rows <= fp.s_off);        // hybrid: a row block of the stored block's rows
         const int src0 = below ? fp.s_off : row0;
-        const int sa = src0 + (int)(u0 - ub), sb = src0 + (int)(ue - ub);   // sources [sa, sb), all >= src0
+        // list positions [ub, ub + SYM_PART_PAD) of a block are virtual (bie_free.cuh): sources [sa, sb), all >= src0
+        const int sa = src0 + (int)max(0LL, (u0 - ub) - SYM_PART_PAD), sb = src0 + (int)max(0LL, (ue - ub) - SYM_PART_PAD);
         double ter[FREE_NT], tei[FREE_NT], acc[FREE_NT];
         int thi[FREE_NT];
         bool live[FREE_NT];
@@ -109,15 +110,10 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
             }
             int buf = 0;
             __syncwarp();
-            // the first chunk of warp w is shorter by 2 w sources (a multiple of SYM_BATCH would be kinder to the batches, but the
-            // tail batch handles any count): the warps reach their poll() calls evenly spread in time instead of all at once
-            int len = 32 - 2 * (warp & 15);
-            for (int base = wa; base < wb; base += len, len = 32, buf ^= 1) {
+            const int len = 32;
+            for (int base = wa; base < wb; base += len, buf ^= 1) {
                 double2* sg = reinterpret_cast<double2*>(stage + buf * sbuf);
-                {   // lanes beyond this chunk stage zero sources (the batches below run over whole multiples of SYM_BATCH)
-                    const bool in = lane < len;
-                    sg[lane] = in ? ne : zero2; sg[32 + lane] = in ? nuw : zero2;
-                }
+                sg[lane] = ne; sg[32 + lane] = nuw;     // lanes beyond wb stage zero sources (the batches run over multiples of SYM_BATCH)
                 __syncwarp();
                 {
                     const int s = base + len + lane;

@@ -95,13 +95,20 @@ __device__ __forceinline__ double warp_sum_partials(const double* p, int G)
     return bie_warp_sum(s);
 }
 
-#ifdef BIE_PHASE_TIMING   // developer build (BIE_NVCC_EXTRA=-DBIE_PHASE_TIMING): CTA 0 prints the mean time per Arnoldi step of each phase
+#ifdef BIE_PHASE_TIMING   // developer build (BIE_NVCC_EXTRA=-DBIE_PHASE_TIMING): three CTAs print the mean time per Arnoldi step of each phase
 #include <cstdio>
 __device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#define PT_DECL unsigned long long pt_t0 = gtime(), pt_acc[6] = {0, 0, 0, 0, 0, 0};
-#define PT(i) { const unsigned long long pt_t1 = gtime(); pt_acc[i] += pt_t1 - pt_t0; pt_t0 = pt_t1; }
+#ifndef BIE_PT_PAIR_ONLY
+#define BIE_PT_PAIR_ONLY 0
+#endif
+__device__ unsigned long long g_pt[3][16];
+__device__ unsigned long long g_pt0[3];
+__device__ unsigned long long g_pair[256], g_gath[256];   // per CTA: accumulated pair-loop / gather time of the current cycle
+__device__ __forceinline__ int pt_slot() { return blockIdx.x == 0 ? 0 : (blockIdx.x == gridDim.x / 2 ? 1 : (blockIdx.x == gridDim.x - 1 ? 2 : -1)); }
+#define PT_RESET { if (threadIdx.x == 0) { g_pair[blockIdx.x] = 0; g_gath[blockIdx.x] = 0; } const int s_ = pt_slot(); if (threadIdx.x == 0 && s_ >= 0) { for (int q_ = 0; q_ < 16; ++q_) g_pt[s_][q_] = 0; g_pt0[s_] = gtime(); } }
+#define PT(i) { const int s_ = pt_slot(); if (threadIdx.x == 0 && s_ >= 0) { const unsigned long long t_ = gtime(); g_pt[s_][i] += t_ - g_pt0[s_]; g_pt0[s_] = t_; } }
 #else
-#define PT_DECL
+#define PT_RESET
 #define PT(i)
 #endif
 
@@ -120,17 +127,20 @@ __device__ __forceinline__ void cta_apply(const GmresArgs& a, int r0, int r1, co
             free_write_tables(a.nt, a.ct, a.fp, r0, r1, xin + r0, red);
             grid_barrier(a.sync, target);
         }
+        PT(6)
         if (MODE == 1) {
+#ifdef BIE_PHASE_TIMING
+            const unsigned long long tp0 = gtime();
+#endif
             free_parts(a.nt, a.ct, a.fp, gpart, cta_team(), NoPoll());
+#ifdef BIE_PHASE_TIMING
+            if (threadIdx.x == 0) g_pair[blockIdx.x] += gtime() - tp0;
+#endif
+            PT(7)
         } else {
             const int warp = threadIdx.x >> 5;
             if (threadIdx.x == 0) { ring.next[0] = 0; ring.next[1] = 0; }
             __syncthreads();
-#ifdef BIE_PHASE_TIMING
-            __shared__ unsigned long long hy_acc[4];
-            if (threadIdx.x == 0 && ring.tile0 == 0) { hy_acc[0] = hy_acc[1] = hy_acc[2] = hy_acc[3] = 0; }
-            const unsigned long long hy_t0 = gtime();
-#endif
             // nwf >= 12: the service warps -- the producer (warp 15) and 15 - nwf consumer warps -- all sit on ONE of the SM's
             // four sub-partitions (warp & 3 == 3: warps 15, 11, 7, 3), so that they do not wait for issue slots behind the
             // pair-loop warps of the other three.  nwf = 12: the pair loops run on exactly three sub-partitions, four warps
@@ -141,9 +151,6 @@ __device__ __forceinline__ void cta_apply(const GmresArgs& a, int r0, int r1, co
             if (warp == GM_WARPS - 1) {
                 if ((threadIdx.x & 31) == 0) ring_produce<STREAM>(ring, xin);
                 __syncwarp();
-#ifdef BIE_PHASE_TIMING
-                if ((threadIdx.x & 31) == 0) hy_acc[2] += gtime() - hy_t0;
-#endif
             } else {
                 if (!service) {
                     Team tm = sub_team(0, a.nwf, 1);
@@ -153,23 +160,9 @@ __device__ __forceinline__ void cta_apply(const GmresArgs& a, int r0, int r1, co
                     }
                     free_parts(a.nt, a.ct, a.fp, gpart, tm, RingPoll{&ring, a.poll_tiles});
                 }
-#ifdef BIE_PHASE_TIMING
-                if (threadIdx.x == 0) hy_acc[0] += gtime() - hy_t0;
-#endif
                 while (ring_consume(ring)) { }
-#ifdef BIE_PHASE_TIMING
-                if (threadIdx.x == 0) hy_acc[1] += gtime() - hy_t0;
-#endif
             }
             __syncthreads();
-#ifdef BIE_PHASE_TIMING
-            if (threadIdx.x == 0) {
-                hy_acc[3] += 1;
-                if (hy_acc[3] == 40 && (blockIdx.x == 0 || blockIdx.x == 100))
-                    printf("cta %d hybrid us/apply: pair loops (warp 0) %.1f, + drain %.1f, producer done %.1f\n", blockIdx.x,
-                           hy_acc[0] * 1e-3 / 40, hy_acc[1] * 1e-3 / 40, hy_acc[2] * 1e-3 / 40);
-            }
-#endif
             // the rows of the stored block this CTA streamed: chunk sums in fixed order -> yd (their owners read it after the barrier)
             for (int r = threadIdx.x; r < ring.r1 - ring.r0; r += blockDim.x) {
                 double sum = 0.0;
@@ -179,7 +172,15 @@ __device__ __forceinline__ void cta_apply(const GmresArgs& a, int r0, int r1, co
             ring.tile0 += (unsigned long long)ring.nunit;
         }
         grid_barrier(a.sync, target);
+        PT(8)
+#ifdef BIE_PHASE_TIMING
+        const unsigned long long tg0 = gtime();
+#endif
         free_gather(a.nt, a.ct, a.fp, r0, r1, xin, scale, gpart, y_local);
+#ifdef BIE_PHASE_TIMING
+        if (threadIdx.x == 0) g_gath[blockIdx.x] += gtime() - tg0;
+#endif
+        PT(9)
         if (MODE == 2) {
             for (int r = threadIdx.x; r < r1 - r0; r += blockDim.x)
                 if (r0 + r < a.nd) y_local[r] = fma(scale, __ldcg(a.yd + r0 + r), y_local[r]);
@@ -414,7 +415,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
         // ---- Arnoldi steps ------------------------------------------------------------------------
         int k = 0;
         bool conv = false;
-        PT_DECL
+        PT_RESET
         for (int j = 0; j < m; ++j) {
             PT(5)
             // a6: y = A (wbuf * inv) = A v_j + V_j c * inv  (c = 0 in the first step of a cycle)
@@ -521,10 +522,20 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
             if (conv || iters >= a.max_iters) break;
         }
 #ifdef BIE_PHASE_TIMING
-        if (threadIdx.x == 0 && blockIdx.x == 0)
-            printf("cycle of %d steps, us per step: operator %.1f | dots1 + barrier1 %.1f | reduce + w1 + tables + dots2 %.1f | barrier2 %.1f | "
-                   "tail %.1f | loop %.1f\n", k, pt_acc[0] * 1e-3 / k, pt_acc[1] * 1e-3 / k, pt_acc[2] * 1e-3 / k,
-                   pt_acc[3] * 1e-3 / k, pt_acc[4] * 1e-3 / k, pt_acc[5] * 1e-3 / k);
+        if (threadIdx.x == 0 && blockIdx.x == 0 && MODE == 1) {
+            printf("pair-loop us per step by CTA:");
+            for (int c = 0; c < (int)gridDim.x; ++c) printf(" %.0f", g_pair[c] * 1e-3 / k);
+            printf("\ngather us per step by CTA:");
+            for (int c = 0; c < (int)gridDim.x; ++c) printf(" %.1f", g_gath[c] * 1e-3 / k);
+            printf("\n");
+        }
+        if (threadIdx.x == 0 && pt_slot() >= 0 && !BIE_PT_PAIR_ONLY) {
+            const unsigned long long* q = g_pt[pt_slot()];
+            printf("cta %3d, cycle of %d steps, us per step: [operator: tables/x %.1f | pair loops or GEMV %.1f | barrier %.1f | gather %.1f | rest %.1f] "
+                   "dots1 + barrier1 %.1f | reduce + w1 + tables + dots2 %.1f | barrier2 %.1f | tail %.1f | loop %.1f\n", (int)blockIdx.x, k,
+                   q[6] * 1e-3 / k, q[7] * 1e-3 / k, q[8] * 1e-3 / k, q[9] * 1e-3 / k, q[0] * 1e-3 / k, q[1] * 1e-3 / k, q[2] * 1e-3 / k,
+                   q[3] * 1e-3 / k, q[4] * 1e-3 / k, q[5] * 1e-3 / k);
+        }
 #endif
         // ---- a9: y = R^{-1} g (CTA 0), x += V y ---------------------------------------------------
         if (blockIdx.x == 0) {

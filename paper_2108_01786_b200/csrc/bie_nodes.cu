@@ -185,7 +185,7 @@ __global__ void bie_sym_tables_kernel(int NB, int NB0, int M0, int n, int npad, 
         pos[b] = k;
         const int row0 = b < NB0 ? b * FREE_ROWS : M0 + (b - NB0) * FREE_ROWS;
         const int src0 = b < first ? s_off : row0;
-        c += (npad - src0);
+        c += SYM_PART_PAD + (npad - src0);     // + the virtual sources that stand for the fixed cost of a part
         cum[k + 1] = c;
     }
     (void)n;
@@ -246,7 +246,7 @@ int bie_free_plan(bie_ctx* ctx, int grid, int s_off, FreePlan* fp, cudaStream_t 
         int* pos = perm + nbmax;
         if (ctx->sym_key[0] != ctx->geom_gen || ctx->sym_key[1] != s_off) {
             long long U = 0;
-            for (int b = 0; b < NB; ++b) U += npad - (b < first ? s_off : row0_of(b));
+            for (int b = 0; b < NB; ++b) U += SYM_PART_PAD + npad - (b < first ? s_off : row0_of(b));
             bie_sym_tables_kernel<<<1, 32, 0, st>>>(NB, fp->NB0, fp->M0, n, npad, s_off, first, cum, perm, pos);
             BIE_CUDA(cudaGetLastError());
             ctx->sym_key[0] = ctx->geom_gen; ctx->sym_key[1] = s_off;
