@@ -43,8 +43,8 @@ METRIC = "matrix build Gentries/s and GMRES solve ms (FP64); % of FP64 / HBM roo
 UNIT = "Gentries/s"
 # FP64-pipe instructions per matrix entry (DFMA + DMUL + DADD), SASS counts from the ncu captures under profiles/
 # (profiles/r02_build.md, profiles/r02_free.md); the hand counts of DESIGN.md section 5 are 10 / 10 / 6.5 + reduction
-FP64_PER_ENTRY_BUILD = 10.0     # bie_build_kernel, difference form
-FP64_PER_ENTRY_SYM = 6.8        # symmetric pair loops: 13 per pair of entries + lane reduction of the reverse sums
+FP64_PER_ENTRY_BUILD = 10.1     # bie_build_kernel, difference form
+FP64_PER_ENTRY_SYM = 6.92       # symmetric pair loops: 13 per pair of entries + lane reduction of the reverse sums
 FP64_PER_PAIR_VORTEX = 13.0     # vortex-sheet matrix, (X, Y) form
 NOMINAL_FP64_INSTR_S = 148 * 64 * 1.965e9   # B200: 148 SMs x 64 FP64 lanes x 1.965 GHz = 18.6 T instr/s
 HBM_FALLBACK_GBS = 6650.0      # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
