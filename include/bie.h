@@ -278,6 +278,10 @@ int bie_solve_host(bie_ctx* ctx, int ncomp, const int32_t* counts, const int32_t
  * *total_fma (host) receives the number of FMAs issued.
  */
 int bie_probe_dfma(bie_ctx* ctx, int64_t fma_per_thread, double* out, int64_t* total_fma, void* stream);
+/* Read-only streaming probe: sums nbytes (multiple of 16) of `buf` (dev, 16-byte aligned) with 128-bit evict-first loads
+ * from every SM, the access pattern of the GEMV, so that bench.py can quote the GEMV against a READ peak measured in the
+ * same run (MEASURED_PEAKS.json's number is a read+write copy).  out: dev, >= 8 bytes. */
+int bie_probe_read(bie_ctx* ctx, const double* buf, int64_t nbytes, double* out, void* stream);
 
 #ifdef __cplusplus
 }

@@ -25,7 +25,7 @@ EXPORTS = ("bie_create", "bie_destroy", "bie_strerror", "bie_device_info", "bie_
            "bie_solve_workspace_bytes", "bie_solve_host", "bie_probe_dfma", "bie_build_cols", "bie_hybrid_cols",
            "bie_set_hybrid_free_warps", "bie_gmres_hybrid", "bie_matvec_rect", "bie_build_normal_velocity",
            "bie_add_cyl_columns", "bie_cauchy_eval_workspace_bytes", "bie_cauchy_eval", "bie_set_symmetric",
-           "bie_build_block", "bie_set_hybrid_poll_tiles", "bie_hybrid_block_bytes")
+           "bie_build_block", "bie_set_hybrid_poll_tiles", "bie_hybrid_block_bytes", "bie_probe_read")
 
 BIE_OK, BIE_MAX_ITERS = 0, 1
 OP_DENSE, OP_FREE, OP_HYBRID = 0, 1, 2
@@ -102,6 +102,8 @@ def lib() -> ctypes.CDLL:
         L.bie_cauchy_eval.argtypes = [vp, i32, ip, ip, vp, vp, i32, vp, i32, vp, vp, vp, sz, vp]
         L.bie_set_symmetric.restype = i32
         L.bie_set_symmetric.argtypes = [vp, i32]
+        L.bie_probe_read.restype = i32
+        L.bie_probe_read.argtypes = [vp, vp, i64, vp, vp]
         L.bie_probe_dfma.restype = i32
         L.bie_probe_dfma.argtypes = [vp, i64, vp, ctypes.POINTER(i64), vp]
         _lib = L
@@ -363,6 +365,11 @@ class Context:
         return int(iters.value), float(relres.value), int(rc)
 
     # ---- roofline probe ----------------------------------------------------------------------------------
+    def bie_probe_read(self, buf, out):
+        """streams the CUDA float64 tensor `buf` once, read-only (roofline denominator of the GEMV)"""
+        nbytes = (buf.numel() * buf.element_size()) // 16 * 16
+        _check(lib().bie_probe_read(self._h, buf.data_ptr(), nbytes, _dev_f64(out, 1), _stream()), "bie_probe_read")
+
     def bie_probe_dfma(self, fma_per_thread: int, out) -> int:
         total = ctypes.c_int64()
         _check(lib().bie_probe_dfma(self._h, int(fma_per_thread), _dev_f64(out, 1), ctypes.byref(total), _stream()),

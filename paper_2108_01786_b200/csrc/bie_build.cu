@@ -23,6 +23,11 @@
 #define BUILD_COLS 2
 #define BUILD_TILE_W (BUILD_THREADS * BUILD_COLS)
 #define BUILD_RB 4
+#ifndef BUILD_MIN_CTAS
+#define BUILD_MIN_CTAS 4      // CTAs of 128 threads per SM the register allocation must allow.  Measured at config 5 (0.411 ms at 4):
+                              // 5 -> 0.414, 6 -> 0.448, 8 -> 0.487 ms: the kernel wants its registers, not more warps; and
+                              // FEWER resident CTAs (shared-memory padding to 3 / 2 per SM) are slower too: 0.45 / 0.55 ms
+#endif
 
 struct SrcCol {
     double er, ei;      // E_s
@@ -59,7 +64,9 @@ __device__ __forceinline__ void bie_block_coef(bool src0, bool tgt0, double qr, 
     else              { al = 2.0 * qr;  be = qi; }       // -Re c  (-G_k0)
 }
 
-__global__ void __launch_bounds__(BUILD_THREADS)
+// TILED: A is the block format of the hybrid operator (bie_common.cuh) instead of row-major with leading dimension lda
+template <bool TILED>
+__global__ void __launch_bounds__(BUILD_THREADS, BUILD_MIN_CTAS)
 bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long lda, int T, int only0, int ncols, int nrows)
 {
     extern __shared__ __align__(16) double2 sm[];  // [T] E_t
@@ -99,13 +106,14 @@ bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long l
         }
         for (int tb = a; tb < b; tb += BUILD_RB) {
             int flag = 0;
+            double* row = TILED ? A : A + (long long)tb * lda + s0;
 #pragma unroll
             for (int r = 0; r < BUILD_RB; ++r) {
                 const int t = min(tb + r, b - 1);  // the tail repeats the last row (same values, same address)
                 const double2 te = sE[t - t0];
                 const double e0 = bie_entry_fast(src[0], te, flag);
                 const double e1 = bie_entry_fast(src[1], te, flag);
-                double* p = A + bie_entry_off(lda, nchT, t, s0);
+                double* p = TILED ? A + bie_entry_off(0, nchT, t, s0) : row + (long long)(t - tb) * lda;
                 if (full) *reinterpret_cast<double2*>(p) = make_double2(e0, e1);
                 else if (part) p[0] = e0;
             }
@@ -122,7 +130,7 @@ bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long l
                             if (__double2hiint(den) < src[c].thi) {
                                 double al, be;
                                 bie_block_coef(scomp[c] == 0, k == 0, sqr[c], sqi[c], al, be);
-                                A[bie_entry_off(lda, nchT, t, s0 + c)] =
+                                A[bie_entry_off(TILED ? 0 : lda, nchT, t, s0 + c)] =
                                     bie_entry_near(nt.DG, nt.XY, al, be, (scomp[c] == k) ? sem[c] : 0.0, s0 + c, t);
                             }
                         }
@@ -134,7 +142,7 @@ bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long l
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Vortex-sheet variant (BIE_VARIANT_VORTEX): the matrix S of Eqs. (4.14) + (4.17) from
+// Vortex-sheet variant (BIE_VARIANT_VORTEX) and normal-velocity operator: the matrix S of Eqs. (4.14) + (4.17) from
 // the adjoint matrices of Eq. (4.7), (K+_jk)_ml = K_jk(alpha_jl, alpha_km)/M_j.  Entry of row
 // t = (k,m), column s = (j,l):   c+ = zeta'_t/(2 M_j) cot((zeta_t - zeta_s)/2) = -(u_t/M_j)(-2X + iY)/den,
 // u_t = zeta'_t/2, i.e. the weight comes from the ROW node and only 1/M_j from the column.  With m_s = 1/M_j folded
@@ -142,88 +150,111 @@ bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long l
 //     Im c+ -> (A, B) = (2 u_i, -u_r)   [k = 0, j = 0: 1/2 I + K+_00]  and  [k, j >= 1: -1/2 I + K+_jk]
 //    -Re c+ -> (-2 u_r, -u_i)           [k = 0, j >= 1: -G+_j0]
 //     Re c+ -> ( 2 u_r,  u_i)           [k >= 1, j = 0:  G+_0k]
-// again 13 FP64-pipe instructions per entry; (A, B) sit in shared memory per target row, one pair for columns
-// on Gamma_0 and one for columns on solids.  Same tiling, near-pair handling and stores as bie_build_kernel.
+// 11 FP64-pipe instructions per entry in the row-side difference form (bie_entry_fast_dagger); the row constants (U, W, B) sit
+// in shared memory per target row, one set for columns on Gamma_0 and one for columns on solids.  Same tiling, near-pair
+// handling and stores as bie_build_kernel.
 struct SrcColD {
     double er, ei;        // E_s
-    double ser, sei, sm;  // m_s E_s, m_s M_s
     double ms;            // 1 / M_j
     int thi;
 };
 
-__device__ __forceinline__ double bie_entry_fast_dagger(const SrcColD& s, const double2 te, const double tm,
-                                                        const double2 ab, int& flag)
+// (A_t, B_t) of the row's weight u_t = zeta'_t / 2 for a column on Gamma_0 (col0) or on a solid:
+//   normal-velocity operator (kap): -G+_00 (3.24) ; K+_j0 (3.19)      row on Gamma_0: K+_00 ; -G+_j0      row on a solid: G+_0k ; K+_jk
+__device__ __forceinline__ double2 bie_dagger_ab(bool kap, bool row0, bool col0, double ur, double ui)
+{
+    const double2 im = make_double2(2.0 * ui, -ur);
+    if (kap)  return col0 ? make_double2(-2.0 * ur, -ui) : im;
+    if (row0) return col0 ? im : make_double2(-2.0 * ur, -ui);
+    return col0 ? make_double2(2.0 * ur, ui) : im;
+}
+
+// Row-side difference form (bie_common.cuh): with d = E_s - E_t,  X = Ei_t dr - Er_t di,  Y = 2 (Er_t dr + Ei_t di) + den, so
+//     (A_t X + B_t Y)/den = (U_t dr + W_t di)/den + B_t,     U_t = A_t Ei_t + 2 B_t Er_t,   W_t = 2 B_t Ei_t - A_t Er_t,
+// row constants per column class; 11 FP64-pipe instructions per entry (13 with the (X, Y) form).
+__device__ __forceinline__ double bie_entry_fast_dagger(const SrcColD& s, const double2 te, const double2 uw, const double bt, int& flag)
 {
     const double dr = s.er - te.x, di = s.ei - te.y;
     const double den = fma(dr, dr, di * di);
-    const double X = fma(te.y, s.ser, -(te.x * s.sei));
-    const double Y = fma(-s.ms, tm, s.sm);
-    const double val = fma(ab.y, Y, ab.x * X);
+    const double num = fma(uw.y, di, uw.x * dr);
     flag |= (__double2hiint(den) < s.thi) ? 1 : 0;
-    return val * bie_rcp3(den);
+    return fma(num, bie_rcp3(den), bt) * s.ms;
 }
 
+template <bool TILED>
 __global__ void __launch_bounds__(BUILD_THREADS)
 bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long lda, int T, int only0, int ncols, int nrows,
                         const double* __restrict__ kappa /* NULL: vortex-sheet S; else the normal-velocity operator */)
 {
-    extern __shared__ __align__(16) double2 sm[];  // [T] E_t, [T] (A,B) for columns on Gamma_0, [T] (A,B) for solids, [T] M_t
+    // [T] E_t, [T] (U,W) for columns on Gamma_0, [T] (U,W) for solids, [T] (B for Gamma_0 columns, B for solids), [T + 256] kappa
+    extern __shared__ __align__(16) double2 sm[];
     const int c0 = blockIdx.x * BUILD_TILE_W;
     const int t0 = blockIdx.y * T;
     const int t1 = min(t0 + T, nrows);   // n; M_0 for the normal-velocity operator (rows on Gamma_0 only); the block's rows
     if (only0 && t0 >= ct.off[1] && c0 >= ct.off[1]) return;
     double2* sE = sm;
-    double2* sAB0 = sm + T;
-    double2* sAB1 = sm + 2 * T;
-    double* sM = reinterpret_cast<double*>(sm + 3 * T);
+    double2* sUW0 = sm + T;
+    double2* sUW1 = sm + 2 * T;
+    double2* sBB = sm + 3 * T;
+    double* sK = reinterpret_cast<double*>(sm + 4 * T);
+    const int M0 = ct.off[1];
     for (int i = threadIdx.x; i < t1 - t0; i += BUILD_THREADS) {
         const int t = t0 + i;
         const int k = nt.COMP[t];
         const double Mk = (double)(ct.off[k + 1] - ct.off[k]);
-        const double2 q = nt.Q[t];
+        const double2 q = nt.Q[t], e = nt.E[t];
         const double ur = q.x * Mk, ui = q.y * Mk;   // zeta'_t / 2
-        sE[i] = nt.E[t];
-        sM[i] = nt.MT[t].x;
-        const double2 im = make_double2(2.0 * ui, -ur);
-        if (kappa)       { sAB0[i] = make_double2(-2.0 * ur, -ui); sAB1[i] = im; }  // -G+_00 (3.24) ; K+_j0 (3.19)
-        else if (k == 0) { sAB0[i] = im; sAB1[i] = make_double2(-2.0 * ur, -ui); }  // K+_00 ; -G+_j0
-        else             { sAB0[i] = make_double2(2.0 * ur, ui); sAB1[i] = im; }     // G+_0k ; K+_jk
+        const double2 ab0 = bie_dagger_ab(kappa != nullptr, k == 0, true, ur, ui);
+        const double2 ab1 = bie_dagger_ab(kappa != nullptr, k == 0, false, ur, ui);
+        sE[i] = e;
+        sUW0[i] = make_double2(fma(ab0.x, e.y, 2.0 * ab0.y * e.x), fma(-ab0.x, e.x, 2.0 * ab0.y * e.y));
+        sUW1[i] = make_double2(fma(ab1.x, e.y, 2.0 * ab1.y * e.x), fma(-ab1.x, e.x, 2.0 * ab1.y * e.y));
+        sBB[i] = make_double2(ab0.y, ab1.y);
     }
+    // the real-cot table of the Gamma_0 - Gamma_0 block of the normal-velocity operator: kappa_{(t - s) mod M_0} for the tile's
+    // differences d = t - s in [t0 - c0 - 255, t1 - 1 - c0]
+    const int dmin = t0 - c0 - (BUILD_TILE_W - 1);
+    if (kappa != nullptr && c0 < M0)
+        for (int i = threadIdx.x; i < (t1 - t0) + BUILD_TILE_W - 1; i += BUILD_THREADS) {
+            int d = (dmin + i) % M0;
+            if (d < 0) d += M0;
+            sK[i] = __ldg(kappa + d);
+        }
     const int s0 = c0 + BUILD_COLS * threadIdx.x;  // < npad by construction
     SrcColD src[BUILD_COLS];
-    const double2* sAB[BUILD_COLS];
-    bool kap[BUILD_COLS];
+    bool col0[BUILD_COLS], kap[BUILD_COLS];
 #pragma unroll
     for (int c = 0; c < BUILD_COLS; ++c) {
         const double2 e = nt.E[s0 + c], mt = nt.MT[s0 + c];
         const int j = nt.COMP[s0 + c];
-        const double ms = (j >= 0) ? 1.0 / (double)(ct.off[j + 1] - ct.off[j]) : 0.0;
+        src[c].ms = (j >= 0) ? 1.0 / (double)(ct.off[j + 1] - ct.off[j]) : 0.0;
         src[c].er = e.x; src[c].ei = e.y;
-        src[c].ser = ms * e.x; src[c].sei = ms * e.y; src[c].sm = ms * mt.x; src[c].ms = ms;
         src[c].thi = __double2hiint(mt.y);
-        sAB[c] = (j == 0) ? sAB0 : sAB1;
+        col0[c] = (j == 0);
         kap[c] = (kappa != nullptr && j == 0);
     }
-    const int M0 = ct.off[1];
-    const bool same_cls = (sAB[0] == sAB[1]);
+    const bool same_cls = (col0[0] == col0[1]);
     __syncthreads();
     const bool full = (s0 + 1 < ncols);
     const bool part = (s0 < ncols);
     const int nchT = (ncols + BIE_TILE_COLS - 1) / BIE_TILE_COLS;   // block format (lda == 0)
+    const double2* sUWa = col0[0] ? sUW0 : sUW1;
+    const double2* sUWb = col0[1] ? sUW0 : sUW1;
     for (int tb = t0; tb < t1; tb += BUILD_RB) {
         int flag = 0;
+        double* row = TILED ? A : A + (long long)tb * lda + s0;
 #pragma unroll
         for (int r = 0; r < BUILD_RB; ++r) {
             const int t = min(tb + r, t1 - 1);  // the tail repeats the last row (same values, same address)
             const double2 te = sE[t - t0];
-            const double tm = sM[t - t0];
-            const double2 ab0 = sAB[0][t - t0];
-            const double2 ab1 = same_cls ? ab0 : sAB[1][t - t0];   // both columns on the same side of M_0, almost always
-            double e0 = bie_entry_fast_dagger(src[0], te, tm, ab0, flag);
-            double e1 = bie_entry_fast_dagger(src[1], te, tm, ab1, flag);
-            if (kap[0]) { const int d = t - s0;     e0 += __ldg(kappa + (d < 0 ? d + M0 : d)); }
-            if (kap[1]) { const int d = t - s0 - 1; e1 += __ldg(kappa + (d < 0 ? d + M0 : d)); }
-            double* p = A + bie_entry_off(lda, nchT, t, s0);
+            const double2 bb = sBB[t - t0];
+            const double2 uwa = sUWa[t - t0];
+            const double2 uwb = same_cls ? uwa : sUWb[t - t0];   // both columns on the same side of M_0, almost always
+            double e0 = bie_entry_fast_dagger(src[0], te, uwa, col0[0] ? bb.x : bb.y, flag);
+            double e1 = bie_entry_fast_dagger(src[1], te, uwb, col0[1] ? bb.x : bb.y, flag);
+            if (kap[0]) e0 += sK[t - s0 - dmin];
+            if (kap[1]) e1 += sK[t - s0 - 1 - dmin];
+            double* p = TILED ? A + bie_entry_off(0, nchT, t, s0) : row + (long long)(t - tb) * lda;
             if (full) *reinterpret_cast<double2*>(p) = make_double2(e0, e1);
             else if (part) p[0] = e0;
         }
@@ -238,11 +269,14 @@ bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long
                         const double dr = src[c].er - te.x, di = src[c].ei - te.y;
                         const double den = fma(dr, dr, di * di);
                         if (__double2hiint(den) < src[c].thi) {
-                            const double2 ab = sAB[c][t - t0];
+                            const int k = nt.COMP[t];
+                            const double Mk = (double)(ct.off[k + 1] - ct.off[k]);
+                            const double2 q = nt.Q[t];
+                            const double2 ab = bie_dagger_ab(kappa != nullptr, k == 0, col0[c], q.x * Mk, q.y * Mk);
                             // (A X' + B Y')/den with cot = (-2X + iY)/den; the diagonal entry is prepared per node
                             double v = bie_entry_near(nt.DG, nt.XY, src[c].ms * ab.x, src[c].ms * ab.y, 0.0, s0 + c, t);
-                            if (kap[c]) { const int d = t - s0 - c; v += __ldg(kappa + (d < 0 ? d + M0 : d)); }
-                            A[bie_entry_off(lda, nchT, t, s0 + c)] = v;
+                            if (kap[c]) v += sK[t - s0 - c - dmin];
+                            A[bie_entry_off(TILED ? 0 : lda, nchT, t, s0 + c)] = v;
                         }
                     }
                 }
@@ -273,8 +307,8 @@ int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int ncols, int nrows,
     // of the default (8192 CTAs = 11.07 waves of 740 at n = 16384) cost 16 % (profiles/r01b_ncu_full_cfg5.md)
     {
         int occ = 0;
-        if (dagger) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bie_build_dagger_kernel, BUILD_THREADS, 7 * 8 * 256 + 16);
-        else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bie_build_kernel, BUILD_THREADS, 2 * 8 * 256 + 16);
+        if (dagger) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bie_build_dagger_kernel<false>, BUILD_THREADS, 64 * 256 + 8 * 512 + 16);
+        else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bie_build_kernel<false>, BUILD_THREADS, 2 * 8 * 256 + 16);
         const long long wave = (long long)ctx->sm_count * (occ > 0 ? occ : 1);
         if ((long long)gx * ((nt_rows + 127) / 128) >= 2 * wave) {
             double best = 0.0;
@@ -286,15 +320,17 @@ int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int ncols, int nrows,
         }
     }
     dim3 grid(gx, (nt_rows + T - 1) / T);
+    const bool tiled = (lda == 0);
+    const double* kap = ctx->variant == BIE_VARIANT_NORMAL_INTERNAL ? ctx->kappa : nullptr;
     if (dagger) {
-        bie_build_dagger_kernel<<<grid, BUILD_THREADS, (3 * sizeof(double2) + sizeof(double)) * T + 16, st>>>(
-            nt, ctx->comps, A, (long long)lda, T, only_comp0, ncols, nt_rows,
-            ctx->variant == BIE_VARIANT_NORMAL_INTERNAL ? ctx->kappa : nullptr);
-        BIE_CUDA(cudaGetLastError());
-        return BIE_OK;
+        const size_t sm = 4 * sizeof(double2) * T + (kap ? sizeof(double) * (T + BUILD_TILE_W) : 0) + 16;
+        if (tiled) bie_build_dagger_kernel<true><<<grid, BUILD_THREADS, sm, st>>>(nt, ctx->comps, A, 0, T, only_comp0, ncols, nt_rows, kap);
+        else bie_build_dagger_kernel<false><<<grid, BUILD_THREADS, sm, st>>>(nt, ctx->comps, A, (long long)lda, T, only_comp0, ncols, nt_rows, kap);
+    } else {
+        const size_t sm = sizeof(double2) * T + 16;
+        if (tiled) bie_build_kernel<true><<<grid, BUILD_THREADS, sm, st>>>(nt, ctx->comps, A, 0, T, only_comp0, ncols, nt_rows);
+        else bie_build_kernel<false><<<grid, BUILD_THREADS, sm, st>>>(nt, ctx->comps, A, (long long)lda, T, only_comp0, ncols, nt_rows);
     }
-    bie_build_kernel<<<grid, BUILD_THREADS, sizeof(double2) * T + 16, st>>>(nt, ctx->comps, A, (long long)lda, T,
-                                                                             only_comp0, ncols, nt_rows);
     BIE_CUDA(cudaGetLastError());
     return BIE_OK;
 }

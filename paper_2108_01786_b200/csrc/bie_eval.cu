@@ -4,10 +4,14 @@
 // sigma_0 = -1 on Gamma_0 (fluid on its right; reading R18), +1 on the solids.  "If z coincides with
 // zeta_k(alpha_m), we set f(z) = f(zeta_k(alpha_m))".
 //
-// Second workload of the same pair arithmetic (bie_common.cuh): one thread per evaluation point, the sources staged tile by
-// tile in shared memory with their factors E_s = e^{i zeta_s}, M_s, q_s = sigma zeta'_s/(2 M_s) and g_s = q_s f_s (per
-// function), so that per pair  cot = (-2X + iY)/den  costs 12 FP64 instructions and each of the 1 + nf complex sums
-// (denominator and numerators) 4 more.  Pairs closer than the near threshold are recomputed from the coordinate differences
+// Second workload of the same pair arithmetic (bie_common.cuh), in its difference form: with d = E_s - E_z = dr + i di,
+//     q_s cot((zeta_s - z)/2) = (A_s dr + B_s di)/den - i q_s,     A_s = 2 i q_s E_s,  B_s = 2 q_s E_s = -i A_s,
+// so with u = dr/den, v = di/den every complex sum (the denominator and the nf numerators, whose source constant is A_s f_s)
+// costs 4 FMAs per pair:  Re += Ar u + Ai v,  Im += Ai u - Ar v;  the constants -i sum_s q_s (f_s) are added per source tile by
+// one thread.  Per pair: 2 sub, 2 den, 3 reciprocal, 2 for (u, v), 4 per sum = 9 + 4 (1 + nf) FP64 instructions (12 + 4 (1 + nf)
+// with the (X, Y) form of round 1).  Two evaluation points per thread share every shared-memory load.
+// One thread per two evaluation points, the sources staged tile by tile in shared memory with E_s, the near threshold and
+// A_s, A_s f_s.  Pairs closer than the near threshold are recomputed from the coordinate differences
 // with the Laurent series (exact to rounding at any distance, which is the whole point of (F.4)); an exact coincidence
 // is recorded and resolved in the second kernel, which also adds the partial sums of the source segments (few points:
 // the sources are split over blockIdx.y so that the GPU is filled) and divides.
@@ -23,32 +27,45 @@ struct EvalComps {
     int surface[BIE_MAX_COMP];   // 1: sigma = -1
 };
 
+#ifndef EVAL_NP
+#define EVAL_NP 2      // evaluation points per thread
+#endif
+
 template <int NF>
 __global__ void __launch_bounds__(EVAL_THREADS)
 bie_cauchy_eval_kernel(EvalComps ec, int n, const double2* __restrict__ zeta, const double2* __restrict__ dzeta,
                        const double2* __restrict__ f, int npts, const double2* __restrict__ zpts, int nseg,
                        double2* __restrict__ part /* [nseg][1+NF][npts] */, int* __restrict__ hit /* [npts] */)
 {
-    __shared__ double2 sE[EVAL_TILE], sMT[EVAL_TILE], sQ[EVAL_TILE], sXY[EVAL_TILE];
+    __shared__ double2 sE[EVAL_TILE], sA[EVAL_TILE], sQ[EVAL_TILE], sXY[EVAL_TILE];
     __shared__ double2 sG[NF][EVAL_TILE];
-    const int p = blockIdx.x * EVAL_THREADS + threadIdx.x;
+    __shared__ int sTH[EVAL_TILE];
+    __shared__ double2 sred[EVAL_THREADS / 32][1 + NF];
     const int seg = blockIdx.y;
     const int per = (((n + nseg - 1) / nseg) + 1) & ~1;
     const int s_lo = seg * per, s_hi = min(s_lo + per, n);
     const double yref = zeta[0].y;
-    // this thread's point
-    const double2 z = zpts[min(p, npts - 1)];
-    double ter, tei, tm;
-    {
-        double s, c;
-        sincos(z.x, &s, &c);
-        const double m = exp(-(z.y - yref));
-        ter = m * c; tei = m * s; tm = m * m;
-    }
-    double Dr = 0.0, Di = 0.0, Nr[NF], Ni[NF];
+    // this thread's points: p0 + k EVAL_THREADS (consecutive threads, consecutive points)
+    const int p0 = blockIdx.x * (EVAL_THREADS * EVAL_NP) + threadIdx.x;
+    double2 z[EVAL_NP];
+    double ter[EVAL_NP], tei[EVAL_NP];
+    double Dr[EVAL_NP], Di[EVAL_NP], Nr[EVAL_NP][NF], Ni[EVAL_NP][NF];
+    int myhit[EVAL_NP];
 #pragma unroll
-    for (int q = 0; q < NF; ++q) { Nr[q] = 0.0; Ni[q] = 0.0; }
-    int myhit = -1;
+    for (int k = 0; k < EVAL_NP; ++k) {
+        z[k] = zpts[min(p0 + k * EVAL_THREADS, npts - 1)];
+        double s, c;
+        sincos(z[k].x, &s, &c);
+        const double m = exp(-(z[k].y - yref));
+        ter[k] = m * c; tei[k] = m * s;
+        Dr[k] = 0.0; Di[k] = 0.0; myhit[k] = -1;
+#pragma unroll
+        for (int q = 0; q < NF; ++q) { Nr[k][q] = 0.0; Ni[k][q] = 0.0; }
+    }
+    // sum_s q_s and sum_s q_s f_s over the segment (the constant -i q_s of the difference form), this thread's share
+    double2 cs[1 + NF];
+#pragma unroll
+    for (int c = 0; c <= NF; ++c) cs[c] = make_double2(0.0, 0.0);
     for (int s0 = s_lo; s0 < s_hi; s0 += EVAL_TILE) {
         __syncthreads();
         for (int i = threadIdx.x; i < EVAL_TILE; i += EVAL_THREADS) {
@@ -59,24 +76,31 @@ bie_cauchy_eval_kernel(EvalComps ec, int n, const double2* __restrict__ zeta, co
                 const double M = (double)(ec.off[k + 1] - ec.off[k]);
                 const double wgt = (ec.surface[k] ? -0.5 : 0.5) / M;
                 const double2 zs = zeta[s], dz = dzeta[s];
-                double sn, cs;
-                sincos(zs.x, &sn, &cs);
+                double sn, cn;
+                sincos(zs.x, &sn, &cn);
                 const double m = exp(-(zs.y - yref));
                 const double2 q = make_double2(wgt * dz.x, wgt * dz.y);
                 double tau = BIE_NEAR_C * sqrt(q.x * q.x + q.y * q.y);
                 tau = fmin(fmax(tau, BIE_NEAR_TAU_MIN), BIE_NEAR_TAU_MAX);
-                sE[i] = make_double2(m * cs, m * sn);
-                sMT[i] = make_double2(m * m, tau * m * m);
+                const double er = m * cn, ei = m * sn;
+                // A_s = 2 i q_s E_s
+                const double qer = q.x * er - q.y * ei, qei = q.x * ei + q.y * er;     // q E
+                const double2 A = make_double2(-2.0 * qei, 2.0 * qer);
+                sE[i] = make_double2(er, ei);
+                sTH[i] = __double2hiint(tau * m * m);
+                sA[i] = A;
                 sQ[i] = q;
                 sXY[i] = zs;
+                cs[0].x += q.x; cs[0].y += q.y;
 #pragma unroll
                 for (int c = 0; c < NF; ++c) {
                     const double2 fv = f[(size_t)c * n + s];
-                    sG[c][i] = make_double2(q.x * fv.x - q.y * fv.y, q.x * fv.y + q.y * fv.x);
+                    sG[c][i] = make_double2(A.x * fv.x - A.y * fv.y, A.x * fv.y + A.y * fv.x);   // A_s f_s
+                    cs[1 + c].x += q.x * fv.x - q.y * fv.y; cs[1 + c].y += q.x * fv.y + q.y * fv.x;
                 }
             } else {   // beyond the segment: zero weight, never near
-                sE[i] = make_double2(0.0, 0.0); sMT[i] = make_double2(0.0, 0.0); sQ[i] = make_double2(0.0, 0.0);
-                sXY[i] = make_double2(0.0, 1.0e3);
+                sE[i] = make_double2(0.0, 0.0); sA[i] = make_double2(0.0, 0.0); sQ[i] = make_double2(0.0, 0.0);
+                sXY[i] = make_double2(0.0, 1.0e3); sTH[i] = 0;
 #pragma unroll
                 for (int c = 0; c < NF; ++c) sG[c][i] = make_double2(0.0, 0.0);
             }
@@ -84,38 +108,71 @@ bie_cauchy_eval_kernel(EvalComps ec, int n, const double2* __restrict__ zeta, co
         __syncthreads();
 #pragma unroll 2
         for (int j = 0; j < EVAL_TILE; ++j) {
-            const double2 e = sE[j], mt = sMT[j];
-            const double dr = e.x - ter, di = e.y - tei;
-            const double den = fma(dr, dr, di * di);
-            const double X = fma(tei, e.x, -(ter * e.y));
-            const double Y = mt.x - tm;
-            const double r = bie_rcp3(den);
-            double cr = -2.0 * X * r, ci = Y * r;            // cot((zeta_s - z)/2) = (-2X + iY)/den
-            if (den < mt.y) {                                  // near pair (rare): from the coordinate differences
-                const double2 zs = sXY[j];
-                const double x = zs.x - z.x, y = zs.y - z.y;
-                // exact coincidence (modulo the period): cot has a pole, (F.4) degenerates to f_s
-                const double xr = x - 6.283185307179586232 * rint(x * 0.15915494309189534561);
-                if (xr == 0.0 && y == 0.0) { myhit = s0 + j; cr = 0.0; ci = 0.0; }
-                else bie_cot_half_near(x, y, &cr, &ci);
-            }
-            const double2 q = sQ[j];
-            Dr = fma(q.x, cr, Dr); Dr = fma(-q.y, ci, Dr);
-            Di = fma(q.x, ci, Di); Di = fma(q.y, cr, Di);
+            const double2 e = sE[j], A = sA[j];
+            const int th = sTH[j];
 #pragma unroll
-            for (int c = 0; c < NF; ++c) {
-                const double2 g = sG[c][j];
-                Nr[c] = fma(g.x, cr, Nr[c]); Nr[c] = fma(-g.y, ci, Nr[c]);
-                Ni[c] = fma(g.x, ci, Ni[c]); Ni[c] = fma(g.y, cr, Ni[c]);
+            for (int k = 0; k < EVAL_NP; ++k) {
+                const double dr = e.x - ter[k], di = e.y - tei[k];
+                const double den = fma(dr, dr, di * di);
+                const double r = bie_rcp3(den);
+                double u = dr * r, v = di * r;
+                if (__double2hiint(den) < th) {                // near pair (rare): from the coordinate differences
+                    const double2 zs = sXY[j], q = sQ[j];
+                    const double x = zs.x - z[k].x, y = zs.y - z[k].y;
+                    u = 0.0; v = 0.0;
+                    // exact coincidence (modulo the period): cot has a pole, (F.4) degenerates to f_s
+                    const double xr = x - 6.283185307179586232 * rint(x * 0.15915494309189534561);
+                    if (xr == 0.0 && y == 0.0) myhit[k] = s0 + j;
+                    else {
+                        double cr, ci;
+                        bie_cot_half_near(x, y, &cr, &ci);
+                        ci += 1.0;                             // + i q_s: the constant below is subtracted for EVERY source
+                        const double wr = q.x * cr - q.y * ci, wi = q.x * ci + q.y * cr;
+                        Dr[k] += wr; Di[k] += wi;
+#pragma unroll
+                        for (int c = 0; c < NF; ++c) {
+                            const double2 fv = f[(size_t)c * n + s0 + j];
+                            Nr[k][c] += wr * fv.x - wi * fv.y; Ni[k][c] += wr * fv.y + wi * fv.x;
+                        }
+                    }
+                }
+                Dr[k] = fma(A.x, u, Dr[k]); Dr[k] = fma(A.y, v, Dr[k]);
+                Di[k] = fma(A.y, u, Di[k]); Di[k] = fma(-A.x, v, Di[k]);
+#pragma unroll
+                for (int c = 0; c < NF; ++c) {
+                    const double2 g = sG[c][j];
+                    Nr[k][c] = fma(g.x, u, Nr[k][c]); Nr[k][c] = fma(g.y, v, Nr[k][c]);
+                    Ni[k][c] = fma(g.y, u, Ni[k][c]); Ni[k][c] = fma(-g.x, v, Ni[k][c]);
+                }
             }
         }
     }
-    if (p < npts) {
-        double2* o = part + (size_t)seg * (1 + NF) * npts;
-        o[p] = make_double2(Dr, Di);
+    // the constants: fixed-order sum over the CTA (lanes by shuffle, warps in order), then -i sum
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
-        for (int c = 0; c < NF; ++c) o[(size_t)(1 + c) * npts + p] = make_double2(Nr[c], Ni[c]);
-        if (myhit >= 0) atomicMax(hit + p, myhit);
+    for (int c = 0; c <= NF; ++c) { cs[c].x = bie_warp_sum(cs[c].x); cs[c].y = bie_warp_sum(cs[c].y); }
+    __syncthreads();
+    if (lane == 0) {
+#pragma unroll
+        for (int c = 0; c <= NF; ++c) sred[warp][c] = cs[c];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int c = 0; c <= NF; ++c) {
+        double sx = 0.0, sy = 0.0;
+        for (int w = 0; w < EVAL_THREADS / 32; ++w) { sx += sred[w][c].x; sy += sred[w][c].y; }
+        cs[c] = make_double2(sx, sy);
+    }
+#pragma unroll
+    for (int k = 0; k < EVAL_NP; ++k) {
+        const int p = p0 + k * EVAL_THREADS;
+        if (p < npts) {
+            double2* o = part + (size_t)seg * (1 + NF) * npts;
+            o[p] = make_double2(Dr[k] + cs[0].y, Di[k] - cs[0].x);        // - i (sx + i sy) = sy - i sx
+#pragma unroll
+            for (int c = 0; c < NF; ++c) o[(size_t)(1 + c) * npts + p] = make_double2(Nr[k][c] + cs[1 + c].y, Ni[k][c] - cs[1 + c].x);
+            if (myhit[k] >= 0) atomicMax(hit + p, myhit[k]);
+        }
     }
 }
 
@@ -147,7 +204,7 @@ bie_cauchy_finish_kernel(int nf, int n, int npts, int nseg, const double2* __res
 size_t bie_cauchy_eval_ws_bytes(int nf, int npts, int sm_count)
 {
     if (nf < 1 || nf > EVAL_MAX_NF || npts < 1) return 0;
-    const int gx = (npts + EVAL_THREADS - 1) / EVAL_THREADS;
+    const int gx = (npts + EVAL_THREADS * EVAL_NP - 1) / (EVAL_THREADS * EVAL_NP);
     int nseg = (4 * sm_count + gx - 1) / gx;
     if (nseg < 1) nseg = 1;
     if (nseg > 64) nseg = 64;
@@ -172,7 +229,7 @@ int bie_launch_cauchy_eval(bie_ctx* ctx, int ncomp, const int32_t* counts, const
     if (n > (1 << 30)) return BIE_ERR_GEOMETRY;
     if ((((uintptr_t)zeta) | ((uintptr_t)dzeta) | ((uintptr_t)fvals) | ((uintptr_t)zpts) | ((uintptr_t)out)) & 15u) return BIE_ERR_LAYOUT;
     if (bie_cauchy_eval_ws_bytes(nf, npts, ctx->sm_count) > ws_bytes) return BIE_ERR_WORKSPACE;
-    const int gx = (npts + EVAL_THREADS - 1) / EVAL_THREADS;
+    const int gx = (npts + EVAL_THREADS * EVAL_NP - 1) / (EVAL_THREADS * EVAL_NP);
     int nseg = (4 * ctx->sm_count + gx - 1) / gx;
     if (nseg < 1) nseg = 1;
     if (nseg > 64) nseg = 64;
