@@ -164,6 +164,66 @@ __device__ __forceinline__ void free_write_tables(const NodeTable& nt, const Com
     }
 }
 
+// The same with the per-source constants of this CTA's rows kept in shared memory for the whole solve (bie_gmres.cu): the
+// tables are x_s times a constant of the geometry, so an application costs no global load besides x itself.
+// K: shared, [3][rows2] double2: the (U, W) coefficients of class 0, of class 1, and (beta_0, beta_1)
+//    (vortex-sheet matrix: (Er, Ei)/M_j, (M, 1)/M_j, unused).
+__device__ __forceinline__ void free_init_row_consts(const NodeTable& nt, const CompTable& ct, const FreePlan& fp, int r0, int r1,
+                                                     double2* K, int rows2)
+{
+    for (int s = r0 + threadIdx.x; s < r1; s += blockDim.x) {
+        const double2 e = nt.E[s], q = nt.Q[s];
+        const int l = s - r0;
+        if (fp.vortex) {
+            const double M = nt.MT[s].x;
+            const int j = nt.COMP[s];
+            const double m = 1.0 / (double)(ct.off[j + 1] - ct.off[j]);
+            K[l] = make_double2(m * e.x, m * e.y);
+            K[rows2 + l] = make_double2(m * M, m);
+            K[2 * rows2 + l] = make_double2(0.0, 0.0);
+            continue;
+        }
+        const bool src0 = (nt.COMP[s] == 0);
+        double a0, b0, a1, b1;
+        if (src0) { a0 = -2.0 * q.y; b0 = q.x;  a1 = 2.0 * q.x;  b1 = q.y; }   // K_00 ; -G_k0
+        else      { a0 = -2.0 * q.x; b0 = -q.y; a1 = -2.0 * q.y; b1 = q.x; }   // G_0j ; K_kj
+        K[l] = make_double2(fma(a0, e.y, 2.0 * b0 * e.x), fma(-a0, e.x, 2.0 * b0 * e.y));
+        K[rows2 + l] = make_double2(fma(a1, e.y, 2.0 * b1 * e.x), fma(-a1, e.x, 2.0 * b1 * e.y));
+        K[2 * rows2 + l] = make_double2(b0, b1);
+    }
+    __syncthreads();
+}
+
+__device__ __forceinline__ void free_write_tables_cached(const FreePlan& fp, int np, int r0, int r1, const double* v, const double2* K,
+                                                         int rows2, double* red)
+{
+    double sb[4] = {0.0, 0.0, 0.0, 0.0};
+    for (int s = r0 + threadIdx.x; s < r1; s += blockDim.x) {
+        const int l = s - r0;
+        const double x = v[l];
+        const double2 k0 = K[l], k1 = K[rows2 + l], bb = K[2 * rows2 + l];
+        fp.T[s]      = make_double2(x * k0.x, x * k0.y);
+        fp.T[np + s] = make_double2(x * k1.x, x * k1.y);
+        if (s >= fp.s_off) { sb[0] = fma(x, bb.x, sb[0]); sb[1] = fma(x, bb.y, sb[1]); }
+        else               { sb[2] = fma(x, bb.x, sb[2]); sb[3] = fma(x, bb.y, sb[3]); }
+    }
+    if (fp.vortex) return;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) sb[q] = bie_warp_sum(sb[q]);
+    __syncthreads();
+    if (lane == 0) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) red[32 * q + warp] = sb[q];
+    }
+    __syncthreads();
+    if (threadIdx.x < 4) {
+        double t = 0.0;
+        for (int w = 0; w < nwarp; ++w) t += red[32 * threadIdx.x + w];
+        fp.SB[threadIdx.x * FREE_SB_LD + blockIdx.x] = t;
+    }
+}
+
 // ---- step 2: this CTA's slab of the (row block x source) list -> partial sums in fp.PB --------------------
 // scratch: shared, free_scratch_doubles() doubles, 16-byte aligned.  All threads of the team must call.
 // poll() is called by every warp after each chunk of 32 sources (the hybrid operator consumes tiles of its stored
@@ -352,7 +412,7 @@ __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable
     __syncthreads();
     // symmetric work split: row t of block J also receives sum_{I < J} PC[I][t] (rows below s_off: nothing, their mirror
     // entries are stored).  These are up to NB - 1 loads per row, each from another L2 line: four threads share a row
-    // (I = q, q + 4, ...; eight loads in flight each) and the four partial sums are added in fixed order.  rsum lives in
+    // (I = q, q + 4, ...; sixteen loads in flight each) and the four partial sums are added in fixed order.  rsum lives in
     // the staging area (free again; fp.sym => the full scratch).
     double* rsum = scratch + FREE_HEAD_DOUBLES;   // [rows]
     if (fp.sym) {
@@ -365,6 +425,13 @@ __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable
             const double* pc = fp.PC + t;
             double a0 = 0.0, a1 = 0.0;
             int I = q;
+            for (; I + 60 < b; I += 64) {                  // sixteen loads in flight
+                double v[16];
+#pragma unroll
+                for (int k = 0; k < 16; ++k) v[k] = __ldcg(pc + (size_t)(I + 4 * k) * nt.npad);
+#pragma unroll
+                for (int k = 0; k < 16; k += 2) { a0 += v[k]; a1 += v[k + 1]; }
+            }
             for (; I + 28 < b; I += 32) {
                 double v[8];
 #pragma unroll

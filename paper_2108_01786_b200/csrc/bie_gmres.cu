@@ -304,11 +304,13 @@ __device__ __forceinline__ int hess_off(int i) { return (i * (i + 3)) >> 1; }
 
 // doubles of shared memory before the operator's scratch: y, w [rows2 each], hcol, hloc, cvec [m + 2 each], cs, sn [m each],
 // g [m + 1], red [130], the packed single-precision Hbar [m (m + 3) / 2 floats]; rounded to 16 bytes
-__host__ __device__ inline int gm_head_doubles(int m, int rows2)
+// + (matrix-free and hybrid operators) the per-source constants of this CTA's rows, [3][rows2] double2
+__host__ __device__ inline int gm_head_doubles(int m, int rows2, bool free_op)
 {
     int o = 2 * rows2 + 3 * (m + 2) + 2 * m + (m + 1) + 130;
     o += (m * (m + 3) / 2 + 1) / 2;
-    return (o + 1) & ~1;
+    o = (o + 1) & ~1;
+    return o + (free_op ? 6 * rows2 : 0);
 }
 
 template <bool STREAM, bool XS, int MODE>
@@ -333,7 +335,8 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
     double* g = sn + m;                   // [m+1]
     double* red = g + (m + 1);            // [130]
     float* Hf = reinterpret_cast<float*>(red + 130);                 // packed Hbar in single precision, m (m + 3) / 2 floats
-    double* gpart = smem + gm_head_doubles(m, rows2);                // GEMV partials or matrix-free scratch (16-byte aligned)
+    double* gpart = smem + gm_head_doubles(m, rows2, FREE);          // GEMV partials or matrix-free scratch (16-byte aligned)
+    double2* Kc = reinterpret_cast<double2*>(gpart) - 3 * rows2;     // FREE: per-source constants of this CTA's rows
     // dense: GEMV partials, then x; matrix-free: the operator's scratch; hybrid: scratch, row sums of the ring's tiles, the ring
     double* ring_part = gpart + (FREE ? a.scratch_doubles : 0);
     double* ring_mem = ring_part + ((MODE == 2) ? ring_part_doubles(a.brows, a.nd, a.chunk) : 0);
@@ -358,6 +361,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
     Basis B;
     B.Vs = red2 + GM_THREADS + rows2;                          // [VS][rows2]
     B.Vg = a.V + r0; B.VS = a.VS; B.rows2 = rows2; B.nld = a.nld;
+    if (FREE) free_init_row_consts(a.nt, a.ct, a.fp, r0, r1, Kc, rows2);
     double* part1 = a.part;
     double* part2 = a.part + (size_t)(m + 2) * G;
     double* part3 = a.part + 2 * (size_t)(m + 2) * G;
@@ -396,7 +400,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
             p = fma(v, v, p);
             a.wbuf[r0 + r] = v;
         }
-        if (FREE) free_write_tables(a.nt, a.ct, a.fp, r0, r1, w_local, red);
+        if (FREE) free_write_tables_cached(a.fp, a.nt.npad, r0, r1, w_local, Kc, rows2, red);
         p = block_sum(p, red);
         if (threadIdx.x == 0) part3[blockIdx.x] = p;
         grid_barrier(a.sync, target);
@@ -434,7 +438,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
                 a.wbuf[r0 + r] = v;                       // the next operator application reads w1 (see the header)
             }
             __syncthreads();
-            if (FREE) free_write_tables(a.nt, a.ct, a.fp, r0, r1, w_local, red);
+            if (FREE) free_write_tables_cached(a.fp, a.nt.npad, r0, r1, w_local, Kc, rows2, red);
             // second pass: h2 = V_j^T w1 and ||w1||^2 in ONE reduction (grid barrier 2)
             local_dots(B, rows, j + 1, w_local, part2, true);
             PT(2)
@@ -465,7 +469,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
                     a.wbuf[r0 + r] = v;
                 }
                 __syncthreads();
-                if (FREE) free_write_tables(a.nt, a.ct, a.fp, r0, r1, w_local, red);
+                if (FREE) free_write_tables_cached(a.fp, a.nt.npad, r0, r1, w_local, Kc, rows2, red);
                 p = block_sum(p, red);
                 if (threadIdx.x == 0) part3[blockIdx.x] = p;
                 grid_barrier(a.sync, target);
@@ -636,7 +640,7 @@ static int gmres_plan(int n, int restart, int sm_count, int max_smem, int l2_byt
     }
     pl->scratch_doubles = free_op ? free_scratch_doubles(vortex, sym) : 0;
     const int rows2 = (pl->rows_per_cta + 1) & ~1;
-    size_t base = (size_t)gm_head_doubles(m, rows2);
+    size_t base = (size_t)gm_head_doubles(m, rows2, free_op);
     if (free_op) base += (size_t)pl->scratch_doubles;
     if (mode == 0) base += (size_t)((gemv_part_doubles(pl->rows_per_cta, n, pl->chunk) + 1) & ~1);
     if (mode == 2) base += (size_t)ring_part_doubles(pl->brows, nd, pl->chunk) + (size_t)ring_doubles(pl->chunk);
