@@ -60,7 +60,8 @@ struct FreePlan {
     int s_off;       // hybrid operator: the leading s_off x s_off block comes from the caller's stored block (0: none)
     int stage_buf;   // doubles of one staging buffer of a warp (free_stage_buf_doubles): fixes the shared-memory strides
     double2* T;      // [2][npad]: (U,W) class 0, (U,W) class 1     (vortex: (P,Q) = mu E, (R,B) = mu (M, 1))
-    double* SB;      // [4][FREE_SB_LD] per-CTA partials of sum_s beta_s x_s: class 0 / 1 over s >= s_off, class 0 / 1 over s < s_off
+    double* SB;      // [2][4][FREE_SB_LD] per-CTA partials of sum_s beta_s x_s: class 0 / 1 over s >= s_off, class 0 / 1 over s < s_off;
+                     // two copies (sb_sel): an application may write its constants while other CTAs still gather the previous one's
     double* PB;      // [(NB + Geff)][FREE_ROWS] partial sums, part id = list position of the row block + CTA
     const double* taubar;     // device scalar: near threshold relative to M_t (bie_near.cu)
     const int* near_ptr;      // CSR near matrix: offsets of the (row, segment) lists, row t = [ptr[8t], ptr[8t+8])
@@ -121,7 +122,7 @@ __device__ __forceinline__ int free_list_block(const FreePlan& fp, long long u)
 // Also leaves this CTA's shares of sum_s beta_s x_s (per class; s >= s_off and s < s_off) in fp.SB.
 // red: shared, >= 128 doubles.  All threads of the CTA must call; no barrier at the end (the caller's next barrier orders `red`).
 __device__ __forceinline__ void free_write_tables(const NodeTable& nt, const CompTable& ct, const FreePlan& fp, int r0,
-                                                  int r1, const double* v /* shared or global, v[s - r0] */, double* red)
+                                                  int r1, const double* v /* shared or global, v[s - r0] */, double* red, int sb_sel = 0)
 {
     const int np = nt.npad;
     double sb[4] = {0.0, 0.0, 0.0, 0.0};
@@ -160,7 +161,7 @@ __device__ __forceinline__ void free_write_tables(const NodeTable& nt, const Com
     if (threadIdx.x < 4) {
         double t = 0.0;
         for (int w = 0; w < nwarp; ++w) t += red[32 * threadIdx.x + w];
-        fp.SB[threadIdx.x * FREE_SB_LD + blockIdx.x] = t;
+        fp.SB[(4 * sb_sel + threadIdx.x) * FREE_SB_LD + blockIdx.x] = t;
     }
 }
 
@@ -195,7 +196,7 @@ __device__ __forceinline__ void free_init_row_consts(const NodeTable& nt, const 
 }
 
 __device__ __forceinline__ void free_write_tables_cached(const FreePlan& fp, int np, int r0, int r1, const double* v, const double2* K,
-                                                         int rows2, double* red)
+                                                         int rows2, double* red, int sb_sel = 0)
 {
     double sb[4] = {0.0, 0.0, 0.0, 0.0};
     for (int s = r0 + threadIdx.x; s < r1; s += blockDim.x) {
@@ -220,7 +221,7 @@ __device__ __forceinline__ void free_write_tables_cached(const FreePlan& fp, int
     if (threadIdx.x < 4) {
         double t = 0.0;
         for (int w = 0; w < nwarp; ++w) t += red[32 * threadIdx.x + w];
-        fp.SB[threadIdx.x * FREE_SB_LD + blockIdx.x] = t;
+        fp.SB[(4 * sb_sel + threadIdx.x) * FREE_SB_LD + blockIdx.x] = t;
     }
 }
 
@@ -372,7 +373,7 @@ __device__ __forceinline__ void free_parts(const NodeTable& nt, const CompTable&
 // xsrc: the vector of step 1 (global, complete).  All threads of the CTA must call; ends with __syncthreads.
 __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable& ct, const FreePlan& fp, int r0, int r1,
                                             const double* __restrict__ xsrc, double scale, double* scratch,
-                                            double* y_local)
+                                            double* y_local, int sb_sel = 0)
 {
     double* csum = scratch + FREE_WARPS * FREE_ROWS;  // [2][BIE_MAX_COMP]: component sums over s >= s_off, over all s
     double* sbs = csum + 2 * BIE_MAX_COMP;            // [4] constants (free_write_tables)
@@ -401,31 +402,54 @@ __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable
             __syncthreads();
         }
     }
-    // sum_s beta_s x_s per class and source range: the per-CTA partials of free_write_tables in fixed order (warps 0..3)
-    if (!fp.vortex && threadIdx.x < 128) {
-        const int q = threadIdx.x >> 5, lane = threadIdx.x & 31;
-        double sb = 0.0;
-        for (int i = lane; i < (int)gridDim.x; i += 32) sb += __ldcg(fp.SB + q * FREE_SB_LD + i);
-        sb = bie_warp_sum(sb);
-        if (lane == 0) sbs[q] = sb;
+    // Everything below is a handful of dependent L2 round trips (about 0.7 us each).  The loads of the independent chains are
+    // ISSUED first and consumed later, so that the chains overlap instead of queueing behind one another:
+    //   A: CSR range of the CTA's rows -> near columns and values -> x at those columns        (3 round trips)
+    //   B: reverse partials of the symmetric loops                                               (1-2)
+    //   C: per-CTA partials of the constants sum beta x                                          (1)
+    //   D: forward partials of the row                                                           (1)
+    const int rows_ = r1 - r0, rows2_ = (rows_ + 1) & ~1;
+    double* rpart = scratch + FREE_HEAD_DOUBLES;             // [4][rows2_] quarter sums of the reverse partials (staging area: free again)
+    double* prod = rpart + 4 * rows2_;                        // products of the near entries with x
+    const int prod_cap = FREE_WARPS * 2 * fp.stage_buf - 4 * rows2_;
+    // A1
+    const int pbeg = fp.near_ptr[8 * (size_t)r0], pend = fp.near_ptr[8 * (size_t)r1];
+    // D (the thread's first row; a thread has more than one row only when n > 512 SMs' worth)
+    const bool rowt = (int)threadIdx.x < rows_;
+    int r_kpos = 0, r_off = 0, r_clo = 0, r_chi = -1;
+    long long r_X0 = 0, r_X1 = 0;
+    double pbv[4] = {0.0, 0.0, 0.0, 0.0};
+    if (rowt) {
+        const int t = r0 + threadIdx.x;
+        int b;
+        if (t < fp.M0) { b = t / FREE_ROWS; r_off = t - b * FREE_ROWS; }
+        else { const int d = t - fp.M0; b = d / FREE_ROWS; r_off = d - b * FREE_ROWS; b += fp.NB0; }
+        r_kpos = fp.sym ? __ldg(fp.sym_pos + b) : b;   // position of the block in the work list
+        r_X0 = fp.sym ? __ldg(fp.sym_cum + r_kpos) : free_list_start(fp, b);
+        r_X1 = fp.sym ? __ldg(fp.sym_cum + r_kpos + 1) : free_list_start(fp, b + 1);
+        r_clo = max((int)(((r_X0 + 1) * fp.Geff + fp.U - 1) / fp.U) - 1, 0);
+        r_chi = min((int)((r_X1 * fp.Geff + fp.U - 1) / fp.U) - 1, fp.Geff - 1);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int c = r_clo + q;
+            if (c <= r_chi) {
+                const long long a = max(free_slab_start(fp, c), r_X0), e = min(free_slab_start(fp, c + 1), r_X1);
+                if (a < e) pbv[q] = __ldcg(fp.PB + (size_t)(r_kpos + c) * FREE_ROWS + r_off);
+            }
+        }
     }
-    __syncthreads();
-    // symmetric work split: row t of block J also receives sum_{I < J} PC[I][t] (rows below s_off: nothing, their mirror
-    // entries are stored).  These are up to NB - 1 loads per row, each from another L2 line: four threads share a row
-    // (I = q, q + 4, ...; sixteen loads in flight each) and the four partial sums are added in fixed order.  rsum lives in
-    // the staging area (free again; fp.sym => the full scratch).
-    double* rsum = scratch + FREE_HEAD_DOUBLES;   // [rows]
+    // B: symmetric work split, row t of block J also receives sum_{I < J} PC[I][t] (rows below s_off: nothing, their mirror
+    // entries are stored).  Up to NB - 1 loads per row, each from another L2 line: four threads share a row (I = q, q + 4, ...;
+    // sixteen loads in flight each); the four partial sums are added in fixed order by the row's thread.
     if (fp.sym) {
-        double* rpart = rsum + ((r1 - r0 + 1) & ~1);   // [4][rows]
-        const int rows = r1 - r0;
-        for (int w = threadIdx.x; w < 4 * rows; w += blockDim.x) {
-            const int q = w / rows, lr = w - q * rows;
+        for (int w = threadIdx.x; w < 4 * rows_; w += blockDim.x) {
+            const int q = w / rows_, lr = w - q * rows_;
             const int t = r0 + lr;
             const int b = t < fp.s_off ? 0 : (t < fp.M0 ? t / FREE_ROWS : fp.NB0 + (t - fp.M0) / FREE_ROWS);
             const double* pc = fp.PC + t;
             double a0 = 0.0, a1 = 0.0;
             int I = q;
-            for (; I + 60 < b; I += 64) {                  // sixteen loads in flight
+            for (; I + 60 < b; I += 64) {
                 double v[16];
 #pragma unroll
                 for (int k = 0; k < 16; ++k) v[k] = __ldcg(pc + (size_t)(I + 4 * k) * nt.npad);
@@ -440,36 +464,60 @@ __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable
                 for (int k = 0; k < 8; k += 2) { a0 += v[k]; a1 += v[k + 1]; }
             }
             for (; I < b; I += 4) a0 += __ldcg(pc + (size_t)I * nt.npad);
-            rpart[q * rows + lr] = a0 + a1;
+            rpart[q * rows2_ + lr] = a0 + a1;
         }
-        __syncthreads();
-        for (int lr = threadIdx.x; lr < rows; lr += blockDim.x)
-            rsum[lr] = (rpart[lr] + rpart[rows + lr]) + (rpart[2 * rows + lr] + rpart[3 * rows + lr]);
-        __syncthreads();
     }
+    // A2, A3: the near entries of this CTA's rows are contiguous in the CSR arrays: all threads multiply them with x in
+    // parallel, each row then adds its run from shared memory.  (Hybrid operator, or more entries than fit: every row walks
+    // its own list below.)
+    const bool flat = (fp.s_off == 0) && (pend - pbeg <= prod_cap);
+    if (flat)
+        for (int p = pbeg + threadIdx.x; p < pend; p += blockDim.x) prod[p - pbeg] = fp.near_val[p] * __ldcg(xsrc + fp.near_col[p]);
+    // C: sum_s beta_s x_s per class and source range, the per-CTA partials of free_write_tables in fixed order (warps 0..3)
+    if (!fp.vortex && threadIdx.x < 128) {
+        const int q = threadIdx.x >> 5, lane = threadIdx.x & 31;
+        double sb = 0.0;
+        for (int i = lane; i < (int)gridDim.x; i += 32) sb += __ldcg(fp.SB + (4 * sb_sel + q) * FREE_SB_LD + i);
+        sb = bie_warp_sum(sb);
+        if (lane == 0) sbs[q] = sb;
+    }
+    __syncthreads();
     for (int t = r0 + threadIdx.x; t < r1; t += blockDim.x) {
-        int b, off;
-        if (t < fp.M0) { b = t / FREE_ROWS; off = t - b * FREE_ROWS; }
-        else { const int d = t - fp.M0; b = d / FREE_ROWS; off = d - b * FREE_ROWS; b += fp.NB0; }
-        const int kpos = fp.sym ? __ldg(fp.sym_pos + b) : b;   // position of the block in the work list
-        const long long X0 = fp.sym ? __ldg(fp.sym_cum + kpos) : free_list_start(fp, b);
-        const long long X1 = fp.sym ? __ldg(fp.sym_cum + kpos + 1) : free_list_start(fp, b + 1);
-        int c_lo = (int)(((X0 + 1) * fp.Geff + fp.U - 1) / fp.U) - 1;
-        int c_hi = (int)((X1 * fp.Geff + fp.U - 1) / fp.U) - 1;
-        c_lo = max(c_lo, 0); c_hi = min(c_hi, fp.Geff - 1);
-        double s = 0.0;
-        for (int c = c_lo; c <= c_hi; ++c) {
-            const long long a = max(free_slab_start(fp, c), X0), e = min(free_slab_start(fp, c + 1), X1);
-            if (a < e) s += __ldcg(fp.PB + (size_t)(kpos + c) * FREE_ROWS + off);
+        const int l = t - r0;
+        double s;
+        if (l == (int)threadIdx.x) {       // the row whose forward partials were loaded above
+            s = (pbv[0] + pbv[1]) + (pbv[2] + pbv[3]);
+            for (int c = r_clo + 4; c <= r_chi; ++c) {
+                const long long a = max(free_slab_start(fp, c), r_X0), e = min(free_slab_start(fp, c + 1), r_X1);
+                if (a < e) s += __ldcg(fp.PB + (size_t)(r_kpos + c) * FREE_ROWS + r_off);
+            }
+        } else {                            // more rows than threads
+            int b, off;
+            if (t < fp.M0) { b = t / FREE_ROWS; off = t - b * FREE_ROWS; }
+            else { const int d = t - fp.M0; b = d / FREE_ROWS; off = d - b * FREE_ROWS; b += fp.NB0; }
+            const int kpos = fp.sym ? __ldg(fp.sym_pos + b) : b;
+            const long long X0 = fp.sym ? __ldg(fp.sym_cum + kpos) : free_list_start(fp, b);
+            const long long X1 = fp.sym ? __ldg(fp.sym_cum + kpos + 1) : free_list_start(fp, b + 1);
+            const int c_lo = max((int)(((X0 + 1) * fp.Geff + fp.U - 1) / fp.U) - 1, 0);
+            const int c_hi = min((int)((X1 * fp.Geff + fp.U - 1) / fp.U) - 1, fp.Geff - 1);
+            s = 0.0;
+            for (int c = c_lo; c <= c_hi; ++c) {
+                const long long a = max(free_slab_start(fp, c), X0), e = min(free_slab_start(fp, c + 1), X1);
+                if (a < e) s += __ldcg(fp.PB + (size_t)(kpos + c) * FREE_ROWS + off);
+            }
         }
-        if (fp.sym) s += rsum[t - r0];   // reverse partials of the earlier row blocks (summed above)
-        // near pairs: exact entries from the CSR near matrix (rows below s_off: only the columns the stored block lacks)
+        if (fp.sym) s += (rpart[l] + rpart[rows2_ + l]) + (rpart[2 * rows2_ + l] + rpart[3 * rows2_ + l]);
+        // near pairs (rows below s_off: only the columns the stored block lacks)
         const bool below = (t < fp.s_off);
         const int p0 = fp.near_ptr[8 * (size_t)t], p1 = fp.near_ptr[8 * (size_t)t + 8];
         double sn = 0.0;
-        for (int p = p0; p < p1; ++p) {
-            const int cix = fp.near_col[p];
-            if (!below || cix >= fp.s_off) sn = fma(fp.near_val[p], __ldcg(xsrc + cix), sn);
+        if (flat) {
+            for (int p = p0; p < p1; ++p) sn += prod[p - pbeg];
+        } else {
+            for (int p = p0; p < p1; ++p) {
+                const int cix = fp.near_col[p];
+                if (!below || cix >= fp.s_off) sn = fma(fp.near_val[p], __ldcg(xsrc + cix), sn);
+            }
         }
         s += sn;
         if (!fp.vortex) {

@@ -118,13 +118,14 @@ __device__ __forceinline__ int pt_slot() { return blockIdx.x == 0 ? 0 : (blockId
 template <bool STREAM, bool XS, int MODE>
 __device__ __forceinline__ void cta_apply(const GmresArgs& a, int r0, int r1, const double* xin, double scale,
                                           double* xs, double* gpart, BlockRing& ring, double* y_local,
-                                          bool tables_ready, double* red, unsigned int& target)
+                                          bool tables_ready, double* red, unsigned int& target, int& sb_sel)
 {
     if (MODE != 0) {
         // xin is complete in global memory; its per-source tables either were written by the row owners before
         // the last grid barrier (tables_ready) or are written here
         if (!tables_ready) {
-            free_write_tables(a.nt, a.ct, a.fp, r0, r1, xin + r0, red);
+            sb_sel ^= 1;
+            free_write_tables(a.nt, a.ct, a.fp, r0, r1, xin + r0, red, sb_sel);
             grid_barrier(a.sync, target);
         }
         PT(6)
@@ -176,7 +177,7 @@ __device__ __forceinline__ void cta_apply(const GmresArgs& a, int r0, int r1, co
 #ifdef BIE_PHASE_TIMING
         const unsigned long long tg0 = gtime();
 #endif
-        free_gather(a.nt, a.ct, a.fp, r0, r1, xin, scale, gpart, y_local);
+        free_gather(a.nt, a.ct, a.fp, r0, r1, xin, scale, gpart, y_local, sb_sel);
 #ifdef BIE_PHASE_TIMING
         if (threadIdx.x == 0) g_gath[blockIdx.x] += gtime() - tg0;
 #endif
@@ -384,13 +385,17 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
     bool done = (bn == 0.0);
     if (a.res_hist && blockIdx.x == 0 && threadIdx.x == 0) a.res_hist[0] = 1.0;
     bool first = true;
+    // which copy of the constants' partials (FreePlan::SB) the last table write filled.  The copies alternate because the
+    // table write at a cycle's start follows the gather of the residual's operator application WITHOUT a grid barrier in
+    // between: a CTA that is done may write while others still read the previous copy.
+    int sb_sel = 0;
     while (!done) {
         // ---- cycle start: r = b - A x ------------------------------------------------------------
         if (first) {
             for (int r = threadIdx.x; r < rows; r += blockDim.x) w_local[r] = a.b[r0 + r];
             first = false;
         } else {
-            cta_apply<STREAM, XS, MODE>(a, r0, r1, a.x, 1.0, xs, gpart, ring, y_local, false, red, target);
+            cta_apply<STREAM, XS, MODE>(a, r0, r1, a.x, 1.0, xs, gpart, ring, y_local, false, red, target, sb_sel);
             for (int r = threadIdx.x; r < rows; r += blockDim.x) w_local[r] = a.b[r0 + r] - y_local[r];
         }
         __syncthreads();
@@ -400,7 +405,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
             p = fma(v, v, p);
             a.wbuf[r0 + r] = v;
         }
-        if (FREE) free_write_tables_cached(a.fp, a.nt.npad, r0, r1, w_local, Kc, rows2, red);
+        if (FREE) { sb_sel ^= 1; free_write_tables_cached(a.fp, a.nt.npad, r0, r1, w_local, Kc, rows2, red, sb_sel); }
         p = block_sum(p, red);
         if (threadIdx.x == 0) part3[blockIdx.x] = p;
         grid_barrier(a.sync, target);
@@ -423,7 +428,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
         for (int j = 0; j < m; ++j) {
             PT(5)
             // a6: y = A (wbuf * inv) = A v_j + V_j c * inv  (c = 0 in the first step of a cycle)
-            cta_apply<STREAM, XS, MODE>(a, r0, r1, a.wbuf, inv, xs, gpart, ring, y_local, true, red, target);
+            cta_apply<STREAM, XS, MODE>(a, r0, r1, a.wbuf, inv, xs, gpart, ring, y_local, true, red, target, sb_sel);
             PT(0)
             // a7, first pass: s = V_j^T y (grid barrier 1), w1 = y - V_j s, h1 = s - c * inv
             local_dots(B, rows, j + 1, y_local, part1, false);
@@ -438,7 +443,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
                 a.wbuf[r0 + r] = v;                       // the next operator application reads w1 (see the header)
             }
             __syncthreads();
-            if (FREE) free_write_tables_cached(a.fp, a.nt.npad, r0, r1, w_local, Kc, rows2, red);
+            if (FREE) { sb_sel ^= 1; free_write_tables_cached(a.fp, a.nt.npad, r0, r1, w_local, Kc, rows2, red, sb_sel); }
             // second pass: h2 = V_j^T w1 and ||w1||^2 in ONE reduction (grid barrier 2)
             local_dots(B, rows, j + 1, w_local, part2, true);
             PT(2)
@@ -469,7 +474,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
                     a.wbuf[r0 + r] = v;
                 }
                 __syncthreads();
-                if (FREE) free_write_tables_cached(a.fp, a.nt.npad, r0, r1, w_local, Kc, rows2, red);
+                if (FREE) { sb_sel ^= 1; free_write_tables_cached(a.fp, a.nt.npad, r0, r1, w_local, Kc, rows2, red, sb_sel); }
                 p = block_sum(p, red);
                 if (threadIdx.x == 0) part3[blockIdx.x] = p;
                 grid_barrier(a.sync, target);
@@ -569,7 +574,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
     // ---- a10: outputs; true residual ||b - A x|| / ||b|| (reported only) -----------------------------
     double relres = 0.0;
     if (a.relres_out && bn != 0.0) {
-        cta_apply<STREAM, XS, MODE>(a, r0, r1, a.x, 1.0, xs, gpart, ring, y_local, false, red, target);
+        cta_apply<STREAM, XS, MODE>(a, r0, r1, a.x, 1.0, xs, gpart, ring, y_local, false, red, target, sb_sel);
         p = 0.0;
         for (int r = threadIdx.x; r < rows; r += blockDim.x) {
             const double v = a.b[r0 + r] - y_local[r];

@@ -168,7 +168,7 @@ size_t bie_free_buf_doubles(int cap)
 {
     // tables [4][cap] double2, then partial sums for (row blocks + CTAs) parts of FREE_ROWS rows, then the per-CTA
     // partials of the constant terms [4][FREE_SB_LD]
-    return 8 * (size_t)cap + ((size_t)cap / FREE_ROWS + 2 + 256) * FREE_ROWS + 4 * FREE_SB_LD;
+    return 8 * (size_t)cap + ((size_t)cap / FREE_ROWS + 2 + 256) * FREE_ROWS + 2 * 4 * FREE_SB_LD;
 }
 
 // work list of the symmetric split (bie_free_sym.cuh), built on the device by one thread (NB <= a few hundred):
