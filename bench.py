@@ -45,7 +45,8 @@ UNIT = "Gentries/s"
 # (profiles/r02_build.md, profiles/r02_free.md); the hand counts of DESIGN.md section 5 are 10 / 10 / 6.5 + reduction
 FP64_PER_ENTRY_BUILD = 10.1     # bie_build_kernel, difference form
 FP64_PER_ENTRY_SYM = 6.92       # symmetric pair loops: 13 per pair of entries + lane reduction of the reverse sums
-FP64_PER_PAIR_VORTEX = 13.0     # vortex-sheet matrix, (X, Y) form
+FP64_PER_ENTRY_VORTEX_BUILD = 11.0   # vortex-sheet / normal-velocity builds: row-side difference form (bie_build.cu)
+FP64_PER_PAIR_VORTEX = 13.0     # vortex-sheet matrix in the matrix-free operator, (X, Y) form
 NOMINAL_FP64_INSTR_S = 148 * 64 * 1.965e9   # B200: 148 SMs x 64 FP64 lanes x 1.965 GHz = 18.6 T instr/s
 HBM_FALLBACK_GBS = 6650.0      # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_dram_traffic.csv")   # dram bytes per launch from `ncu --set full`
@@ -596,7 +597,8 @@ def main():
         vx = timer(lambda: ctx.bie_build(g.counts, g.kinds, z, dz, d2z, A, variant=2), 10)
         next_rows["vortex_sheet_matrix"] = {"call": "bie_build(variant=BIE_VARIANT_VORTEX)", "ms": vx["median_ms"], "best_ms": vx["best_ms"],
                                             "gentries_per_s": n * n / (vx["median_ms"] * 1e-3) / 1e9,
-                                            "fp64_frac_of_probe": n * n * FP64_PER_PAIR_VORTEX / (vx["median_ms"] * 1e-3) / dfma_per_s,
+                                            "fp64_instr_per_entry": FP64_PER_ENTRY_VORTEX_BUILD,
+                                            "fp64_frac_of_probe": n * n * FP64_PER_ENTRY_VORTEX_BUILD / (vx["median_ms"] * 1e-3) / dfma_per_s,
                                             "hbm_write_frac": 8.0 * n * n / (vx["median_ms"] * 1e-3) / 1e9 / peak}
         ctx.bie_set_geometry(g.counts, g.kinds, z, dz, d2z, variant=2)
         vmf = timer(lambda: ctx.bie_matvec_free(xv, yv), 20)
@@ -617,7 +619,7 @@ def main():
         f_e = dev(np.vstack([np.exp(1j * g.zeta), np.exp(2j * g.zeta)]))
         out_e = torch.empty((2, npts_e), dtype=torch.complex128, device="cuda")
         ev = timer(lambda: ctx.bie_cauchy_eval(g.counts, g.kinds, z, dz, f_e, zp_e, out=out_e), 5)
-        ev_instr = 12 + 4 * 3     # FP64-pipe instructions per pair: cot (12) + denominator and two numerators (4 each)
+        ev_instr = 9 + 4 * 3      # FP64-pipe instructions per pair: differences, denominator, reciprocal (9) + four per numerator (Cauchy sum and nf = 2 functions)
         next_rows["cauchy_eval_near_boundary"] = {"call": "bie_cauchy_eval (nf = 2)", "points": npts_e, "sources": n, "ms": ev["median_ms"],
                                                   "gpairs_per_s": npts_e * n / (ev["median_ms"] * 1e-3) / 1e9,
                                                   "fp64_instr_per_pair": ev_instr,

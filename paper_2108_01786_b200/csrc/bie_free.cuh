@@ -79,9 +79,10 @@ struct FreePlan {
 #define SYM_BATCH 8
 #endif
 #ifndef SYM_PART_PAD
-#define SYM_PART_PAD 256      // symmetric work list: every row block's list is longer by this many VIRTUAL sources (no work): the fixed
-                              // cost of starting a part (target loads, exposed first loads of its segments, warp-sum reduction; measured
-                              // about 5 us = the time of 250-300 sources), so that cutting the list into equal slabs equalises TIME
+#define SYM_PART_PAD 144      // symmetric work list: every row block's list is longer by this many VIRTUAL sources (no work): the fixed
+                              // cost of starting a list (target loads, exposed first loads of its segments, warp-sum reduction) is
+                              // 2.3-2.7 us = the time of 125-145 sources (least-squares fit of the CTAs' pair-loop times to their
+                              // sources and list starts, config 5), so that cutting the list into equal slabs equalises TIME
 #endif
 #define SYM_COL_STRIDE 33                                         // [SYM_BATCH][33] doubles per warp: lane-private slots, no bank conflicts
 #define SYM_COL_DOUBLES (FREE_WARPS * SYM_BATCH * SYM_COL_STRIDE)

@@ -103,23 +103,27 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
                     tu[i] = uw.x; tw[i] = uw.y;
                 }
             }
-            double2 ne = zero2, nuw = zero2;
-            if (wa + lane < wb) {
-                const int s = wa + lane;
-                ne = nt.E[s]; nuw = __ldcg(TUW + s);
-            }
+            // warp-private double buffer filled by cp.async (no registers held across a chunk), zero-filled past wb: the batches
+            // run over multiples of SYM_BATCH and the sources beyond wb must be zero sources
+            auto issue = [&](int base_, int bufi) {
+                const int s = base_ + lane;
+                const bool ok = s < wb;
+                const int sc = ok ? s : wa;
+                const unsigned sz = ok ? 16u : 0u;
+                double2* sgi = reinterpret_cast<double2*>(stage + bufi * sbuf);
+                free_cp_async16(sgi + lane, nt.E + sc, sz);
+                free_cp_async16(sgi + 32 + lane, TUW + sc, sz);
+                asm volatile("cp.async.commit_group;" ::: "memory");
+            };
             int buf = 0;
             __syncwarp();
+            issue(wa, 0);
             const int len = 32;
             for (int base = wa; base < wb; base += len, buf ^= 1) {
-                double2* sg = reinterpret_cast<double2*>(stage + buf * sbuf);
-                sg[lane] = ne; sg[32 + lane] = nuw;     // lanes beyond wb stage zero sources (the batches run over multiples of SYM_BATCH)
-                __syncwarp();
-                {
-                    const int s = base + len + lane;
-                    ne = zero2; nuw = zero2;
-                    if (s < wb) { ne = nt.E[s]; nuw = __ldcg(TUW + s); }
-                }
+                const double2* sg = reinterpret_cast<const double2*>(stage + buf * sbuf);
+                asm volatile("cp.async.wait_group 0;" ::: "memory");
+                __syncwarp();                                   // chunk landed for all lanes; the other buffer is no longer read
+                if (base + len < wb) issue(base + len, buf ^ 1);
                 const int cnt = min(len, wb - base);
                 if (!rev) {
 #pragma unroll 2
@@ -136,10 +140,14 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
                     }
                 } else {
                     for (int j0 = 0; j0 < cnt; j0 += SYM_BATCH) {   // sources beyond cnt are zero sources; not written
+                        // the next source's operands are loaded BEFORE this source's reverse sum is stored: the compiler
+                        // cannot move a shared load above a shared store it cannot tell apart, and would serialise the sources
+                        double2 e = sg[j0], uw = sg[32 + j0];
 #pragma unroll
                         for (int u = 0; u < SYM_BATCH; ++u) {
                             const int j = j0 + u;
-                            const double2 e = sg[j], uw = sg[32 + j];
+                            double2 en = e, uwn = uw;
+                            if (u + 1 < SYM_BATCH) { en = sg[j + 1]; uwn = sg[32 + j + 1]; }
                             double s_rev0 = 0.0, s_rev1 = 0.0;
 #pragma unroll
                             for (int i = 0; i < FREE_NT; ++i) {
@@ -153,6 +161,7 @@ __device__ __forceinline__ void free_parts_sym(const NodeTable& nt, const FreePl
                                 const double vr = fma(tw[i], di, tu[i] * dr);
                                 if (i & 1) s_rev1 = fma(vr, r, s_rev1); else s_rev0 = fma(vr, r, s_rev0);
                             }
+                            e = en; uw = uwn;
                             col[u * SYM_COL_STRIDE + lane] = s_rev0 + s_rev1;
                         }
                         // lane reduction of the SYM_BATCH reverse sums through shared memory: 32 / SYM_BATCH lanes share a source,

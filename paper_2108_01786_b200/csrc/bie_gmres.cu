@@ -457,6 +457,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
                 if (threadIdx.x == 0) red[128] = ss;
             }
             __syncthreads();
+            PT(10)
             const double nu = hloc[j + 1], ss = red[128];
             double hn;
             const bool pyth = (ss <= 0.01 * nu);           // identical in every CTA (same bits)
@@ -480,6 +481,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
                 grid_barrier(a.sync, target);
                 hn = sqrt(warp_sum_partials(part3, G));
             }
+            PT(11)
             inv = (hn != 0.0) ? 1.0 / hn : 0.0;
             {
                 double* vn = (j + 1 < B.VS) ? B.Vs + (size_t)(j + 1) * rows2 : B.Vg + (size_t)(j + 1) * a.nld;
@@ -487,6 +489,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
             }
             for (int i = threadIdx.x; i <= j; i += blockDim.x) hcol[i] += hloc[i];
             __syncthreads();
+            PT(12)
             // column j of Hbar (single precision copy), then c = Hbar_j h2 for the next step
             for (int i = threadIdx.x; i <= j + 1; i += blockDim.x) Hf[hess_off(j) + i] = (float)(i <= j ? hcol[i] : hn);
             __syncthreads();
@@ -501,6 +504,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
                 c += __shfl_xor_sync(0xffffffffu, c, 2);
                 if (q == 0 && kk <= j + 1) cvec[kk] = c;
             }
+            PT(13)
             // a8: Givens rotations on column j, new rotation, recurrence residual
             if (threadIdx.x == GM_THREADS - 1) {
                 hcol[j + 1] = hn;
@@ -519,6 +523,7 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
                 g[j] = cs[j] * g[j];
             }
             __syncthreads();
+            PT(14)
             if (blockIdx.x == 0)
                 for (int i = threadIdx.x; i <= j; i += blockDim.x) a.R[(size_t)j * (m + 1) + i] = hcol[i];
             ++iters;
@@ -541,9 +546,9 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
         if (threadIdx.x == 0 && pt_slot() >= 0 && !BIE_PT_PAIR_ONLY) {
             const unsigned long long* q = g_pt[pt_slot()];
             printf("cta %3d, cycle of %d steps, us per step: [operator: tables/x %.1f | pair loops or GEMV %.1f | barrier %.1f | gather %.1f | rest %.1f] "
-                   "dots1 + barrier1 %.1f | reduce + w1 + tables + dots2 %.1f | barrier2 %.1f | tail %.1f | loop %.1f\n", (int)blockIdx.x, k,
+                   "dots1 + barrier1 %.1f | reduce + w1 + tables + dots2 %.1f | barrier2 %.1f | tail %.1f (reduce2 %.1f, combine2 %.1f, v/hcol %.1f, Hf/c %.1f, Givens %.1f) | loop %.1f\n", (int)blockIdx.x, k,
                    q[6] * 1e-3 / k, q[7] * 1e-3 / k, q[8] * 1e-3 / k, q[9] * 1e-3 / k, q[0] * 1e-3 / k, q[1] * 1e-3 / k, q[2] * 1e-3 / k,
-                   q[3] * 1e-3 / k, q[4] * 1e-3 / k, q[5] * 1e-3 / k);
+                   q[3] * 1e-3 / k, q[4] * 1e-3 / k, q[10] * 1e-3 / k, q[11] * 1e-3 / k, q[12] * 1e-3 / k, q[13] * 1e-3 / k, q[14] * 1e-3 / k, q[5] * 1e-3 / k);
         }
 #endif
         // ---- a9: y = R^{-1} g (CTA 0), x += V y ---------------------------------------------------
