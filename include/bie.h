@@ -55,6 +55,7 @@ extern "C" {
 #define BIE_ERR_WORKSPACE (-4) /* workspace too small (see bie_*_workspace_bytes)                    */
 #define BIE_ERR_DEVICE (-5)    /* not a compute-capability-10.x device                               */
 #define BIE_ERR_ARG (-6)       /* restart < 1, max_iters < 0, tol < 0, unknown variant/flags         */
+#define BIE_ERR_NOALLOC_SIZE (-9) /* bie_gmres_noalloc: (n, restart) needs more than the static scratch */
 #define BIE_ERR_CUDA_BASE (-100)
 
 #define BIE_KIND_SURFACE 0
@@ -245,6 +246,25 @@ int bie_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, const double* r
               double tol, int restart, int max_iters,
               double* x, int32_t* iters_out, double* relres_out, int32_t* status_out, double* res_hist,
               void* workspace, size_t workspace_bytes, void* stream);
+
+/* The same solve with the stored matrix for callers that must not allocate (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): there is no workspace argument, the workspace is a file-scope device
+ * array of BIE_NOALLOC_SCRATCH_BYTES inside the library (every GPU that loads the library holds it until exit), and the
+ * call itself calls no cudaMalloc, cudaFree or allocating library routine.  The ctx must exist already (bie_create
+ * allocates; do that at set-up).  The first call on a device looks up the array's device address (cudaGetSymbolAddress,
+ * not an allocation).
+ * A != NULL (dev, lda as in bie_gmres): only the stored-matrix operator is served -- the matrix-free and hybrid operators
+ * build a near matrix whose size depends on the geometry.  rhs, x, iters_out, relres_out, status_out: as in bie_gmres.
+ * Limit: bie_gmres_workspace_bytes(n, restart) <= BIE_NOALLOC_SCRATCH_BYTES (4 MiB: n = 4608 with restart 50 takes
+ * 2.3 MB, n = 8192 with restart 50 3.8 MB); anything larger returns BIE_ERR_NOALLOC_SIZE and launches nothing.
+ * ALL calls, from all ctxs and streams of a process, share the one array per device: two calls that overlap on the GPU
+ * race (keep them on one stream or order them with events).  The array keeps the previous call's contents; the solve
+ * writes every part before reading it and clears the grid-barrier counter on the stream before the launch. */
+#define BIE_NOALLOC_SCRATCH_BYTES (4u << 20)
+size_t bie_gmres_noalloc_max_bytes(void);
+int bie_gmres_noalloc(bie_ctx* ctx, int n, const double* A, int64_t lda, const double* rhs,
+                      double tol, int restart, int max_iters,
+                      double* x, int32_t* iters_out, double* relres_out, int32_t* status_out, void* stream);
 
 /* Same solve with the hybrid operator: A holds the leading ncols_dense x ncols_dense block of the matrix of the ctx's
  * current geometry in the block format (bie_build_block), ncols_dense a row-block boundary as described at

@@ -25,7 +25,8 @@ EXPORTS = ("bie_create", "bie_destroy", "bie_strerror", "bie_device_info", "bie_
            "bie_solve_workspace_bytes", "bie_solve_host", "bie_probe_dfma", "bie_build_cols", "bie_hybrid_cols",
            "bie_set_hybrid_free_warps", "bie_gmres_hybrid", "bie_matvec_rect", "bie_build_normal_velocity",
            "bie_add_cyl_columns", "bie_cauchy_eval_workspace_bytes", "bie_cauchy_eval", "bie_set_symmetric",
-           "bie_build_block", "bie_set_hybrid_poll_tiles", "bie_hybrid_block_bytes", "bie_probe_read")
+           "bie_build_block", "bie_set_hybrid_poll_tiles", "bie_hybrid_block_bytes", "bie_probe_read",
+           "bie_gmres_noalloc", "bie_gmres_noalloc_max_bytes")
 
 BIE_OK, BIE_MAX_ITERS = 0, 1
 OP_DENSE, OP_FREE, OP_HYBRID = 0, 1, 2
@@ -71,6 +72,10 @@ def lib() -> ctypes.CDLL:
         L.bie_gmres_workspace_bytes.argtypes = [i32, i32]
         L.bie_gmres.restype = i32
         L.bie_gmres.argtypes = [vp, i32, vp, i64, vp, dbl, i32, i32, vp, vp, vp, vp, vp, vp, sz, vp]
+        L.bie_gmres_noalloc.restype = i32
+        L.bie_gmres_noalloc.argtypes = [vp, i32, vp, i64, vp, dbl, i32, i32, vp, vp, vp, vp, vp]
+        L.bie_gmres_noalloc_max_bytes.restype = sz
+        L.bie_gmres_noalloc_max_bytes.argtypes = []
         L.bie_solve_workspace_bytes.restype = sz
         L.bie_solve_workspace_bytes.argtypes = [i32, i32, i32]
         L.bie_solve_host.restype = i32
@@ -317,6 +322,25 @@ class Context:
                                out_i32.data_ptr() + 4,
                                None if res_hist is None else _dev_f64(res_hist, int(max_iters) + 1),
                                workspace.data_ptr(), ws_bytes, _stream()), "bie_gmres")
+        return x
+
+    @staticmethod
+    def bie_gmres_noalloc_max_bytes() -> int:
+        return int(lib().bie_gmres_noalloc_max_bytes())
+
+    def bie_gmres_noalloc(self, A, rhs, x, tol: float, restart: int, max_iters: int, out_i32, out_f64,
+                          lda: Optional[int] = None):
+        """Asynchronous.  bie_gmres with the stored matrix A and NO workspace argument: the workspace is a static device
+        array inside the library (bie_gmres_workspace_bytes(n, restart) must not exceed bie_gmres_noalloc_max_bytes());
+        the call allocates nothing.  Calls that overlap on the GPU race: they share the array.  Outputs as bie_gmres."""
+        import torch
+        n = rhs.numel()
+        lda = int(lda if lda is not None else A.stride(0))
+        pA = _dev_f64(A, (n - 1) * lda + n)
+        assert out_i32.is_cuda and out_i32.dtype == torch.int32 and out_i32.numel() >= 2
+        _check(lib().bie_gmres_noalloc(self._h, n, pA, lda, _dev_f64(rhs, n), float(tol), int(restart), int(max_iters),
+                                       _dev_f64(x, n), out_i32.data_ptr(), _dev_f64(out_f64, 1),
+                                       out_i32.data_ptr() + 4, _stream()), "bie_gmres_noalloc")
         return x
 
     def bie_gmres_hybrid(self, A, ncols_dense: int, rhs, x, tol: float, restart: int, max_iters: int, workspace,

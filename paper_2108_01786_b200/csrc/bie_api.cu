@@ -82,6 +82,7 @@ const char* bie_strerror(int code)
         case BIE_ERR_WORKSPACE: return "workspace too small";
         case BIE_ERR_DEVICE: return "no usable compute-capability-10.x device";
         case BIE_ERR_ARG: return "bad argument";
+        case BIE_ERR_NOALLOC_SIZE: return "bie_gmres_noalloc: (n, restart) needs more workspace than the static scratch (BIE_NOALLOC_SCRATCH_BYTES)";
         default: return code <= BIE_ERR_CUDA_BASE ? "CUDA runtime error (code = -100 - cudaError_t)" : "unknown code";
     }
 }
