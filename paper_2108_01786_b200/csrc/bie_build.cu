@@ -44,6 +44,17 @@ __device__ __forceinline__ double bie_entry_fast(const SrcCol& s, const double2 
     return fma(val, bie_rcp3(den), -s.cst);
 }
 
+// the same entry; instead of a flag the smallest high word of den seen so far (one integer min per entry; the near
+// test den < thr_s is made once per block of rows)
+__device__ __forceinline__ double bie_entry_fast_min(const SrcCol& s, const double2 te, int& mn)
+{
+    const double dr = s.er - te.x, di = s.ei - te.y;
+    const double den = fma(dr, dr, di * di);
+    const double val = fma(s.w, di, s.u * dr);
+    mn = min(mn, __double2hiint(den));
+    return fma(val, bie_rcp3(den), -s.cst);
+}
+
 // exact value of a near entry (rare): Laurent series from the coordinate differences, or the diagonal limit
 static __device__ __noinline__ double bie_entry_near(const double2* __restrict__ DG, const double2* __restrict__ XY,
                                                      double sa, double sb, double sem, int sidx, int tidx)
@@ -62,6 +73,28 @@ __device__ __forceinline__ void bie_block_coef(bool src0, bool tgt0, double qr, 
     if (src0 == tgt0) { al = -2.0 * qi; be = qr; }       // Im c
     else if (tgt0)    { al = -2.0 * qr; be = -qi; }      // Re c   (G_0j)
     else              { al = 2.0 * qr;  be = qi; }       // -Re c  (-G_k0)
+}
+
+// rows [ta, tb) of a thread that saw a near pair: its near entries are overwritten with the exact value
+static __device__ __forceinline__ void bie_build_fix_near(const NodeTable& nt, const SrcCol* src, const int* scomp, const double* sqr,
+                                                       const double* sqi, const double* sem, const double2* sE, int t0, int ta, int tb,
+                                                       int k, int s0, int ncols, double* A, long long lda, int nchT, bool tiled)
+{
+    for (int t = ta; t < tb; ++t) {
+        const double2 te = sE[t - t0];
+#pragma unroll
+        for (int c = 0; c < BUILD_COLS; ++c) {
+            if (s0 + c >= ncols) continue;
+            const double dr = src[c].er - te.x, di = src[c].ei - te.y;
+            const double den = fma(dr, dr, di * di);
+            if (__double2hiint(den) < src[c].thi) {
+                double al, be;
+                bie_block_coef(scomp[c] == 0, k == 0, sqr[c], sqi[c], al, be);
+                A[bie_entry_off(tiled ? 0 : lda, nchT, t, s0 + c)] =
+                    bie_entry_near(nt.DG, nt.XY, al, be, (scomp[c] == k) ? sem[c] : 0.0, s0 + c, t);
+            }
+        }
+    }
 }
 
 // TILED: A is the block format of the hybrid operator (bie_common.cuh) instead of row-major with leading dimension lda
@@ -92,6 +125,7 @@ bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long l
     __syncthreads();
     const bool full = (s0 + 1 < ncols);   // ncols = n, or the width of the hybrid operator's block
     const bool part = (s0 < ncols);
+    const bool wfull = __all_sync(0xffffffffu, full);   // warp-uniform: the fast row loop votes per block of rows
     const int nchT = (ncols + BIE_TILE_COLS - 1) / BIE_TILE_COLS;   // block format (lda == 0)
     for (int k = 0; k < ct.ncomp; ++k) {
         const int a = max(t0, ct.off[k]), b = min(t1, ct.off[k + 1]);
@@ -104,7 +138,29 @@ bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long l
             src[c].w = fma(-al, src[c].er, 2.0 * be * src[c].ei);
             src[c].cst = be + ((scomp[c] == k) ? sem[c] : 0.0);
         }
-        for (int tb = a; tb < b; tb += BUILD_RB) {
+        int tb = a;
+        if (!TILED && wfull) {
+            // whole blocks of BUILD_RB rows, both columns of every lane inside the matrix (all but the last warp of the last tile
+            // column): no clamp, no store predicate, the row pointer advanced by additions -- 17 instead of 26 issued
+            // instructions per entry (the kernel is issue-bound before it is write-bound)
+            double* p = A + (long long)a * lda + s0;
+            const double2* se = sE + (a - t0);
+            for (; tb + BUILD_RB <= b; tb += BUILD_RB, p += BUILD_RB * lda, se += BUILD_RB) {
+                int m0 = 0x7fffffff, m1 = 0x7fffffff;
+#pragma unroll
+                for (int r = 0; r < BUILD_RB; ++r) {
+                    const double2 te = se[r];
+                    const double e0 = bie_entry_fast_min(src[0], te, m0);
+                    const double e1 = bie_entry_fast_min(src[1], te, m1);
+                    *reinterpret_cast<double2*>(p + (long long)r * lda) = make_double2(e0, e1);
+                }
+                const int flag = (m0 < src[0].thi) | (m1 < src[1].thi);
+                if (__any_sync(0xffffffffu, flag)) {
+                    if (flag) bie_build_fix_near(nt, src, scomp, sqr, sqi, sem, sE, t0, tb, tb + BUILD_RB, k, s0, ncols, A, lda, nchT, false);
+                }
+            }
+        }
+        for (; tb < b; tb += BUILD_RB) {
             int flag = 0;
             double* row = TILED ? A : A + (long long)tb * lda + s0;
 #pragma unroll
@@ -118,24 +174,7 @@ bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long l
                 else if (part) p[0] = e0;
             }
             if (__any_sync(0xffffffffu, flag)) {
-                if (flag) {
-                    const int te_ = min(tb + BUILD_RB, b);
-                    for (int t = tb; t < te_; ++t) {
-                        const double2 te = sE[t - t0];
-#pragma unroll
-                        for (int c = 0; c < BUILD_COLS; ++c) {
-                            if (s0 + c >= ncols) continue;
-                            const double dr = src[c].er - te.x, di = src[c].ei - te.y;
-                            const double den = fma(dr, dr, di * di);
-                            if (__double2hiint(den) < src[c].thi) {
-                                double al, be;
-                                bie_block_coef(scomp[c] == 0, k == 0, sqr[c], sqi[c], al, be);
-                                A[bie_entry_off(TILED ? 0 : lda, nchT, t, s0 + c)] =
-                                    bie_entry_near(nt.DG, nt.XY, al, be, (scomp[c] == k) ? sem[c] : 0.0, s0 + c, t);
-                            }
-                        }
-                    }
-                }
+                if (flag) bie_build_fix_near(nt, src, scomp, sqr, sqi, sem, sE, t0, tb, min(tb + BUILD_RB, b), k, s0, ncols, A, lda, nchT, TILED);
             }
         }
     }
@@ -181,12 +220,55 @@ __device__ __forceinline__ double bie_entry_fast_dagger(const SrcColD& s, const 
     return fma(num, bie_rcp3(den), bt) * s.ms;
 }
 
+// rows [ta, tb) of a thread that saw a near pair: its near entries are overwritten with the exact value
+static __device__ __forceinline__ void bie_dagger_fix_near(const NodeTable& nt, const CompTable& ct, const SrcColD* src, const bool* col0,
+                                                           const bool* kap, const double2* sE, const double* sK, int dmin, int t0, int ta,
+                                                           int tb, int s0, int ncols, double* A, long long lda, int nchT, bool tiled, bool nv)
+{
+    for (int t = ta; t < tb; ++t) {
+        const double2 te = sE[t - t0];
+#pragma unroll
+        for (int c = 0; c < BUILD_COLS; ++c) {
+            if (s0 + c >= ncols) continue;
+            const double dr = src[c].er - te.x, di = src[c].ei - te.y;
+            const double den = fma(dr, dr, di * di);
+            if (__double2hiint(den) < src[c].thi) {
+                const int k = nt.COMP[t];
+                const double Mk = (double)(ct.off[k + 1] - ct.off[k]);
+                const double2 q = nt.Q[t];
+                const double2 ab = bie_dagger_ab(nv, k == 0, col0[c], q.x * Mk, q.y * Mk);
+                // (A X' + B Y')/den with cot = (-2X + iY)/den; the diagonal entry is prepared per node
+                double v = bie_entry_near(nt.DG, nt.XY, src[c].ms * ab.x, src[c].ms * ab.y, 0.0, s0 + c, t);
+                if (kap[c]) v += sK[t - s0 - c - dmin];
+                A[bie_entry_off(tiled ? 0 : lda, nchT, t, s0 + c)] = v;
+            }
+        }
+    }
+}
+
+// the same entry with the smallest high word of den instead of a flag (bie_entry_fast_min)
+__device__ __forceinline__ double bie_entry_fast_dagger_min(const SrcColD& s, const double2 te, const double2 uw, const double bt, int& mn)
+{
+    const double dr = s.er - te.x, di = s.ei - te.y;
+    const double den = fma(dr, dr, di * di);
+    const double num = fma(uw.y, di, uw.x * dr);
+    mn = min(mn, __double2hiint(den));
+    return fma(num, bie_rcp3(den), bt) * s.ms;
+}
+
+// shared memory of bie_build_dagger_kernel in bytes (kap: with the two copies of the real-cot table)
+static inline size_t bie_dagger_smem(int T, bool kap)
+{
+    return 4 * sizeof(double2) * (size_t)T + (kap ? sizeof(double) * (2 * (size_t)(T + BUILD_TILE_W) + 2) : 0) + 16;
+}
+
 template <bool TILED>
 __global__ void __launch_bounds__(BUILD_THREADS)
 bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long lda, int T, int only0, int ncols, int nrows,
                         const double* __restrict__ kappa /* NULL: vortex-sheet S; else the normal-velocity operator */)
 {
-    // [T] E_t, [T] (U,W) for columns on Gamma_0, [T] (U,W) for solids, [T] (B for Gamma_0 columns, B for solids), [T + 256] kappa
+    // [T] E_t, [T] (U,W) for columns on Gamma_0, [T] (U,W) for solids, [T] B for Gamma_0 columns, [T] B for solids,
+    // [T + 256] kappa (KA), [T + 258] kappa shifted by one (KB[x] = KA[x - 1])
     extern __shared__ __align__(16) double2 sm[];
     const int c0 = blockIdx.x * BUILD_TILE_W;
     const int t0 = blockIdx.y * T;
@@ -195,8 +277,10 @@ bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long
     double2* sE = sm;
     double2* sUW0 = sm + T;
     double2* sUW1 = sm + 2 * T;
-    double2* sBB = sm + 3 * T;
-    double* sK = reinterpret_cast<double*>(sm + 4 * T);
+    double* sB0 = reinterpret_cast<double*>(sm + 3 * T);
+    double* sB1 = sB0 + T;
+    double* sK = reinterpret_cast<double*>(sm + 4 * T);          // KA
+    double* sKB = sK + (T + BUILD_TILE_W);
     const int M0 = ct.off[1];
     for (int i = threadIdx.x; i < t1 - t0; i += BUILD_THREADS) {
         const int t = t0 + i;
@@ -209,16 +293,21 @@ bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long
         sE[i] = e;
         sUW0[i] = make_double2(fma(ab0.x, e.y, 2.0 * ab0.y * e.x), fma(-ab0.x, e.x, 2.0 * ab0.y * e.y));
         sUW1[i] = make_double2(fma(ab1.x, e.y, 2.0 * ab1.y * e.x), fma(-ab1.x, e.x, 2.0 * ab1.y * e.y));
-        sBB[i] = make_double2(ab0.y, ab1.y);
+        sB0[i] = ab0.y; sB1[i] = ab1.y;
     }
     // the real-cot table of the Gamma_0 - Gamma_0 block of the normal-velocity operator: kappa_{(t - s) mod M_0} for the tile's
-    // differences d = t - s in [t0 - c0 - 255, t1 - 1 - c0]
+    // differences d = t - s in [t0 - c0 - 255, t1 - 1 - c0].  Entry (t, s0) takes KA[i], entry (t, s0 + 1) takes KA[i - 1],
+    // i = t - s0 - dmin >= 1: for odd i the pair is an aligned double2 of KA, for even i of the shifted copy KB -- one
+    // 128-bit load per row and thread, consecutive lanes on consecutive 16 bytes (two 64-bit loads at a 16-byte stride
+    // have two-way bank conflicts)
     const int dmin = t0 - c0 - (BUILD_TILE_W - 1);
-    if (kappa != nullptr && c0 < M0)
+    const bool have_k = (kappa != nullptr && c0 < M0);
+    if (have_k)
         for (int i = threadIdx.x; i < (t1 - t0) + BUILD_TILE_W - 1; i += BUILD_THREADS) {
             int d = (dmin + i) % M0;
             if (d < 0) d += M0;
-            sK[i] = __ldg(kappa + d);
+            const double kv = __ldg(kappa + d);
+            sK[i] = kv; sKB[i + 1] = kv;
         }
     const int s0 = c0 + BUILD_COLS * threadIdx.x;  // < npad by construction
     SrcColD src[BUILD_COLS];
@@ -240,18 +329,51 @@ bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long
     const int nchT = (ncols + BIE_TILE_COLS - 1) / BIE_TILE_COLS;   // block format (lda == 0)
     const double2* sUWa = col0[0] ? sUW0 : sUW1;
     const double2* sUWb = col0[1] ? sUW0 : sUW1;
-    for (int tb = t0; tb < t1; tb += BUILD_RB) {
+    const double* sBa = col0[0] ? sB0 : sB1;
+    const double* sBb = col0[1] ? sB0 : sB1;
+    int tb = t0;
+    if (!TILED && __all_sync(0xffffffffu, full && same_cls)) {
+        // whole blocks of BUILD_RB rows; both columns of every lane inside the matrix and on the same side of M_0 (all warps
+        // but the one that holds column M_0 - 1 when M_0 is odd, and the last one of a ragged matrix): one set of row constants
+        // per row, no clamp, no store predicate, the row pointer advanced by additions
+        double* p = A + (long long)t0 * lda + s0;
+        const bool kp = kap[0];
+        const int i0 = t0 - s0 - dmin;
+        const double2* kx = reinterpret_cast<const double2*>((i0 & 1) ? sK : sKB);    // rows with even r
+        const double2* ky = reinterpret_cast<const double2*>((i0 & 1) ? sKB : sK);    // rows with odd r
+        for (; tb + BUILD_RB <= t1; tb += BUILD_RB, p += BUILD_RB * lda) {
+            int m0 = 0x7fffffff, m1 = 0x7fffffff;
+#pragma unroll
+            for (int r = 0; r < BUILD_RB; ++r) {
+                const int i = tb - t0 + r;
+                const double2 te = sE[i];
+                const double2 uw = sUWa[i];
+                const double bt = sBa[i];
+                double e0 = bie_entry_fast_dagger_min(src[0], te, uw, bt, m0);
+                double e1 = bie_entry_fast_dagger_min(src[1], te, uw, bt, m1);
+                if (kp) {
+                    const double2 kv = ((r & 1) ? ky : kx)[(i0 + i) >> 1];
+                    e0 += kv.y; e1 += kv.x;
+                }
+                *reinterpret_cast<double2*>(p + (long long)r * lda) = make_double2(e0, e1);
+            }
+            const int flag = (m0 < src[0].thi) | (m1 < src[1].thi);
+            if (__any_sync(0xffffffffu, flag)) {
+                if (flag) bie_dagger_fix_near(nt, ct, src, col0, kap, sE, sK, dmin, t0, tb, tb + BUILD_RB, s0, ncols, A, lda, nchT, false, kappa != nullptr);
+            }
+        }
+    }
+    for (; tb < t1; tb += BUILD_RB) {
         int flag = 0;
         double* row = TILED ? A : A + (long long)tb * lda + s0;
 #pragma unroll
         for (int r = 0; r < BUILD_RB; ++r) {
             const int t = min(tb + r, t1 - 1);  // the tail repeats the last row (same values, same address)
             const double2 te = sE[t - t0];
-            const double2 bb = sBB[t - t0];
             const double2 uwa = sUWa[t - t0];
             const double2 uwb = same_cls ? uwa : sUWb[t - t0];   // both columns on the same side of M_0, almost always
-            double e0 = bie_entry_fast_dagger(src[0], te, uwa, col0[0] ? bb.x : bb.y, flag);
-            double e1 = bie_entry_fast_dagger(src[1], te, uwb, col0[1] ? bb.x : bb.y, flag);
+            double e0 = bie_entry_fast_dagger(src[0], te, uwa, sBa[t - t0], flag);
+            double e1 = bie_entry_fast_dagger(src[1], te, uwb, sBb[t - t0], flag);
             if (kap[0]) e0 += sK[t - s0 - dmin];
             if (kap[1]) e1 += sK[t - s0 - 1 - dmin];
             double* p = TILED ? A + bie_entry_off(0, nchT, t, s0) : row + (long long)(t - tb) * lda;
@@ -259,28 +381,7 @@ bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long
             else if (part) p[0] = e0;
         }
         if (__any_sync(0xffffffffu, flag)) {
-            if (flag) {
-                const int te_ = min(tb + BUILD_RB, t1);
-                for (int t = tb; t < te_; ++t) {
-                    const double2 te = sE[t - t0];
-#pragma unroll
-                    for (int c = 0; c < BUILD_COLS; ++c) {
-                        if (s0 + c >= ncols) continue;
-                        const double dr = src[c].er - te.x, di = src[c].ei - te.y;
-                        const double den = fma(dr, dr, di * di);
-                        if (__double2hiint(den) < src[c].thi) {
-                            const int k = nt.COMP[t];
-                            const double Mk = (double)(ct.off[k + 1] - ct.off[k]);
-                            const double2 q = nt.Q[t];
-                            const double2 ab = bie_dagger_ab(kappa != nullptr, k == 0, col0[c], q.x * Mk, q.y * Mk);
-                            // (A X' + B Y')/den with cot = (-2X + iY)/den; the diagonal entry is prepared per node
-                            double v = bie_entry_near(nt.DG, nt.XY, src[c].ms * ab.x, src[c].ms * ab.y, 0.0, s0 + c, t);
-                            if (kap[c]) v += sK[t - s0 - c - dmin];
-                            A[bie_entry_off(TILED ? 0 : lda, nchT, t, s0 + c)] = v;
-                        }
-                    }
-                }
-            }
+            if (flag) bie_dagger_fix_near(nt, ct, src, col0, kap, sE, sK, dmin, t0, tb, min(tb + BUILD_RB, t1), s0, ncols, A, lda, nchT, TILED, kappa != nullptr);
         }
     }
 }
@@ -307,7 +408,7 @@ int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int ncols, int nrows,
     // of the default (8192 CTAs = 11.07 waves of 740 at n = 16384) cost 16 % (profiles/r01b_ncu_full_cfg5.md)
     {
         int occ = 0;
-        if (dagger) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bie_build_dagger_kernel<false>, BUILD_THREADS, 64 * 256 + 8 * 512 + 16);
+        if (dagger) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bie_build_dagger_kernel<false>, BUILD_THREADS, bie_dagger_smem(256, ctx->variant == BIE_VARIANT_NORMAL_INTERNAL));
         else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bie_build_kernel<false>, BUILD_THREADS, 2 * 8 * 256 + 16);
         const long long wave = (long long)ctx->sm_count * (occ > 0 ? occ : 1);
         if ((long long)gx * ((nt_rows + 127) / 128) >= 2 * wave) {
@@ -323,7 +424,7 @@ int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int ncols, int nrows,
     const bool tiled = (lda == 0);
     const double* kap = ctx->variant == BIE_VARIANT_NORMAL_INTERNAL ? ctx->kappa : nullptr;
     if (dagger) {
-        const size_t sm = 4 * sizeof(double2) * T + (kap ? sizeof(double) * (T + BUILD_TILE_W) : 0) + 16;
+        const size_t sm = bie_dagger_smem(T, kap != nullptr);
         if (tiled) bie_build_dagger_kernel<true><<<grid, BUILD_THREADS, sm, st>>>(nt, ctx->comps, A, 0, T, only_comp0, ncols, nt_rows, kap);
         else bie_build_dagger_kernel<false><<<grid, BUILD_THREADS, sm, st>>>(nt, ctx->comps, A, (long long)lda, T, only_comp0, ncols, nt_rows, kap);
     } else {

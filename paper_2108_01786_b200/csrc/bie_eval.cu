@@ -30,9 +30,14 @@ struct EvalComps {
 #ifndef EVAL_NP
 #define EVAL_NP 2      // evaluation points per thread
 #endif
+#ifndef EVAL_UNROLL
+#define EVAL_UNROLL 2  // sources per unrolled step of the fast pass
+#endif
+constexpr int kEvalUnroll = EVAL_UNROLL;
+#define EVAL_RESIDENT 4   // CTAs per SM the register allocation must allow; eval_nseg() fills whole waves of them
 
 template <int NF>
-__global__ void __launch_bounds__(EVAL_THREADS)
+__global__ void __launch_bounds__(EVAL_THREADS, EVAL_RESIDENT)
 bie_cauchy_eval_kernel(EvalComps ec, int n, const double2* __restrict__ zeta, const double2* __restrict__ dzeta,
                        const double2* __restrict__ f, int npts, const double2* __restrict__ zpts, int nseg,
                        double2* __restrict__ part /* [nseg][1+NF][npts] */, int* __restrict__ hit /* [npts] */)
@@ -106,36 +111,28 @@ bie_cauchy_eval_kernel(EvalComps ec, int n, const double2* __restrict__ zeta, co
             }
         }
         __syncthreads();
-#pragma unroll 2
-        for (int j = 0; j < EVAL_TILE; ++j) {
+        // fast pass, branch-free: a near pair (rare) gets a ZERO reciprocal -- one select on the high word of the hardware
+        // approximation, which the refinement of bie_rcp3 carries through (e = 1, r0 (1 + e + e^2) = 0) -- and raises a flag
+        const int jn = min(EVAL_TILE, s_hi - s0);
+        int flag[EVAL_NP];
+#pragma unroll
+        for (int k = 0; k < EVAL_NP; ++k) flag[k] = 0;
+#pragma unroll kEvalUnroll
+        for (int j = 0; j < jn; ++j) {
             const double2 e = sE[j], A = sA[j];
             const int th = sTH[j];
 #pragma unroll
             for (int k = 0; k < EVAL_NP; ++k) {
                 const double dr = e.x - ter[k], di = e.y - tei[k];
                 const double den = fma(dr, dr, di * di);
-                const double r = bie_rcp3(den);
-                double u = dr * r, v = di * r;
-                if (__double2hiint(den) < th) {                // near pair (rare): from the coordinate differences
-                    const double2 zs = sXY[j], q = sQ[j];
-                    const double x = zs.x - z[k].x, y = zs.y - z[k].y;
-                    u = 0.0; v = 0.0;
-                    // exact coincidence (modulo the period): cot has a pole, (F.4) degenerates to f_s
-                    const double xr = x - 6.283185307179586232 * rint(x * 0.15915494309189534561);
-                    if (xr == 0.0 && y == 0.0) myhit[k] = s0 + j;
-                    else {
-                        double cr, ci;
-                        bie_cot_half_near(x, y, &cr, &ci);
-                        ci += 1.0;                             // + i q_s: the constant below is subtracted for EVERY source
-                        const double wr = q.x * cr - q.y * ci, wi = q.x * ci + q.y * cr;
-                        Dr[k] += wr; Di[k] += wi;
-#pragma unroll
-                        for (int c = 0; c < NF; ++c) {
-                            const double2 fv = f[(size_t)c * n + s0 + j];
-                            Nr[k][c] += wr * fv.x - wi * fv.y; Ni[k][c] += wr * fv.y + wi * fv.x;
-                        }
-                    }
-                }
+                const bool near = __double2hiint(den) < th;
+                flag[k] |= near ? 1 : 0;
+                double r0;
+                asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r0) : "d"(den));
+                r0 = __hiloint2double(near ? 0 : __double2hiint(r0), 0);   // the approximation has a zero low word
+                const double er_ = fma(-den, r0, 1.0);
+                const double r = fma(r0, fma(er_, er_, er_), r0);
+                const double u = dr * r, v = di * r;
                 Dr[k] = fma(A.x, u, Dr[k]); Dr[k] = fma(A.y, v, Dr[k]);
                 Di[k] = fma(A.y, u, Di[k]); Di[k] = fma(-A.x, v, Di[k]);
 #pragma unroll
@@ -143,6 +140,32 @@ bie_cauchy_eval_kernel(EvalComps ec, int n, const double2* __restrict__ zeta, co
                     const double2 g = sG[c][j];
                     Nr[k][c] = fma(g.x, u, Nr[k][c]); Nr[k][c] = fma(g.y, v, Nr[k][c]);
                     Ni[k][c] = fma(g.y, u, Ni[k][c]); Ni[k][c] = fma(-g.x, v, Ni[k][c]);
+                }
+            }
+        }
+        // near pairs of this tile (threads that saw one revisit the tile): from the coordinate differences
+#pragma unroll
+        for (int k = 0; k < EVAL_NP; ++k) {
+            if (!flag[k]) continue;
+            for (int j = 0; j < jn; ++j) {
+                const double2 e = sE[j];
+                const double dr = e.x - ter[k], di = e.y - tei[k];
+                const double den = fma(dr, dr, di * di);          // the same bits as in the fast pass
+                if (__double2hiint(den) >= sTH[j]) continue;
+                const double2 zs = sXY[j], q = sQ[j];
+                const double x = zs.x - z[k].x, y = zs.y - z[k].y;
+                // exact coincidence (modulo the period): cot has a pole, (F.4) degenerates to f_s
+                const double xr = x - 6.283185307179586232 * rint(x * 0.15915494309189534561);
+                if (xr == 0.0 && y == 0.0) { myhit[k] = s0 + j; continue; }
+                double cr, ci;
+                bie_cot_half_near(x, y, &cr, &ci);
+                ci += 1.0;                             // + i q_s: the constant below is subtracted for EVERY source
+                const double wr = q.x * cr - q.y * ci, wi = q.x * ci + q.y * cr;
+                Dr[k] += wr; Di[k] += wi;
+#pragma unroll
+                for (int c = 0; c < NF; ++c) {
+                    const double2 fv = f[(size_t)c * n + s0 + j];
+                    Nr[k][c] += wr * fv.x - wi * fv.y; Ni[k][c] += wr * fv.y + wi * fv.x;
                 }
             }
         }
@@ -201,13 +224,29 @@ bie_cauchy_finish_kernel(int nf, int n, int npts, int nseg, const double2* __res
     }
 }
 
+// Source segments (blockIdx.y).  All CTAs take equally long (points per CTA x sources per segment), so the grid of
+// gx x nseg CTAs should fill whole waves of sm_count x EVAL_RESIDENT resident CTAs: with the former rule (just enough CTAs
+// for four per SM) 65 536 points gave 768 CTAs = 1.3 waves.  Smallest nseg that gives at least one wave and wastes < 3 %
+// of the last one, else the best of 1 .. 64.
+static int eval_nseg(int npts, int sm_count)
+{
+    const int gx = (npts + EVAL_THREADS * EVAL_NP - 1) / (EVAL_THREADS * EVAL_NP);
+    const long long wave = (long long)sm_count * EVAL_RESIDENT;
+    int best = 1;
+    double best_eff = 0.0;
+    for (int s = 1; s <= 64; ++s) {
+        const long long units = (long long)gx * s;
+        const double eff = (double)units / (double)(((units + wave - 1) / wave) * wave);
+        if (units >= wave && eff >= 0.97) return s;
+        if (eff > best_eff + 1e-9) { best_eff = eff; best = s; }
+    }
+    return best;
+}
+
 size_t bie_cauchy_eval_ws_bytes(int nf, int npts, int sm_count)
 {
     if (nf < 1 || nf > EVAL_MAX_NF || npts < 1) return 0;
-    const int gx = (npts + EVAL_THREADS * EVAL_NP - 1) / (EVAL_THREADS * EVAL_NP);
-    int nseg = (4 * sm_count + gx - 1) / gx;
-    if (nseg < 1) nseg = 1;
-    if (nseg > 64) nseg = 64;
+    const int nseg = eval_nseg(npts, sm_count);
     return sizeof(double2) * (size_t)nseg * (1 + nf) * npts + sizeof(int) * (size_t)npts + 256;
 }
 
@@ -230,9 +269,7 @@ int bie_launch_cauchy_eval(bie_ctx* ctx, int ncomp, const int32_t* counts, const
     if ((((uintptr_t)zeta) | ((uintptr_t)dzeta) | ((uintptr_t)fvals) | ((uintptr_t)zpts) | ((uintptr_t)out)) & 15u) return BIE_ERR_LAYOUT;
     if (bie_cauchy_eval_ws_bytes(nf, npts, ctx->sm_count) > ws_bytes) return BIE_ERR_WORKSPACE;
     const int gx = (npts + EVAL_THREADS * EVAL_NP - 1) / (EVAL_THREADS * EVAL_NP);
-    int nseg = (4 * ctx->sm_count + gx - 1) / gx;
-    if (nseg < 1) nseg = 1;
-    if (nseg > 64) nseg = 64;
+    int nseg = eval_nseg(npts, ctx->sm_count);
     if (nseg > (int)((n + 1) / 2)) nseg = (int)((n + 1) / 2);
     double2* part = (double2*)(((uintptr_t)ws + 255) & ~(uintptr_t)255);
     int* hit = (int*)(part + (size_t)nseg * (1 + nf) * npts);
