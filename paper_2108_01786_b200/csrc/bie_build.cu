@@ -22,12 +22,28 @@
 #define BUILD_THREADS 128
 #define BUILD_COLS 2
 #define BUILD_TILE_W (BUILD_THREADS * BUILD_COLS)
+#ifndef BUILD_RB
 #define BUILD_RB 4
+#endif
 #ifndef BUILD_MIN_CTAS
 #define BUILD_MIN_CTAS 4      // CTAs of 128 threads per SM the register allocation must allow.  Measured at config 5 (0.411 ms at 4):
                               // 5 -> 0.414, 6 -> 0.448, 8 -> 0.487 ms: the kernel wants its registers, not more warps; and
                               // FEWER resident CTAs (shared-memory padding to 3 / 2 per SM) are slower too: 0.45 / 0.55 ms
 #endif
+
+// Tile of CTA L of the one-dimensional grid.  The tiles that hold the diagonal go FIRST (two per block of T rows: the
+// tile columns that the rows [t0, t0 + T) can meet, T <= 256): their near entries take the slow path, which makes
+// such a CTA several times slower than the others -- in launch order the ones of the last wave finished 50 us after
+// everything else at n = 16384 (0.41 ms with them anywhere, 0.35 ms without the near path; measured).  The other tiles
+// keep the row-major order (x fastest), so that concurrently running CTAs write the same rows.
+__device__ __forceinline__ void bie_build_tile(int L, int gx, int gy, int T, int& bx, int& by)
+{
+    if (gx < 3) { bx = L % gx; by = L / gx; return; }
+    int j;
+    if (L < 2 * gy) { by = L >> 1; j = L & 1; }
+    else { const int r = L - 2 * gy; by = r / (gx - 2); j = 2 + r % (gx - 2); }
+    bx = (int)(((long long)by * T / BUILD_TILE_W + j) % gx);
+}
 
 struct SrcCol {
     double er, ei;      // E_s
@@ -100,11 +116,13 @@ static __device__ __forceinline__ void bie_build_fix_near(const NodeTable& nt, c
 // TILED: A is the block format of the hybrid operator (bie_common.cuh) instead of row-major with leading dimension lda
 template <bool TILED>
 __global__ void __launch_bounds__(BUILD_THREADS, BUILD_MIN_CTAS)
-bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long lda, int T, int only0, int ncols, int nrows)
+bie_build_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long lda, int T, int only0, int ncols, int nrows, int gx, int gy)
 {
     extern __shared__ __align__(16) double2 sm[];  // [T] E_t
-    const int c0 = blockIdx.x * BUILD_TILE_W;
-    const int t0 = blockIdx.y * T;
+    int bx, by;
+    bie_build_tile(blockIdx.x, gx, gy, T, bx, by);
+    const int c0 = bx * BUILD_TILE_W;
+    const int t0 = by * T;
     const int t1 = min(t0 + T, nrows);      // nrows = n, or the rows of the hybrid operator's block
     if (only0 && t0 >= ct.off[1] && c0 >= ct.off[1]) return;  // a4: solid-solid tiles stay
     double2* sE = sm;
@@ -265,13 +283,15 @@ static inline size_t bie_dagger_smem(int T, bool kap)
 template <bool TILED>
 __global__ void __launch_bounds__(BUILD_THREADS)
 bie_build_dagger_kernel(NodeTable nt, CompTable ct, double* __restrict__ A, long long lda, int T, int only0, int ncols, int nrows,
-                        const double* __restrict__ kappa /* NULL: vortex-sheet S; else the normal-velocity operator */)
+                        const double* __restrict__ kappa /* NULL: vortex-sheet S; else the normal-velocity operator */, int gx, int gy)
 {
     // [T] E_t, [T] (U,W) for columns on Gamma_0, [T] (U,W) for solids, [T] B for Gamma_0 columns, [T] B for solids,
     // [T + 256] kappa (KA), [T + 258] kappa shifted by one (KB[x] = KA[x - 1])
     extern __shared__ __align__(16) double2 sm[];
-    const int c0 = blockIdx.x * BUILD_TILE_W;
-    const int t0 = blockIdx.y * T;
+    int bx, by;
+    bie_build_tile(blockIdx.x, gx, gy, T, bx, by);
+    const int c0 = bx * BUILD_TILE_W;
+    const int t0 = by * T;
     const int t1 = min(t0 + T, nrows);   // n; M_0 for the normal-velocity operator (rows on Gamma_0 only); the block's rows
     if (only0 && t0 >= ct.off[1] && c0 >= ct.off[1]) return;
     double2* sE = sm;
@@ -420,17 +440,18 @@ int bie_launch_build(bie_ctx* ctx, double* A, int64_t lda, int ncols, int nrows,
             }
         }
     }
-    dim3 grid(gx, (nt_rows + T - 1) / T);
+    const int gy = (nt_rows + T - 1) / T;
+    const unsigned grid = (unsigned)gx * (unsigned)gy;     // one-dimensional: bie_build_tile orders the tiles
     const bool tiled = (lda == 0);
     const double* kap = ctx->variant == BIE_VARIANT_NORMAL_INTERNAL ? ctx->kappa : nullptr;
     if (dagger) {
         const size_t sm = bie_dagger_smem(T, kap != nullptr);
-        if (tiled) bie_build_dagger_kernel<true><<<grid, BUILD_THREADS, sm, st>>>(nt, ctx->comps, A, 0, T, only_comp0, ncols, nt_rows, kap);
-        else bie_build_dagger_kernel<false><<<grid, BUILD_THREADS, sm, st>>>(nt, ctx->comps, A, (long long)lda, T, only_comp0, ncols, nt_rows, kap);
+        if (tiled) bie_build_dagger_kernel<true><<<grid, BUILD_THREADS, sm, st>>>(nt, ctx->comps, A, 0, T, only_comp0, ncols, nt_rows, kap, gx, gy);
+        else bie_build_dagger_kernel<false><<<grid, BUILD_THREADS, sm, st>>>(nt, ctx->comps, A, (long long)lda, T, only_comp0, ncols, nt_rows, kap, gx, gy);
     } else {
         const size_t sm = sizeof(double2) * T + 16;
-        if (tiled) bie_build_kernel<true><<<grid, BUILD_THREADS, sm, st>>>(nt, ctx->comps, A, 0, T, only_comp0, ncols, nt_rows);
-        else bie_build_kernel<false><<<grid, BUILD_THREADS, sm, st>>>(nt, ctx->comps, A, (long long)lda, T, only_comp0, ncols, nt_rows);
+        if (tiled) bie_build_kernel<true><<<grid, BUILD_THREADS, sm, st>>>(nt, ctx->comps, A, 0, T, only_comp0, ncols, nt_rows, gx, gy);
+        else bie_build_kernel<false><<<grid, BUILD_THREADS, sm, st>>>(nt, ctx->comps, A, (long long)lda, T, only_comp0, ncols, nt_rows, gx, gy);
     }
     BIE_CUDA(cudaGetLastError());
     return BIE_OK;

@@ -9,8 +9,8 @@
 // so with u = dr/den, v = di/den every complex sum (the denominator and the nf numerators, whose source constant is A_s f_s)
 // costs 4 FMAs per pair:  Re += Ar u + Ai v,  Im += Ai u - Ar v;  the constants -i sum_s q_s (f_s) are added per source tile by
 // one thread.  Per pair: 2 sub, 2 den, 3 reciprocal, 2 for (u, v), 4 per sum = 9 + 4 (1 + nf) FP64 instructions (12 + 4 (1 + nf)
-// with the (X, Y) form of round 1).  Two evaluation points per thread share every shared-memory load.
-// One thread per two evaluation points, the sources staged tile by tile in shared memory with E_s, the near threshold and
+// with the (X, Y) form of round 1).  Three or four evaluation points per thread share every shared-memory load (eval_np);
+// the sources are staged tile by tile in shared memory with E_s, the near threshold and
 // A_s, A_s f_s.  Pairs closer than the near threshold are recomputed from the coordinate differences
 // with the Laurent series (exact to rounding at any distance, which is the whole point of (F.4)); an exact coincidence
 // is recorded and resolved in the second kernel, which also adds the partial sums of the source segments (few points:
@@ -27,16 +27,19 @@ struct EvalComps {
     int surface[BIE_MAX_COMP];   // 1: sigma = -1
 };
 
-#ifndef EVAL_NP
-#define EVAL_NP 2      // evaluation points per thread
-#endif
+// evaluation points per thread (they share every shared-memory load): measured at 65 536 points x 16 384 sources, as a share of
+// the probed FP64 rate, (points, resident CTAs) = (2, 4) / (4, 3) / (3, 3): nf = 1 0.68 / 0.71 / 0.68, nf = 2 0.67 / 0.72 / 0.67,
+// nf = 4 0.70 / 0.69 / 0.71
+static inline int eval_np(int nf) { return nf <= 2 ? 4 : 3; }
 #ifndef EVAL_UNROLL
 #define EVAL_UNROLL 2  // sources per unrolled step of the fast pass
 #endif
 constexpr int kEvalUnroll = EVAL_UNROLL;
-#define EVAL_RESIDENT 4   // CTAs per SM the register allocation must allow; eval_nseg() fills whole waves of them
+#ifndef EVAL_RESIDENT
+#define EVAL_RESIDENT 3   // CTAs per SM the register allocation must allow; eval_nseg() fills whole waves of them
+#endif
 
-template <int NF>
+template <int NF, int EVAL_NP>
 __global__ void __launch_bounds__(EVAL_THREADS, EVAL_RESIDENT)
 bie_cauchy_eval_kernel(EvalComps ec, int n, const double2* __restrict__ zeta, const double2* __restrict__ dzeta,
                        const double2* __restrict__ f, int npts, const double2* __restrict__ zpts, int nseg,
@@ -228,9 +231,9 @@ bie_cauchy_finish_kernel(int nf, int n, int npts, int nseg, const double2* __res
 // gx x nseg CTAs should fill whole waves of sm_count x EVAL_RESIDENT resident CTAs: with the former rule (just enough CTAs
 // for four per SM) 65 536 points gave 768 CTAs = 1.3 waves.  Smallest nseg that gives at least one wave and wastes < 3 %
 // of the last one, else the best of 1 .. 64.
-static int eval_nseg(int npts, int sm_count)
+static int eval_nseg(int nf, int npts, int sm_count)
 {
-    const int gx = (npts + EVAL_THREADS * EVAL_NP - 1) / (EVAL_THREADS * EVAL_NP);
+    const int gx = (npts + EVAL_THREADS * eval_np(nf) - 1) / (EVAL_THREADS * eval_np(nf));
     const long long wave = (long long)sm_count * EVAL_RESIDENT;
     int best = 1;
     double best_eff = 0.0;
@@ -246,7 +249,7 @@ static int eval_nseg(int npts, int sm_count)
 size_t bie_cauchy_eval_ws_bytes(int nf, int npts, int sm_count)
 {
     if (nf < 1 || nf > EVAL_MAX_NF || npts < 1) return 0;
-    const int nseg = eval_nseg(npts, sm_count);
+    const int nseg = eval_nseg(nf, npts, sm_count);
     return sizeof(double2) * (size_t)nseg * (1 + nf) * npts + sizeof(int) * (size_t)npts + 256;
 }
 
@@ -268,8 +271,8 @@ int bie_launch_cauchy_eval(bie_ctx* ctx, int ncomp, const int32_t* counts, const
     if (n > (1 << 30)) return BIE_ERR_GEOMETRY;
     if ((((uintptr_t)zeta) | ((uintptr_t)dzeta) | ((uintptr_t)fvals) | ((uintptr_t)zpts) | ((uintptr_t)out)) & 15u) return BIE_ERR_LAYOUT;
     if (bie_cauchy_eval_ws_bytes(nf, npts, ctx->sm_count) > ws_bytes) return BIE_ERR_WORKSPACE;
-    const int gx = (npts + EVAL_THREADS * EVAL_NP - 1) / (EVAL_THREADS * EVAL_NP);
-    int nseg = eval_nseg(npts, ctx->sm_count);
+    const int gx = (npts + EVAL_THREADS * eval_np(nf) - 1) / (EVAL_THREADS * eval_np(nf));
+    int nseg = eval_nseg(nf, npts, ctx->sm_count);
     if (nseg > (int)((n + 1) / 2)) nseg = (int)((n + 1) / 2);
     double2* part = (double2*)(((uintptr_t)ws + 255) & ~(uintptr_t)255);
     int* hit = (int*)(part + (size_t)nseg * (1 + nf) * npts);
@@ -277,10 +280,10 @@ int bie_launch_cauchy_eval(bie_ctx* ctx, int ncomp, const int32_t* counts, const
     dim3 grid(gx, nseg);
     const double2 *z2 = (const double2*)zeta, *d2 = (const double2*)dzeta, *f2 = (const double2*)fvals, *p2 = (const double2*)zpts;
     switch (nf) {
-        case 1: bie_cauchy_eval_kernel<1><<<grid, EVAL_THREADS, 0, st>>>(ec, (int)n, z2, d2, f2, npts, p2, nseg, part, hit); break;
-        case 2: bie_cauchy_eval_kernel<2><<<grid, EVAL_THREADS, 0, st>>>(ec, (int)n, z2, d2, f2, npts, p2, nseg, part, hit); break;
-        case 3: bie_cauchy_eval_kernel<3><<<grid, EVAL_THREADS, 0, st>>>(ec, (int)n, z2, d2, f2, npts, p2, nseg, part, hit); break;
-        default: bie_cauchy_eval_kernel<4><<<grid, EVAL_THREADS, 0, st>>>(ec, (int)n, z2, d2, f2, npts, p2, nseg, part, hit); break;
+        case 1: bie_cauchy_eval_kernel<1, 4><<<grid, EVAL_THREADS, 0, st>>>(ec, (int)n, z2, d2, f2, npts, p2, nseg, part, hit); break;
+        case 2: bie_cauchy_eval_kernel<2, 4><<<grid, EVAL_THREADS, 0, st>>>(ec, (int)n, z2, d2, f2, npts, p2, nseg, part, hit); break;
+        case 3: bie_cauchy_eval_kernel<3, 3><<<grid, EVAL_THREADS, 0, st>>>(ec, (int)n, z2, d2, f2, npts, p2, nseg, part, hit); break;
+        default: bie_cauchy_eval_kernel<4, 3><<<grid, EVAL_THREADS, 0, st>>>(ec, (int)n, z2, d2, f2, npts, p2, nseg, part, hit); break;
     }
     bie_cauchy_finish_kernel<<<(npts + 255) / 256, 256, 0, st>>>(nf, (int)n, npts, nseg, part, hit, f2, (double2*)out);
     BIE_CUDA(cudaGetLastError());
