@@ -730,6 +730,13 @@ int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, int nd, 
     // align the caller's workspace to 256 bytes
     uintptr_t base = ((uintptr_t)ws + 255) & ~(uintptr_t)255;
     if (base - (uintptr_t)ws + pl.total > ws_bytes) return BIE_ERR_WORKSPACE;
+    if (mode == 0) {
+        // small stored-matrix systems: one thread-block cluster, cluster barriers and distributed shared memory
+        // instead of grid barriers and L2 (bie_gmres_cluster.cu); same workspace layout
+        rc = bie_launch_gmres_cluster(ctx, n, A, lda, rhs, tol, restart, max_iters, x, iters_out, relres_out, status_out, res_hist,
+                                      (double*)(base + pl.offV), pl.nld, (double*)(base + pl.offR), st);
+        if (rc != BIE_CLUSTER_NOT_TAKEN) return rc;
+    }
     a.A = A; a.lda = lda; a.n = n; a.b = rhs; a.tol = tol; a.m = restart; a.max_iters = max_iters;
     a.x = x; a.iters_out = iters_out; a.relres_out = relres_out; a.status_out = status_out; a.res_hist = res_hist;
     a.V = (double*)(base + pl.offV);

@@ -759,14 +759,14 @@ def check_iters(it, ito, case=None, band=None):
         assert abs(it - ito) <= 1, (case, it, ito)
 
 
-def gpu_gmres(ctx, A, b, tol, restart, max_iters=1000):
+def gpu_gmres(ctx, A, b, tol, restart, max_iters=1000, lda=None):
     from paper_2108_01786_b200 import bie
     n = b.size
     ws = torch.empty(bie.Context.bie_gmres_workspace_bytes(n, restart), dtype=torch.uint8, device="cuda")
     oi = torch.full((2,), -7, dtype=torch.int32, device="cuda")
     of = torch.full((1,), -7.0, dtype=torch.float64, device="cuda")
     x = torch.empty(n + (n & 1), dtype=torch.float64, device="cuda")
-    ctx.bie_gmres(A, dev(b), x[:n], tol, restart, max_iters, ws, oi, of)
+    ctx.bie_gmres(A, dev(b), x[:n], tol, restart, max_iters, ws, oi, of, lda=lda)
     torch.cuda.synchronize()
     return x[:n].cpu().numpy(), int(oi[0]), float(of[0]), int(oi[1])
 
@@ -949,7 +949,48 @@ def test_gmres_restart_and_iteration_cap(ctx):
     assert abs(rr - rro) <= 1e-6 * rro
 
 
-def test_gmres_degenerate_cases(ctx):
+@pytest.mark.parametrize("cluster", [1, 0])
+@pytest.mark.parametrize("n,lda,restart", [(640, 640, 50), (37, 40, 50), (301, 302, 7), (600, 608, 20), (16, 16, 4), (5, 6, 50)])
+def test_gmres_small_systems_cluster_and_grid_kernels(ctx, n, lda, restart, cluster):
+    """stored-matrix solves up to n = 640 run on one thread-block cluster (bie_gmres_cluster.cu) unless bie_set_cluster_gmres(0);
+    both kernels against the oracle: odd n, lda > n, fewer rows than CTAs, several restart cycles, the iteration cap"""
+    rng = np.random.default_rng(1000 + n)
+    if n == 640:
+        P = cfg(1)
+        Ao, b = oracle_build(P.geometry), P.rhs[0]
+    else:
+        Ao = 0.5 * np.eye(n) + rng.standard_normal((n, n)) * (0.3 / np.sqrt(n))
+        b = rng.standard_normal(n)
+    Ad = torch.full((n, lda), 7.0, dtype=torch.float64, device="cuda")
+    Ad[:, :n] = dev(Ao)
+    ctx.bie_set_cluster_gmres(cluster)
+    try:
+        xo, ito, rro, _, sto = oracle.gmres(Ao, b, 1e-13, restart, 1000)
+        x, it, rr, st = gpu_gmres(ctx, Ad, b, 1e-13, restart, 1000, lda=lda)
+        assert (st, sto) == (0, 0) and abs(it - ito) <= 1, (it, ito)
+        assert np.linalg.norm(x - xo) / np.linalg.norm(xo) <= TOL_X
+        assert rr <= 1e-12
+        x2, it2, rr2, st2 = gpu_gmres(ctx, Ad, b, 1e-13, restart, 1000, lda=lda)      # deterministic: the same bits again
+        assert it2 == it and np.array_equal(x, x2) and rr2 == rr
+        cap = max(1, ito // 2)
+        xo, ito, rro, _, sto = oracle.gmres(Ao, b, 1e-13, restart, cap)
+        x, it, rr, st = gpu_gmres(ctx, Ad, b, 1e-13, restart, cap, lda=lda)
+        assert (sto, ito) == (1, cap) and (st, it) == (1, cap)
+        assert np.linalg.norm(x - xo) / np.linalg.norm(xo) <= 1e-9 and abs(rr - rro) <= 1e-6 * rro
+    finally:
+        ctx.bie_set_cluster_gmres(1)
+
+
+@pytest.mark.parametrize("cluster", [1, 0])
+def test_gmres_degenerate_cases(ctx, cluster):
+    ctx.bie_set_cluster_gmres(cluster)
+    try:
+        _gmres_degenerate_cases(ctx)
+    finally:
+        ctx.bie_set_cluster_gmres(1)
+
+
+def _gmres_degenerate_cases(ctx):
     rng = np.random.default_rng(0)
     # zero right-hand side: x = 0, 0 iterations
     A = np.eye(6) + 0.1 * rng.standard_normal((6, 6))
