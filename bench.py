@@ -437,6 +437,18 @@ def measure_config(torch, bie, ctx, c, timer, dfma_per_s):
         r.update({"iters_last_stage": it, "status": st, "relres_true": rr,
                   "us_per_iter_median": r["median_ms"] * 1e3 / max(1, it * len(P.stages))})
         steps[op] = r
+    if n <= 1024 and "dense" in steps:
+        # small stored-matrix solves run on one thread-block cluster when the rows of A fit its shared memory (bie_gmres_cluster.cu);
+        # the grid-wide kernel on the same system, for comparison
+        ctx.bie_set_cluster_gmres(0)
+        r = timer(lambda: W.step("dense"), 10)
+        ctx.bie_set_cluster_gmres(1)
+        it, st, rr = W.result()
+        r.update({"iters_last_stage": it, "status": st, "relres_true": rr,
+                  "us_per_iter_median": r["median_ms"] * 1e3 / max(1, it * len(P.stages))})
+        out["dense_grid_wide_kernel"] = r
+        out["dense_solver_note"] = ("`dense` ran on one thread-block cluster when all but four rows of A per CTA fit the cluster's shared "
+                                    "memory (n <= 640), else on the grid-wide kernel; `dense_grid_wide_kernel` is the latter, forced")
     best = min(steps, key=lambda k: steps[k]["median_ms"])
     out["step"] = steps
     out["operator_chosen"] = best

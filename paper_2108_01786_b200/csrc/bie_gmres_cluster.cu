@@ -27,6 +27,7 @@ namespace cg = cooperative_groups;
 #ifdef BIE_PHASE_TIMING   // developer build: CTA 0 prints the mean time per Arnoldi step of each phase
 #include <cstdio>
 __device__ __forceinline__ unsigned long long cl_gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+__device__ unsigned long long g_gemv_t[4];
 #define CPT_DECL __shared__ unsigned long long cpt[16]; __shared__ unsigned long long cpt0; if (threadIdx.x == 0) { for (int q_ = 0; q_ < 16; ++q_) cpt[q_] = 0; cpt0 = cl_gtime(); }
 #define CPT(i) { if (threadIdx.x == 0) { const unsigned long long t_ = cl_gtime(); cpt[i] += t_ - cpt0; cpt0 = t_; } }
 #else
@@ -194,6 +195,9 @@ __device__ __forceinline__ void cl_gemv(const ClusterCtx& c, const ClusterArgs& 
             if (lane == 0) gpart[q * CL_WARPS + warp] = s;
         }
     };
+#ifdef BIE_PHASE_TIMING
+    const unsigned long long tg0 = cl_gtime();
+#endif
     if (ng > 0) issue(0);
     // up to CL_RW rows of a warp together: one load of the x pair serves them all (the shared-memory bandwidth, 128 B per
     // clock, is what bounds this loop), and their lane reductions overlap
@@ -221,6 +225,10 @@ __device__ __forceinline__ void cl_gemv(const ClusterCtx& c, const ClusterArgs& 
             if (lane == 0 && r < nsm) y[r] = t;
         }
     }
+#ifdef BIE_PHASE_TIMING
+    __syncthreads();
+    if (threadIdx.x == 0) g_gemv_t[0] += cl_gtime() - tg0;
+#endif
     for (int g0 = 0; g0 < ng; g0 += CL_GB) {
         consume(g0);
         __syncthreads();
@@ -498,6 +506,7 @@ __global__ void __launch_bounds__(CL_THREADS, 1) bie_gmres_cluster_kernel(const 
                "allreduce2 %.2f | combine2 + v %.2f | allgather + Givens %.2f | barrier3 %.2f | rest %.2f\n", iters, cpt[0] * 1e-3, cpt[1] * 1e-3,
                cpt[2] * 1e-3 / iters, cpt[3] * 1e-3 / iters, cpt[4] * 1e-3 / iters, cpt[5] * 1e-3 / iters, cpt[6] * 1e-3 / iters, cpt[7] * 1e-3 / iters,
                cpt[8] * 1e-3 / iters, cpt[9] * 1e-3 / iters, cpt[10] * 1e-3 / iters, cpt[11] * 1e-3 / iters);
+    if (c.rank == 0 && threadIdx.x == 0 && iters > 0) { printf("   gemv: shared-memory rows %.2f us per call\n", g_gemv_t[0] * 1e-3 / (iters + 1)); g_gemv_t[0] = 0; }
     if (c.rank == 0 && threadIdx.x == 0 && iters > 0) printf("   ss %.2f | combine2 %.2f | hn %.2f\n", cpt[12] * 1e-3 / iters, cpt[13] * 1e-3 / iters, cpt[14] * 1e-3 / iters);
 #endif
     if (c.rank == 0 && threadIdx.x == 0) {
