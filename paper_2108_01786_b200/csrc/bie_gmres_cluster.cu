@@ -24,16 +24,6 @@
 
 namespace cg = cooperative_groups;
 
-#ifdef BIE_PHASE_TIMING   // developer build: CTA 0 prints the mean time per Arnoldi step of each phase
-#include <cstdio>
-__device__ __forceinline__ unsigned long long cl_gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-__device__ unsigned long long g_gemv_t[4];
-#define CPT_DECL __shared__ unsigned long long cpt[16]; __shared__ unsigned long long cpt0; if (threadIdx.x == 0) { for (int q_ = 0; q_ < 16; ++q_) cpt[q_] = 0; cpt0 = cl_gtime(); }
-#define CPT(i) { if (threadIdx.x == 0) { const unsigned long long t_ = cl_gtime(); cpt[i] += t_ - cpt0; cpt0 = t_; } }
-#else
-#define CPT_DECL
-#define CPT(i)
-#endif
 
 #define CL_THREADS 512
 #define CL_WARPS (CL_THREADS / 32)
@@ -195,9 +185,6 @@ __device__ __forceinline__ void cl_gemv(const ClusterCtx& c, const ClusterArgs& 
             if (lane == 0) gpart[q * CL_WARPS + warp] = s;
         }
     };
-#ifdef BIE_PHASE_TIMING
-    const unsigned long long tg0 = cl_gtime();
-#endif
     if (ng > 0) issue(0);
     // up to CL_RW rows of a warp together: one load of the x pair serves them all (the shared-memory bandwidth, 128 B per
     // clock, is what bounds this loop), and their lane reductions overlap
@@ -225,10 +212,6 @@ __device__ __forceinline__ void cl_gemv(const ClusterCtx& c, const ClusterArgs& 
             if (lane == 0 && r < nsm) y[r] = t;
         }
     }
-#ifdef BIE_PHASE_TIMING
-    __syncthreads();
-    if (threadIdx.x == 0) g_gemv_t[0] += cl_gtime() - tg0;
-#endif
     for (int g0 = 0; g0 < ng; g0 += CL_GB) {
         consume(g0);
         __syncthreads();
@@ -303,7 +286,6 @@ __global__ void __launch_bounds__(CL_THREADS, 1) bie_gmres_cluster_kernel(const 
     double* dl = smem + c.L.dl;  double* hloc = smem + c.L.hloc;  double* hcol = smem + c.L.hcol;
     double* cs = smem + c.L.cs;  double* sn = smem + c.L.sn;  double* g = smem + c.L.g;  double* red = smem + c.L.red;
     __shared__ double comb[CL_THREADS];
-    CPT_DECL
 
     // ---- this CTA's rows of A -> shared memory ----------------------------------------------------------------
     {
@@ -317,7 +299,6 @@ __global__ void __launch_bounds__(CL_THREADS, 1) bie_gmres_cluster_kernel(const 
         }
     }
     __syncthreads();
-    CPT(0)
     // ---- a5: ||b||, x = 0 ---------------------------------------------------------------------------------------
     double p = 0.0;
     for (int r = threadIdx.x; r < rows; r += CL_THREADS) {
@@ -374,29 +355,20 @@ __global__ void __launch_bounds__(CL_THREADS, 1) bie_gmres_cluster_kernel(const 
         // ---- Arnoldi steps ------------------------------------------------------------------------------------------
         int k = 0;
         bool conv = false;
-        CPT(1)
         for (int j = 0; j < m; ++j) {
             cl_gemv(c, a, y, comb);                                              // a6: y = A v_j
-            CPT(2)
             // a7, first pass: s = V_j^T y, w1 = y - V_j s
             cl_local_dots(c, a, j + 1, y, dl, false);
-            CPT(3)
             cl_allreduce(c, dl, j + 1, hloc);
-            CPT(4)
             for (int i = threadIdx.x; i <= j; i += CL_THREADS) hcol[i] = hloc[i];
             for (int r = threadIdx.x; r < rows; r += CL_THREADS) w[r] = y[r];
             __syncthreads();
             cl_subtract_combination(c, a, j + 1, hloc, w, comb);
-            CPT(5)
             // second pass: h2 = V_j^T w1 and ||w1||^2 in one reduction
             cl_local_dots(c, a, j + 1, w, dl, true);
-            CPT(6)
             cl_allreduce(c, dl, j + 2, hloc, red + 34);                   // red[34] = ||h2||^2
-            CPT(7)
             const double nu = hloc[j + 1], ss = red[34];
-            CPT(12)
             cl_subtract_combination(c, a, j + 1, hloc, w, comb);         // w2 = w1 - V_j h2
-            CPT(13)
             double hn;
             if (ss <= 0.01 * nu) {                                         // identical in every CTA (same bits)
                 hn = sqrt(nu - ss);                                        // Pythagoras: no cancellation, ss << nu
@@ -409,7 +381,6 @@ __global__ void __launch_bounds__(CL_THREADS, 1) bie_gmres_cluster_kernel(const 
                 cl_allreduce(c, dl, 1, red + 36);
                 hn = sqrt(red[36]);
             }
-            CPT(14)
             for (int i = threadIdx.x; i <= j; i += CL_THREADS) hcol[i] += hloc[i];
             {
                 const double inv = (hn != 0.0) ? 1.0 / hn : 0.0;
@@ -417,7 +388,6 @@ __global__ void __launch_bounds__(CL_THREADS, 1) bie_gmres_cluster_kernel(const 
                 for (int r = threadIdx.x; r < rows; r += CL_THREADS) { const double v = w[r] * inv; vn[r] = v; w[r] = v; }
             }
             __syncthreads();
-            CPT(8)
             cl_allgather_rows(c, w);                                       // v_{j+1} -> xs of every CTA
             __syncthreads();
             cg_cluster_arrive();                                           // barrier 3, split: the Givens sweep runs while it completes
@@ -438,10 +408,8 @@ __global__ void __launch_bounds__(CL_THREADS, 1) bie_gmres_cluster_kernel(const 
                 g[j + 1] = -sn[j] * g[j];
                 g[j] = cs[j] * g[j];
             }
-            CPT(9)
             cg_cluster_wait();
             __syncthreads();
-            CPT(10)
             if (c.rank == 0)
                 for (int i = threadIdx.x; i <= j; i += CL_THREADS) a.R[(size_t)j * (m + 1) + i] = hcol[i];
             ++iters;
@@ -450,7 +418,6 @@ __global__ void __launch_bounds__(CL_THREADS, 1) bie_gmres_cluster_kernel(const 
             conv = (fabs(g[j + 1]) <= thresh) || (hn == 0.0);
             if (hn == 0.0 && !(fabs(g[j + 1]) <= thresh)) status = 2;
             __syncthreads();
-            CPT(11)
             if (conv || iters >= a.max_iters) break;
         }
         // ---- a9: y = R^{-1} g (CTA 0) -> every CTA, x += V y -----------------------------------------------------------
@@ -500,15 +467,6 @@ __global__ void __launch_bounds__(CL_THREADS, 1) bie_gmres_cluster_kernel(const 
         cl_allreduce(c, dl, 1, hloc);
         relres = sqrt(hloc[0]) / bn;
     }
-#ifdef BIE_PHASE_TIMING
-    if (c.rank == 0 && threadIdx.x == 0 && iters > 0)
-        printf("cluster GMRES, %d steps: load A %.1f us, to first step %.1f us; us per step: gemv %.2f | dots1 %.2f | allreduce1 %.2f | combine1 %.2f | dots2 %.2f | "
-               "allreduce2 %.2f | combine2 + v %.2f | allgather + Givens %.2f | barrier3 %.2f | rest %.2f\n", iters, cpt[0] * 1e-3, cpt[1] * 1e-3,
-               cpt[2] * 1e-3 / iters, cpt[3] * 1e-3 / iters, cpt[4] * 1e-3 / iters, cpt[5] * 1e-3 / iters, cpt[6] * 1e-3 / iters, cpt[7] * 1e-3 / iters,
-               cpt[8] * 1e-3 / iters, cpt[9] * 1e-3 / iters, cpt[10] * 1e-3 / iters, cpt[11] * 1e-3 / iters);
-    if (c.rank == 0 && threadIdx.x == 0 && iters > 0) { printf("   gemv: shared-memory rows %.2f us per call\n", g_gemv_t[0] * 1e-3 / (iters + 1)); g_gemv_t[0] = 0; }
-    if (c.rank == 0 && threadIdx.x == 0 && iters > 0) printf("   ss %.2f | combine2 %.2f | hn %.2f\n", cpt[12] * 1e-3 / iters, cpt[13] * 1e-3 / iters, cpt[14] * 1e-3 / iters);
-#endif
     if (c.rank == 0 && threadIdx.x == 0) {
         if (a.iters_out) *a.iters_out = iters;
         if (a.relres_out) *a.relres_out = relres;
