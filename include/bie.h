@@ -176,13 +176,14 @@ int bie_matvec_free(bie_ctx* ctx, int n, const double* x, double* y, void* strea
  * ones.  Same results to rounding; all are deterministic. */
 int bie_set_symmetric(bie_ctx* ctx, int on);
 
-/* Small stored-matrix solves (n <= 1024): bie_gmres and bie_gmres_noalloc run the same restarted GMRES (rows a5-a10;
+/* Small stored-matrix solves (n <= 640 at restart 50): bie_gmres and bie_gmres_noalloc run the same restarted GMRES (rows a5-a10;
  * PAPER.md:L855, stopping rule PAPER.md:L869) on ONE thread-block cluster of 16 (else 8) CTAs -- the rows of A and of the
- * Krylov basis in the CTAs' shared memory, hardware cluster barriers and distributed shared memory instead of grid
- * barriers and L2 round trips -- when the device can co-schedule such a cluster; otherwise, and for larger n, the
- * grid-wide kernel.  Same arguments, workspace, outputs and tolerances; deterministic; iteration counts of the two
- * kernels agree within one step (their reductions differ in order).  on = 1 (default) / 0: use it / never use it. */
-int bie_set_cluster_gmres(bie_ctx* ctx, int on);
+ * Krylov basis in the CTAs' shared memory, exchanges by asynchronous stores into the peers' shared memory with mbarrier
+ * transaction counts instead of grid barriers and L2 round trips -- when all but four rows of A per CTA fit and the device can
+ * co-schedule such a cluster; otherwise, and for larger n, the grid-wide kernel.  Same arguments, workspace, outputs and
+ * tolerances; deterministic; iteration counts of the two kernels agree within one step (their sums differ in order).
+ * on = 1 (default) / 0: use it / never use it. */
+int bie_set_small_gmres(bie_ctx* ctx, int on);
 
 /* stream function prescribed on the solids, circulation parameters
  * a_m = <1_m, omega> unknown.  Adds, in place, the rank-(N-1) correction of Eq. (B.2) to a matrix A that holds

@@ -26,7 +26,7 @@ EXPORTS = ("bie_create", "bie_destroy", "bie_strerror", "bie_device_info", "bie_
            "bie_set_hybrid_free_warps", "bie_gmres_hybrid", "bie_matvec_rect", "bie_build_normal_velocity",
            "bie_add_cyl_columns", "bie_cauchy_eval_workspace_bytes", "bie_cauchy_eval", "bie_set_symmetric",
            "bie_build_block", "bie_set_hybrid_poll_tiles", "bie_hybrid_block_bytes", "bie_probe_read",
-           "bie_gmres_noalloc", "bie_gmres_noalloc_max_bytes", "bie_set_cluster_gmres")
+           "bie_gmres_noalloc", "bie_gmres_noalloc_max_bytes", "bie_set_small_gmres")
 
 BIE_OK, BIE_MAX_ITERS = 0, 1
 OP_DENSE, OP_FREE, OP_HYBRID = 0, 1, 2
@@ -107,8 +107,8 @@ def lib() -> ctypes.CDLL:
         L.bie_cauchy_eval.argtypes = [vp, i32, ip, ip, vp, vp, i32, vp, i32, vp, vp, vp, sz, vp]
         L.bie_set_symmetric.restype = i32
         L.bie_set_symmetric.argtypes = [vp, i32]
-        L.bie_set_cluster_gmres.restype = i32
-        L.bie_set_cluster_gmres.argtypes = [vp, i32]
+        L.bie_set_small_gmres.restype = i32
+        L.bie_set_small_gmres.argtypes = [vp, i32]
         L.bie_probe_read.restype = i32
         L.bie_probe_read.argtypes = [vp, vp, i64, vp, vp]
         L.bie_probe_dfma.restype = i32
@@ -290,9 +290,9 @@ class Context:
                                      _stream()), "bie_cauchy_eval")
         return out
 
-    def bie_set_cluster_gmres(self, on):
-        """1 (default): stored-matrix solves with n <= 1024 run on one thread-block cluster; 0: always the grid-wide kernel"""
-        _check(lib().bie_set_cluster_gmres(self._h, int(on)), "bie_set_cluster_gmres")
+    def bie_set_small_gmres(self, on):
+        """1 (default): stored-matrix solves up to n = 640 run on one thread-block cluster (bie_gmres_cluster.cu); 0: always the grid-wide kernel"""
+        _check(lib().bie_set_small_gmres(self._h, int(on)), "bie_set_small_gmres")
 
     def bie_set_symmetric(self, on):
         """0: one-directional pair loops; 1 (default): symmetric loops in the whole-matrix matrix-free operator; 2: also in

@@ -36,7 +36,7 @@ int bie_create(bie_ctx** out, int device)
     for (int i = 0; i < 4; ++i) c->sym_key[i] = -1;
     for (int i = 0; i < 16; ++i) c->smem_set[i] = 0;
     c->use_sym = 1;   // bie_set_symmetric
-    c->cluster_gmres = 1; c->cluster_size = 0;   // bie_set_cluster_gmres; probed at the first small solve
+    c->small_gmres = 1; c->cluster_size = 0;   // bie_set_small_gmres; the cluster size is probed at the first small solve
     if (cudaMalloc((void**)&c->sync_buf, 256 * (BIE_SYNC_SLOTS + 1)) != cudaSuccess ||
         cudaMallocHost((void**)&c->pinned_i, 4 * sizeof(int32_t)) != cudaSuccess ||
         cudaMallocHost((void**)&c->pinned_d, 4 * sizeof(double)) != cudaSuccess) {
@@ -183,11 +183,11 @@ int bie_set_symmetric(bie_ctx* c, int on)
     return BIE_OK;
 }
 
-int bie_set_cluster_gmres(bie_ctx* c, int on)
+int bie_set_small_gmres(bie_ctx* c, int on)
 {
     if (!c) return BIE_ERR_NULL;
     if (on < 0 || on > 1) return BIE_ERR_ARG;
-    c->cluster_gmres = on;
+    c->small_gmres = on;
     return BIE_OK;
 }
 

@@ -33,7 +33,7 @@
 #define BIE_HYBRID_POLL_TILES 0         // hybrid operator: tiles of the stored block a pair-loop warp may take between two source chunks
 #define BIE_HYBRID_FREE_WARPS 12       // hybrid operator: warps of a CTA on the pair loops (of 16; one warp issues the bulk copies)
 #define BIE_HYBRID_DENSE_FRACTION 0.5625 // hybrid operator: edge of the stored leading block as a share of n (32 % of the entries)
-#define BIE_CLUSTER_MAX_N 1024         // stored-matrix GMRES on one thread-block cluster up to this n (bie_gmres_cluster.cu)
+#define BIE_CLUSTER_MAX_N 1024         // stored-matrix GMRES on one thread-block cluster at most up to this n (bie_gmres_cluster.cu)
 #define BIE_CLUSTER_NOT_TAKEN 1        // bie_launch_gmres_cluster: not for the cluster kernel, use the grid-wide one
 #define BIE_SYNC_SLOTS 16             // grid-barrier counters of a ctx (bie_matvec_free cycles through them), 256 B apart
 
@@ -86,7 +86,7 @@ struct bie_ctx {
     int hybrid_poll_tiles;   // hybrid operator: tiles a pair-loop warp may take between two source chunks (0: it never does)
     unsigned int* sync_buf;  // BIE_SYNC_SLOTS grid-barrier counters (256 B apart) + two device scalars behind them
     int sync_next;           // next counter slot (bie_matvec_free); bie_gmres keeps its counter in the caller's workspace
-    int cluster_gmres;       // bie_set_cluster_gmres: small stored-matrix solves run on one thread-block cluster (default 1)
+    int small_gmres;         // bie_set_small_gmres: small stored-matrix solves run on one thread-block cluster (default 1)
     int cluster_size;        // 0: not probed yet; -1: the device cannot co-schedule such a cluster; else 16 or 8
     int cap;
     // current geometry (host copies)

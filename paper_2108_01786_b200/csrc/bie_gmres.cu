@@ -730,13 +730,6 @@ int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, int nd, 
     // align the caller's workspace to 256 bytes
     uintptr_t base = ((uintptr_t)ws + 255) & ~(uintptr_t)255;
     if (base - (uintptr_t)ws + pl.total > ws_bytes) return BIE_ERR_WORKSPACE;
-    if (mode == 0) {
-        // small stored-matrix systems: one thread-block cluster, cluster barriers and distributed shared memory
-        // instead of grid barriers and L2 (bie_gmres_cluster.cu); same workspace layout
-        rc = bie_launch_gmres_cluster(ctx, n, A, lda, rhs, tol, restart, max_iters, x, iters_out, relres_out, status_out, res_hist,
-                                      (double*)(base + pl.offV), pl.nld, (double*)(base + pl.offR), st);
-        if (rc != BIE_CLUSTER_NOT_TAKEN) return rc;
-    }
     a.A = A; a.lda = lda; a.n = n; a.b = rhs; a.tol = tol; a.m = restart; a.max_iters = max_iters;
     a.x = x; a.iters_out = iters_out; a.relres_out = relres_out; a.status_out = status_out; a.res_hist = res_hist;
     a.V = (double*)(base + pl.offV);
@@ -751,6 +744,13 @@ int bie_launch_gmres(bie_ctx* ctx, int n, const double* A, int64_t lda, int nd, 
     a.res_pairs = (mode == 0 && pl.stream)
         ? bie_gemv_resident_pairs(ctx->l2_bytes, n, (long long)lda, pl.rows_per_cta, sizeof(double) * (size_t)(restart + 2) * pl.nld) : 0;
     BIE_CUDA(cudaMemsetAsync(a.sync, 0, sizeof(unsigned int), st));
+    if (mode == 0) {
+        // small stored-matrix systems: one thread-block cluster, distributed shared memory instead of grid barriers and L2
+        // (bie_gmres_cluster.cu); same workspace layout
+        rc = bie_launch_gmres_cluster(ctx, n, A, lda, rhs, tol, restart, max_iters, x, iters_out, relres_out, status_out, res_hist,
+                                      a.V, pl.nld, a.R, st);
+        if (rc != BIE_CLUSTER_NOT_TAKEN) return rc;
+    }
     if (mode == 1) return launch_gmres<false, false, 1>(ctx, a, pl, st);
     if (mode == 2) return pl.stream ? launch_gmres<true, true, 2>(ctx, a, pl, st) : launch_gmres<false, true, 2>(ctx, a, pl, st);
     if (pl.stream) return pl.xs ? launch_gmres<true, true, 0>(ctx, a, pl, st) : launch_gmres<true, false, 0>(ctx, a, pl, st);

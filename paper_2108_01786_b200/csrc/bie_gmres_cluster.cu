@@ -4,21 +4,28 @@
 // Why: with a stored matrix of a few MB the grid-wide kernel of bie_gmres.cu is a chain of L2 round trips -- two grid
 // barriers through a global counter (1.5-2 us each) and two reductions of per-CTA partials read back from L2 (1.4-2.3 us
 // each) per Arnoldi step: 13.5 us per step at n = 640 against 0.5 us for the GEMV itself.  A cluster of 16 (or 8) CTAs has
-// what such a solve needs ON the chip: the hardware cluster barrier instead of a spin on a global counter, and
-// distributed shared memory instead of L2 for everything that crosses CTAs.
+// what such a solve needs ON the chip: distributed shared memory instead of L2 for everything that crosses CTAs.
 //   - CTA c owns a contiguous block of rows of A, of every Krylov vector and of x.  Its rows of A sit in its shared
-//     memory for the whole solve (at n = 640: 37 of its 40 rows; the others stream from L2 first in every GEMV).
-//   - all-gather by remote stores: a CTA writes its rows of the next Krylov vector (or its partial dot products) into
-//     the shared memory of EVERY CTA of the cluster (mapa / st.shared::cluster), one cluster barrier makes them
-//     visible, and every CTA adds the partials in the same fixed order -- all CTAs hold bit-identical coefficients,
-//     Givens rotations and residuals and take the same branches without further communication.
-//   - Arnoldi step j: y = A v_j (shared memory);  s = V_j^T y (all-gather + barrier 1);  w1 = y - V_j s;
-//     h2 = V_j^T w1 and ||w1||^2 (all-gather + barrier 2);  hn^2 = ||w1||^2 - ||h2||^2 (Pythagoras, as bie_gmres.cu;
-//     explicit norm with one more barrier when h2 is not small);  v_{j+1} = (w1 - V_j h2)/hn -> all CTAs (barrier 3).
-//     Classical Gram-Schmidt twice (CGS2), h = s + h2, Givens and the recurrence residual as in bie_gmres.cu (a8),
-//     back-substitution by CTA 0 at the end of a cycle (a9), true residual at the end (a10).
-// The partial-sum buffers alternate between two copies: a CTA that is ahead writes the NEXT reduction's partials while
-// a slower one still adds the previous ones; two reductions back every CTA has passed a barrier in between.
+//     memory for the whole solve (at n = 640: 36 of its 40 rows; the others stream from L2, split over all warps and
+//     issued before the shared-memory rows of every GEMV).
+//   - exchanges: a CTA sends its rows of the next Krylov vector (or its partial dot products) into the shared memory
+//     of EVERY CTA of the cluster with st.async, whose completion the hardware counts in bytes on an mbarrier of the
+//     RECEIVER (mbarrier::complete_tx); the receiver states how many bytes the exchange brings (arrive.expect_tx) and
+//     waits for the phase.  No cluster-wide barrier and no fence per exchange (the first version used remote stores +
+//     barrier.cluster: its release/acquire fences were 2.3 of 15 stall cycles per issue, profiles/r02b_cluster.md).  Every CTA
+//     adds the partials by the same xor-shuffle tree -- all CTAs hold bit-identical coefficients, Givens rotations and
+//     residuals and take the same branches without further communication.
+//   - Arnoldi step j: y = A v_j (shared memory);  s = V_j^T y (exchange 1);  w1 = y - V_j s;
+//     h2 = V_j^T w1 and ||w1||^2 (exchange 2);  hn^2 = ||w1||^2 - ||h2||^2 (Pythagoras, as bie_gmres.cu;
+//     explicit norm with one more exchange when h2 is not small);  v_{j+1} = (w1 - V_j h2)/hn -> all CTAs (exchange 3, which
+//     lands while one thread runs the Givens sweep).  Classical Gram-Schmidt twice (CGS2), h = s + h2, Givens and the
+//     recurrence residual as in bie_gmres.cu (a8), back-substitution by CTA 0 at the end of a cycle (a9), true residual at
+//     the end (a10).
+// Buffer reuse needs no extra synchronisation: the partial buffers alternate between two copies (each with its own
+// mbarrier), and a CTA can send exchange k + 2 only after it has received everyone's exchange k + 1, which every CTA sends
+// after it has consumed exchange k.  A variant with the whole basis REPLICATED in every CTA of the full grid (one grid
+// barrier per step, Gram-Schmidt local and redundant) was built too and is slower (14-20 us per step at n = 640: four passes
+// over the basis per step through one SM's shared-memory port): DESIGN.md section 7d.
 #include <cooperative_groups.h>
 #include "bie_common.cuh"
 
@@ -94,9 +101,33 @@ __device__ __forceinline__ double cl_block_sum(double v, double* red)
     return red[32];
 }
 
-// split cluster barrier: every thread arrives (release) ... waits (acquire)
-__device__ __forceinline__ void cg_cluster_arrive() { asm volatile("barrier.cluster.arrive.release;" ::: "memory"); }
-__device__ __forceinline__ void cg_cluster_wait() { asm volatile("barrier.cluster.wait.acquire;" ::: "memory"); }
+// ---- exchange primitives: st.async into a peer's shared memory, completion counted in bytes on the PEER's mbarrier ----
+__device__ __forceinline__ uint32_t cl_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint32_t cl_mapa(uint32_t addr, int rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void cl_st_async(uint32_t remote_addr, double v, uint32_t remote_mbar)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b64 [%0], %1, [%2];"
+                 :: "r"(remote_addr), "l"(__double_as_longlong(v)), "r"(remote_mbar) : "memory");
+}
+__device__ __forceinline__ void cl_mbar_init(uint32_t mb, int count) { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(mb), "r"(count) : "memory"); }
+__device__ __forceinline__ void cl_mbar_expect(uint32_t mb, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(mb), "r"(bytes) : "memory");
+}
+// all bytes of the phase with this parity have landed (and are visible: acquire at cluster scope)
+__device__ __forceinline__ void cl_mbar_wait(uint32_t mb, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(mb), "r"(parity) : "memory");
+    } while (!done);
+}
 
 struct ClusterCtx {
     cg::cluster_group cl;
@@ -104,7 +135,9 @@ struct ClusterCtx {
     int r0, rows, rows2, n, n2, mp;
     double* smem;
     ClusterSmem L;
-    int pb;          // partial buffer to use next
+    unsigned kP;     // exchanges of partial sums so far: exchange k uses buffer and mbarrier k & 1, phase parity (k >> 1) & 1
+    unsigned kX;     // all-gathers of a vector into xs so far (one mbarrier, parity kX & 1)
+    uint32_t mbP, mbX, mbY;   // shared addresses of the mbarriers: partial sums [2], vector, the solution of the small least-squares problem
 };
 
 // vals[0..cnt) (shared) of every CTA -> out[i] = sum over the CTAs, in every CTA: the same fixed tree everywhere (lane q of a
@@ -112,14 +145,17 @@ struct ClusterCtx {
 // out[i]^2 over i < cnt - 1 (the norm of h2 in the second Gram-Schmidt pass), by warp 0 in fixed order.  Ends with __syncthreads.
 __device__ __forceinline__ void cl_allreduce(ClusterCtx& c, const double* vals, int cnt, double* out, double* ssq = nullptr)
 {
-    double* P = c.smem + c.L.P + c.pb * c.CS * c.mp;
-    c.pb ^= 1;
+    const unsigned k = c.kP++;
+    double* P = c.smem + c.L.P + (k & 1) * c.CS * c.mp;
+    const uint32_t mb = c.mbP + 8 * (k & 1);
     const int sh = (c.CS == 16) ? 4 : 3;                      // CS is 16 or 8
+    if (threadIdx.x == 0) cl_mbar_expect(mb, (uint32_t)(cnt << sh) * 8u);      // every CTA (this one too) sends cnt doubles
+    const uint32_t slot = cl_smem_u32(P + c.rank * c.mp);
     for (int t = threadIdx.x; t < (cnt << sh); t += CL_THREADS) {
         const int peer = t & (c.CS - 1), i = t >> sh;
-        c.cl.map_shared_rank(P, peer)[c.rank * c.mp + i] = vals[i];
+        cl_st_async(cl_mapa(slot + 8 * i, peer), vals[i], cl_mapa(mb, peer));
     }
-    c.cl.sync();
+    cl_mbar_wait(mb, (k >> 1) & 1);
     const int per = CL_THREADS >> sh;                          // values per pass of the whole CTA
     for (int i0 = 0; i0 < cnt; i0 += per) {
         const int i = i0 + (threadIdx.x >> sh), q = threadIdx.x & (c.CS - 1);
@@ -139,14 +175,20 @@ __device__ __forceinline__ void cl_allreduce(ClusterCtx& c, const double* vals, 
     }
 }
 
-// this CTA's rows of a vector (shared, v[0..rows)) -> xs of every CTA.  The caller synchronises the cluster afterwards.
+// this CTA's rows of a vector (shared, v[0..rows)) -> xs of every CTA (non-blocking); cl_xs_wait() before xs is read
 __device__ __forceinline__ void cl_allgather_rows(ClusterCtx& c, const double* v)
 {
-    double* xs = c.smem + c.L.xs;
+    const uint32_t xs0 = cl_smem_u32(c.smem + c.L.xs + c.r0);
+    if (threadIdx.x == 0) cl_mbar_expect(c.mbX, (uint32_t)c.n * 8u);           // all n entries arrive, this CTA's own too
     for (int t = threadIdx.x; t < c.rows * c.CS; t += CL_THREADS) {
         const int peer = t / c.rows, i = t - peer * c.rows;
-        c.cl.map_shared_rank(xs, peer)[c.r0 + i] = v[i];
+        cl_st_async(cl_mapa(xs0 + 8 * i, peer), v[i], cl_mapa(c.mbX, peer));
     }
+}
+__device__ __forceinline__ void cl_xs_wait(ClusterCtx& c)
+{
+    cl_mbar_wait(c.mbX, c.kX & 1);
+    ++c.kX;
 }
 
 // y[r] = A[r0 + r, :] xs for this CTA's rows.  Rows in shared memory: one warp per row.  The rows that did not fit stream
@@ -279,7 +321,14 @@ __global__ void __launch_bounds__(CL_THREADS, 1) bie_gmres_cluster_kernel(const 
     c.r0 = min(c.rank * a.rows_per_cta, a.n);
     c.rows = min(c.r0 + a.rows_per_cta, a.n) - c.r0;      // may be 0 for the last CTAs of a tiny system
     c.rows2 = (a.rows_per_cta + 1) & ~1;
-    c.smem = smem; c.pb = 0;
+    c.smem = smem; c.kP = 0; c.kX = 0;
+    __shared__ __align__(8) unsigned long long mbar[4];
+    c.mbP = cl_smem_u32(&mbar[0]); c.mbX = cl_smem_u32(&mbar[2]); c.mbY = cl_smem_u32(&mbar[3]);
+    if (threadIdx.x == 0) {
+        for (int q = 0; q < 4; ++q) cl_mbar_init(c.mbP + 8 * q, 1);      // one arrival per phase: the thread that states the expected bytes
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    unsigned kY = 0;
     c.L = cluster_smem(a.n, a.m, a.rows_per_cta, a.mp, c.CS, a.VS, a.rows_smem);
     const int m = a.m, rows = c.rows, r0 = c.r0;
     double* y = smem + c.L.y;  double* w = smem + c.L.w;  double* xl = smem + c.L.xl;
@@ -326,7 +375,7 @@ __global__ void __launch_bounds__(CL_THREADS, 1) bie_gmres_cluster_kernel(const 
             __syncthreads();
         } else {
             cl_allgather_rows(c, xl);
-            c.cl.sync();
+            cl_xs_wait(c);
             cl_gemv(c, a, y, comb);
             for (int r = threadIdx.x; r < rows; r += CL_THREADS) w[r] = a.b[r0 + r] - y[r];
             __syncthreads();
@@ -347,7 +396,7 @@ __global__ void __launch_bounds__(CL_THREADS, 1) bie_gmres_cluster_kernel(const 
             for (int r = threadIdx.x; r < rows; r += CL_THREADS) { const double v = w[r] * inv; v0[r] = v; w[r] = v; }
             __syncthreads();
             cl_allgather_rows(c, w);
-            c.cl.sync();
+            cl_xs_wait(c);
         }
         if (threadIdx.x == 0) g[0] = beta;
         __syncthreads();
@@ -388,9 +437,7 @@ __global__ void __launch_bounds__(CL_THREADS, 1) bie_gmres_cluster_kernel(const 
                 for (int r = threadIdx.x; r < rows; r += CL_THREADS) { const double v = w[r] * inv; vn[r] = v; w[r] = v; }
             }
             __syncthreads();
-            cl_allgather_rows(c, w);                                       // v_{j+1} -> xs of every CTA
-            __syncthreads();
-            cg_cluster_arrive();                                           // barrier 3, split: the Givens sweep runs while it completes
+            cl_allgather_rows(c, w);                                       // v_{j+1} -> xs of every CTA; the Givens sweep runs while it lands
             // a8: Givens rotations on column j, new rotation, recurrence residual (one thread, the same bits in every CTA)
             if (threadIdx.x == CL_THREADS - 1) {
                 hcol[j + 1] = hn;
@@ -408,7 +455,7 @@ __global__ void __launch_bounds__(CL_THREADS, 1) bie_gmres_cluster_kernel(const 
                 g[j + 1] = -sn[j] * g[j];
                 g[j] = cs[j] * g[j];
             }
-            cg_cluster_wait();
+            cl_xs_wait(c);
             __syncthreads();
             if (c.rank == 0)
                 for (int i = threadIdx.x; i <= j; i += CL_THREADS) a.R[(size_t)j * (m + 1) + i] = hcol[i];
@@ -434,12 +481,15 @@ __global__ void __launch_bounds__(CL_THREADS, 1) bie_gmres_cluster_kernel(const 
                 }
             }
             __syncthreads();
-            for (int t = threadIdx.x; t < k * (c.CS - 1); t += CL_THREADS) {
-                const int peer = 1 + t / k, i = t - (peer - 1) * k;
-                c.cl.map_shared_rank(hloc, peer)[i] = hloc[i];
+            for (int t = threadIdx.x; t < k * c.CS; t += CL_THREADS) {         // y -> hloc of every CTA (this one too: the same values)
+                const int peer = t / k, i = t - peer * k;
+                cl_st_async(cl_mapa(cl_smem_u32(hloc + i), peer), hloc[i], cl_mapa(c.mbY, peer));
             }
         }
-        c.cl.sync();
+        if (threadIdx.x == 0) cl_mbar_expect(c.mbY, (uint32_t)k * 8u);
+        cl_mbar_wait(c.mbY, kY & 1);
+        ++kY;
+        __syncthreads();
         for (int r = threadIdx.x; r < rows; r += CL_THREADS) w[r] = -xl[r];
         __syncthreads();
         cl_subtract_combination(c, a, k, hloc, w, comb);                  // w = -(x + V y)
@@ -454,7 +504,7 @@ __global__ void __launch_bounds__(CL_THREADS, 1) bie_gmres_cluster_kernel(const 
     double relres = 0.0;
     if (a.relres_out && bn != 0.0) {
         cl_allgather_rows(c, xl);
-        c.cl.sync();
+        cl_xs_wait(c);
         cl_gemv(c, a, y, comb);
         p = 0.0;
         for (int r = threadIdx.x; r < rows; r += CL_THREADS) {
@@ -512,7 +562,7 @@ int bie_launch_gmres_cluster(bie_ctx* ctx, int n, const double* A, int64_t lda, 
                              int max_iters, double* x, int32_t* iters_out, double* relres_out, int32_t* status_out,
                              double* res_hist, double* Vg, int nld, double* R, cudaStream_t st)
 {
-    if (!ctx->cluster_gmres || n > BIE_CLUSTER_MAX_N) return BIE_CLUSTER_NOT_TAKEN;
+    if (!ctx->small_gmres || n > BIE_CLUSTER_MAX_N) return BIE_CLUSTER_NOT_TAKEN;
     const int CS = cluster_probe(ctx);
     if (CS < 8) return BIE_CLUSTER_NOT_TAKEN;
     const int m = restart;

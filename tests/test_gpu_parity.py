@@ -949,10 +949,10 @@ def test_gmres_restart_and_iteration_cap(ctx):
     assert abs(rr - rro) <= 1e-6 * rro
 
 
-@pytest.mark.parametrize("cluster", [1, 0])
-@pytest.mark.parametrize("n,lda,restart", [(640, 640, 50), (37, 40, 50), (301, 302, 7), (600, 608, 20), (16, 16, 4), (5, 6, 50)])
-def test_gmres_small_systems_cluster_and_grid_kernels(ctx, n, lda, restart, cluster):
-    """stored-matrix solves up to n = 640 run on one thread-block cluster (bie_gmres_cluster.cu) unless bie_set_cluster_gmres(0);
+@pytest.mark.parametrize("small", [1, 0])
+@pytest.mark.parametrize("n,lda,restart", [(640, 640, 50), (37, 40, 50), (301, 302, 7), (600, 608, 20), (16, 16, 4), (5, 6, 50), (700, 700, 60)])
+def test_gmres_small_systems_both_kernels(ctx, n, lda, restart, small):
+    """stored-matrix solves up to n = 640 run on one thread-block cluster (bie_gmres_cluster.cu) unless bie_set_small_gmres(0);
     both kernels against the oracle: odd n, lda > n, fewer rows than CTAs, several restart cycles, the iteration cap"""
     rng = np.random.default_rng(1000 + n)
     if n == 640:
@@ -963,7 +963,7 @@ def test_gmres_small_systems_cluster_and_grid_kernels(ctx, n, lda, restart, clus
         b = rng.standard_normal(n)
     Ad = torch.full((n, lda), 7.0, dtype=torch.float64, device="cuda")
     Ad[:, :n] = dev(Ao)
-    ctx.bie_set_cluster_gmres(cluster)
+    ctx.bie_set_small_gmres(small)
     try:
         xo, ito, rro, _, sto = oracle.gmres(Ao, b, 1e-13, restart, 1000)
         x, it, rr, st = gpu_gmres(ctx, Ad, b, 1e-13, restart, 1000, lda=lda)
@@ -978,16 +978,16 @@ def test_gmres_small_systems_cluster_and_grid_kernels(ctx, n, lda, restart, clus
         assert (sto, ito) == (1, cap) and (st, it) == (1, cap)
         assert np.linalg.norm(x - xo) / np.linalg.norm(xo) <= 1e-9 and abs(rr - rro) <= 1e-6 * rro
     finally:
-        ctx.bie_set_cluster_gmres(1)
+        ctx.bie_set_small_gmres(1)
 
 
-@pytest.mark.parametrize("cluster", [1, 0])
-def test_gmres_degenerate_cases(ctx, cluster):
-    ctx.bie_set_cluster_gmres(cluster)
+@pytest.mark.parametrize("small", [1, 0])
+def test_gmres_degenerate_cases(ctx, small):
+    ctx.bie_set_small_gmres(small)
     try:
         _gmres_degenerate_cases(ctx)
     finally:
-        ctx.bie_set_cluster_gmres(1)
+        ctx.bie_set_small_gmres(1)
 
 
 def _gmres_degenerate_cases(ctx):
