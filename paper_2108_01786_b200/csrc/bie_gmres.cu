@@ -554,13 +554,25 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
         // ---- a9: y = R^{-1} g (CTA 0), x += V y ---------------------------------------------------
         if (blockIdx.x == 0) {
             __syncthreads();
+            // R lives in global memory (this CTA wrote it); a back-substitution that reads it from there waits one L2 round trip per
+            // unknown (0.8 us each: 80 us for a full cycle of 100).  Staged into shared memory first -- the operator's scratch or the
+            // slot of x, both idle here -- when the packed triangle fits.
+            double* Rst = (MODE == 0) ? xs : gpart;
+            const int cap = (MODE == 0) ? (XS ? n : 0) : a.scratch_doubles;
+            const bool staged = (k * (k + 1) / 2 <= cap);
+            if (staged) {
+                for (int q = threadIdx.x >> 5; q < k; q += (int)(blockDim.x >> 5))
+                    for (int i = threadIdx.x & 31; i <= q; i += 32) Rst[q * (q + 1) / 2 + i] = __ldcg(a.R + (size_t)q * (m + 1) + i);
+                __syncthreads();
+            }
             if (threadIdx.x < 32) {
                 const int lane = threadIdx.x;
                 for (int i = k - 1; i >= 0; --i) {
                     double s = 0.0;
-                    for (int c = i + 1 + lane; c < k; c += 32) s = fma(a.R[(size_t)c * (m + 1) + i], hloc[c], s);
+                    if (staged) for (int c = i + 1 + lane; c < k; c += 32) s = fma(Rst[c * (c + 1) / 2 + i], hloc[c], s);
+                    else for (int c = i + 1 + lane; c < k; c += 32) s = fma(a.R[(size_t)c * (m + 1) + i], hloc[c], s);
                     s = bie_warp_sum(s);
-                    if (lane == 0) hloc[i] = (g[i] - s) / a.R[(size_t)i * (m + 1) + i];
+                    if (lane == 0) hloc[i] = (g[i] - s) / (staged ? Rst[i * (i + 1) / 2 + i] : a.R[(size_t)i * (m + 1) + i]);
                     __syncwarp();
                 }
                 for (int i = lane; i < k; i += 32) a.yv[i] = hloc[i];

@@ -470,13 +470,23 @@ __global__ void __launch_bounds__(CL_THREADS, 1) bie_gmres_cluster_kernel(const 
         // ---- a9: y = R^{-1} g (CTA 0) -> every CTA, x += V y -----------------------------------------------------------
         if (c.rank == 0) {
             __syncthreads();
+            // R (global, written by this CTA) is staged into the partial buffers first -- idle here: no CTA sends partial sums before it has
+            // the solution of this cycle -- so that the back-substitution does not wait one L2 round trip per unknown
+            double* Rst = smem + c.L.P;
+            const bool staged = (k * (k + 1) / 2 <= 2 * c.CS * c.mp);
+            if (staged) {
+                for (int q = threadIdx.x >> 5; q < k; q += CL_WARPS)
+                    for (int i = threadIdx.x & 31; i <= q; i += 32) Rst[q * (q + 1) / 2 + i] = __ldcg(a.R + (size_t)q * (m + 1) + i);
+                __syncthreads();
+            }
             if (threadIdx.x < 32) {
                 const int lane = threadIdx.x;
                 for (int i = k - 1; i >= 0; --i) {
                     double s = 0.0;
-                    for (int q = i + 1 + lane; q < k; q += 32) s = fma(a.R[(size_t)q * (m + 1) + i], hloc[q], s);
+                    if (staged) for (int q = i + 1 + lane; q < k; q += 32) s = fma(Rst[q * (q + 1) / 2 + i], hloc[q], s);
+                    else for (int q = i + 1 + lane; q < k; q += 32) s = fma(a.R[(size_t)q * (m + 1) + i], hloc[q], s);
                     s = bie_warp_sum(s);
-                    if (lane == 0) hloc[i] = (g[i] - s) / a.R[(size_t)i * (m + 1) + i];
+                    if (lane == 0) hloc[i] = (g[i] - s) / (staged ? Rst[i * (i + 1) / 2 + i] : a.R[(size_t)i * (m + 1) + i]);
                     __syncwarp();
                 }
             }
