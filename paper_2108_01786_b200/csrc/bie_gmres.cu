@@ -33,6 +33,9 @@
 #define GM_THREADS 512
 #endif
 #define GM_WARPS (GM_THREADS / 32)
+#ifndef GM_WIDE_FROM
+#define GM_WIDE_FROM 0      // rows of a reduction from which reduce_partials takes its seven-row form (developer knob)
+#endif
 
 struct GmresArgs {
     const double* A;
@@ -275,12 +278,41 @@ __device__ __forceinline__ void local_dots(const Basis& B, int rows, int cnt, co
     }
 }
 
-// out[i] = sum over the G per-CTA partials of row i < cnt, same order in every CTA; the loads of up to four rows are
-// in flight together.  Ends with __syncthreads.
+// out[i] = sum over the G per-CTA partials of row i < cnt, same order in every CTA.  G even and <= 192 (one CTA per SM on a
+// B200: 148): a row is at most three 128-bit loads per lane and a warp keeps SEVEN rows in flight, so that the restart + 2 <= 112
+// rows of a reduction are ONE round of L2 latency for the 16 warps (four rows of 64-bit loads need two rounds from j = 63 on).
+// Same box, A/B/A/B: config 5 26.66 -> 26.35 ms per solve, config 3 33.8 -> 31.9 us per iteration, config 2 0.597 -> 0.592 ms; taking
+// this form only beyond 64 rows gives half of the gain.  Ends with __syncthreads.
 __device__ __forceinline__ void reduce_partials(const double* part_slot, int cnt, double* out)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
     const int G = gridDim.x;
+    if ((G & 1) == 0 && G <= 192 && cnt > GM_WIDE_FROM) {
+        constexpr int RP = 7;
+        const int g2 = G >> 1;
+        for (int i0 = warp; i0 < cnt; i0 += RP * nwarp) {
+            double2 v[RP][3];
+#pragma unroll
+            for (int q = 0; q < RP; ++q) {
+                const int i = i0 + q * nwarp;
+                const double2* row = reinterpret_cast<const double2*>(part_slot + (size_t)i * G);
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    const int c = lane + 32 * k;
+                    v[q][k] = (i < cnt && c < g2) ? __ldcg(row + c) : make_double2(0.0, 0.0);
+                }
+            }
+#pragma unroll
+            for (int q = 0; q < RP; ++q) {
+                const int i = i0 + q * nwarp;
+                if (i >= cnt) break;                       // warp-uniform
+                const double h = bie_warp_sum(((v[q][0].x + v[q][0].y) + (v[q][1].x + v[q][1].y)) + (v[q][2].x + v[q][2].y));
+                if (lane == 0) out[i] = h;
+            }
+        }
+        __syncthreads();
+        return;
+    }
     for (int i0 = warp; i0 < cnt; i0 += 4 * nwarp) {
         double s[4];
 #pragma unroll
@@ -508,12 +540,16 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
             // a8: Givens rotations on column j, new rotation, recurrence residual
             if (threadIdx.x == GM_THREADS - 1) {
                 hcol[j + 1] = hn;
+                // rotation i maps (a, h_{i+1}) to (c a + s h_{i+1}, -s a + c h_{i+1}) and hands the second value on as the next a:
+                // the products with the FRESH entry h_{i+1} are off the chain, which is one FMA per rotation
+                double carry = hcol[0];
                 for (int i = 0; i < j; ++i) {
-                    const double t0 = cs[i] * hcol[i] + sn[i] * hcol[i + 1];
-                    const double t1 = -sn[i] * hcol[i] + cs[i] * hcol[i + 1];
-                    hcol[i] = t0;
-                    hcol[i + 1] = t1;
+                    const double hn1 = hcol[i + 1];
+                    const double p = cs[i] * hn1, q = sn[i] * hn1;
+                    hcol[i] = fma(cs[i], carry, q);
+                    carry = fma(-sn[i], carry, p);
                 }
+                hcol[j] = carry;
                 const double d = hypot(hcol[j], hcol[j + 1]);
                 if (d == 0.0) { cs[j] = 1.0; sn[j] = 0.0; }
                 else { cs[j] = hcol[j] / d; sn[j] = hcol[j + 1] / d; }
