@@ -542,8 +542,22 @@ __global__ void __launch_bounds__(GM_THREADS, 1) bie_gmres_kernel(const GmresArg
                 hcol[j + 1] = hn;
                 // rotation i maps (a, h_{i+1}) to (c a + s h_{i+1}, -s a + c h_{i+1}) and hands the second value on as the next a:
                 // the products with the FRESH entry h_{i+1} are off the chain, which is one FMA per rotation
+                // (blocks of four with all loads first: a store to hcol[i] would otherwise hold back the loads of the next rotation)
                 double carry = hcol[0];
-                for (int i = 0; i < j; ++i) {
+                int i = 0;
+                for (; i + 4 <= j; i += 4) {
+                    double c4[4], s4[4], h4[4], o4[4];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) { c4[q] = cs[i + q]; s4[q] = sn[i + q]; h4[q] = hcol[i + q + 1]; }
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        o4[q] = fma(c4[q], carry, s4[q] * h4[q]);
+                        carry = fma(-s4[q], carry, c4[q] * h4[q]);
+                    }
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) hcol[i + q] = o4[q];
+                }
+                for (; i < j; ++i) {
                     const double hn1 = hcol[i + 1];
                     const double p = cs[i] * hn1, q = sn[i] * hn1;
                     hcol[i] = fma(cs[i], carry, q);
