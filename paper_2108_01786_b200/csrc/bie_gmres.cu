@@ -262,19 +262,30 @@ __device__ __forceinline__ void local_dots(const Basis& B, int rows, int cnt, co
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
     const int G = gridDim.x;
     const int tot = cnt + (with_norm ? 1 : 0);
-    for (int i = warp; i < tot; i += nwarp) {
-        double s = 0.0;
-        if (i == cnt) {
-            for (int r = lane; r < rows; r += 32) s = fma(w_local[r], w_local[r], s);
-        } else if (i < B.VS) {
-            const double* vi = B.Vs + (size_t)i * B.rows2;
-            for (int r = lane; r < rows; r += 32) s = fma(vi[r], w_local[r], s);
-        } else {
-            const double* vi = B.Vg + (size_t)i * B.nld;
-            for (int r = lane; r < rows; r += 32) s = fma(__ldcg(vi + r), w_local[r], s);
+    // a warp takes TWO vectors at a time (i and i + nwarp): their loads and their lane reductions overlap
+    for (int i = warp; i < tot; i += 2 * nwarp) {
+        const int i2 = i + nwarp;
+        const bool two = (i2 < tot);
+        double s = 0.0, s2 = 0.0;
+        const double* va = (i == cnt) ? w_local : ((i < B.VS) ? B.Vs + (size_t)i * B.rows2 : B.Vg + (size_t)i * B.nld);
+        const double* vb = !two ? w_local : ((i2 == cnt) ? w_local : ((i2 < B.VS) ? B.Vs + (size_t)i2 * B.rows2 : B.Vg + (size_t)i2 * B.nld));
+        const bool ga = (i != cnt && i >= B.VS), gb = (two && i2 != cnt && i2 >= B.VS);      // in the global basis (L2)
+        for (int r = lane; r < rows; r += 32) {
+            const double wr = w_local[r];
+            const double a = ga ? __ldcg(va + r) : va[r];
+            const double b = gb ? __ldcg(vb + r) : vb[r];
+            s = fma(a, wr, s);
+            s2 = fma(b, wr, s2);
         }
-        s = bie_warp_sum(s);
-        if (lane == 0) part_slot[(size_t)i * G + blockIdx.x] = s;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            s += __shfl_xor_sync(0xffffffffu, s, o);
+            s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+        }
+        if (lane == 0) {
+            part_slot[(size_t)i * G + blockIdx.x] = s;
+            if (two) part_slot[(size_t)i2 * G + blockIdx.x] = s2;
+        }
     }
 }
 
@@ -302,12 +313,26 @@ __device__ __forceinline__ void reduce_partials(const double* part_slot, int cnt
                     v[q][k] = (i < cnt && c < g2) ? __ldcg(row + c) : make_double2(0.0, 0.0);
                 }
             }
+            // the lane reductions of the rows in two interleaved groups (four and three rows; the second only if it has a row)
+            double h[RP];
+#pragma unroll
+            for (int q = 0; q < RP; ++q) h[q] = ((v[q][0].x + v[q][0].y) + (v[q][1].x + v[q][1].y)) + (v[q][2].x + v[q][2].y);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) h[q] += __shfl_xor_sync(0xffffffffu, h[q], o);
+            }
+            if (i0 + 4 * nwarp < cnt) {                    // warp-uniform
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+                    for (int q = 4; q < RP; ++q) h[q] += __shfl_xor_sync(0xffffffffu, h[q], o);
+                }
+            }
 #pragma unroll
             for (int q = 0; q < RP; ++q) {
                 const int i = i0 + q * nwarp;
-                if (i >= cnt) break;                       // warp-uniform
-                const double h = bie_warp_sum(((v[q][0].x + v[q][0].y) + (v[q][1].x + v[q][1].y)) + (v[q][2].x + v[q][2].y));
-                if (lane == 0) out[i] = h;
+                if (i < cnt && lane == 0) out[i] = h[q];
             }
         }
         __syncthreads();
