@@ -230,6 +230,9 @@ __device__ __forceinline__ void bie_cot_half_near(double x, double y, double* re
     *im = -zi * inv - fma(zr, pi, zi * pr);
 }
 
+#ifndef BIE_BARRIER_RELACQ
+#define BIE_BARRIER_RELACQ 1
+#endif
 // ---- grid barrier (cooperative launch guarantees co-residency) -------------------------------------
 __device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p)
 {
@@ -242,10 +245,17 @@ __device__ __forceinline__ void grid_barrier(unsigned int* ctr, unsigned int& ta
     __syncthreads();
     if (threadIdx.x == 0) {
         target += gridDim.x;
+#if BIE_BARRIER_RELACQ
+        // release on the arrival (cumulative over the writes the CTA's threads made before the block barrier above), acquire on
+        // the poll: no separate fences
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" :: "l"(ctr) : "memory");
+        while (ld_acquire_u32(ctr) < target) { }
+#else
         __threadfence();
         atomicAdd(ctr, 1u);
         while (ld_acquire_u32(ctr) < target) { }
         __threadfence();
+#endif
     }
     __syncthreads();
 }
