@@ -14,9 +14,13 @@
 //     Im c  ->  (alpha, beta) = (-2 qi,  qr)     [k = 0, j = 0]  and  [k >= 1, j >= 1]
 //     Re c  ->  (alpha, beta) = (-2 qr, -qi)     [k = 0, j >= 1]
 //    -Re c  ->  (alpha, beta) = ( 2 qr,  qi)     [k >= 1, j = 0]
-// The inner loop has no branch: it only ORs a "near" flag (den < thr_s, which includes s == t).  After every
-// BUILD_RB rows the warp votes; if any lane saw a near pair, those rows are revisited and the near entries are
-// overwritten with the Laurent-series value, or with the precomputed diagonal entry when s == t.
+// The inner loop has no branch: it only tracks the smallest high word of den per column (the generic loop: ORs a "near"
+// flag, den < thr_s, which includes s == t).  After every BUILD_RB rows the warp votes; if any lane saw a near pair, those
+// rows are revisited and the near entries are overwritten with the Laurent-series value, or with the precomputed diagonal
+// entry when s == t.  Whole blocks of rows of a warp whose columns all lie inside the matrix take the FAST row
+// loop (no row clamp, no store predicate, the row pointer advanced by additions: 18.7 issued instructions per entry instead
+// of 26); tails, the last warp of a ragged matrix and the block format of the hybrid operator take the generic one.
+// The grid is one-dimensional and bie_build_tile() puts the tiles that hold the diagonal first (see there).
 #include "bie_common.cuh"
 
 #define BUILD_THREADS 128
@@ -26,9 +30,8 @@
 #define BUILD_RB 4
 #endif
 #ifndef BUILD_MIN_CTAS
-#define BUILD_MIN_CTAS 4      // CTAs of 128 threads per SM the register allocation must allow.  Measured at config 5 (0.411 ms at 4):
-                              // 5 -> 0.414, 6 -> 0.448, 8 -> 0.487 ms: the kernel wants its registers, not more warps; and
-                              // FEWER resident CTAs (shared-memory padding to 3 / 2 per SM) are slower too: 0.45 / 0.55 ms
+#define BUILD_MIN_CTAS 4      // CTAs of 128 threads per SM the register allocation must allow.  Measured at config 5 in round 1 (0.411 ms
+                              // at 4): 5 -> 0.414, 6 -> 0.448, 8 -> 0.487 ms; with the fast row loop 3, 4 and 5 are within 1 % of each other
 #endif
 
 // Tile of CTA L of the one-dimensional grid.  The tiles that hold the diagonal go FIRST (two per block of T rows: the
