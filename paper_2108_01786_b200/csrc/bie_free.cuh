@@ -379,30 +379,14 @@ __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable
     double* csum = scratch + FREE_WARPS * FREE_ROWS;  // [2][BIE_MAX_COMP]: component sums over s >= s_off, over all s
     double* sbs = csum + 2 * BIE_MAX_COMP;            // [4] constants (free_write_tables)
     double* wred = scratch;   // [2][32] (the warp-sum area is free again)
-    {   // sum of x over each OBSTACLE component (em != 0) that owns one of this CTA's rows: all warps share the
-        // component, lanes strided, warp sums added in fixed order -- every CTA gets the same bits.  Rows below s_off
-        // (hybrid) only want the sources from s_off on, the stored block has the others.
-        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
-        for (int k = 0; k < ct.ncomp; ++k) {
-            if (!(ct.off[k] < r1 && ct.off[k + 1] > r0)) continue;      // CTA-uniform
-            if (nt.DG[ct.off[k]].y == 0.0) { if (threadIdx.x == 0) { csum[k] = 0.0; csum[BIE_MAX_COMP + k] = 0.0; } continue; }
-            double shi = 0.0, slo = 0.0;
-            for (int i = ct.off[k] + threadIdx.x; i < ct.off[k + 1]; i += blockDim.x) {
-                const double xv = __ldcg(xsrc + i);
-                if (i >= fp.s_off) shi += xv; else slo += xv;
-            }
-            shi = bie_warp_sum(shi); slo = bie_warp_sum(slo);
-            if (lane == 0) { wred[warp] = shi; wred[32 + warp] = slo; }
-            __syncthreads();
-            if (threadIdx.x == 0) {
-                double th = 0.0, tl = 0.0;
-                for (int w = 0; w < nwarp; ++w) { th += wred[w]; tl += wred[32 + w]; }
-                csum[k] = th;
-                csum[BIE_MAX_COMP + k] = th + tl;
-            }
-            __syncthreads();
-        }
+    // the E_k weights of the first two components this CTA's rows meet: loaded here, looked at only when the component sums are formed
+    int ek0 = -1, ek1 = -1;
+    for (int k = 0; k < ct.ncomp; ++k) {
+        if (!(ct.off[k] < r1 && ct.off[k + 1] > r0)) continue;          // CTA-uniform
+        if (ek0 < 0) ek0 = k; else if (ek1 < 0) ek1 = k;
     }
+    const double em0 = (ek0 >= 0) ? nt.DG[ct.off[ek0]].y : 0.0;
+    const double em1 = (ek1 >= 0) ? nt.DG[ct.off[ek1]].y : 0.0;
     // Everything below is a handful of dependent L2 round trips (about 0.7 us each).  The loads of the independent chains are
     // ISSUED first and consumed later, so that the chains overlap instead of queueing behind one another:
     //   A: CSR range of the CTA's rows -> near columns and values -> x at those columns        (3 round trips)
@@ -481,6 +465,33 @@ __device__ __forceinline__ void free_gather(const NodeTable& nt, const CompTable
         for (int i = lane; i < (int)gridDim.x; i += 32) sb += __ldcg(fp.SB + (4 * sb_sel + q) * FREE_SB_LD + i);
         sb = bie_warp_sum(sb);
         if (lane == 0) sbs[q] = sb;
+    }
+    // (the component sums come last, with the component's weight loaded at the top: stand-alone operator 0.1615 -> 0.158 ms at
+    // config 5; the GMRES step did not change)
+    {   // sum of x over each OBSTACLE component (em != 0) that owns one of this CTA's rows: all warps share the
+        // component, lanes strided, warp sums added in fixed order -- every CTA gets the same bits.  Rows below s_off
+        // (hybrid) only want the sources from s_off on, the stored block has the others.
+        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+        for (int k = 0; k < ct.ncomp; ++k) {
+            if (!(ct.off[k] < r1 && ct.off[k + 1] > r0)) continue;      // CTA-uniform
+            const double emk = (k == ek0) ? em0 : ((k == ek1) ? em1 : nt.DG[ct.off[k]].y);
+            if (emk == 0.0) { if (threadIdx.x == 0) { csum[k] = 0.0; csum[BIE_MAX_COMP + k] = 0.0; } continue; }
+            double shi = 0.0, slo = 0.0;
+            for (int i = ct.off[k] + threadIdx.x; i < ct.off[k + 1]; i += blockDim.x) {
+                const double xv = __ldcg(xsrc + i);
+                if (i >= fp.s_off) shi += xv; else slo += xv;
+            }
+            shi = bie_warp_sum(shi); slo = bie_warp_sum(slo);
+            if (lane == 0) { wred[warp] = shi; wred[32 + warp] = slo; }
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                double th = 0.0, tl = 0.0;
+                for (int w = 0; w < nwarp; ++w) { th += wred[w]; tl += wred[32 + w]; }
+                csum[k] = th;
+                csum[BIE_MAX_COMP + k] = th + tl;
+            }
+            __syncthreads();
+        }
     }
     __syncthreads();
     for (int t = r0 + threadIdx.x; t < r1; t += blockDim.x) {
